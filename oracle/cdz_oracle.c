@@ -1,0 +1,1241 @@
+/*
+ * cdz_oracle.c -- CPU ORACLE (test infrastructure, NOT the product; see cdz_oracle.h).
+ *
+ * Everything here is written for legibility against PAPER.md and DESIGN.md, in
+ * long double, with no blocking / fusion / scaling tricks.  Unscaled long double
+ * holds e^{+-11356}, i.e. log Z up to ~1.1e4, enough for n <= ~8000 nt with the
+ * synthetic model (log Z ~ 1.33 nat/nt); larger designs are checked window-wise.
+ */
+#include "cdz_oracle.h"
+
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef long double real;
+
+struct orc_tt {
+  int n;
+  int* sigma; /* [n+1] bond dimensions, sigma[0] must be 1 */
+  int* start; /* [n+1] operator list offsets */
+  orc_op* ops;
+};
+
+/* ------------------------------------------------------------------------- */
+/* genetic code, codon index = 16 b0 + 4 b1 + b2 with A,C,G,U = 0..3           */
+/* (the sense codons per amino acid are those listed in PAPER.md lines 859-881) */
+/* ------------------------------------------------------------------------- */
+static const char GENETIC_CODE[65] =
+    "KNKNTTTTRSRSIIMI"
+    "QHQHPPPPRRRRLLLL"
+    "EDEDAAAAGGGGVVVV"
+    "*Y*YSSSS*CWCLFLF";
+
+static int codons_of(char aa, int* out) {
+  int k = 0;
+  for (int c = 0; c < 64; ++c)
+    if (GENETIC_CODE[c] == aa && aa != '*') out[k++] = c;
+  return k;
+}
+
+static int rank_in(const int* set, int count, int v) {
+  for (int r = 0; r < count; ++r)
+    if (set[r] == v) return r;
+  return -1;
+}
+
+/* distinct values of base `pos` (0,1,2) among codons, ascending */
+static int distinct_bases(const int* cod, int deg, int pos, int* out) {
+  int k = 0;
+  for (int b = 0; b < 4; ++b)
+    for (int t = 0; t < deg; ++t) {
+      int cb = (cod[t] >> (2 * (2 - pos))) & 3;
+      if (cb == b) { out[k++] = b; break; }
+    }
+  return k;
+}
+
+int orc_tt_build(const char* aa, int L, int kind, const double* codon_logw, const double* pair_logw,
+                 orc_tt** out) {
+  if (L <= 0 || !aa || !out) return -1;
+  int n = 3 * L;
+  orc_tt* tt = (orc_tt*)calloc(1, sizeof(orc_tt));
+  tt->n = n;
+  tt->sigma = (int*)calloc(n + 1, sizeof(int));
+  tt->start = (int*)calloc(n + 1, sizeof(int));
+  tt->ops = (orc_op*)calloc((size_t)L * 48 + 8, sizeof(orc_op));
+  int nops = 0;
+  int prev[6], pdeg = 1;
+  prev[0] = -1; /* fictitious one-codon predecessor */
+  for (int k = 0; k < L; ++k) {
+    int cod[6];
+    int deg = codons_of(aa[k], cod);
+    if (deg == 0) { orc_tt_free(tt); return -2; }
+    if (kind == 0) {
+      /* single-codon TT: eq 3.4 (line 151), operator lists S3c.i (lines 559-563) */
+      int fb[4], tb[4];
+      int nf = distinct_bases(cod, deg, 0, fb), nt = distinct_bases(cod, deg, 2, tb);
+      tt->sigma[3 * k] = 1;
+      tt->sigma[3 * k + 1] = nf;
+      tt->sigma[3 * k + 2] = nt;
+      tt->start[3 * k] = nops;
+      for (int r = 0; r < nf; ++r) tt->ops[nops++] = (orc_op){0, fb[r], r, 1.0};
+      tt->start[3 * k + 1] = nops;
+      for (int t = 0; t < deg; ++t) {
+        int b0 = cod[t] >> 4, b1 = (cod[t] >> 2) & 3, b2 = cod[t] & 3;
+        double x = codon_logw ? exp(codon_logw[cod[t]]) : 1.0; /* line 157 */
+        tt->ops[nops++] = (orc_op){rank_in(fb, nf, b0), b1, rank_in(tb, nt, b2), x};
+      }
+      tt->start[3 * k + 2] = nops;
+      for (int r = 0; r < nt; ++r) tt->ops[nops++] = (orc_op){r, tb[r], 0, 1.0};
+    } else {
+      /* codon-pair TT: eq 3.3 (line 145) in the S3c.ii form (lines 565-569):
+       * transition + pair weight on the 5' base, codon weight on the middle base */
+      tt->sigma[3 * k] = pdeg;
+      tt->sigma[3 * k + 1] = deg;
+      tt->sigma[3 * k + 2] = deg;
+      tt->start[3 * k] = nops;
+      for (int a = 0; a < pdeg; ++a)
+        for (int c = 0; c < deg; ++c) {
+          double x = (k > 0 && pair_logw) ? exp(pair_logw[prev[a] * 64 + cod[c]]) : 1.0; /* line 163 */
+          tt->ops[nops++] = (orc_op){a, cod[c] >> 4, c, x};
+        }
+      tt->start[3 * k + 1] = nops;
+      for (int c = 0; c < deg; ++c) {
+        double x = codon_logw ? exp(codon_logw[cod[c]]) : 1.0;
+        tt->ops[nops++] = (orc_op){c, (cod[c] >> 2) & 3, c, x};
+      }
+      tt->start[3 * k + 2] = nops;
+      for (int c = 0; c < deg; ++c) tt->ops[nops++] = (orc_op){c, cod[c] & 3, c, 1.0};
+      memcpy(prev, cod, sizeof(cod));
+      pdeg = deg;
+    }
+  }
+  tt->start[n] = nops;
+  tt->sigma[n] = (kind == 0) ? 1 : pdeg;
+  *out = tt;
+  return 0;
+}
+
+int orc_tt_from_ops(int n, const int* counts, const orc_op* ops, orc_tt** out) {
+  if (n <= 0) return -1;
+  orc_tt* tt = (orc_tt*)calloc(1, sizeof(orc_tt));
+  tt->n = n;
+  tt->sigma = (int*)calloc(n + 1, sizeof(int));
+  tt->start = (int*)calloc(n + 1, sizeof(int));
+  int tot = 0;
+  for (int i = 0; i < n; ++i) { tt->start[i] = tot; tot += counts[i]; }
+  tt->start[n] = tot;
+  tt->ops = (orc_op*)calloc(tot + 1, sizeof(orc_op));
+  memcpy(tt->ops, ops, sizeof(orc_op) * tot);
+  for (int i = 0; i <= n; ++i) tt->sigma[i] = 1;
+  for (int i = 0; i < n; ++i)
+    for (int z = tt->start[i]; z < tt->start[i + 1]; ++z) {
+      if (ops[z].a + 1 > tt->sigma[i]) tt->sigma[i] = ops[z].a + 1;
+      if (ops[z].c + 1 > tt->sigma[i + 1]) tt->sigma[i + 1] = ops[z].c + 1;
+    }
+  *out = tt;
+  return 0;
+}
+
+void orc_tt_free(orc_tt* tt) {
+  if (!tt) return;
+  free(tt->sigma); free(tt->start); free(tt->ops); free(tt);
+}
+int orc_tt_n(const orc_tt* tt) { return tt->n; }
+int orc_tt_nops(const orc_tt* tt) { return tt->start[tt->n]; }
+void orc_tt_get(const orc_tt* tt, int* sigma, int* counts, orc_op* ops) {
+  if (sigma) memcpy(sigma, tt->sigma, sizeof(int) * (tt->n + 1));
+  if (counts) for (int i = 0; i < tt->n; ++i) counts[i] = tt->start[i + 1] - tt->start[i];
+  if (ops) memcpy(ops, tt->ops, sizeof(orc_op) * tt->start[tt->n]);
+}
+
+/* eq 3.2, open chain: e_0^T Tbar_0 ... Tbar_{n-1} 1 */
+double orc_tt_logsum(const orc_tt* tt) {
+  int maxs = 1;
+  for (int i = 0; i <= tt->n; ++i) if (tt->sigma[i] > maxs) maxs = tt->sigma[i];
+  real* v = (real*)calloc(maxs, sizeof(real));
+  real* w = (real*)calloc(maxs, sizeof(real));
+  v[0] = 1.0L;
+  for (int i = 0; i < tt->n; ++i) {
+    for (int c = 0; c < maxs; ++c) w[c] = 0;
+    for (int z = tt->start[i]; z < tt->start[i + 1]; ++z) w[tt->ops[z].c] += v[tt->ops[z].a] * (real)tt->ops[z].x;
+    memcpy(v, w, sizeof(real) * maxs);
+  }
+  real s = 0;
+  for (int c = 0; c < tt->sigma[tt->n]; ++c) s += v[c];
+  free(v); free(w);
+  return (double)logl(s);
+}
+
+/* ------------------------------------------------------------------------- */
+/* energy model                                                              */
+/* ------------------------------------------------------------------------- */
+static const int PTYPE[4][4] = {
+    /* A */ {-1, -1, -1, 0},
+    /* C */ {-1, -1, 1, -1},
+    /* G */ {-1, 2, -1, 4},
+    /* U */ {3, -1, 5, -1}};
+
+static double model_kT(const orc_model* m) { return (8.31446261815324 / 4184.0) * m->temperature_K; }
+
+static int can_pair(const orc_model* m, int x, int y) { return m->allow_all_pairs || PTYPE[x][y] >= 0; }
+static int ptype(int x, int y) { return PTYPE[x][y] >= 0 ? PTYPE[x][y] : 0; }
+
+static double hairpin_init(const orc_model* m, int l) {
+  return m->hairpin_a + m->hairpin_b * model_kT(m) * log((double)l / m->hairpin_l0);
+}
+
+/* E(phi,s): sum over loops of the nearest-neighbour decomposition */
+double orc_energy(const orc_model* m, int n, const uint8_t* seq, const int32_t* pair, int* valid) {
+  double E = 0.0;
+  *valid = 1;
+  for (int i = 0; i < n; ++i) {
+    int j = pair[i];
+    if (j < 0) continue;
+    if (j >= n || pair[j] != i || j == i) { *valid = 0; return 0; }
+    if (j < i) continue;
+    if (!can_pair(m, seq[i], seq[j])) { *valid = 0; return 0; }
+    /* loop closed by (i,j): scan its interior */
+    int branches = 0, unpaired = 0, k1 = -1, l1p = -1;
+    for (int p = i + 1; p < j;) {
+      if (pair[p] < 0) { ++unpaired; ++p; continue; }
+      if (pair[p] < p || pair[p] > j) { *valid = 0; return 0; } /* crossing */
+      if (branches == 0) { k1 = p; l1p = pair[p]; }
+      ++branches;
+      p = pair[p] + 1;
+    }
+    int P = ptype(seq[i], seq[j]);
+    if (branches == 0) {
+      int l = j - i - 1;
+      if (l < m->min_hairpin) { *valid = 0; return 0; }
+      E += hairpin_init(m, l) + m->tmm[P][seq[i + 1]][seq[j - 1]];
+    } else if (branches == 1) {
+      int la = k1 - i - 1, lb = j - l1p - 1;
+      int Pin = ptype(seq[k1], seq[l1p]);
+      if (la + lb > m->max_interior) { *valid = 0; return 0; }
+      if (la == 0 && lb == 0) {
+        E += m->stack[P][Pin];
+      } else if (la == 0 || lb == 0) {
+        int l = la + lb;
+        E += m->bulge_init[l] + (l == 1 ? m->stack[P][Pin] : 0.0);
+      } else {
+        E += m->interior_init[la + lb] + m->tmm[P][seq[i + 1]][seq[j - 1]] +
+             m->tmm[ptype(seq[l1p], seq[k1])][seq[l1p + 1]][seq[k1 - 1]];
+      }
+    } else {
+      E += m->ml_a + m->ml_c * (branches + 1) + m->ml_b * unpaired;
+    }
+  }
+  return E;
+}
+
+/* W(phi): e_0^T prod_i T_i^{phi_i} 1 (eq 3.1 with open boundaries) */
+static real tt_seq_weight(const orc_tt* tt, const uint8_t* seq) {
+  int maxs = 1;
+  for (int i = 0; i <= tt->n; ++i) if (tt->sigma[i] > maxs) maxs = tt->sigma[i];
+  real v[64], w[64];
+  if (maxs > 64) return 0;
+  for (int c = 0; c < maxs; ++c) v[c] = 0;
+  v[0] = 1;
+  for (int i = 0; i < tt->n; ++i) {
+    for (int c = 0; c < maxs; ++c) w[c] = 0;
+    for (int z = tt->start[i]; z < tt->start[i + 1]; ++z)
+      if (tt->ops[z].b == seq[i]) w[tt->ops[z].c] += v[tt->ops[z].a] * (real)tt->ops[z].x;
+    memcpy(v, w, sizeof(real) * maxs);
+  }
+  real s = 0;
+  for (int c = 0; c < tt->sigma[tt->n]; ++c) s += v[c];
+  return s;
+}
+
+double orc_logweight(const orc_model* m, const orc_tt* tt, const uint8_t* seq, const int32_t* pair) {
+  int valid;
+  double E = orc_energy(m, tt->n, seq, pair, &valid);
+  real W = tt_seq_weight(tt, seq);
+  if (!valid || W <= 0) return -INFINITY;
+  return (double)(logl(W) - (real)(E / model_kT(m)));
+}
+
+/* ---- brute force: enumerate operator paths x structures -------------------- */
+typedef struct {
+  const orc_model* m;
+  const orc_tt* tt;
+  int n;
+  uint8_t* seq;
+  int32_t* pair;
+  int* stack; /* open right ends */
+  int sp;
+  real W;     /* weight of current sequence */
+  real Z;
+  real* bpp; real* base; real* codon;
+  double nstates;
+  double beta;
+} bf_ctx;
+
+static void bf_structures(bf_ctx* c, int i) {
+  int n = c->n;
+  if (i == n) {
+    int valid;
+    double E = orc_energy(c->m, n, c->seq, c->pair, &valid);
+    if (!valid) return;
+    real w = c->W * expl(-(real)E * (real)c->beta);
+    c->Z += w;
+    c->nstates += 1.0;
+    if (c->bpp)
+      for (int p = 0; p < n; ++p) {
+        if (c->pair[p] < 0) c->bpp[p * n + p] += w;
+        else if (c->pair[p] > p) c->bpp[p * n + c->pair[p]] += w;
+      }
+    if (c->base) for (int p = 0; p < n; ++p) c->base[p * 4 + c->seq[p]] += w;
+    if (c->codon)
+      for (int k = 0; k < n / 3; ++k)
+        c->codon[k * 64 + 16 * c->seq[3 * k] + 4 * c->seq[3 * k + 1] + c->seq[3 * k + 2]] += w;
+    return;
+  }
+  if (c->sp > 0 && c->stack[c->sp - 1] == i) { /* i closes the innermost open pair */
+    --c->sp;
+    bf_structures(c, i + 1);
+    c->stack[c->sp++] = i;
+    return;
+  }
+  c->pair[i] = -1;
+  bf_structures(c, i + 1);
+  int lim = c->sp > 0 ? c->stack[c->sp - 1] : n;
+  for (int j = i + c->m->min_hairpin + 1; j < lim; ++j) {
+    if (!can_pair(c->m, c->seq[i], c->seq[j])) continue;
+    c->pair[i] = j; c->pair[j] = i;
+    c->stack[c->sp++] = j;
+    bf_structures(c, i + 1);
+    --c->sp;
+    c->pair[i] = -1; c->pair[j] = -1;
+  }
+}
+
+static void bf_sequences(bf_ctx* c, int i, int bond, real W) {
+  if (i == c->n) {
+    c->W = W;
+    for (int p = 0; p < c->n; ++p) c->pair[p] = -1;
+    c->sp = 0;
+    bf_structures(c, 0);
+    return;
+  }
+  for (int z = c->tt->start[i]; z < c->tt->start[i + 1]; ++z) {
+    const orc_op* o = &c->tt->ops[z];
+    if (o->a != bond) continue;
+    c->seq[i] = (uint8_t)o->b;
+    bf_sequences(c, i + 1, o->c, W * (real)o->x);
+  }
+}
+
+int orc_brute_force(const orc_model* m, const orc_tt* tt, double* logZ, double* bpp, double* base,
+                    double* codon, double* n_states) {
+  int n = tt->n;
+  bf_ctx c;
+  memset(&c, 0, sizeof(c));
+  c.m = m; c.tt = tt; c.n = n;
+  c.seq = (uint8_t*)calloc(n, 1);
+  c.pair = (int32_t*)calloc(n, sizeof(int32_t));
+  c.stack = (int*)calloc(n + 1, sizeof(int));
+  c.beta = 1.0 / model_kT(m);
+  if (bpp) c.bpp = (real*)calloc((size_t)n * n, sizeof(real));
+  if (base) c.base = (real*)calloc((size_t)n * 4, sizeof(real));
+  if (codon) c.codon = (real*)calloc((size_t)(n / 3) * 64, sizeof(real));
+  bf_sequences(&c, 0, 0, 1.0L);
+  if (logZ) *logZ = (double)logl(c.Z);
+  if (n_states) *n_states = c.nstates;
+  if (bpp) { for (int p = 0; p < n * n; ++p) bpp[p] = (double)(c.bpp[p] / c.Z); free(c.bpp); }
+  if (base) { for (int p = 0; p < n * 4; ++p) base[p] = (double)(c.base[p] / c.Z); free(c.base); }
+  if (codon) { for (int p = 0; p < (n / 3) * 64; ++p) codon[p] = (double)(c.codon[p] / c.Z); free(c.codon); }
+  free(c.seq); free(c.pair); free(c.stack);
+  return 0;
+}
+
+double orc_count_structures(int n, int min_hairpin, int max_interior) {
+  orc_model m;
+  memset(&m, 0, sizeof(m));
+  m.temperature_K = 310.15;
+  m.hairpin_l0 = 1.0;
+  m.max_interior = max_interior;
+  m.min_hairpin = min_hairpin;
+  m.allow_all_pairs = 1;
+  int* counts = (int*)calloc(n, sizeof(int));
+  orc_op* ops = (orc_op*)calloc(n, sizeof(orc_op));
+  for (int i = 0; i < n; ++i) { counts[i] = 1; ops[i] = (orc_op){0, 0, 0, 1.0}; }
+  orc_tt* tt;
+  orc_tt_from_ops(n, counts, ops, &tt);
+  double ns = 0;
+  orc_brute_force(&m, tt, NULL, NULL, NULL, NULL, &ns);
+  orc_tt_free(tt); free(counts); free(ops);
+  return ns;
+}
+
+/* ---- scalar fixed-sequence McCaskill, textbook decomposition ----------------
+ * Q(i,j)  : all structures on [i..j]            (exterior, energy 0)
+ * Qb(i,j) : i.j paired
+ * Qm(i,j) : >=1 branch inside a multiloop,  Qm = sum_k [w_b^{k-i} + Qm(i,k-1)] Qm1(k,j)
+ * Qm1(i,j): exactly one branch starting at i, trailing unpaired.
+ * Deliberately a different decomposition from the tensor recursion below.       */
+double orc_mccaskill(const orc_model* m, int n, const uint8_t* seq) {
+  double beta = 1.0 / model_kT(m);
+#define IX(i, j) ((size_t)(i) * n + (j))
+  real* Q = (real*)calloc((size_t)n * n, sizeof(real));
+  real* Qb = (real*)calloc((size_t)n * n, sizeof(real));
+  real* Qm = (real*)calloc((size_t)n * n, sizeof(real));
+  real* Qm1 = (real*)calloc((size_t)n * n, sizeof(real));
+  real wa = expl(-(real)(m->ml_a * beta)), wb = expl(-(real)(m->ml_b * beta)), wc = expl(-(real)(m->ml_c * beta));
+  for (int d = 0; d < n; ++d)
+    for (int i = 0; i + d < n; ++i) {
+      int j = i + d;
+      real qb = 0;
+      if (d >= m->min_hairpin + 1 && can_pair(m, seq[i], seq[j])) {
+        int P = ptype(seq[i], seq[j]);
+        qb += expl(-(real)((hairpin_init(m, d - 1) + m->tmm[P][seq[i + 1]][seq[j - 1]]) * beta));
+        for (int k = i + 1; k < j; ++k)
+          for (int l = j - 1; l > k; --l) {
+            int la = k - i - 1, lb = j - l - 1;
+            if (la + lb > m->max_interior) break;
+            if (Qb[IX(k, l)] == 0) continue;
+            int Pin = ptype(seq[k], seq[l]);
+            double e;
+            if (la == 0 && lb == 0) e = m->stack[P][Pin];
+            else if (la == 0 || lb == 0) e = m->bulge_init[la + lb] + (la + lb == 1 ? m->stack[P][Pin] : 0.0);
+            else e = m->interior_init[la + lb] + m->tmm[P][seq[i + 1]][seq[j - 1]] +
+                     m->tmm[ptype(seq[l], seq[k])][seq[l + 1]][seq[k - 1]];
+            qb += expl(-(real)(e * beta)) * Qb[IX(k, l)];
+          }
+        /* multiloop: at least two branches in [i+1..j-1] */
+        for (int k = i + 2; k <= j - 1; ++k)
+          qb += wa * wc * Qm[IX(i + 1, k - 1)] * Qm1[IX(k, j - 1)];
+      }
+      Qb[IX(i, j)] = qb;
+      Qm1[IX(i, j)] = wc * qb + (j > i ? wb * Qm1[IX(i, j - 1)] : 0);
+      real qm = 0, wlead = 1;
+      for (int k = i; k <= j; ++k) {
+        qm += (wlead + (k > i ? Qm[IX(i, k - 1)] : 0)) * Qm1[IX(k, j)];
+        wlead *= wb;
+      }
+      Qm[IX(i, j)] = qm;
+      /* exterior: j unpaired, or j pairs with k */
+      real q = (j > i ? Q[IX(i, j - 1)] : 1.0L);
+      for (int k = i; k <= j; ++k) q += (k > i ? Q[IX(i, k - 1)] : 1.0L) * Qb[IX(k, j)];
+      Q[IX(i, j)] = q;
+    }
+  double r = (double)logl(Q[IX(0, n - 1)]);
+  free(Q); free(Qb); free(Qm); free(Qm1);
+#undef IX
+  return r;
+}
+
+/* ------------------------------------------------------------------------- */
+/* tensor-valued inside recursion */
+/* ------------------------------------------------------------------------- */
+struct orc_tables {
+  int n;
+  orc_tt* tt; /* private copy */
+  orc_model model;
+  int* sig;
+  real** Td; /* Td[i][(a*4+x)*sig[i+1]+c]  = T_i[a,x,c]  (eq S3.7) */
+  real** Tb; /* Tb[i][a*sig[i+1]+c]        = Tbar_i      (line 135) */
+  real** E;  /* E(i,j) = Tbar_i..Tbar_j, index i*(n+1)+(j+1), j >= i-1 (identity) */
+  real **qb, **qbs, **qm1, **qml, **m2, **qm; /* index i*n+j */
+  real** qext; /* qext[j+1][c], qext[0] = [1] */
+  real wst[6][6], wtm[6][4][4], wbu[31], win[31], wa, wb, wc;
+  double beta;
+};
+
+#define SG(t, i) ((t)->sig[i])
+static real* cell_alloc(size_t k) { return (real*)calloc(k ? k : 1, sizeof(real)); }
+
+static const real* getE(const orc_tables* t, int i, int j) { return t->E[(size_t)i * (t->n + 1) + (j + 1)]; }
+
+/* Up(p,q)[a,u,v,c] = sum T_p[a,u,.] E(p+1,q-1) T_q[.,v,c]  (p<q);  Up(p,p)[a,u,v,c] = delta_uv T_p[a,u,c] */
+static void compute_Up(const orc_tables* t, int p, int q, real* out) {
+  int Sa = SG(t, p), Sc = SG(t, q + 1);
+  for (int k = 0; k < Sa * 16 * Sc; ++k) out[k] = 0;
+  const orc_tt* tt = t->tt;
+  if (p == q) {
+    for (int z = tt->start[p]; z < tt->start[p + 1]; ++z) {
+      const orc_op* o = &tt->ops[z];
+      out[((o->a * 4 + o->b) * 4 + o->b) * Sc + o->c] += (real)o->x;
+    }
+    return;
+  }
+  const real* Em = getE(t, p + 1, q - 1);
+  int Sm = SG(t, q); /* columns of E(p+1,q-1) */
+  for (int z = tt->start[p]; z < tt->start[p + 1]; ++z)
+    for (int y = tt->start[q]; y < tt->start[q + 1]; ++y) {
+      const orc_op *o = &tt->ops[z], *r = &tt->ops[y];
+      out[((o->a * 4 + o->b) * 4 + r->b) * Sc + r->c] += (real)o->x * Em[o->c * Sm + r->a] * (real)r->x;
+    }
+}
+
+/* one closed cell: Qb(i,j)[a,x,y,c] following SURVEY App. A.2 term by term */
+static void compute_qb(orc_tables* t, int i, int j) {
+  const orc_model* m = &t->model;
+  int n = t->n, d = j - i;
+  int Si = SG(t, i), Sj1 = SG(t, j + 1);
+  real* qb = t->qb[(size_t)i * n + j];
+  if (d < m->min_hairpin + 1) return;
+  int Sa = SG(t, i + 1), Sc = SG(t, j); /* a' in Sigma_{i+1}, c' in Sigma_j */
+  /* inner[x][y][a'][c'] */
+  real* inner = cell_alloc((size_t)16 * Sa * Sc);
+#define INNER(x, y, a, c) inner[(((x) * 4 + (y)) * Sa + (a)) * Sc + (c)]
+  int maxS = 1;
+  for (int p = i; p <= j + 1; ++p) if (SG(t, p) > maxS) maxS = SG(t, p);
+  real* UpL = cell_alloc((size_t)maxS * 16 * maxS);
+  real* UpR = cell_alloc((size_t)maxS * 16 * maxS);
+  real* A1 = cell_alloc((size_t)maxS * 16 * 16 * maxS); /* [a'][u][u'][x'][y'][t] */
+  real* A2 = cell_alloc((size_t)maxS * 16 * maxS);      /* [a'][u][v'][t] */
+  real* A3 = cell_alloc((size_t)maxS * 16 * maxS);      /* [a'][u][v][c'] */
+
+  /* hairpin: sum_{u,v} exp(-beta(H(d-1)+tmm[p(x,y)][u][v])) Up(i+1,j-1)[a',u,v,c'] */
+  {
+    compute_Up(t, i + 1, j - 1, UpL);
+    real wh = expl(-(real)(hairpin_init(m, d - 1) * t->beta));
+    for (int x = 0; x < 4; ++x)
+      for (int y = 0; y < 4; ++y) {
+        if (!can_pair(m, x, y)) continue;
+        int P = ptype(x, y);
+        for (int a = 0; a < Sa; ++a)
+          for (int u = 0; u < 4; ++u)
+            for (int v = 0; v < 4; ++v)
+              for (int c = 0; c < Sc; ++c)
+                INNER(x, y, a, c) += wh * t->wtm[P][u][v] * UpL[((a * 4 + u) * 4 + v) * Sc + c];
+      }
+  }
+  /* one inner pair (k,l): k ascending, l descending */
+  for (int k = i + 1; k < j; ++k)
+    for (int l = j - 1; l > k; --l) {
+      int l1 = k - i - 1, l2 = j - l - 1;
+      if (l1 + l2 > m->max_interior) break;
+      if (l - k < m->min_hairpin + 1) continue;
+      const real* qin = t->qb[(size_t)k * n + l]; /* [s][x'][y'][tt] */
+      int Ss = SG(t, k), St = SG(t, l + 1);
+      if (l1 == 0 && l2 == 0) {
+        /* stack: Ss == Sa, St == Sc */
+        for (int x = 0; x < 4; ++x)
+          for (int y = 0; y < 4; ++y) {
+            if (!can_pair(m, x, y)) continue;
+            for (int xp = 0; xp < 4; ++xp)
+              for (int yp = 0; yp < 4; ++yp) {
+                if (!can_pair(m, xp, yp)) continue;
+                real w = t->wst[ptype(x, y)][ptype(xp, yp)];
+                for (int a = 0; a < Sa; ++a)
+                  for (int c = 0; c < Sc; ++c) INNER(x, y, a, c) += w * qin[((a * 4 + xp) * 4 + yp) * St + c];
+              }
+          }
+      } else if (l2 == 0) {
+        /* left bulge: sum_s E(i+1,k-1)[a',s] Qb(k,l)[s,x',y',c'] */
+        const real* El = getE(t, i + 1, k - 1);
+        for (int x = 0; x < 4; ++x)
+          for (int y = 0; y < 4; ++y) {
+            if (!can_pair(m, x, y)) continue;
+            for (int xp = 0; xp < 4; ++xp)
+              for (int yp = 0; yp < 4; ++yp) {
+                if (!can_pair(m, xp, yp)) continue;
+                real w = t->wbu[l1] * (l1 == 1 ? t->wst[ptype(x, y)][ptype(xp, yp)] : 1.0L);
+                for (int a = 0; a < Sa; ++a)
+                  for (int s = 0; s < Ss; ++s)
+                    for (int c = 0; c < Sc; ++c)
+                      INNER(x, y, a, c) += w * El[a * Ss + s] * qin[((s * 4 + xp) * 4 + yp) * St + c];
+              }
+          }
+      } else if (l1 == 0) {
+        /* right bulge: sum_t Qb(k,l)[a',x',y',t] E(l+1,j-1)[t,c'] */
+        const real* Er = getE(t, l + 1, j - 1);
+        for (int x = 0; x < 4; ++x)
+          for (int y = 0; y < 4; ++y) {
+            if (!can_pair(m, x, y)) continue;
+            for (int xp = 0; xp < 4; ++xp)
+              for (int yp = 0; yp < 4; ++yp) {
+                if (!can_pair(m, xp, yp)) continue;
+                real w = t->wbu[l2] * (l2 == 1 ? t->wst[ptype(x, y)][ptype(xp, yp)] : 1.0L);
+                for (int a = 0; a < Sa; ++a)
+                  for (int tt_ = 0; tt_ < St; ++tt_)
+                    for (int c = 0; c < Sc; ++c)
+                      INNER(x, y, a, c) += w * qin[((a * 4 + xp) * 4 + yp) * St + tt_] * Er[tt_ * Sc + c];
+              }
+          }
+      } else {
+        /* generic interior loop, contracted in four explicit stages:
+         *  sum exp(-beta(In(l1+l2)+tmm[p(x,y)][u][v]+tmm[p(y',x')][v'][u']))
+         *      Up(i+1,k-1)[a',u,u',s] Qb(k,l)[s,x',y',t] Up(l+1,j-1)[t,v',v,c']        */
+        compute_Up(t, i + 1, k - 1, UpL); /* [a'][u][u'][s]  */
+        compute_Up(t, l + 1, j - 1, UpR); /* [t][v'][v][c']  */
+        for (int q = 0; q < Sa * 16 * 16 * St; ++q) A1[q] = 0;
+        for (int a = 0; a < Sa; ++a)
+          for (int u = 0; u < 4; ++u)
+            for (int up = 0; up < 4; ++up)
+              for (int s = 0; s < Ss; ++s) {
+                real w = UpL[((a * 4 + u) * 4 + up) * Ss + s];
+                if (w == 0) continue;
+                for (int xy = 0; xy < 16; ++xy)
+                  for (int tt_ = 0; tt_ < St; ++tt_)
+                    A1[((((a * 4 + u) * 4 + up) * 16) + xy) * St + tt_] += w * qin[(s * 16 + xy) * St + tt_];
+              }
+        for (int q = 0; q < Sa * 16 * St; ++q) A2[q] = 0;
+        for (int a = 0; a < Sa; ++a)
+          for (int u = 0; u < 4; ++u)
+            for (int up = 0; up < 4; ++up)
+              for (int xp = 0; xp < 4; ++xp)
+                for (int yp = 0; yp < 4; ++yp) {
+                  if (!can_pair(m, xp, yp)) continue;
+                  int Pin = ptype(yp, xp); /* inner pair seen from the loop: (phi_l, phi_k) */
+                  for (int vp = 0; vp < 4; ++vp)
+                    for (int tt_ = 0; tt_ < St; ++tt_)
+                      A2[((a * 4 + u) * 4 + vp) * St + tt_] +=
+                          t->wtm[Pin][vp][up] * A1[((((a * 4 + u) * 4 + up) * 16) + xp * 4 + yp) * St + tt_];
+                }
+        for (int q = 0; q < Sa * 16 * Sc; ++q) A3[q] = 0;
+        for (int a = 0; a < Sa; ++a)
+          for (int u = 0; u < 4; ++u)
+            for (int vp = 0; vp < 4; ++vp)
+              for (int tt_ = 0; tt_ < St; ++tt_) {
+                real w = A2[((a * 4 + u) * 4 + vp) * St + tt_];
+                if (w == 0) continue;
+                for (int v = 0; v < 4; ++v)
+                  for (int c = 0; c < Sc; ++c) A3[((a * 4 + u) * 4 + v) * Sc + c] += w * UpR[((tt_ * 4 + vp) * 4 + v) * Sc + c];
+              }
+        real wi = t->win[l1 + l2];
+        for (int x = 0; x < 4; ++x)
+          for (int y = 0; y < 4; ++y) {
+            if (!can_pair(m, x, y)) continue;
+            int P = ptype(x, y);
+            for (int a = 0; a < Sa; ++a)
+              for (int u = 0; u < 4; ++u)
+                for (int v = 0; v < 4; ++v)
+                  for (int c = 0; c < Sc; ++c)
+                    INNER(x, y, a, c) += wi * t->wtm[P][u][v] * A3[((a * 4 + u) * 4 + v) * Sc + c];
+          }
+      }
+    }
+  /* multiloop closure: w_a w_c M2(i+1,j-1)[a',c'] */
+  if (j - 1 >= i + 1) {
+    const real* m2 = t->m2[(size_t)(i + 1) * n + (j - 1)];
+    for (int x = 0; x < 4; ++x)
+      for (int y = 0; y < 4; ++y) {
+        if (!can_pair(m, x, y)) continue;
+        for (int a = 0; a < Sa; ++a)
+          for (int c = 0; c < Sc; ++c) INNER(x, y, a, c) += t->wa * t->wc * m2[a * Sc + c];
+      }
+  }
+  /* dress with T_i, T_j: Qb[a,x,y,c] = can(x,y) sum_{a',c'} T_i[a,x,a'] T_j[c',y,c] inner[x,y;a',c'] */
+  const real *Ti = t->Td[i], *Tj = t->Td[j];
+  for (int a = 0; a < Si; ++a)
+    for (int x = 0; x < 4; ++x)
+      for (int y = 0; y < 4; ++y) {
+        if (!can_pair(m, x, y)) continue;
+        for (int c = 0; c < Sj1; ++c) {
+          real s = 0;
+          for (int ap = 0; ap < Sa; ++ap)
+            for (int cp = 0; cp < Sc; ++cp)
+              s += Ti[(a * 4 + x) * Sa + ap] * Tj[(cp * 4 + y) * Sj1 + c] * INNER(x, y, ap, cp);
+          qb[((a * 4 + x) * 4 + y) * Sj1 + c] = s;
+        }
+      }
+#undef INNER
+  free(inner); free(UpL); free(UpR); free(A1); free(A2); free(A3);
+}
+
+static void compute_cell(orc_tables* t, int i, int j) {
+  int n = t->n;
+  int Si = SG(t, i), Sj1 = SG(t, j + 1);
+  size_t ci = (size_t)i * n + j;
+  compute_qb(t, i, j);
+  real *qb = t->qb[ci], *qbs = t->qbs[ci], *qm1 = t->qm1[ci], *qml = t->qml[ci], *m2 = t->m2[ci], *qm = t->qm[ci];
+  /* Qbs[a,c] = sum_{x,y} Qb[a,x,y,c] */
+  for (int a = 0; a < Si; ++a)
+    for (int xy = 0; xy < 16; ++xy)
+      for (int c = 0; c < Sj1; ++c) qbs[a * Sj1 + c] += qb[(a * 16 + xy) * Sj1 + c];
+  /* Qm1(i,j) = w_c Qbs(i,j) + w_b Qm1(i,j-1) Tbar_j */
+  for (int a = 0; a < Si; ++a)
+    for (int c = 0; c < Sj1; ++c) qm1[a * Sj1 + c] = t->wc * qbs[a * Sj1 + c];
+  if (j - 1 >= i) {
+    const real* p = t->qm1[(size_t)i * n + (j - 1)];
+    int Sj = SG(t, j);
+    for (int a = 0; a < Si; ++a)
+      for (int s = 0; s < Sj; ++s)
+        for (int c = 0; c < Sj1; ++c) qm1[a * Sj1 + c] += t->wb * p[a * Sj + s] * t->Tb[j][s * Sj1 + c];
+  }
+  /* Qml(i,j) = Qm1(i,j) + w_b Tbar_i Qml(i+1,j) */
+  for (int k = 0; k < Si * Sj1; ++k) qml[k] = qm1[k];
+  if (i + 1 <= j) {
+    const real* p = t->qml[(size_t)(i + 1) * n + j];
+    int Si1 = SG(t, i + 1);
+    for (int a = 0; a < Si; ++a)
+      for (int s = 0; s < Si1; ++s)
+        for (int c = 0; c < Sj1; ++c) qml[a * Sj1 + c] += t->wb * t->Tb[i][a * Si1 + s] * p[s * Sj1 + c];
+  }
+  /* M2(i,j) = sum_{k=i+1}^{j} Qm(i,k-1) Qm1(k,j)   (eq 3.5 first line, line 172, on the packed index space) */
+  for (int k = i + 1; k <= j; ++k) {
+    const real* A = t->qm[(size_t)i * n + (k - 1)];
+    const real* B = t->qm1[(size_t)k * n + j];
+    int Sk = SG(t, k);
+    for (int a = 0; a < Si; ++a)
+      for (int s = 0; s < Sk; ++s) {
+        real w = A[a * Sk + s];
+        if (w == 0) continue;
+        for (int c = 0; c < Sj1; ++c) m2[a * Sj1 + c] += w * B[s * Sj1 + c];
+      }
+  }
+  for (int k = 0; k < Si * Sj1; ++k) qm[k] = qml[k] + m2[k];
+}
+
+int orc_inside(const orc_model* m, const orc_tt* tt_in, int nthreads, orc_tables** out, double* logZ) {
+  int n = tt_in->n;
+  orc_tables* t = (orc_tables*)calloc(1, sizeof(orc_tables));
+  t->n = n;
+  t->model = *m;
+  /* private TT copy */
+  t->tt = (orc_tt*)calloc(1, sizeof(orc_tt));
+  t->tt->n = n;
+  t->tt->sigma = (int*)malloc(sizeof(int) * (n + 1));
+  t->tt->start = (int*)malloc(sizeof(int) * (n + 1));
+  memcpy(t->tt->sigma, tt_in->sigma, sizeof(int) * (n + 1));
+  memcpy(t->tt->start, tt_in->start, sizeof(int) * (n + 1));
+  t->tt->ops = (orc_op*)malloc(sizeof(orc_op) * (tt_in->start[n] + 1));
+  memcpy(t->tt->ops, tt_in->ops, sizeof(orc_op) * tt_in->start[n]);
+  t->sig = t->tt->sigma;
+  double kT = model_kT(m);
+  t->beta = 1.0 / kT;
+  for (int p = 0; p < 6; ++p) {
+    for (int q = 0; q < 6; ++q) t->wst[p][q] = expl(-(real)(m->stack[p][q] * t->beta));
+    for (int x = 0; x < 4; ++x)
+      for (int y = 0; y < 4; ++y) t->wtm[p][x][y] = expl(-(real)(m->tmm[p][x][y] * t->beta));
+  }
+  for (int l = 0; l < 31; ++l) {
+    t->wbu[l] = l >= 1 ? expl(-(real)(m->bulge_init[l] * t->beta)) : 0;
+    t->win[l] = l >= 2 ? expl(-(real)(m->interior_init[l] * t->beta)) : 0;
+  }
+  t->wa = expl(-(real)(m->ml_a * t->beta));
+  t->wb = expl(-(real)(m->ml_b * t->beta));
+  t->wc = expl(-(real)(m->ml_c * t->beta));
+  /* dense cores (eq S3.7) and transfer matrices */
+  t->Td = (real**)calloc(n, sizeof(real*));
+  t->Tb = (real**)calloc(n, sizeof(real*));
+  for (int i = 0; i < n; ++i) {
+    int Sa = SG(t, i), Sc = SG(t, i + 1);
+    t->Td[i] = cell_alloc((size_t)Sa * 4 * Sc);
+    t->Tb[i] = cell_alloc((size_t)Sa * Sc);
+    for (int z = t->tt->start[i]; z < t->tt->start[i + 1]; ++z) {
+      const orc_op* o = &t->tt->ops[z];
+      t->Td[i][(o->a * 4 + o->b) * Sc + o->c] += (real)o->x;
+      t->Tb[i][o->a * Sc + o->c] += (real)o->x;
+    }
+  }
+  /* stretches E(i,j) */
+  t->E = (real**)calloc((size_t)(n + 1) * (n + 1), sizeof(real*));
+  for (int i = 0; i <= n; ++i) {
+    int Sa = SG(t, i);
+    real* id = cell_alloc((size_t)Sa * Sa);
+    for (int a = 0; a < Sa; ++a) id[a * Sa + a] = 1;
+    t->E[(size_t)i * (n + 1) + i] = id; /* E(i,i-1) = I */
+    for (int j = i; j < n; ++j) {
+      int Sj = SG(t, j), Sj1 = SG(t, j + 1);
+      const real* prev = t->E[(size_t)i * (n + 1) + j];
+      real* e = cell_alloc((size_t)Sa * Sj1);
+      for (int a = 0; a < Sa; ++a)
+        for (int s = 0; s < Sj; ++s)
+          for (int c = 0; c < Sj1; ++c) e[a * Sj1 + c] += prev[a * Sj + s] * t->Tb[j][s * Sj1 + c];
+      t->E[(size_t)i * (n + 1) + (j + 1)] = e;
+    }
+  }
+  size_t nn = (size_t)n * n;
+  t->qb = (real**)calloc(nn, sizeof(real*));
+  t->qbs = (real**)calloc(nn, sizeof(real*));
+  t->qm1 = (real**)calloc(nn, sizeof(real*));
+  t->qml = (real**)calloc(nn, sizeof(real*));
+  t->m2 = (real**)calloc(nn, sizeof(real*));
+  t->qm = (real**)calloc(nn, sizeof(real*));
+  for (int i = 0; i < n; ++i)
+    for (int j = i; j < n; ++j) {
+      size_t ci = (size_t)i * n + j, s2 = (size_t)SG(t, i) * SG(t, j + 1);
+      t->qb[ci] = cell_alloc(s2 * 16);
+      t->qbs[ci] = cell_alloc(s2);
+      t->qm1[ci] = cell_alloc(s2);
+      t->qml[ci] = cell_alloc(s2);
+      t->m2[ci] = cell_alloc(s2);
+      t->qm[ci] = cell_alloc(s2);
+    }
+#ifdef _OPENMP
+  if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+  (void)nthreads;
+#endif
+  for (int d = 0; d < n; ++d) {
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int i = 0; i < n - d; ++i) compute_cell(t, i, i + d);
+  }
+  /* exterior (eq 3.7): Qext(j) = Qext(j-1) Tbar_j + sum_k Qext(k-1) Qbs(k,j) */
+  t->qext = (real**)calloc(n + 1, sizeof(real*));
+  t->qext[0] = cell_alloc(SG(t, 0));
+  t->qext[0][0] = 1;
+  for (int j = 0; j < n; ++j) {
+    int Sj = SG(t, j), Sj1 = SG(t, j + 1);
+    real* q = cell_alloc(Sj1);
+    for (int s = 0; s < Sj; ++s)
+      for (int c = 0; c < Sj1; ++c) q[c] += t->qext[j][s] * t->Tb[j][s * Sj1 + c];
+    for (int k = 0; k <= j; ++k) {
+      const real* qbs = t->qbs[(size_t)k * n + j];
+      int Sk = SG(t, k);
+      for (int s = 0; s < Sk; ++s)
+        for (int c = 0; c < Sj1; ++c) q[c] += t->qext[k][s] * qbs[s * Sj1 + c];
+    }
+    t->qext[j + 1] = q;
+  }
+  real Z = 0;
+  for (int c = 0; c < SG(t, n); ++c) Z += t->qext[n][c];
+  if (logZ) *logZ = (double)logl(Z);
+  if (out) *out = t; else orc_tables_free(t);
+  return 0;
+}
+
+void orc_tables_free(orc_tables* t) {
+  if (!t) return;
+  int n = t->n;
+  for (int i = 0; i < n; ++i) { free(t->Td[i]); free(t->Tb[i]); }
+  free(t->Td); free(t->Tb);
+  for (size_t k = 0; k < (size_t)(n + 1) * (n + 1); ++k) free(t->E[k]);
+  free(t->E);
+  for (size_t k = 0; k < (size_t)n * n; ++k) {
+    free(t->qb[k]); free(t->qbs[k]); free(t->qm1[k]); free(t->qml[k]); free(t->m2[k]); free(t->qm[k]);
+  }
+  free(t->qb); free(t->qbs); free(t->qm1); free(t->qml); free(t->m2); free(t->qm);
+  for (int j = 0; j <= n; ++j) free(t->qext[j]);
+  free(t->qext);
+  orc_tt_free(t->tt);
+  free(t);
+}
+
+int orc_tables_cell(const orc_tables* t, int which, int i, int j, int shift, double* out) {
+  if (i < 0 || j < i || j >= t->n) return -1;
+  size_t ci = (size_t)i * t->n + j;
+  real** tabs[6] = {t->qb, t->qbs, t->qm1, t->qml, t->m2, t->qm};
+  if (which < 0 || which > 5) return -1;
+  size_t cnt = (size_t)SG(t, i) * SG(t, j + 1) * (which == 0 ? 16 : 1);
+  for (size_t k = 0; k < cnt; ++k) out[k] = (double)ldexpl(tabs[which][ci][k], -shift);
+  return (int)cnt;
+}
+
+double orc_tables_logqext(const orc_tables* t, int j, int c) {
+  real v = t->qext[j + 1][c];
+  return v > 0 ? (double)logl(v) : -INFINITY;
+}
+
+/* ------------------------------------------------------------------------- */
+/* stochastic traceback                        */
+/* ------------------------------------------------------------------------- */
+static uint64_t mix64(uint64_t z) {
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+  return z ^ (z >> 31);
+}
+double orc_uniform(uint64_t seed, uint64_t sample, uint64_t kind, uint64_t i, uint64_t j) {
+  uint64_t h = seed;
+  uint64_t v[4] = {sample, kind, i, j};
+  for (int k = 0; k < 4; ++k) h = mix64(h + 0x9E3779B97F4A7C15ULL * (v[k] + 1));
+  return (double)(h >> 11) * (1.0 / 9007199254740992.0);
+}
+
+enum { K_TOP = 0, K_EXT = 1, K_QB = 2, K_QM = 3, K_QML = 4, K_QM1 = 5, K_CHAIN = 6, K_HAIRPIN = 7, K_ILOOP = 8 };
+enum { IT_QB = 0, IT_QM = 1, IT_QML = 2, IT_QM1 = 3 };
+typedef struct { int type, i, j, a, x, y, c; } tb_item;
+
+/* a growing list of alternative weights; pick() returns the first index whose running sum exceeds u*total */
+typedef struct { real* w; int n, cap; } altlist;
+static void alt_reset(altlist* L) { L->n = 0; }
+static void alt_push(altlist* L, real w) {
+  if (L->n == L->cap) { L->cap = L->cap ? 2 * L->cap : 256; L->w = (real*)realloc(L->w, sizeof(real) * L->cap); }
+  L->w[L->n++] = w;
+}
+static int alt_pick(const altlist* L, double u) {
+  real tot = 0;
+  for (int k = 0; k < L->n; ++k) tot += L->w[k];
+  real thr = (real)u * tot, run = 0;
+  int last = -1;
+  for (int k = 0; k < L->n; ++k) {
+    if (L->w[k] <= 0) continue;
+    run += L->w[k];
+    last = k;
+    if (run > thr) return k;
+  }
+  return last;
+}
+
+typedef struct {
+  const orc_tables* t;
+  uint64_t seed; int sample;
+  uint8_t* seq; int32_t* pair;
+  altlist L;
+  tb_item* stk; int sp, cap;
+} tb_ctx;
+
+static void tb_push(tb_ctx* c, tb_item it) {
+  if (c->sp == c->cap) { c->cap = c->cap ? 2 * c->cap : 64; c->stk = (tb_item*)realloc(c->stk, sizeof(tb_item) * c->cap); }
+  c->stk[c->sp++] = it;
+}
+static double tb_u(const tb_ctx* c, int kind, int i, int j) {
+  return orc_uniform(c->seed, (uint64_t)c->sample, (uint64_t)kind, (uint64_t)i, (uint64_t)j);
+}
+
+/* CHAIN(p,q,s,t): unpaired stretch p..q with fixed end bonds; choose z_m prop. to x(z) b_{m+1}[c(z)],
+ * b_m = Tbar_m ... Tbar_q e_t */
+static void tb_chain(tb_ctx* c, int p, int q, int s, int tend) {
+  const orc_tables* t = c->t;
+  if (p > q) return;
+  int cur = s;
+  for (int mpos = p; mpos <= q; ++mpos) {
+    alt_reset(&c->L);
+    int z0 = t->tt->start[mpos], z1 = t->tt->start[mpos + 1];
+    const real* Er = getE(t, mpos + 1, q); /* b_{m+1}[.] = E(m+1,q)[., tend] */
+    int Sq1 = SG(t, q + 1);
+    for (int z = z0; z < z1; ++z) {
+      const orc_op* o = &t->tt->ops[z];
+      alt_push(&c->L, o->a == cur ? (real)o->x * Er[o->c * Sq1 + tend] : 0);
+    }
+    int k = alt_pick(&c->L, tb_u(c, K_CHAIN, mpos, 0));
+    const orc_op* o = &t->tt->ops[z0 + k];
+    c->seq[mpos] = (uint8_t)o->b;
+    cur = o->c;
+  }
+}
+
+static void tb_qb(tb_ctx* c, tb_item it) {
+  const orc_tables* t = c->t;
+  const orc_model* m = &t->model;
+  const orc_tt* tt = t->tt;
+  int n = t->n, i = it.i, j = it.j, d = j - i, x = it.x, y = it.y;
+  int P = ptype(x, y);
+  c->seq[i] = (uint8_t)x; c->seq[j] = (uint8_t)y;
+  c->pair[i] = j; c->pair[j] = i;
+  real wh = expl(-(real)(hairpin_init(m, d - 1) * t->beta));
+  int Sc = SG(t, j);
+  /* level A: (z_i, z_j) x {hairpin, (k asc, l desc), multiloop (k asc, s asc)} */
+  typedef struct { int zi, zj, kind, k, l, s; } altA;
+  altA* desc = NULL; int nd = 0, capd = 0;
+#define PUSHA(W, ...) do { if (nd == capd) { capd = capd ? 2 * capd : 512; desc = (altA*)realloc(desc, sizeof(altA) * capd); } \
+    desc[nd++] = (altA){__VA_ARGS__}; alt_push(&c->L, (W)); } while (0)
+  alt_reset(&c->L);
+  int maxS = 1;
+  for (int p = i; p <= j + 1; ++p) if (SG(t, p) > maxS) maxS = SG(t, p);
+  real* UpL = cell_alloc((size_t)maxS * 16 * maxS);
+  real* UpR = cell_alloc((size_t)maxS * 16 * maxS);
+  for (int zi = tt->start[i]; zi < tt->start[i + 1]; ++zi) {
+    const orc_op* oi = &tt->ops[zi];
+    if (oi->a != it.a || oi->b != x) continue;
+    for (int zj = tt->start[j]; zj < tt->start[j + 1]; ++zj) {
+      const orc_op* oj = &tt->ops[zj];
+      if (oj->b != y || oj->c != it.c) continue;
+      real w0 = (real)oi->x * (real)oj->x;
+      int ap = oi->c, cp = oj->a;
+      /* hairpin */
+      {
+        compute_Up(t, i + 1, j - 1, UpL);
+        real s = 0;
+        for (int u = 0; u < 4; ++u)
+          for (int v = 0; v < 4; ++v) s += wh * t->wtm[P][u][v] * UpL[((ap * 4 + u) * 4 + v) * Sc + cp];
+        PUSHA(w0 * s, zi, zj, 0, 0, 0, 0);
+      }
+      for (int k = i + 1; k < j; ++k)
+        for (int l = j - 1; l > k; --l) {
+          int l1 = k - i - 1, l2 = j - l - 1;
+          if (l1 + l2 > m->max_interior) break;
+          if (l - k < m->min_hairpin + 1) continue;
+          const real* qin = t->qb[(size_t)k * n + l];
+          int Ss = SG(t, k), St = SG(t, l + 1);
+          real s = 0;
+          for (int xp = 0; xp < 4; ++xp)
+            for (int yp = 0; yp < 4; ++yp) {
+              if (!can_pair(m, xp, yp)) continue;
+              if (l1 == 0 && l2 == 0) {
+                s += t->wst[P][ptype(xp, yp)] * qin[((ap * 4 + xp) * 4 + yp) * St + cp];
+              } else if (l2 == 0) {
+                const real* El = getE(t, i + 1, k - 1);
+                real w = t->wbu[l1] * (l1 == 1 ? t->wst[P][ptype(xp, yp)] : 1.0L);
+                for (int sb = 0; sb < Ss; ++sb) s += w * El[ap * Ss + sb] * qin[((sb * 4 + xp) * 4 + yp) * St + cp];
+              } else if (l1 == 0) {
+                const real* Er = getE(t, l + 1, j - 1);
+                real w = t->wbu[l2] * (l2 == 1 ? t->wst[P][ptype(xp, yp)] : 1.0L);
+                for (int tb = 0; tb < St; ++tb) s += w * qin[((ap * 4 + xp) * 4 + yp) * St + tb] * Er[tb * Sc + cp];
+              }
+            }
+          if (l1 > 0 && l2 > 0) {
+            compute_Up(t, i + 1, k - 1, UpL);
+            compute_Up(t, l + 1, j - 1, UpR);
+            for (int u = 0; u < 4; ++u)
+              for (int up = 0; up < 4; ++up)
+                for (int sb = 0; sb < Ss; ++sb) {
+                  real wl = UpL[((ap * 4 + u) * 4 + up) * Ss + sb];
+                  if (wl == 0) continue;
+                  for (int xp = 0; xp < 4; ++xp)
+                    for (int yp = 0; yp < 4; ++yp) {
+                      if (!can_pair(m, xp, yp)) continue;
+                      for (int tb = 0; tb < St; ++tb) {
+                        real wq = qin[((sb * 4 + xp) * 4 + yp) * St + tb];
+                        if (wq == 0) continue;
+                        for (int vp = 0; vp < 4; ++vp)
+                          for (int v = 0; v < 4; ++v)
+                            s += t->win[l1 + l2] * t->wtm[P][u][v] * t->wtm[ptype(yp, xp)][vp][up] * wl * wq *
+                                 UpR[((tb * 4 + vp) * 4 + v) * Sc + cp];
+                      }
+                    }
+                }
+          }
+          PUSHA(w0 * s, zi, zj, 1, k, l, 0);
+        }
+      /* multiloop: k = 5' end of the last branch */
+      for (int k = i + 2; k <= j - 1; ++k) {
+        const real* A = t->qm[(size_t)(i + 1) * n + (k - 1)];
+        const real* B = t->qm1[(size_t)k * n + (j - 1)];
+        int Sk = SG(t, k);
+        for (int sb = 0; sb < Sk; ++sb) PUSHA(w0 * t->wa * t->wc * A[ap * Sk + sb] * B[sb * Sc + cp], zi, zj, 2, k, 0, sb);
+      }
+    }
+  }
+#undef PUSHA
+  int pick = alt_pick(&c->L, tb_u(c, K_QB, i, j));
+  altA A = desc[pick];
+  free(desc);
+  const orc_op *oi = &tt->ops[A.zi], *oj = &tt->ops[A.zj];
+  int ap = oi->c, cp = oj->a;
+  if (A.kind == 0) {
+    /* hairpin ends: joint choice of the operators at i+1 and j-1 (K_HAIRPIN), then the interior chain */
+    int p = i + 1, q = j - 1;
+    const real* Em = getE(t, p + 1, q - 1);
+    int Sm = SG(t, q);
+    alt_reset(&c->L);
+    int zp0 = tt->start[p], zp1 = tt->start[p + 1], zq0 = tt->start[q], zq1 = tt->start[q + 1];
+    for (int zp = zp0; zp < zp1; ++zp)
+      for (int zq = zq0; zq < zq1; ++zq) {
+        const orc_op *o = &tt->ops[zp], *r = &tt->ops[zq];
+        real w = 0;
+        if (o->a == ap && r->c == cp) w = (real)o->x * (real)r->x * Em[o->c * Sm + r->a] * t->wtm[P][o->b][r->b];
+        alt_push(&c->L, w);
+      }
+    int k = alt_pick(&c->L, tb_u(c, K_HAIRPIN, i, j));
+    const orc_op *o = &tt->ops[zp0 + k / (zq1 - zq0)], *r = &tt->ops[zq0 + k % (zq1 - zq0)];
+    c->seq[p] = (uint8_t)o->b; c->seq[q] = (uint8_t)r->b;
+    tb_chain(c, p + 1, q - 1, o->c, r->a);
+  } else if (A.kind == 1) {
+    /* one inner pair (k,l): level B (K_ILOOP) chooses the stretch end operators and (x',y') */
+    int k = A.k, l = A.l, l1 = k - i - 1, l2 = j - l - 1;
+    const real* qin = t->qb[(size_t)k * n + l];
+    int St = SG(t, l + 1);
+    /* left side alternatives: (operator at i+1, operator at k-1) with resulting (u,u',s) */
+    typedef struct { int z1, z2, u, up, s; real w; } side;
+    side *Ls = NULL, *Rs = NULL; int nL = 0, nR = 0;
+    Ls = (side*)calloc(4096, sizeof(side)); Rs = (side*)calloc(4096, sizeof(side));
+    if (l1 == 0) { Ls[nL++] = (side){-1, -1, 0, 0, ap, 1}; }
+    else if (l1 == 1) {
+      for (int z = tt->start[i + 1]; z < tt->start[i + 2]; ++z) {
+        const orc_op* o = &tt->ops[z];
+        if (o->a == ap) Ls[nL++] = (side){z, -1, o->b, o->b, o->c, (real)o->x};
+      }
+    } else {
+      const real* Em = getE(t, i + 2, k - 2);
+      int Sm = SG(t, k - 1);
+      for (int z = tt->start[i + 1]; z < tt->start[i + 2]; ++z)
+        for (int z2 = tt->start[k - 1]; z2 < tt->start[k]; ++z2) {
+          const orc_op *o = &tt->ops[z], *r = &tt->ops[z2];
+          if (o->a == ap) Ls[nL++] = (side){z, z2, o->b, r->b, r->c, (real)o->x * Em[o->c * Sm + r->a] * (real)r->x};
+        }
+    }
+    if (l2 == 0) { Rs[nR++] = (side){-1, -1, 0, 0, cp, 1}; }
+    else if (l2 == 1) {
+      for (int z = tt->start[j - 1]; z < tt->start[j]; ++z) {
+        const orc_op* o = &tt->ops[z];
+        if (o->c == cp) Rs[nR++] = (side){z, -1, o->b, o->b, o->a, (real)o->x};
+      }
+    } else {
+      const real* Em = getE(t, l + 2, j - 2);
+      int Sm = SG(t, j - 1);
+      /* z1 = operator at l+1 (gives v'), z2 = operator at j-1 (gives v); s = left bond of l+1 */
+      for (int z = tt->start[l + 1]; z < tt->start[l + 2]; ++z)
+        for (int z2 = tt->start[j - 1]; z2 < tt->start[j]; ++z2) {
+          const orc_op *o = &tt->ops[z], *r = &tt->ops[z2];
+          if (r->c == cp) Rs[nR++] = (side){z, z2, r->b, o->b, o->a, (real)o->x * Em[o->c * Sm + r->a] * (real)r->x};
+        }
+    }
+    /* for the right side: .u = v (at j-1), .up = v' (at l+1), .s = t (right bond of the inner cell) */
+    alt_reset(&c->L);
+    for (int a_ = 0; a_ < nL; ++a_)
+      for (int b_ = 0; b_ < nR; ++b_)
+        for (int xp = 0; xp < 4; ++xp)
+          for (int yp = 0; yp < 4; ++yp) {
+            real w = 0;
+            if (can_pair(m, xp, yp)) {
+              real e;
+              if (l1 == 0 && l2 == 0) e = t->wst[P][ptype(xp, yp)];
+              else if (l1 == 0 || l2 == 0) e = t->wbu[l1 + l2] * (l1 + l2 == 1 ? t->wst[P][ptype(xp, yp)] : 1.0L);
+              else e = t->win[l1 + l2] * t->wtm[P][Ls[a_].u][Rs[b_].u] * t->wtm[ptype(yp, xp)][Rs[b_].up][Ls[a_].up];
+              w = e * Ls[a_].w * Rs[b_].w * qin[((Ls[a_].s * 4 + xp) * 4 + yp) * St + Rs[b_].s];
+            }
+            alt_push(&c->L, w);
+          }
+    int pk = alt_pick(&c->L, tb_u(c, K_ILOOP, i, j));
+    int yp = pk % 4, xp = (pk / 4) % 4, b_ = (pk / 16) % nR, a_ = pk / (16 * nR);
+    side SL = Ls[a_], SR = Rs[b_];
+    if (l1 == 1) { c->seq[i + 1] = (uint8_t)SL.u; }
+    else if (l1 >= 2) {
+      c->seq[i + 1] = (uint8_t)SL.u; c->seq[k - 1] = (uint8_t)SL.up;
+      tb_chain(c, i + 2, k - 2, tt->ops[SL.z1].c, tt->ops[SL.z2].a);
+    }
+    if (l2 == 1) { c->seq[j - 1] = (uint8_t)SR.u; }
+    else if (l2 >= 2) {
+      c->seq[j - 1] = (uint8_t)SR.u; c->seq[l + 1] = (uint8_t)SR.up;
+      tb_chain(c, l + 2, j - 2, tt->ops[SR.z1].c, tt->ops[SR.z2].a);
+    }
+    tb_push(c, (tb_item){IT_QB, k, l, SL.s, xp, yp, SR.s});
+    free(Ls); free(Rs);
+  } else {
+    tb_push(c, (tb_item){IT_QM, i + 1, A.k - 1, ap, 0, 0, A.s});
+    tb_push(c, (tb_item){IT_QM1, A.k, j - 1, A.s, 0, 0, cp});
+  }
+  free(UpL); free(UpR);
+}
+
+static void tb_run(tb_ctx* c) {
+  const orc_tables* t = c->t;
+  const orc_model* m = &t->model;
+  const orc_tt* tt = t->tt;
+  int n = t->n;
+  for (int p = 0; p < n; ++p) { c->seq[p] = 255; c->pair[p] = -1; }
+  c->sp = 0;
+  /* TOP */
+  alt_reset(&c->L);
+  for (int cc = 0; cc < SG(t, n); ++cc) alt_push(&c->L, t->qext[n][cc]);
+  int cb = alt_pick(&c->L, tb_u(c, K_TOP, 0, 0));
+  /* EXT(j,c) */
+  int j = n - 1;
+  while (j >= 0) {
+    alt_reset(&c->L);
+    int z0 = tt->start[j], z1 = tt->start[j + 1];
+    for (int z = z0; z < z1; ++z) {
+      const orc_op* o = &tt->ops[z];
+      alt_push(&c->L, o->c == cb ? t->qext[j][o->a] * (real)o->x : 0);
+    }
+    int nops = z1 - z0;
+    int Sj1 = SG(t, j + 1);
+    /* k ascending, s ascending, (x,y) lexicographic */
+    int* koff = (int*)calloc(j + 2, sizeof(int));
+    for (int k = 0; k <= j - (m->min_hairpin + 1); ++k) {
+      koff[k] = c->L.n;
+      const real* qb = t->qb[(size_t)k * n + j];
+      for (int s = 0; s < SG(t, k); ++s)
+        for (int xy = 0; xy < 16; ++xy) alt_push(&c->L, t->qext[k][s] * qb[(s * 16 + xy) * Sj1 + cb]);
+    }
+    int pk = alt_pick(&c->L, tb_u(c, K_EXT, j, 0));
+    if (pk < nops) {
+      const orc_op* o = &tt->ops[z0 + pk];
+      c->seq[j] = (uint8_t)o->b;
+      cb = o->a;
+      j = j - 1;
+    } else {
+      int k = 0;
+      while (k + 1 <= j - (m->min_hairpin + 1) && koff[k + 1] <= pk) ++k;
+      int r = pk - koff[k];
+      int s = r / 16, xy = r % 16;
+      tb_push(c, (tb_item){IT_QB, k, j, s, xy / 4, xy % 4, cb});
+      cb = s;
+      j = k - 1;
+    }
+    free(koff);
+  }
+  while (c->sp > 0) {
+    tb_item it = c->stk[--c->sp];
+    int i = it.i;
+    j = it.j;
+    int Sj1 = SG(t, j + 1);
+    if (it.type == IT_QB) {
+      tb_qb(c, it);
+    } else if (it.type == IT_QM) {
+      /* QM(i,j,a,c): {QML part}, then {k asc, s asc: Qm(i,k-1)[a,s] Qm1(k,j)[s,c]} */
+      alt_reset(&c->L);
+      alt_push(&c->L, t->qml[(size_t)i * n + j][it.a * Sj1 + it.c]);
+      int* koff = (int*)calloc(j + 2, sizeof(int));
+      for (int k = i + 1; k <= j; ++k) {
+        koff[k] = c->L.n;
+        const real* A = t->qm[(size_t)i * n + (k - 1)];
+        const real* B = t->qm1[(size_t)k * n + j];
+        int Sk = SG(t, k);
+        for (int s = 0; s < Sk; ++s) alt_push(&c->L, A[it.a * Sk + s] * B[s * Sj1 + it.c]);
+      }
+      int pk = alt_pick(&c->L, tb_u(c, K_QM, i, j));
+      if (pk == 0) tb_push(c, (tb_item){IT_QML, i, j, it.a, 0, 0, it.c});
+      else {
+        int k = i + 1;
+        while (k + 1 <= j && koff[k + 1] <= pk) ++k;
+        int s = pk - koff[k];
+        tb_push(c, (tb_item){IT_QM, i, k - 1, it.a, 0, 0, s});
+        tb_push(c, (tb_item){IT_QM1, k, j, s, 0, 0, it.c});
+      }
+      free(koff);
+    } else if (it.type == IT_QML) {
+      /* QML(i,j,a,c): {Qm1(i,j)[a,c]}, then {z at i with a(z)=a: w_b x(z) Qml(i+1,j)[c(z),c]} */
+      alt_reset(&c->L);
+      alt_push(&c->L, t->qm1[(size_t)i * n + j][it.a * Sj1 + it.c]);
+      int z0 = tt->start[i], z1 = tt->start[i + 1];
+      for (int z = z0; z < z1; ++z) {
+        const orc_op* o = &tt->ops[z];
+        real w = 0;
+        if (o->a == it.a && i + 1 <= j) w = t->wb * (real)o->x * t->qml[(size_t)(i + 1) * n + j][o->c * Sj1 + it.c];
+        alt_push(&c->L, w);
+      }
+      int pk = alt_pick(&c->L, tb_u(c, K_QML, i, j));
+      if (pk == 0) tb_push(c, (tb_item){IT_QM1, i, j, it.a, 0, 0, it.c});
+      else {
+        const orc_op* o = &tt->ops[z0 + pk - 1];
+        c->seq[i] = (uint8_t)o->b;
+        tb_push(c, (tb_item){IT_QML, i + 1, j, o->c, 0, 0, it.c});
+      }
+    } else {
+      /* QM1(i,j,a,c): {(x,y): w_c Qb(i,j)[a,x,y,c]}, then {z at j with c(z)=c: w_b Qm1(i,j-1)[a,a(z)] x(z)} */
+      alt_reset(&c->L);
+      const real* qb = t->qb[(size_t)i * n + j];
+      for (int xy = 0; xy < 16; ++xy) alt_push(&c->L, t->wc * qb[(it.a * 16 + xy) * Sj1 + it.c]);
+      int z0 = tt->start[j], z1 = tt->start[j + 1];
+      for (int z = z0; z < z1; ++z) {
+        const orc_op* o = &tt->ops[z];
+        real w = 0;
+        if (o->c == it.c && j - 1 >= i) w = t->wb * t->qm1[(size_t)i * n + (j - 1)][it.a * SG(t, j) + o->a] * (real)o->x;
+        alt_push(&c->L, w);
+      }
+      int pk = alt_pick(&c->L, tb_u(c, K_QM1, i, j));
+      if (pk < 16) tb_push(c, (tb_item){IT_QB, i, j, it.a, pk / 4, pk % 4, it.c});
+      else {
+        const orc_op* o = &tt->ops[z0 + pk - 16];
+        c->seq[j] = (uint8_t)o->b;
+        tb_push(c, (tb_item){IT_QM1, i, j - 1, it.a, 0, 0, o->a});
+      }
+    }
+  }
+}
+
+int orc_sample(const orc_tables* t, int J, uint64_t seed, uint8_t* seq, int32_t* pair) {
+  int n = t->n;
+#pragma omp parallel
+  {
+    tb_ctx c;
+    memset(&c, 0, sizeof(c));
+    c.t = t; c.seed = seed;
+#pragma omp for schedule(dynamic, 1)
+    for (int s = 0; s < J; ++s) {
+      c.sample = s;
+      c.seq = seq + (size_t)s * n;
+      c.pair = pair + (size_t)s * n;
+      tb_run(&c);
+    }
+    free(c.L.w); free(c.stk);
+  }
+  return 0;
+}
+
+int orc_marginals(orc_tables* t, double* bpp, double* base, double* codon) {
+  (void)t; (void)bpp; (void)base; (void)codon;
+  return -99; /* implemented in cdz_oracle_outside.c */
+}
