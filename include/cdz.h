@@ -1,0 +1,156 @@
+/*
+ * cdz.h -- C ABI of the B200 (sm_100a) codon-design inside-pass library.
+ *
+ * Hot path of arXiv 2604.19718 ("Direct RNA sequence design under codon constraints
+ * using expressive tensor-based secondary structure models"), specialised as
+ * BASELINE.json `north_star` fixes it: the tensor-valued inside (partition-function)
+ * recursion over all coding sequences Phi(psi) (eqs 2.1-2.4, lines 57-72)
+ * and all unpseudoknotted structures, with a McCaskill-style nearest-neighbour loop
+ * model; sequence summation enters through the RNA-sequence tensor train (eq 3.1,
+ * line 131) exactly as in chi-hat (eq 3.8).
+ *
+ * Conventions
+ *   positions 0..n-1 (n = 3L); nucleotides A,C,G,U = 0..3 (line 548); codon index
+ *   16*b0 + 4*b1 + b2; pair types AU=0 CG=1 GC=2 UA=3 GU=4 UG=5.
+ *   Pointers named *_dev are CUDA device pointers, all others are host pointers.
+ *   `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *   All functions return 0 on success or a negative cdz_status; the text of the
+ *   last error of the calling thread is available from cdz_last_error().
+ *   Handles are created by the library, owned by the caller and released with the
+ *   matching *_destroy.  The library never falls back to a CPU implementation.
+ */
+#ifndef CDZ_H
+#define CDZ_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  CDZ_OK = 0,
+  CDZ_EINVAL = -1,    /* bad argument, unknown residue, non-finite weight */
+  CDZ_ENOMEM = -2,    /* host or device allocation failed / workspace too small */
+  CDZ_ECUDA = -3,     /* a CUDA runtime call or kernel failed */
+  CDZ_EOVERFLOW = -4, /* dynamic range left the representable window despite rescaling */
+  CDZ_ESTATE = -5     /* call order (e.g. sampling before the inside pass finished) */
+} cdz_status;
+
+enum { CDZ_TT_SINGLE_CODON = 0, CDZ_TT_CODON_PAIR = 1 };
+enum { CDZ_FP64 = 0, CDZ_FP32_SCALED = 1 };
+
+/* Nearest-neighbour loop model (BASELINE.json configs[0]); energies in kcal/mol.
+ *   hairpin(l)  = hairpin_a + hairpin_b * kT * ln(l / hairpin_l0) + tmm[p(i,j)][phi_{i+1}][phi_{j-1}],  l >= min_hairpin
+ *   stack       = stack[p(i,j)][p(k,l)]            closing pair (phi_i,phi_j), inner pair (phi_k,phi_l)
+ *   bulge(l)    = bulge_init[l] (+ stack[..] if l == 1),  1 <= l <= max_interior
+ *   interior    = interior_init[l1+l2] + tmm[p(i,j)][phi_{i+1}][phi_{j-1}] + tmm[p(l,k)][phi_{l+1}][phi_{k-1}]
+ *   multiloop   = ml_a + ml_b * unpaired + ml_c * (branches + 1);   exterior loop = 0
+ * kT = R * temperature_K, R = 8.31446261815324/4184 kcal/(mol K).  No symmetry is enforced. */
+typedef struct {
+  double temperature_K;
+  double stack[6][6];
+  double tmm[6][4][4];
+  double hairpin_a, hairpin_b, hairpin_l0;
+  double bulge_init[31];    /* index 1..30 */
+  double interior_init[31]; /* index 2..30 */
+  double ml_a, ml_b, ml_c;
+  int32_t max_interior;     /* <= 30 */
+  int32_t min_hairpin;      /* >= 3 */
+  int32_t allow_all_pairs;  /* test mode: any two nucleotides may pair (non-canonical use pair type 0) */
+} cdz_nn_params;
+
+/* One tensor-train operator (a,b,c,x) of PAPER.md S3c (lines 545-557):
+ * T_i[a,b,c] += x, a in [Sigma_i], b a nucleotide, c in [Sigma_{i+1}], x > 0. */
+typedef struct { int32_t a, b, c; double x; } cdz_op;
+
+typedef struct cdz_model cdz_model;
+typedef struct cdz_tt cdz_tt;
+typedef struct cdz_tables cdz_tables;
+
+/* Result / accounting record filled by cdz_tables_info (host). */
+typedef struct {
+  int32_t n;                /* nucleotides */
+  int32_t sigma_bar;        /* sum_{i<n} Sigma_i */
+  int32_t n_left_states;    /* sum_i |L_i|, distinct (sigma_i, phi_i) */
+  int32_t n_right_states;   /* sum_j |R_j|, distinct (phi_j, sigma_{j+1}) */
+  int32_t precision;
+  int32_t n_rescales;       /* dynamic rescale events during the pass */
+  double n_cc;              /* structurally non-zero split-point terms (i,k,j) */
+  double n_loop;            /* one-inner-pair terms (i,j,l1,l2) */
+  double split_mac;         /* exact multiply-adds of the split-point contraction */
+  double table_bytes;       /* device bytes held by the handle */
+  double bytes_per_cell;    /* table_bytes / (n(n+1)/2) */
+  double log_scale;         /* sum_m s_m ln 2 added back into log Z */
+  double inside_ms;         /* device time of the last inside pass (CUDA events) */
+} cdz_info;
+
+const char* cdz_last_error(void);
+int cdz_version(void);
+
+/* ---- model ---------------------------------------------------------------- */
+int cdz_model_create(const cdz_nn_params* params, cdz_model** out);
+void cdz_model_destroy(cdz_model* m);
+
+/* ---- tensor train (host, O(n)) -------------------------------------------- */
+/* Codon tensor train of an amino-acid string aa[0..L) over "ACDEFGHIKLMNPQRSTVWY".
+ *   kind = CDZ_TT_SINGLE_CODON: eq 3.4 (line 151), operator lists of S3c.i (lines 559-563);
+ *   kind = CDZ_TT_CODON_PAIR  : eq 3.3 (line 145) in the S3c.ii form (lines 565-569).
+ * codon_logw: [64] (or NULL): factor e^{+w} on the middle-base operator of that codon (line 157).
+ * pair_logw : [64*64] row = 5' codon (or NULL; CODON_PAIR only): factor on the 5'-base operator (line 163).
+ * Open chain: Sigma_0 = 1, the last bond is summed out. */
+int cdz_tt_build(const char* aa, int L, int kind, const double* codon_logw, const double* pair_logw, cdz_tt** out);
+/* Generic operator lists (lines 545-557, noncoding bases line 573). counts[n], ops[sum counts]. Bond dims <= 8. */
+int cdz_tt_from_operators(int n, const int32_t* counts, const cdz_op* ops, cdz_tt** out);
+void cdz_tt_destroy(cdz_tt* tt);
+int cdz_tt_length(const cdz_tt* tt);
+/* sigma[n+1], counts[n] (either may be NULL); returns total operator count */
+int cdz_tt_describe(const cdz_tt* tt, int32_t* sigma, int32_t* counts);
+
+/* ---- inside pass (device) -------------------------------------------------- */
+/* Device bytes cdz_inside needs for (tt, precision); the caller may allocate them
+ * (e.g. as a torch uint8 tensor) and pass the pointer as workspace_dev. */
+int cdz_workspace_bytes(const cdz_tt* tt, int precision, size_t* bytes);
+/* Runs the whole inside recursion (all anti-diagonals, exterior, log Z) asynchronously on `stream`.
+ * workspace_dev may be NULL (the library allocates and owns the tables) or a device
+ * buffer of >= cdz_workspace_bytes bytes that must outlive the handle.
+ * logZ_host (may be NULL) is written by a host-side epilogue after the pass: the call
+ * synchronises `stream` only if logZ_host != NULL; otherwise use cdz_tables_logz. */
+int cdz_inside(const cdz_model* m, const cdz_tt* tt, int precision, void* workspace_dev, size_t workspace_bytes,
+               void* stream, cdz_tables** out, double* logZ_host);
+/* B independent designs advanced together (BASELINE.json configs[4]); workspace_dev[b] may be NULL. */
+int cdz_inside_batch(const cdz_model* m, const cdz_tt* const* tts, int B, int precision, void* const* workspace_dev,
+                     const size_t* workspace_bytes, void* stream, cdz_tables** out, double* logZ_host);
+/* Re-run the pass on an existing handle (same tt/model); used by the timing harness. */
+int cdz_inside_rerun(cdz_tables* t, void* stream);
+int cdz_inside_rerun_batch(cdz_tables* const* t, int B, void* stream);
+/* Synchronises the handle's stream and returns log Z = -q_psi (eq 2.4). */
+int cdz_tables_logz(cdz_tables* t, double* logZ_host);
+int cdz_tables_info(cdz_tables* t, cdz_info* info);
+void cdz_tables_destroy(cdz_tables* t);
+/* Debug / parity access: copy one cell to host as doubles (true value * 2^-shift_out).
+ * which: 0 Qb as [a][x][y][c] dense, 1 Qbs, 2 Qm1, 3 Qml, 4 M2, 5 Qm (all [a][c]). Returns element count. */
+int cdz_tables_cell(cdz_tables* t, int which, int i, int j, double* out_host, int* shift_out);
+/* log Qext(j)[c] (natural log, scale included) */
+int cdz_tables_logqext(cdz_tables* t, int j, int c, double* out_host);
+
+/* ---- exact Boltzmann samples (device) ------------------------------------- */
+/* J i.i.d. samples (phi, s) ~ W(phi) exp(-E/kT) / Z by stochastic traceback (PAPER.md S4c,
+ * Alg S4.4; decision order in DESIGN.md).  seq_dev [J][n] uint8 (0..3),
+ * pair_dev [J][n] int32 partner or -1.  Uniforms are U(seed, sample, kind, i, j). */
+int cdz_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* pair_dev, void* stream);
+
+/* ---- marginals (device) ---------------------------------------------------- */
+/* bpp_dev [n][n]: upper triangle P(i.j) (eq 2.5), diagonal P(i unpaired); base_dev [n][4] (eq 2.6);
+ * codon_dev [L][64] (eq 2.7).  Any may be NULL. */
+int cdz_marginals(cdz_tables* t, double* bpp_dev, double* base_dev, double* codon_dev, void* stream);
+
+/* ---- convenience: host buffers end to end (used for the e2e timing) -------- */
+/* Builds nothing: runs cdz_inside_rerun, samples J states and copies them to host buffers. */
+int cdz_run_host(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_host, int32_t* pair_host, double* logZ_host,
+                 void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

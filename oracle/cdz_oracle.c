@@ -867,6 +867,19 @@ static int alt_pick(const altlist* L, double u) {
   return last;
 }
 
+/* same, with the total taken from the stored table entry that the alternatives decompose */
+static int alt_pick_total(const altlist* L, double u, real tot) {
+  real thr = (real)u * tot, run = 0;
+  int last = -1;
+  for (int k = 0; k < L->n; ++k) {
+    if (L->w[k] <= 0) continue;
+    run += L->w[k];
+    last = k;
+    if (run > thr) return k;
+  }
+  return last;
+}
+
 typedef struct {
   const orc_tables* t;
   uint64_t seed; int sample;
@@ -915,7 +928,10 @@ static void tb_qb(tb_ctx* c, tb_item it) {
   c->pair[i] = j; c->pair[j] = i;
   real wh = expl(-(real)(hairpin_init(m, d - 1) * t->beta));
   int Sc = SG(t, j);
-  /* level A: (z_i, z_j) x {hairpin, (k asc, l desc), multiloop (k asc, s asc)} */
+  /* level A, in the order of DESIGN.md "Traceback order":
+   *   hairpin | stack | multiloop (k asc, s asc) | one inner pair by l1+l2 = 1,2,.. then l1 asc;
+   * within each, the operator pairs (z_i, z_j) in list order (z_i outer).  For the multiloop the
+   * operator pair is the outer loop.  The threshold is u * (stored Qb entry). */
   typedef struct { int zi, zj, kind, k, l, s; } altA;
   altA* desc = NULL; int nd = 0, capd = 0;
 #define PUSHA(W, ...) do { if (nd == capd) { capd = capd ? 2 * capd : 512; desc = (altA*)realloc(desc, sizeof(altA) * capd); } \
@@ -925,80 +941,98 @@ static void tb_qb(tb_ctx* c, tb_item it) {
   for (int p = i; p <= j + 1; ++p) if (SG(t, p) > maxS) maxS = SG(t, p);
   real* UpL = cell_alloc((size_t)maxS * 16 * maxS);
   real* UpR = cell_alloc((size_t)maxS * 16 * maxS);
-  for (int zi = tt->start[i]; zi < tt->start[i + 1]; ++zi) {
-    const orc_op* oi = &tt->ops[zi];
-    if (oi->a != it.a || oi->b != x) continue;
+  /* the operator pairs compatible with (a,x) and (y,c) */
+  int npz = 0;
+  int* pzi = (int*)calloc((size_t)(tt->start[i + 1] - tt->start[i]) * (tt->start[j + 1] - tt->start[j]) + 1, sizeof(int));
+  int* pzj = (int*)calloc((size_t)(tt->start[i + 1] - tt->start[i]) * (tt->start[j + 1] - tt->start[j]) + 1, sizeof(int));
+  for (int zi = tt->start[i]; zi < tt->start[i + 1]; ++zi)
     for (int zj = tt->start[j]; zj < tt->start[j + 1]; ++zj) {
-      const orc_op* oj = &tt->ops[zj];
-      if (oj->b != y || oj->c != it.c) continue;
-      real w0 = (real)oi->x * (real)oj->x;
-      int ap = oi->c, cp = oj->a;
-      /* hairpin */
-      {
-        compute_Up(t, i + 1, j - 1, UpL);
-        real s = 0;
-        for (int u = 0; u < 4; ++u)
-          for (int v = 0; v < 4; ++v) s += wh * t->wtm[P][u][v] * UpL[((ap * 4 + u) * 4 + v) * Sc + cp];
-        PUSHA(w0 * s, zi, zj, 0, 0, 0, 0);
-      }
-      for (int k = i + 1; k < j; ++k)
-        for (int l = j - 1; l > k; --l) {
-          int l1 = k - i - 1, l2 = j - l - 1;
-          if (l1 + l2 > m->max_interior) break;
-          if (l - k < m->min_hairpin + 1) continue;
-          const real* qin = t->qb[(size_t)k * n + l];
-          int Ss = SG(t, k), St = SG(t, l + 1);
-          real s = 0;
-          for (int xp = 0; xp < 4; ++xp)
-            for (int yp = 0; yp < 4; ++yp) {
-              if (!can_pair(m, xp, yp)) continue;
-              if (l1 == 0 && l2 == 0) {
-                s += t->wst[P][ptype(xp, yp)] * qin[((ap * 4 + xp) * 4 + yp) * St + cp];
-              } else if (l2 == 0) {
-                const real* El = getE(t, i + 1, k - 1);
-                real w = t->wbu[l1] * (l1 == 1 ? t->wst[P][ptype(xp, yp)] : 1.0L);
-                for (int sb = 0; sb < Ss; ++sb) s += w * El[ap * Ss + sb] * qin[((sb * 4 + xp) * 4 + yp) * St + cp];
-              } else if (l1 == 0) {
-                const real* Er = getE(t, l + 1, j - 1);
-                real w = t->wbu[l2] * (l2 == 1 ? t->wst[P][ptype(xp, yp)] : 1.0L);
-                for (int tb = 0; tb < St; ++tb) s += w * qin[((ap * 4 + xp) * 4 + yp) * St + tb] * Er[tb * Sc + cp];
-              }
-            }
-          if (l1 > 0 && l2 > 0) {
-            compute_Up(t, i + 1, k - 1, UpL);
-            compute_Up(t, l + 1, j - 1, UpR);
-            for (int u = 0; u < 4; ++u)
-              for (int up = 0; up < 4; ++up)
-                for (int sb = 0; sb < Ss; ++sb) {
-                  real wl = UpL[((ap * 4 + u) * 4 + up) * Ss + sb];
-                  if (wl == 0) continue;
-                  for (int xp = 0; xp < 4; ++xp)
-                    for (int yp = 0; yp < 4; ++yp) {
-                      if (!can_pair(m, xp, yp)) continue;
-                      for (int tb = 0; tb < St; ++tb) {
-                        real wq = qin[((sb * 4 + xp) * 4 + yp) * St + tb];
-                        if (wq == 0) continue;
-                        for (int vp = 0; vp < 4; ++vp)
-                          for (int v = 0; v < 4; ++v)
-                            s += t->win[l1 + l2] * t->wtm[P][u][v] * t->wtm[ptype(yp, xp)][vp][up] * wl * wq *
-                                 UpR[((tb * 4 + vp) * 4 + v) * Sc + cp];
-                      }
-                    }
-                }
-          }
-          PUSHA(w0 * s, zi, zj, 1, k, l, 0);
-        }
-      /* multiloop: k = 5' end of the last branch */
-      for (int k = i + 2; k <= j - 1; ++k) {
-        const real* A = t->qm[(size_t)(i + 1) * n + (k - 1)];
-        const real* B = t->qm1[(size_t)k * n + (j - 1)];
-        int Sk = SG(t, k);
-        for (int sb = 0; sb < Sk; ++sb) PUSHA(w0 * t->wa * t->wc * A[ap * Sk + sb] * B[sb * Sc + cp], zi, zj, 2, k, 0, sb);
-      }
+      const orc_op *oi = &tt->ops[zi], *oj = &tt->ops[zj];
+      if (oi->a != it.a || oi->b != x || oj->b != y || oj->c != it.c) continue;
+      pzi[npz] = zi; pzj[npz] = zj; ++npz;
     }
+  int tmax = d - 2 - (m->min_hairpin + 1);
+  if (tmax > m->max_interior) tmax = m->max_interior;
+  for (int seg = 0; seg < 3 + (tmax >= 1 ? tmax : 0); ++seg) {
+    /* seg 0 hairpin, 1 stack, 2 multiloop, 3.. one inner pair of total size seg-2 */
+    int tot_sz = seg == 1 ? 0 : seg - 2;
+    if (seg == 1 && tmax < 0) continue;
+    int nl1 = (seg == 0 || seg == 2) ? 1 : tot_sz + 1;
+    if (seg == 2) {
+      for (int pz = 0; pz < npz; ++pz) {
+        const orc_op *oi = &tt->ops[pzi[pz]], *oj = &tt->ops[pzj[pz]];
+        real w0 = (real)oi->x * (real)oj->x;
+        int ap = oi->c, cp = oj->a;
+        for (int k = i + 2; k <= j - 1; ++k) {
+          const real* A = t->qm[(size_t)(i + 1) * n + (k - 1)];
+          const real* B = t->qm1[(size_t)k * n + (j - 1)];
+          int Sk = SG(t, k);
+          for (int sb = 0; sb < Sk; ++sb) PUSHA(w0 * t->wa * t->wc * A[ap * Sk + sb] * B[sb * Sc + cp], pzi[pz], pzj[pz], 2, k, 0, sb);
+        }
+      }
+      continue;
+    }
+    for (int l1 = 0; l1 < nl1; ++l1)
+      for (int pz = 0; pz < npz; ++pz) {
+        const orc_op *oi = &tt->ops[pzi[pz]], *oj = &tt->ops[pzj[pz]];
+        real w0 = (real)oi->x * (real)oj->x;
+        int ap = oi->c, cp = oj->a;
+        if (seg == 0) {
+          compute_Up(t, i + 1, j - 1, UpL);
+          real s = 0;
+          for (int u = 0; u < 4; ++u)
+            for (int v = 0; v < 4; ++v) s += wh * t->wtm[P][u][v] * UpL[((ap * 4 + u) * 4 + v) * Sc + cp];
+          PUSHA(w0 * s, pzi[pz], pzj[pz], 0, 0, 0, 0);
+          continue;
+        }
+        int l2 = tot_sz - l1;
+        int k = i + 1 + l1, l = j - 1 - l2;
+        const real* qin = t->qb[(size_t)k * n + l];
+        int Ss = SG(t, k), St = SG(t, l + 1);
+        real s = 0;
+        for (int xp = 0; xp < 4; ++xp)
+          for (int yp = 0; yp < 4; ++yp) {
+            if (!can_pair(m, xp, yp)) continue;
+            if (l1 == 0 && l2 == 0) {
+              s += t->wst[P][ptype(xp, yp)] * qin[((ap * 4 + xp) * 4 + yp) * St + cp];
+            } else if (l2 == 0) {
+              const real* El = getE(t, i + 1, k - 1);
+              real w = t->wbu[l1] * (l1 == 1 ? t->wst[P][ptype(xp, yp)] : 1.0L);
+              for (int sb = 0; sb < Ss; ++sb) s += w * El[ap * Ss + sb] * qin[((sb * 4 + xp) * 4 + yp) * St + cp];
+            } else if (l1 == 0) {
+              const real* Er = getE(t, l + 1, j - 1);
+              real w = t->wbu[l2] * (l2 == 1 ? t->wst[P][ptype(xp, yp)] : 1.0L);
+              for (int tb = 0; tb < St; ++tb) s += w * qin[((ap * 4 + xp) * 4 + yp) * St + tb] * Er[tb * Sc + cp];
+            }
+          }
+        if (l1 > 0 && l2 > 0) {
+          compute_Up(t, i + 1, k - 1, UpL);
+          compute_Up(t, l + 1, j - 1, UpR);
+          for (int u = 0; u < 4; ++u)
+            for (int up = 0; up < 4; ++up)
+              for (int sb = 0; sb < Ss; ++sb) {
+                real wl = UpL[((ap * 4 + u) * 4 + up) * Ss + sb];
+                if (wl == 0) continue;
+                for (int xp = 0; xp < 4; ++xp)
+                  for (int yp = 0; yp < 4; ++yp) {
+                    if (!can_pair(m, xp, yp)) continue;
+                    for (int tb = 0; tb < St; ++tb) {
+                      real wq = qin[((sb * 4 + xp) * 4 + yp) * St + tb];
+                      if (wq == 0) continue;
+                      for (int vp = 0; vp < 4; ++vp)
+                        for (int v = 0; v < 4; ++v)
+                          s += t->win[l1 + l2] * t->wtm[P][u][v] * t->wtm[ptype(yp, xp)][vp][up] * wl * wq *
+                               UpR[((tb * 4 + vp) * 4 + v) * Sc + cp];
+                    }
+                  }
+              }
+        }
+        PUSHA(w0 * s, pzi[pz], pzj[pz], 1, k, l, 0);
+      }
   }
+  free(pzi); free(pzj);
 #undef PUSHA
-  int pick = alt_pick(&c->L, tb_u(c, K_QB, i, j));
+  int pick = alt_pick_total(&c->L, tb_u(c, K_QB, i, j), t->qb[(size_t)i * n + j][((it.a * 4 + x) * 4 + y) * SG(t, j + 1) + it.c]);
   altA A = desc[pick];
   free(desc);
   const orc_op *oi = &tt->ops[A.zi], *oj = &tt->ops[A.zj];
@@ -1129,7 +1163,7 @@ static void tb_run(tb_ctx* c) {
       for (int s = 0; s < SG(t, k); ++s)
         for (int xy = 0; xy < 16; ++xy) alt_push(&c->L, t->qext[k][s] * qb[(s * 16 + xy) * Sj1 + cb]);
     }
-    int pk = alt_pick(&c->L, tb_u(c, K_EXT, j, 0));
+    int pk = alt_pick_total(&c->L, tb_u(c, K_EXT, j, 0), t->qext[j + 1][cb]);
     if (pk < nops) {
       const orc_op* o = &tt->ops[z0 + pk];
       c->seq[j] = (uint8_t)o->b;
@@ -1165,7 +1199,7 @@ static void tb_run(tb_ctx* c) {
         int Sk = SG(t, k);
         for (int s = 0; s < Sk; ++s) alt_push(&c->L, A[it.a * Sk + s] * B[s * Sj1 + it.c]);
       }
-      int pk = alt_pick(&c->L, tb_u(c, K_QM, i, j));
+      int pk = alt_pick_total(&c->L, tb_u(c, K_QM, i, j), t->qm[(size_t)i * n + j][it.a * Sj1 + it.c]);
       if (pk == 0) tb_push(c, (tb_item){IT_QML, i, j, it.a, 0, 0, it.c});
       else {
         int k = i + 1;
@@ -1186,7 +1220,7 @@ static void tb_run(tb_ctx* c) {
         if (o->a == it.a && i + 1 <= j) w = t->wb * (real)o->x * t->qml[(size_t)(i + 1) * n + j][o->c * Sj1 + it.c];
         alt_push(&c->L, w);
       }
-      int pk = alt_pick(&c->L, tb_u(c, K_QML, i, j));
+      int pk = alt_pick_total(&c->L, tb_u(c, K_QML, i, j), t->qml[(size_t)i * n + j][it.a * Sj1 + it.c]);
       if (pk == 0) tb_push(c, (tb_item){IT_QM1, i, j, it.a, 0, 0, it.c});
       else {
         const orc_op* o = &tt->ops[z0 + pk - 1];
@@ -1205,7 +1239,7 @@ static void tb_run(tb_ctx* c) {
         if (o->c == it.c && j - 1 >= i) w = t->wb * t->qm1[(size_t)i * n + (j - 1)][it.a * SG(t, j) + o->a] * (real)o->x;
         alt_push(&c->L, w);
       }
-      int pk = alt_pick(&c->L, tb_u(c, K_QM1, i, j));
+      int pk = alt_pick_total(&c->L, tb_u(c, K_QM1, i, j), t->qm1[(size_t)i * n + j][it.a * Sj1 + it.c]);
       if (pk < 16) tb_push(c, (tb_item){IT_QB, i, j, it.a, pk / 4, pk % 4, it.c});
       else {
         const orc_op* o = &tt->ops[z0 + pk - 16];

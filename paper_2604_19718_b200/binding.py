@@ -1,0 +1,287 @@
+"""Thin ctypes binding of libcdz.so (include/cdz.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of csrc/; torch is used for device
+memory (workspace, outputs) and streams.  There is no CPU fallback: if the shared library
+is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcdz.so")
+
+TT_SINGLE_CODON, TT_CODON_PAIR = 0, 1
+FP64, FP32_SCALED = 0, 1
+
+EXPORTS = [
+    "cdz_last_error", "cdz_version", "cdz_model_create", "cdz_model_destroy", "cdz_tt_build",
+    "cdz_tt_from_operators", "cdz_tt_destroy", "cdz_tt_length", "cdz_tt_describe", "cdz_workspace_bytes",
+    "cdz_inside", "cdz_inside_batch", "cdz_inside_rerun", "cdz_inside_rerun_batch", "cdz_tables_logz",
+    "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample",
+    "cdz_marginals", "cdz_run_host",
+]
+
+
+class CdzError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"cdz error {code}: {msg}")
+        self.code = code
+
+
+class NNParams(C.Structure):
+    _fields_ = [
+        ("temperature_K", C.c_double), ("stack", C.c_double * 36), ("tmm", C.c_double * 96),
+        ("hairpin_a", C.c_double), ("hairpin_b", C.c_double), ("hairpin_l0", C.c_double),
+        ("bulge_init", C.c_double * 31), ("interior_init", C.c_double * 31),
+        ("ml_a", C.c_double), ("ml_b", C.c_double), ("ml_c", C.c_double),
+        ("max_interior", C.c_int32), ("min_hairpin", C.c_int32), ("allow_all_pairs", C.c_int32),
+    ]
+
+
+class Op(C.Structure):
+    _fields_ = [("a", C.c_int32), ("b", C.c_int32), ("c", C.c_int32), ("x", C.c_double)]
+
+
+class Info(C.Structure):
+    _fields_ = [
+        ("n", C.c_int32), ("sigma_bar", C.c_int32), ("n_left_states", C.c_int32), ("n_right_states", C.c_int32),
+        ("precision", C.c_int32), ("n_rescales", C.c_int32), ("n_cc", C.c_double), ("n_loop", C.c_double),
+        ("split_mac", C.c_double), ("table_bytes", C.c_double), ("bytes_per_cell", C.c_double),
+        ("log_scale", C.c_double), ("inside_ms", C.c_double),
+    ]
+
+
+_lib = None
+
+
+def lib():
+    """Load libcdz.so; fails loudly if it has not been built (python -m paper_2604_19718_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python paper_2604_19718_b200/build.py` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, dp = C.c_void_p, C.POINTER(C.c_double)
+    L.cdz_last_error.restype = C.c_char_p
+    L.cdz_model_create.argtypes = [C.POINTER(NNParams), C.POINTER(vp)]
+    L.cdz_model_destroy.argtypes = [vp]
+    L.cdz_model_destroy.restype = None
+    L.cdz_tt_build.argtypes = [C.c_char_p, C.c_int, C.c_int, dp, dp, C.POINTER(vp)]
+    L.cdz_tt_from_operators.argtypes = [C.c_int, C.POINTER(C.c_int32), C.POINTER(Op), C.POINTER(vp)]
+    L.cdz_tt_destroy.argtypes = [vp]
+    L.cdz_tt_destroy.restype = None
+    L.cdz_tt_length.argtypes = [vp]
+    L.cdz_tt_describe.argtypes = [vp, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+    L.cdz_workspace_bytes.argtypes = [vp, C.c_int, C.POINTER(C.c_size_t)]
+    L.cdz_inside.argtypes = [vp, vp, C.c_int, vp, C.c_size_t, vp, C.POINTER(vp), dp]
+    L.cdz_inside_batch.argtypes = [vp, C.POINTER(vp), C.c_int, C.c_int, C.POINTER(vp), C.POINTER(C.c_size_t), vp,
+                                   C.POINTER(vp), dp]
+    L.cdz_inside_rerun.argtypes = [vp, vp]
+    L.cdz_inside_rerun_batch.argtypes = [C.POINTER(vp), C.c_int, vp]
+    L.cdz_tables_logz.argtypes = [vp, dp]
+    L.cdz_tables_info.argtypes = [vp, C.POINTER(Info)]
+    L.cdz_tables_destroy.argtypes = [vp]
+    L.cdz_tables_destroy.restype = None
+    L.cdz_tables_cell.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
+    L.cdz_tables_logqext.argtypes = [vp, C.c_int, C.c_int, dp]
+    L.cdz_sample.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, vp]
+    L.cdz_marginals.argtypes = [vp, vp, vp, vp, vp]
+    L.cdz_run_host.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, dp, vp]
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc < 0:
+        raise CdzError(rc, lib().cdz_last_error().decode())
+    return rc
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double)) if a is not None else None
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return C.c_void_p(getattr(stream, "cuda_stream", stream))
+
+
+class Model:
+    """cdz_model_create / cdz_model_destroy."""
+
+    def __init__(self, m):
+        p = NNParams()
+        p.temperature_K = float(m.temperature_K)
+        p.stack[:] = [float(v) for v in np.asarray(m.stack, dtype=np.float64).reshape(-1)]
+        p.tmm[:] = [float(v) for v in np.asarray(m.tmm, dtype=np.float64).reshape(-1)]
+        p.hairpin_a, p.hairpin_b, p.hairpin_l0 = float(m.hairpin_a), float(m.hairpin_b), float(m.hairpin_l0)
+        p.bulge_init[:] = [float(v) for v in np.asarray(m.bulge_init, dtype=np.float64)]
+        p.interior_init[:] = [float(v) for v in np.asarray(m.interior_init, dtype=np.float64)]
+        p.ml_a, p.ml_b, p.ml_c = float(m.ml_a), float(m.ml_b), float(m.ml_c)
+        p.max_interior, p.min_hairpin, p.allow_all_pairs = int(m.max_interior), int(m.min_hairpin), int(m.allow_all_pairs)
+        self.h = C.c_void_p()
+        _check(lib().cdz_model_create(C.byref(p), C.byref(self.h)))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            lib().cdz_model_destroy(self.h)
+            self.h = None
+
+
+class TensorTrain:
+    """cdz_tt_build / cdz_tt_from_operators / cdz_tt_destroy."""
+
+    def __init__(self, handle):
+        self.h = handle
+        self.n = lib().cdz_tt_length(handle)
+
+    @classmethod
+    def build(cls, aa: str, kind: int, codon_logw=None, pair_logw=None):
+        cw = np.ascontiguousarray(codon_logw, dtype=np.float64) if codon_logw is not None else None
+        pw = np.ascontiguousarray(pair_logw, dtype=np.float64).reshape(-1) if pair_logw is not None else None
+        h = C.c_void_p()
+        _check(lib().cdz_tt_build(aa.encode(), len(aa), kind, _dp(cw), _dp(pw), C.byref(h)))
+        return cls(h)
+
+    @classmethod
+    def from_operators(cls, ops_per_pos):
+        n = len(ops_per_pos)
+        counts = (C.c_int32 * n)(*[len(o) for o in ops_per_pos])
+        flat = [o for pos in ops_per_pos for o in pos]
+        arr = (Op * max(1, len(flat)))()
+        for k, (a, b, c, x) in enumerate(flat):
+            arr[k] = Op(a, b, c, x)
+        h = C.c_void_p()
+        _check(lib().cdz_tt_from_operators(n, counts, arr, C.byref(h)))
+        return cls(h)
+
+    def describe(self):
+        sigma = (C.c_int32 * (self.n + 1))()
+        counts = (C.c_int32 * self.n)()
+        nops = _check(lib().cdz_tt_describe(self.h, sigma, counts))
+        return list(sigma), list(counts), nops
+
+    def workspace_bytes(self, precision=FP64) -> int:
+        b = C.c_size_t()
+        _check(lib().cdz_workspace_bytes(self.h, precision, C.byref(b)))
+        return b.value
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            lib().cdz_tt_destroy(self.h)
+            self.h = None
+
+
+class Tables:
+    """Handle returned by inside(); owns the torch workspace that backs the device tables."""
+
+    def __init__(self, handle, model, tt, workspace):
+        self.h, self.model, self.tt, self.workspace, self.n = handle, model, tt, workspace, tt.n
+
+    def logz(self) -> float:
+        v = C.c_double()
+        _check(lib().cdz_tables_logz(self.h, C.byref(v)))
+        return v.value
+
+    def rerun(self, stream=None):
+        _check(lib().cdz_inside_rerun(self.h, _stream_ptr(stream)))
+
+    def info(self) -> dict:
+        i = Info()
+        _check(lib().cdz_tables_info(self.h, C.byref(i)))
+        return {k: getattr(i, k) for k, _ in Info._fields_}
+
+    def cell(self, which, i, j):
+        out = np.zeros(16 * 64)
+        sh = C.c_int()
+        cnt = _check(lib().cdz_tables_cell(self.h, which, i, j, _dp(out), C.byref(sh)))
+        return out[:cnt].copy(), sh.value
+
+    def logqext(self, j, c) -> float:
+        v = C.c_double()
+        _check(lib().cdz_tables_logqext(self.h, j, c, C.byref(v)))
+        return v.value
+
+    def sample(self, J: int, seed: int, stream=None):
+        """cdz_sample: returns (seq uint8 [J,n], pair int32 [J,n]) as CUDA tensors."""
+        import torch
+
+        seq = torch.empty((J, self.n), dtype=torch.uint8, device="cuda")
+        pair = torch.empty((J, self.n), dtype=torch.int32, device="cuda")
+        _check(lib().cdz_sample(self.h, J, seed, C.c_void_p(seq.data_ptr()), C.c_void_p(pair.data_ptr()),
+                                _stream_ptr(stream)))
+        return seq, pair
+
+    def marginals(self, stream=None):
+        import torch
+
+        n = self.n
+        bpp = torch.zeros((n, n), dtype=torch.float64, device="cuda")
+        base = torch.zeros((n, 4), dtype=torch.float64, device="cuda")
+        codon = torch.zeros((n // 3, 64), dtype=torch.float64, device="cuda")
+        _check(lib().cdz_marginals(self.h, C.c_void_p(bpp.data_ptr()), C.c_void_p(base.data_ptr()),
+                                   C.c_void_p(codon.data_ptr()), _stream_ptr(stream)))
+        return bpp, base, codon
+
+    def run_host(self, J: int, seed: int, seq_host=None, pair_host=None, stream=None) -> float:
+        """cdz_run_host: host buffers in / out (pinned torch tensors or numpy arrays), returns log Z."""
+        v = C.c_double()
+        sp = C.c_void_p(seq_host.data_ptr()) if seq_host is not None else None
+        pp = C.c_void_p(pair_host.data_ptr()) if pair_host is not None else None
+        _check(lib().cdz_run_host(self.h, J, seed, sp, pp, C.byref(v), _stream_ptr(stream)))
+        return v.value
+
+    def destroy(self):
+        if getattr(self, "h", None):
+            lib().cdz_tables_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        self.destroy()
+
+
+def _alloc_workspace(tt, precision):
+    import torch
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("no CUDA device: paper_2604_19718_b200 has no CPU fallback")
+    nbytes = tt.workspace_bytes(precision)
+    return torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+
+
+def inside(model: Model, tt: TensorTrain, precision=FP64, stream=None, sync=True):
+    """cdz_inside: returns (Tables, logZ or None)."""
+    ws = _alloc_workspace(tt, precision)
+    h, lz = C.c_void_p(), C.c_double()
+    _check(lib().cdz_inside(model.h, tt.h, precision, C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(stream),
+                            C.byref(h), C.byref(lz) if sync else None))
+    return Tables(h, model, tt, ws), (lz.value if sync else None)
+
+
+def inside_batch(model: Model, tts, precision=FP64, stream=None):
+    """cdz_inside_batch: returns ([Tables], [logZ])."""
+    B = len(tts)
+    wss = [_alloc_workspace(t, precision) for t in tts]
+    tt_arr = (C.c_void_p * B)(*[t.h for t in tts])
+    ws_arr = (C.c_void_p * B)(*[w.data_ptr() for w in wss])
+    wb_arr = (C.c_size_t * B)(*[w.numel() for w in wss])
+    out = (C.c_void_p * B)()
+    lz = (C.c_double * B)()
+    _check(lib().cdz_inside_batch(model.h, tt_arr, B, precision, ws_arr, wb_arr, _stream_ptr(stream), out, lz))
+    return [Tables(C.c_void_p(out[b]), model, tts[b], wss[b]) for b in range(B)], list(lz)
+
+
+def inside_rerun_batch(tables, stream=None):
+    B = len(tables)
+    arr = (C.c_void_p * B)(*[t.h.value for t in tables])
+    _check(lib().cdz_inside_rerun_batch(arr, B, _stream_ptr(stream)))

@@ -1,0 +1,124 @@
+// cdz_internal.h -- host/device structures shared by the translation units of libcdz (CUDA path only).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/cdz.h"
+
+#define CDZ_MAX_BOND 8     // bond dimension limit of the kernels
+#define CDZ_MAX_STATES 16  // |L_i|, |R_j| limit
+#define CDZ_WARPS 8        // warps (cells) per CTA in the cell kernel
+
+// ---- Boltzmann factors of the loop model (constant memory image) -------------------------------
+struct CModel {
+  double wst[6][6];
+  double wtm[6][4][4];
+  double wbu[32];
+  double win[32];
+  double wa, wb, wc, wac;
+  int max_interior, min_hairpin, allow_all, nps;  // nps = number of pair slots (6 or 16)
+  int8_t pslot[16];                               // (x*4+y) -> pair slot or -1
+  int8_t ptype[16];                               // (x*4+y) -> pair type for energy lookup
+  int8_t slot_x[16], slot_y[16];                  // inverse of pslot
+};
+
+struct cdz_model {
+  cdz_nn_params p;
+  CModel c;
+  double kT;
+};
+
+// ---- tensor train, host side ---------------------------------------------------------------------
+struct cdz_tt {
+  int n = 0, kind = -1;
+  std::vector<int> sigma;    // [n+1]
+  std::vector<int> opstart;  // [n+1]
+  std::vector<cdz_op> ops;
+  // derived
+  int S = 0, LS = 0, RS = 0, MS = 1, maxL = 1, maxR = 1, maxOps = 1;
+  std::vector<int> off;                   // [n+2] bond offsets
+  std::vector<int> loff, roff;            // [n+1]
+  std::vector<uint8_t> ls_a, ls_x;        // [LS]
+  std::vector<uint8_t> rs_y, rs_c;        // [RS]
+  std::vector<uint8_t> op_l, op_r;        // per operator: local left / right state index
+};
+
+// ---- device views --------------------------------------------------------------------------------
+struct DevTT {
+  int n, S, LS, RS, MS, maxL, maxR;
+  const int* sig;      // [n+1]
+  const int* off;      // [n+2]
+  const int* opstart;  // [n+1]
+  const uint8_t *op_a, *op_b, *op_c, *op_l, *op_r;
+  double* op_x;        // scaled operator weights
+  const int* loff;     // [n+1]
+  const int* roff;     // [n+1]
+  const uint8_t *ls_a, *ls_x, *rs_y, *rs_c;
+  const int* bondpos;  // [S+1?] position of each bond index (as left bond of that position), bondpos[off[i]+a] = i
+  const int* lspos;    // [LS]
+  const int* rspos;    // [RS]
+  double* Tbar;        // [n][MS*MS], scaled
+  const double* wh;    // [n+1] hairpin Boltzmann factor by loop length
+};
+
+// All tables are square row-major matrices over the packed index spaces (bonds S, left states LS, right
+// states RS); cell (i,j) occupies the block rows(i) x cols(j).
+template <typename T>
+struct DevTabT {
+  T *QB;    // LS x RS : Qb(i,j)[l][r]
+  T *DD;    // LS x RS : mismatch-dressed extension of Qb(k,l), stored at cell (k-1,l+1)
+  T *D1;    // LS x S  : DD summed over the right nucleotide
+  T *D2;    // S  x RS : DD summed over the left nucleotide
+  T *GI;    // S  x S  : DD summed over both
+  T *QBS;   // S x S
+  T *QM;    // S x S   : row (i,a), column (j+1,c)
+  T *QM1T;  // S x S   : transposed: row (j+1,c), column (i,a)
+  T *QML;   // S x S
+  T *M2;    // S x S
+  T *EM;    // S x S   : E(i,j) = Tbar_i..Tbar_j
+  T *Qext;  // [n+1][MS]
+  int* cellexp;  // [n] exponent of max |Qm| of the cell of the current diagonal at row i
+  int* scale;    // [n+1] prefix sums P of the per-position scale bits s_m (true = stored * 2^{P[j+1]-P[i]})
+  int* ctrl;     // control block: [0]=n_rescales [1]=flags(overflow) ...
+  double* result; // [0]=logZ [1]=log mantissa sum etc.
+};
+typedef DevTabT<double> DevTab;
+
+struct Ctx {
+  DevTT tt;
+  DevTab tab;
+  const CModel* cm;  // Boltzmann tables (device copy inside the workspace)
+};
+
+struct cdz_tables {
+  const cdz_model* model = nullptr;
+  const cdz_tt* tt = nullptr;
+  int precision = CDZ_FP64;
+  cudaStream_t stream = nullptr;
+  void* base = nullptr;  // device allocation (owned if owns_base)
+  bool owns_base = false;
+  size_t bytes = 0;
+  Ctx h;         // host copy of the device view
+  Ctx* d_ctx = nullptr;  // device copy (inside base)
+  int n_rescales = 0;
+  double inside_ms = 0;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  bool done = false;
+};
+
+// ---- internal entry points -----------------------------------------------------------------------
+void cdz_set_error(const std::string& s);
+int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st);
+int cdz_launch_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* pair_dev, cudaStream_t st);
+
+#define CDZ_CUDA(call)                                                                       \
+  do {                                                                                       \
+    cudaError_t e__ = (call);                                                                \
+    if (e__ != cudaSuccess) {                                                                \
+      cdz_set_error(std::string(#call) + ": " + cudaGetErrorString(e__));                    \
+      return CDZ_ECUDA;                                                                      \
+    }                                                                                        \
+  } while (0)

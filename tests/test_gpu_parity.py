@@ -1,0 +1,130 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_2604_19718_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+LOGZ_RTOL = 1e-9  # BASELINE.json north_star: 1e-9 relative in log Z for fp64
+
+
+def rows(name):
+    with open(os.path.join(GOLD, name)) as f:
+        return [ln.split() for ln in f if ln.strip() and not ln.startswith("#")]
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2604_19718_b200 import binding, build
+
+    build.build()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import oracle
+
+    return oracle
+
+
+def both(B, O, model, aa, kind, cw, pw):
+    tto = O.TT.build(aa, kind, cw, pw)
+    ttg = B.TensorTrain.build(aa, kind, cw, pw)
+    to = O.inside(model, tto)
+    tg, lz = B.inside(B.Model(model), ttg)
+    return to, tg, lz
+
+
+@pytest.mark.parametrize("row", rows("appendix_b.txt"), ids=lambda r: "-".join(r[:5]))
+def test_logz_appendix_b(B, O, row):
+    aa, kind, cw, pw, mi = row[0], int(row[1]), int(row[2]), int(row[3]), int(row[4])
+    m = I.tm1_model()
+    m.max_interior = mi
+    to, tg, lz = both(B, O, m, aa, kind, I.tm1_codon_logw() if cw else None, I.tm1_pair_logw() if pw else None)
+    assert abs(lz - to.logZ) <= LOGZ_RTOL * max(abs(to.logZ), 1e-3)
+    assert abs(lz - float(row[5])) <= 1e-9 * max(1.0, abs(float(row[5])))
+
+
+@pytest.mark.parametrize("cfg,L", [(1, 20), (2, 20), (5, 10), (5, 40), (2, 45), (1, 67)])
+def test_logz_and_tables_vs_oracle(B, O, cfg, L):
+    """Every stored cell (Qb, Qbs, Qm1, Qml, M2, Qm) of every (i,j) agrees with the oracle."""
+    m = I.nn_model()
+    d = I.design(cfg, 0, L)
+    to, tg, lz = both(B, O, m, d.aa, d.kind, d.codon_logw, d.pair_logw)
+    assert abs(lz - to.logZ) <= LOGZ_RTOL * abs(to.logZ)
+    n = d.n
+    rng = np.random.default_rng(0)
+    cells = [(i, j) for i in range(n) for j in range(i, n)]
+    if len(cells) > 1500:
+        idx = rng.choice(len(cells), 1500, replace=False)
+        cells = [cells[k] for k in idx] + [(0, n - 1), (1, n - 2), (0, n - 2)]
+    for (i, j) in cells:
+        for which in range(6):
+            g, sh = tg.cell(which, i, j)
+            o = to.cell(which, i, j, sh)
+            scale = max(np.abs(o).max(), 1e-300)
+            assert np.abs(g - o).max() <= 1e-11 * scale, (which, i, j)
+    for j in (0, n // 2, n - 1):
+        for c in range(1):
+            assert abs(tg.logqext(j, c) - to.logqext(j, c)) <= 1e-11 * max(1.0, abs(to.logqext(j, c)))
+
+
+@pytest.mark.parametrize("n", [12, 24, 37, 40, 50])
+def test_zero_energy_closed_form(B, O, n):
+    """Z = #structures for one fixed sequence, all pairs allowed, zero energies (tests/golden/structure_counts.txt)."""
+    tab = {(k, int(a)): int(v) for k, a, v in rows("structure_counts.txt")}
+    m = I.zero_energy_model()
+    tt = B.TensorTrain.from_operators([[(0, 0, 0, 1.0)]] * n)
+    tg, lz = B.inside(B.Model(m), tt)
+    want = tab[("limit30", n)] if n >= 38 else tab[("unlimited", n)]
+    assert abs(math.exp(lz) / want - 1) < 1e-12
+
+
+def test_zero_energy_sequences_times_structures(B, O):
+    m = I.zero_energy_model()
+    for aa, want in (("LSR", 6912), ("RSLG", 236736), ("GAVLI", 2858112)):
+        for kind in (0, 1):
+            tg, lz = B.inside(B.Model(m), B.TensorTrain.build(aa, kind))
+            assert abs(math.exp(lz) / want - 1) < 1e-12
+
+
+def test_generic_operator_lists(B, O):
+    m = I.tm1_model()
+    ops = [[(0, b, 0, 1.0 + 0.1 * b + 0.01 * i) for b in range(4)] for i in range(14)]
+    lo = O.inside(m, O.TT.from_ops(ops)).logZ
+    tg, lz = B.inside(B.Model(m), B.TensorTrain.from_operators(ops))
+    assert abs(lz - lo) <= LOGZ_RTOL * abs(lo)
+
+
+@pytest.mark.parametrize("cfg,L,J", [(1, 20, 1000), (5, 12, 300), (2, 20, 300), (5, 40, 64)])
+def test_samples_bit_exact(B, O, cfg, L, J):
+    """Same seed, same decision uniforms -> identical (sequence, structure) as the oracle traceback."""
+    m = I.nn_model()
+    d = I.design(cfg, 0, L)
+    to, tg, lz = both(B, O, m, d.aa, d.kind, d.codon_logw, d.pair_logw)
+    so, po = to.sample(J, d.sample_seed)
+    sg, pg = tg.sample(J, d.sample_seed)
+    sg, pg = sg.cpu().numpy(), pg.cpu().numpy()
+    bad = [k for k in range(J) if not ((so[k] == sg[k]).all() and (po[k] == pg[k]).all())]
+    assert not bad, f"{len(bad)} of {J} samples differ, first {bad[:3]}"
+    # every sample is a valid state of the ensemble
+    tto = O.TT.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
+    for k in range(0, J, max(1, J // 20)):
+        assert np.isfinite(O.logweight(m, tto, sg[k], pg[k]))
+    # determinism
+    sg2, pg2 = tg.sample(J, d.sample_seed)
+    assert (sg2.cpu().numpy() == sg).all() and (pg2.cpu().numpy() == pg).all()
+
+
+def test_errors(B):
+    m = B.Model(I.nn_model())
+    tt = B.TensorTrain.build("MW", 0)
+    tg, lz = B.inside(m, tt)
+    with pytest.raises(B.CdzError):
+        tg.cell(9, 0, 0)
