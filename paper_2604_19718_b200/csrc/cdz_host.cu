@@ -112,15 +112,31 @@ std::map<int, int> rank_map(const std::vector<int>& vals) {
 
 int finalize_tt(cdz_tt* tt) {
   const int n = tt->n;
-  tt->off.assign(n + 2, 0);
   tt->MS = 1;
+  tt->sigma_bar = 0;
   for (int i = 0; i <= n; ++i) {
-    tt->off[i + 1] = tt->off[i] + tt->sigma[i];
     tt->MS = std::max(tt->MS, tt->sigma[i]);
+    if (i < n) tt->sigma_bar += tt->sigma[i];
   }
-  tt->S = tt->off[n + 1];
   if (tt->MS > CDZ_MAX_BOND) { cdz_set_error("tensor train bond dimension exceeds 8"); return CDZ_EINVAL; }
   if (tt->sigma[0] != 1) { cdz_set_error("Sigma_0 must be 1 (open chain)"); return CDZ_EINVAL; }
+  // position blocks: greedy runs of bond positions 0..n holding at most CDZ_TB bonds; the bond index space is padded so
+  // that block b owns exactly [b*CDZ_TB, (b+1)*CDZ_TB); padding rows / columns stay zero
+  tt->off.assign(n + 2, 0);
+  tt->posblk.assign(n + 1, 0);
+  tt->blk_start.clear();
+  tt->blk_start.push_back(0);
+  int cur = 0, blk = 0;
+  for (int i = 0; i <= n; ++i) {
+    if (cur + tt->sigma[i] > CDZ_TB) { ++blk; cur = 0; tt->blk_start.push_back(i); }
+    tt->off[i] = blk * CDZ_TB + cur;
+    tt->posblk[i] = blk;
+    cur += tt->sigma[i];
+  }
+  tt->NB = blk + 1;
+  tt->blk_start.push_back(n + 1);
+  tt->S = tt->NB * CDZ_TB;
+  tt->off[n + 1] = tt->S;
   // state lists: L_i = distinct (a, b) sorted lexicographically, R_j = distinct (b, c) sorted by (b, c)
   tt->loff.assign(n + 1, 0);
   tt->roff.assign(n + 1, 0);
@@ -296,6 +312,7 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   Ctx& x = c ? *c : tmp;
   DevTT& t = x.tt;
   t.n = (int)n; t.S = (int)S; t.LS = (int)LS; t.RS = (int)RS; t.MS = (int)MS; t.maxL = tt->maxL; t.maxR = tt->maxR;
+  t.NB = tt->NB;
   Ctx* dc = k.take<Ctx>(1);
   if (d_ctx) *d_ctx = dc;
   t.sig = k.take<int>(n + 1);
@@ -304,6 +321,10 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   t.op_a = k.take<uint8_t>(nops); t.op_b = k.take<uint8_t>(nops); t.op_c = k.take<uint8_t>(nops);
   t.op_l = k.take<uint8_t>(nops); t.op_r = k.take<uint8_t>(nops);
   t.op_x = k.take<double>(nops);
+  t.op_x0 = k.take<double>(nops);
+  t.blk_start = k.take<int>(tt->NB + 1);
+  t.posblk = k.take<int>(n + 1);
+  t.Tbar0 = k.take<double>(n * MS * MS);
   t.loff = k.take<int>(n + 1);
   t.roff = k.take<int>(n + 1);
   t.ls_a = k.take<uint8_t>(LS); t.ls_x = k.take<uint8_t>(LS);
@@ -314,11 +335,20 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   t.Tbar = k.take<double>(n * MS * MS);
   t.wh = k.take<double>(n + 1);
   DevTab& b = x.tab;
-  b.cellexp = k.take<int>(n + 1);
   b.scale = k.take<int>(n + 2);
+  b.dP = k.take<int>(n + 2);
+  b.EB = k.take<int>(S);
+  b.EL = k.take<int>(LS);
+  b.ER = k.take<int>(RS);
+  b.R = k.take<double>(S);
+  {
+    size_t tiles = 1;
+    for (int D = 2; D < tt->NB; ++D) tiles = std::max(tiles, (size_t)(tt->NB - D) * cdz_nsplit(tt->NB, D, 1));
+    b.GP = k.take<double>(tiles * CDZ_TB * CDZ_TB);
+  }
   b.ctrl = k.take<int>(64);
   b.result = k.take<double>(16);
-  b.Qext = k.take<double>((n + 1) * MS);
+  b.Qext = k.take<double>(S);
   b.QB = k.take<double>(LS * RS);
   b.DD = k.take<double>(LS * RS);
   b.D1 = k.take<double>(LS * S);
@@ -354,7 +384,9 @@ static int upload(cdz_tables* T) {
   std::vector<uint8_t> oa, ob, oc;
   std::vector<double> ox;
   for (const cdz_op& o : tt->ops) { oa.push_back(o.a); ob.push_back(o.b); oc.push_back(o.c); ox.push_back(o.x); }
+  // padding bond indices map to the first position of the next block (their table entries are zero)
   std::vector<int> bondpos(tt->S + 1, n), lspos(tt->LS), rspos(tt->RS);
+  for (int kb = 0; kb < tt->S; ++kb) bondpos[kb] = std::min(n, tt->blk_start[kb / CDZ_TB + 1]);
   for (int i = 0; i <= n; ++i)
     for (int a = 0; a < tt->sigma[i]; ++a) bondpos[tt->off[i] + a] = i;
   for (int i = 0; i < n; ++i) {
@@ -378,6 +410,9 @@ static int upload(cdz_tables* T) {
   CDZ_CUDA(up(t.op_l, tt->op_l.data(), oa.size()));
   CDZ_CUDA(up(t.op_r, tt->op_r.data(), oa.size()));
   CDZ_CUDA(up(t.op_x, ox.data(), sizeof(double) * ox.size()));
+  CDZ_CUDA(up(t.op_x0, ox.data(), sizeof(double) * ox.size()));
+  CDZ_CUDA(up(t.blk_start, tt->blk_start.data(), sizeof(int) * (tt->NB + 1)));
+  CDZ_CUDA(up(t.posblk, tt->posblk.data(), sizeof(int) * (n + 1)));
   CDZ_CUDA(up(t.loff, tt->loff.data(), sizeof(int) * (n + 1)));
   CDZ_CUDA(up(t.roff, tt->roff.data(), sizeof(int) * (n + 1)));
   CDZ_CUDA(up(t.ls_a, tt->ls_a.data(), tt->LS));
@@ -388,6 +423,7 @@ static int upload(cdz_tables* T) {
   CDZ_CUDA(up(t.lspos, lspos.data(), sizeof(int) * tt->LS));
   CDZ_CUDA(up(t.rspos, rspos.data(), sizeof(int) * tt->RS));
   CDZ_CUDA(up(t.Tbar, tbar.data(), sizeof(double) * tbar.size()));
+  CDZ_CUDA(up(t.Tbar0, tbar.data(), sizeof(double) * tbar.size()));
   CDZ_CUDA(up(t.wh, wh.data(), sizeof(double) * (n + 1)));
   CDZ_CUDA(up(T->h.cm, &m->c, sizeof(CModel)));
   CDZ_CUDA(up(T->d_ctx, &T->h, sizeof(Ctx)));
@@ -421,6 +457,12 @@ static int make_tables(const cdz_model* m, const cdz_tt* tt, int precision, void
     T->owns_base = true;
   }
   carve(tt, T->base, &T->h, &T->d_ctx);
+  // padding rows / columns of the packed tables are never written by the kernels and must read as zero
+  if (cudaMemsetAsync(T->base, 0, need, st) != cudaSuccess) {
+    cdz_set_error("cudaMemsetAsync of the DP tables failed");
+    cdz_tables_destroy(T);
+    return CDZ_ECUDA;
+  }
   cudaEventCreate(&T->ev0);
   cudaEventCreate(&T->ev1);
   int rc = upload(T);
@@ -509,7 +551,7 @@ extern "C" int cdz_tables_info(cdz_tables* t, cdz_info* info) {
   memset(info, 0, sizeof(*info));
   const int n = tt->n;
   info->n = n;
-  info->sigma_bar = tt->off[n];
+  info->sigma_bar = tt->sigma_bar;
   info->n_left_states = tt->LS;
   info->n_right_states = tt->RS;
   info->precision = t->precision;

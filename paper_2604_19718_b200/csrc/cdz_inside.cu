@@ -1,12 +1,24 @@
-// cdz_inside.cu -- wavefront inside kernels (sm_100a).
+// cdz_inside.cu -- blocked wavefront inside pass (sm_100a).
 //
-// One warp computes one DP cell (i,j) of the current anti-diagonal d = j-i.  Every quantity of the cell
-// is a small dense tensor over tensor-train bond indices and boundary nucleotides (eq 3.8,
-// lines 203-211); the recursion is DESIGN.md "Recursion".  All tables are
-// row-major matrices over the packed bond / boundary-state index spaces, so the
-// split-point sum  M2(i,j) = sum_k Qm(i,k-1) Qm1(k,j)  is the paper's flattened product
-// Q_{i,k} Q_{j,k}^T (eq 3.5, Alg S4.2): a dot product of two contiguous rows.
+// Every DP cell (i,j) is a small dense tensor over tensor-train bond indices and boundary nucleotides
+// (eq 3.8); the recursion is DESIGN.md "Recursion".  All tables
+// are row-major matrices over the packed (block-padded) bond / boundary-state index spaces,
+// so the split-point sum  M2(i,j) = sum_k Qm(i,k-1) Qm1(k,j)  is the paper's flattened product
+// Q_{i,k} Q_{j,k}^T (eq 3.5, Alg S4.2).
+//
+// Schedule: positions are grouped into blocks of <= CDZ_TB bonds; block (I,J) holds the cells whose row bond
+// sigma_i lies in block I and whose column bond sigma_{j+1} lies in block J.  Block diagonals D = J-I are swept
+// in order; on each one
+//   1. gemm_kernel   : M2[I,J] += QM[I,K] QM1T[J,K]^T over the finished blocks I < K < J  (fp64 tensor-core
+//                      mma.sync m8n8k4, cp.async pipeline, split-K partial tiles summed in fixed order),
+//   2. block_kernel  : one CTA per block walks the in-block anti-diagonals (one warp per cell): closed cells Qb
+//                      (hairpin, stack, bulge, interior <= 30, multiloop closure), Qm1 / Qml rank updates and the
+//                      two in-block edge ranges of the split sum,
+//   3. at D = 1,2,4,..: plan_kernel + rescale_kernel re-centre the per-position power-of-two scales (a-7).
+// ext_kernel then runs the exterior recursion block column by block column.
 #include <math.h>
+
+#include <algorithm>
 
 #include "cdz_internal.h"
 
@@ -91,7 +103,7 @@ __device__ __forceinline__ Scratch carve_scratch(double* s, int MS, int nps, int
 // one cell (i,j); kb_lo..kb_hi: bond-index range of the split sum handled here (v1: the whole range)
 // ------------------------------------------------------------------------------------------------
 __device__ void compute_cell(const DevTT& t, const DevTab& b, const CModel& m, const Scratch& sc, int lane, int i,
-                             int j) {
+                             int j, int I, int J, int nsplit) {
   const int n = t.n, S = t.S, RS = t.RS, MS = t.MS;
   const int d = j - i;
   const int Si = t.sig[i], Sj1 = t.sig[j + 1];
@@ -307,25 +319,37 @@ __device__ void compute_cell(const DevTT& t, const DevTab& b, const CModel& m, c
   }
   __syncwarp();
 
-  // ---- M2(i,j) = sum_k Qm(i,k-1) Qm1(k,j): contiguous-row dot products; Qm = Qml + M2 --------------------
+  // ---- M2(i,j) = sum_k Qm(i,k-1) Qm1(k,j); Qm = Qml + M2 --------------------------------------------------
+  // blocks I < K < J: partial tiles of gemm_kernel, summed in split order; then the bonds of positions
+  // k > i inside block I and k <= j inside block J as contiguous-row dot products
   {
-    const int kb0 = t.off[i + 1], kb1 = offj1;
-    double mx = 0.0;
+    int ra0, ra1, rb0 = 0, rb1 = 0;
+    if (I == J) {
+      ra0 = t.off[i + 1];
+      ra1 = offj1;
+    } else {
+      ra1 = (I + 1) * CDZ_TB;
+      ra0 = t.posblk[i + 1] == I ? t.off[i + 1] : ra1;
+      rb0 = J * CDZ_TB;
+      rb1 = offj1;
+    }
+    const double* gp = b.GP + (size_t)I * nsplit * (CDZ_TB * CDZ_TB) + (size_t)(offi - I * CDZ_TB) * CDZ_TB +
+                       (offj1 - J * CDZ_TB);
     for (int e = 0; e < Si * Sj1; ++e) {
       const int a = e / Sj1, c = e % Sj1;
       const double* A = b.QM + (size_t)(offi + a) * S;
       const double* Bt = b.QM1T + (size_t)(offj1 + c) * S;
       double acc = 0.0;
-      for (int kb = kb0 + lane; kb < kb1; kb += 32) acc += A[kb] * Bt[kb];
+      for (int kb = ra0 + lane; kb < ra1; kb += 32) acc += A[kb] * Bt[kb];
+      for (int kb = rb0 + lane; kb < rb1; kb += 32) acc += A[kb] * Bt[kb];
       for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+      for (int sp = 0; sp < nsplit; ++sp) acc += gp[(size_t)sp * (CDZ_TB * CDZ_TB) + a * CDZ_TB + c];
       const double qm = sc.V1[e] + acc;
       if (lane == 0) {
         b.M2[(size_t)(offi + a) * S + offj1 + c] = acc;
         b.QM[(size_t)(offi + a) * S + offj1 + c] = qm;
       }
-      mx = fmax(mx, qm);
     }
-    if (lane == 0) b.cellexp[i] = mx > 0.0 ? ilogb(mx) : -100000;
   }
 
   // ---- mismatch-dressed extension of Qb(i,j) to [i-1..j+1] (stored at cell (i-1,j+1)) ----------------------
@@ -387,10 +411,16 @@ __device__ void compute_cell(const DevTT& t, const DevTab& b, const CModel& m, c
   }
 }
 
-__global__ void __launch_bounds__(CDZ_WARPS * 32) cell_kernel(const Ctx* ctxs, int d, int scr) {
+// ------------------------------------------------------------------------------------------------
+// block kernel: one CTA per block (I, I+D); in-block anti-diagonals in order, one warp per cell
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(CDZ_WARPS * 32) block_kernel(const Ctx* ctxs, int D, int nsplit, int scr) {
   extern __shared__ double smem[];
   __shared__ CModel cm;
   const Ctx& cx = ctxs[blockIdx.y];
+  const DevTT& t = cx.tt;
+  const int I = blockIdx.x, J = I + D;
+  if (J >= t.NB) return;
   {
     const int* src = (const int*)cx.cm;
     int* dst = (int*)&cm;
@@ -398,72 +428,314 @@ __global__ void __launch_bounds__(CDZ_WARPS * 32) cell_kernel(const Ctx* ctxs, i
   }
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int i = blockIdx.x * CDZ_WARPS + warp;
-  if (i + d >= cx.tt.n) return;
-  Scratch sc = carve_scratch(smem + (size_t)warp * scr, cx.tt.MS, cm.nps, cx.tt.maxL, cx.tt.maxR);
-  compute_cell(cx.tt, cx.tab, cm, sc, lane, i, i + d);
+  const int n = t.n;
+  // rows i in [i0,i1), columns j in [j0,j1): bond position j+1 lies in block J
+  const int i0 = t.blk_start[I], i1 = min(t.blk_start[I + 1], n);
+  const int j0 = max(t.blk_start[J], 1) - 1, j1 = t.blk_start[J + 1] - 1;
+  const Scratch sc = carve_scratch(smem + (size_t)warp * scr, t.MS, cm.nps, t.maxL, t.maxR);
+  const int dmin = max(0, j0 - (i1 - 1)), dmax = (j1 - 1) - i0;
+  for (int d = dmin; d <= dmax; ++d) {
+    const int ilo = max(i0, j0 - d), ihi = min(i1 - 1, j1 - 1 - d);
+    for (int i = ilo + warp; i <= ihi; i += CDZ_WARPS) compute_cell(t, cx.tab, cm, sc, lane, i, i + d, I, J, nsplit);
+    __syncthreads();
+  }
 }
 
-// Qext(j) = Qext(j-1) Tbar_j + sum_k Qext(k-1) Qbs(k,j); Z = sum_c Qext(n-1)[c]  (eq 3.7; App. A.3)
-__global__ void __launch_bounds__(1024) exterior_kernel(const Ctx* ctxs) {
+// ------------------------------------------------------------------------------------------------
+// split-point GEMM: GP[I][split] = QM[I, K-range] * QM1T[J, K-range]^T, 64x64 tile per CTA, fp64 mma.sync m8n8k4
+// ------------------------------------------------------------------------------------------------
+constexpr int GEMM_BK = 16, GEMM_LD = 20, GEMM_STAGES = 3, GEMM_THREADS = 128;
+constexpr int GEMM_SMEM = GEMM_STAGES * 2 * CDZ_TB * GEMM_LD * (int)sizeof(double);
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem_src));
+}
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(c[0]), "+d"(c[1])
+               : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(GEMM_THREADS) gemm_kernel(const Ctx* ctxs, int D, int nsplit) {
+  extern __shared__ double gsm[];
+  const Ctx& cx = ctxs[blockIdx.y];
+  const int I = blockIdx.x / nsplit, sp = blockIdx.x % nsplit, J = I + D;
+  if (J >= cx.tt.NB) return;
+  const size_t S = (size_t)cx.tt.S;
+  const int nk = D - 1;  // K blocks I+1 .. J-1
+  const int kbeg = (I + 1 + (int)((long long)sp * nk / nsplit)) * CDZ_TB;
+  const int kend = (I + 1 + (int)((long long)(sp + 1) * nk / nsplit)) * CDZ_TB;
+  const double* A = cx.tab.QM + (size_t)I * CDZ_TB * S;
+  const double* Bm = cx.tab.QM1T + (size_t)J * CDZ_TB * S;
+  double* As = gsm;
+  double* Bs = gsm + GEMM_STAGES * CDZ_TB * GEMM_LD;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = (warp >> 1) * 32, wn = (warp & 1) * 32;
+
+  auto load_stage = [&](int st, int kk) {
+    double* as = As + st * CDZ_TB * GEMM_LD;
+    double* bs = Bs + st * CDZ_TB * GEMM_LD;
+#pragma unroll
+    for (int r = 0; r < (CDZ_TB * GEMM_BK / 2) / GEMM_THREADS; ++r) {
+      const int c = tid + r * GEMM_THREADS, row = c >> 3, ch = (c & 7) * 2;
+      cp_async16(as + row * GEMM_LD + ch, A + (size_t)row * S + kk + ch);
+      cp_async16(bs + row * GEMM_LD + ch, Bm + (size_t)row * S + kk + ch);
+    }
+  };
+
+  double acc[4][4][2];
+#pragma unroll
+  for (int mi = 0; mi < 4; ++mi)
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni) acc[mi][ni][0] = acc[mi][ni][1] = 0.0;
+
+  const int nkt = (kend - kbeg) / GEMM_BK;
+#pragma unroll
+  for (int st = 0; st < GEMM_STAGES - 1; ++st) {
+    if (st < nkt) load_stage(st, kbeg + st * GEMM_BK);
+    asm volatile("cp.async.commit_group;\n" ::);
+  }
+  for (int kt = 0; kt < nkt; ++kt) {
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(GEMM_STAGES - 2));
+    __syncthreads();
+    const int nxt = kt + GEMM_STAGES - 1;
+    if (nxt < nkt) load_stage(nxt % GEMM_STAGES, kbeg + nxt * GEMM_BK);
+    asm volatile("cp.async.commit_group;\n" ::);
+    const double* as = As + (kt % GEMM_STAGES) * CDZ_TB * GEMM_LD + (wm + (lane >> 2)) * GEMM_LD + (lane & 3);
+    const double* bs = Bs + (kt % GEMM_STAGES) * CDZ_TB * GEMM_LD + (wn + (lane >> 2)) * GEMM_LD + (lane & 3);
+#pragma unroll
+    for (int k4 = 0; k4 < GEMM_BK / 4; ++k4) {
+      double af[4], bf[4];
+#pragma unroll
+      for (int mi = 0; mi < 4; ++mi) af[mi] = as[mi * 8 * GEMM_LD + k4 * 4];
+#pragma unroll
+      for (int ni = 0; ni < 4; ++ni) bf[ni] = bs[ni * 8 * GEMM_LD + k4 * 4];
+#pragma unroll
+      for (int mi = 0; mi < 4; ++mi)
+#pragma unroll
+        for (int ni = 0; ni < 4; ++ni) dmma884(acc[mi][ni], af[mi], bf[ni]);
+    }
+  }
+  asm volatile("cp.async.wait_group 0;\n" ::);
+  double* C = cx.tab.GP + ((size_t)I * nsplit + sp) * (CDZ_TB * CDZ_TB);
+#pragma unroll
+  for (int mi = 0; mi < 4; ++mi)
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni) {
+      const int r = wm + mi * 8 + (lane >> 2), c = wn + ni * 8 + 2 * (lane & 3);
+      *reinterpret_cast<double2*>(C + r * CDZ_TB + c) = make_double2(acc[mi][ni][0], acc[mi][ni][1]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// per-position power-of-two scaling (replaces the random-vector Renormalize of PAPER.md line 622)
+// ------------------------------------------------------------------------------------------------
+// One CTA per design.  After block diagonal D: the longest cell of every block (I, I+D) gives a local growth
+// rate (bits per position); positions take the mean rate of the windows covering them, the rounded prefix sums
+// dP are added to the scale prefix P and every stored quantity over [i..j] is multiplied by 2^-(dP[j+1]-dP[i]).
+__global__ void __launch_bounds__(1024) plan_kernel(const Ctx* ctxs, int D) {
+  extern __shared__ double rate[];  // [NB] (NaN-free: 0 when the window holds no mass)
+  __shared__ int s_maxe;
   const Ctx& cx = ctxs[blockIdx.x];
   const DevTT& t = cx.tt;
   const DevTab& b = cx.tab;
-  const int n = t.n, S = t.S, MS = t.MS;
-  const int mh1 = cx.cm->min_hairpin + 1;
-  __shared__ double red[32][CDZ_MAX_BOND];
-  // Qext is addressed by bond index: QX[off[k]+s] = Qext(k-1)[s]
-  double* QX = b.Qext;
-  if (threadIdx.x == 0) QX[0] = 1.0;
+  const int n = t.n, NB = t.NB, nw = NB - D;
+  if (nw <= 0) return;
+  const size_t S = (size_t)t.S;
+  if (threadIdx.x == 0) s_maxe = 0;
   __syncthreads();
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  for (int j = 0; j < n; ++j) {
-    const int Sj1 = t.sig[j + 1];
-    const int kend = j - mh1 >= 0 ? t.off[j - mh1 + 1] : 0;  // bonds of positions k <= j - mh1
-    double acc[CDZ_MAX_BOND];
-#pragma unroll
-    for (int c = 0; c < CDZ_MAX_BOND; ++c) acc[c] = 0.0;
-    for (int kb = threadIdx.x; kb < kend; kb += blockDim.x) {
-      const double q = QX[kb];
-      const double* row = b.QBS + (size_t)kb * S + t.off[j + 1];
-#pragma unroll
-      for (int c = 0; c < CDZ_MAX_BOND; ++c)
-        if (c < Sj1) acc[c] += q * row[c];
+  for (int I = threadIdx.x; I < nw; I += blockDim.x) {
+    const int i0 = t.blk_start[I], jj = min(t.blk_start[I + D + 1] - 1, n);
+    double r = 0.0;
+    if (jj > i0) {
+      double mx = 0.0;
+      for (int a = 0; a < t.sig[i0]; ++a)
+        for (int c = 0; c < t.sig[jj]; ++c) mx = fmax(mx, b.QM[(size_t)(t.off[i0] + a) * S + t.off[jj] + c]);
+      if (mx > 0.0 && mx < 1.0e308) {
+        const int e = ilogb(mx);
+        r = (double)e / (double)(jj - i0);
+        atomicMax(&s_maxe, abs(e));
+      } else if (!(mx < 1.0e308)) {
+        atomicMax(&s_maxe, 2000);
+      }
     }
-#pragma unroll
-    for (int c = 0; c < CDZ_MAX_BOND; ++c) {
-      for (int o = 16; o > 0; o >>= 1) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], o);
-      if (lane == 0) red[warp][c] = acc[c];
-    }
-    __syncthreads();
-    if (threadIdx.x < Sj1) {
-      const int c = threadIdx.x;
-      double v = 0.0;
-      for (int w = 0; w < (int)(blockDim.x >> 5); ++w) v += red[w][c];
-      const int Sj = t.sig[j];
-      for (int s = 0; s < Sj; ++s) v += QX[t.off[j] + s] * t.Tbar[((size_t)j * MS + s) * MS + c];
-      QX[t.off[j + 1] + c] = v;
-    }
-    __syncthreads();
+    rate[I] = r;
   }
+  __syncthreads();
+  double* delta = b.R;  // scratch until the exterior phase
+  for (int mpos = threadIdx.x; mpos < n; mpos += blockDim.x) {
+    const int bm = t.posblk[mpos];
+    const int lo = max(0, bm - D), hi = min(bm, nw - 1);
+    double s = 0.0;
+    for (int I = lo; I <= hi; ++I) s += rate[I];
+    delta[mpos] = hi >= lo ? s / (double)(hi - lo + 1) : 0.0;
+  }
+  __syncthreads();
   if (threadIdx.x == 0) {
-    double Z = 0.0;
-    for (int c = 0; c < t.sig[n]; ++c) Z += QX[t.off[n] + c];
-    const double ls = 0.6931471805599453 * (double)b.scale[n];
-    b.result[0] = log(Z) + ls;
-    b.result[1] = Z;
-    b.result[2] = ls;
+    double acc = 0.0;
+    int any = 0;
+    b.dP[0] = 0;
+    for (int mpos = 0; mpos < n; ++mpos) {
+      acc += delta[mpos];
+      const int v = (int)rint(acc);
+      b.dP[mpos + 1] = v;
+      any |= v;
+    }
+    b.dP[n + 1] = b.dP[n];
+    b.ctrl[0] += 1;
+    b.ctrl[2] = max(b.ctrl[2], s_maxe);
+    if (s_maxe > 900) b.ctrl[1] = 1;
+    b.ctrl[3] = any != 0;
+  }
+  __syncthreads();
+  if (b.ctrl[3] == 0) return;
+  for (int k = threadIdx.x; k <= n + 1; k += blockDim.x) b.scale[k] += b.dP[k];
+  for (int k = threadIdx.x; k < t.S; k += blockDim.x) b.EB[k] = b.dP[t.bondpos[k]];
+  for (int k = threadIdx.x; k < t.LS; k += blockDim.x) b.EL[k] = b.dP[t.lspos[k]];
+  for (int k = threadIdx.x; k < t.RS; k += blockDim.x) b.ER[k] = b.dP[t.rspos[k] + 1];
+  const int MS = t.MS;
+  for (int mpos = threadIdx.x; mpos < n; mpos += blockDim.x) {
+    const int e = -(b.dP[mpos + 1] - b.dP[mpos]);
+    if (e == 0) continue;
+    for (int z = t.opstart[mpos]; z < t.opstart[mpos + 1]; ++z) t.op_x[z] = scalbn(t.op_x[z], e);
+    for (int k = 0; k < MS * MS; ++k) t.Tbar[(size_t)mpos * MS * MS + k] = scalbn(t.Tbar[(size_t)mpos * MS * MS + k], e);
+  }
+}
+
+// rows of one table over the block diagonals <= D+2 (by storage location); rowsp/colsp: 0 bond space, 1 state space
+__global__ void __launch_bounds__(256) rescale_kernel(const Ctx* ctxs, int which, int D) {
+  const Ctx& cx = ctxs[blockIdx.y];
+  const DevTT& t = cx.tt;
+  const DevTab& b = cx.tab;
+  if (b.ctrl[3] == 0) return;
+  double* tab;
+  int rowsp = 0, colsp = 0, lower = 0;
+  switch (which) {
+    case 0: tab = b.QB; rowsp = 1; colsp = 1; break;
+    case 1: tab = b.DD; rowsp = 1; colsp = 1; break;
+    case 2: tab = b.D1; rowsp = 1; break;
+    case 3: tab = b.D2; colsp = 1; break;
+    case 4: tab = b.GI; break;
+    case 5: tab = b.QBS; break;
+    case 6: tab = b.QM; break;
+    case 7: tab = b.QML; break;
+    case 8: tab = b.M2; break;
+    case 9: tab = b.EM; break;
+    default: tab = b.QM1T; lower = 1; break;
+  }
+  const int nrows = rowsp ? t.LS : t.S;
+  const size_t ld = colsp ? (size_t)t.RS : (size_t)t.S;
+  const int* Erow = rowsp ? b.EL : b.EB;
+  const int* Ecol = colsp ? b.ER : b.EB;
+  const int n = t.n, NB = t.NB;
+  for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
+    const int rb = rowsp ? t.posblk[t.lspos[row]] : row / CDZ_TB;
+    int c0, c1;
+    if (lower) {
+      c0 = max(0, rb - D - 2) * CDZ_TB;
+      c1 = (rb + 1) * CDZ_TB;
+    } else {
+      const int cb = min(NB, rb + D + 3);
+      if (colsp) {
+        c0 = t.roff[min(n, t.blk_start[rb])];
+        c1 = t.roff[min(n, t.blk_start[cb])];
+      } else {
+        c0 = rb * CDZ_TB;
+        c1 = cb * CDZ_TB;
+      }
+    }
+    const int er = Erow[row];
+    double* p = tab + (size_t)row * ld;
+    for (int c = c0 + threadIdx.x; c < c1; c += blockDim.x) {
+      const int e = lower ? er - Ecol[c] : Ecol[c] - er;
+      if (e != 0) p[c] = scalbn(p[c], -e);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// exterior: Qext(j) = Qext(j-1) Tbar_j + sum_k Qext(k-1) Qbs(k,j); Z = sum_c Qext(n-1)[c]  (eq 3.7; App. A.3)
+// ------------------------------------------------------------------------------------------------
+// QX[off[k]+s] = Qext(k-1)[s].  Launch K finishes the bond positions of block K (every CTA repeats the short
+// serial in-block part from a shared-memory copy of the diagonal tile of QBS) and pushes their contribution
+// sum_{kb in K} QX[kb] QBS[kb, c'] into the accumulator R of every later column c'.
+__global__ void __launch_bounds__(256) ext_kernel(const Ctx* ctxs, int K) {
+  const Ctx& cx = ctxs[blockIdx.y];
+  const DevTT& t = cx.tt;
+  const DevTab& b = cx.tab;
+  if (K >= t.NB) return;
+  __shared__ double Dg[CDZ_TB * (CDZ_TB + 1)];
+  __shared__ double qx[CDZ_TB];
+  const int n = t.n, MS = t.MS;
+  const size_t S = (size_t)t.S;
+  const int base = K * CDZ_TB;
+  for (int e = threadIdx.x; e < CDZ_TB * CDZ_TB; e += blockDim.x) {
+    const int r = e / CDZ_TB, c = e % CDZ_TB;
+    Dg[r * (CDZ_TB + 1) + c] = b.QBS[(size_t)(base + r) * S + base + c];
+  }
+  if (threadIdx.x < CDZ_TB) qx[threadIdx.x] = 0.0;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    const int lane = threadIdx.x;
+    const int p0 = t.blk_start[K], p1 = min(t.blk_start[K + 1], n + 1);
+    for (int jj = p0; jj < p1; ++jj) {
+      const int Sj = t.sig[jj], oj = t.off[jj] - base;
+      for (int c = 0; c < Sj; ++c) {
+        double v = 0.0;
+        if (jj == 0) {
+          v = 1.0;
+        } else {
+          double part = qx[lane] * Dg[lane * (CDZ_TB + 1) + oj + c] + qx[lane + 32] * Dg[(lane + 32) * (CDZ_TB + 1) + oj + c];
+          for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+          v = b.R[base + oj + c] + part;
+          const int Sp = t.sig[jj - 1], op = t.off[jj - 1];
+          for (int s = 0; s < Sp; ++s) {
+            const double q = op >= base ? qx[op - base + s] : b.Qext[op + s];
+            v += q * t.Tbar[((size_t)(jj - 1) * MS + s) * MS + c];
+          }
+        }
+        __syncwarp();
+        if (lane == 0) qx[oj + c] = v;
+        __syncwarp();
+      }
+    }
+  }
+  __syncthreads();
+  if (blockIdx.x == 0) {
+    if (threadIdx.x < CDZ_TB) b.Qext[base + threadIdx.x] = qx[threadIdx.x];
+    if (K == t.NB - 1 && threadIdx.x == 0) {
+      double Z = 0.0;
+      for (int c = 0; c < t.sig[n]; ++c) Z += qx[t.off[n] - base + c];
+      const double ls = 0.6931471805599453 * (double)b.scale[n];
+      b.result[0] = log(Z) + ls;
+      b.result[1] = Z;
+      b.result[2] = ls;
+    }
+  }
+  for (int col = base + CDZ_TB + blockIdx.x * blockDim.x + threadIdx.x; col < t.S; col += gridDim.x * blockDim.x) {
+    double acc = 0.0;
+#pragma unroll 8
+    for (int r = 0; r < CDZ_TB; ++r) acc += qx[r] * b.QBS[(size_t)(base + r) * S + col];
+    b.R[col] += acc;
   }
 }
 
 __global__ void init_kernel(const Ctx* ctxs) {
   const Ctx& cx = ctxs[blockIdx.y];
-  const int n = cx.tt.n;
-  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k <= n + 1; k += gridDim.x * blockDim.x) {
-    cx.tab.scale[k] = 0;
-    if (k <= n) cx.tab.cellexp[k] = -100000;
-    if (k < 64) cx.tab.ctrl[k] = 0;
-  }
+  const DevTT& t = cx.tt;
+  const int n = t.n, MS = t.MS;
+  const int nops = t.opstart[n];
+  const int stride = gridDim.x * blockDim.x, k0 = blockIdx.x * blockDim.x + threadIdx.x;
+  for (int k = k0; k <= n + 1; k += stride) { cx.tab.scale[k] = 0; cx.tab.dP[k] = 0; }
+  for (int k = k0; k < 64; k += stride) cx.tab.ctrl[k] = 0;
+  for (int k = k0; k < nops; k += stride) t.op_x[k] = t.op_x0[k];
+  for (int k = k0; k < n * MS * MS; k += stride) t.Tbar[k] = t.Tbar0[k];
+}
+
+__global__ void zero_kernel(const Ctx* ctxs) {
+  const Ctx& cx = ctxs[blockIdx.y];
+  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < cx.tt.S; k += gridDim.x * blockDim.x) cx.tab.R[k] = 0.0;
 }
 
 }  // namespace
@@ -482,15 +754,16 @@ static void fill_lut() {
 
 int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
   fill_lut();
-  // contexts of a batch must be contiguous on the device: stage them into the first handle's workspace? No:
-  // each handle holds its own Ctx; for B > 1 we build a temporary array.
-  int nmax = 0, MS = 1, maxL = 1, maxR = 1, nps = 6;
+  int NBmax = 1, Smax = 0, nrmax = 0, MS = 1, maxL = 1, maxR = 1, nps = 6;
   for (int b = 0; b < B; ++b) {
-    nmax = ts[b]->tt->n > nmax ? ts[b]->tt->n : nmax;
-    MS = ts[b]->tt->MS > MS ? ts[b]->tt->MS : MS;
-    maxL = ts[b]->tt->maxL > maxL ? ts[b]->tt->maxL : maxL;
-    maxR = ts[b]->tt->maxR > maxR ? ts[b]->tt->maxR : maxR;
-    if (ts[b]->model->c.nps > nps) nps = ts[b]->model->c.nps;
+    const cdz_tt* tt = ts[b]->tt;
+    NBmax = std::max(NBmax, tt->NB);
+    Smax = std::max(Smax, tt->S);
+    nrmax = std::max(nrmax, std::max(tt->S, tt->LS));
+    MS = std::max(MS, tt->MS);
+    maxL = std::max(maxL, tt->maxL);
+    maxR = std::max(maxR, tt->maxR);
+    nps = std::max(nps, ts[b]->model->c.nps);
   }
   const Ctx* d_ctxs = ts[0]->d_ctx;
   Ctx* tmp = nullptr;
@@ -504,14 +777,28 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
   }
   const int scr = scratch_doubles(MS, nps, maxL, maxR);
   const size_t smem = (size_t)scr * CDZ_WARPS * sizeof(double);
-  CDZ_CUDA(cudaFuncSetAttribute(cell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  init_kernel<<<dim3(8, B), 256, 0, st>>>(d_ctxs);
-  for (int d = 0; d < nmax; ++d) {
-    const int cells = nmax - d;
-    dim3 grid((cells + CDZ_WARPS - 1) / CDZ_WARPS, B);
-    cell_kernel<<<grid, CDZ_WARPS * 32, smem, st>>>(d_ctxs, d, scr);
+  CDZ_CUDA(cudaFuncSetAttribute(block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  CDZ_CUDA(cudaFuncSetAttribute(gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
+  init_kernel<<<dim3(32, B), 256, 0, st>>>(d_ctxs);
+  int next_event = 1;
+  for (int D = 0; D < NBmax; ++D) {
+    const int nblk = NBmax - D;
+    const int nsplit = cdz_nsplit(NBmax, D, B);
+    if (nsplit > 0) gemm_kernel<<<dim3(nblk * nsplit, B), GEMM_THREADS, GEMM_SMEM, st>>>(d_ctxs, D, nsplit);
+    block_kernel<<<dim3(nblk, B), CDZ_WARPS * 32, smem, st>>>(d_ctxs, D, nsplit, scr);
+    if (D == next_event && D + 1 < NBmax) {
+      next_event *= 2;
+      plan_kernel<<<B, 1024, NBmax * sizeof(double), st>>>(d_ctxs, D);
+      const int gx = std::min(nrmax, 148 * 8);
+      for (int which = 0; which <= 10; ++which) rescale_kernel<<<dim3(gx, B), 256, 0, st>>>(d_ctxs, which, D);
+    }
   }
-  exterior_kernel<<<B, 1024, 0, st>>>(d_ctxs);
+  zero_kernel<<<dim3(32, B), 256, 0, st>>>(d_ctxs);
+  for (int K = 0; K < NBmax; ++K) {
+    const int rem = Smax - (K + 1) * CDZ_TB;
+    const int gx = std::max(1, std::min(148, (rem + 511) / 512));
+    ext_kernel<<<dim3(gx, B), 256, 0, st>>>(d_ctxs, K);
+  }
   CDZ_CUDA(cudaGetLastError());
   if (tmp) CDZ_CUDA(cudaFreeAsync(tmp, st));
   return CDZ_OK;

@@ -10,7 +10,9 @@
 
 #define CDZ_MAX_BOND 8     // bond dimension limit of the kernels
 #define CDZ_MAX_STATES 16  // |L_i|, |R_j| limit
-#define CDZ_WARPS 8        // warps (cells) per CTA in the cell kernel
+#define CDZ_WARPS 16       // warps per CTA in the block kernel (one cell per warp per in-block diagonal)
+#define CDZ_TB 64          // bond-space tile: every position block holds at most CDZ_TB bonds, padded to exactly CDZ_TB
+#define CDZ_MAX_SPLIT 16   // split-K limit of the split-point GEMM
 
 // ---- Boltzmann factors of the loop model (constant memory image) -------------------------------
 struct CModel {
@@ -39,7 +41,10 @@ struct cdz_tt {
   std::vector<cdz_op> ops;
   // derived
   int S = 0, LS = 0, RS = 0, MS = 1, maxL = 1, maxR = 1, maxOps = 1;
-  std::vector<int> off;                   // [n+2] bond offsets
+  std::vector<int> off;                   // [n+2] padded bond offsets: block b owns [b*CDZ_TB, (b+1)*CDZ_TB)
+  int NB = 0, sigma_bar = 0;              // number of position blocks; sum_{i<n} Sigma_i
+  std::vector<int> blk_start;             // [NB+1] first bond position (0..n) of every block, blk_start[NB] = n+1
+  std::vector<int> posblk;                // [n+1] block of bond position i
   std::vector<int> loff, roff;            // [n+1]
   std::vector<uint8_t> ls_a, ls_x;        // [LS]
   std::vector<uint8_t> rs_y, rs_c;        // [RS]
@@ -48,7 +53,11 @@ struct cdz_tt {
 
 // ---- device views --------------------------------------------------------------------------------
 struct DevTT {
-  int n, S, LS, RS, MS, maxL, maxR;
+  int n, S, LS, RS, MS, maxL, maxR, NB;
+  const int* blk_start;  // [NB+1]
+  const int* posblk;     // [n+1]
+  const double* op_x0;   // unscaled operator weights
+  const double* Tbar0;   // unscaled transfer matrices
   const int* sig;      // [n+1]
   const int* off;      // [n+2]
   const int* opstart;  // [n+1]
@@ -80,10 +89,15 @@ struct DevTabT {
   T *M2;    // S x S
   T *EM;    // S x S   : E(i,j) = Tbar_i..Tbar_j
   T *Qext;  // [n+1][MS]
-  int* cellexp;  // [n] exponent of max |Qm| of the cell of the current diagonal at row i
-  int* scale;    // [n+1] prefix sums P of the per-position scale bits s_m (true = stored * 2^{P[j+1]-P[i]})
-  int* ctrl;     // control block: [0]=n_rescales [1]=flags(overflow) ...
-  double* result; // [0]=logZ [1]=log mantissa sum etc.
+  T *GP;    // split-point GEMM partial sums: [block row I][split][CDZ_TB*CDZ_TB]
+  T *R;     // [S] exterior accumulator
+  int* scale;    // [n+2] prefix sums P of the per-position scale bits s_m (true = stored * 2^{P[j+1]-P[i]})
+  int* dP;       // [n+2] increment of P decided by the last rescale event
+  int* EB;       // [S]  dP at the position of every bond index
+  int* EL;       // [LS] dP at the position of every left state
+  int* ER;       // [RS] dP at (position + 1) of every right state
+  int* ctrl;     // control block: [0]=n_rescales [1]=overflow flag [2]=max |exponent| seen at an event
+  double* result; // [0]=logZ [1]=Z mantissa [2]=log scale
 };
 typedef DevTabT<double> DevTab;
 
@@ -104,10 +118,21 @@ struct cdz_tables {
   Ctx h;         // host copy of the device view
   Ctx* d_ctx = nullptr;  // device copy (inside base)
   int n_rescales = 0;
+  int gp_tiles = 0;  // capacity of GP in tiles
   double inside_ms = 0;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool done = false;
 };
+
+// number of K-splits of the split-point GEMM on block diagonal D (B designs advanced together)
+inline int cdz_nsplit(int NB, int D, int B) {
+  if (D < 2) return 0;
+  const int nblk = (NB - D) * B, ks = D - 1;
+  int s = (444 + nblk - 1) / nblk;
+  if (s > ks) s = ks;
+  if (s > CDZ_MAX_SPLIT) s = CDZ_MAX_SPLIT;
+  return s < 1 ? 1 : s;
+}
 
 // ---- internal entry points -----------------------------------------------------------------------
 void cdz_set_error(const std::string& s);
