@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the codon-design inside pass on B200 (one JSON line on stdout).
+
+A "step" is one pass of the whole hot path over one synthetic design: the inside pass
+(stretch products, closed cells, split-point GEMM, per-position rescaling, exterior, log Z) followed by the
+stochastic traceback of the config's sample count.  The tensor train and the loop Boltzmann tables are built on the
+host before the timed region (8a-1/8a-2 are O(n) host work) and are resident in HBM when it starts.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cdz|reference] [--config C] [--L aa]
+
+Workload at N=1: BASELINE.json configs[3], the 5000-aa (15000-nt) design the metric is quoted on.
+N>1 (torchrun): replicas only -- one design does not shard; every rank runs the same
+design independently, no data-path collective, `value` = N x units / max-over-ranks time ("scaling": "weak").
+--impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "DP-cell-contractions/s per design (N_cc + N_loop terms of the inside pass / step time)"
+UNIT = "cell-contractions/s"
+SAMPLES = {1: 1000, 2: 0, 3: 0, 4: 100, 5: 256}
+WORKLOADS = {
+    1: "configs[0]: 20-aa protein, single-codon TT, fp64, 1000 samples",
+    2: "configs[1]: 300-aa protein, codon-pair TT, fp64",
+    4: "configs[3]: 5000-aa protein (15000 nt), single-codon TT, codon weights, fp64 inside pass + 100 samples",
+    5: "configs[4]: 150-aa protein, codon-pair TT, fp64, 256 samples (one item of the batch)",
+}
+
+
+def counts(n: int, min_hairpin: int = 3, max_interior: int = 30):
+    """N_cc and N_loop of SURVEY.md 8(d) (closed forms, independent of the library)."""
+    mh1 = min_hairpin + 1
+    ncc = nloop = 0
+    per_d = {}
+    for d in range(n):
+        ncc += (n - d) * max(0, d - 2 * mh1)
+        key = min(d, 2 * max_interior + 16)
+        if key not in per_d:
+            per_d[key] = sum(1 for l1 in range(max_interior + 1) for l2 in range(max_interior + 1 - l1)
+                             if d - 2 - l1 - l2 >= mh1)
+        nloop += (n - d) * per_d[key]
+    return float(ncc), float(nloop)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for k, nm in enumerate(names):
+                if len(r) > 2 + k and r[2 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(cfg: int, L_sample: int):
+    """Time the CPU oracle's inside pass, as it stands, on the first L_sample residues of the workload."""
+    from oracle import oracle as O
+    from paper_2604_19718_b200 import inputs as I
+
+    d = I.design(cfg, 0, L_sample)
+    tt = O.TT.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
+    t0 = time.perf_counter()
+    tab = O.inside(I.nn_model(), tt, 0)
+    dt = time.perf_counter() - t0
+    ncc, nloop = counts(d.n)
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    return dict(value=(ncc + nloop) / dt, seconds=dt, cores=cores, n=d.n, logZ=tab.logZ,
+                sample=f"oracle inside pass (orc_inside, OpenMP over the cells of a diagonal) on the first {L_sample} aa "
+                       f"({d.n} nt) of the workload's design: {ncc + nloop:.3e} cell-contractions in {dt:.1f} s")
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = args.config
+    L_sample = args.oracle_L or {1: 20, 2: 60, 4: 100, 5: 60}[cfg]
+    vals = []
+    for _ in range(args.warmup):
+        pass  # the oracle has no warm state; warm-up steps are no-ops
+    last = None
+    for _ in range(max(1, args.steps)):
+        last = oracle_sample(cfg, L_sample)
+        vals.append(last)
+    tot_units = sum(v["value"] * v["seconds"] for v in vals)
+    tot_s = sum(v["seconds"] for v in vals)
+    value = tot_units / tot_s
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / len(vals),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64 (long double oracle)",
+        "data": "synthetic", "config": {"workload": WORKLOADS[cfg], "bounded_sample": last["sample"]},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": last["cores"], "kind": "oracle", "sample": last["sample"]},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out), flush=True)
+
+
+def run_cdz(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2604_19718_b200 import binding as B
+    from paper_2604_19718_b200 import build
+    from paper_2604_19718_b200 import inputs as I
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the library has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    build.build()
+
+    cfg = args.config
+    d = I.design(cfg, 0, args.L)
+    J = SAMPLES[cfg] if args.samples is None else args.samples
+    model = B.Model(I.nn_model())
+    tt = B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
+    tab, logz0 = B.inside(model, tt)  # allocation + first pass (untimed)
+    n = d.n
+    ncc, nloop = counts(n)
+    units = ncc + nloop
+    stream = torch.cuda.current_stream()
+    seq = torch.empty((max(J, 1), n), dtype=torch.uint8, device="cuda")
+    pair = torch.empty((max(J, 1), n), dtype=torch.int32, device="cuda")
+
+    def step():
+        tab.rerun(stream)
+        if J > 0:
+            B._check(B.lib().cdz_sample(tab.h, J, d.sample_seed, B.C.c_void_p(seq.data_ptr()),
+                                        B.C.c_void_p(pair.data_ptr()), B._stream_ptr(stream)))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-timed region -------------------------------------------------------------------------------------
+    for _ in range(max(args.warmup, 3)):
+        step()
+    tab.set_profiling(True)
+    barrier()
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    prof_ms = {}
+    prof_launches = {}
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    prof = tab.profile()  # events of the last timed step
+    prof_ms, prof_launches = prof["ms"], prof["launches"]
+    logz = tab.logz()
+    info = tab.info()
+    clk = clocks.stop() if rank == 0 else None
+    tab.set_profiling(False)
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    value = world * units / (ms_step * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers --------------------------------------------------------------
+    seq_h = torch.empty((max(J, 1), n), dtype=torch.uint8).pin_memory()
+    pair_h = torch.empty((max(J, 1), n), dtype=torch.int32).pin_memory()
+    sigma, cnts, nops = tt.describe()
+    h2d = nops * (5 + 8 * 2) + 4 * (5 * (n + 2)) + 8 * 2 * n * info_ms2(sigma) + 8 * (n + 1)
+    d2h = (J * n * 5 if J > 0 else 0) + 8 * 4 + 4 * 4
+    e2e_steps = max(1, min(args.steps, 3))
+    tab.run_host(J, d.sample_seed, seq_h if J else None, pair_h if J else None, stream)  # warm-up
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        lz_e2e = tab.run_host(J, d.sample_seed, seq_h if J else None, pair_h if J else None, stream)
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = world * units / float(t.item())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel -----------------------------------------------------------------------------
+    peaks = {}
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            peaks = json.load(f)
+    except OSError:
+        pass
+    dmma = B.measure_peak(1)
+    dfma = B.measure_peak(0)
+    bf16 = peaks.get("bf16_tflops")
+    sbar_n = info["sigma_bar"] / n
+    loop_mac = nloop * 2.0 * sbar_n ** 3
+    cls = {k: v for k, v in prof_ms.items() if k in ("gemm", "block", "rescale", "exterior", "sample")}
+    dominant = max(cls, key=cls.get) if cls else "gemm"
+    gemm_ms, gemm_l = prof_ms.get("gemm", 0.0), prof_launches.get("gemm", 0)
+    roof_gemm = None
+    if gemm_ms > 0:
+        ach = 2.0 * info["split_mac"] / (gemm_ms * 1e-3) / 1e12
+        roof_gemm = {"kernel": "gemm_kernel (split-point contraction, fp64 mma.sync m8n8k4)", "bound": "tensor",
+                     "achieved": ach, "peak": dmma, "unit": "TFLOP/s", "frac": ach / dmma, "traffic": None,
+                     "launches": gemm_l, "avg_launch_ms": gemm_ms / max(gemm_l, 1),
+                     "algorithmic_flop_per_step": 2.0 * info["split_mac"],
+                     "peak_source": "in-run register-resident mma.sync.m8n8k4.f64 loop (cdz_measure_peak); "
+                                    "MEASURED_PEAKS.json has no fp64 entry; rule-derived alternative = bf16_tflops x "
+                                    "45/2250 = %s" % (None if bf16 is None else round(bf16 * 45.0 / 2250.0, 2)),
+                     "share_of_step": gemm_ms / ms_step}
+    block_ms, block_l = prof_ms.get("block", 0.0), prof_launches.get("block", 0)
+    roof_block = None
+    if block_ms > 0:
+        ach = 2.0 * loop_mac / (block_ms * 1e-3) / 1e12
+        roof_block = {"kernel": "block_kernel (closed cells: hairpin/stack/bulge/interior<=30/multiloop closure, edge splits)",
+                      "bound": "alu", "achieved": ach, "peak": dfma, "unit": "TFLOP/s", "frac": ach / dfma,
+                      "traffic": None, "launches": block_l, "avg_launch_ms": block_ms / max(block_l, 1),
+                      "algorithmic_flop_per_step": 2.0 * loop_mac,
+                      "peak_source": "in-run register-resident fp64 FMA loop (cdz_measure_peak)",
+                      "share_of_step": block_ms / ms_step}
+    roofline = roof_block if dominant == "block" and roof_block else (roof_gemm or roof_block)
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        o = oracle_sample(cfg, args.oracle_L or {1: 20, 2: 60, 4: 100, 5: 60}[cfg])
+        cpu = {"value": o["value"], "unit": UNIT, "cores": o["cores"], "kind": "oracle", "sample": o["sample"]}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": WORKLOADS.get(cfg, f"config {cfg}") + (f" [L overridden to {args.L}]" if args.L else ""),
+                   "n_nt": n, "sigma_bar": info["sigma_bar"], "samples_per_step": J, "parallelism": "replicas only",
+                   "l2": "tables (%.1f GB) larger than L2; no flush needed" % (info["table_bytes"] / 1e9)
+                   if info["table_bytes"] > 2.5e8 else "tables smaller than L2: warm-cache number",
+                   "seed": d.seed, "nn_model_seed": 19718},
+        "inside_ms": info["inside_ms"], "n_cc": ncc, "n_loop": nloop, "n_cc_per_s": ncc / (info["inside_ms"] * 1e-3),
+        "split_mac": info["split_mac"], "logZ": logz, "table_bytes": info["table_bytes"],
+        "bytes_per_cell": info["bytes_per_cell"], "n_rescales": info["n_rescales"],
+        "kernel_ms": prof_ms, "kernel_launches": prof_launches,
+        "gpu_launches": int(sum(prof_launches.values())) * args.steps,
+        "roofline": roofline, "roofline_gemm": roof_gemm, "roofline_block": roof_block,
+        "peaks": {"fp64_fma_tflops": dfma, "fp64_mma_tflops": dmma, "hbm_gbs": peaks.get("hbm_gbs"),
+                  "bf16_tflops": bf16},
+        "cpu_baseline": cpu,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "ms_per_step": 1e3 * e2e_s, "logZ": lz_e2e},
+        "clocks": clk,
+    }
+    print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def info_ms2(sigma) -> int:
+    ms = max(sigma)
+    return ms * ms
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cdz", choices=["cdz", "reference"])
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 4, 5])
+    ap.add_argument("--L", type=int, default=None, help="override the protein length (development only)")
+    ap.add_argument("--samples", type=int, default=None)
+    ap.add_argument("--oracle-L", type=int, default=None, dest="oracle_L")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cdz(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -88,6 +88,11 @@ typedef struct {
 const char* cdz_last_error(void);
 int cdz_version(void);
 
+/* Register-resident issue-rate microbenchmark on device 0 (blocking): kind 0 = fp64 FMA, 1 = fp64 mma.sync m8n8k4,
+ * 2 = fp32 FMA; TFLOP/s (best of 3 after one warm-up).  Denominators of the fp64 / fp32 rooflines, which
+ * MEASURED_PEAKS.json does not hold. */
+int cdz_measure_peak(int kind, double* tflops_out);
+
 /* ---- model ---------------------------------------------------------------- */
 int cdz_model_create(const cdz_nn_params* params, cdz_model** out);
 void cdz_model_destroy(cdz_model* m);
@@ -128,6 +133,12 @@ int cdz_inside_rerun_batch(cdz_tables* const* t, int B, void* stream);
 int cdz_tables_logz(cdz_tables* t, double* logZ_host);
 int cdz_tables_info(cdz_tables* t, cdz_info* info);
 void cdz_tables_destroy(cdz_tables* t);
+/* Kernel accounting of the last pass on this handle.  cdz_set_profiling(t, 1) makes the next passes record a CUDA
+ * event between consecutive launches on the pass's stream; cdz_profile then synchronises the stream and returns, per
+ * kernel class (0 split-point GEMM, 1 block/cell kernel, 2 rescale, 3 exterior, 4 init, 5 traceback; [8] each),
+ * the summed device milliseconds (0 when profiling was off) and the launch counts (always counted). */
+int cdz_set_profiling(cdz_tables* t, int on);
+int cdz_profile(cdz_tables* t, double* ms_out, int64_t* launches_out);
 /* Debug / parity access: copy one cell to host as doubles (true value * 2^-shift_out).
  * which: 0 Qb as [a][x][y][c] dense, 1 Qbs, 2 Qm1, 3 Qml, 4 M2, 5 Qm (all [a][c]). Returns element count. */
 int cdz_tables_cell(cdz_tables* t, int which, int i, int j, double* out_host, int* shift_out);

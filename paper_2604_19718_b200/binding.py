@@ -22,7 +22,7 @@ EXPORTS = [
     "cdz_tt_from_operators", "cdz_tt_destroy", "cdz_tt_length", "cdz_tt_describe", "cdz_workspace_bytes",
     "cdz_inside", "cdz_inside_batch", "cdz_inside_rerun", "cdz_inside_rerun_batch", "cdz_tables_logz",
     "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample",
-    "cdz_marginals", "cdz_run_host",
+    "cdz_marginals", "cdz_run_host", "cdz_set_profiling", "cdz_profile", "cdz_measure_peak",
 ]
 
 
@@ -88,6 +88,9 @@ def lib():
     L.cdz_tables_info.argtypes = [vp, C.POINTER(Info)]
     L.cdz_tables_destroy.argtypes = [vp]
     L.cdz_tables_destroy.restype = None
+    L.cdz_measure_peak.argtypes = [C.c_int, dp]
+    L.cdz_set_profiling.argtypes = [vp, C.c_int]
+    L.cdz_profile.argtypes = [vp, dp, C.POINTER(C.c_int64)]
     L.cdz_tables_cell.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
     L.cdz_tables_logqext.argtypes = [vp, C.c_int, C.c_int, dp]
     L.cdz_sample.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, vp]
@@ -115,6 +118,13 @@ def _stream_ptr(stream):
     return C.c_void_p(getattr(stream, "cuda_stream", stream))
 
 
+def measure_peak(kind: int) -> float:
+    """cdz_measure_peak: 0 fp64 FMA, 1 fp64 mma.sync, 2 fp32 FMA (TFLOP/s)."""
+    v = C.c_double()
+    _check(lib().cdz_measure_peak(kind, C.byref(v)))
+    return v.value
+
+
 class Model:
     """cdz_model_create / cdz_model_destroy."""
 
@@ -132,8 +142,8 @@ class Model:
         _check(lib().cdz_model_create(C.byref(p), C.byref(self.h)))
 
     def __del__(self):
-        if getattr(self, "h", None):
-            lib().cdz_model_destroy(self.h)
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.cdz_model_destroy(self.h)
             self.h = None
 
 
@@ -176,8 +186,8 @@ class TensorTrain:
         return b.value
 
     def __del__(self):
-        if getattr(self, "h", None):
-            lib().cdz_tt_destroy(self.h)
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.cdz_tt_destroy(self.h)
             self.h = None
 
 
@@ -199,6 +209,17 @@ class Tables:
         i = Info()
         _check(lib().cdz_tables_info(self.h, C.byref(i)))
         return {k: getattr(i, k) for k, _ in Info._fields_}
+
+    def set_profiling(self, on: bool):
+        _check(lib().cdz_set_profiling(self.h, 1 if on else 0))
+
+    def profile(self) -> dict:
+        """cdz_profile: per-kernel-class device ms and launch counts of the last pass."""
+        ms = (C.c_double * 8)()
+        ln = (C.c_int64 * 8)()
+        _check(lib().cdz_profile(self.h, ms, ln))
+        names = ["gemm", "block", "rescale", "exterior", "init", "sample", "c6", "c7"]
+        return {"ms": dict(zip(names, list(ms))), "launches": dict(zip(names, list(ln)))}
 
     def cell(self, which, i, j):
         out = np.zeros(16 * 64)
@@ -241,8 +262,8 @@ class Tables:
         return v.value
 
     def destroy(self):
-        if getattr(self, "h", None):
-            lib().cdz_tables_destroy(self.h)
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.cdz_tables_destroy(self.h)
             self.h = None
             self.workspace = None
 

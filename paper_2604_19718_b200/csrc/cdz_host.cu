@@ -476,6 +476,7 @@ extern "C" void cdz_tables_destroy(cdz_tables* t) {
   if (t->owns_base && t->base) cudaFree(t->base);
   if (t->ev0) cudaEventDestroy(t->ev0);
   if (t->ev1) cudaEventDestroy(t->ev1);
+  for (cudaEvent_t e : t->evs) cudaEventDestroy(e);
   delete t;
 }
 
@@ -589,6 +590,29 @@ extern "C" int cdz_tables_info(cdz_tables* t, cdz_info* info) {
   }
   info->log_scale = sc;
   info->inside_ms = t->inside_ms;
+  return CDZ_OK;
+}
+
+extern "C" int cdz_set_profiling(cdz_tables* t, int on) {
+  if (!t) { cdz_set_error("cdz_set_profiling: null handle"); return CDZ_EINVAL; }
+  t->profile = on != 0;
+  return CDZ_OK;
+}
+
+extern "C" int cdz_profile(cdz_tables* t, double* ms_out, int64_t* launches_out) {
+  if (!t) { cdz_set_error("cdz_profile: null handle"); return CDZ_EINVAL; }
+  if (!t->done) { cdz_set_error("inside pass has not been launched"); return CDZ_ESTATE; }
+  CDZ_CUDA(cudaStreamSynchronize(t->stream));
+  if (ms_out) {
+    for (int k = 0; k < CDZ_NCLASS; ++k) ms_out[k] = 0.0;
+    for (size_t k = 0; k + 1 < t->ev_class.size() && k + 1 < t->evs.size(); ++k) {
+      float ms = 0;
+      if (t->ev_class[k] >= 0 && cudaEventElapsedTime(&ms, t->evs[k], t->evs[k + 1]) == cudaSuccess)
+        ms_out[t->ev_class[k]] += ms;
+    }
+  }
+  if (launches_out)
+    for (int k = 0; k < CDZ_NCLASS; ++k) launches_out[k] = t->launches[k];
   return CDZ_OK;
 }
 

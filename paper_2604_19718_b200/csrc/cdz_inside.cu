@@ -779,26 +779,47 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
   const size_t smem = (size_t)scr * CDZ_WARPS * sizeof(double);
   CDZ_CUDA(cudaFuncSetAttribute(block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   CDZ_CUDA(cudaFuncSetAttribute(gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
+  // accounting: launch counts always; with profiling on, one event before every launch group (class of the group
+  // that follows) so that consecutive event pairs give per-class device time on this stream
+  cdz_tables* T0 = ts[0];
+  for (int k = 0; k < CDZ_NCLASS; ++k) if (k != 5) T0->launches[k] = 0;
+  T0->ev_class.clear();
+  size_t nev = 0;
+  auto mark = [&](int cls, int count) {
+    T0->launches[cls] += count;
+    if (!T0->profile) return;
+    if (nev == T0->evs.size()) { cudaEvent_t e; cudaEventCreate(&e); T0->evs.push_back(e); }
+    cudaEventRecord(T0->evs[nev++], st);
+    T0->ev_class.push_back(cls);
+  };
+  mark(4, 1);
   init_kernel<<<dim3(32, B), 256, 0, st>>>(d_ctxs);
   int next_event = 1;
   for (int D = 0; D < NBmax; ++D) {
     const int nblk = NBmax - D;
     const int nsplit = cdz_nsplit(NBmax, D, B);
-    if (nsplit > 0) gemm_kernel<<<dim3(nblk * nsplit, B), GEMM_THREADS, GEMM_SMEM, st>>>(d_ctxs, D, nsplit);
+    if (nsplit > 0) {
+      mark(0, 1);
+      gemm_kernel<<<dim3(nblk * nsplit, B), GEMM_THREADS, GEMM_SMEM, st>>>(d_ctxs, D, nsplit);
+    }
+    mark(1, 1);
     block_kernel<<<dim3(nblk, B), CDZ_WARPS * 32, smem, st>>>(d_ctxs, D, nsplit, scr);
     if (D == next_event && D + 1 < NBmax) {
       next_event *= 2;
+      mark(2, 12);
       plan_kernel<<<B, 1024, NBmax * sizeof(double), st>>>(d_ctxs, D);
       const int gx = std::min(nrmax, 148 * 8);
       for (int which = 0; which <= 10; ++which) rescale_kernel<<<dim3(gx, B), 256, 0, st>>>(d_ctxs, which, D);
     }
   }
+  mark(3, 1 + NBmax);
   zero_kernel<<<dim3(32, B), 256, 0, st>>>(d_ctxs);
   for (int K = 0; K < NBmax; ++K) {
     const int rem = Smax - (K + 1) * CDZ_TB;
     const int gx = std::max(1, std::min(148, (rem + 511) / 512));
     ext_kernel<<<dim3(gx, B), 256, 0, st>>>(d_ctxs, K);
   }
+  mark(7, 0);  // closing event
   CDZ_CUDA(cudaGetLastError());
   if (tmp) CDZ_CUDA(cudaFreeAsync(tmp, st));
   return CDZ_OK;

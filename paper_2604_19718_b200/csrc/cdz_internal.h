@@ -12,6 +12,7 @@
 #define CDZ_MAX_STATES 16  // |L_i|, |R_j| limit
 #define CDZ_WARPS 16       // warps per CTA in the block kernel (one cell per warp per in-block diagonal)
 #define CDZ_TB 64          // bond-space tile: every position block holds at most CDZ_TB bonds, padded to exactly CDZ_TB
+#define CDZ_NCLASS 8       // kernel classes of cdz_profile: 0 gemm, 1 block, 2 rescale, 3 exterior, 4 init, 5 sample
 #define CDZ_MAX_SPLIT 16   // split-K limit of the split-point GEMM
 
 // ---- Boltzmann factors of the loop model (constant memory image) -------------------------------
@@ -118,7 +119,11 @@ struct cdz_tables {
   Ctx h;         // host copy of the device view
   Ctx* d_ctx = nullptr;  // device copy (inside base)
   int n_rescales = 0;
-  int gp_tiles = 0;  // capacity of GP in tiles
+  // per-kernel-class device times of the last pass (cdz_set_profiling): events between consecutive launches
+  bool profile = false;
+  std::vector<cudaEvent_t> evs;
+  std::vector<int> ev_class;
+  long launches[CDZ_NCLASS] = {0, 0, 0, 0, 0, 0, 0, 0};
   double inside_ms = 0;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool done = false;

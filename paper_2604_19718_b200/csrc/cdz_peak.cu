@@ -1,0 +1,86 @@
+// cdz_peak.cu -- register-resident fp64 / fp32 issue-rate microbenchmarks.
+// MEASURED_PEAKS.json holds HBM and bf16 numbers only; the roofline of the fp64 split-point contraction needs the
+// fp64 vector (DFMA) and tensor (mma.sync m8n8k4 f64, "DMMA") peaks of the same GPU under the same clocks.
+#include <algorithm>
+
+#include "cdz_internal.h"
+
+namespace {
+__global__ void __launch_bounds__(512) peak_dfma(double* out, int iters) {
+  double a[16];
+  const double x = 1.0 + 1e-9 * threadIdx.x, y = 1e-9;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) a[k] = k + threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) a[k] = fma(a[k], x, y);
+  }
+  double s = 0;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) s += a[k];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+__global__ void __launch_bounds__(512) peak_dmma(double* out, int iters) {
+  double c[8][2];
+  const double a = 1.0 + 1e-9 * threadIdx.x, b = 1e-9 * threadIdx.x;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) c[k][0] = c[k][1] = k;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+      asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                   : "+d"(c[k][0]), "+d"(c[k][1])
+                   : "d"(a), "d"(b));
+  }
+  double s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += c[k][0] + c[k][1];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+__global__ void __launch_bounds__(512) peak_ffma(float* out, int iters) {
+  float a[16];
+  const float x = 1.0f + 1e-6f * threadIdx.x, y = 1e-6f;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) a[k] = k + threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) a[k] = fmaf(a[k], x, y);
+  }
+  float s = 0;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) s += a[k];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+}  // namespace
+
+extern "C" int cdz_measure_peak(int kind, double* tflops_out) {
+  if (!tflops_out || kind < 0 || kind > 2) { cdz_set_error("cdz_measure_peak: bad argument"); return CDZ_EINVAL; }
+  cudaDeviceProp prop;
+  CDZ_CUDA(cudaGetDeviceProperties(&prop, 0));
+  const int threads = 512, blocks = prop.multiProcessorCount * 4, iters = 20000;
+  double* out = nullptr;
+  CDZ_CUDA(cudaMalloc((void**)&out, sizeof(double) * threads * blocks));
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  double best = 0;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0);
+    if (kind == 0) peak_dfma<<<blocks, threads>>>(out, iters);
+    else if (kind == 1) peak_dmma<<<blocks, threads>>>(out, iters);
+    else peak_ffma<<<blocks, threads>>>((float*)out, iters);
+    cudaEventRecord(e1);
+    cudaEventSynchronize(e1);
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double flop = kind == 1 ? 2.0 * blocks * (threads / 32) * 8.0 * 256.0 * iters
+                                  : 2.0 * blocks * threads * 16.0 * iters;
+    if (rep > 0) best = std::max(best, flop / ms / 1e9);
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(out);
+  CDZ_CUDA(cudaGetLastError());
+  *tflops_out = best;
+  return CDZ_OK;
+}

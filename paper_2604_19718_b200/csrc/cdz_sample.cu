@@ -478,7 +478,17 @@ int cdz_launch_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int
   Item* stacks = nullptr;
   CDZ_CUDA(cudaMallocAsync((void**)&stacks, sizeof(Item) * (size_t)cap * J, st));
   const int wpb = 4;
+  t->launches[5] = 1;
+  auto mark = [&](int cls) {
+    if (!t->profile) return;
+    const size_t k = t->ev_class.size();
+    if (k >= t->evs.size()) { cudaEvent_t e; cudaEventCreate(&e); t->evs.push_back(e); }
+    cudaEventRecord(t->evs[k], st);
+    t->ev_class.push_back(cls);
+  };
+  mark(5);
   sample_kernel<<<(J + wpb - 1) / wpb, wpb * 32, 0, st>>>(t->d_ctx, J, seed, seq_dev, pair_dev, stacks, cap);
+  mark(7);
   CDZ_CUDA(cudaGetLastError());
   CDZ_CUDA(cudaFreeAsync(stacks, st));
   return CDZ_OK;
