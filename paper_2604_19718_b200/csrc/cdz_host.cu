@@ -360,6 +360,7 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   b.QML = k.take<double>(S * S);
   b.M2 = k.take<double>(S * S);
   b.EM = k.take<double>(S * S);
+  b.ES = k.take<double>(n * 31 * MS * MS);
   x.cm = k.take<CModel>(1);
   return (k.used + 255) & ~size_t(255);
 }

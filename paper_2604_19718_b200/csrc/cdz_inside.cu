@@ -102,8 +102,17 @@ __device__ __forceinline__ Scratch carve_scratch(double* s, int MS, int nps, int
 // ------------------------------------------------------------------------------------------------
 // one cell (i,j); kb_lo..kb_hi: bond-index range of the split sum handled here (v1: the whole range)
 // ------------------------------------------------------------------------------------------------
+// side stretch ES(p,len)[a][c] = (Tbar_p .. Tbar_{p+len-1})[a][c], row stride MS
+__device__ __forceinline__ const double* ESp(const DevTT& t, const DevTab& b, int p, int len) {
+  return b.ES + ((size_t)p * 31 + len) * (t.MS * t.MS);
+}
+
+constexpr int XU = 27;  // interior-loop totals u = l1 + l2 = 4 .. 30 with l1, l2 >= 2
+
+// xs: shared-memory state of column j: X_u(i,j)[a2][c2] at xs[((u-4)*MS + a2)*Sc + c2], the bond-only body
+// sum_{l1+l2=u} E(i+2,k-2) Gi(k,l) E(l+2,j-2) of SURVEY App. A.5 (unweighted); bottom: first row of an off-diagonal block
 __device__ void compute_cell(const DevTT& t, const DevTab& b, const CModel& m, const Scratch& sc, int lane, int i,
-                             int j, int I, int J, int nsplit) {
+                             int j, int I, int J, int nsplit, double* xs, bool bottom) {
   const int n = t.n, S = t.S, RS = t.RS, MS = t.MS;
   const int d = j - i;
   const int Si = t.sig[i], Sj1 = t.sig[j + 1];
@@ -124,6 +133,70 @@ __device__ void compute_cell(const DevTT& t, const DevTab& b, const CModel& m, c
     }
   }
 
+  // ---- X_u(i,j), u = 4..30: direct sum on the first row of an off-diagonal block, else the row recursion
+  //      X_u(i,j) = Tbar_{i+2} X_{u-1}(i+1,j) + Gi(i+3, j+1-u) E(j+3-u, j-2)   (l1 >= 3 terms | l1 = 2 term)
+  if (d >= 4) {
+    const int Sa = t.sig[i + 2], Sc = t.sig[j - 1];
+    const int nX = XU * Sa * Sc;
+    if (bottom) {
+      for (int e = lane; e < nX; e += 32) {
+        const int c2 = e % Sc, a2 = (e / Sc) % Sa, u = 4 + e / (Sc * Sa);
+        double acc = 0.0;
+        for (int l1 = 2; l1 <= u - 2; ++l1) {
+          const int l2 = u - l1, rp = i + l1, cp = j + 1 - l2;  // Gi(k,l) sits at row position k-1, column position l+2
+          if (cp - rp - 3 < mh1) continue;                       // inner span l - k
+          const int Sk = t.sig[rp], Sl = t.sig[cp];
+          const double* EL = ESp(t, b, i + 2, l1 - 2) + a2 * MS;
+          const double* ER = ESp(t, b, cp, l2 - 2) + c2;
+          const double* g = b.GI + (size_t)t.off[rp] * S + t.off[cp];
+          for (int s2 = 0; s2 < Sk; ++s2) {
+            const double el = EL[s2];
+            if (el == 0.0) continue;
+            double r = 0.0;
+            for (int u2 = 0; u2 < Sl; ++u2) r += g[(size_t)s2 * S + u2] * ER[u2 * MS];
+            acc += el * r;
+          }
+        }
+        xs[((u - 4) * MS + a2) * Sc + c2] = acc;
+      }
+      __syncwarp();
+    } else {
+      const int Sa3 = t.sig[i + 3];
+      const double* Tb = t.Tbar + (size_t)(i + 2) * MS * MS;
+      // in place, descending element order: element (u,..) reads old elements of u-1 only
+      for (int hi = nX; hi > 0; hi -= 64) {
+        double val[2];
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+          const int e = hi - 1 - (r * 32 + lane);
+          val[r] = 0.0;
+          if (e < 0) continue;
+          const int c2 = e % Sc, a2 = (e / Sc) % Sa, u = 4 + e / (Sc * Sa);
+          double acc = 0.0;
+          if (u > 4)
+            for (int a3 = 0; a3 < Sa3; ++a3) acc += Tb[a2 * MS + a3] * xs[((u - 5) * MS + a3) * Sc + c2];
+          const int cp = j + 3 - u;
+          if (cp - (i + 2) - 3 >= mh1) {
+            const int Sl = t.sig[cp];
+            const double* g = b.GI + (size_t)(t.off[i + 2] + a2) * S + t.off[cp];
+            const double* ER = ESp(t, b, cp, u - 4) + c2;
+            for (int u2 = 0; u2 < Sl; ++u2) acc += g[u2] * ER[u2 * MS];
+          }
+          val[r] = acc;
+        }
+        __syncwarp();
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+          const int e = hi - 1 - (r * 32 + lane);
+          if (e < 0) continue;
+          const int c2 = e % Sc, a2 = (e / Sc) % Sa, u = 4 + e / (Sc * Sa);
+          xs[((u - 4) * MS + a2) * Sc + c2] = val[r];
+        }
+        __syncwarp();
+      }
+    }
+  }
+
   if (d >= mh1) {
     const int p = i + 1, q = j - 1;
     const int S1 = t.sig[p], S2 = t.sig[j];         // a' in Sigma_{i+1}, c' in Sigma_j
@@ -133,27 +206,12 @@ __device__ void compute_cell(const DevTT& t, const DevTab& b, const CModel& m, c
     const int opp0 = t.opstart[p], opp1 = t.opstart[p + 1], opq0 = t.opstart[q], opq1 = t.opstart[q + 1];
     const int span = q - p;
 
-    // ---- X: interior loops with l1,l2 >= 2 on the mismatch-dressed inner cells ----
+    // ---- XE = sum_u win[u] X_u + hairpin interior (X_u state updated above) -----------------------------------
     {
-      int tmax = min(maxint, span - mh1);
-      int nT = tmax >= 4 ? (tmax - 3) * (tmax - 2) / 2 : 0;
-      warp_terms(lane, Sp1 * Sq, nT, sc.XE, [&](int e, int tt) {
+      warp_terms(lane, Sp1 * Sq, XU, sc.XE, [&](int e, int tt) {
         const int a2 = e / Sq, c2 = e % Sq;
-        const int l1 = c_l1[tt], l2 = c_l2[tt];
-        const int k = p + l1, l = q - l2;
-        const int Sk = t.sig[k - 1], Sl = t.sig[l + 2];
-        const double* g = b.GI + (size_t)t.off[k - 1] * S + t.off[l + 2];
-        double sum = 0.0;
-        for (int s = 0; s < Sk; ++s) {
-          const double el = Eval(t, b, p + 1, k - 2, a2, s);
-          if (el == 0.0) continue;
-          double r = 0.0;
-          for (int u = 0; u < Sl; ++u) r += g[(size_t)s * S + u] * Eval(t, b, l + 2, q - 1, u, c2);
-          sum += el * r;
-        }
-        return m.win[l1 + l2] * sum;
+        return tt + 4 <= maxint ? m.win[tt + 4] * xs[(tt * MS + a2) * Sq + c2] : 0.0;
       });
-      // hairpin interior enters the same way: XE += wh(d-1) E(p+1,q-1)
       const double wh = t.wh[d - 1];
       for (int e = lane; e < Sp1 * Sq; e += 32) sc.XE[e] += wh * Eval(t, b, p + 1, q - 1, e / Sq, e % Sq);
       __syncwarp();
@@ -166,17 +224,17 @@ __device__ void compute_cell(const DevTT& t, const DevTab& b, const CModel& m, c
         const int l1 = tt + 1, k = p + l1;
         if (l1 > maxint || q - k < mh1) return 0.0;
         const int Sk = t.sig[k];
+        const double* EL = ESp(t, b, p, l1) + a1 * MS;
         double sum = 0.0;
-        for (int s = 0; s < Sk; ++s)
-          sum += Eval(t, b, p, k - 1, a1, s) * b.QBS[(size_t)(t.off[k] + s) * S + t.off[q + 1] + c1];
+        for (int s = 0; s < Sk; ++s) sum += EL[s] * b.QBS[(size_t)(t.off[k] + s) * S + t.off[q + 1] + c1];
         return m.wbu[l1] * sum;
       }
       const int l2 = tt - 28, l = q - l2;  // right bulge
       if (l2 > maxint || l - p < mh1) return 0.0;
       const int Sl = t.sig[l + 1];
+      const double* ER = ESp(t, b, l + 1, l2) + c1;
       double sum = 0.0;
-      for (int u = 0; u < Sl; ++u)
-        sum += b.QBS[(size_t)(t.off[p] + a1) * S + t.off[l + 1] + u] * Eval(t, b, l + 1, q, u, c1);
+      for (int u = 0; u < Sl; ++u) sum += b.QBS[(size_t)(t.off[p] + a1) * S + t.off[l + 1] + u] * ER[u * MS];
       return m.wbu[l2] * sum;
     });
     // ---- Z1: l1 = 1, l2 >= 2 ------------------------------------------------------------------------
@@ -186,8 +244,9 @@ __device__ void compute_cell(const DevTT& t, const DevTab& b, const CModel& m, c
       if (1 + l2 > maxint || l - (p + 1) < mh1) return 0.0;
       const int Sl = t.sig[l + 2];
       const double* dd = b.D1 + (size_t)(loffp + lst) * S + t.off[l + 2];
+      const double* ER = ESp(t, b, l + 2, l2 - 2) + c2;
       double sum = 0.0;
-      for (int u = 0; u < Sl; ++u) sum += dd[u] * Eval(t, b, l + 2, q - 1, u, c2);
+      for (int u = 0; u < Sl; ++u) sum += dd[u] * ER[u * MS];
       return m.win[1 + l2] * sum;
     });
     // ---- Z2: l2 = 1, l1 >= 2 ------------------------------------------------------------------------
@@ -196,9 +255,9 @@ __device__ void compute_cell(const DevTT& t, const DevTab& b, const CModel& m, c
       const int l1 = tt + 2, k = p + l1;
       if (l1 + 1 > maxint || (q - 1) - k < mh1) return 0.0;
       const int Sk = t.sig[k - 1];
+      const double* EL = ESp(t, b, p + 1, l1 - 2) + a2 * MS;
       double sum = 0.0;
-      for (int s = 0; s < Sk; ++s)
-        sum += Eval(t, b, p + 1, k - 2, a2, s) * b.D2[(size_t)(t.off[k - 1] + s) * RS + roffq + r];
+      for (int s = 0; s < Sk; ++s) sum += EL[s] * b.D2[(size_t)(t.off[k - 1] + s) * RS + roffq + r];
       return m.win[l1 + 1] * sum;
     });
     // ---- Y[(a',u),(v,c')]: everything that carries the closing mismatch tmm[p(x,y)][u][v] -----------------
@@ -414,9 +473,10 @@ __device__ void compute_cell(const DevTT& t, const DevTab& b, const CModel& m, c
 // ------------------------------------------------------------------------------------------------
 // block kernel: one CTA per block (I, I+D); in-block anti-diagonals in order, one warp per cell
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(CDZ_WARPS * 32) block_kernel(const Ctx* ctxs, int D, int nsplit, int scr) {
+__global__ void __launch_bounds__(CDZ_WARPS * 32) block_kernel(const Ctx* ctxs, int D, int nsplit, int scr, int xsz) {
   extern __shared__ double smem[];
   __shared__ CModel cm;
+  __shared__ int xoff[CDZ_TB + 2];
   const Ctx& cx = ctxs[blockIdx.y];
   const DevTT& t = cx.tt;
   const int I = blockIdx.x, J = I + D;
@@ -426,18 +486,59 @@ __global__ void __launch_bounds__(CDZ_WARPS * 32) block_kernel(const Ctx* ctxs, 
     int* dst = (int*)&cm;
     for (int k = threadIdx.x; k < (int)(sizeof(CModel) / 4); k += blockDim.x) dst[k] = src[k];
   }
-  __syncthreads();
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
   const int n = t.n;
   // rows i in [i0,i1), columns j in [j0,j1): bond position j+1 lies in block J
   const int i0 = t.blk_start[I], i1 = min(t.blk_start[I + 1], n);
   const int j0 = max(t.blk_start[J], 1) - 1, j1 = t.blk_start[J + 1] - 1;
-  const Scratch sc = carve_scratch(smem + (size_t)warp * scr, t.MS, cm.nps, t.maxL, t.maxR);
+  // per-column X_u state (27 * MS * Sigma_{j-1} doubles each), zero = empty body
+  double* xstate = smem;
+  if (threadIdx.x == 0) {
+    int acc = 0;
+    for (int j = j0; j < j1; ++j) {
+      xoff[j - j0] = acc;
+      acc += XU * t.MS * (j >= 1 ? t.sig[j - 1] : 0);
+    }
+  }
+  for (int k = threadIdx.x; k < xsz; k += blockDim.x) xstate[k] = 0.0;
+  __syncthreads();
+  const Scratch sc = carve_scratch(smem + xsz + (size_t)warp * scr, t.MS, cm.nps, t.maxL, t.maxR);
   const int dmin = max(0, j0 - (i1 - 1)), dmax = (j1 - 1) - i0;
   for (int d = dmin; d <= dmax; ++d) {
     const int ilo = max(i0, j0 - d), ihi = min(i1 - 1, j1 - 1 - d);
-    for (int i = ilo + warp; i <= ihi; i += CDZ_WARPS) compute_cell(t, cx.tab, cm, sc, lane, i, i + d, I, J, nsplit);
+    for (int i = ilo + warp; i <= ihi; i += nw)
+      compute_cell(t, cx.tab, cm, sc, lane, i, i + d, I, J, nsplit, xstate + xoff[i + d - j0], I != J && i == i1 - 1);
     __syncthreads();
+  }
+}
+
+// side stretches ES(p,len), len = 0..30, from the (scaled) transfer matrices; one thread per start position
+__global__ void __launch_bounds__(128) side_kernel(const Ctx* ctxs) {
+  const Ctx& cx = ctxs[blockIdx.y];
+  const DevTT& t = cx.tt;
+  const int n = t.n, MS = t.MS, M2 = MS * MS;
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n) return;
+  double* out = cx.tab.ES + (size_t)p * 31 * M2;
+  const int Sp = t.sig[p];
+  for (int e = 0; e < M2; ++e) out[e] = (e / MS == e % MS && e / MS < Sp) ? 1.0 : 0.0;
+  for (int len = 1; len <= 30; ++len) {
+    const double* prev = out + (size_t)(len - 1) * M2;
+    double* cur = out + (size_t)len * M2;
+    const int pos = p + len - 1;
+    if (pos >= n) {
+      for (int e = 0; e < M2; ++e) cur[e] = 0.0;
+      continue;
+    }
+    const double* Tb = t.Tbar + (size_t)pos * M2;
+    const int Sm = t.sig[pos], Sn = t.sig[pos + 1];
+    for (int a = 0; a < MS; ++a)
+      for (int c = 0; c < MS; ++c) {
+        double v = 0.0;
+        if (a < Sp && c < Sn)
+          for (int s2 = 0; s2 < Sm; ++s2) v += prev[a * MS + s2] * Tb[s2 * MS + c];
+        cur[a * MS + c] = v;
+      }
   }
 }
 
@@ -776,7 +877,11 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
     d_ctxs = tmp;
   }
   const int scr = scratch_doubles(MS, nps, maxL, maxR);
-  const size_t smem = (size_t)scr * CDZ_WARPS * sizeof(double);
+  const int xsz = XU * MS * (CDZ_TB + 2 * MS);
+  int nwarps = CDZ_WARPS;
+  while (nwarps > 1 && ((size_t)xsz + (size_t)scr * nwarps) * sizeof(double) > 220 * 1024) --nwarps;
+  const size_t smem = ((size_t)xsz + (size_t)scr * nwarps) * sizeof(double);
+  if (smem > 220 * 1024) { cdz_set_error("block kernel: shared-memory need exceeds 220 KB"); return CDZ_ENOMEM; }
   CDZ_CUDA(cudaFuncSetAttribute(block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   CDZ_CUDA(cudaFuncSetAttribute(gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
   // accounting: launch counts always; with profiling on, one event before every launch group (class of the group
@@ -792,8 +897,11 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
     cudaEventRecord(T0->evs[nev++], st);
     T0->ev_class.push_back(cls);
   };
-  mark(4, 1);
+  mark(4, 2);
   init_kernel<<<dim3(32, B), 256, 0, st>>>(d_ctxs);
+  int nmax = 0;
+  for (int b = 0; b < B; ++b) nmax = std::max(nmax, ts[b]->tt->n);
+  side_kernel<<<dim3((nmax + 127) / 128, B), 128, 0, st>>>(d_ctxs);
   int next_event = 1;
   for (int D = 0; D < NBmax; ++D) {
     const int nblk = NBmax - D;
@@ -803,13 +911,14 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
       gemm_kernel<<<dim3(nblk * nsplit, B), GEMM_THREADS, GEMM_SMEM, st>>>(d_ctxs, D, nsplit);
     }
     mark(1, 1);
-    block_kernel<<<dim3(nblk, B), CDZ_WARPS * 32, smem, st>>>(d_ctxs, D, nsplit, scr);
+    block_kernel<<<dim3(nblk, B), nwarps * 32, smem, st>>>(d_ctxs, D, nsplit, scr, xsz);
     if (D == next_event && D + 1 < NBmax) {
       next_event *= 2;
-      mark(2, 12);
+      mark(2, 13);
       plan_kernel<<<B, 1024, NBmax * sizeof(double), st>>>(d_ctxs, D);
       const int gx = std::min(nrmax, 148 * 8);
       for (int which = 0; which <= 10; ++which) rescale_kernel<<<dim3(gx, B), 256, 0, st>>>(d_ctxs, which, D);
+      side_kernel<<<dim3((nmax + 127) / 128, B), 128, 0, st>>>(d_ctxs);
     }
   }
   mark(3, 1 + NBmax);

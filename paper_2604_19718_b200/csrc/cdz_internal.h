@@ -89,6 +89,7 @@ struct DevTabT {
   T *QML;   // S x S
   T *M2;    // S x S
   T *EM;    // S x S   : E(i,j) = Tbar_i..Tbar_j
+  T *ES;    // [n][31][MS*MS] : side stretches ES(p,len) = Tbar_p..Tbar_{p+len-1}, len <= 30 (zero when p+len > n)
   T *Qext;  // [n+1][MS]
   T *GP;    // split-point GEMM partial sums: [block row I][split][CDZ_TB*CDZ_TB]
   T *R;     // [S] exterior accumulator
