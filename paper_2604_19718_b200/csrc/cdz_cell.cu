@@ -1,0 +1,669 @@
+// cdz_cell.cu -- the per-cell part of the blocked wavefront inside pass (sm_100a): closed cells Qb (hairpin, stack,
+// bulge, interior <= 30, multiloop closure), Qbs / Qm1 / Qml, the in-block edge ranges of the split-point sum, Qm, and
+// the mismatch-dressed extensions that later interior loops read (
+// sequence sums as in chi-hat, eq 3.8).
+//
+// One CTA per block (I, J = I + D).  The in-block anti-diagonals are walked in order; on each one ALL cells are
+// advanced together in a few phases separated by __syncthreads, every phase a flat loop over items
+// (row object of one cell) x (column object), one thread per item:
+//   P1  everything that depends only on finished diagonals, all item types in one flat loop:
+//         M2 edge ranges (4 lanes per entry), band sums Bl / Br (bulges >= 2 + multiloop closure), Z1 / Z2 (l1 = 1 / l2 = 1
+//         interior loops), X_u row recursion + XE (generic interior bodies + hairpin), SB (stack, bulge 1),
+//         the recursive parts of Qm1 / Qml, E(i,j)
+//   P2  Y   = everything that carries the closing mismatch
+//   P3a IN  = inner[slot][a'][c'];   P3b Qb
+//   P4  Qbs, Qm1, Qml, M2, Qm (+ transposed copies)  and  DD = dressed extension of Qb(i,j) over [i-1..j+1]
+//   P5  GI, D1, D2T (DD summed over one or both nucleotides)
+// Every band sum is a dot product of two CONTIGUOUS row segments of row-major tables (transposed copies EMT, QBST,
+// D2T, QM1T exist for that purpose), so the loads of consecutive iterations share sectors and are independent.
+// Position metadata and the dense cores TL_i[(a,x)][c], TR_j[a][(y,c)] of the block's rows / columns live in
+// shared memory; the per-cell intermediates live in a shared-memory scratch slab.
+#include <math.h>
+
+#include <algorithm>
+
+#include "cdz_internal.h"
+
+namespace {
+
+struct PosMeta { int off, sig, loff, nL, roff, nR, ops, nops; };  // 32 bytes, one per position of a window
+
+constexpr int XU = 27;       // interior totals u = l1 + l2 = 4..30 with l1, l2 >= 2
+constexpr int ROWPAD = 34;   // row window  [i0-1, i1+ROWPAD-2]
+constexpr int COLPAD = 34;   // column window [j0-COLPAD+1, j1+1]
+
+struct Dims {
+  int M, ML, MR, nps;  // bond / left-state / right-state / pair-slot dimensions (strides of the scratch arrays)
+  int lgM, lgR, lgP;   // ceil log2 of M, MR, nps (item decoding)
+  __host__ __device__ int percell() const { return 6 * M * M + ML * M + M * MR + 2 * ML * MR + 2 * nps * M * M; }
+};
+
+__host__ __device__ inline int clog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+
+struct Scr {  // scratch of one cell
+  double *XE, *Bl, *Br, *Z1, *Z2, *Y, *SB, *IN, *QBc, *M2s, *R1, *R2;
+};
+__device__ __forceinline__ Scr scr_of(double* base, const Dims& D, int ci) {
+  double* s = base + (size_t)ci * D.percell();
+  Scr k;
+  const int MM = D.M * D.M;
+  k.XE = s; s += MM;
+  k.Bl = s; s += MM;
+  k.Br = s; s += MM;
+  k.M2s = s; s += MM;
+  k.R1 = s; s += MM;
+  k.R2 = s; s += MM;
+  k.Z1 = s; s += D.ML * D.M;
+  k.Z2 = s; s += D.M * D.MR;
+  k.Y = s; s += D.ML * D.MR;
+  k.QBc = s; s += D.ML * D.MR;
+  k.SB = s; s += D.nps * MM;
+  k.IN = s;
+  return k;
+}
+
+// shared-memory plan (bytes), identical on host and device
+struct Plan {
+  int nrow, ncol;        // window lengths (positions)
+  int maxbond, maxls;    // compact row lists (bonds / left states of the row window)
+  int ntl, ntr;          // positions with a dense TL / TR core
+  size_t o_rowm, o_colm, o_crow, o_rbpos, o_rlpos, o_tl, o_tr, o_scr, total;
+};
+__host__ __device__ inline Plan make_plan(int maxpos, const Dims& D, int C) {
+  Plan p;
+  p.nrow = maxpos + ROWPAD;
+  p.ncol = maxpos + COLPAD + 2;
+  p.maxbond = p.nrow * D.M;
+  p.maxls = p.nrow * D.ML;
+  p.ntl = maxpos + 2;
+  p.ntr = maxpos + 3;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 15) & ~size_t(15); return r; };
+  p.o_rowm = take(sizeof(PosMeta) * p.nrow);
+  p.o_colm = take(sizeof(PosMeta) * p.ncol);
+  p.o_crow = take(sizeof(int) * (p.nrow + 1));
+  p.o_rbpos = take(sizeof(short) * p.maxbond);
+  p.o_rlpos = take(sizeof(short) * p.maxls);
+  p.o_tl = take(sizeof(double) * (size_t)p.ntl * D.ML * D.M);
+  p.o_tr = take(sizeof(double) * (size_t)p.ntr * D.M * D.MR);
+  p.o_scr = take(sizeof(double) * (size_t)C * D.percell());
+  p.total = o;
+  return p;
+}
+
+}  // namespace
+
+namespace {
+
+constexpr int CELL_THREADS = 512;
+
+struct KArgs {
+  int D, nsplit, C, maxpos;
+  Dims dm;
+};
+
+__global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, KArgs ka) {
+  extern __shared__ __align__(16) unsigned char smraw[];
+  __shared__ CModel cm;
+  const Ctx& cx = ctxs[blockIdx.y];
+  const DevTT& t = cx.tt;
+  const DevTab& b = cx.tab;
+  const int I = blockIdx.x, J = I + ka.D;
+  if (J >= t.NB) return;
+  const Dims dm = ka.dm;
+  const Plan pl = make_plan(ka.maxpos, dm, ka.C);
+  PosMeta* rowm = (PosMeta*)(smraw + pl.o_rowm);
+  PosMeta* colm = (PosMeta*)(smraw + pl.o_colm);
+  int* crow = (int*)(smraw + pl.o_crow);
+  short* rbpos = (short*)(smraw + pl.o_rbpos);
+  short* rlpos = (short*)(smraw + pl.o_rlpos);
+  double* TLs = (double*)(smraw + pl.o_tl);
+  double* TRs = (double*)(smraw + pl.o_tr);
+  double* scrb = (double*)(smraw + pl.o_scr);
+  const int tid = threadIdx.x, NT = blockDim.x;
+  const int n = t.n, MS = t.MS, MS2 = MS * MS;
+  const size_t S = (size_t)t.S, RS = (size_t)t.RS;
+  const int M = dm.M, ML = dm.ML, MR = dm.MR, nps = dm.nps, MM = M * M;
+  const int lgM = dm.lgM, lgR = dm.lgR, lgP = dm.lgP;
+  const int Mp = 1 << lgM, MRp = 1 << lgR, NPp = 1 << lgP;
+
+  // rows i in [i0,i1), columns j in [j0,j1): bond position j+1 lies in block J
+  const int i0 = t.blk_start[I], i1 = min(t.blk_start[I + 1], n);
+  const int j0 = max(t.blk_start[J], 1) - 1, j1 = t.blk_start[J + 1] - 1;
+  const int rbase = max(i0 - 1, 0), rend = min(i1 + ROWPAD - 2, n);
+  const int cbase = max(j0 - COLPAD + 1, 0), cend = min(j1 + 1, n);
+  const int nrp = rend - rbase + 1, ncp = cend - cbase + 1;
+  const int tlbase = rbase, ntl = min(i1, n - 1) - tlbase + 1;
+  const int trbase = max(j0 - 1, 0), ntr = min(j1, n - 1) - trbase + 1;
+
+  // ---- stage the model, the position metadata and the dense cores ----------------------------------------------
+  {
+    const int* src = (const int*)cx.cm;
+    int* dst = (int*)&cm;
+    for (int k = tid; k < (int)(sizeof(CModel) / 4); k += NT) dst[k] = src[k];
+  }
+  auto load_meta = [&](int p) {
+    PosMeta m;
+    m.off = t.off[p];
+    m.sig = t.sig[p];
+    if (p < n) {
+      m.loff = t.loff[p]; m.nL = t.loff[p + 1] - m.loff;
+      m.roff = t.roff[p]; m.nR = t.roff[p + 1] - m.roff;
+      m.ops = t.opstart[p]; m.nops = t.opstart[p + 1] - m.ops;
+    } else {
+      m.loff = t.loff[n]; m.nL = 0; m.roff = t.roff[n]; m.nR = 0; m.ops = t.opstart[n]; m.nops = 0;
+    }
+    return m;
+  };
+  for (int k = tid; k < nrp; k += NT) rowm[k] = load_meta(rbase + k);
+  for (int k = tid; k < ncp; k += NT) colm[k] = load_meta(cbase + k);
+  for (int k = tid; k < ntl * ML * M; k += NT) TLs[k] = 0.0;
+  for (int k = tid; k < ntr * M * MR; k += NT) TRs[k] = 0.0;
+  __syncthreads();
+  if (tid == 0) {
+    int acc = 0;
+    for (int k = 0; k < nrp; ++k) { crow[k] = acc; acc += rowm[k].sig; }
+    crow[nrp] = acc;
+  }
+  __syncthreads();
+  const int L0 = rowm[0].loff;
+  for (int k = tid; k < nrp; k += NT) {
+    const PosMeta m = rowm[k];
+    for (int a = 0; a < m.sig; ++a) rbpos[crow[k] + a] = (short)k;
+    for (int l = 0; l < m.nL; ++l) rlpos[m.loff - L0 + l] = (short)k;
+  }
+  for (int k = tid; k < ntl; k += NT) {
+    const int p = tlbase + k;
+    if (p < n)
+      for (int z = t.opstart[p]; z < t.opstart[p + 1]; ++z) TLs[(k * ML + t.op_l[z]) * M + t.op_c[z]] += t.op_x[z];
+  }
+  for (int k = tid; k < ntr; k += NT) {
+    const int p = trbase + k;
+    if (p < n)
+      for (int z = t.opstart[p]; z < t.opstart[p + 1]; ++z) TRs[(k * M + t.op_a[z]) * MR + t.op_r[z]] += t.op_x[z];
+  }
+  __syncthreads();
+
+  const int mh1 = cm.min_hairpin + 1, maxint = cm.max_interior;
+  const uint8_t* __restrict__ ls_a = t.ls_a;
+  const uint8_t* __restrict__ ls_x = t.ls_x;
+  const uint8_t* __restrict__ rs_y = t.rs_y;
+  const uint8_t* __restrict__ rs_c = t.rs_c;
+  const double* __restrict__ Tbar = t.Tbar;
+
+  // compact row ranges of the bond rows / left-state rows of positions [lo, hi] of the row window
+  auto bond_rows = [&](int lo, int hi, int& r0) {
+    lo = max(lo, rbase); hi = min(hi, rend);
+    if (hi < lo) { r0 = 0; return 0; }
+    r0 = crow[lo - rbase];
+    return crow[hi + 1 - rbase] - r0;
+  };
+  auto ls_rows = [&](int lo, int hi, int& r0) {
+    lo = max(lo, rbase); hi = min(hi, min(rend, n - 1));
+    if (hi < lo) { r0 = 0; return 0; }
+    r0 = rowm[lo - rbase].loff - L0;
+    return rowm[hi - rbase].loff + rowm[hi - rbase].nL - L0 - r0;
+  };
+
+  const int dmin = max(0, j0 - (i1 - 1)), dmax = (j1 - 1) - i0;
+  for (int d = dmin; d <= dmax; ++d) {
+    const int ilo = max(i0, j0 - d), ihi = min(i1 - 1, j1 - 1 - d);
+    const bool closed = d >= mh1;
+    for (int clo = ilo; clo <= ihi; clo += ka.C) {
+      const int chi = min(ihi, clo + ka.C - 1);
+      // ================= P1: everything that reads finished diagonals only =======================================
+      int rb0, rb1, rb2, rl1;
+      const int nb0 = bond_rows(clo, chi, rb0);          // bonds of position i
+      const int nb1 = bond_rows(clo + 1, chi + 1, rb1);  // bonds of position p = i+1
+      const int nb2 = bond_rows(clo + 2, chi + 2, rb2);  // bonds of position i+2
+      const int nl1 = ls_rows(clo + 1, chi + 1, rl1);    // left states of position p
+      // ---- M2 edge ranges: 4 lanes per entry (a,c) of cell (i,j) ------------------------------------------------
+      {
+        const int cnt = nb0 << (lgM + 2), cntp = (cnt + 31) & ~31;
+        for (int it = tid; it < cntp; it += NT) {
+          double acc = 0.0;
+          bool valid = false;
+          int ci = 0, a = 0, c = 0;
+          const int sub = it & 3;
+          if (it < cnt) {
+            c = (it >> 2) & (Mp - 1);
+            const int rr = rb0 + (it >> (lgM + 2)), kp = rbpos[rr];
+            a = rr - crow[kp];
+            const int i = rbase + kp, j = i + d;
+            ci = i - clo;
+            const PosMeta mj1 = colm[j + 1 - cbase];
+            if (c < mj1.sig) {
+              valid = true;
+              const int offi = rowm[kp].off, offj1 = mj1.off;
+              int ra0, ra1, q0 = 0, q1 = 0;
+              if (I == J) {
+                ra0 = rowm[kp + 1].off;
+                ra1 = offj1;
+              } else {
+                ra1 = (I + 1) * CDZ_TB;
+                ra0 = rowm[kp + 1].off < ra1 ? rowm[kp + 1].off : ra1;
+                q0 = J * CDZ_TB;
+                q1 = offj1;
+              }
+              const double* A = b.QM + (size_t)(offi + a) * S;
+              const double* Bt = b.QM1T + (size_t)(offj1 + c) * S;
+              double acc2 = 0.0;
+              for (int kb = ra0 + sub; kb < ra1; kb += 4) acc += A[kb] * Bt[kb];
+              for (int kb = q0 + sub; kb < q1; kb += 4) acc2 += A[kb] * Bt[kb];
+              acc += acc2;
+              const double* gp = b.GP + (size_t)I * ka.nsplit * (CDZ_TB * CDZ_TB) +
+                                 (size_t)(offi - I * CDZ_TB + a) * CDZ_TB + (offj1 - J * CDZ_TB + c);
+              for (int sp = sub; sp < ka.nsplit; sp += 4) acc += gp[(size_t)sp * (CDZ_TB * CDZ_TB)];
+            }
+          }
+          acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+          acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+          if (valid && sub == 0) scr_of(scrb, dm, ci).M2s[a * M + c] = acc;
+        }
+      }
+      // ---- all other item types in one flat index space -----------------------------------------------------------
+      {
+        const int n3 = closed ? nb1 << lgM : 0;            // Bl
+        const int n4 = n3;                                 // Br
+        const int n5 = closed ? nl1 << lgM : 0;            // Z1
+        const int n6 = closed ? nb2 << lgR : 0;            // Z2
+        const int n2 = d >= 4 ? nb2 << lgM : 0;            // X / XE
+        const int n7 = closed ? nb1 << (lgM + lgP) : 0;    // SB
+        const int n8 = nb0 << lgM;                         // recursive parts of Qm1, Qml
+        const int e3 = n3, e4 = e3 + n4, e5 = e4 + n5, e6 = e5 + n6, e2 = e6 + n2, e7 = e2 + n7, e8 = e7 + n8,
+                  e1 = e8 + n8;
+        for (int g = tid; g < e1; g += NT) {
+          if (g < e4) {
+            // ---- Bl: multiloop closure + left bulges l1 >= 2;  Br: right bulges l2 >= 2 --------------------------
+            const bool left = g < e3;
+            const int it = left ? g : g - e3;
+            const int c1 = it & (Mp - 1), rr = rb1 + (it >> lgM), kp = rbpos[rr], a1 = rr - crow[kp];
+            const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
+            const PosMeta mj = colm[j - cbase];
+            if (c1 >= mj.sig) continue;
+            const int offp = rowm[kp].off;
+            double acc = 0.0;
+            if (left) {
+              acc = cm.wac * b.M2[(size_t)(offp + a1) * S + mj.off + c1];
+              const double* A = b.EM + (size_t)(offp + a1) * S;
+              const double* Bv = b.QBST + (size_t)(mj.off + c1) * S;
+              const int lmax = min(maxint, q - mh1 - p);
+              for (int l1 = 2; l1 <= lmax; ++l1) {
+                const PosMeta mk = rowm[kp + l1];
+                double s = 0.0;
+                for (int u = 0; u < mk.sig; ++u) s += A[mk.off + u] * Bv[mk.off + u];
+                acc += cm.wbu[l1] * s;
+              }
+              scr_of(scrb, dm, i - clo).Bl[a1 * M + c1] = acc;
+            } else {
+              const double* A = b.QBS + (size_t)(offp + a1) * S;
+              const double* Bv = b.EMT + (size_t)(mj.off + c1) * S;
+              const int lmax = min(maxint, q - mh1 - p);
+              for (int l2 = 2; l2 <= lmax; ++l2) {
+                const PosMeta mm = colm[q - l2 + 1 - cbase];
+                double s = 0.0;
+                for (int u = 0; u < mm.sig; ++u) s += A[mm.off + u] * Bv[mm.off + u];
+                acc += cm.wbu[l2] * s;
+              }
+              scr_of(scrb, dm, i - clo).Br[a1 * M + c1] = acc;
+            }
+          } else if (g < e5) {
+            // ---- Z1[lst][c2]: l1 = 1, l2 >= 2 -------------------------------------------------------------------------
+            const int it = g - e4;
+            const int c2 = it & (Mp - 1), ll = rl1 + (it >> lgM), kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
+            const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
+            const PosMeta mq = colm[q - cbase];
+            if (c2 >= mq.sig) continue;
+            const double* A = b.D1 + (size_t)(rowm[kp].loff + lst) * S;
+            const double* Bv = b.EMT + (size_t)(mq.off + c2) * S;
+            const int lmax = min(maxint - 1, q - mh1 - (p + 1));
+            double acc = 0.0;
+            for (int l2 = 2; l2 <= lmax; ++l2) {
+              const PosMeta mm = colm[q - l2 + 2 - cbase];
+              double s = 0.0;
+              for (int u = 0; u < mm.sig; ++u) s += A[mm.off + u] * Bv[mm.off + u];
+              acc += cm.win[1 + l2] * s;
+            }
+            scr_of(scrb, dm, i - clo).Z1[lst * M + c2] = acc;
+          } else if (g < e6) {
+            // ---- Z2[a2][r]: l2 = 1, l1 >= 2 ------------------------------------------------------------------------------
+            const int it = g - e5;
+            const int r = it & (MRp - 1), rr = rb2 + (it >> lgR), kp = rbpos[rr], a2 = rr - crow[kp];
+            const int i = rbase + kp - 2, p = i + 1, j = i + d, q = j - 1;
+            const PosMeta mq = colm[q - cbase];
+            if (r >= mq.nR) continue;
+            const double* A = b.EM + (size_t)(rowm[kp].off + a2) * S;
+            const double* Bv = b.D2T + (size_t)(mq.roff + r) * S;
+            const int lmax = min(maxint - 1, (q - 1) - mh1 - p);
+            double acc = 0.0;
+            for (int l1 = 2; l1 <= lmax; ++l1) {
+              const PosMeta mk = rowm[kp - 1 + l1 - 1];  // position k-1 = p + l1 - 1; kp is position p+1
+              double s = 0.0;
+              for (int u = 0; u < mk.sig; ++u) s += A[mk.off + u] * Bv[mk.off + u];
+              acc += cm.win[l1 + 1] * s;
+            }
+            scr_of(scrb, dm, i - clo).Z2[a2 * MR + r] = acc;
+          } else if (g < e2) {
+            // ---- X_u(i,j) row recursion, XE = sum_u win[u] X_u + hairpin interior ---------------------------------
+            const int it = g - e6;
+            const int c2 = it & (Mp - 1), rr = rb2 + (it >> lgM), kp = rbpos[rr], a2 = rr - crow[kp];
+            const int i = rbase + kp - 2, j = i + d;
+            const PosMeta mq = colm[j - 1 - cbase];
+            if (c2 >= mq.sig) continue;
+            const int offa = rowm[kp].off + a2, Sa3 = rowm[kp + 1].sig;
+            const double* Tb = Tbar + (size_t)(i + 2) * MS2 + a2 * MS;
+            const double* xo = b.XS + ((size_t)((i + 1) & 1) * n + j) * (XU * MS2) + c2;
+            double* xn = b.XS + ((size_t)(i & 1) * n + j) * (XU * MS2) + a2 * MS + c2;
+            const double* gi = b.GI + (size_t)offa * S;
+            const double* em = b.EMT + (size_t)(mq.off + c2) * S;
+            const bool hasold = d - 1 >= 4;
+            double xe = 0.0;
+            for (int u = 4; u <= 30; ++u) {
+              double acc = 0.0;
+              if (hasold && u > 4)
+                for (int a3 = 0; a3 < Sa3; ++a3) acc += Tb[a3] * xo[(u - 5) * MS2 + a3 * MS];
+              const int cp = j + 3 - u;
+              if (cp - (i + 2) - 3 >= mh1) {
+                const PosMeta mc = colm[cp - cbase];
+                for (int u2 = 0; u2 < mc.sig; ++u2) acc += gi[mc.off + u2] * em[mc.off + u2];
+              }
+              xn[(u - 4) * MS2] = acc;
+              if (u <= maxint) xe += cm.win[u] * acc;
+            }
+            if (closed) xe += t.wh[d - 1] * b.EM[(size_t)offa * S + mq.off + c2];
+            scr_of(scrb, dm, i - clo).XE[a2 * M + c2] = xe;
+          } else if (g < e7) {
+            // ---- SB[a'][slot'][c']: inner pair identity kept (stack, bulges of size 1) ------------------------------
+            const int it = g - e2;
+            const int c1 = it & (Mp - 1), sl = (it >> lgM) & (NPp - 1), rr = rb1 + (it >> (lgM + lgP));
+            const int kp = rbpos[rr], a1 = rr - crow[kp];
+            const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
+            const PosMeta mj = colm[j - cbase];
+            if (c1 >= mj.sig || sl >= nps) continue;
+            const PosMeta mp = rowm[kp], mq = colm[q - cbase];
+            const int xp = cm.slot_x[sl], yp = cm.slot_y[sl];
+            int lst = -1, r = -1;
+            for (int l = 0; l < mp.nL; ++l)
+              if (ls_a[mp.loff + l] == a1 && ls_x[mp.loff + l] == xp) lst = l;
+            for (int k = 0; k < mq.nR; ++k)
+              if (rs_y[mq.roff + k] == yp && rs_c[mq.roff + k] == c1) r = k;
+            double v = 0.0;
+            if (q - p >= mh1 && lst >= 0 && r >= 0) v = b.QB[(size_t)(mp.loff + lst) * RS + mq.roff + r];
+            if (maxint >= 1 && q - (p + 1) >= mh1) {
+              double s1 = 0.0, s2 = 0.0;
+              if (r >= 0) {
+                const PosMeta mp1 = rowm[kp + 1];
+                for (int l2 = 0; l2 < mp1.nL; ++l2)
+                  if (ls_x[mp1.loff + l2] == xp)
+                    s1 += Tbar[(size_t)p * MS2 + a1 * MS + ls_a[mp1.loff + l2]] *
+                          b.QB[(size_t)(mp1.loff + l2) * RS + mq.roff + r];
+              }
+              if (lst >= 0) {
+                const PosMeta mq1 = colm[q - 1 - cbase];
+                for (int r2 = 0; r2 < mq1.nR; ++r2)
+                  if (rs_y[mq1.roff + r2] == yp)
+                    s2 += b.QB[(size_t)(mp.loff + lst) * RS + mq1.roff + r2] *
+                          Tbar[(size_t)q * MS2 + rs_c[mq1.roff + r2] * MS + c1];
+              }
+              v += cm.wbu[1] * (s1 + s2);
+            }
+            scr_of(scrb, dm, i - clo).SB[(a1 * nps + sl) * M + c1] = v;
+          } else {
+            // ---- recursive parts of Qm1 / Qml (g < e8) and E(i,j) (g >= e8) -----------------------------------------
+            const bool rec = g < e8;
+            const int it = rec ? g - e7 : g - e8;
+            const int c = it & (Mp - 1), rr = rb0 + (it >> lgM), kp = rbpos[rr], a = rr - crow[kp];
+            const int i = rbase + kp, j = i + d;
+            const PosMeta mj1 = colm[j + 1 - cbase];
+            if (c >= mj1.sig) continue;
+            const PosMeta mj = colm[j - cbase];
+            const int offi = rowm[kp].off;
+            const double* Tj = Tbar + (size_t)j * MS2 + c;
+            if (rec) {
+              double r1 = 0.0, r2 = 0.0;
+              if (d >= 1) {
+                for (int s = 0; s < mj.sig; ++s) r1 += b.QM1T[(size_t)(mj.off + s) * S + offi + a] * Tj[s * MS];
+                const PosMeta mi1 = rowm[kp + 1];
+                const double* Ti = Tbar + (size_t)i * MS2 + a * MS;
+                for (int s = 0; s < mi1.sig; ++s) r2 += Ti[s] * b.QML[(size_t)(mi1.off + s) * S + mj1.off + c];
+              }
+              Scr sc = scr_of(scrb, dm, i - clo);
+              sc.R1[a * M + c] = cm.wb * r1;
+              sc.R2[a * M + c] = cm.wb * r2;
+            } else {
+              double v = 0.0;
+              for (int s = 0; s < mj.sig; ++s) v += b.EM[(size_t)(offi + a) * S + mj.off + s] * Tj[s * MS];
+              b.EM[(size_t)(offi + a) * S + mj1.off + c] = v;
+              b.EMT[(size_t)(mj1.off + c) * S + offi + a] = v;
+            }
+          }
+        }
+      }
+      __syncthreads();
+      if (closed) {
+        // ================= P2: Y[(a',u)][(v,c')] -- everything that carries the closing mismatch =================
+        const bool v11 = maxint >= 2 && d - 4 >= mh1;  // 1x1 interior loop: inner pair (p+1, q-1)
+        for (int it = tid; it < (nl1 << lgR); it += NT) {
+          const int r = it & (MRp - 1), ll = rl1 + (it >> lgR), kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
+          const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
+          const PosMeta mq = colm[q - cbase];
+          if (r >= mq.nR) continue;
+          const Scr sc = scr_of(scrb, dm, i - clo);
+          const int Sp1 = rowm[kp + 1].sig, Sq = mq.sig;
+          const double* TLp = TLs + ((p - tlbase) * ML + lst) * M;
+          const double* TRq = TRs + (size_t)(q - trbase) * M * MR + r;
+          double y = v11 ? cm.win[2] * b.DD[(size_t)(rowm[kp].loff + lst) * RS + mq.roff + r] : 0.0;
+          for (int cz = 0; cz < Sp1; ++cz) {
+            const double tl = TLp[cz];
+            if (tl == 0.0) continue;
+            double s = sc.Z2[cz * MR + r];
+            for (int aw = 0; aw < Sq; ++aw) s += sc.XE[cz * M + aw] * TRq[aw * MR];
+            y += tl * s;
+          }
+          for (int aw = 0; aw < Sq; ++aw) y += sc.Z1[lst * M + aw] * TRq[aw * MR];
+          sc.Y[lst * MR + r] = y;
+        }
+        __syncthreads();
+        // ================= P3a: inner[slot][a'][c'] ======================================================================
+        for (int it = tid; it < (nb1 << (lgM + lgP)); it += NT) {
+          const int c1 = it & (Mp - 1), sl = (it >> lgM) & (NPp - 1), rr = rb1 + (it >> (lgM + lgP));
+          const int kp = rbpos[rr], a1 = rr - crow[kp];
+          const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
+          const PosMeta mj = colm[j - cbase];
+          if (c1 >= mj.sig || sl >= nps) continue;
+          const PosMeta mp = rowm[kp], mq = colm[q - cbase];
+          const Scr sc = scr_of(scrb, dm, i - clo);
+          const int P = cm.ptype[cm.slot_x[sl] * 4 + cm.slot_y[sl]];
+          double v = sc.Bl[a1 * M + c1] + sc.Br[a1 * M + c1];
+          for (int l = 0; l < mp.nL; ++l) {
+            if (ls_a[mp.loff + l] != a1) continue;
+            const int u = ls_x[mp.loff + l];
+            for (int k = 0; k < mq.nR; ++k)
+              if (rs_c[mq.roff + k] == c1) v += cm.wtm[P][u][rs_y[mq.roff + k]] * sc.Y[l * MR + k];
+          }
+          for (int s2 = 0; s2 < nps; ++s2)
+            v += cm.wst[P][cm.ptype[cm.slot_x[s2] * 4 + cm.slot_y[s2]]] * sc.SB[(a1 * nps + s2) * M + c1];
+          sc.IN[(sl * M + a1) * M + c1] = v;
+        }
+        __syncthreads();
+      }
+      // ================= P3b: Qb[(a,x)][(y,c)] = can(x,y) sum T_i[a,x,a'] T_j[c',y,c] inner ============================
+      {
+        int rl0;
+        const int nl0 = ls_rows(clo, chi, rl0);
+        for (int it = tid; it < (nl0 << lgR); it += NT) {
+          const int r = it & (MRp - 1), ll = rl0 + (it >> lgR), kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
+          const int i = rbase + kp, j = i + d;
+          const PosMeta mj = colm[j - cbase];
+          if (r >= mj.nR) continue;
+          const Scr sc = scr_of(scrb, dm, i - clo);
+          double v = 0.0;
+          if (closed) {
+            const int sl = cm.pslot[ls_x[rowm[kp].loff + lst] * 4 + rs_y[mj.roff + r]];
+            if (sl >= 0) {
+              const int S1 = rowm[kp + 1].sig, S2 = mj.sig;
+              const double* TLi = TLs + ((i - tlbase) * ML + lst) * M;
+              const double* TRj = TRs + (size_t)(j - trbase) * M * MR + r;
+              const double* IN = sc.IN + sl * MM;
+              for (int a1 = 0; a1 < S1; ++a1) {
+                const double tl = TLi[a1];
+                if (tl == 0.0) continue;
+                double s = 0.0;
+                for (int c1 = 0; c1 < S2; ++c1) s += TRj[c1 * MR] * IN[a1 * M + c1];
+                v += tl * s;
+              }
+            }
+          }
+          sc.QBc[lst * MR + r] = v;
+          b.QB[(size_t)(rowm[kp].loff + lst) * RS + mj.roff + r] = v;
+        }
+      }
+      __syncthreads();
+      // ================= P4: Qbs, Qm1, Qml, M2, Qm;  DD = mismatch-dressed extension of Qb(i,j) over [i-1..j+1] ==========
+      const bool dress = closed && maxint >= 2;
+      int rlm = 0, nlm = 0, rbm = 0, nbm = 0;
+      if (dress) {
+        // cells with i >= 1 and j <= n-2, i.e. i <= n-2-d
+        const int hi = min(chi, n - 2 - d);
+        nlm = ls_rows(max(clo, 1) - 1, hi - 1, rlm);
+        nbm = bond_rows(max(clo, 1) - 1, hi - 1, rbm);
+      }
+      {
+        const int n4 = nb0 << lgM, n5 = nlm << lgR;
+        for (int g = tid; g < n4 + n5; g += NT) {
+          if (g < n4) {
+            const int c = g & (Mp - 1), rr = rb0 + (g >> lgM), kp = rbpos[rr], a = rr - crow[kp];
+            const int i = rbase + kp, j = i + d;
+            const PosMeta mj1 = colm[j + 1 - cbase];
+            if (c >= mj1.sig) continue;
+            const PosMeta mi = rowm[kp], mj = colm[j - cbase];
+            const Scr sc = scr_of(scrb, dm, i - clo);
+            double qbs = 0.0;
+            for (int l = 0; l < mi.nL; ++l)
+              if (ls_a[mi.loff + l] == a)
+                for (int k = 0; k < mj.nR; ++k)
+                  if (rs_c[mj.roff + k] == c) qbs += sc.QBc[l * MR + k];
+            const double qm1 = cm.wc * qbs + sc.R1[a * M + c];
+            const double qml = qm1 + sc.R2[a * M + c];
+            const double m2 = sc.M2s[a * M + c];
+            const size_t rc = (size_t)(mi.off + a) * S + mj1.off + c, cr = (size_t)(mj1.off + c) * S + mi.off + a;
+            b.QBS[rc] = qbs;
+            b.QBST[cr] = qbs;
+            b.QM1T[cr] = qm1;
+            b.QML[rc] = qml;
+            b.M2[rc] = m2;
+            b.QM[rc] = qml + m2;
+          } else {
+            const int it = g - n4;
+            const int r = it & (MRp - 1), ll = rlm + (it >> lgR), kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
+            const int pi = rbase + kp, i = pi + 1, j = i + d, pj = j + 1;
+            const PosMeta mpj = colm[pj - cbase];
+            if (r >= mpj.nR) continue;
+            const PosMeta mi = rowm[kp + 1], mj = colm[j - cbase];
+            const Scr sc = scr_of(scrb, dm, i - clo);
+            const int up = ls_x[rowm[kp].loff + lst], vp = rs_y[mpj.roff + r];
+            const double* TLm = TLs + ((pi - tlbase) * ML + lst) * M;
+            const double* TRp = TRs + (size_t)(pj - trbase) * M * MR + r;
+            double v = 0.0;
+            for (int l2 = 0; l2 < mi.nL; ++l2) {
+              const double tl = TLm[ls_a[mi.loff + l2]];
+              if (tl == 0.0) continue;
+              const int x = ls_x[mi.loff + l2];
+              double s = 0.0;
+              for (int r2 = 0; r2 < mj.nR; ++r2) {
+                const int y = rs_y[mj.roff + r2];
+                if (cm.pslot[x * 4 + y] < 0) continue;
+                s += TRp[rs_c[mj.roff + r2] * MR] * cm.wtm[cm.ptype[y * 4 + x]][vp][up] * sc.QBc[l2 * MR + r2];
+              }
+              v += tl * s;
+            }
+            sc.Y[lst * MR + r] = v;
+            b.DD[(size_t)(rowm[kp].loff + lst) * RS + mpj.roff + r] = v;
+          }
+        }
+      }
+      __syncthreads();
+      // ================= P5: GI, D1, D2T = DD summed over both / the right / the left nucleotide =========================
+      if (dress) {
+        const int n1 = nbm << lgM, n2 = nlm << lgM, n3 = nbm << lgR;
+        for (int g = tid; g < n1 + n2 + n3; g += NT) {
+          if (g < n1 || g >= n1 + n2) {
+            const bool gi = g < n1;
+            const int it = gi ? g : g - n1 - n2, lg = gi ? lgM : lgR;
+            const int c = it & ((1 << lg) - 1), rr = rbm + (it >> lg), kp = rbpos[rr], a = rr - crow[kp];
+            const int pi = rbase + kp, i = pi + 1, j = i + d, pj = j + 1;
+            const PosMeta mpi = rowm[kp], mpj = colm[pj - cbase];
+            const Scr sc = scr_of(scrb, dm, i - clo);
+            if (gi) {
+              const PosMeta mpj1 = colm[pj + 1 - cbase];
+              if (c >= mpj1.sig) continue;
+              double v = 0.0;
+              for (int l = 0; l < mpi.nL; ++l)
+                if (ls_a[mpi.loff + l] == a)
+                  for (int k = 0; k < mpj.nR; ++k)
+                    if (rs_c[mpj.roff + k] == c) v += sc.Y[l * MR + k];
+              b.GI[(size_t)(mpi.off + a) * S + mpj1.off + c] = v;
+            } else {
+              if (c >= mpj.nR) continue;
+              double v = 0.0;
+              for (int l = 0; l < mpi.nL; ++l)
+                if (ls_a[mpi.loff + l] == a) v += sc.Y[l * MR + c];
+              b.D2T[(size_t)(mpj.roff + c) * S + mpi.off + a] = v;
+            }
+          } else {
+            const int it = g - n1;
+            const int c = it & (Mp - 1), ll = rlm + (it >> lgM), kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
+            const int pi = rbase + kp, i = pi + 1, j = i + d, pj = j + 1;
+            const PosMeta mpj = colm[pj - cbase], mpj1 = colm[pj + 1 - cbase];
+            if (c >= mpj1.sig) continue;
+            const Scr sc = scr_of(scrb, dm, i - clo);
+            double v = 0.0;
+            for (int k = 0; k < mpj.nR; ++k)
+              if (rs_c[mpj.roff + k] == c) v += sc.Y[lst * MR + k];
+            b.D1[(size_t)(rowm[kp].loff + lst) * S + mpj1.off + c] = v;
+          }
+        }
+      }
+      // the next phase that writes this scratch (P1 of the next chunk / diagonal) is separated from these reads by the
+      // barrier after P1 only for Y; P1 itself writes other arrays, so no barrier is needed here
+    }
+  }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+int cdz_cell_config(cdz_tables* const* ts, int B, cdz_cell_cfg* cfg) {
+  Dims dm{1, 1, 1, 6, 0, 0, 0};
+  int maxpos = 1;
+  for (int k = 0; k < B; ++k) {
+    const cdz_tt* tt = ts[k]->tt;
+    dm.M = std::max(dm.M, tt->MS);
+    dm.ML = std::max(dm.ML, tt->maxL);
+    dm.MR = std::max(dm.MR, tt->maxR);
+    dm.nps = std::max(dm.nps, ts[k]->model->c.nps);
+    for (int bk = 0; bk < tt->NB; ++bk) maxpos = std::max(maxpos, std::min(tt->blk_start[bk + 1], tt->n + 1) - tt->blk_start[bk]);
+  }
+  dm.lgM = clog2(dm.M);
+  dm.lgR = clog2(dm.MR);
+  dm.lgP = clog2(dm.nps);
+  const size_t budget = 200 * 1024;
+  int C = maxpos;
+  while (C > 1 && make_plan(maxpos, dm, C).total > budget) --C;
+  const Plan pl = make_plan(maxpos, dm, C);
+  if (pl.total > budget) { cdz_set_error("cell kernel: shared-memory need exceeds 200 KB"); return CDZ_ENOMEM; }
+  cfg->M = dm.M; cfg->ML = dm.ML; cfg->MR = dm.MR; cfg->nps = dm.nps;
+  cfg->maxpos = maxpos; cfg->C = C; cfg->smem = pl.total;
+  CDZ_CUDA(cudaFuncSetAttribute(cell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.total));
+  return CDZ_OK;
+}
+
+void cdz_launch_cells(const Ctx* d_ctxs, int B, int nblk, int D, int nsplit, const cdz_cell_cfg* cfg, cudaStream_t st) {
+  KArgs ka;
+  ka.D = D; ka.nsplit = nsplit; ka.C = cfg->C; ka.maxpos = cfg->maxpos;
+  ka.dm.M = cfg->M; ka.dm.ML = cfg->ML; ka.dm.MR = cfg->MR; ka.dm.nps = cfg->nps;
+  ka.dm.lgM = clog2(cfg->M); ka.dm.lgR = clog2(cfg->MR); ka.dm.lgP = clog2(cfg->nps);
+  cell_kernel<<<dim3(nblk, B), CELL_THREADS, cfg->smem, st>>>(d_ctxs, ka);
+}

@@ -352,7 +352,7 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   b.QB = k.take<double>(LS * RS);
   b.DD = k.take<double>(LS * RS);
   b.D1 = k.take<double>(LS * S);
-  b.D2 = k.take<double>(S * RS);
+  b.D2T = k.take<double>(RS * S);
   b.GI = k.take<double>(S * S);
   b.QBS = k.take<double>(S * S);
   b.QM = k.take<double>(S * S);
@@ -360,7 +360,9 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   b.QML = k.take<double>(S * S);
   b.M2 = k.take<double>(S * S);
   b.EM = k.take<double>(S * S);
-  b.ES = k.take<double>(n * 31 * MS * MS);
+  b.EMT = k.take<double>(S * S);
+  b.QBST = k.take<double>(S * S);
+  b.XS = k.take<double>(2 * n * 27 * MS * MS);
   x.cm = k.take<CModel>(1);
   return (k.used + 255) & ~size_t(255);
 }

@@ -10,7 +10,6 @@
 
 #define CDZ_MAX_BOND 8     // bond dimension limit of the kernels
 #define CDZ_MAX_STATES 16  // |L_i|, |R_j| limit
-#define CDZ_WARPS 16       // warps per CTA in the block kernel (one cell per warp per in-block diagonal)
 #define CDZ_TB 64          // bond-space tile: every position block holds at most CDZ_TB bonds, padded to exactly CDZ_TB
 #define CDZ_NCLASS 8       // kernel classes of cdz_profile: 0 gemm, 1 block, 2 rescale, 3 exterior, 4 init, 5 sample
 #define CDZ_MAX_SPLIT 16   // split-K limit of the split-point GEMM
@@ -81,15 +80,17 @@ struct DevTabT {
   T *QB;    // LS x RS : Qb(i,j)[l][r]
   T *DD;    // LS x RS : mismatch-dressed extension of Qb(k,l), stored at cell (k-1,l+1)
   T *D1;    // LS x S  : DD summed over the right nucleotide
-  T *D2;    // S  x RS : DD summed over the left nucleotide
+  T *D2T;   // RS x S  : DD summed over the left nucleotide, transposed: row (l+1; v',t), column (k-1, s)
   T *GI;    // S  x S  : DD summed over both
   T *QBS;   // S x S
   T *QM;    // S x S   : row (i,a), column (j+1,c)
   T *QM1T;  // S x S   : transposed: row (j+1,c), column (i,a)
   T *QML;   // S x S
   T *M2;    // S x S
-  T *EM;    // S x S   : E(i,j) = Tbar_i..Tbar_j
-  T *ES;    // [n][31][MS*MS] : side stretches ES(p,len) = Tbar_p..Tbar_{p+len-1}, len <= 30 (zero when p+len > n)
+  T *EM;    // S x S   : E(i,j) = Tbar_i..Tbar_j; the diagonal holds E(i,i-1) = identity
+  T *EMT;   // S x S   : EM transposed (row (j+1,c), column (i,a))
+  T *QBST;  // S x S   : QBS transposed
+  T *XS;    // [2][n][27][MS*MS] : interior-loop bodies X_u(i,j), u = 4..30, of the last two rows of every column j
   T *Qext;  // [n+1][MS]
   T *GP;    // split-point GEMM partial sums: [block row I][split][CDZ_TB*CDZ_TB]
   T *R;     // [S] exterior accumulator
@@ -142,6 +143,9 @@ inline int cdz_nsplit(int NB, int D, int B) {
 
 // ---- internal entry points -----------------------------------------------------------------------
 void cdz_set_error(const std::string& s);
+struct cdz_cell_cfg { int M, ML, MR, nps, maxpos, C; size_t smem; };
+int cdz_cell_config(cdz_tables* const* ts, int B, cdz_cell_cfg* cfg);
+void cdz_launch_cells(const Ctx* d_ctxs, int B, int nblk, int D, int nsplit, const cdz_cell_cfg* cfg, cudaStream_t st);
 int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st);
 int cdz_launch_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* pair_dev, cudaStream_t st);
 
