@@ -67,9 +67,10 @@ struct Plan {
   int nrow, ncol;        // window lengths (positions)
   int maxbond, maxls;    // compact row lists (bonds / left states of the row window)
   int ntl, ntr;          // positions with a dense TL / TR core
-  size_t o_rowm, o_colm, o_crow, o_rbpos, o_rlpos, o_tl, o_tr, o_scr, total;
+  size_t o_rowm, o_colm, o_crow, o_rbpos, o_rlpos, o_rbp, o_cbp, o_tl, o_tr, o_scr, total;
 };
-__host__ __device__ inline Plan make_plan(int maxpos, const Dims& D, int C) {
+// span: largest extent, in global (block-padded) bond indices, of a row / column window
+__host__ __device__ inline Plan make_plan(int maxpos, int span, const Dims& D, int C) {
   Plan p;
   p.nrow = maxpos + ROWPAD;
   p.ncol = maxpos + COLPAD + 2;
@@ -84,6 +85,8 @@ __host__ __device__ inline Plan make_plan(int maxpos, const Dims& D, int C) {
   p.o_crow = take(sizeof(int) * (p.nrow + 1));
   p.o_rbpos = take(sizeof(short) * p.maxbond);
   p.o_rlpos = take(sizeof(short) * p.maxls);
+  p.o_rbp = take(span);
+  p.o_cbp = take(span);
   p.o_tl = take(sizeof(double) * (size_t)p.ntl * D.ML * D.M);
   p.o_tr = take(sizeof(double) * (size_t)p.ntr * D.M * D.MR);
   p.o_scr = take(sizeof(double) * (size_t)C * D.percell());
@@ -98,7 +101,7 @@ namespace {
 constexpr int CELL_THREADS = 512;
 
 struct KArgs {
-  int D, nsplit, C, maxpos;
+  int D, nsplit, C, maxpos, span;
   Dims dm;
 };
 
@@ -111,12 +114,14 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   const int I = blockIdx.x, J = I + ka.D;
   if (J >= t.NB) return;
   const Dims dm = ka.dm;
-  const Plan pl = make_plan(ka.maxpos, dm, ka.C);
+  const Plan pl = make_plan(ka.maxpos, ka.span, dm, ka.C);
   PosMeta* rowm = (PosMeta*)(smraw + pl.o_rowm);
   PosMeta* colm = (PosMeta*)(smraw + pl.o_colm);
   int* crow = (int*)(smraw + pl.o_crow);
   short* rbpos = (short*)(smraw + pl.o_rbpos);
   short* rlpos = (short*)(smraw + pl.o_rlpos);
+  uint8_t* rbp = smraw + pl.o_rbp;  // bond index -> position (relative to the window base), row / column window
+  uint8_t* cbp = smraw + pl.o_cbp;
   double* TLs = (double*)(smraw + pl.o_tl);
   double* TRs = (double*)(smraw + pl.o_tr);
   double* scrb = (double*)(smraw + pl.o_scr);
@@ -157,6 +162,10 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   };
   for (int k = tid; k < nrp; k += NT) rowm[k] = load_meta(rbase + k);
   for (int k = tid; k < ncp; k += NT) colm[k] = load_meta(cbase + k);
+  const int rkb0 = t.off[rbase], rkb1 = t.off[rend] + t.sig[rend];
+  const int ckb0 = t.off[cbase], ckb1 = t.off[cend] + t.sig[cend];
+  for (int k = tid; k < rkb1 - rkb0; k += NT) rbp[k] = (uint8_t)min(t.bondpos[rkb0 + k] - rbase, 255);
+  for (int k = tid; k < ckb1 - ckb0; k += NT) cbp[k] = (uint8_t)min(t.bondpos[ckb0 + k] - cbase, 255);
   for (int k = tid; k < ntl * ML * M; k += NT) TLs[k] = 0.0;
   for (int k = tid; k < ntr * M * MR; k += NT) TRs[k] = 0.0;
   __syncthreads();
@@ -217,169 +226,170 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
       const int nb1 = bond_rows(clo + 1, chi + 1, rb1);  // bonds of position p = i+1
       const int nb2 = bond_rows(clo + 2, chi + 2, rb2);  // bonds of position i+2
       const int nl1 = ls_rows(clo + 1, chi + 1, rl1);    // left states of position p
-      // ---- M2 edge ranges: 4 lanes per entry (a,c) of cell (i,j) ------------------------------------------------
+      // ---- cooperative items: 8 consecutive lanes share one item and split its contiguous bond range -----------------
+      //   M2 edge ranges | Bl | Br | Z1 | Z2 : weighted dot products of two row segments;   X : lanes split u = 4..30
       {
-        const int cnt = nb0 << (lgM + 2), cntp = (cnt + 31) & ~31;
-        for (int it = tid; it < cntp; it += NT) {
+        const int n9 = nb0 << lgM;                          // M2 edge: (bond row of i) x c
+        const int n3 = closed ? nb1 << lgM : 0;             // Bl, Br: (bond row of p) x c1
+        const int n5 = closed ? nl1 << lgM : 0;             // Z1: (left state of p) x c2
+        const int n6 = closed ? nb2 << lgR : 0;             // Z2: (bond row of i+2) x r
+        const int n2 = d >= 4 ? nb2 << lgM : 0;             // X : (bond row of i+2) x c2
+        const int e9 = n9, e3 = e9 + n3, e4 = e3 + n3, e5 = e4 + n5, e6 = e5 + n6, e2 = e6 + n2;
+        const int nts = ((e2 << 3) + 31) & ~31;
+        for (int ts = tid; ts < nts; ts += NT) {
+          const int g = ts >> 3, sub = ts & 7;
           double acc = 0.0;
-          bool valid = false;
-          int ci = 0, a = 0, c = 0;
-          const int sub = it & 3;
-          if (it < cnt) {
-            c = (it >> 2) & (Mp - 1);
-            const int rr = rb0 + (it >> (lgM + 2)), kp = rbpos[rr];
-            a = rr - crow[kp];
-            const int i = rbase + kp, j = i + d;
-            ci = i - clo;
-            const PosMeta mj1 = colm[j + 1 - cbase];
-            if (c < mj1.sig) {
-              valid = true;
-              const int offi = rowm[kp].off, offj1 = mj1.off;
-              int ra0, ra1, q0 = 0, q1 = 0;
-              if (I == J) {
-                ra0 = rowm[kp + 1].off;
-                ra1 = offj1;
-              } else {
-                ra1 = (I + 1) * CDZ_TB;
-                ra0 = rowm[kp + 1].off < ra1 ? rowm[kp + 1].off : ra1;
-                q0 = J * CDZ_TB;
-                q1 = offj1;
+          double* out = nullptr;
+          if (g < e6) {
+            // ---- decode into: acc = sum_{kb in [lo,hi)} wt[sg * pos(kb) + cst] A[kb] Bv[kb]  (+ second range for M2) ----
+            const double *A = nullptr, *Bv = nullptr, *wt = nullptr;
+            const uint8_t* bp = rbp;
+            int lo = 0, hi = 0, lo2 = 0, hi2 = 0, kb0 = rkb0, pb = rbase, sg = 0, cst = 0;
+            double add = 0.0;
+            if (g < e9) {
+              const int c = g & (Mp - 1), rr = rb0 + (g >> lgM), kp = rbpos[rr], a = rr - crow[kp];
+              const int i = rbase + kp, j = i + d;
+              const PosMeta mj1 = colm[j + 1 - cbase];
+              if (c < mj1.sig) {
+                const int offi = rowm[kp].off, offj1 = mj1.off;
+                if (I == J) {
+                  lo = rowm[kp + 1].off;
+                  hi = offj1;
+                } else {
+                  hi = (I + 1) * CDZ_TB;
+                  lo = rowm[kp + 1].off < hi ? rowm[kp + 1].off : hi;
+                  lo2 = J * CDZ_TB;
+                  hi2 = offj1;
+                }
+                A = b.QM + (size_t)(offi + a) * S;
+                Bv = b.QM1T + (size_t)(offj1 + c) * S;
+                out = scr_of(scrb, dm, i - clo).M2s + a * M + c;
+                const double* gp = b.GP + (size_t)I * ka.nsplit * (CDZ_TB * CDZ_TB) +
+                                   (size_t)(offi - I * CDZ_TB + a) * CDZ_TB + (offj1 - J * CDZ_TB + c);
+                for (int sp = sub; sp < ka.nsplit; sp += 8) add += gp[(size_t)sp * (CDZ_TB * CDZ_TB)];
               }
-              const double* A = b.QM + (size_t)(offi + a) * S;
-              const double* Bt = b.QM1T + (size_t)(offj1 + c) * S;
-              double acc2 = 0.0;
-              for (int kb = ra0 + sub; kb < ra1; kb += 4) acc += A[kb] * Bt[kb];
-              for (int kb = q0 + sub; kb < q1; kb += 4) acc2 += A[kb] * Bt[kb];
-              acc += acc2;
-              const double* gp = b.GP + (size_t)I * ka.nsplit * (CDZ_TB * CDZ_TB) +
-                                 (size_t)(offi - I * CDZ_TB + a) * CDZ_TB + (offj1 - J * CDZ_TB + c);
-              for (int sp = sub; sp < ka.nsplit; sp += 4) acc += gp[(size_t)sp * (CDZ_TB * CDZ_TB)];
-            }
-          }
-          acc += __shfl_xor_sync(0xffffffffu, acc, 1);
-          acc += __shfl_xor_sync(0xffffffffu, acc, 2);
-          if (valid && sub == 0) scr_of(scrb, dm, ci).M2s[a * M + c] = acc;
-        }
-      }
-      // ---- all other item types in one flat index space -----------------------------------------------------------
-      {
-        const int n3 = closed ? nb1 << lgM : 0;            // Bl
-        const int n4 = n3;                                 // Br
-        const int n5 = closed ? nl1 << lgM : 0;            // Z1
-        const int n6 = closed ? nb2 << lgR : 0;            // Z2
-        const int n2 = d >= 4 ? nb2 << lgM : 0;            // X / XE
-        const int n7 = closed ? nb1 << (lgM + lgP) : 0;    // SB
-        const int n8 = nb0 << lgM;                         // recursive parts of Qm1, Qml
-        const int e3 = n3, e4 = e3 + n4, e5 = e4 + n5, e6 = e5 + n6, e2 = e6 + n2, e7 = e2 + n7, e8 = e7 + n8,
-                  e1 = e8 + n8;
-        for (int g = tid; g < e1; g += NT) {
-          if (g < e4) {
-            // ---- Bl: multiloop closure + left bulges l1 >= 2;  Br: right bulges l2 >= 2 --------------------------
-            const bool left = g < e3;
-            const int it = left ? g : g - e3;
-            const int c1 = it & (Mp - 1), rr = rb1 + (it >> lgM), kp = rbpos[rr], a1 = rr - crow[kp];
-            const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
-            const PosMeta mj = colm[j - cbase];
-            if (c1 >= mj.sig) continue;
-            const int offp = rowm[kp].off;
-            double acc = 0.0;
-            if (left) {
-              acc = cm.wac * b.M2[(size_t)(offp + a1) * S + mj.off + c1];
-              const double* A = b.EM + (size_t)(offp + a1) * S;
-              const double* Bv = b.QBST + (size_t)(mj.off + c1) * S;
-              const int lmax = min(maxint, q - mh1 - p);
-              for (int l1 = 2; l1 <= lmax; ++l1) {
-                const PosMeta mk = rowm[kp + l1];
-                double s = 0.0;
-                for (int u = 0; u < mk.sig; ++u) s += A[mk.off + u] * Bv[mk.off + u];
-                acc += cm.wbu[l1] * s;
+            } else if (g < e4) {
+              const bool left = g < e3;
+              const int it = left ? g - e9 : g - e3;
+              const int c1 = it & (Mp - 1), rr = rb1 + (it >> lgM), kp = rbpos[rr], a1 = rr - crow[kp];
+              const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
+              const PosMeta mj = colm[j - cbase];
+              if (c1 < mj.sig) {
+                const int offp = rowm[kp].off;
+                const int lmax = min(maxint, q - mh1 - p);
+                wt = cm.wbu;
+                if (left) {
+                  // multiloop closure + left bulges l1 = 2..lmax: E(p,k-1)[a1,s] Qbs(k,q)[s,c1], k = p + l1
+                  if (sub == 0) add = cm.wac * b.M2[(size_t)(offp + a1) * S + mj.off + c1];
+                  A = b.EM + (size_t)(offp + a1) * S;
+                  Bv = b.QBST + (size_t)(mj.off + c1) * S;
+                  if (lmax >= 2) { lo = rowm[kp + 2].off; hi = rowm[kp + lmax].off + rowm[kp + lmax].sig; }
+                  sg = 1; cst = -p;
+                  out = scr_of(scrb, dm, i - clo).Bl + a1 * M + c1;
+                } else {
+                  // right bulges l2 = 2..lmax: Qbs(p,l)[a1,u] E(l+1,q)[u,c1], l = q - l2
+                  A = b.QBS + (size_t)(offp + a1) * S;
+                  Bv = b.EMT + (size_t)(mj.off + c1) * S;
+                  if (lmax >= 2) { lo = colm[q - lmax + 1 - cbase].off; hi = colm[q - 1 - cbase].off + colm[q - 1 - cbase].sig; }
+                  bp = cbp; kb0 = ckb0; pb = cbase; sg = -1; cst = j;
+                  out = scr_of(scrb, dm, i - clo).Br + a1 * M + c1;
+                }
               }
-              scr_of(scrb, dm, i - clo).Bl[a1 * M + c1] = acc;
+            } else if (g < e5) {
+              // Z1[lst][c2]: l1 = 1, l2 = 2..lmax: D1(p; l+2)[lst,u] E(l+2,q-1)[u,c2], l = q - l2, weight win[1+l2]
+              const int it = g - e4;
+              const int c2 = it & (Mp - 1), ll = rl1 + (it >> lgM), kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
+              const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
+              const PosMeta mq = colm[q - cbase];
+              if (c2 < mq.sig) {
+                const int lmax = min(maxint - 1, q - mh1 - (p + 1));
+                A = b.D1 + (size_t)(rowm[kp].loff + lst) * S;
+                Bv = b.EMT + (size_t)(mq.off + c2) * S;
+                if (lmax >= 2) { lo = colm[q - lmax + 2 - cbase].off; hi = mq.off + mq.sig; }
+                bp = cbp; kb0 = ckb0; pb = cbase; wt = cm.win; sg = -1; cst = j + 2;
+                out = scr_of(scrb, dm, i - clo).Z1 + lst * M + c2;
+              }
             } else {
-              const double* A = b.QBS + (size_t)(offp + a1) * S;
-              const double* Bv = b.EMT + (size_t)(mj.off + c1) * S;
-              const int lmax = min(maxint, q - mh1 - p);
-              for (int l2 = 2; l2 <= lmax; ++l2) {
-                const PosMeta mm = colm[q - l2 + 1 - cbase];
-                double s = 0.0;
-                for (int u = 0; u < mm.sig; ++u) s += A[mm.off + u] * Bv[mm.off + u];
-                acc += cm.wbu[l2] * s;
+              // Z2[a2][r]: l2 = 1, l1 = 2..lmax: E(p+1,k-2)[a2,s] D2(k-1; q)[s,r], k = p + l1, weight win[l1+1]
+              const int it = g - e5;
+              const int r = it & (MRp - 1), rr = rb2 + (it >> lgR), kp = rbpos[rr], a2 = rr - crow[kp];
+              const int i = rbase + kp - 2, p = i + 1, j = i + d, q = j - 1;
+              const PosMeta mq = colm[q - cbase];
+              if (r < mq.nR) {
+                const int lmax = min(maxint - 1, (q - 1) - mh1 - p);
+                A = b.EM + (size_t)(rowm[kp].off + a2) * S;
+                Bv = b.D2T + (size_t)(mq.roff + r) * S;
+                if (lmax >= 2) { lo = rowm[kp].off; hi = rowm[kp + lmax - 2].off + rowm[kp + lmax - 2].sig; }
+                wt = cm.win; sg = 1; cst = 2 - p;
+                out = scr_of(scrb, dm, i - clo).Z2 + a2 * MR + r;
               }
-              scr_of(scrb, dm, i - clo).Br[a1 * M + c1] = acc;
             }
-          } else if (g < e5) {
-            // ---- Z1[lst][c2]: l1 = 1, l2 >= 2 -------------------------------------------------------------------------
-            const int it = g - e4;
-            const int c2 = it & (Mp - 1), ll = rl1 + (it >> lgM), kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
-            const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
-            const PosMeta mq = colm[q - cbase];
-            if (c2 >= mq.sig) continue;
-            const double* A = b.D1 + (size_t)(rowm[kp].loff + lst) * S;
-            const double* Bv = b.EMT + (size_t)(mq.off + c2) * S;
-            const int lmax = min(maxint - 1, q - mh1 - (p + 1));
-            double acc = 0.0;
-            for (int l2 = 2; l2 <= lmax; ++l2) {
-              const PosMeta mm = colm[q - l2 + 2 - cbase];
-              double s = 0.0;
-              for (int u = 0; u < mm.sig; ++u) s += A[mm.off + u] * Bv[mm.off + u];
-              acc += cm.win[1 + l2] * s;
+            if (wt) {
+#pragma unroll 4
+              for (int kb = lo + sub; kb < hi; kb += 8) acc += wt[sg * (pb + bp[kb - kb0]) + cst] * (A[kb] * Bv[kb]);
+            } else {
+              double acc2 = 0.0;
+#pragma unroll 4
+              for (int kb = lo + sub; kb < hi; kb += 8) acc += A[kb] * Bv[kb];
+#pragma unroll 4
+              for (int kb = lo2 + sub; kb < hi2; kb += 8) acc2 += A[kb] * Bv[kb];
+              acc += acc2;
             }
-            scr_of(scrb, dm, i - clo).Z1[lst * M + c2] = acc;
-          } else if (g < e6) {
-            // ---- Z2[a2][r]: l2 = 1, l1 >= 2 ------------------------------------------------------------------------------
-            const int it = g - e5;
-            const int r = it & (MRp - 1), rr = rb2 + (it >> lgR), kp = rbpos[rr], a2 = rr - crow[kp];
-            const int i = rbase + kp - 2, p = i + 1, j = i + d, q = j - 1;
-            const PosMeta mq = colm[q - cbase];
-            if (r >= mq.nR) continue;
-            const double* A = b.EM + (size_t)(rowm[kp].off + a2) * S;
-            const double* Bv = b.D2T + (size_t)(mq.roff + r) * S;
-            const int lmax = min(maxint - 1, (q - 1) - mh1 - p);
-            double acc = 0.0;
-            for (int l1 = 2; l1 <= lmax; ++l1) {
-              const PosMeta mk = rowm[kp - 1 + l1 - 1];  // position k-1 = p + l1 - 1; kp is position p+1
-              double s = 0.0;
-              for (int u = 0; u < mk.sig; ++u) s += A[mk.off + u] * Bv[mk.off + u];
-              acc += cm.win[l1 + 1] * s;
-            }
-            scr_of(scrb, dm, i - clo).Z2[a2 * MR + r] = acc;
+            acc += add;
           } else if (g < e2) {
-            // ---- X_u(i,j) row recursion, XE = sum_u win[u] X_u + hairpin interior ---------------------------------
+            // ---- X_u(i,j) = Tbar_{i+2} X_{u-1}(i+1,j) + GI(i+3, j+1-u) E(j+3-u, j-2), lanes split u; XE = sum_u win[u] X_u ----
             const int it = g - e6;
             const int c2 = it & (Mp - 1), rr = rb2 + (it >> lgM), kp = rbpos[rr], a2 = rr - crow[kp];
             const int i = rbase + kp - 2, j = i + d;
             const PosMeta mq = colm[j - 1 - cbase];
-            if (c2 >= mq.sig) continue;
-            const int offa = rowm[kp].off + a2, Sa3 = rowm[kp + 1].sig;
-            const double* Tb = Tbar + (size_t)(i + 2) * MS2 + a2 * MS;
-            const double* xo = b.XS + ((size_t)((i + 1) & 1) * n + j) * (XU * MS2) + c2;
-            double* xn = b.XS + ((size_t)(i & 1) * n + j) * (XU * MS2) + a2 * MS + c2;
-            const double* gi = b.GI + (size_t)offa * S;
-            const double* em = b.EMT + (size_t)(mq.off + c2) * S;
-            const bool hasold = d - 1 >= 4;
-            double xe = 0.0;
-            for (int u = 4; u <= 30; ++u) {
-              double acc = 0.0;
-              if (hasold && u > 4)
-                for (int a3 = 0; a3 < Sa3; ++a3) acc += Tb[a3] * xo[(u - 5) * MS2 + a3 * MS];
-              const int cp = j + 3 - u;
-              if (cp - (i + 2) - 3 >= mh1) {
-                const PosMeta mc = colm[cp - cbase];
-                for (int u2 = 0; u2 < mc.sig; ++u2) acc += gi[mc.off + u2] * em[mc.off + u2];
+            if (c2 < mq.sig) {
+              const int offa = rowm[kp].off + a2, Sa3 = rowm[kp + 1].sig;
+              const double* Tb = Tbar + (size_t)(i + 2) * MS2 + a2 * MS;
+              const double* xo = b.XS + ((size_t)((i + 1) & 1) * n + j) * (XU * MS2) + c2;
+              double* xn = b.XS + ((size_t)(i & 1) * n + j) * (XU * MS2) + a2 * MS + c2;
+              const double* gi = b.GI + (size_t)offa * S;
+              const double* em = b.EMT + (size_t)(mq.off + c2) * S;
+              const bool hasold = d - 1 >= 4;
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                const int u = 4 + sub + 8 * k;
+                if (u > 30) break;
+                double x = 0.0;
+                if (hasold && u > 4)
+                  for (int a3 = 0; a3 < Sa3; ++a3) x += Tb[a3] * xo[(u - 5) * MS2 + a3 * MS];
+                const int cp = j + 3 - u;
+                if (cp - (i + 2) - 3 >= mh1) {
+                  const PosMeta mc = colm[cp - cbase];
+                  for (int u2 = 0; u2 < mc.sig; ++u2) x += gi[mc.off + u2] * em[mc.off + u2];
+                }
+                xn[(u - 4) * MS2] = x;
+                if (u <= maxint) acc += cm.win[u] * x;
               }
-              xn[(u - 4) * MS2] = acc;
-              if (u <= maxint) xe += cm.win[u] * acc;
+              if (closed && sub == 0) acc += t.wh[d - 1] * b.EM[(size_t)offa * S + mq.off + c2];
+              out = scr_of(scrb, dm, i - clo).XE + a2 * M + c2;
             }
-            if (closed) xe += t.wh[d - 1] * b.EM[(size_t)offa * S + mq.off + c2];
-            scr_of(scrb, dm, i - clo).XE[a2 * M + c2] = xe;
-          } else if (g < e7) {
+          }
+          acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+          acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+          acc += __shfl_xor_sync(0xffffffffu, acc, 4);
+          if (out != nullptr && sub == 0) *out = acc;
+        }
+      }
+      // ---- single-lane items: SB | recursive parts of Qm1, Qml | E(i,j) ----------------------------------------------------
+      {
+        const int npm = nps << lgM;
+        const int n7 = closed ? nb1 * npm : 0;
+        const int n8 = nb0 << lgM;
+        const int e7 = n7, e8 = e7 + n8, e1 = e8 + n8;
+        for (int g = tid; g < e1; g += NT) {
+          if (g < e7) {
             // ---- SB[a'][slot'][c']: inner pair identity kept (stack, bulges of size 1) ------------------------------
-            const int it = g - e2;
-            const int c1 = it & (Mp - 1), sl = (it >> lgM) & (NPp - 1), rr = rb1 + (it >> (lgM + lgP));
+            const int rq = g / npm, it = g - rq * npm;
+            const int c1 = it & (Mp - 1), sl = it >> lgM, rr = rb1 + rq;
             const int kp = rbpos[rr], a1 = rr - crow[kp];
             const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
             const PosMeta mj = colm[j - cbase];
-            if (c1 >= mj.sig || sl >= nps) continue;
+            if (c1 >= mj.sig) continue;
             const PosMeta mp = rowm[kp], mq = colm[q - cbase];
             const int xp = cm.slot_x[sl], yp = cm.slot_y[sl];
             int lst = -1, r = -1;
@@ -409,6 +419,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             }
             scr_of(scrb, dm, i - clo).SB[(a1 * nps + sl) * M + c1] = v;
           } else {
+
             // ---- recursive parts of Qm1 / Qml (g < e8) and E(i,j) (g >= e8) -----------------------------------------
             const bool rec = g < e8;
             const int it = rec ? g - e7 : g - e8;
@@ -649,20 +660,33 @@ int cdz_cell_config(cdz_tables* const* ts, int B, cdz_cell_cfg* cfg) {
   dm.lgM = clog2(dm.M);
   dm.lgR = clog2(dm.MR);
   dm.lgP = clog2(dm.nps);
+  int span = 1;
+  for (int k = 0; k < B; ++k) {
+    const cdz_tt* tt = ts[k]->tt;
+    const int n = tt->n;
+    for (int bk = 0; bk < tt->NB; ++bk) {
+      const int i0 = tt->blk_start[bk], i1 = std::min(tt->blk_start[bk + 1], n);
+      const int rbase = std::max(i0 - 1, 0), rend = std::min(i1 + ROWPAD - 2, n);
+      span = std::max(span, tt->off[rend] + tt->sigma[rend] - tt->off[rbase]);
+      const int j0 = std::max(tt->blk_start[bk], 1) - 1, j1 = tt->blk_start[bk + 1] - 1;
+      const int cbase = std::max(j0 - COLPAD + 1, 0), cend = std::min(j1 + 1, n);
+      span = std::max(span, tt->off[cend] + tt->sigma[cend] - tt->off[cbase]);
+    }
+  }
   const size_t budget = 200 * 1024;
   int C = maxpos;
-  while (C > 1 && make_plan(maxpos, dm, C).total > budget) --C;
-  const Plan pl = make_plan(maxpos, dm, C);
+  while (C > 1 && make_plan(maxpos, span, dm, C).total > budget) --C;
+  const Plan pl = make_plan(maxpos, span, dm, C);
   if (pl.total > budget) { cdz_set_error("cell kernel: shared-memory need exceeds 200 KB"); return CDZ_ENOMEM; }
   cfg->M = dm.M; cfg->ML = dm.ML; cfg->MR = dm.MR; cfg->nps = dm.nps;
-  cfg->maxpos = maxpos; cfg->C = C; cfg->smem = pl.total;
+  cfg->maxpos = maxpos; cfg->span = span; cfg->C = C; cfg->smem = pl.total;
   CDZ_CUDA(cudaFuncSetAttribute(cell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.total));
   return CDZ_OK;
 }
 
 void cdz_launch_cells(const Ctx* d_ctxs, int B, int nblk, int D, int nsplit, const cdz_cell_cfg* cfg, cudaStream_t st) {
   KArgs ka;
-  ka.D = D; ka.nsplit = nsplit; ka.C = cfg->C; ka.maxpos = cfg->maxpos;
+  ka.D = D; ka.nsplit = nsplit; ka.C = cfg->C; ka.maxpos = cfg->maxpos; ka.span = cfg->span;
   ka.dm.M = cfg->M; ka.dm.ML = cfg->ML; ka.dm.MR = cfg->MR; ka.dm.nps = cfg->nps;
   ka.dm.lgM = clog2(cfg->M); ka.dm.lgR = clog2(cfg->MR); ka.dm.lgP = clog2(cfg->nps);
   cell_kernel<<<dim3(nblk, B), CELL_THREADS, cfg->smem, st>>>(d_ctxs, ka);

@@ -143,7 +143,7 @@ inline int cdz_nsplit(int NB, int D, int B) {
 
 // ---- internal entry points -----------------------------------------------------------------------
 void cdz_set_error(const std::string& s);
-struct cdz_cell_cfg { int M, ML, MR, nps, maxpos, C; size_t smem; };
+struct cdz_cell_cfg { int M, ML, MR, nps, maxpos, span, C; size_t smem; };
 int cdz_cell_config(cdz_tables* const* ts, int B, cdz_cell_cfg* cfg);
 void cdz_launch_cells(const Ctx* d_ctxs, int B, int nblk, int D, int nsplit, const cdz_cell_cfg* cfg, cudaStream_t st);
 int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st);
