@@ -226,153 +226,209 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
       const int nb1 = bond_rows(clo + 1, chi + 1, rb1);  // bonds of position p = i+1
       const int nb2 = bond_rows(clo + 2, chi + 2, rb2);  // bonds of position i+2
       const int nl1 = ls_rows(clo + 1, chi + 1, rl1);    // left states of position p
-      // ---- cooperative items: 8 consecutive lanes share one item and split its contiguous bond range -----------------
-      //   M2 edge ranges | Bl | Br | Z1 | Z2 : weighted dot products of two row segments;   X : lanes split u = 4..30
+      // ---- cooperative row items: 8 consecutive lanes share one row object (a bond row or a left state of one cell), split
+      //      its contiguous bond range between them and keep up to 4 column accumulators per pass.
+      //      M2 edge ranges | Bl | Br | Z1 | Z2 : weighted dot products of row segments;   X : the lanes split u = 4..30
       {
-        const int n9 = nb0 << lgM;                          // M2 edge: (bond row of i) x c
-        const int n3 = closed ? nb1 << lgM : 0;             // Bl, Br: (bond row of p) x c1
-        const int n5 = closed ? nl1 << lgM : 0;             // Z1: (left state of p) x c2
-        const int n6 = closed ? nb2 << lgR : 0;             // Z2: (bond row of i+2) x r
-        const int n2 = d >= 4 ? nb2 << lgM : 0;             // X : (bond row of i+2) x c2
+        const int n9 = nb0;               // M2 edge: bond row of i    x  c  < Sigma_{j+1}
+        const int n3 = closed ? nb1 : 0;  // Bl, Br : bond row of p    x  c1 < Sigma_j
+        const int n5 = closed ? nl1 : 0;  // Z1     : left state of p  x  c2 < Sigma_q
+        const int n6 = closed ? nb2 : 0;  // Z2     : bond row of i+2  x  r  < |R_q|
+        const int n2 = d >= 4 ? nb2 : 0;  // X      : bond row of i+2  x  c2 < Sigma_q
         const int e9 = n9, e3 = e9 + n3, e4 = e3 + n3, e5 = e4 + n5, e6 = e5 + n6, e2 = e6 + n2;
-        const int nts = ((e2 << 3) + 31) & ~31;
-        for (int ts = tid; ts < nts; ts += NT) {
+        const unsigned gmask = 0xFFu << (tid & 24);
+        for (int ts = tid; ts < (e2 << 3); ts += NT) {
           const int g = ts >> 3, sub = ts & 7;
-          double acc = 0.0;
-          double* out = nullptr;
           if (g < e6) {
-            // ---- decode into: acc = sum_{kb in [lo,hi)} wt[sg * pos(kb) + cst] A[kb] Bv[kb]  (+ second range for M2) ----
-            const double *A = nullptr, *Bv = nullptr, *wt = nullptr;
+            // ---- decode: out[c] = add[c] + sum_{kb in [lo,hi) (+ [lo2,hi2))} wt[sg * pos(kb) + cst] A[kb] B0[c * S + kb] -------
+            const double *A = nullptr, *B0 = nullptr, *wt = nullptr, *addp = nullptr;
+            double* out = nullptr;
             const uint8_t* bp = rbp;
-            int lo = 0, hi = 0, lo2 = 0, hi2 = 0, kb0 = rkb0, pb = rbase, sg = 0, cst = 0;
-            double add = 0.0;
+            int ncol = 0, lo = 0, hi = 0, lo2 = 0, hi2 = 0, kb0 = rkb0, pb = rbase, sg = 0, cst = 0, nadd = 0;
+            double addw = 1.0;
             if (g < e9) {
-              const int c = g & (Mp - 1), rr = rb0 + (g >> lgM), kp = rbpos[rr], a = rr - crow[kp];
+              const int rr = rb0 + g, kp = rbpos[rr], a = rr - crow[kp];
               const int i = rbase + kp, j = i + d;
               const PosMeta mj1 = colm[j + 1 - cbase];
-              if (c < mj1.sig) {
-                const int offi = rowm[kp].off, offj1 = mj1.off;
-                if (I == J) {
-                  lo = rowm[kp + 1].off;
-                  hi = offj1;
-                } else {
-                  hi = (I + 1) * CDZ_TB;
-                  lo = rowm[kp + 1].off < hi ? rowm[kp + 1].off : hi;
-                  lo2 = J * CDZ_TB;
-                  hi2 = offj1;
-                }
-                A = b.QM + (size_t)(offi + a) * S;
-                Bv = b.QM1T + (size_t)(offj1 + c) * S;
-                out = scr_of(scrb, dm, i - clo).M2s + a * M + c;
-                const double* gp = b.GP + (size_t)I * ka.nsplit * (CDZ_TB * CDZ_TB) +
-                                   (size_t)(offi - I * CDZ_TB + a) * CDZ_TB + (offj1 - J * CDZ_TB + c);
-                for (int sp = sub; sp < ka.nsplit; sp += 8) add += gp[(size_t)sp * (CDZ_TB * CDZ_TB)];
+              const int offi = rowm[kp].off, offj1 = mj1.off;
+              ncol = mj1.sig;
+              if (I == J) {
+                lo = rowm[kp + 1].off;
+                hi = offj1;
+              } else {
+                hi = (I + 1) * CDZ_TB;
+                lo = rowm[kp + 1].off < hi ? rowm[kp + 1].off : hi;
+                lo2 = J * CDZ_TB;
+                hi2 = offj1;
               }
+              A = b.QM + (size_t)(offi + a) * S;
+              B0 = b.QM1T + (size_t)offj1 * S;
+              out = scr_of(scrb, dm, i - clo).M2s + a * M;
+              addp = b.GP + (size_t)I * ka.nsplit * (CDZ_TB * CDZ_TB) + (size_t)(offi - I * CDZ_TB + a) * CDZ_TB +
+                     (offj1 - J * CDZ_TB);
+              nadd = ka.nsplit;
             } else if (g < e4) {
               const bool left = g < e3;
-              const int it = left ? g - e9 : g - e3;
-              const int c1 = it & (Mp - 1), rr = rb1 + (it >> lgM), kp = rbpos[rr], a1 = rr - crow[kp];
+              const int rr = rb1 + (left ? g - e9 : g - e3), kp = rbpos[rr], a1 = rr - crow[kp];
               const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
               const PosMeta mj = colm[j - cbase];
-              if (c1 < mj.sig) {
-                const int offp = rowm[kp].off;
-                const int lmax = min(maxint, q - mh1 - p);
-                wt = cm.wbu;
-                if (left) {
-                  // multiloop closure + left bulges l1 = 2..lmax: E(p,k-1)[a1,s] Qbs(k,q)[s,c1], k = p + l1
-                  if (sub == 0) add = cm.wac * b.M2[(size_t)(offp + a1) * S + mj.off + c1];
-                  A = b.EM + (size_t)(offp + a1) * S;
-                  Bv = b.QBST + (size_t)(mj.off + c1) * S;
-                  if (lmax >= 2) { lo = rowm[kp + 2].off; hi = rowm[kp + lmax].off + rowm[kp + lmax].sig; }
-                  sg = 1; cst = -p;
-                  out = scr_of(scrb, dm, i - clo).Bl + a1 * M + c1;
-                } else {
-                  // right bulges l2 = 2..lmax: Qbs(p,l)[a1,u] E(l+1,q)[u,c1], l = q - l2
-                  A = b.QBS + (size_t)(offp + a1) * S;
-                  Bv = b.EMT + (size_t)(mj.off + c1) * S;
-                  if (lmax >= 2) { lo = colm[q - lmax + 1 - cbase].off; hi = colm[q - 1 - cbase].off + colm[q - 1 - cbase].sig; }
-                  bp = cbp; kb0 = ckb0; pb = cbase; sg = -1; cst = j;
-                  out = scr_of(scrb, dm, i - clo).Br + a1 * M + c1;
-                }
+              const int offp = rowm[kp].off;
+              const int lmax = min(maxint, q - mh1 - p);
+              ncol = mj.sig;
+              wt = cm.wbu;
+              if (left) {
+                // multiloop closure + left bulges l1 = 2..lmax: E(p,k-1)[a1,s] Qbs(k,q)[s,c1], k = p + l1
+                addp = b.M2 + (size_t)(offp + a1) * S + mj.off;
+                nadd = 1;
+                addw = cm.wac;
+                A = b.EM + (size_t)(offp + a1) * S;
+                B0 = b.QBST + (size_t)mj.off * S;
+                if (lmax >= 2) { lo = rowm[kp + 2].off; hi = rowm[kp + lmax].off + rowm[kp + lmax].sig; }
+                sg = 1; cst = -p;
+                out = scr_of(scrb, dm, i - clo).Bl + a1 * M;
+              } else {
+                // right bulges l2 = 2..lmax: Qbs(p,l)[a1,u] E(l+1,q)[u,c1], l = q - l2
+                A = b.QBS + (size_t)(offp + a1) * S;
+                B0 = b.EMT + (size_t)mj.off * S;
+                if (lmax >= 2) { lo = colm[q - lmax + 1 - cbase].off; hi = colm[q - 1 - cbase].off + colm[q - 1 - cbase].sig; }
+                bp = cbp; kb0 = ckb0; pb = cbase; sg = -1; cst = j;
+                out = scr_of(scrb, dm, i - clo).Br + a1 * M;
               }
             } else if (g < e5) {
               // Z1[lst][c2]: l1 = 1, l2 = 2..lmax: D1(p; l+2)[lst,u] E(l+2,q-1)[u,c2], l = q - l2, weight win[1+l2]
-              const int it = g - e4;
-              const int c2 = it & (Mp - 1), ll = rl1 + (it >> lgM), kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
+              const int ll = rl1 + (g - e4), kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
               const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
               const PosMeta mq = colm[q - cbase];
-              if (c2 < mq.sig) {
-                const int lmax = min(maxint - 1, q - mh1 - (p + 1));
-                A = b.D1 + (size_t)(rowm[kp].loff + lst) * S;
-                Bv = b.EMT + (size_t)(mq.off + c2) * S;
-                if (lmax >= 2) { lo = colm[q - lmax + 2 - cbase].off; hi = mq.off + mq.sig; }
-                bp = cbp; kb0 = ckb0; pb = cbase; wt = cm.win; sg = -1; cst = j + 2;
-                out = scr_of(scrb, dm, i - clo).Z1 + lst * M + c2;
-              }
+              const int lmax = min(maxint - 1, q - mh1 - (p + 1));
+              ncol = mq.sig;
+              A = b.D1 + (size_t)(rowm[kp].loff + lst) * S;
+              B0 = b.EMT + (size_t)mq.off * S;
+              if (lmax >= 2) { lo = colm[q - lmax + 2 - cbase].off; hi = mq.off + mq.sig; }
+              bp = cbp; kb0 = ckb0; pb = cbase; wt = cm.win; sg = -1; cst = j + 2;
+              out = scr_of(scrb, dm, i - clo).Z1 + lst * M;
             } else {
               // Z2[a2][r]: l2 = 1, l1 = 2..lmax: E(p+1,k-2)[a2,s] D2(k-1; q)[s,r], k = p + l1, weight win[l1+1]
-              const int it = g - e5;
-              const int r = it & (MRp - 1), rr = rb2 + (it >> lgR), kp = rbpos[rr], a2 = rr - crow[kp];
+              const int rr = rb2 + (g - e5), kp = rbpos[rr], a2 = rr - crow[kp];
               const int i = rbase + kp - 2, p = i + 1, j = i + d, q = j - 1;
               const PosMeta mq = colm[q - cbase];
-              if (r < mq.nR) {
-                const int lmax = min(maxint - 1, (q - 1) - mh1 - p);
-                A = b.EM + (size_t)(rowm[kp].off + a2) * S;
-                Bv = b.D2T + (size_t)(mq.roff + r) * S;
-                if (lmax >= 2) { lo = rowm[kp].off; hi = rowm[kp + lmax - 2].off + rowm[kp + lmax - 2].sig; }
-                wt = cm.win; sg = 1; cst = 2 - p;
-                out = scr_of(scrb, dm, i - clo).Z2 + a2 * MR + r;
+              const int lmax = min(maxint - 1, (q - 1) - mh1 - p);
+              ncol = mq.nR;
+              A = b.EM + (size_t)(rowm[kp].off + a2) * S;
+              B0 = b.D2T + (size_t)mq.roff * S;
+              if (lmax >= 2) { lo = rowm[kp].off; hi = rowm[kp + lmax - 2].off + rowm[kp + lmax - 2].sig; }
+              wt = cm.win; sg = 1; cst = 2 - p;
+              out = scr_of(scrb, dm, i - clo).Z2 + a2 * MR;
+            }
+            for (int cc = 0; cc < ncol; cc += 4) {
+              const int nc4 = min(4, ncol - cc);
+              const double* Bc = B0 + (size_t)cc * S;
+              double add = 0.0;
+              if (sub < nc4)
+                for (int sp = 0; sp < nadd; ++sp) add += addp[(size_t)sp * (CDZ_TB * CDZ_TB) + cc + sub];
+              double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+              if (wt) {
+#pragma unroll 2
+                for (int kb = lo + sub; kb < hi; kb += 8) {
+                  const double w = wt[sg * (pb + bp[kb - kb0]) + cst] * A[kb];
+                  a0 += w * Bc[kb];
+                  if (nc4 > 1) a1 += w * Bc[S + kb];
+                  if (nc4 > 2) a2 += w * Bc[2 * S + kb];
+                  if (nc4 > 3) a3 += w * Bc[3 * S + kb];
+                }
+              } else {
+#pragma unroll 2
+                for (int kb = lo + sub; kb < hi; kb += 8) {
+                  const double w = A[kb];
+                  a0 += w * Bc[kb];
+                  if (nc4 > 1) a1 += w * Bc[S + kb];
+                  if (nc4 > 2) a2 += w * Bc[2 * S + kb];
+                  if (nc4 > 3) a3 += w * Bc[3 * S + kb];
+                }
+#pragma unroll 2
+                for (int kb = lo2 + sub; kb < hi2; kb += 8) {
+                  const double w = A[kb];
+                  a0 += w * Bc[kb];
+                  if (nc4 > 1) a1 += w * Bc[S + kb];
+                  if (nc4 > 2) a2 += w * Bc[2 * S + kb];
+                  if (nc4 > 3) a3 += w * Bc[3 * S + kb];
+                }
               }
+#pragma unroll
+              for (int o = 1; o < 8; o <<= 1) {
+                a0 += __shfl_xor_sync(gmask, a0, o);
+                a1 += __shfl_xor_sync(gmask, a1, o);
+                a2 += __shfl_xor_sync(gmask, a2, o);
+                a3 += __shfl_xor_sync(gmask, a3, o);
+              }
+              if (sub < nc4) out[cc + sub] = addw * add + (sub == 0 ? a0 : sub == 1 ? a1 : sub == 2 ? a2 : a3);
             }
-            if (wt) {
-#pragma unroll 4
-              for (int kb = lo + sub; kb < hi; kb += 8) acc += wt[sg * (pb + bp[kb - kb0]) + cst] * (A[kb] * Bv[kb]);
-            } else {
-              double acc2 = 0.0;
-#pragma unroll 4
-              for (int kb = lo + sub; kb < hi; kb += 8) acc += A[kb] * Bv[kb];
-#pragma unroll 4
-              for (int kb = lo2 + sub; kb < hi2; kb += 8) acc2 += A[kb] * Bv[kb];
-              acc += acc2;
-            }
-            acc += add;
-          } else if (g < e2) {
+          } else {
             // ---- X_u(i,j) = Tbar_{i+2} X_{u-1}(i+1,j) + GI(i+3, j+1-u) E(j+3-u, j-2), lanes split u; XE = sum_u win[u] X_u ----
-            const int it = g - e6;
-            const int c2 = it & (Mp - 1), rr = rb2 + (it >> lgM), kp = rbpos[rr], a2 = rr - crow[kp];
+            const int rr = rb2 + (g - e6), kp = rbpos[rr], a2 = rr - crow[kp];
             const int i = rbase + kp - 2, j = i + d;
             const PosMeta mq = colm[j - 1 - cbase];
-            if (c2 < mq.sig) {
-              const int offa = rowm[kp].off + a2, Sa3 = rowm[kp + 1].sig;
-              const double* Tb = Tbar + (size_t)(i + 2) * MS2 + a2 * MS;
-              const double* xo = b.XS + ((size_t)((i + 1) & 1) * n + j) * (XU * MS2) + c2;
-              double* xn = b.XS + ((size_t)(i & 1) * n + j) * (XU * MS2) + a2 * MS + c2;
-              const double* gi = b.GI + (size_t)offa * S;
-              const double* em = b.EMT + (size_t)(mq.off + c2) * S;
-              const bool hasold = d - 1 >= 4;
+            const int offa = rowm[kp].off + a2, Sa3 = rowm[kp + 1].sig;
+            const double* Tb = Tbar + (size_t)(i + 2) * MS2 + a2 * MS;
+            const double* xo = b.XS + ((size_t)((i + 1) & 1) * n + j) * (XU * MS2);
+            double* xn = b.XS + ((size_t)(i & 1) * n + j) * (XU * MS2) + a2 * MS;
+            const double* gi = b.GI + (size_t)offa * S;
+            const double* em = b.EMT + (size_t)mq.off * S;
+            const bool hasold = d - 1 >= 4;
+            double* out = scr_of(scrb, dm, i - clo).XE + a2 * M;
+            for (int cc = 0; cc < mq.sig; cc += 4) {
+              const int nc4 = min(4, mq.sig - cc);
+              double e0 = 0.0, e1 = 0.0, e2x = 0.0, e3x = 0.0;
 #pragma unroll
               for (int k = 0; k < 4; ++k) {
                 const int u = 4 + sub + 8 * k;
                 if (u > 30) break;
-                double x = 0.0;
-                if (hasold && u > 4)
-                  for (int a3 = 0; a3 < Sa3; ++a3) x += Tb[a3] * xo[(u - 5) * MS2 + a3 * MS];
+                double x0 = 0.0, x1 = 0.0, x2 = 0.0, x3 = 0.0;
+                if (hasold && u > 4) {
+                  const double* xr = xo + (u - 5) * MS2 + cc;
+                  for (int a3 = 0; a3 < Sa3; ++a3) {
+                    const double tb = Tb[a3];
+                    x0 += tb * xr[a3 * MS];
+                    if (nc4 > 1) x1 += tb * xr[a3 * MS + 1];
+                    if (nc4 > 2) x2 += tb * xr[a3 * MS + 2];
+                    if (nc4 > 3) x3 += tb * xr[a3 * MS + 3];
+                  }
+                }
                 const int cp = j + 3 - u;
                 if (cp - (i + 2) - 3 >= mh1) {
                   const PosMeta mc = colm[cp - cbase];
-                  for (int u2 = 0; u2 < mc.sig; ++u2) x += gi[mc.off + u2] * em[mc.off + u2];
+                  const double* er = em + (size_t)cc * S + mc.off;
+                  for (int u2 = 0; u2 < mc.sig; ++u2) {
+                    const double gv = gi[mc.off + u2];
+                    x0 += gv * er[u2];
+                    if (nc4 > 1) x1 += gv * er[S + u2];
+                    if (nc4 > 2) x2 += gv * er[2 * S + u2];
+                    if (nc4 > 3) x3 += gv * er[3 * S + u2];
+                  }
                 }
-                xn[(u - 4) * MS2] = x;
-                if (u <= maxint) acc += cm.win[u] * x;
+                double* xw = xn + (u - 4) * MS2 + cc;
+                xw[0] = x0;
+                if (nc4 > 1) xw[1] = x1;
+                if (nc4 > 2) xw[2] = x2;
+                if (nc4 > 3) xw[3] = x3;
+                if (u <= maxint) {
+                  const double w = cm.win[u];
+                  e0 += w * x0; e1 += w * x1; e2x += w * x2; e3x += w * x3;
+                }
               }
-              if (closed && sub == 0) acc += t.wh[d - 1] * b.EM[(size_t)offa * S + mq.off + c2];
-              out = scr_of(scrb, dm, i - clo).XE + a2 * M + c2;
+#pragma unroll
+              for (int o = 1; o < 8; o <<= 1) {
+                e0 += __shfl_xor_sync(gmask, e0, o);
+                e1 += __shfl_xor_sync(gmask, e1, o);
+                e2x += __shfl_xor_sync(gmask, e2x, o);
+                e3x += __shfl_xor_sync(gmask, e3x, o);
+              }
+              if (sub < nc4) {
+                double v = sub == 0 ? e0 : sub == 1 ? e1 : sub == 2 ? e2x : e3x;
+                if (closed) v += t.wh[d - 1] * b.EM[(size_t)offa * S + mq.off + cc + sub];
+                out[cc + sub] = v;
+              }
             }
           }
-          acc += __shfl_xor_sync(0xffffffffu, acc, 1);
-          acc += __shfl_xor_sync(0xffffffffu, acc, 2);
-          acc += __shfl_xor_sync(0xffffffffu, acc, 4);
-          if (out != nullptr && sub == 0) *out = acc;
         }
       }
       // ---- single-lane items: SB | recursive parts of Qm1, Qml | E(i,j) ----------------------------------------------------
