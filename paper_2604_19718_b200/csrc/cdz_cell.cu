@@ -35,6 +35,7 @@ constexpr int COLPAD = 34;   // column window [j0-COLPAD+1, j1+1]
 struct Dims {
   int M, ML, MR, nps;  // bond / left-state / right-state / pair-slot dimensions (strides of the scratch arrays)
   int lgM, lgR, lgP;   // ceil log2 of M, MR, nps (item decoding)
+  int pc;              // percell(), filled by the host
   __host__ __device__ int percell() const { return 6 * M * M + ML * M + M * MR + 2 * ML * MR + 2 * nps * M * M; }
 };
 
@@ -44,7 +45,7 @@ struct Scr {  // scratch of one cell
   double *XE, *Bl, *Br, *Z1, *Z2, *Y, *SB, *IN, *QBc, *M2s, *R1, *R2;
 };
 __device__ __forceinline__ Scr scr_of(double* base, const Dims& D, int ci) {
-  double* s = base + (size_t)ci * D.percell();
+  double* s = base + ci * D.pc;
   Scr k;
   const int MM = D.M * D.M;
   k.XE = s; s += MM;
@@ -214,6 +215,12 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
     return rowm[hi - rbase].loff + rowm[hi - rbase].nL - L0 - r0;
   };
 
+#ifdef CDZ_PHASE_TIMING
+  long long tph[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tlast = clock64();
+#define CDZ_TICK(k) do { const long long now__ = clock64(); tph[k] += now__ - tlast; tlast = now__; } while (0)
+#else
+#define CDZ_TICK(k)
+#endif
   const int dmin = max(0, j0 - (i1 - 1)), dmax = (j1 - 1) - i0;
   for (int d = dmin; d <= dmax; ++d) {
     const int ilo = max(i0, j0 - d), ihi = min(i1 - 1, j1 - 1 - d);
@@ -327,30 +334,50 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
                 for (int sp = 0; sp < nadd; ++sp) add += addp[(size_t)sp * (CDZ_TB * CDZ_TB) + cc + sub];
               double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
               if (wt) {
-#pragma unroll 2
-                for (int kb = lo + sub; kb < hi; kb += 8) {
-                  const double w = wt[sg * (pb + bp[kb - kb0]) + cst] * A[kb];
-                  a0 += w * Bc[kb];
-                  if (nc4 > 1) a1 += w * Bc[S + kb];
-                  if (nc4 > 2) a2 += w * Bc[2 * S + kb];
-                  if (nc4 > 3) a3 += w * Bc[3 * S + kb];
+                const double* B1 = Bc + (nc4 > 1 ? S : 0);
+                const double* B2 = Bc + (nc4 > 2 ? 2 * S : 0);
+                const double* B3 = Bc + (nc4 > 3 ? 3 * S : 0);
+                if (nc4 == 1) {
+#pragma unroll 4
+                  for (int kb = lo + sub; kb < hi; kb += 8)
+                    a0 += wt[sg * (pb + bp[kb - kb0]) + cst] * A[kb] * Bc[kb];
+                } else if (nc4 == 2) {
+#pragma unroll 4
+                  for (int kb = lo + sub; kb < hi; kb += 8) {
+                    const double w = wt[sg * (pb + bp[kb - kb0]) + cst] * A[kb];
+                    a0 += w * Bc[kb];
+                    a1 += w * B1[kb];
+                  }
+                } else {
+#pragma unroll 4
+                  for (int kb = lo + sub; kb < hi; kb += 8) {
+                    const double w = wt[sg * (pb + bp[kb - kb0]) + cst] * A[kb];
+                    a0 += w * Bc[kb];
+                    a1 += w * B1[kb];
+                    a2 += w * B2[kb];
+                    a3 += w * B3[kb];
+                  }
                 }
               } else {
-#pragma unroll 2
-                for (int kb = lo + sub; kb < hi; kb += 8) {
-                  const double w = A[kb];
-                  a0 += w * Bc[kb];
-                  if (nc4 > 1) a1 += w * Bc[S + kb];
-                  if (nc4 > 2) a2 += w * Bc[2 * S + kb];
-                  if (nc4 > 3) a3 += w * Bc[3 * S + kb];
-                }
-#pragma unroll 2
-                for (int kb = lo2 + sub; kb < hi2; kb += 8) {
-                  const double w = A[kb];
-                  a0 += w * Bc[kb];
-                  if (nc4 > 1) a1 += w * Bc[S + kb];
-                  if (nc4 > 2) a2 += w * Bc[2 * S + kb];
-                  if (nc4 > 3) a3 += w * Bc[3 * S + kb];
+                const double* B1 = Bc + (nc4 > 1 ? S : 0);
+                const double* B2 = Bc + (nc4 > 2 ? 2 * S : 0);
+                const double* B3 = Bc + (nc4 > 3 ? 3 * S : 0);
+                if (nc4 <= 2) {
+#pragma unroll 4
+                  for (int kb = lo + sub; kb < hi; kb += 8) { const double w = A[kb]; a0 += w * Bc[kb]; a1 += w * B1[kb]; }
+#pragma unroll 4
+                  for (int kb = lo2 + sub; kb < hi2; kb += 8) { const double w = A[kb]; a0 += w * Bc[kb]; a1 += w * B1[kb]; }
+                } else {
+#pragma unroll 4
+                  for (int kb = lo + sub; kb < hi; kb += 8) {
+                    const double w = A[kb];
+                    a0 += w * Bc[kb]; a1 += w * B1[kb]; a2 += w * B2[kb]; a3 += w * B3[kb];
+                  }
+#pragma unroll 4
+                  for (int kb = lo2 + sub; kb < hi2; kb += 8) {
+                    const double w = A[kb];
+                    a0 += w * Bc[kb]; a1 += w * B1[kb]; a2 += w * B2[kb]; a3 += w * B3[kb];
+                  }
                 }
               }
 #pragma unroll
@@ -431,6 +458,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           }
         }
       }
+      CDZ_TICK(0);
       // ---- single-lane items: SB | recursive parts of Qm1, Qml | E(i,j) ----------------------------------------------------
       {
         const int npm = nps << lgM;
@@ -506,7 +534,9 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           }
         }
       }
+      CDZ_TICK(1);
       __syncthreads();
+      CDZ_TICK(2);
       if (closed) {
         // ================= P2: Y[(a',u)][(v,c')] -- everything that carries the closing mismatch =================
         const bool v11 = maxint >= 2 && d - 4 >= mh1;  // 1x1 interior loop: inner pair (p+1, q-1)
@@ -554,6 +584,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
         }
         __syncthreads();
       }
+      CDZ_TICK(3);
       // ================= P3b: Qb[(a,x)][(y,c)] = can(x,y) sum T_i[a,x,a'] T_j[c',y,c] inner ============================
       {
         int rl0;
@@ -586,6 +617,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
         }
       }
       __syncthreads();
+      CDZ_TICK(4);
       // ================= P4: Qbs, Qm1, Qml, M2, Qm;  DD = mismatch-dressed extension of Qb(i,j) over [i-1..j+1] ==========
       const bool dress = closed && maxint >= 2;
       int rlm = 0, nlm = 0, rbm = 0, nbm = 0;
@@ -650,6 +682,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
         }
       }
       __syncthreads();
+      CDZ_TICK(5);
       // ================= P5: GI, D1, D2T = DD summed over both / the right / the left nucleotide =========================
       if (dress) {
         const int n1 = nbm << lgM, n2 = nlm << lgM, n3 = nbm << lgR;
@@ -691,10 +724,16 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           }
         }
       }
+      CDZ_TICK(6);
       // the next phase that writes this scratch (P1 of the next chunk / diagonal) is separated from these reads by the
       // barrier after P1 only for Y; P1 itself writes other arrays, so no barrier is needed here
     }
   }
+#ifdef CDZ_PHASE_TIMING
+  if (blockIdx.x == 3 && blockIdx.y == 0 && (tid == 0 || tid == 37 || tid == 300 || tid == 511) && (ka.D == 5 || ka.D == 60 || ka.D == 300))
+    printf("D=%d tid=%d coop=%lld single=%lld barwait=%lld P2P3a=%lld P3b=%lld P4=%lld P5=%lld steps=%d\n", ka.D, tid, tph[0], tph[1],
+           tph[2], tph[3], tph[4], tph[5], tph[6], dmax - dmin + 1);
+#endif
 }
 
 }  // namespace
@@ -703,7 +742,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
 // host side
 // ------------------------------------------------------------------------------------------------
 int cdz_cell_config(cdz_tables* const* ts, int B, cdz_cell_cfg* cfg) {
-  Dims dm{1, 1, 1, 6, 0, 0, 0};
+  Dims dm{1, 1, 1, 6, 0, 0, 0, 0};
   int maxpos = 1;
   for (int k = 0; k < B; ++k) {
     const cdz_tt* tt = ts[k]->tt;
@@ -745,5 +784,6 @@ void cdz_launch_cells(const Ctx* d_ctxs, int B, int nblk, int D, int nsplit, con
   ka.D = D; ka.nsplit = nsplit; ka.C = cfg->C; ka.maxpos = cfg->maxpos; ka.span = cfg->span;
   ka.dm.M = cfg->M; ka.dm.ML = cfg->ML; ka.dm.MR = cfg->MR; ka.dm.nps = cfg->nps;
   ka.dm.lgM = clog2(cfg->M); ka.dm.lgR = clog2(cfg->MR); ka.dm.lgP = clog2(cfg->nps);
+  ka.dm.pc = ka.dm.percell();
   cell_kernel<<<dim3(nblk, B), CELL_THREADS, cfg->smem, st>>>(d_ctxs, ka);
 }
