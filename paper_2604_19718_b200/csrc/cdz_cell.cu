@@ -476,11 +476,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             if (c1 >= mj.sig) continue;
             const PosMeta mp = rowm[kp], mq = colm[q - cbase];
             const int xp = cm.slot_x[sl], yp = cm.slot_y[sl];
-            int lst = -1, r = -1;
-            for (int l = 0; l < mp.nL; ++l)
-              if (ls_a[mp.loff + l] == a1 && ls_x[mp.loff + l] == xp) lst = l;
-            for (int k = 0; k < mq.nR; ++k)
-              if (rs_y[mq.roff + k] == yp && rs_c[mq.roff + k] == c1) r = k;
+            const int lst = t.lsidx[((size_t)p * MS + a1) * 4 + xp], r = t.rsidx[((size_t)q * 4 + yp) * MS + c1];
             double v = 0.0;
             if (q - p >= mh1 && lst >= 0 && r >= 0) v = b.QB[(size_t)(mp.loff + lst) * RS + mq.roff + r];
             if (maxint >= 1 && q - (p + 1) >= mh1) {

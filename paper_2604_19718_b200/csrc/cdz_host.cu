@@ -329,6 +329,8 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   t.roff = k.take<int>(n + 1);
   t.ls_a = k.take<uint8_t>(LS); t.ls_x = k.take<uint8_t>(LS);
   t.rs_y = k.take<uint8_t>(RS); t.rs_c = k.take<uint8_t>(RS);
+  t.lsidx = k.take<int8_t>(n * MS * 4);
+  t.rsidx = k.take<int8_t>(n * 4 * MS);
   t.bondpos = k.take<int>(S + 1);
   t.lspos = k.take<int>(LS);
   t.rspos = k.take<int>(RS);
@@ -397,6 +399,11 @@ static int upload(cdz_tables* T) {
     for (int r = tt->roff[i]; r < tt->roff[i + 1]; ++r) rspos[r] = i;
   }
   const int MS = tt->MS;
+  std::vector<int8_t> lsidx((size_t)n * MS * 4, -1), rsidx((size_t)n * 4 * MS, -1);
+  for (int i = 0; i < n; ++i) {
+    for (int l = tt->loff[i]; l < tt->loff[i + 1]; ++l) lsidx[((size_t)i * MS + tt->ls_a[l]) * 4 + tt->ls_x[l]] = (int8_t)(l - tt->loff[i]);
+    for (int r = tt->roff[i]; r < tt->roff[i + 1]; ++r) rsidx[((size_t)i * 4 + tt->rs_y[r]) * MS + tt->rs_c[r]] = (int8_t)(r - tt->roff[i]);
+  }
   std::vector<double> tbar((size_t)n * MS * MS, 0.0);
   for (int i = 0; i < n; ++i)
     for (int z = tt->opstart[i]; z < tt->opstart[i + 1]; ++z)
@@ -422,6 +429,8 @@ static int upload(cdz_tables* T) {
   CDZ_CUDA(up(t.ls_x, tt->ls_x.data(), tt->LS));
   CDZ_CUDA(up(t.rs_y, tt->rs_y.data(), tt->RS));
   CDZ_CUDA(up(t.rs_c, tt->rs_c.data(), tt->RS));
+  CDZ_CUDA(up(t.lsidx, lsidx.data(), lsidx.size()));
+  CDZ_CUDA(up(t.rsidx, rsidx.data(), rsidx.size()));
   CDZ_CUDA(up(t.bondpos, bondpos.data(), sizeof(int) * (tt->S + 1)));
   CDZ_CUDA(up(t.lspos, lspos.data(), sizeof(int) * tt->LS));
   CDZ_CUDA(up(t.rspos, rspos.data(), sizeof(int) * tt->RS));

@@ -66,6 +66,8 @@ struct DevTT {
   const int* loff;     // [n+1]
   const int* roff;     // [n+1]
   const uint8_t *ls_a, *ls_x, *rs_y, *rs_c;
+  const int8_t* lsidx;  // [n][MS][4]: local index of left state (a,x) at a position, -1 if absent
+  const int8_t* rsidx;  // [n][4][MS]: local index of right state (y,c)
   const int* bondpos;  // [S+1?] position of each bond index (as left bond of that position), bondpos[off[i]+a] = i
   const int* lspos;    // [LS]
   const int* rspos;    // [RS]

@@ -75,9 +75,9 @@ struct View {
     return b.EM[(size_t)(t.off[p] + a) * t.S + t.off[q + 1] + c];
   }
   __device__ double QB(int i, int j, int a, int x, int y, int c) const {  // dense view of the state-list cell
-    int l = -1, r = -1;
-    for (int k = t.loff[i]; k < t.loff[i + 1]; ++k) if (t.ls_a[k] == a && t.ls_x[k] == x) { l = k; break; }
-    for (int k = t.roff[j]; k < t.roff[j + 1]; ++k) if (t.rs_y[k] == y && t.rs_c[k] == c) { r = k; break; }
+    const int ll = t.lsidx[((size_t)i * t.MS + a) * 4 + x], rr = t.rsidx[((size_t)j * 4 + y) * t.MS + c];
+    if (ll < 0 || rr < 0) return 0.0;
+    const int l = t.loff[i] + ll, r = t.roff[j] + rr;
     if (l < 0 || r < 0) return 0.0;
     return b.QB[(size_t)l * t.RS + r];
   }
