@@ -269,7 +269,7 @@ def run_cdz(args):
     roof_block = None
     if block_ms > 0:
         ach = 2.0 * loop_mac / (block_ms * 1e-3) / 1e12
-        roof_block = {"kernel": "block_kernel (closed cells: hairpin/stack/bulge/interior<=30/multiloop closure, edge splits)",
+        roof_block = {"kernel": "cell_kernel (closed cells: hairpin/stack/bulge/interior<=30/multiloop closure, Qm1/Qml, in-block edge splits)",
                       "bound": "alu", "achieved": ach, "peak": dfma, "unit": "TFLOP/s", "frac": ach / dfma,
                       "traffic": None, "launches": block_l, "avg_launch_ms": block_ms / max(block_l, 1),
                       "algorithmic_flop_per_step": 2.0 * loop_mac,

@@ -100,6 +100,7 @@ __host__ __device__ inline Plan make_plan(int maxpos, int span, const Dims& D, i
 namespace {
 
 constexpr int CELL_THREADS = 512;
+constexpr int LG = 4, GL = 1 << LG;  // lanes that share one row item of the cooperative P1 loop
 
 struct KArgs {
   int D, nsplit, C, maxpos, span;
@@ -130,8 +131,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   const int n = t.n, MS = t.MS, MS2 = MS * MS;
   const size_t S = (size_t)t.S, RS = (size_t)t.RS;
   const int M = dm.M, ML = dm.ML, MR = dm.MR, nps = dm.nps, MM = M * M;
-  const int lgM = dm.lgM, lgR = dm.lgR, lgP = dm.lgP;
-  const int Mp = 1 << lgM, MRp = 1 << lgR, NPp = 1 << lgP;
+  const int lgM = dm.lgM, lgR = dm.lgR;
+  const int Mp = 1 << lgM, MRp = 1 << lgR;
 
   // rows i in [i0,i1), columns j in [j0,j1): bond position j+1 lies in block J
   const int i0 = t.blk_start[I], i1 = min(t.blk_start[I + 1], n);
@@ -217,6 +218,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
 
 #ifdef CDZ_PHASE_TIMING
   long long tph[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tlast = clock64();
+  long long ttyp[6] = {0, 0, 0, 0, 0, 0};
 #define CDZ_TICK(k) do { const long long now__ = clock64(); tph[k] += now__ - tlast; tlast = now__; } while (0)
 #else
 #define CDZ_TICK(k)
@@ -243,9 +245,13 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
         const int n6 = closed ? nb2 : 0;  // Z2     : bond row of i+2  x  r  < |R_q|
         const int n2 = d >= 4 ? nb2 : 0;  // X      : bond row of i+2  x  c2 < Sigma_q
         const int e9 = n9, e3 = e9 + n3, e4 = e3 + n3, e5 = e4 + n5, e6 = e5 + n6, e2 = e6 + n2;
-        const unsigned gmask = 0xFFu << (tid & 24);
-        for (int ts = tid; ts < (e2 << 3); ts += NT) {
-          const int g = ts >> 3, sub = ts & 7;
+        const unsigned gmask = ((1u << GL) - 1u) << (tid & 31 & ~(GL - 1));
+        for (int ts = tid; ts < (e2 << LG); ts += NT) {
+          const int g = ts >> LG, sub = ts & (GL - 1);
+#ifdef CDZ_PHASE_TIMING
+          const long long tr0 = clock64();
+          const int ttype = g < e9 ? 0 : g < e3 ? 1 : g < e4 ? 2 : g < e5 ? 3 : g < e6 ? 4 : 5;
+#endif
           if (g < e6) {
             // ---- decode: out[c] = add[c] + sum_{kb in [lo,hi) (+ [lo2,hi2))} wt[sg * pos(kb) + cst] A[kb] B0[c * S + kb] -------
             const double *A = nullptr, *B0 = nullptr, *wt = nullptr, *addp = nullptr;
@@ -339,18 +345,18 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
                 const double* B3 = Bc + (nc4 > 3 ? 3 * S : 0);
                 if (nc4 == 1) {
 #pragma unroll 4
-                  for (int kb = lo + sub; kb < hi; kb += 8)
+                  for (int kb = lo + sub; kb < hi; kb += GL)
                     a0 += wt[sg * (pb + bp[kb - kb0]) + cst] * A[kb] * Bc[kb];
                 } else if (nc4 == 2) {
 #pragma unroll 4
-                  for (int kb = lo + sub; kb < hi; kb += 8) {
+                  for (int kb = lo + sub; kb < hi; kb += GL) {
                     const double w = wt[sg * (pb + bp[kb - kb0]) + cst] * A[kb];
                     a0 += w * Bc[kb];
                     a1 += w * B1[kb];
                   }
                 } else {
 #pragma unroll 4
-                  for (int kb = lo + sub; kb < hi; kb += 8) {
+                  for (int kb = lo + sub; kb < hi; kb += GL) {
                     const double w = wt[sg * (pb + bp[kb - kb0]) + cst] * A[kb];
                     a0 += w * Bc[kb];
                     a1 += w * B1[kb];
@@ -364,24 +370,24 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
                 const double* B3 = Bc + (nc4 > 3 ? 3 * S : 0);
                 if (nc4 <= 2) {
 #pragma unroll 4
-                  for (int kb = lo + sub; kb < hi; kb += 8) { const double w = A[kb]; a0 += w * Bc[kb]; a1 += w * B1[kb]; }
+                  for (int kb = lo + sub; kb < hi; kb += GL) { const double w = A[kb]; a0 += w * Bc[kb]; a1 += w * B1[kb]; }
 #pragma unroll 4
-                  for (int kb = lo2 + sub; kb < hi2; kb += 8) { const double w = A[kb]; a0 += w * Bc[kb]; a1 += w * B1[kb]; }
+                  for (int kb = lo2 + sub; kb < hi2; kb += GL) { const double w = A[kb]; a0 += w * Bc[kb]; a1 += w * B1[kb]; }
                 } else {
 #pragma unroll 4
-                  for (int kb = lo + sub; kb < hi; kb += 8) {
+                  for (int kb = lo + sub; kb < hi; kb += GL) {
                     const double w = A[kb];
                     a0 += w * Bc[kb]; a1 += w * B1[kb]; a2 += w * B2[kb]; a3 += w * B3[kb];
                   }
 #pragma unroll 4
-                  for (int kb = lo2 + sub; kb < hi2; kb += 8) {
+                  for (int kb = lo2 + sub; kb < hi2; kb += GL) {
                     const double w = A[kb];
                     a0 += w * Bc[kb]; a1 += w * B1[kb]; a2 += w * B2[kb]; a3 += w * B3[kb];
                   }
                 }
               }
 #pragma unroll
-              for (int o = 1; o < 8; o <<= 1) {
+              for (int o = 1; o < GL; o <<= 1) {
                 a0 += __shfl_xor_sync(gmask, a0, o);
                 a1 += __shfl_xor_sync(gmask, a1, o);
                 a2 += __shfl_xor_sync(gmask, a2, o);
@@ -405,57 +411,70 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             for (int cc = 0; cc < mq.sig; cc += 4) {
               const int nc4 = min(4, mq.sig - cc);
               double e0 = 0.0, e1 = 0.0, e2x = 0.0, e3x = 0.0;
+              constexpr int KX = (XU + GL - 1) / GL;
+              double xv[KX][4];
+              const double hp = (closed && sub < nc4) ? t.wh[d - 1] * b.EM[(size_t)offa * S + mq.off + cc + sub] : 0.0;
+              // all loads first (the stores below go to the same array XS and would otherwise order them)
 #pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                const int u = 4 + sub + 8 * k;
-                if (u > 30) break;
+              for (int k = 0; k < KX; ++k) {
+                const int u = 4 + sub + GL * k;
                 double x0 = 0.0, x1 = 0.0, x2 = 0.0, x3 = 0.0;
-                if (hasold && u > 4) {
-                  const double* xr = xo + (u - 5) * MS2 + cc;
-                  for (int a3 = 0; a3 < Sa3; ++a3) {
-                    const double tb = Tb[a3];
-                    x0 += tb * xr[a3 * MS];
-                    if (nc4 > 1) x1 += tb * xr[a3 * MS + 1];
-                    if (nc4 > 2) x2 += tb * xr[a3 * MS + 2];
-                    if (nc4 > 3) x3 += tb * xr[a3 * MS + 3];
+                if (u <= 30) {
+                  if (hasold && u > 4) {
+                    const double* xr = xo + (u - 5) * MS2 + cc;
+                    for (int a3 = 0; a3 < Sa3; ++a3) {
+                      const double tb = Tb[a3];
+                      x0 += tb * xr[a3 * MS];
+                      if (nc4 > 1) x1 += tb * xr[a3 * MS + 1];
+                      if (nc4 > 2) x2 += tb * xr[a3 * MS + 2];
+                      if (nc4 > 3) x3 += tb * xr[a3 * MS + 3];
+                    }
+                  }
+                  const int cp = j + 3 - u;
+                  if (cp - (i + 2) - 3 >= mh1) {
+                    const PosMeta mc = colm[cp - cbase];
+                    const double* er = em + (size_t)cc * S + mc.off;
+                    for (int u2 = 0; u2 < mc.sig; ++u2) {
+                      const double gv = gi[mc.off + u2];
+                      x0 += gv * er[u2];
+                      if (nc4 > 1) x1 += gv * er[S + u2];
+                      if (nc4 > 2) x2 += gv * er[2 * S + u2];
+                      if (nc4 > 3) x3 += gv * er[3 * S + u2];
+                    }
+                  }
+                  if (u <= maxint) {
+                    const double w = cm.win[u];
+                    e0 += w * x0; e1 += w * x1; e2x += w * x2; e3x += w * x3;
                   }
                 }
-                const int cp = j + 3 - u;
-                if (cp - (i + 2) - 3 >= mh1) {
-                  const PosMeta mc = colm[cp - cbase];
-                  const double* er = em + (size_t)cc * S + mc.off;
-                  for (int u2 = 0; u2 < mc.sig; ++u2) {
-                    const double gv = gi[mc.off + u2];
-                    x0 += gv * er[u2];
-                    if (nc4 > 1) x1 += gv * er[S + u2];
-                    if (nc4 > 2) x2 += gv * er[2 * S + u2];
-                    if (nc4 > 3) x3 += gv * er[3 * S + u2];
-                  }
-                }
-                double* xw = xn + (u - 4) * MS2 + cc;
-                xw[0] = x0;
-                if (nc4 > 1) xw[1] = x1;
-                if (nc4 > 2) xw[2] = x2;
-                if (nc4 > 3) xw[3] = x3;
-                if (u <= maxint) {
-                  const double w = cm.win[u];
-                  e0 += w * x0; e1 += w * x1; e2x += w * x2; e3x += w * x3;
+                xv[k][0] = x0; xv[k][1] = x1; xv[k][2] = x2; xv[k][3] = x3;
+              }
+#pragma unroll
+              for (int k = 0; k < KX; ++k) {
+                const int u = 4 + sub + GL * k;
+                if (u <= 30) {
+                  double* xw = xn + (u - 4) * MS2 + cc;
+                  xw[0] = xv[k][0];
+                  if (nc4 > 1) xw[1] = xv[k][1];
+                  if (nc4 > 2) xw[2] = xv[k][2];
+                  if (nc4 > 3) xw[3] = xv[k][3];
                 }
               }
 #pragma unroll
-              for (int o = 1; o < 8; o <<= 1) {
+              for (int o = 1; o < GL; o <<= 1) {
                 e0 += __shfl_xor_sync(gmask, e0, o);
                 e1 += __shfl_xor_sync(gmask, e1, o);
                 e2x += __shfl_xor_sync(gmask, e2x, o);
                 e3x += __shfl_xor_sync(gmask, e3x, o);
               }
               if (sub < nc4) {
-                double v = sub == 0 ? e0 : sub == 1 ? e1 : sub == 2 ? e2x : e3x;
-                if (closed) v += t.wh[d - 1] * b.EM[(size_t)offa * S + mq.off + cc + sub];
-                out[cc + sub] = v;
+                out[cc + sub] = hp + (sub == 0 ? e0 : sub == 1 ? e1 : sub == 2 ? e2x : e3x);
               }
             }
           }
+#ifdef CDZ_PHASE_TIMING
+          ttyp[ttype] += clock64() - tr0;
+#endif
         }
       }
       CDZ_TICK(0);
@@ -558,8 +577,10 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
         }
         __syncthreads();
         // ================= P3a: inner[slot][a'][c'] ======================================================================
-        for (int it = tid; it < (nb1 << (lgM + lgP)); it += NT) {
-          const int c1 = it & (Mp - 1), sl = (it >> lgM) & (NPp - 1), rr = rb1 + (it >> (lgM + lgP));
+        const int npm3 = nps << lgM;
+        for (int it0 = tid; it0 < nb1 * npm3; it0 += NT) {
+          const int rq = it0 / npm3, it = it0 - rq * npm3;
+          const int c1 = it & (Mp - 1), sl = it >> lgM, rr = rb1 + rq;
           const int kp = rbpos[rr], a1 = rr - crow[kp];
           const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
           const PosMeta mj = colm[j - cbase];
@@ -727,8 +748,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   }
 #ifdef CDZ_PHASE_TIMING
   if (blockIdx.x == 3 && blockIdx.y == 0 && (tid == 0 || tid == 37 || tid == 300 || tid == 511) && (ka.D == 5 || ka.D == 60 || ka.D == 300))
-    printf("D=%d tid=%d coop=%lld single=%lld barwait=%lld P2P3a=%lld P3b=%lld P4=%lld P5=%lld steps=%d\n", ka.D, tid, tph[0], tph[1],
-           tph[2], tph[3], tph[4], tph[5], tph[6], dmax - dmin + 1);
+    printf("D=%d tid=%d coop=%lld single=%lld barwait=%lld P2P3a=%lld P3b=%lld P4=%lld P5=%lld steps=%d | M2=%lld Bl=%lld Br=%lld Z1=%lld Z2=%lld X=%lld\n", ka.D, tid, tph[0], tph[1],
+           tph[2], tph[3], tph[4], tph[5], tph[6], dmax - dmin + 1, ttyp[0], ttyp[1], ttyp[2], ttyp[3], ttyp[4], ttyp[5]);
 #endif
 }
 
