@@ -98,6 +98,22 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def reduce_max(value: float, device="cpu") -> float:
+    """Max over ranks of a per-rank time (the only collective besides the barrier: replicas share no data)."""
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_rank: float, world: int, ms_max: float) -> float:
+    """Replicas only: every rank processes the same units, the job takes the slowest rank's time."""
+    return world * units_per_rank / (ms_max * 1e-3)
+
+
 def oracle_sample(cfg: int, L_sample: int):
     """Time the CPU oracle's inside pass, as it stands, on the first L_sample residues of the workload."""
     from oracle import oracle as O
@@ -209,11 +225,8 @@ def run_cdz(args):
     info = tab.info()
     clk = clocks.stop() if rank == 0 else None
     tab.set_profiling(False)
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
-    value = world * units / (ms_step * 1e-3)
+    ms_step = reduce_max(ms_total, "cuda") / args.steps
+    value = whole_job_value(units, world, ms_step)
 
     # ---- end to end through the C ABI with host buffers --------------------------------------------------------------
     seq_h = torch.empty((max(J, 1), n), dtype=torch.uint8).pin_memory()
@@ -229,10 +242,7 @@ def run_cdz(args):
         lz_e2e = tab.run_host(J, d.sample_seed, seq_h if J else None, pair_h if J else None, stream)
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
-    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * units / float(t.item())
+    e2e_value = whole_job_value(units, world, 1e3 * reduce_max(e2e_s, "cuda"))
 
     if rank != 0:
         if world > 1:
