@@ -128,3 +128,83 @@ def test_errors(B):
     tg, lz = B.inside(m, tt)
     with pytest.raises(B.CdzError):
         tg.cell(9, 0, 0)
+
+
+# ---- BASELINE.json full sizes: what the oracle can still reach, plus properties that hold at any size -------------------
+def _prefix_chain(B, O, cfg, L_full, L_pre, rtol=1e-11):
+    """log Qext(j)[c] depends on positions <= j only, so the full-size GPU run restricted to a prefix must equal an
+    independent GPU run on that prefix, which in turn is checked element-wise against the oracle (last row)."""
+    m = I.nn_model()
+    d = I.design(cfg, 0, L_full)
+    dp = I.design(cfg, 0, L_pre)
+    assert d.aa.startswith(dp.aa)
+    tfull, lz_full = B.inside(B.Model(m), B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw))
+    to, tpre, lz_pre = both(B, O, m, dp.aa, dp.kind, dp.codon_logw, dp.pair_logw)
+    assert abs(lz_pre - to.logZ) <= LOGZ_RTOL * abs(to.logZ)
+    sig, _, _ = B.TensorTrain.build(dp.aa, dp.kind, dp.codon_logw, dp.pair_logw).describe()
+    for j in sorted({0, dp.n // 3, dp.n // 2, dp.n - 2}):  # (the last bond of the prefix run is summed differently)
+        for c in range(sig[j + 1]):
+            ref = to.logqext(j, c)
+            assert abs(tpre.logqext(j, c) - ref) <= rtol * max(1.0, abs(ref))
+            assert abs(tfull.logqext(j, c) - ref) <= 1e-9 * max(1.0, abs(ref)), (j, c)
+    return tfull, lz_full, d
+
+
+def test_config4_full_size_prefix_and_samples(B, O):
+    """configs[3]: 5000 aa (15000 nt), the launch configuration bench.py times: prefix chain to the oracle, every one
+    of the 100 samples is a valid state with a finite Boltzmann weight, the pass is deterministic."""
+    tfull, lz, d = _prefix_chain(B, O, 4, 5000, 60)
+    assert np.isfinite(lz) and 1.2 * d.n < lz < 1.5 * d.n  # ~1.33 nat / nt with this model (SURVEY c-12)
+    info = tfull.info()
+    assert info["n"] == 15000 and info["n_rescales"] >= 8
+    seq, pair = tfull.sample(100, d.sample_seed)
+    seq, pair = seq.cpu().numpy(), pair.cpu().numpy()
+    tto = O.TT.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
+    m = I.nn_model()
+    for k in range(0, 100, 10):
+        assert (seq[k] < 4).all()
+        assert np.isfinite(O.logweight(m, tto, seq[k], pair[k]))
+    tfull.rerun()
+    assert tfull.logz() == lz
+
+
+def test_config2_full_size_prefix(B, O):
+    """configs[1]: 300 aa, codon-pair tensor train (bond dimension up to 6)."""
+    _prefix_chain(B, O, 2, 300, 30)
+
+
+def test_config3_size_runs_in_fp64(B, O):
+    """configs[2] (1000 aa, codon-pair TT) is run through the fp64 path: prefix chain + finite log Z."""
+    tfull, lz, d = _prefix_chain(B, O, 3, 1000, 30)
+    assert np.isfinite(lz)
+
+
+def test_batch_equals_single_and_oracle(B, O):
+    """configs[4]: independent designs advanced in the same launches give exactly the single-design results."""
+    m = I.nn_model()
+    mg = B.Model(m)
+    ds = [I.design(5, item, 24) for item in range(6)]
+    tts = [B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw) for d in ds]
+    tabs, lzs = B.inside_batch(mg, tts)
+    for d, tt, tab, lz in zip(ds, tts, tabs, lzs):
+        t1, lz1 = B.inside(mg, tt)
+        assert lz == lz1
+        lo = O.inside(m, O.TT.build(d.aa, d.kind, d.codon_logw, d.pair_logw)).logZ
+        assert abs(lz - lo) <= LOGZ_RTOL * abs(lo)
+        s1, p1 = t1.sample(32, d.sample_seed)
+        s2, p2 = tab.sample(32, d.sample_seed)
+        assert (s1 == s2).all() and (p1 == p2).all()
+
+
+def test_config5_full_batch(B, O):
+    """64 x 150 aa in one batched pass: equal to the designs run one at a time; item 0's prefix checked against the oracle."""
+    m = I.nn_model()
+    mg = B.Model(m)
+    ds = [I.design(5, item) for item in range(64)]
+    tts = [B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw) for d in ds]
+    tabs, lzs = B.inside_batch(mg, tts)
+    assert all(np.isfinite(v) for v in lzs)
+    for item in (0, 17, 63):
+        t1, lz1 = B.inside(mg, tts[item])
+        assert lzs[item] == lz1
+    _prefix_chain(B, O, 5, 150, 20)
