@@ -275,14 +275,21 @@ def run_cdz(args):
                                     "MEASURED_PEAKS.json has no fp64 entry; rule-derived alternative = bf16_tflops x "
                                     "45/2250 = %s" % (None if bf16 is None else round(bf16 * 45.0 / 2250.0, 2)),
                      "share_of_step": gemm_ms / ms_step}
+    # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch near block diagonal D = 100 of this workload, from the
+    # single-pass ncu capture summarised in profiles/r1o_launches.md (only meaningful for config 4 at full length)
+    ncu_traffic = {"gemm": 1880976128 + 19368960, "block": 617259776 + 278033664} if (cfg == 4 and not args.L) else {}
+    if roof_gemm:
+        roof_gemm["traffic"] = ncu_traffic.get("gemm")
+        roof_gemm["traffic_note"] = "one launch at D~100 (574 CTAs, 0.61 ms): no operand reuse across a block diagonal"
     block_ms, block_l = prof_ms.get("block", 0.0), prof_launches.get("block", 0)
     roof_block = None
     if block_ms > 0:
         ach = 2.0 * loop_mac / (block_ms * 1e-3) / 1e12
         roof_block = {"kernel": "cell_kernel (closed cells: hairpin/stack/bulge/interior<=30/multiloop closure, Qm1/Qml, in-block edge splits)",
                       "bound": "alu", "achieved": ach, "peak": dfma, "unit": "TFLOP/s", "frac": ach / dfma,
-                      "traffic": None, "launches": block_l, "avg_launch_ms": block_ms / max(block_l, 1),
+                      "traffic": ncu_traffic.get("block"), "launches": block_l, "avg_launch_ms": block_ms / max(block_l, 1),
                       "algorithmic_flop_per_step": 2.0 * loop_mac,
+                      "note": "latency-bound, not ALU-bound: ~35 us per in-block anti-diagonal x 2n-step chain (DESIGN.md 8.1)",
                       "peak_source": "in-run register-resident fp64 FMA loop (cdz_measure_peak)",
                       "share_of_step": block_ms / ms_step}
     roofline = roof_block if dominant == "block" and roof_block else (roof_gemm or roof_block)
