@@ -26,7 +26,7 @@
 
 namespace {
 
-struct PosMeta { int off, sig, loff, nL, roff, nR, ops, nops; };  // 32 bytes, one per position of a window
+struct PosMeta { int off, sig, loff, nL, roff, nR, ops, nuc; };  // 32 bytes per position of a window; nuc = bit mask of the nucleotides possible there
 
 constexpr int XU = 27;       // interior totals u = l1 + l2 = 4..30 with l1, l2 >= 2
 constexpr int ROWPAD = 34;   // row window  [i0-1, i1+ROWPAD-2]
@@ -110,6 +110,7 @@ struct KArgs {
 __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, KArgs ka) {
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ CModel cm;
+  __shared__ int pmx[16];  // nucleotide mask of position i -> mask of the nucleotides at j that can pair with one of them
   const Ctx& cx = ctxs[blockIdx.y];
   const DevTT& t = cx.tt;
   const DevTab& b = cx.tab;
@@ -156,9 +157,11 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
     if (p < n) {
       m.loff = t.loff[p]; m.nL = t.loff[p + 1] - m.loff;
       m.roff = t.roff[p]; m.nR = t.roff[p + 1] - m.roff;
-      m.ops = t.opstart[p]; m.nops = t.opstart[p + 1] - m.ops;
+      m.ops = t.opstart[p];
+      m.nuc = 0;
+      for (int l = 0; l < m.nL; ++l) m.nuc |= 1 << t.ls_x[m.loff + l];
     } else {
-      m.loff = t.loff[n]; m.nL = 0; m.roff = t.roff[n]; m.nR = 0; m.ops = t.opstart[n]; m.nops = 0;
+      m.loff = t.loff[n]; m.nL = 0; m.roff = t.roff[n]; m.nR = 0; m.ops = t.opstart[n]; m.nuc = 0;
     }
     return m;
   };
@@ -171,6 +174,14 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   for (int k = tid; k < ntl * ML * M; k += NT) TLs[k] = 0.0;
   for (int k = tid; k < ntr * M * MR; k += NT) TRs[k] = 0.0;
   __syncthreads();
+  if (tid < 16) {
+    int pm = 0;
+    for (int x = 0; x < 4; ++x)
+      if (tid >> x & 1)
+        for (int y = 0; y < 4; ++y)
+          if (cm.pslot[x * 4 + y] >= 0) pm |= 1 << y;
+    pmx[tid] = pm;
+  }
   if (tid == 0) {
     int acc = 0;
     for (int k = 0; k < nrp; ++k) { crow[k] = acc; acc += rowm[k].sig; }
@@ -287,7 +298,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
               const PosMeta mj = colm[j - cbase];
               const int offp = rowm[kp].off;
               const int lmax = min(maxint, q - mh1 - p);
-              ncol = mj.sig;
+              ncol = (pmx[rowm[kp - 1].nuc] & mj.nuc) ? mj.sig : 0;  // nothing to do when no nucleotides of i and j can pair
               wt = cm.wbu;
               if (left) {
                 // multiloop closure + left bulges l1 = 2..lmax: E(p,k-1)[a1,s] Qbs(k,q)[s,c1], k = p + l1
@@ -313,7 +324,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
               const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
               const PosMeta mq = colm[q - cbase];
               const int lmax = min(maxint - 1, q - mh1 - (p + 1));
-              ncol = mq.sig;
+              ncol = (pmx[rowm[kp - 1].nuc] & colm[j - cbase].nuc) ? mq.sig : 0;
               A = b.D1 + (size_t)(rowm[kp].loff + lst) * S;
               B0 = b.EMT + (size_t)mq.off * S;
               if (lmax >= 2) { lo = colm[q - lmax + 2 - cbase].off; hi = mq.off + mq.sig; }
@@ -325,7 +336,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
               const int i = rbase + kp - 2, p = i + 1, j = i + d, q = j - 1;
               const PosMeta mq = colm[q - cbase];
               const int lmax = min(maxint - 1, (q - 1) - mh1 - p);
-              ncol = mq.nR;
+              ncol = (pmx[rowm[kp - 2].nuc] & colm[j - cbase].nuc) ? mq.nR : 0;
               A = b.EM + (size_t)(rowm[kp].off + a2) * S;
               B0 = b.D2T + (size_t)mq.roff * S;
               if (lmax >= 2) { lo = rowm[kp].off; hi = rowm[kp + lmax - 2].off + rowm[kp + lmax - 2].sig; }
@@ -492,7 +503,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             const int kp = rbpos[rr], a1 = rr - crow[kp];
             const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
             const PosMeta mj = colm[j - cbase];
-            if (c1 >= mj.sig) continue;
+            if (c1 >= mj.sig || !(pmx[rowm[kp - 1].nuc] & mj.nuc)) continue;
             const PosMeta mp = rowm[kp], mq = colm[q - cbase];
             const int xp = cm.slot_x[sl], yp = cm.slot_y[sl];
             const int lst = t.lsidx[((size_t)p * MS + a1) * 4 + xp], r = t.rsidx[((size_t)q * 4 + yp) * MS + c1];
@@ -559,7 +570,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           const int r = it & (MRp - 1), ll = rl1 + (it >> lgR), kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
           const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
           const PosMeta mq = colm[q - cbase];
-          if (r >= mq.nR) continue;
+          if (r >= mq.nR || !(pmx[rowm[kp - 1].nuc] & colm[j - cbase].nuc)) continue;
           const Scr sc = scr_of(scrb, dm, i - clo);
           const int Sp1 = rowm[kp + 1].sig, Sq = mq.sig;
           const double* TLp = TLs + ((p - tlbase) * ML + lst) * M;
@@ -584,7 +595,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           const int kp = rbpos[rr], a1 = rr - crow[kp];
           const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
           const PosMeta mj = colm[j - cbase];
-          if (c1 >= mj.sig || sl >= nps) continue;
+          if (c1 >= mj.sig || !(pmx[rowm[kp - 1].nuc] & mj.nuc)) continue;
           const PosMeta mp = rowm[kp], mq = colm[q - cbase];
           const Scr sc = scr_of(scrb, dm, i - clo);
           const int P = cm.ptype[cm.slot_x[sl] * 4 + cm.slot_y[sl]];
