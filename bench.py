@@ -326,6 +326,78 @@ def run_cdz(args):
         dist.destroy_process_group()
 
 
+def run_batch(args):
+    """configs[4]: B independent 150-aa designs (distinct seeds) advanced together by cdz_inside_batch, 256 samples each.
+    Secondary measurement (small-design throughput); the default bench line is the 5000-aa design."""
+    import torch
+
+    from paper_2604_19718_b200 import binding as B
+    from paper_2604_19718_b200 import build
+    from paper_2604_19718_b200 import inputs as I
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the library has no CPU fallback)")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    build.build()
+    nb = args.batch
+    J = SAMPLES[5] if args.samples is None else args.samples
+    ds = [I.design(5, item, args.L) for item in range(nb)]
+    model = B.Model(I.nn_model())
+    tts = [B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw) for d in ds]
+    tabs, lzs = B.inside_batch(model, tts)
+    n = ds[0].n
+    ncc, nloop = counts(n)
+    units = nb * (ncc + nloop)
+    stream = torch.cuda.current_stream()
+    seq = torch.empty((nb, max(J, 1), n), dtype=torch.uint8, device="cuda")
+    pair = torch.empty((nb, max(J, 1), n), dtype=torch.int32, device="cuda")
+
+    side = [torch.cuda.Stream() for _ in range(min(16, nb))]  # the designs' tracebacks are independent: run them concurrently
+
+    def step():
+        B.inside_rerun_batch(tabs, stream)
+        if J > 0:
+            done = torch.cuda.Event()
+            done.record(stream)
+            for k, (tab, d) in enumerate(zip(tabs, ds)):
+                st = side[k % len(side)]
+                st.wait_event(done)
+                B._check(B.lib().cdz_sample(tab.h, J, d.sample_seed, B.C.c_void_p(seq[k].data_ptr()),
+                                            B.C.c_void_p(pair[k].data_ptr()), B._stream_ptr(st)))
+            for st in side:
+                stream.wait_stream(st)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    clocks = ClockSampler(0)
+    clocks.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    ev[0].record(stream)
+    for _ in range(args.steps):
+        B.inside_rerun_batch(tabs, stream)
+    ev[1].record(stream)
+    for _ in range(args.steps):
+        step()
+    ev[2].record(stream)
+    torch.cuda.synchronize()
+    inside_ms = ev[0].elapsed_time(ev[1]) / args.steps
+    ms_step = ev[1].elapsed_time(ev[2]) / args.steps
+    clk = clocks.stop()
+    lz2 = [t.logz() for t in tabs]
+    out = {
+        "metric": METRIC, "value": units / (ms_step * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"configs[4]: batch of {nb} independent {n // 3}-aa proteins ({n} nt), codon-pair TT, fp64 inside pass "
+                               f"+ {J} samples each, one batched launch sequence", "batch": nb, "n_nt": n, "samples_per_step": nb * J,
+                   "l2": "tables of the batch smaller than L2 at small B: warm-cache number"},
+        "inside_ms": inside_ms, "designs_per_s": nb / (ms_step * 1e-3), "logZ_first": lzs[0],
+        "deterministic": lz2 == lzs, "clocks": clk,
+    }
+    print(json.dumps(out), flush=True)
+
+
 def info_ms2(sigma) -> int:
     ms = max(sigma)
     return ms * ms
@@ -342,9 +414,12 @@ def main():
     ap.add_argument("--samples", type=int, default=None)
     ap.add_argument("--oracle-L", type=int, default=None, dest="oracle_L")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--batch", type=int, default=0, help="configs[4]: number of independent 150-aa designs advanced together")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.batch > 0:
+        run_batch(args)
     else:
         run_cdz(args)
 
