@@ -145,27 +145,100 @@ __device__ __forceinline__ double loop_factor(const View& V, int P, int l1, int 
   if (l1 == 0 || l2 == 0) return m.wbu[l1 + l2] * (l1 + l2 == 1 ? m.wst[P][V.pt(xp, yp)] : 1.0);
   return m.win[l1 + l2] * m.wtm[P][L.u][R.u] * m.wtm[V.pt(yp, xp)][R.up][L.up];
 }
-// total weight of inner pair (k,l) for closing (i,j,x,y) with a' = ap, c' = cp (sequential, one lane)
+// total weight of inner pair (k,l) for closing (i,j,x,y) with a' = ap, c' = cp (sequential, one lane).
+// Same quantity as the explicit sum over side operators and inner nucleotides (the oracle's level A), evaluated from the
+// pre-contracted tables the inside pass keeps: Qbs for bulges >= 2, the
+// mismatch-dressed extensions DD / D1 / D2T / GI of Qb(k,l) for interior loops.
 __device__ double iloop_total(const View& V, int i, int j, int k, int l, int P, int ap, int cp) {
-  const int l1 = k - i - 1, l2 = j - l - 1;
-  const int nl = left_count(V.t, i, k), nr = right_count(V.t, j, l);
+  const DevTT& t = V.t;
+  const DevTab& b = V.b;
+  const CModel& m = V.m;
+  const int l1 = k - i - 1, l2 = j - l - 1, MS = t.MS;
+  const size_t S = (size_t)t.S, RS = (size_t)t.RS;
+  if (l1 == 0 && l2 == 0) {
+    double tot = 0.0;
+    for (int sl = 0; sl < m.nps; ++sl) {
+      const int xp = m.slot_x[sl], yp = m.slot_y[sl];
+      tot += m.wst[P][V.pt(xp, yp)] * V.QB(k, l, ap, xp, yp, cp);
+    }
+    return tot;
+  }
+  if (l2 == 0 || l1 == 0) {
+    const int len = l1 + l2;
+    if (len >= 2) {
+      double tot = 0.0;
+      if (l2 == 0) {
+        for (int s = 0; s < t.sig[k]; ++s) tot += V.E(i + 1, k - 1, ap, s) * b.QBS[(size_t)(t.off[k] + s) * S + t.off[l + 1] + cp];
+      } else {
+        for (int u = 0; u < t.sig[l + 1]; ++u) tot += b.QBS[(size_t)(t.off[k] + ap) * S + t.off[l + 1] + u] * V.E(l + 1, j - 1, u, cp);
+      }
+      return m.wbu[len] * tot;
+    }
+    // size-1 bulge: the stack term keeps the identity of the inner pair
+    double tot = 0.0;
+    for (int sl = 0; sl < m.nps; ++sl) {
+      const int xp = m.slot_x[sl], yp = m.slot_y[sl];
+      double q = 0.0;
+      if (l2 == 0) {
+        for (int s = 0; s < t.sig[k]; ++s) q += t.Tbar[((size_t)(i + 1) * MS + ap) * MS + s] * V.QB(k, l, s, xp, yp, cp);
+      } else {
+        for (int u = 0; u < t.sig[l + 1]; ++u) q += V.QB(k, l, ap, xp, yp, u) * t.Tbar[((size_t)(j - 1) * MS + u) * MS + cp];
+      }
+      tot += m.wst[P][V.pt(xp, yp)] * q;
+    }
+    return m.wbu[1] * tot;
+  }
+  // interior loops: mismatch at the closing pair from the operators at i+1 / j-1, the inner pair's mismatch is in the tables
+  const int pl = k - 1, pr = l + 1;  // positions dressed onto Qb(k,l)
   double tot = 0.0;
-  for (int la = 0; la < nl; ++la) {
-    const SideL L = left_side(V, i, k, ap, la);
-    if (L.w == 0.0) continue;
-    for (int ra = 0; ra < nr; ++ra) {
-      const SideL R = right_side(V, j, l, cp, ra);
-      if (R.w == 0.0) continue;
-      for (int xy = 0; xy < 16; ++xy) {
-        const int xp = xy >> 2, yp = xy & 3;
-        if (!V.can(xp, yp)) continue;
-        const double q = V.QB(k, l, L.s, xp, yp, R.s);
-        if (q == 0.0) continue;
-        tot += loop_factor(V, P, l1, l2, xp, yp, L, R) * L.w * R.w * q;
+  if (l1 == 1 && l2 == 1) {
+    for (int lst = t.loff[pl]; lst < t.loff[pl + 1]; ++lst) {
+      if (t.ls_a[lst] != ap) continue;
+      for (int r = t.roff[pr]; r < t.roff[pr + 1]; ++r)
+        if (t.rs_c[r] == cp) tot += m.wtm[P][t.ls_x[lst]][t.rs_y[r]] * b.DD[(size_t)lst * RS + r];
+    }
+  } else if (l1 == 1) {
+    for (int lst = t.loff[pl]; lst < t.loff[pl + 1]; ++lst) {
+      if (t.ls_a[lst] != ap) continue;
+      const double* d1 = b.D1 + (size_t)lst * S + t.off[l + 2];
+      for (int w = t.opstart[j - 1]; w < t.opstart[j]; ++w) {
+        if (t.op_c[w] != cp) continue;
+        double s = 0.0;
+        for (int t2 = 0; t2 < t.sig[l + 2]; ++t2) s += d1[t2] * V.E(l + 2, j - 2, t2, t.op_a[w]);
+        tot += t.op_x[w] * m.wtm[P][t.ls_x[lst]][t.op_b[w]] * s;
+      }
+    }
+  } else if (l2 == 1) {
+    for (int r = t.roff[pr]; r < t.roff[pr + 1]; ++r) {
+      if (t.rs_c[r] != cp) continue;
+      const double* d2 = b.D2T + (size_t)r * S + t.off[k - 1];
+      for (int z = t.opstart[i + 1]; z < t.opstart[i + 2]; ++z) {
+        if (t.op_a[z] != ap) continue;
+        double s = 0.0;
+        for (int s2 = 0; s2 < t.sig[k - 1]; ++s2) s += V.E(i + 2, k - 2, t.op_c[z], s2) * d2[s2];
+        tot += t.op_x[z] * m.wtm[P][t.op_b[z]][t.rs_y[r]] * s;
+      }
+    }
+  } else {
+    const double* gi = b.GI + (size_t)t.off[k - 1] * S + t.off[l + 2];
+    const int Sk = t.sig[k - 1], Sl = t.sig[l + 2];
+    for (int z = t.opstart[i + 1]; z < t.opstart[i + 2]; ++z) {
+      if (t.op_a[z] != ap) continue;
+      for (int w = t.opstart[j - 1]; w < t.opstart[j]; ++w) {
+        if (t.op_c[w] != cp) continue;
+        double s = 0.0;
+        for (int s2 = 0; s2 < Sk; ++s2) {
+          const double el = V.E(i + 2, k - 2, t.op_c[z], s2);
+          if (el == 0.0) continue;
+          double r2 = 0.0;
+          for (int t2 = 0; t2 < Sl; ++t2) r2 += gi[(size_t)s2 * S + t2] * V.E(l + 2, j - 2, t2, t.op_a[w]);
+          s += el * r2;
+        }
+        tot += t.op_x[z] * t.op_x[w] * m.wtm[P][t.op_b[z]][t.op_b[w]] * s;
       }
     }
   }
-  return tot;
+  return m.win[l1 + l2] * tot;
 }
 
 __global__ void __launch_bounds__(128) sample_kernel(const Ctx* ctxp, int J, uint64_t seed, uint8_t* seq_out,
