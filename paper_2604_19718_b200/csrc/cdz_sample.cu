@@ -459,19 +459,45 @@ __global__ void __launch_bounds__(128) sample_kernel(const Ctx* ctxp, int J, uin
       const int base2 = base1 + n1;
       const int kb0 = t.off[i + 2], kb1 = t.off[j];  // bonds of positions k = i+2 .. j-1
       const int nml = kb1 > kb0 ? kb1 - kb0 : 0;
-      if (!done && nml > 0)
-        done = scan_segment(lane, pk, base2, npair * nml, [&](int idx) {
+      auto mlw = [&](int idx) {
+        int ap, cp;
+        const double w0 = zw(idx / nml, ap, cp);
+        if (w0 == 0.0) return 0.0;
+        const int kb = kb0 + idx % nml;
+        return w0 * cm.wac * b.QM[(size_t)(t.off[p] + ap) * S + kb] * b.QM1T[(size_t)(t.off[q + 1] + cp) * S + kb];
+      };
+      // The segment's total is known in closed form (w_a w_c M2(p,q), stored by the inside pass): when the threshold lies
+      // clearly beyond it, the O(d) scan over split points is skipped; within 1e-9 of its end it is scanned in order.
+      bool skipped2 = false;
+      double run2 = 0.0;
+      int last2 = -1;
+      if (!done && nml > 0) {
+        const double tot2 = warp_total(lane, npair, [&](int pz) {
           int ap, cp;
-          const double w0 = zw(idx / nml, ap, cp);
-          if (w0 == 0.0) return 0.0;
-          const int kb = kb0 + idx % nml;
-          return w0 * cm.wac * b.QM[(size_t)(t.off[p] + ap) * S + kb] * b.QM1T[(size_t)(t.off[q + 1] + cp) * S + kb];
+          const double w0 = zw(pz, ap, cp);
+          return w0 == 0.0 ? 0.0 : w0 * cm.wac * b.M2[(size_t)(t.off[p] + ap) * S + t.off[q + 1] + cp];
         });
+        if (pk.thr > (pk.run + tot2) * (1.0 + 1e-9)) {
+          skipped2 = true;
+          run2 = pk.run;
+          last2 = pk.last;
+          pk.run += tot2;
+          if (tot2 > 0.0) pk.last = base2 + npair * nml - 1;
+        } else {
+          done = scan_segment(lane, pk, base2, npair * nml, mlw);
+        }
+      }
       // segment 3: one inner pair with l1 + l2 >= 1, term outer, (z_i,z_j) inner
       const int base3 = base2 + npair * nml;
       if (!done && nterm > 1)
         done = scan_segment(lane, pk, base3, (nterm - 1) * npair,
                             [&](int idx) { return loopw(1 + idx / npair, idx % npair); });
+      if (pk.hit < 0 && skipped2 && pk.last == base2 + npair * nml - 1) {
+        // rounding left the threshold beyond every alternative and the last positive one is a split point: find it
+        pk.run = run2;
+        pk.last = last2;
+        scan_segment(lane, pk, base2, npair * nml, mlw);
+      }
       const int pick = pk.hit >= 0 ? pk.hit : pk.last;
       int ap, cp;
       if (pick < npair) {
