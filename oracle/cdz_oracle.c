@@ -446,6 +446,7 @@ struct orc_tables {
   real** qext; /* qext[j+1][c], qext[0] = [1] */
   real wst[6][6], wtm[6][4][4], wbu[31], win[31], wa, wb, wc;
   double beta;
+  int forbid_i, forbid_j; /* pair excluded from every structure (-1: none); used by orc_marginals */
 };
 
 #define SG(t, i) ((t)->sig[i])
@@ -481,6 +482,7 @@ static void compute_qb(orc_tables* t, int i, int j) {
   int Si = SG(t, i), Sj1 = SG(t, j + 1);
   real* qb = t->qb[(size_t)i * n + j];
   if (d < m->min_hairpin + 1) return;
+  if (i == t->forbid_i && j == t->forbid_j) return; /* restricted ensemble without the pair (i,j) */
   int Sa = SG(t, i + 1), Sc = SG(t, j); /* a' in Sigma_{i+1}, c' in Sigma_j */
   /* inner[x][y][a'][c'] */
   real* inner = cell_alloc((size_t)16 * Sa * Sc);
@@ -686,10 +688,13 @@ static void compute_cell(orc_tables* t, int i, int j) {
   for (int k = 0; k < Si * Sj1; ++k) qm[k] = qml[k] + m2[k];
 }
 
-int orc_inside(const orc_model* m, const orc_tt* tt_in, int nthreads, orc_tables** out, double* logZ) {
+static int inside_impl(const orc_model* m, const orc_tt* tt_in, int nthreads, int forbid_i, int forbid_j, orc_tables** out,
+                       double* logZ) {
   int n = tt_in->n;
   orc_tables* t = (orc_tables*)calloc(1, sizeof(orc_tables));
   t->n = n;
+  t->forbid_i = forbid_i;
+  t->forbid_j = forbid_j;
   t->model = *m;
   /* private TT copy */
   t->tt = (orc_tt*)calloc(1, sizeof(orc_tt));
@@ -793,6 +798,10 @@ int orc_inside(const orc_model* m, const orc_tt* tt_in, int nthreads, orc_tables
   if (logZ) *logZ = (double)logl(Z);
   if (out) *out = t; else orc_tables_free(t);
   return 0;
+}
+
+int orc_inside(const orc_model* m, const orc_tt* tt_in, int nthreads, orc_tables** out, double* logZ) {
+  return inside_impl(m, tt_in, nthreads, -1, -1, out, logZ);
 }
 
 void orc_tables_free(orc_tables* t) {
@@ -1269,7 +1278,67 @@ int orc_sample(const orc_tables* t, int J, uint64_t seed, uint8_t* seq, int32_t*
   return 0;
 }
 
+/* Marginals by their definitions as constrained sums (eqs 2.5-2.7, lines 85-96), each ratio taken from a full inside
+ * pass over a restricted ensemble -- O(n^2) passes, for small designs only (the fast way is an outside pass; this is the
+ * definition written out):
+ *   P(i.j)        = 1 - Z[pair (i,j) forbidden] / Z      (a structure either contains the pair or it does not)
+ *   P(phi_m = b)  = Z[operators at m restricted to nucleotide b] / Z
+ *   p_k(codon)    = Z[operators at 3k, 3k+1, 3k+2 restricted to the codon's three nucleotides] / Z
+ * bpp: upper triangle P(i.j), diagonal P(i unpaired) = 1 - sum_j P(i.j). */
+static double restricted_logz(const orc_tables* t, int npos, const int* pos, const int* nuc) {
+  const orc_tt* src = t->tt;
+  int n = src->n;
+  orc_tt r;
+  r.n = n;
+  r.sigma = src->sigma;
+  r.start = (int*)malloc(sizeof(int) * (n + 1));
+  r.ops = (orc_op*)malloc(sizeof(orc_op) * (src->start[n] + 1));
+  int k = 0, empty = 0;
+  for (int i = 0; i < n; ++i) {
+    r.start[i] = k;
+    int want = -1;
+    for (int q = 0; q < npos; ++q)
+      if (pos[q] == i) want = nuc[q];
+    for (int z = src->start[i]; z < src->start[i + 1]; ++z)
+      if (want < 0 || src->ops[z].b == want) r.ops[k++] = src->ops[z];
+    if (k == r.start[i]) empty = 1;
+  }
+  r.start[n] = k;
+  double lz = -INFINITY;
+  if (!empty) inside_impl(&t->model, &r, 0, -1, -1, NULL, &lz);
+  free(r.start);
+  free(r.ops);
+  return lz;
+}
+
 int orc_marginals(orc_tables* t, double* bpp, double* base, double* codon) {
-  (void)t; (void)bpp; (void)base; (void)codon;
-  return -99; /* implemented in cdz_oracle_outside.c */
+  int n = t->n;
+  real Z = 0;
+  for (int c = 0; c < SG(t, n); ++c) Z += t->qext[n][c];
+  double logZ = (double)logl(Z);
+  if (bpp) {
+    for (int k = 0; k < n * n; ++k) bpp[k] = 0;
+    for (int i = 0; i < n; ++i)
+      for (int j = i + t->model.min_hairpin + 1; j < n; ++j) {
+        double lz = 0;
+        inside_impl(&t->model, t->tt, 0, i, j, NULL, &lz);
+        double p = -expm1(lz - logZ);
+        bpp[i * n + j] = p > 0 ? p : 0;
+      }
+    for (int i = 0; i < n; ++i) {
+      double s = 0;
+      for (int j = 0; j < n; ++j) s += j > i ? bpp[i * n + j] : (j < i ? bpp[j * n + i] : 0);
+      bpp[i * n + i] = 1.0 - s;
+    }
+  }
+  if (base)
+    for (int m = 0; m < n; ++m)
+      for (int b = 0; b < 4; ++b) base[m * 4 + b] = exp(restricted_logz(t, 1, &m, &b) - logZ);
+  if (codon)
+    for (int k = 0; k < n / 3; ++k)
+      for (int c = 0; c < 64; ++c) {
+        int pos[3] = {3 * k, 3 * k + 1, 3 * k + 2}, nuc[3] = {c >> 4, (c >> 2) & 3, c & 3};
+        codon[k * 64 + c] = exp(restricted_logz(t, 3, pos, nuc) - logZ);
+      }
+  return 0;
 }

@@ -83,7 +83,9 @@ int orc_sample(const orc_tables* t, int J, uint64_t seed, uint8_t* seq /*[J][n]*
 /* decision uniform U(seed, sample, kind, i, j) */
 double orc_uniform(uint64_t seed, uint64_t sample, uint64_t kind, uint64_t i, uint64_t j);
 
-/* ---- marginals by the outside (reverse) recursion, eqs 2.5-2.7 / 4.1-4.3 ---- */
+/* ---- marginals, eqs 2.5-2.7 / 4.1-4.3, by their definitions as constrained sums: one inside pass per pair / nucleotide / codon
+ *      (O(n^2) passes: small designs only).  Pinned by the brute-force marginals.  No CUDA counterpart exists yet (DESIGN.md
+ *      section 9): parity unpinned for marginals. ---- */
 int orc_marginals(orc_tables* t, double* bpp /*[n*n]*/, double* base /*[n*4]*/, double* codon /*[L*64]*/);
 
 #ifdef __cplusplus

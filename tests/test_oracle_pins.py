@@ -369,3 +369,39 @@ def test_sampler_marginals_chi2_config1_prefix():
     unp = (pair < 0).mean(0)
     np.testing.assert_allclose(unp, np.diag(bf["bpp"]), atol=5 * 0.5 / math.sqrt(J))
     assert _chi2_pvalue(stat, dof) > 1e-3
+
+
+# ---------------------------------------------------------------- marginals by constrained inside passes
+@pytest.mark.parametrize("aa,kind,cw,pw", [("RSLG", 0, 1, 0), ("LSR", 1, 1, 1), ("MFL", 1, 1, 1), ("GRL", 0, 0, 0)])
+def test_marginals_equal_brute_force(aa, kind, cw, pw):
+    """orc_marginals (eqs 2.5-2.7 as ratios of restricted partition functions) against explicit enumeration of every
+    (sequence, structure): base-pair matrix, base marginals, codon marginals."""
+    m = I.tm1_model()
+    tt = build(aa, kind, cw, pw)
+    bf = O.brute_force(m, tt, marginals=True)
+    bpp, base, codon = O.inside(m, tt).marginals()
+    np.testing.assert_allclose(bpp, bf["bpp"], atol=1e-12)
+    np.testing.assert_allclose(base, bf["base"], atol=1e-12)
+    np.testing.assert_allclose(codon, bf["codon"], atol=1e-12)
+
+
+def test_marginals_sum_rules_24nt():
+    """Beyond brute force (n = 24): rows of the pair matrix + unpaired probability sum to 1, base and codon
+    marginals are normalised, foreign codons carry zero mass, base marginals are the codon marginals summed per nucleotide."""
+    m = I.nn_model()
+    d = I.design(1, 0, 8)
+    tt = O.TT.build(d.aa, d.kind, d.codon_logw)
+    bpp, base, codon = O.inside(m, tt).marginals()
+    P = np.triu(bpp, 1)
+    np.testing.assert_allclose((P + P.T).sum(1) + np.diag(bpp), 1.0, atol=1e-12)
+    assert (np.diag(bpp) >= -1e-15).all() and (P >= 0).all()
+    np.testing.assert_allclose(base.sum(1), 1.0, atol=1e-12)
+    np.testing.assert_allclose(codon.sum(1), 1.0, atol=1e-12)
+    code = "KNKNTTTTRSRSIIMIQHQHPPPPRRRRLLLLEDEDAAAAGGGGVVVV*Y*YSSSS*CWCLFLF"
+    for k, a in enumerate(d.aa):
+        foreign = np.array([code[c] != a for c in range(64)])
+        assert codon[k][foreign].sum() == 0.0
+        for pos in range(3):
+            for b in range(4):
+                sel = np.array([((c >> (2 * (2 - pos))) & 3) == b for c in range(64)])
+                assert abs(codon[k][sel].sum() - base[3 * k + pos, b]) < 1e-12
