@@ -68,7 +68,7 @@ struct Plan {
   int nrow, ncol;        // window lengths (positions)
   int maxbond, maxls;    // compact row lists (bonds / left states of the row window)
   int ntl, ntr;          // positions with a dense TL / TR core
-  size_t o_rowm, o_colm, o_crow, o_rbpos, o_rlpos, o_rbp, o_cbp, o_tl, o_tr, o_scr, total;
+  size_t o_rowm, o_colm, o_crow, o_rbpos, o_rlpos, o_rbp, o_cbp, o_tl, o_tr, o_xoff, o_xst, o_scr, total;
 };
 // span: largest extent, in global (block-padded) bond indices, of a row / column window
 __host__ __device__ inline Plan make_plan(int maxpos, int span, const Dims& D, int C) {
@@ -90,6 +90,8 @@ __host__ __device__ inline Plan make_plan(int maxpos, int span, const Dims& D, i
   p.o_cbp = take(span);
   p.o_tl = take(sizeof(double) * (size_t)p.ntl * D.ML * D.M);
   p.o_tr = take(sizeof(double) * (size_t)p.ntr * D.M * D.MR);
+  p.o_xoff = take(sizeof(int) * (maxpos + 2));
+  p.o_xst = take(sizeof(double) * (size_t)XU * D.M * (CDZ_TB + 2 * D.M));  // X_u state of every column: 27 x M x Sigma_{j-1}
   p.o_scr = take(sizeof(double) * (size_t)C * D.percell());
   p.total = o;
   return p;
@@ -98,6 +100,94 @@ __host__ __device__ inline Plan make_plan(int maxpos, int span, const Dims& D, i
 }  // namespace
 
 namespace {
+
+// One warp advances the interior-loop bodies of one cell:  X_u(i,j) = Tbar_{i+2} X_{u-1}(i+1,j) + GI(i+3, j+1-u) E(j+3-u, j-2)
+// for u = 4..30 (lane = u - 4), in place in the shared-memory state xs of column j (layout [u][a2 < M][c2 < Sc]), and
+// XE[a2][c2] = sum_u win[u] X_u + hairpin.  Columns are processed W at a time so that every lane keeps MA x W accumulators;
+// all lanes finish reading X_{u-1} before any lane writes X_u.
+template <int MA, int W>
+__device__ __forceinline__ void x_cell(int lane, double* xs, int Mst, int Sa, int Sa3, int Sc, bool hasold, bool closed, int mh1,
+                                       int maxint, int i, int j, const double* Tb, int MS, const double* gi, const double* em,
+                                       size_t S, const PosMeta* colm, int cbase, const double* win, double hpw,
+                                       const double* emh, double* xe_out, int Mxe) {
+  const int u = 4 + lane;
+  const bool live = lane < XU;
+  const int cp = j + 3 - u;
+  const bool hasnew = live && cp - (i + 2) - 3 >= mh1;
+  int cpo = 0, cps = 0;
+  if (hasnew) { const PosMeta mc = colm[cp - cbase]; cpo = mc.off; cps = mc.sig; }
+  const double wu = (live && u <= maxint) ? win[u] : 0.0;
+  for (int cc = 0; cc < Sc; cc += W) {
+    const int ncw = min(W, Sc - cc);
+    double acc[MA][W];
+#pragma unroll
+    for (int a = 0; a < MA; ++a)
+#pragma unroll
+      for (int w = 0; w < W; ++w) acc[a][w] = 0.0;
+    if (live && hasold && u > 4) {
+      const double* xo = xs + (size_t)(u - 5) * Mst * Sc + cc;
+      for (int a3 = 0; a3 < Sa3; ++a3) {
+        double xv[W];
+#pragma unroll
+        for (int w = 0; w < W; ++w) xv[w] = w < ncw ? xo[a3 * Sc + w] : 0.0;
+#pragma unroll
+        for (int a = 0; a < MA; ++a) {
+          if (a < Sa) {
+            const double tb = Tb[a * MS + a3];
+#pragma unroll
+            for (int w = 0; w < W; ++w) acc[a][w] += tb * xv[w];
+          }
+        }
+      }
+    }
+    for (int u2 = 0; u2 < cps; ++u2) {
+      double ev[W];
+#pragma unroll
+      for (int w = 0; w < W; ++w) ev[w] = w < ncw ? em[(size_t)(cc + w) * S + cpo + u2] : 0.0;
+#pragma unroll
+      for (int a = 0; a < MA; ++a) {
+        if (a < Sa) {
+          const double gv = gi[(size_t)a * S + cpo + u2];
+#pragma unroll
+          for (int w = 0; w < W; ++w) acc[a][w] += gv * ev[w];
+        }
+      }
+    }
+    __syncwarp();
+    if (live) {
+      double* xn = xs + (size_t)(u - 4) * Mst * Sc + cc;
+#pragma unroll
+      for (int a = 0; a < MA; ++a)
+        if (a < Sa)
+#pragma unroll
+          for (int w = 0; w < W; ++w)
+            if (w < ncw) xn[a * Sc + w] = acc[a][w];
+    }
+    // XE: weighted sum over the lanes; MA*W (= 16) values are reduced together, halving the value set at every shuffle step
+    static_assert(MA * W == 16, "transpose-reduce below assumes 16 values per lane");
+    double v[16];
+#pragma unroll
+    for (int a = 0; a < MA; ++a)
+#pragma unroll
+      for (int w = 0; w < W; ++w) v[a * W + w] = wu * acc[a][w];
+#pragma unroll
+    for (int half = 8, bit = 16; half >= 1; half >>= 1, bit >>= 1) {
+      const bool up = (lane & bit) != 0;
+#pragma unroll
+      for (int k = 0; k < half; ++k) {
+        const double send = up ? v[k] : v[k + half];
+        const double keep = up ? v[k + half] : v[k];
+        v[k] = keep + __shfl_xor_sync(0xffffffffu, send, bit);
+      }
+    }
+    v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
+    if ((lane & 1) == 0) {
+      const int e = lane >> 1, a = e / W, w = e % W;
+      if (a < Sa && w < ncw) xe_out[a * Mxe + cc + w] = v[0] + (closed ? hpw * emh[(size_t)a * S + cc + w] : 0.0);
+    }
+    __syncwarp();
+  }
+}
 
 constexpr int CELL_THREADS = 512;
 constexpr int LG = 4, GL = 1 << LG;  // lanes that share one row item of the cooperative P1 loop
@@ -127,6 +217,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   uint8_t* cbp = smraw + pl.o_cbp;
   double* TLs = (double*)(smraw + pl.o_tl);
   double* TRs = (double*)(smraw + pl.o_tr);
+  int* xoff = (int*)(smraw + pl.o_xoff);      // start of column j's X state in xst (units of M doubles per u)
+  double* xst = (double*)(smraw + pl.o_xst);  // X_u(i+1, j) of every column of the block, u = 4..30
   double* scrb = (double*)(smraw + pl.o_scr);
   const int tid = threadIdx.x, NT = blockDim.x;
   const int n = t.n, MS = t.MS, MS2 = MS * MS;
@@ -206,6 +298,25 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   }
   __syncthreads();
 
+  // ---- interior-loop body state of the block's columns: X_u(i1, j) comes from the block below (global XS), zero on the diagonal ----
+  const int ncolj = j1 - j0;
+  if (tid == 0) {
+    int acc = 0;
+    for (int jc = 0; jc < ncolj; ++jc) { xoff[jc] = acc; acc += (j0 + jc >= 1) ? colm[j0 + jc - 1 - cbase].sig : 0; }
+    xoff[ncolj] = acc;
+  }
+  __syncthreads();
+  for (int jc = 0; jc < ncolj; ++jc) {
+    const int j = j0 + jc, Sc = xoff[jc + 1] - xoff[jc];
+    double* xs = xst + (size_t)XU * M * xoff[jc];
+    const double* src = b.XS + (size_t)j * (XU * MS2);
+    for (int e = tid; e < XU * MS * Sc; e += NT) {
+      const int c2 = e % Sc, a2 = (e / Sc) % MS, u4 = e / (Sc * MS);
+      xs[((size_t)u4 * M + a2) * Sc + c2] = (I != J) ? src[u4 * MS2 + a2 * MS + c2] : 0.0;
+    }
+  }
+  __syncthreads();
+
   const int mh1 = cm.min_hairpin + 1, maxint = cm.max_interior;
   const uint8_t* __restrict__ ls_a = t.ls_a;
   const uint8_t* __restrict__ ls_x = t.ls_x;
@@ -246,6 +357,27 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
       const int nb1 = bond_rows(clo + 1, chi + 1, rb1);  // bonds of position p = i+1
       const int nb2 = bond_rows(clo + 2, chi + 2, rb2);  // bonds of position i+2
       const int nl1 = ls_rows(clo + 1, chi + 1, rl1);    // left states of position p
+      // ---- X_u / XE: one warp per cell, state of column j in shared memory ------------------------------------------------------
+      if (d >= 4) {
+        const int lane = tid & 31;
+        for (int i = clo + (tid >> 5); i <= chi; i += NT >> 5) {
+          const int j = i + d, kp2 = i + 2 - rbase;
+          const PosMeta mq = colm[j - 1 - cbase];
+          double* xs = xst + (size_t)XU * M * xoff[j - j0];
+          const double* Tb = Tbar + (size_t)(i + 2) * MS2;
+          const double* gi = b.GI + (size_t)rowm[kp2].off * S;
+          const double* em = b.EMT + (size_t)mq.off * S;
+          const double* emh = b.EM + (size_t)rowm[kp2].off * S + mq.off;
+          double* xe = scr_of(scrb, dm, i - clo).XE;
+          const double hpw = closed ? t.wh[d - 1] : 0.0;
+          if (M <= 4)
+            x_cell<4, 4>(lane, xs, M, rowm[kp2].sig, rowm[kp2 + 1].sig, mq.sig, d - 1 >= 4, closed, mh1, maxint, i, j, Tb, MS, gi, em, S,
+                         colm, cbase, cm.win, hpw, emh, xe, M);
+          else
+            x_cell<8, 2>(lane, xs, M, rowm[kp2].sig, rowm[kp2 + 1].sig, mq.sig, d - 1 >= 4, closed, mh1, maxint, i, j, Tb, MS, gi, em, S,
+                         colm, cbase, cm.win, hpw, emh, xe, M);
+        }
+      }
       // ---- cooperative row items: 8 consecutive lanes share one row object (a bond row or a left state of one cell), split
       //      its contiguous bond range between them and keep up to 4 column accumulators per pass.
       //      M2 edge ranges | Bl | Br | Z1 | Z2 : weighted dot products of row segments;   X : the lanes split u = 4..30
@@ -254,7 +386,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
         const int n3 = closed ? nb1 : 0;  // Bl, Br : bond row of p    x  c1 < Sigma_j
         const int n5 = closed ? nl1 : 0;  // Z1     : left state of p  x  c2 < Sigma_q
         const int n6 = closed ? nb2 : 0;  // Z2     : bond row of i+2  x  r  < |R_q|
-        const int n2 = d >= 4 ? nb2 : 0;  // X      : bond row of i+2  x  c2 < Sigma_q
+        const int n2 = 0;                 // (X is advanced by one warp per cell, below)
         const int e9 = n9, e3 = e9 + n3, e4 = e3 + n3, e5 = e4 + n5, e6 = e5 + n6, e2 = e6 + n2;
         const unsigned gmask = ((1u << GL) - 1u) << (tid & 31 & ~(GL - 1));
         for (int ts = tid; ts < (e2 << LG); ts += NT) {
@@ -405,82 +537,6 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
                 a3 += __shfl_xor_sync(gmask, a3, o);
               }
               if (sub < nc4) out[cc + sub] = addw * add + (sub == 0 ? a0 : sub == 1 ? a1 : sub == 2 ? a2 : a3);
-            }
-          } else {
-            // ---- X_u(i,j) = Tbar_{i+2} X_{u-1}(i+1,j) + GI(i+3, j+1-u) E(j+3-u, j-2), lanes split u; XE = sum_u win[u] X_u ----
-            const int rr = rb2 + (g - e6), kp = rbpos[rr], a2 = rr - crow[kp];
-            const int i = rbase + kp - 2, j = i + d;
-            const PosMeta mq = colm[j - 1 - cbase];
-            const int offa = rowm[kp].off + a2, Sa3 = rowm[kp + 1].sig;
-            const double* Tb = Tbar + (size_t)(i + 2) * MS2 + a2 * MS;
-            const double* xo = b.XS + ((size_t)((i + 1) & 1) * n + j) * (XU * MS2);
-            double* xn = b.XS + ((size_t)(i & 1) * n + j) * (XU * MS2) + a2 * MS;
-            const double* gi = b.GI + (size_t)offa * S;
-            const double* em = b.EMT + (size_t)mq.off * S;
-            const bool hasold = d - 1 >= 4;
-            double* out = scr_of(scrb, dm, i - clo).XE + a2 * M;
-            for (int cc = 0; cc < mq.sig; cc += 4) {
-              const int nc4 = min(4, mq.sig - cc);
-              double e0 = 0.0, e1 = 0.0, e2x = 0.0, e3x = 0.0;
-              constexpr int KX = (XU + GL - 1) / GL;
-              double xv[KX][4];
-              const double hp = (closed && sub < nc4) ? t.wh[d - 1] * b.EM[(size_t)offa * S + mq.off + cc + sub] : 0.0;
-              // all loads first (the stores below go to the same array XS and would otherwise order them)
-#pragma unroll
-              for (int k = 0; k < KX; ++k) {
-                const int u = 4 + sub + GL * k;
-                double x0 = 0.0, x1 = 0.0, x2 = 0.0, x3 = 0.0;
-                if (u <= 30) {
-                  if (hasold && u > 4) {
-                    const double* xr = xo + (u - 5) * MS2 + cc;
-                    for (int a3 = 0; a3 < Sa3; ++a3) {
-                      const double tb = Tb[a3];
-                      x0 += tb * xr[a3 * MS];
-                      if (nc4 > 1) x1 += tb * xr[a3 * MS + 1];
-                      if (nc4 > 2) x2 += tb * xr[a3 * MS + 2];
-                      if (nc4 > 3) x3 += tb * xr[a3 * MS + 3];
-                    }
-                  }
-                  const int cp = j + 3 - u;
-                  if (cp - (i + 2) - 3 >= mh1) {
-                    const PosMeta mc = colm[cp - cbase];
-                    const double* er = em + (size_t)cc * S + mc.off;
-                    for (int u2 = 0; u2 < mc.sig; ++u2) {
-                      const double gv = gi[mc.off + u2];
-                      x0 += gv * er[u2];
-                      if (nc4 > 1) x1 += gv * er[S + u2];
-                      if (nc4 > 2) x2 += gv * er[2 * S + u2];
-                      if (nc4 > 3) x3 += gv * er[3 * S + u2];
-                    }
-                  }
-                  if (u <= maxint) {
-                    const double w = cm.win[u];
-                    e0 += w * x0; e1 += w * x1; e2x += w * x2; e3x += w * x3;
-                  }
-                }
-                xv[k][0] = x0; xv[k][1] = x1; xv[k][2] = x2; xv[k][3] = x3;
-              }
-#pragma unroll
-              for (int k = 0; k < KX; ++k) {
-                const int u = 4 + sub + GL * k;
-                if (u <= 30) {
-                  double* xw = xn + (u - 4) * MS2 + cc;
-                  xw[0] = xv[k][0];
-                  if (nc4 > 1) xw[1] = xv[k][1];
-                  if (nc4 > 2) xw[2] = xv[k][2];
-                  if (nc4 > 3) xw[3] = xv[k][3];
-                }
-              }
-#pragma unroll
-              for (int o = 1; o < GL; o <<= 1) {
-                e0 += __shfl_xor_sync(gmask, e0, o);
-                e1 += __shfl_xor_sync(gmask, e1, o);
-                e2x += __shfl_xor_sync(gmask, e2x, o);
-                e3x += __shfl_xor_sync(gmask, e3x, o);
-              }
-              if (sub < nc4) {
-                out[cc + sub] = hp + (sub == 0 ? e0 : sub == 1 ? e1 : sub == 2 ? e2x : e3x);
-              }
             }
           }
 #ifdef CDZ_PHASE_TIMING
@@ -757,6 +813,17 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
       // barrier after P1 only for Y; P1 itself writes other arrays, so no barrier is needed here
     }
   }
+  // ---- hand the column states (now X_u(i0, j)) to the block above ------------------------------------------------------------
+  __syncthreads();
+  for (int jc = 0; jc < ncolj; ++jc) {
+    const int j = j0 + jc, Sc = xoff[jc + 1] - xoff[jc];
+    const double* xs = xst + (size_t)XU * M * xoff[jc];
+    double* dst = b.XS + (size_t)j * (XU * MS2);
+    for (int e = tid; e < XU * MS * Sc; e += NT) {
+      const int c2 = e % Sc, a2 = (e / Sc) % MS, u4 = e / (Sc * MS);
+      dst[u4 * MS2 + a2 * MS + c2] = xs[((size_t)u4 * M + a2) * Sc + c2];
+    }
+  }
 #ifdef CDZ_PHASE_TIMING
   if (blockIdx.x == 3 && blockIdx.y == 0 && (tid == 0 || tid == 37 || tid == 300 || tid == 511) && (ka.D == 5 || ka.D == 60 || ka.D == 300))
     printf("D=%d tid=%d coop=%lld single=%lld barwait=%lld P2P3a=%lld P3b=%lld P4=%lld P5=%lld steps=%d | M2=%lld Bl=%lld Br=%lld Z1=%lld Z2=%lld X=%lld\n", ka.D, tid, tph[0], tph[1],
@@ -796,7 +863,7 @@ int cdz_cell_config(cdz_tables* const* ts, int B, cdz_cell_cfg* cfg) {
       span = std::max(span, tt->off[cend] + tt->sigma[cend] - tt->off[cbase]);
     }
   }
-  const size_t budget = 200 * 1024;
+  const size_t budget = 225 * 1024;
   int C = maxpos;
   while (C > 1 && make_plan(maxpos, span, dm, C).total > budget) --C;
   const Plan pl = make_plan(maxpos, span, dm, C);

@@ -364,7 +364,7 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   b.EM = k.take<double>(S * S);
   b.EMT = k.take<double>(S * S);
   b.QBST = k.take<double>(S * S);
-  b.XS = k.take<double>(2 * n * 27 * MS * MS);
+  b.XS = k.take<double>(n * 27 * MS * MS);
   x.cm = k.take<CModel>(1);
   return (k.used + 255) & ~size_t(255);
 }

@@ -241,7 +241,7 @@ __global__ void __launch_bounds__(256) rescale_kernel(const Ctx* ctxs, int which
 }
 
 // Interior-loop body state XS: after block diagonal D, column j (bond position j+1 in block Jc) was last advanced by
-// block (Jc-D, Jc); the next block up reads the state of that block's top row i0 (parity i0 & 1), a quantity over
+// block (Jc-D, Jc); the next block up reads the state of that block's top row i0, a quantity over
 // [i0+2 .. j-2], so it is multiplied by 2^-(dP[j-1] - dP[i0+2]).
 __global__ void __launch_bounds__(256) rescale_xs_kernel(const Ctx* ctxs, int D) {
   const Ctx& cx = ctxs[blockIdx.y];
@@ -256,7 +256,7 @@ __global__ void __launch_bounds__(256) rescale_xs_kernel(const Ctx* ctxs, int D)
     if (j - 1 < i0 + 2) continue;
     const int e = b.dP[j - 1] - b.dP[i0 + 2];
     if (e == 0) continue;
-    double* p = b.XS + ((size_t)(i0 & 1) * n + j) * per;
+    double* p = b.XS + (size_t)j * per;
     for (int k = threadIdx.x; k < per; k += blockDim.x) p[k] = scalbn(p[k], -e);
   }
 }

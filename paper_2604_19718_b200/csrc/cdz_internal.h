@@ -92,7 +92,7 @@ struct DevTabT {
   T *EM;    // S x S   : E(i,j) = Tbar_i..Tbar_j; the diagonal holds E(i,i-1) = identity
   T *EMT;   // S x S   : EM transposed (row (j+1,c), column (i,a))
   T *QBST;  // S x S   : QBS transposed
-  T *XS;    // [2][n][27][MS*MS] : interior-loop bodies X_u(i,j), u = 4..30, of the last two rows of every column j
+  T *XS;    // [n][27][MS*MS] : interior-loop bodies X_u(i0,j), u = 4..30, of the top row of the last block of every column j
   T *Qext;  // [n+1][MS]
   T *GP;    // split-point GEMM partial sums: [block row I][split][CDZ_TB*CDZ_TB]
   T *R;     // [S] exterior accumulator
