@@ -38,7 +38,7 @@ typedef enum {
 } cdz_status;
 
 enum { CDZ_TT_SINGLE_CODON = 0, CDZ_TT_CODON_PAIR = 1 };
-enum { CDZ_FP64 = 0, CDZ_FP32_SCALED = 1 };
+enum { CDZ_FP64 = 0, CDZ_FP32_SCALED = 1 };  /* CDZ_FP32_SCALED is declared but not built: CDZ_EINVAL */
 
 /* Nearest-neighbour loop model (BASELINE.json configs[0]); energies in kcal/mol.
  *   hairpin(l)  = hairpin_a + hairpin_b * kT * ln(l / hairpin_l0) + tmm[p(i,j)][phi_{i+1}][phi_{j-1}],  l >= min_hairpin
@@ -153,7 +153,8 @@ int cdz_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* p
 
 /* ---- marginals (device) ---------------------------------------------------- */
 /* bpp_dev [n][n]: upper triangle P(i.j) (eq 2.5), diagonal P(i unpaired); base_dev [n][4] (eq 2.6);
- * codon_dev [L][64] (eq 2.7).  Any may be NULL. */
+ * codon_dev [L][64] (eq 2.7).  Any may be NULL.
+ * NOT BUILT YET (needs the outside / adjoint pass): always returns CDZ_ESTATE and writes nothing. */
 int cdz_marginals(cdz_tables* t, double* bpp_dev, double* base_dev, double* codon_dev, void* stream);
 
 /* ---- convenience: host buffers end to end (used for the e2e timing) -------- */

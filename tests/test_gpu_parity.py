@@ -208,3 +208,19 @@ def test_config5_full_batch(B, O):
         t1, lz1 = B.inside(mg, tts[item])
         assert lzs[item] == lz1
     _prefix_chain(B, O, 5, 150, 20)
+
+
+def _stored_oracle_rows():
+    path = os.path.join(GOLD, "oracle_logz.txt")
+    return rows("oracle_logz.txt") if os.path.exists(path) else []
+
+
+@pytest.mark.parametrize("row", _stored_oracle_rows(), ids=lambda r: f"config{r[0]}-L{r[2]}")
+def test_full_size_logz_vs_stored_oracle(B, row):
+    """log Z of whole BASELINE designs against the value the plain CPU oracle computed for them (minutes to hours of CPU time,
+    hence stored: tests/golden/oracle_logz.txt, written by tests/golden/make_golden.py which calls only oracle/)."""
+    cfg, item, L, want = int(row[0]), int(row[1]), int(row[2]), float(row[4])
+    d = I.design(cfg, item, L)
+    assert d.n == int(row[3])
+    tg, lz = B.inside(B.Model(I.nn_model()), B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw))
+    assert abs(lz - want) <= LOGZ_RTOL * abs(want), (lz, want)
