@@ -201,6 +201,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ CModel cm;
   __shared__ int pmx[16];  // nucleotide mask of position i -> mask of the nucleotides at j that can pair with one of them
+  __shared__ int p1ctr[4];  // work counters of P1: warps take X cells / 32-slot chunks of the item loops as they become free
   const Ctx& cx = ctxs[blockIdx.y];
   const DevTT& t = cx.tt;
   const DevTab& b = cx.tab;
@@ -275,6 +276,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
     pmx[tid] = pm;
   }
   if (tid == 0) {
+    p1ctr[0] = p1ctr[1] = p1ctr[2] = 0;
     int acc = 0;
     for (int k = 0; k < nrp; ++k) { crow[k] = acc; acc += rowm[k].sig; }
     crow[nrp] = acc;
@@ -345,6 +347,12 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
 #else
 #define CDZ_TICK(k)
 #endif
+  // dynamic distribution of the P1 work: lane 0 takes the next unit, the warp follows
+  auto grab = [&](int* c) {
+    int w = 0;
+    if ((tid & 31) == 0) w = atomicAdd(c, 1);
+    return __shfl_sync(0xffffffffu, w, 0);
+  };
   const int dmin = max(0, j0 - (i1 - 1)), dmax = (j1 - 1) - i0;
   for (int d = dmin; d <= dmax; ++d) {
     const int ilo = max(i0, j0 - d), ihi = min(i1 - 1, j1 - 1 - d);
@@ -360,8 +368,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
       // ---- X_u / XE: one warp per cell, state of column j in shared memory ------------------------------------------------------
       if (d >= 4) {
         const int lane = tid & 31;
-        for (int i = clo + (tid >> 5); i <= chi; i += NT >> 5) {
-          const int j = i + d, kp2 = i + 2 - rbase;
+        for (int w; (w = grab(&p1ctr[0])) <= chi - clo;) {
+          const int i = clo + w, j = i + d, kp2 = i + 2 - rbase;
           const PosMeta mq = colm[j - 1 - cbase];
           double* xs = xst + (size_t)XU * M * xoff[j - j0];
           const double* Tb = Tbar + (size_t)(i + 2) * MS2;
@@ -389,7 +397,9 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
         const int n2 = 0;                 // (X is advanced by one warp per cell, below)
         const int e9 = n9, e3 = e9 + n3, e4 = e3 + n3, e5 = e4 + n5, e6 = e5 + n6, e2 = e6 + n2;
         const unsigned gmask = ((1u << GL) - 1u) << (tid & 31 & ~(GL - 1));
-        for (int ts = tid; ts < (e2 << LG); ts += NT) {
+        for (int w; (w = grab(&p1ctr[1])) < (((e2 << LG) + 31) >> 5);) {
+          const int ts = (w << 5) + (tid & 31);
+          if (ts >= (e2 << LG)) continue;
           const int g = ts >> LG, sub = ts & (GL - 1);
 #ifdef CDZ_PHASE_TIMING
           const long long tr0 = clock64();
@@ -551,7 +561,9 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
         const int n7 = closed ? nb1 * npm : 0;
         const int n8 = nb0 << lgM;
         const int e7 = n7, e8 = e7 + n8, e1 = e8 + n8;
-        for (int g = tid; g < e1; g += NT) {
+        for (int w; (w = grab(&p1ctr[2])) < ((e1 + 31) >> 5);) {
+          const int g = (w << 5) + (tid & 31);
+          if (g >= e1) continue;
           if (g < e7) {
             // ---- SB[a'][slot'][c']: inner pair identity kept (stack, bulges of size 1) ------------------------------
             const int rq = g / npm, it = g - rq * npm;
@@ -618,6 +630,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
       }
       CDZ_TICK(1);
       __syncthreads();
+      if (tid == 0) p1ctr[0] = p1ctr[1] = p1ctr[2] = 0;  // every warp has left P1; the next P1 is several barriers away
       CDZ_TICK(2);
       if (closed) {
         // ================= P2: Y[(a',u)][(v,c')] -- everything that carries the closing mismatch =================
