@@ -126,21 +126,26 @@ __device__ __forceinline__ void x_cell(int lane, double* xs, int Mst, int Sa, in
       for (int w = 0; w < W; ++w) acc[a][w] = 0.0;
     if (live && hasold && u > 4) {
       const double* xo = xs + (size_t)(u - 5) * Mst * Sc + cc;
-      for (int a3 = 0; a3 < Sa3; ++a3) {
-        double xv[W];
 #pragma unroll
-        for (int w = 0; w < W; ++w) xv[w] = w < ncw ? xo[a3 * Sc + w] : 0.0;
+      for (int a3 = 0; a3 < MA; ++a3) {  // fixed trip count + predicates: all loads of the pass can be issued before the first FMA
+        if (a3 < Sa3) {
+          double xv[W];
 #pragma unroll
-        for (int a = 0; a < MA; ++a) {
-          if (a < Sa) {
-            const double tb = Tb[a * MS + a3];
+          for (int w = 0; w < W; ++w) xv[w] = w < ncw ? xo[a3 * Sc + w] : 0.0;
 #pragma unroll
-            for (int w = 0; w < W; ++w) acc[a][w] += tb * xv[w];
+          for (int a = 0; a < MA; ++a) {
+            if (a < Sa) {
+              const double tb = Tb[a * MS + a3];
+#pragma unroll
+              for (int w = 0; w < W; ++w) acc[a][w] += tb * xv[w];
+            }
           }
         }
       }
     }
-    for (int u2 = 0; u2 < cps; ++u2) {
+#pragma unroll
+    for (int u2 = 0; u2 < MA; ++u2) {
+      if (u2 >= cps) break;
       double ev[W];
 #pragma unroll
       for (int w = 0; w < W; ++w) ev[w] = w < ncw ? em[(size_t)(cc + w) * S + cpo + u2] : 0.0;
