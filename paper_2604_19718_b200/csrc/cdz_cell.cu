@@ -579,6 +579,11 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             if (c1 >= mj.sig || !(pmx[rowm[kp - 1].nuc] & mj.nuc)) continue;
             const PosMeta mp = rowm[kp], mq = colm[q - cbase];
             const int xp = cm.slot_x[sl], yp = cm.slot_y[sl];
+            // the inner pair (x', y') sits at (p, q), (p+1, q) or (p, q-1): nothing to add when x' or y' cannot occur there
+            if (!(((mp.nuc | rowm[kp + 1].nuc) >> xp) & 1) || !(((mq.nuc | colm[q - 1 - cbase].nuc) >> yp) & 1)) {
+              scr_of(scrb, dm, i - clo).SB[(a1 * nps + sl) * M + c1] = 0.0;
+              continue;
+            }
             const int lst = t.lsidx[((size_t)p * MS + a1) * 4 + xp], r = t.rsidx[((size_t)q * 4 + yp) * MS + c1];
             double v = 0.0;
             if (q - p >= mh1 && lst >= 0 && r >= 0) v = b.QB[(size_t)(mp.loff + lst) * RS + mq.roff + r];
@@ -672,6 +677,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           if (c1 >= mj.sig || !(pmx[rowm[kp - 1].nuc] & mj.nuc)) continue;
           const PosMeta mp = rowm[kp], mq = colm[q - cbase];
           const Scr sc = scr_of(scrb, dm, i - clo);
+          // inner[slot] is read by Qb(i,j) only for slots whose nucleotides occur at i and j
+          if (!((rowm[kp - 1].nuc >> cm.slot_x[sl]) & 1) || !((mj.nuc >> cm.slot_y[sl]) & 1)) continue;
           const int P = cm.ptype[cm.slot_x[sl] * 4 + cm.slot_y[sl]];
           double v = sc.Bl[a1 * M + c1] + sc.Br[a1 * M + c1];
           for (int l = 0; l < mp.nL; ++l) {
