@@ -28,6 +28,21 @@ namespace {
 
 struct PosMeta { int off, sig, loff, nL, roff, nR, ops, nuc; };  // 32 bytes per position of a window; nuc = bit mask of the nucleotides possible there
 
+// window of position records in shared memory; -DCDZ_CHECK (development) traps on an index outside the window
+struct MetaWin {
+  PosMeta* p;
+  int n, tag;
+  __device__ __forceinline__ PosMeta& operator[](int k) const {
+#ifdef CDZ_CHECK
+    if (k < 0 || k >= n) {
+      printf("cdz: position window %d: index %d outside [0,%d) (block %d,%d thread %d)\n", tag, k, n, blockIdx.x, blockIdx.y, threadIdx.x);
+      __trap();
+    }
+#endif
+    return p[k];
+  }
+};
+
 constexpr int XU = 27;       // interior totals u = l1 + l2 = 4..30 with l1, l2 >= 2
 constexpr int ROWPAD = 34;   // row window  [i0-1, i1+ROWPAD-2]
 constexpr int COLPAD = 34;   // column window [j0-COLPAD+1, j1+1]
@@ -214,8 +229,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   if (J >= t.NB) return;
   const Dims dm = ka.dm;
   const Plan pl = make_plan(ka.maxpos, ka.span, dm, ka.C);
-  PosMeta* rowm = (PosMeta*)(smraw + pl.o_rowm);
-  PosMeta* colm = (PosMeta*)(smraw + pl.o_colm);
+  MetaWin rowm{(PosMeta*)(smraw + pl.o_rowm), 0, 0};
+  MetaWin colm{(PosMeta*)(smraw + pl.o_colm), 0, 1};
   int* crow = (int*)(smraw + pl.o_crow);
   short* rbpos = (short*)(smraw + pl.o_rbpos);
   short* rlpos = (short*)(smraw + pl.o_rlpos);
@@ -239,6 +254,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   const int rbase = max(i0 - 1, 0), rend = min(i1 + ROWPAD - 2, n);
   const int cbase = max(j0 - COLPAD + 1, 0), cend = min(j1 + 1, n);
   const int nrp = rend - rbase + 1, ncp = cend - cbase + 1;
+  rowm.n = nrp;
+  colm.n = ncp;
   const int tlbase = rbase, ntl = min(i1, n - 1) - tlbase + 1;
   const int trbase = max(j0 - 1, 0), ntr = min(j1, n - 1) - trbase + 1;
 
@@ -385,10 +402,10 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           const double hpw = closed ? t.wh[d - 1] : 0.0;
           if (M <= 4)
             x_cell<4, 4>(lane, xs, M, rowm[kp2].sig, rowm[kp2 + 1].sig, mq.sig, d - 1 >= 4, closed, mh1, maxint, i, j, Tb, MS, gi, em, S,
-                         colm, cbase, cm.win, hpw, emh, xe, M);
+                         colm.p, cbase, cm.win, hpw, emh, xe, M);
           else
             x_cell<8, 2>(lane, xs, M, rowm[kp2].sig, rowm[kp2 + 1].sig, mq.sig, d - 1 >= 4, closed, mh1, maxint, i, j, Tb, MS, gi, em, S,
-                         colm, cbase, cm.win, hpw, emh, xe, M);
+                         colm.p, cbase, cm.win, hpw, emh, xe, M);
         }
       }
       // ---- cooperative row items: 8 consecutive lanes share one row object (a bond row or a left state of one cell), split
