@@ -3,21 +3,22 @@
 // the mismatch-dressed extensions that later interior loops read (
 // sequence sums as in chi-hat, eq 3.8).
 //
-// One CTA per block (I, J = I + D).  The in-block anti-diagonals are walked in order; on each one ALL cells are
-// advanced together in a few phases separated by __syncthreads, every phase a flat loop over items
-// (row object of one cell) x (column object), one thread per item:
-//   P1  everything that depends only on finished diagonals, all item types in one flat loop:
-//         M2 edge ranges (4 lanes per entry), band sums Bl / Br (bulges >= 2 + multiloop closure), Z1 / Z2 (l1 = 1 / l2 = 1
-//         interior loops), X_u row recursion + XE (generic interior bodies + hairpin), SB (stack, bulge 1),
-//         the recursive parts of Qm1 / Qml, E(i,j)
+// One CTA (512 threads) per block (I, J = I + D).  The in-block anti-diagonals are walked in order; on each one ALL cells are
+// advanced together in a few phases separated by __syncthreads:
+//   P1  everything that depends only on finished diagonals; the work is handed out dynamically (shared counters), in this order:
+//         X   one warp per cell: interior-loop bodies X_u (row recursion, state of every column in shared memory) and
+//             XE = sum_u win[u] X_u + hairpin
+//         row items, 16 lanes each over a contiguous bond range: M2 edge ranges, Bl / Br (multiloop closure + bulges >= 2),
+//             Z1 / Z2 (l1 = 1 / l2 = 1 interior loops)
+//         single-lane items: SB (stack, bulge 1), the recursive parts of Qm1 / Qml, E(i,j)
 //   P2  Y   = everything that carries the closing mismatch
 //   P3a IN  = inner[slot][a'][c'];   P3b Qb
 //   P4  Qbs, Qm1, Qml, M2, Qm (+ transposed copies)  and  DD = dressed extension of Qb(i,j) over [i-1..j+1]
 //   P5  GI, D1, D2T (DD summed over one or both nucleotides)
 // Every band sum is a dot product of two CONTIGUOUS row segments of row-major tables (transposed copies EMT, QBST,
-// D2T, QM1T exist for that purpose), so the loads of consecutive iterations share sectors and are independent.
+// D2T, QM1T exist for that purpose), so the loads of the lanes of a group are coalesced and independent.
 // Position metadata and the dense cores TL_i[(a,x)][c], TR_j[a][(y,c)] of the block's rows / columns live in
-// shared memory; the per-cell intermediates live in a shared-memory scratch slab.
+// shared memory; the per-cell intermediates live in a shared-memory scratch slab (DESIGN.md section 8.1).
 #include <math.h>
 
 #include <algorithm>
@@ -408,9 +409,9 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
                          colm.p, cbase, cm.win, hpw, emh, xe, M);
         }
       }
-      // ---- cooperative row items: 8 consecutive lanes share one row object (a bond row or a left state of one cell), split
+      // ---- cooperative row items: GL consecutive lanes share one row object (a bond row or a left state of one cell), split
       //      its contiguous bond range between them and keep up to 4 column accumulators per pass.
-      //      M2 edge ranges | Bl | Br | Z1 | Z2 : weighted dot products of row segments;   X : the lanes split u = 4..30
+      //      M2 edge ranges | Bl | Br | Z1 | Z2 : weighted dot products of row segments
       {
         const int n9 = nb0;               // M2 edge: bond row of i    x  c  < Sigma_{j+1}
         const int n3 = closed ? nb1 : 0;  // Bl, Br : bond row of p    x  c1 < Sigma_j
