@@ -8,7 +8,7 @@
 //   P1  everything that depends only on finished diagonals; the work is handed out dynamically (shared counters), in this order:
 //         X   one warp per cell: interior-loop bodies X_u (row recursion, state of every column in shared memory) and
 //             XE = sum_u win[u] X_u + hairpin
-//         row items, 16 lanes each over a contiguous bond range: M2 edge ranges, Bl / Br (multiloop closure + bulges >= 2),
+//         row items, GL = 4 lanes each over a contiguous bond range: M2 edge ranges, Bl / Br (multiloop closure + bulges >= 2),
 //             Z1 / Z2 (l1 = 1 / l2 = 1 interior loops)
 //         single-lane items: SB (stack, bulge 1), the recursive parts of Qm1 / Qml, E(i,j)
 //   P2  Y   = everything that carries the closing mismatch
@@ -211,7 +211,7 @@ __device__ __forceinline__ void x_cell(int lane, double* xs, int Mst, int Sa, in
 }
 
 constexpr int CELL_THREADS = 512;
-constexpr int LG = 4, GL = 1 << LG;  // lanes that share one row item of the cooperative P1 loop
+constexpr int LG = 2, GL = 1 << LG;  // lanes that share one row item of the cooperative P1 loop
 
 struct KArgs {
   int D, nsplit, C, maxpos, span;
@@ -419,7 +419,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
         const int n6 = closed ? nb2 : 0;  // Z2     : bond row of i+2  x  r  < |R_q|
         const int n2 = 0;                 // (X is advanced by one warp per cell, below)
         const int e9 = n9, e3 = e9 + n3, e4 = e3 + n3, e5 = e4 + n5, e6 = e5 + n6, e2 = e6 + n2;
-        const unsigned gmask = ((1u << GL) - 1u) << (tid & 31 & ~(GL - 1));
+        const unsigned gmask = GL >= 32 ? 0xffffffffu : ((1u << (GL & 31)) - 1u) << (tid & 31 & ~(GL - 1));
         for (int w; (w = grab(&p1ctr[1])) < (((e2 << LG) + 31) >> 5);) {
           const int ts = (w << 5) + (tid & 31);
           if (ts >= (e2 << LG)) continue;
@@ -511,9 +511,17 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             for (int cc = 0; cc < ncol; cc += 4) {
               const int nc4 = min(4, ncol - cc);
               const double* Bc = B0 + (size_t)cc * S;
-              double add = 0.0;
-              if (sub < nc4)
-                for (int sp = 0; sp < nadd; ++sp) add += addp[(size_t)sp * (CDZ_TB * CDZ_TB) + cc + sub];
+              // the additive terms of the (up to 4) columns of this pass; lane c of the group takes column c (every lane when GL < 4)
+              double add = 0.0, addv[4] = {0.0, 0.0, 0.0, 0.0};
+              if (GL >= 4) {
+                if (sub < nc4)
+                  for (int sp = 0; sp < nadd; ++sp) add += addp[(size_t)sp * (CDZ_TB * CDZ_TB) + cc + sub];
+              } else if (sub == 0) {
+                for (int sp = 0; sp < nadd; ++sp)
+#pragma unroll
+                  for (int c = 0; c < 4; ++c)
+                    if (c < nc4) addv[c] += addp[(size_t)sp * (CDZ_TB * CDZ_TB) + cc + c];
+              }
               double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
               if (wt) {
                 const double* B1 = Bc + (nc4 > 1 ? S : 0);
@@ -569,7 +577,14 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
                 a2 += __shfl_xor_sync(gmask, a2, o);
                 a3 += __shfl_xor_sync(gmask, a3, o);
               }
-              if (sub < nc4) out[cc + sub] = addw * add + (sub == 0 ? a0 : sub == 1 ? a1 : sub == 2 ? a2 : a3);
+              if (GL >= 4) {
+                if (sub < nc4) out[cc + sub] = addw * add + (sub == 0 ? a0 : sub == 1 ? a1 : sub == 2 ? a2 : a3);
+              } else if (sub == 0) {
+                out[cc] = addw * addv[0] + a0;
+                if (nc4 > 1) out[cc + 1] = addw * addv[1] + a1;
+                if (nc4 > 2) out[cc + 2] = addw * addv[2] + a2;
+                if (nc4 > 3) out[cc + 3] = addw * addv[3] + a3;
+              }
             }
           }
 #ifdef CDZ_PHASE_TIMING
