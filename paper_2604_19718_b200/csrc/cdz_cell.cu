@@ -827,42 +827,48 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
       CDZ_TICK(5);
       // ================= P5: GI, D1, D2T = DD summed over both / the right / the left nucleotide =========================
       if (dress) {
-        const int n1 = nbm << lgM, n2 = nlm << lgM, n3 = nbm << lgR;
-        for (int g = tid; g < n1 + n2 + n3; g += NT) {
-          if (g < n1 || g >= n1 + n2) {
-            const bool gi = g < n1;
-            const int it = gi ? g : g - n1 - n2, lg = gi ? lgM : lgR;
-            const int c = it & ((1 << lg) - 1), rr = rbm + (it >> lg), kp = rbpos[rr], a = rr - crow[kp];
-            const int pi = rbase + kp, i = pi + 1, j = i + d, pj = j + 1;
-            const PosMeta mpi = rowm[kp], mpj = colm[pj - cbase];
-            const Scr sc = scr_of(scrb, dm, i - clo);
-            if (gi) {
-              const PosMeta mpj1 = colm[pj + 1 - cbase];
-              if (c >= mpj1.sig) continue;
-              double v = 0.0;
-              for (int l = 0; l < mpi.nL; ++l)
-                if (ls_a[mpi.loff + l] == a)
-                  for (int k = 0; k < mpj.nR; ++k)
-                    if (rs_c[mpj.roff + k] == c) v += sc.Y[l * MR + k];
-              b.GI[(size_t)(mpi.off + a) * S + mpj1.off + c] = v;
-            } else {
-              if (c >= mpj.nR) continue;
-              double v = 0.0;
-              for (int l = 0; l < mpi.nL; ++l)
-                if (ls_a[mpi.loff + l] == a) v += sc.Y[l * MR + c];
-              b.D2T[(size_t)(mpj.roff + c) * S + mpi.off + a] = v;
-            }
-          } else {
-            const int it = g - n1;
-            const int c = it & (Mp - 1), ll = rlm + (it >> lgM), kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
+        // one lane per ROW of the dressed extension (few, longer items): a left state gives its D1 row, a bond row gives its
+        // D2T column and its GI row
+        for (int g = tid; g < nlm + nbm; g += NT) {
+          if (g < nlm) {
+            const int ll = rlm + g, kp = rlpos[ll], lst = ll - (rowm[kp].loff - L0);
             const int pi = rbase + kp, i = pi + 1, j = i + d, pj = j + 1;
             const PosMeta mpj = colm[pj - cbase], mpj1 = colm[pj + 1 - cbase];
-            if (c >= mpj1.sig) continue;
-            const Scr sc = scr_of(scrb, dm, i - clo);
-            double v = 0.0;
-            for (int k = 0; k < mpj.nR; ++k)
-              if (rs_c[mpj.roff + k] == c) v += sc.Y[lst * MR + k];
-            b.D1[(size_t)(rowm[kp].loff + lst) * S + mpj1.off + c] = v;
+            const double* y = scr_of(scrb, dm, i - clo).Y + lst * MR;
+            double* out = b.D1 + (size_t)(rowm[kp].loff + lst) * S + mpj1.off;
+            for (int c = 0; c < mpj1.sig; ++c) {
+              double v = 0.0;
+              for (int k = 0; k < mpj.nR; ++k)
+                if (rs_c[mpj.roff + k] == c) v += y[k];
+              out[c] = v;
+            }
+          } else {
+            const int rr = rbm + (g - nlm), kp = rbpos[rr], a = rr - crow[kp];
+            const int pi = rbase + kp, i = pi + 1, j = i + d, pj = j + 1;
+            const PosMeta mpi = rowm[kp], mpj = colm[pj - cbase], mpj1 = colm[pj + 1 - cbase];
+            const double* y = scr_of(scrb, dm, i - clo).Y;
+            // left states with bond a are contiguous in the (a, x)-sorted list
+            int l0 = 0, l1 = 0;
+            for (int l = 0; l < mpi.nL; ++l) {
+              const int la = ls_a[mpi.loff + l];
+              l0 += la < a;
+              l1 += la <= a;
+            }
+            double gi[CDZ_MAX_BOND];
+#pragma unroll
+            for (int c = 0; c < CDZ_MAX_BOND; ++c) gi[c] = 0.0;
+            for (int k = 0; k < mpj.nR; ++k) {
+              double v = 0.0;
+              for (int l = l0; l < l1; ++l) v += y[l * MR + k];
+              b.D2T[(size_t)(mpj.roff + k) * S + mpi.off + a] = v;
+              const int c = rs_c[mpj.roff + k];
+#pragma unroll
+              for (int cc = 0; cc < CDZ_MAX_BOND; ++cc) gi[cc] += cc == c ? v : 0.0;
+            }
+            double* out = b.GI + (size_t)(mpi.off + a) * S + mpj1.off;
+#pragma unroll
+            for (int c = 0; c < CDZ_MAX_BOND; ++c)
+              if (c < mpj1.sig) out[c] = gi[c];
           }
         }
       }
