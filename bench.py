@@ -276,8 +276,8 @@ def run_cdz(args):
                                     "45/2250 = %s" % (None if bf16 is None else round(bf16 * 45.0 / 2250.0, 2)),
                      "share_of_step": gemm_ms / ms_step}
     # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch near block diagonal D = 100 of this workload, from the
-    # single-pass ncu capture summarised in profiles/r1z_launches.md (only meaningful for config 4 at full length)
-    ncu_traffic = {"gemm": 1880975360 + 19477760, "block": 244755200 + 120663552} if (cfg == 4 and not args.L) else {}
+    # single-pass ncu capture summarised in profiles/r1f_launches.md (only meaningful for config 4 at full length)
+    ncu_traffic = {"gemm": 1900156160 + 0, "block": 367922432 + 0} if (cfg == 4 and not args.L) else {}
     if roof_gemm:
         roof_gemm["traffic"] = ncu_traffic.get("gemm")
         roof_gemm["traffic_note"] = "one launch at D~100 (574 CTAs, 0.61 ms): no operand reuse across a block diagonal"
