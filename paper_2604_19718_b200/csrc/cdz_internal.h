@@ -136,11 +136,16 @@ struct cdz_tables {
 // number of K-splits of the split-point GEMM on block diagonal D (B designs advanced together)
 inline int cdz_nsplit(int NB, int D, int B) {
   if (D < 2) return 0;
+  // 64x64 tiles, 3 CTAs per SM by shared memory: one wave = 444 CTAs.  With s splits the launch takes
+  // ceil(nblk * s / 444) waves of K/s each: take the s <= 16 that minimises waves / s (smallest s on ties).
   const int nblk = (NB - D) * B, ks = D - 1;
-  int s = (444 + nblk - 1) / nblk;
-  if (s > ks) s = ks;
-  if (s > CDZ_MAX_SPLIT) s = CDZ_MAX_SPLIT;
-  return s < 1 ? 1 : s;
+  int best = 1;
+  double bestc = 1e30;
+  for (int s = 1; s <= CDZ_MAX_SPLIT && s <= ks; ++s) {
+    const double c = (double)((nblk * s + 443) / 444) / (double)s;
+    if (c < bestc - 1e-12) { bestc = c; best = s; }
+  }
+  return best;
 }
 
 // ---- internal entry points -----------------------------------------------------------------------
