@@ -12,7 +12,7 @@
 //             Z1 / Z2 (l1 = 1 / l2 = 1 interior loops)
 //         single-lane items: SB (stack, bulge 1), the recursive parts of Qm1 / Qml, E(i,j)
 //   P2  Y   = everything that carries the closing mismatch
-//   P3a IN  = inner[slot][a'][c'];   P3b Qb
+//   P3  Qb  (inner[x,y;a',c'] expanded in place from Bl, Br, SB and Y)
 //   P4  Qbs, Qm1, Qml, M2, Qm (+ transposed copies)  and  DD = dressed extension of Qb(i,j) over [i-1..j+1]
 //   P5  GI, D1, D2T (DD summed over one or both nucleotides)
 // Every band sum is a dot product of two CONTIGUOUS row segments of row-major tables (transposed copies EMT, QBST,
@@ -52,13 +52,13 @@ struct Dims {
   int M, ML, MR, nps;  // bond / left-state / right-state / pair-slot dimensions (strides of the scratch arrays)
   int lgM, lgR, lgP;   // ceil log2 of M, MR, nps (item decoding)
   int pc;              // percell(), filled by the host
-  __host__ __device__ int percell() const { return 6 * M * M + ML * M + M * MR + 2 * ML * MR + 2 * nps * M * M; }
+  __host__ __device__ int percell() const { return 6 * M * M + ML * M + M * MR + 2 * ML * MR + nps * M * M; }
 };
 
 __host__ __device__ inline int clog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
 
 struct Scr {  // scratch of one cell
-  double *XE, *Bl, *Br, *Z1, *Z2, *Y, *SB, *IN, *QBc, *M2s, *R1, *R2;
+  double *XE, *Bl, *Br, *Z1, *Z2, *Y, *SB, *QBc, *M2s, *R1, *R2;
 };
 __device__ __forceinline__ Scr scr_of(double* base, const Dims& D, int ci) {
   double* s = base + ci * D.pc;
@@ -74,8 +74,7 @@ __device__ __forceinline__ Scr scr_of(double* base, const Dims& D, int ci) {
   k.Z2 = s; s += D.M * D.MR;
   k.Y = s; s += D.ML * D.MR;
   k.QBc = s; s += D.ML * D.MR;
-  k.SB = s; s += D.nps * MM;
-  k.IN = s;
+  k.SB = s;
   return k;
 }
 
@@ -245,7 +244,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   const int tid = threadIdx.x, NT = blockDim.x;
   const int n = t.n, MS = t.MS, MS2 = MS * MS;
   const size_t S = (size_t)t.S, RS = (size_t)t.RS;
-  const int M = dm.M, ML = dm.ML, MR = dm.MR, nps = dm.nps, MM = M * M;
+  const int M = dm.M, ML = dm.ML, MR = dm.MR, nps = dm.nps;
   const int lgM = dm.lgM, lgR = dm.lgR;
   const int Mp = 1 << lgM, MRp = 1 << lgR;
 
@@ -699,32 +698,6 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           sc.Y[lst * MR + r] = y;
         }
         __syncthreads();
-        // ================= P3a: inner[slot][a'][c'] ======================================================================
-        const int npm3 = nps << lgM;
-        for (int it0 = tid; it0 < nb1 * npm3; it0 += NT) {
-          const int rq = it0 / npm3, it = it0 - rq * npm3;
-          const int c1 = it & (Mp - 1), sl = it >> lgM, rr = rb1 + rq;
-          const int kp = rbpos[rr], a1 = rr - crow[kp];
-          const int p = rbase + kp, i = p - 1, j = i + d, q = j - 1;
-          const PosMeta mj = colm[j - cbase];
-          if (c1 >= mj.sig || !(pmx[rowm[kp - 1].nuc] & mj.nuc)) continue;
-          const PosMeta mp = rowm[kp], mq = colm[q - cbase];
-          const Scr sc = scr_of(scrb, dm, i - clo);
-          // inner[slot] is read by Qb(i,j) only for slots whose nucleotides occur at i and j
-          if (!((rowm[kp - 1].nuc >> cm.slot_x[sl]) & 1) || !((mj.nuc >> cm.slot_y[sl]) & 1)) continue;
-          const int P = cm.ptype[cm.slot_x[sl] * 4 + cm.slot_y[sl]];
-          double v = sc.Bl[a1 * M + c1] + sc.Br[a1 * M + c1];
-          for (int l = 0; l < mp.nL; ++l) {
-            if (ls_a[mp.loff + l] != a1) continue;
-            const int u = ls_x[mp.loff + l];
-            for (int k = 0; k < mq.nR; ++k)
-              if (rs_c[mq.roff + k] == c1) v += cm.wtm[P][u][rs_y[mq.roff + k]] * sc.Y[l * MR + k];
-          }
-          for (int s2 = 0; s2 < nps; ++s2)
-            v += cm.wst[P][cm.ptype[cm.slot_x[s2] * 4 + cm.slot_y[s2]]] * sc.SB[(a1 * nps + s2) * M + c1];
-          sc.IN[(sl * M + a1) * M + c1] = v;
-        }
-        __syncthreads();
       }
       CDZ_TICK(3);
       // ================= P3b: Qb[(a,x)][(y,c)] = can(x,y) sum T_i[a,x,a'] T_j[c',y,c] inner ============================
@@ -739,17 +712,33 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           const Scr sc = scr_of(scrb, dm, i - clo);
           double v = 0.0;
           if (closed) {
-            const int sl = cm.pslot[ls_x[rowm[kp].loff + lst] * 4 + rs_y[mj.roff + r]];
-            if (sl >= 0) {
-              const int S1 = rowm[kp + 1].sig, S2 = mj.sig;
+            const int x = ls_x[rowm[kp].loff + lst], y = rs_y[mj.roff + r];
+            if (cm.pslot[x * 4 + y] >= 0) {
+              // Qb = sum_{a',c'} T_i[a,x,a'] T_j[c',y,c] inner[x,y;a',c'] with inner expanded in place (no per-slot table):
+              //   inner = Bl + Br + sum_slots wst[P][P'] SB[a'][slot'][c']  +  sum_{(a',u),(v,c')} wtm[P][u][v] Y[(a',u)][(v,c')]
+              const int P = cm.ptype[x * 4 + y];
+              const PosMeta mp = rowm[kp + 1], mq = colm[j - 1 - cbase];
+              const int S1 = mp.sig, S2 = mj.sig;
               const double* TLi = TLs + ((i - tlbase) * ML + lst) * M;
               const double* TRj = TRs + (size_t)(j - trbase) * M * MR + r;
-              const double* IN = sc.IN + sl * MM;
               for (int a1 = 0; a1 < S1; ++a1) {
                 const double tl = TLi[a1];
                 if (tl == 0.0) continue;
+                for (int c1 = 0; c1 < S2; ++c1) {
+                  const double tr = TRj[c1 * MR];
+                  if (tr == 0.0) continue;
+                  double s = sc.Bl[a1 * M + c1] + sc.Br[a1 * M + c1];
+                  for (int s2 = 0; s2 < nps; ++s2)
+                    s += cm.wst[P][cm.ptype[cm.slot_x[s2] * 4 + cm.slot_y[s2]]] * sc.SB[(a1 * nps + s2) * M + c1];
+                  v += tl * tr * s;
+                }
+              }
+              for (int l = 0; l < mp.nL; ++l) {
+                const double tl = TLi[ls_a[mp.loff + l]];
+                if (tl == 0.0) continue;
+                const int u = ls_x[mp.loff + l];
                 double s = 0.0;
-                for (int c1 = 0; c1 < S2; ++c1) s += TRj[c1 * MR] * IN[a1 * M + c1];
+                for (int k = 0; k < mq.nR; ++k) s += TRj[rs_c[mq.roff + k] * MR] * cm.wtm[P][u][rs_y[mq.roff + k]] * sc.Y[l * MR + k];
                 v += tl * s;
               }
             }
