@@ -276,8 +276,8 @@ def run_cdz(args):
                                     "45/2250 = %s" % (None if bf16 is None else round(bf16 * 45.0 / 2250.0, 2)),
                      "share_of_step": gemm_ms / ms_step}
     # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch near block diagonal D = 100 of this workload, from the
-    # single-pass ncu capture summarised in profiles/r1g_launches.md (only meaningful for config 4 at full length)
-    ncu_traffic = {"gemm": 1908359680 + 0, "block": 377759744 + 0} if (cfg == 4 and not args.L) else {}
+    # single-pass ncu capture summarised in profiles/r1h_launches.md (only meaningful for config 4 at full length)
+    ncu_traffic = {"gemm": 1908146432 + 0, "block": 376736768 + 0} if (cfg == 4 and not args.L) else {}
     if roof_gemm:
         roof_gemm["traffic"] = ncu_traffic.get("gemm")
         roof_gemm["traffic_note"] = "one launch at D~100: no operand reuse across a block diagonal"
