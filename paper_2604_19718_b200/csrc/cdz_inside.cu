@@ -281,13 +281,37 @@ __global__ void __launch_bounds__(256) ext_kernel(const Ctx* ctxs, int K) {
     const int r = e / CDZ_TB, c = e % CDZ_TB;
     Dg[r * (CDZ_TB + 1) + c] = b.QBS[(size_t)(base + r) * S + base + c];
   }
-  if (threadIdx.x < CDZ_TB) qx[threadIdx.x] = 0.0;
+  // everything the serial in-block recursion reads from global memory is staged first (it is a chain of ~64 dependent steps)
+  __shared__ double Rs[CDZ_TB];                                  // accumulated contributions of the earlier block rows
+  __shared__ double Tbs[(CDZ_TB + CDZ_MAX_BOND) * CDZ_MAX_BOND];  // Tbar of positions p0-1 .. p1-2, compact: Sigma_pos x Sigma_{pos+1} each
+  __shared__ int tof[CDZ_TB + 2];                                // their offsets in Tbs
+  __shared__ double qprev[CDZ_MAX_BOND];                         // Qext of the last position of the previous block
+  __shared__ int sg[CDZ_TB + 2], of[CDZ_TB + 2];                 // sigma / offset of positions p0-1 .. p1-1
+  const int p0 = t.blk_start[K], p1 = min(t.blk_start[K + 1], n + 1);
+  if (threadIdx.x < CDZ_TB) { qx[threadIdx.x] = 0.0; Rs[threadIdx.x] = b.R[base + threadIdx.x]; }
+  for (int k = threadIdx.x; k <= p1 - p0; k += blockDim.x) {
+    const int pos = p0 - 1 + k;
+    sg[k] = pos >= 0 ? t.sig[pos] : 0;
+    of[k] = pos >= 0 ? t.off[pos] : 0;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int acc = 0;
+    for (int k = 0; k < p1 - p0; ++k) { tof[k] = acc; acc += sg[k] * sg[k + 1]; }
+  }
+  __syncthreads();
+  for (int k = threadIdx.x / 64; k < p1 - p0; k += blockDim.x / 64) {  // 64 lanes per position
+    const int pos = p0 - 1 + k, Sa = sg[k], Sc = sg[k + 1];
+    for (int e = threadIdx.x % 64; e < Sa * Sc; e += 64)
+      Tbs[tof[k] + e] = pos >= 0 ? t.Tbar[((size_t)pos * MS + e / Sc) * MS + e % Sc] : 0.0;
+  }
+  if (threadIdx.x < CDZ_MAX_BOND) qprev[threadIdx.x] = (p0 >= 1 && threadIdx.x < t.sig[p0 - 1]) ? b.Qext[t.off[p0 - 1] + threadIdx.x] : 0.0;
   __syncthreads();
   if (threadIdx.x < 32) {
     const int lane = threadIdx.x;
-    const int p0 = t.blk_start[K], p1 = min(t.blk_start[K + 1], n + 1);
     for (int jj = p0; jj < p1; ++jj) {
-      const int Sj = t.sig[jj], oj = t.off[jj] - base;
+      const int kk = jj - p0 + 1;  // index of position jj in sg / of; position jj-1 is kk-1
+      const int Sj = sg[kk], oj = of[kk] - base;
       for (int c = 0; c < Sj; ++c) {
         double v = 0.0;
         if (jj == 0) {
@@ -295,11 +319,12 @@ __global__ void __launch_bounds__(256) ext_kernel(const Ctx* ctxs, int K) {
         } else {
           double part = qx[lane] * Dg[lane * (CDZ_TB + 1) + oj + c] + qx[lane + 32] * Dg[(lane + 32) * (CDZ_TB + 1) + oj + c];
           for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-          v = b.R[base + oj + c] + part;
-          const int Sp = t.sig[jj - 1], op = t.off[jj - 1];
+          v = Rs[oj + c] + part;
+          const int Sp = sg[kk - 1], op = of[kk - 1];
+          const double* Tb = Tbs + tof[kk - 1];
           for (int s = 0; s < Sp; ++s) {
-            const double q = op >= base ? qx[op - base + s] : b.Qext[op + s];
-            v += q * t.Tbar[((size_t)(jj - 1) * MS + s) * MS + c];
+            const double q = op >= base ? qx[op - base + s] : qprev[s];
+            v += q * Tb[s * Sj + c];
           }
         }
         __syncwarp();
@@ -413,7 +438,7 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
   zero_kernel<<<dim3(32, B), 256, 0, st>>>(d_ctxs);
   for (int K = 0; K < NBmax; ++K) {
     const int rem = Smax - (K + 1) * CDZ_TB;
-    const int gx = std::max(1, std::min(148, (rem + 511) / 512));
+    const int gx = std::max(1, std::min(296, (rem + 255) / 256));  // one column per thread: the push part is latency-bound
     ext_kernel<<<dim3(gx, B), 256, 0, st>>>(d_ctxs, K);
   }
   mark(7, 0);  // closing event
