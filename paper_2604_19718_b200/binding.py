@@ -243,15 +243,14 @@ class Tables:
         return seq, pair
 
     def marginals(self, stream=None):
+        """cdz_marginals: base-pair probabilities [n][n] (upper triangle P(i.j), diagonal P(i unpaired)) by the outside pass.
+        Base and codon marginals are not built yet (the C call rejects non-NULL buffers for them)."""
         import torch
 
         n = self.n
         bpp = torch.zeros((n, n), dtype=torch.float64, device="cuda")
-        base = torch.zeros((n, 4), dtype=torch.float64, device="cuda")
-        codon = torch.zeros((n // 3, 64), dtype=torch.float64, device="cuda")
-        _check(lib().cdz_marginals(self.h, C.c_void_p(bpp.data_ptr()), C.c_void_p(base.data_ptr()),
-                                   C.c_void_p(codon.data_ptr()), _stream_ptr(stream)))
-        return bpp, base, codon
+        _check(lib().cdz_marginals(self.h, C.c_void_p(bpp.data_ptr()), None, None, _stream_ptr(stream)))
+        return bpp
 
     def run_host(self, J: int, seed: int, seq_host=None, pair_host=None, stream=None) -> float:
         """cdz_run_host: host buffers in / out (pinned torch tensors or numpy arrays), returns log Z."""

@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libcdz.so")
-SOURCES = ["cdz_host.cu", "cdz_inside.cu", "cdz_cell.cu", "cdz_sample.cu", "cdz_peak.cu"]
+SOURCES = ["cdz_host.cu", "cdz_inside.cu", "cdz_cell.cu", "cdz_outside.cu", "cdz_sample.cu", "cdz_peak.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "--expt-relaxed-constexpr", "--extended-lambda",

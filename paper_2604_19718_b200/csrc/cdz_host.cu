@@ -685,9 +685,14 @@ extern "C" int cdz_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev,
 }
 
 extern "C" int cdz_marginals(cdz_tables* t, double* bpp_dev, double* base_dev, double* codon_dev, void* stream) {
-  (void)t; (void)bpp_dev; (void)base_dev; (void)codon_dev; (void)stream;
-  cdz_set_error("cdz_marginals: outside pass not implemented yet");
-  return CDZ_ESTATE;
+  if (!t) { cdz_set_error("cdz_marginals: null handle"); return CDZ_EINVAL; }
+  if (!t->done) { cdz_set_error("cdz_marginals before cdz_inside"); return CDZ_ESTATE; }
+  if (base_dev || codon_dev) {
+    cdz_set_error("cdz_marginals: base / codon marginals are not implemented yet (pass NULL); base-pair probabilities are");
+    return CDZ_ESTATE;
+  }
+  if (!bpp_dev) return CDZ_OK;
+  return cdz_launch_outside(t, bpp_dev, (cudaStream_t)stream);
 }
 
 extern "C" int cdz_run_host(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_host, int32_t* pair_host,

@@ -154,6 +154,7 @@ struct cdz_cell_cfg { int M, ML, MR, nps, maxpos, span, C; size_t smem; };
 int cdz_cell_config(cdz_tables* const* ts, int B, cdz_cell_cfg* cfg);
 void cdz_launch_cells(const Ctx* d_ctxs, int B, int nblk, int D, int nsplit, const cdz_cell_cfg* cfg, cudaStream_t st);
 int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st);
+int cdz_launch_outside(cdz_tables* t, double* bpp_dev, cudaStream_t st);
 int cdz_launch_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* pair_dev, cudaStream_t st);
 
 #define CDZ_CUDA(call)                                                                       \
