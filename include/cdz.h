@@ -152,9 +152,12 @@ int cdz_tables_logqext(cdz_tables* t, int j, int c, double* out_host);
 int cdz_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* pair_dev, void* stream);
 
 /* ---- marginals (device) ---------------------------------------------------- */
-/* bpp_dev [n][n]: upper triangle P(i.j) (eq 2.5), diagonal P(i unpaired); base_dev [n][4] (eq 2.6);
- * codon_dev [L][64] (eq 2.7).  Any may be NULL.
- * NOT BUILT YET (needs the outside / adjoint pass): always returns CDZ_ESTATE and writes nothing. */
+/* Outside (adjoint) pass over the tables of a finished inside pass (eq 2.5 line 85, eq 4.1; DESIGN.md
+ * section 9).  bpp_dev: device, [n][n] doubles, caller-owned, fully overwritten: upper triangle P(i.j), diagonal
+ * P(i unpaired), lower triangle 0.  May be NULL (no work).  The adjoint workspace is allocated and freed inside the call
+ * (CDZ_ENOMEM if it does not fit); the call synchronises `stream` before it returns.
+ * base_dev [n][4] (eq 2.6) and codon_dev [L][64] (eq 2.7) are NOT BUILT YET: they must be NULL, otherwise the call returns
+ * CDZ_ESTATE and writes nothing.  CDZ_ESTATE also before cdz_inside. */
 int cdz_marginals(cdz_tables* t, double* bpp_dev, double* base_dev, double* codon_dev, void* stream);
 
 /* ---- convenience: host buffers end to end (used for the e2e timing) -------- */
