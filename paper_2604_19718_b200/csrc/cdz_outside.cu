@@ -16,12 +16,14 @@
 //   G(i,j)[a',u,v,c'] = sum_{x,y} I(i,j)[x,y;a',c'] e^{-beta tmm[p(x,y)][u][v]}  (closing mismatch applied once per cell).
 // All tables are the scaled ones the inside pass leaves behind: scaling every core by a power of two is a change of the
 // operator weights under which the recursion is unchanged, and the probabilities are ratios.
-// This first version is a plain gather (one CTA per cell, one launch per diagonal, no tensor cores): correct, not fast.
+// This version is a plain gather (one CTA per cell, one launch per diagonal, no tensor cores); the interior-loop term is
+// factored over the operator pair next to the inner pair (one warp per operator pair, lane = l1).
 #include "cdz_internal.h"
 
 namespace {
 
 constexpr int OT = 256;    // threads per CTA
+constexpr int OPV = 1024;   // operator pairs (z2 at k-1, z1' at l+1) per pass of the interior-loop term
 constexpr int ORING = 34;  // diagonals of I / G kept: a closing pair lies at most 32 diagonals above its inner pair
 
 struct Adj {
@@ -101,12 +103,14 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   const int nent = Si * Sj1;
   __shared__ double part[OT];
   __shared__ double am[64], aml[64], abs_[64], ab[256], ibs[16 * 64];
-  __shared__ uint8_t lp1[512], lp2[512];
+  __shared__ uint8_t lp1[128], lp2[128];
+  __shared__ double pv[OPV];
   __shared__ int nlp;
   if (tid == 0) {
     int c = 0;
     for (int l1 = 0; l1 <= m.max_interior; ++l1)
-      for (int l2 = 0; l1 + l2 <= m.max_interior; ++l2) { lp1[c] = (uint8_t)l1; lp2[c] = (uint8_t)l2; ++c; }
+      for (int l2 = 0; l1 + l2 <= m.max_interior; ++l2)
+        if (l1 == 0 || l2 == 0) { lp1[c] = (uint8_t)l1; lp2[c] = (uint8_t)l2; ++c; }  // stack + bulges; interior loops below
     nlp = c;
   }
   const int ngrp = OT / nent, e = tid % nent, grp = tid / nent;
@@ -175,6 +179,64 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   const int k = i, l = j;
   const int nL = t.loff[k + 1] - t.loff[k], nR = t.roff[l + 1] - t.roff[l], npair = nL * nR;
   const bool closable = d >= m.min_hairpin + 1;
+  // ---- interior loops l1, l2 >= 1 of the closing pairs (i0,j0) = (k-1-l1, l+1+l2), factored over the operator pair (z2 at k-1, z1' at l+1):
+  //   pv[z2,z1'] = sum_{l1,l2} win[l1+l2] sum_{z1 at i0+1, z2' at j0-1} x_z1 E(i0+2,k-2)[c(z1),a(z2)] E(l+2,j0-2)[c(z1'),a(z2')] x_z2'
+  //                                       G(i0,j0)[a(z1),b(z1),b(z2'),c(z2')]
+  //   Qb-bar(k,l)[s,x',y',t] += sum_{z2: c = s} sum_{z1': a = t} e^{-beta tmm[p(y',x')][b(z1')][b(z2)]} x_z2 x_z1' pv[z2,z1']
+  // One warp per operator pair, lane = l1 - 1, fixed-order shuffle tree: deterministic.
+  double accI = 0.0;
+  if (closable && k >= 2 && l + 2 <= n - 1) {
+    const int e2 = tid % npair;
+    const int ll = e2 / nR, rr = e2 % nR;
+    const int s = t.ls_a[t.loff[k] + ll], xp = t.ls_x[t.loff[k] + ll];
+    const int yp = t.rs_y[t.roff[l] + rr], tt_ = t.rs_c[t.roff[l] + rr];
+    const bool mine = tid < npair && m.pslot[xp * 4 + yp] >= 0;
+    const int Pin_il = m.ptype[yp * 4 + xp];
+    const int z2b = t.opstart[k - 1], z1pb = t.opstart[l + 1], nz1p = t.opstart[l + 2] - z1pb;
+    const int npv = (t.opstart[k] - z2b) * nz1p;
+    const int warp = tid >> 5, lane = tid & 31;
+    for (int base = 0; base < npv; base += OPV) {
+      const int cnt = min(OPV, npv - base);
+      for (int p = warp; p < cnt; p += OT / 32) {
+        const int z2 = z2b + (base + p) / nz1p, z1p = z1pb + (base + p) % nz1p;
+        double v = 0.0;
+        for (int l1 = 1 + lane; l1 < m.max_interior; l1 += 32) {
+          const int i0 = k - 1 - l1;
+          if (i0 < 0) break;
+          const int z1lo = l1 == 1 ? z2 : t.opstart[i0 + 1], z1hi = l1 == 1 ? z2 + 1 : t.opstart[i0 + 2];
+          for (int l2 = 1; l1 + l2 <= m.max_interior; ++l2) {
+            const int j0 = l + 1 + l2;
+            if (j0 > n - 1) break;
+            const int z2lo = l2 == 1 ? z1p : t.opstart[j0 - 1], z2hi = l2 == 1 ? z1p + 1 : t.opstart[j0];
+            const double* G = A.G + ((size_t)((j0 - i0) % ORING) * n + i0) * 16 * MS2;
+            double in = 0.0;
+            for (int z1 = z1lo; z1 < z1hi; ++z1) {
+              const double wl = l1 == 1 ? 1.0 : t.op_x[z1] * V.E(i0 + 2, k - 2, t.op_c[z1], t.op_a[z2]);
+              if (wl == 0.0) continue;
+              const double* Gz = G + (t.op_b[z1] * 4) * MS2 + t.op_a[z1] * MS;
+              double r = 0.0;
+              for (int z2p = z2lo; z2p < z2hi; ++z2p) {
+                const double wr = l2 == 1 ? 1.0 : V.E(l + 2, j0 - 2, t.op_c[z1p], t.op_a[z2p]) * t.op_x[z2p];
+                r += wr * Gz[t.op_b[z2p] * MS2 + t.op_c[z2p]];
+              }
+              in += wl * r;
+            }
+            v += m.win[l1 + l2] * in;
+          }
+        }
+        for (int o = 16; o; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (lane == 0) pv[p] = v;
+      }
+      __syncthreads();
+      if (mine)
+        for (int p = 0; p < cnt; ++p) {
+          const int z2 = z2b + (base + p) / nz1p, z1p = z1pb + (base + p) % nz1p;
+          if (t.op_c[z2] != s || t.op_a[z1p] != tt_) continue;
+          accI += m.wtm[Pin_il][t.op_b[z1p]][t.op_b[z2]] * t.op_x[z2] * t.op_x[z1p] * pv[p];
+        }
+      __syncthreads();
+    }
+  }
   {
     const int ng2 = OT / npair, e2 = tid % npair, g2 = tid / npair;
     const int ll = e2 / nR, rr = e2 % nR;
@@ -184,7 +246,6 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     double acc = 0.0;
     if (g2 < ng2 && closable && pairable) {
       const int Pin_st = m.ptype[xp * 4 + yp];  // inner pair as (phi_k, phi_l): stacks and size-1 bulges
-      const int Pin_il = m.ptype[yp * 4 + xp];  // inner pair seen from the loop, (phi_l, phi_k): interior mismatch
       for (int q = g2; q < nlp; q += ng2) {
         const int l1 = lp1[q], l2 = lp2[q];
         const int i0 = k - 1 - l1, j0 = l + 1 + l2;
@@ -192,7 +253,6 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
         const int dd = j0 - i0;
         const int Sa = t.sig[i0 + 1], Sc = t.sig[j0];
         const double* ib = A.IB + ((size_t)(dd % ORING) * n + i0) * 16 * MS2;
-        const double* G = A.G + ((size_t)(dd % ORING) * n + i0) * 16 * MS2;
         if (l1 == 0 && l2 == 0) {
           for (int sl = 0; sl < m.nps; ++sl)
             acc += m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][Pin_st] * ib[sl * MS2 + s * MS + tt_];
@@ -212,39 +272,13 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
             for (int c = 0; c < Sc; ++c) v += ib[sl * MS2 + s * MS + c] * V.E(l + 1, j0 - 1, tt_, c);
             acc += w * v;
           }
-        } else {
-          // interior loop: Up(i0+1,k-1)[a',u,u',s] G[a',u,v,c'] Up(l+1,j0-1)[t,v',v,c'] e^{-beta tmm[p(y',x')][v'][u']}
-          double v = 0.0;
-          for (int z2 = t.opstart[k - 1]; z2 < t.opstart[k]; ++z2) {
-            if (t.op_c[z2] != s) continue;
-            const int up = t.op_b[z2];
-            for (int z1p = t.opstart[l + 1]; z1p < t.opstart[l + 2]; ++z1p) {
-              if (t.op_a[z1p] != tt_) continue;
-              const int vp = t.op_b[z1p];
-              const double wm = m.wtm[Pin_il][vp][up] * t.op_x[z2] * t.op_x[z1p];
-              double in = 0.0;
-              const int z1lo = l1 == 1 ? z2 : t.opstart[i0 + 1], z1hi = l1 == 1 ? z2 + 1 : t.opstart[i0 + 2];
-              const int z2lo = l2 == 1 ? z1p : t.opstart[j0 - 1], z2hi = l2 == 1 ? z1p + 1 : t.opstart[j0];
-              for (int z1 = z1lo; z1 < z1hi; ++z1) {
-                const double wl = l1 == 1 ? 1.0 : t.op_x[z1] * V.E(i0 + 2, k - 2, t.op_c[z1], t.op_a[z2]);
-                if (wl == 0.0) continue;
-                const int ap = t.op_a[z1], u = t.op_b[z1];
-                for (int z2p = z2lo; z2p < z2hi; ++z2p) {
-                  const double wr = l2 == 1 ? 1.0 : V.E(l + 2, j0 - 2, t.op_c[z1p], t.op_a[z2p]) * t.op_x[z2p];
-                  in += wl * wr * G[(u * 4 + t.op_b[z2p]) * MS2 + ap * MS + t.op_c[z2p]];
-                }
-              }
-              v += wm * in;
-            }
-          }
-          acc += m.win[l1 + l2] * v;
         }
       }
     }
     const double v = group_total(part, acc, npair);
     if (tid < npair) {
       double w = 0.0;
-      if (closable && pairable) w = v + abs_[s * Sj1 + tt_];
+      if (closable && pairable) w = v + accI + abs_[s * Sj1 + tt_];
       ab[tid] = w;
       A.AB[(size_t)(t.loff[k] + ll) * RS + t.roff[l] + rr] = w;
       part[tid] = w * b.QB[(size_t)(t.loff[k] + ll) * RS + t.roff[l] + rr];
