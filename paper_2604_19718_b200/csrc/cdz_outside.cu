@@ -27,7 +27,7 @@ constexpr int OPV = 1024;   // operator pairs (z2 at k-1, z1' at l+1) per pass o
 constexpr int ORING = 34;  // diagonals of I / G kept: a closing pair lies at most 32 diagonals above its inner pair
 
 struct Adj {
-  double *AB, *AM2, *AML, *AM1, *AX, *IB, *G;
+  double *AB, *AM2, *AML, *AM1, *AX, *IB, *G, *H;
 };
 
 // Qext-bar, sequential over bond positions k = n .. 0 (one CTA)
@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   __shared__ double part[OT];
   __shared__ double am[64], aml[64], abs_[64], ab[256], ibs[16 * 64];
   __shared__ uint8_t lp1[128], lp2[128];
-  __shared__ double pv[OPV];
+  __shared__ double pv[OPV], pvg[64];
   __shared__ int nlp;
   if (tid == 0) {
     int c = 0;
@@ -195,34 +195,63 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     const int z2b = t.opstart[k - 1], z1pb = t.opstart[l + 1], nz1p = t.opstart[l + 2] - z1pb;
     const int npv = (t.opstart[k] - z2b) * nz1p;
     const int warp = tid >> 5, lane = tid & 31;
+    const int MI = m.max_interior;
+    // l1, l2 >= 2: both side stretches are E products, so the term depends on (z2, z1') only through the bonds a(z2), c(z1'):
+    //   pvg[a2,c1'] = sum_{l1,l2>=2} win[l1+l2] sum_{c1,a2'} E(i0+2,k-2)[c1,a2] H(i0,j0)[c1,a2'] E(l+2,j0-2)[c1',a2']
+    const int Sk1 = t.sig[k - 1], Sl2 = t.sig[l + 2], nentg = Sk1 * Sl2;
+    {
+      const int eg = tid % nentg, gg = tid / nentg, ngg = OT / nentg;
+      const int a2 = eg / Sl2, c1p = eg % Sl2;
+      double acc = 0.0;
+      if (gg < ngg)
+        for (int l1 = 2 + gg; l1 <= MI - 2; l1 += ngg) {
+          const int i0 = k - 1 - l1;
+          if (i0 < 0) break;
+          const int S1 = t.sig[i0 + 2];
+          for (int l2 = 2; l1 + l2 <= MI; ++l2) {
+            const int j0 = l + 1 + l2;
+            if (j0 > n - 1) break;
+            const int S2 = t.sig[j0 - 1];
+            const double* H = A.H + ((size_t)((j0 - i0) % ORING) * n + i0) * MS2;
+            double in = 0.0;
+            for (int c1 = 0; c1 < S1; ++c1) {
+              const double wl = V.E(i0 + 2, k - 2, c1, a2);
+              if (wl == 0.0) continue;
+              double r = 0.0;
+              for (int a2p = 0; a2p < S2; ++a2p) r += H[c1 * MS + a2p] * V.E(l + 2, j0 - 2, c1p, a2p);
+              in += wl * r;
+            }
+            acc += m.win[l1 + l2] * in;
+          }
+        }
+      const double tot = group_total(part, acc, nentg);
+      if (tid < nentg) pvg[tid] = tot;
+    }
     for (int base = 0; base < npv; base += OPV) {
       const int cnt = min(OPV, npv - base);
       for (int p = warp; p < cnt; p += OT / 32) {
         const int z2 = z2b + (base + p) / nz1p, z1p = z1pb + (base + p) % nz1p;
         double v = 0.0;
-        for (int l1 = 1 + lane; l1 < m.max_interior; l1 += 32) {
-          const int i0 = k - 1 - l1;
-          if (i0 < 0) break;
+        for (int it = lane; it < 2 * MI - 3; it += 32) {  // (1, 1..MI-1) and (2..MI-1, 1)
+          const int l1 = it < MI - 1 ? 1 : it - (MI - 1) + 2, l2 = it < MI - 1 ? it + 1 : 1;
+          const int i0 = k - 1 - l1, j0 = l + 1 + l2;
+          if (i0 < 0 || j0 > n - 1) continue;
           const int z1lo = l1 == 1 ? z2 : t.opstart[i0 + 1], z1hi = l1 == 1 ? z2 + 1 : t.opstart[i0 + 2];
-          for (int l2 = 1; l1 + l2 <= m.max_interior; ++l2) {
-            const int j0 = l + 1 + l2;
-            if (j0 > n - 1) break;
-            const int z2lo = l2 == 1 ? z1p : t.opstart[j0 - 1], z2hi = l2 == 1 ? z1p + 1 : t.opstart[j0];
-            const double* G = A.G + ((size_t)((j0 - i0) % ORING) * n + i0) * 16 * MS2;
-            double in = 0.0;
-            for (int z1 = z1lo; z1 < z1hi; ++z1) {
-              const double wl = l1 == 1 ? 1.0 : t.op_x[z1] * V.E(i0 + 2, k - 2, t.op_c[z1], t.op_a[z2]);
-              if (wl == 0.0) continue;
-              const double* Gz = G + (t.op_b[z1] * 4) * MS2 + t.op_a[z1] * MS;
-              double r = 0.0;
-              for (int z2p = z2lo; z2p < z2hi; ++z2p) {
-                const double wr = l2 == 1 ? 1.0 : V.E(l + 2, j0 - 2, t.op_c[z1p], t.op_a[z2p]) * t.op_x[z2p];
-                r += wr * Gz[t.op_b[z2p] * MS2 + t.op_c[z2p]];
-              }
-              in += wl * r;
+          const int z2lo = l2 == 1 ? z1p : t.opstart[j0 - 1], z2hi = l2 == 1 ? z1p + 1 : t.opstart[j0];
+          const double* G = A.G + ((size_t)((j0 - i0) % ORING) * n + i0) * 16 * MS2;
+          double in = 0.0;
+          for (int z1 = z1lo; z1 < z1hi; ++z1) {
+            const double wl = l1 == 1 ? 1.0 : t.op_x[z1] * V.E(i0 + 2, k - 2, t.op_c[z1], t.op_a[z2]);
+            if (wl == 0.0) continue;
+            const double* Gz = G + (t.op_b[z1] * 4) * MS2 + t.op_a[z1] * MS;
+            double r = 0.0;
+            for (int z2p = z2lo; z2p < z2hi; ++z2p) {
+              const double wr = l2 == 1 ? 1.0 : V.E(l + 2, j0 - 2, t.op_c[z1p], t.op_a[z2p]) * t.op_x[z2p];
+              r += wr * Gz[t.op_b[z2p] * MS2 + t.op_c[z2p]];
             }
-            v += m.win[l1 + l2] * in;
+            in += wl * r;
           }
+          v += m.win[l1 + l2] * in;
         }
         for (int o = 16; o; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
         if (lane == 0) pv[p] = v;
@@ -232,7 +261,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
         for (int p = 0; p < cnt; ++p) {
           const int z2 = z2b + (base + p) / nz1p, z1p = z1pb + (base + p) % nz1p;
           if (t.op_c[z2] != s || t.op_a[z1p] != tt_) continue;
-          accI += m.wtm[Pin_il][t.op_b[z1p]][t.op_b[z2]] * t.op_x[z2] * t.op_x[z1p] * pv[p];
+          accI += m.wtm[Pin_il][t.op_b[z1p]][t.op_b[z2]] * t.op_x[z2] * t.op_x[z1p] * (pv[p] + pvg[t.op_a[z2] * Sl2 + t.op_c[z1p]]);
         }
       __syncthreads();
     }
@@ -319,6 +348,22 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       v += ibs[sl * MS2 + r] * m.wtm[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][uv >> 2][uv & 3];
     go[q] = v;
   }
+  // ---- H(i,j)[c1,a2'] = sum_{z1 at i+1: c = c1} sum_{z2' at j-1: a = a2'} x_z1 x_z2' G(i,j)[a(z1),b(z1),b(z2'),c(z2')]
+  //      (both loop-side operators of an interior loop with l1, l2 >= 2 closed by this pair)
+  __syncthreads();
+  double* ho = A.H + ((size_t)(d % ORING) * n + i) * MS2;
+  for (int q = tid; q < MS2; q += OT) {
+    const int c1 = q / MS, a2p = q % MS;
+    double v = 0.0;
+    if (closable && j - 1 > i + 1)
+      for (int z1 = t.opstart[i + 1]; z1 < t.opstart[i + 2]; ++z1) {
+        if (t.op_c[z1] != c1) continue;
+        const double* Gz = go + (t.op_b[z1] * 4) * MS2 + t.op_a[z1] * MS;
+        for (int z2p = t.opstart[j - 1]; z2p < t.opstart[j]; ++z2p)
+          if (t.op_a[z2p] == a2p) v += t.op_x[z1] * t.op_x[z2p] * Gz[t.op_b[z2p] * MS2 + t.op_c[z2p]];
+      }
+    ho[q] = v;
+  }
 }
 
 __global__ void unpaired_kernel(int n, double* __restrict__ bpp) {
@@ -338,7 +383,8 @@ int cdz_launch_outside(cdz_tables* t, double* bpp_dev, cudaStream_t st) {
   const cdz_tt* tt = t->tt;
   const size_t n = tt->n, S = tt->S, LS = tt->LS, RS = tt->RS, MS = tt->MS;
   const size_t nSS = S * S, nAB = LS * RS, nAX = (n + 1) * MS, nR = (size_t)ORING * n * 16 * MS * MS;
-  const size_t total = 3 * nSS + nAB + nAX + 2 * nR;
+  const size_t nH = (size_t)ORING * n * MS * MS;
+  const size_t total = 3 * nSS + nAB + nAX + 2 * nR + nH;
   double* ws = nullptr;
   if (cudaMalloc(&ws, total * sizeof(double)) != cudaSuccess) {
     cudaGetLastError();
@@ -354,6 +400,7 @@ int cdz_launch_outside(cdz_tables* t, double* bpp_dev, cudaStream_t st) {
   A.AX = p; p += nAX;
   A.IB = p; p += nR;
   A.G = p; p += nR;
+  A.H = p; p += nH;
   cudaError_t e = cudaMemsetAsync(ws, 0, total * sizeof(double), st);
   if (e == cudaSuccess) e = cudaMemsetAsync(bpp_dev, 0, n * n * sizeof(double), st);
   if (e == cudaSuccess) {
