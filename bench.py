@@ -244,6 +244,22 @@ def run_cdz(args):
     e2e_s = (time.perf_counter() - t0) / e2e_steps
     e2e_value = whole_job_value(units, world, 1e3 * reduce_max(e2e_s, "cuda"))
 
+    # ---- optional: outside pass (base-pair probabilities) on the tables of the last inside pass; outside the timed step
+    marg = None
+    if args.marginals and rank == 0:
+        tab.rerun(stream)
+        bpp = tab.marginals(stream)  # warm-up (allocates / frees its own workspace)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        bpp = tab.marginals(stream)
+        torch.cuda.synchronize()
+        marg_ms = 1e3 * (time.perf_counter() - t0)
+        up = torch.triu(bpp, 1)
+        marg = {"what": "base-pair probabilities P(i.j), eq 2.5 (cdz_marginals: outside / adjoint pass, DESIGN.md section 9)",
+                "ms": marg_ms, "gpu_launches": n + 2, "expected_pairs": float(up.sum()),
+                "max_row_sum_error": float(((up + up.T).sum(1) + torch.diagonal(bpp) - 1.0).abs().max()),
+                "timing": "host clock around the call (it synchronises the stream before returning), workspace allocation included"}
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -321,6 +337,8 @@ def run_cdz(args):
                 "ms_per_step": 1e3 * e2e_s, "logZ": lz_e2e},
         "clocks": clk,
     }
+    if marg is not None:
+        out["marginals"] = marg
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -414,6 +432,7 @@ def main():
     ap.add_argument("--samples", type=int, default=None)
     ap.add_argument("--oracle-L", type=int, default=None, dest="oracle_L")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--marginals", action="store_true", help="also time cdz_marginals (base-pair probabilities) after the timed steps")
     ap.add_argument("--batch", type=int, default=0, help="configs[4]: number of independent 150-aa designs advanced together")
     args = ap.parse_args()
     if args.impl == "reference":

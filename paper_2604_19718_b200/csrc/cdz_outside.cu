@@ -16,18 +16,19 @@
 //   G(i,j)[a',u,v,c'] = sum_{x,y} I(i,j)[x,y;a',c'] e^{-beta tmm[p(x,y)][u][v]}  (closing mismatch applied once per cell).
 // All tables are the scaled ones the inside pass leaves behind: scaling every core by a power of two is a change of the
 // operator weights under which the recursion is unchanged, and the probabilities are ratios.
-// This version is a plain gather (one CTA per cell, one launch per diagonal, no tensor cores); the interior-loop term is
-// factored over the operator pair next to the inner pair (one warp per operator pair, lane = l1).
+// This version is a plain gather (one CTA per cell, one launch per diagonal, no tensor cores); the interior-loop term goes through
+// per-closing-pair tables H / H1 / H2 (loop-side operators pre-contracted with G), so the inner cell only sums bond-indexed products.
 #include "cdz_internal.h"
 
 namespace {
 
 constexpr int OT = 256;    // threads per CTA
-constexpr int OPV = 1024;   // operator pairs (z2 at k-1, z1' at l+1) per pass of the interior-loop term
-constexpr int ORING = 34;  // diagonals of I / G kept: a closing pair lies at most 32 diagonals above its inner pair
+constexpr int OPV = 1024;   // doubles of the per-operator scratch of the interior-loop term
+constexpr int OZC = OPV / CDZ_MAX_BOND;  // operators per pass
+constexpr int ORING = 34;  // diagonals of I / G / H / H1 / H2 kept: a closing pair lies at most 32 diagonals above its inner pair
 
 struct Adj {
-  double *AB, *AM2, *AML, *AM1, *AX, *IB, *G, *H;
+  double *AB, *AM2, *AML, *AM1, *AX, *IB, *G, *H, *H1, *H2;
 };
 
 // Qext-bar, sequential over bond positions k = n .. 0 (one CTA)
@@ -179,11 +180,11 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   const int k = i, l = j;
   const int nL = t.loff[k + 1] - t.loff[k], nR = t.roff[l + 1] - t.roff[l], npair = nL * nR;
   const bool closable = d >= m.min_hairpin + 1;
-  // ---- interior loops l1, l2 >= 1 of the closing pairs (i0,j0) = (k-1-l1, l+1+l2), factored over the operator pair (z2 at k-1, z1' at l+1):
-  //   pv[z2,z1'] = sum_{l1,l2} win[l1+l2] sum_{z1 at i0+1, z2' at j0-1} x_z1 E(i0+2,k-2)[c(z1),a(z2)] E(l+2,j0-2)[c(z1'),a(z2')] x_z2'
-  //                                       G(i0,j0)[a(z1),b(z1),b(z2'),c(z2')]
-  //   Qb-bar(k,l)[s,x',y',t] += sum_{z2: c = s} sum_{z1': a = t} e^{-beta tmm[p(y',x')][b(z1')][b(z2)]} x_z2 x_z1' pv[z2,z1']
-  // One warp per operator pair, lane = l1 - 1, fixed-order shuffle tree: deterministic.
+  // ---- interior loops l1, l2 >= 1 of the closing pairs (i0,j0) = (k-1-l1, l+1+l2).  With z2 at k-1 and z1' at l+1 the operators next to
+  //      the inner pair,   Qb-bar(k,l)[s,x',y',t] += sum_{z2: c = s} sum_{z1': a = t} e^{-beta tmm[p(y',x')][b(z1')][b(z2)]} x_z2 x_z1' * in(z2,z1'),
+  //      in = win[2] G(k-2,l+2)[a(z2),b(z2),b(z1'),c(z1')]  (1 x 1)  +  pv1[z2,c(z1')]  (l1 = 1)  +  pv2[z1',a(z2)]  (l2 = 1)  +  pvg[a(z2),c(z1')]
+  //      where the loop-side operators of the closing pair were pre-contracted with G by the closing cell (H, H1, H2 below) and the
+  //      unpaired stretches are E products.  Every sum runs in a fixed order: deterministic.
   double accI = 0.0;
   if (closable && k >= 2 && l + 2 <= n - 1) {
     const int e2 = tid % npair;
@@ -193,8 +194,6 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     const bool mine = tid < npair && m.pslot[xp * 4 + yp] >= 0;
     const int Pin_il = m.ptype[yp * 4 + xp];
     const int z2b = t.opstart[k - 1], z1pb = t.opstart[l + 1], nz1p = t.opstart[l + 2] - z1pb;
-    const int npv = (t.opstart[k] - z2b) * nz1p;
-    const int warp = tid >> 5, lane = tid & 31;
     const int MI = m.max_interior;
     // l1, l2 >= 2: both side stretches are E products, so the term depends on (z2, z1') only through the bonds a(z2), c(z1'):
     //   pvg[a2,c1'] = sum_{l1,l2>=2} win[l1+l2] sum_{c1,a2'} E(i0+2,k-2)[c1,a2] H(i0,j0)[c1,a2'] E(l+2,j0-2)[c1',a2']
@@ -227,41 +226,76 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       const double tot = group_total(part, acc, nentg);
       if (tid < nentg) pvg[tid] = tot;
     }
-    for (int base = 0; base < npv; base += OPV) {
-      const int cnt = min(OPV, npv - base);
-      for (int p = warp; p < cnt; p += OT / 32) {
-        const int z2 = z2b + (base + p) / nz1p, z1p = z1pb + (base + p) % nz1p;
-        double v = 0.0;
-        for (int it = lane; it < 2 * MI - 3; it += 32) {  // (1, 1..MI-1) and (2..MI-1, 1)
-          const int l1 = it < MI - 1 ? 1 : it - (MI - 1) + 2, l2 = it < MI - 1 ? it + 1 : 1;
-          const int i0 = k - 1 - l1, j0 = l + 1 + l2;
-          if (i0 < 0 || j0 > n - 1) continue;
-          const int z1lo = l1 == 1 ? z2 : t.opstart[i0 + 1], z1hi = l1 == 1 ? z2 + 1 : t.opstart[i0 + 2];
-          const int z2lo = l2 == 1 ? z1p : t.opstart[j0 - 1], z2hi = l2 == 1 ? z1p + 1 : t.opstart[j0];
-          const double* G = A.G + ((size_t)((j0 - i0) % ORING) * n + i0) * 16 * MS2;
-          double in = 0.0;
-          for (int z1 = z1lo; z1 < z1hi; ++z1) {
-            const double wl = l1 == 1 ? 1.0 : t.op_x[z1] * V.E(i0 + 2, k - 2, t.op_c[z1], t.op_a[z2]);
-            if (wl == 0.0) continue;
-            const double* Gz = G + (t.op_b[z1] * 4) * MS2 + t.op_a[z1] * MS;
-            double r = 0.0;
-            for (int z2p = z2lo; z2p < z2hi; ++z2p) {
-              const double wr = l2 == 1 ? 1.0 : V.E(l + 2, j0 - 2, t.op_c[z1p], t.op_a[z2p]) * t.op_x[z2p];
-              r += wr * Gz[t.op_b[z2p] * MS2 + t.op_c[z2p]];
-            }
-            in += wl * r;
-          }
-          v += m.win[l1 + l2] * in;
+    __syncthreads();  // pvg
+    // 1 x 1 loops (closing pair (k-2, l+2): G directly) and the generic part
+    const int nz2 = t.opstart[k] - z2b;
+    if (mine) {
+      const double* G11 = A.G + ((size_t)(((l + 2) - (k - 2)) % ORING) * n + (k - 2)) * 16 * MS2;
+      for (int z2 = z2b; z2 < z2b + nz2; ++z2) {
+        if (t.op_c[z2] != s) continue;
+        for (int z1p = z1pb; z1p < z1pb + nz1p; ++z1p) {
+          if (t.op_a[z1p] != tt_) continue;
+          accI += m.wtm[Pin_il][t.op_b[z1p]][t.op_b[z2]] * t.op_x[z2] * t.op_x[z1p] *
+                  (pvg[t.op_a[z2] * Sl2 + t.op_c[z1p]] +
+                   m.win[2] * G11[(t.op_b[z2] * 4 + t.op_b[z1p]) * MS2 + t.op_a[z2] * MS + t.op_c[z1p]]);
         }
-        for (int o = 16; o; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-        if (lane == 0) pv[p] = v;
+      }
+    }
+    // l1 = 1, l2 >= 2: z1 = z2 carries both left mismatches; the right side is an E product ->
+    //   pv[z2,c1'] = sum_{l2} win[1+l2] sum_{a2'} E(l+2,j0-2)[c1',a2'] H1(k-2,j0)[a(z2),b(z2),a2']
+    for (int zb = 0; zb < nz2; zb += OZC) {
+      const int zc = min(OZC, nz2 - zb);
+      for (int e = tid; e < zc * Sl2; e += OT) {
+        const int z2 = z2b + zb + e / Sl2, c1p = e % Sl2, i0 = k - 2;
+        double v = 0.0;
+        for (int l2 = 2; l2 <= MI - 1; ++l2) {
+          const int j0 = l + 1 + l2;
+          if (j0 > n - 1) break;
+          const double* H1 = A.H1 + ((size_t)((j0 - i0) % ORING) * n + i0) * 4 * MS2 + (t.op_b[z2] * MS + t.op_a[z2]) * MS;
+          const int S2 = t.sig[j0 - 1];
+          double r = 0.0;
+          for (int a2p = 0; a2p < S2; ++a2p) r += V.E(l + 2, j0 - 2, c1p, a2p) * H1[a2p];
+          v += m.win[1 + l2] * r;
+        }
+        pv[e] = v;
       }
       __syncthreads();
       if (mine)
-        for (int p = 0; p < cnt; ++p) {
-          const int z2 = z2b + (base + p) / nz1p, z1p = z1pb + (base + p) % nz1p;
-          if (t.op_c[z2] != s || t.op_a[z1p] != tt_) continue;
-          accI += m.wtm[Pin_il][t.op_b[z1p]][t.op_b[z2]] * t.op_x[z2] * t.op_x[z1p] * (pv[p] + pvg[t.op_a[z2] * Sl2 + t.op_c[z1p]]);
+        for (int z2 = z2b + zb; z2 < z2b + zb + zc; ++z2) {
+          if (t.op_c[z2] != s) continue;
+          for (int z1p = z1pb; z1p < z1pb + nz1p; ++z1p) {
+            if (t.op_a[z1p] != tt_) continue;
+            accI += m.wtm[Pin_il][t.op_b[z1p]][t.op_b[z2]] * t.op_x[z2] * t.op_x[z1p] * pv[(z2 - z2b - zb) * Sl2 + t.op_c[z1p]];
+          }
+        }
+      __syncthreads();
+    }
+    // l2 = 1, l1 >= 2: z2' = z1' carries both right mismatches ->
+    //   pv[z1',a2] = sum_{l1} win[l1+1] sum_{c1} E(i0+2,k-2)[c1,a2] H2(i0,l+2)[c1,b(z1'),c(z1')]
+    for (int zb = 0; zb < nz1p; zb += OZC) {
+      const int zc = min(OZC, nz1p - zb);
+      for (int e = tid; e < zc * Sk1; e += OT) {
+        const int z1p = z1pb + zb + e / Sk1, a2 = e % Sk1, j0 = l + 2;
+        double v = 0.0;
+        for (int l1 = 2; l1 <= MI - 1; ++l1) {
+          const int i0 = k - 1 - l1;
+          if (i0 < 0) break;
+          const double* H2 = A.H2 + ((size_t)((j0 - i0) % ORING) * n + i0) * 4 * MS2 + (t.op_b[z1p] * MS) * MS + t.op_c[z1p];
+          const int S1 = t.sig[i0 + 2];
+          double r = 0.0;
+          for (int c1 = 0; c1 < S1; ++c1) r += V.E(i0 + 2, k - 2, c1, a2) * H2[c1 * MS];
+          v += m.win[l1 + 1] * r;
+        }
+        pv[e] = v;
+      }
+      __syncthreads();
+      if (mine)
+        for (int z1p = z1pb + zb; z1p < z1pb + zb + zc; ++z1p) {
+          if (t.op_a[z1p] != tt_) continue;
+          for (int z2 = z2b; z2 < z2b + nz2; ++z2) {
+            if (t.op_c[z2] != s) continue;
+            accI += m.wtm[Pin_il][t.op_b[z1p]][t.op_b[z2]] * t.op_x[z2] * t.op_x[z1p] * pv[(z1p - z1pb - zb) * Sk1 + t.op_a[z2]];
+          }
         }
       __syncthreads();
     }
@@ -364,6 +398,25 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       }
     ho[q] = v;
   }
+  // ---- H1(i,j)[u,a,a2'] = sum_{z2' at j-1: a = a2'} x_z2' G[a,u,b(z2'),c(z2')]   (l1 = 1: the operator at i+1 stays open)
+  //      H2(i,j)[v,c1,c'] = sum_{z1 at i+1: c = c1} x_z1 G[a(z1),b(z1),v,c']       (l2 = 1: the operator at j-1 stays open)
+  double* h1o = A.H1 + ((size_t)(d % ORING) * n + i) * 4 * MS2;
+  double* h2o = A.H2 + ((size_t)(d % ORING) * n + i) * 4 * MS2;
+  for (int q = tid; q < 8 * MS2; q += OT) {
+    const int which = q / (4 * MS2), r = q % (4 * MS2);
+    const int uv = r / MS2, x1 = (r % MS2) / MS, x2 = r % MS;
+    double v = 0.0;
+    if (closable && j - 1 > i + 1) {
+      if (which == 0) {  // u = uv, a = x1, a2' = x2
+        for (int z2p = t.opstart[j - 1]; z2p < t.opstart[j]; ++z2p)
+          if (t.op_a[z2p] == x2) v += t.op_x[z2p] * go[(uv * 4 + t.op_b[z2p]) * MS2 + x1 * MS + t.op_c[z2p]];
+      } else {  // v = uv, c1 = x1, c' = x2
+        for (int z1 = t.opstart[i + 1]; z1 < t.opstart[i + 2]; ++z1)
+          if (t.op_c[z1] == x1) v += t.op_x[z1] * go[(t.op_b[z1] * 4 + uv) * MS2 + t.op_a[z1] * MS + x2];
+      }
+    }
+    (which == 0 ? h1o : h2o)[r] = v;
+  }
 }
 
 __global__ void unpaired_kernel(int n, double* __restrict__ bpp) {
@@ -378,13 +431,13 @@ __global__ void unpaired_kernel(int n, double* __restrict__ bpp) {
 }  // namespace
 
 // Base-pair probabilities of a finished inside pass: bpp_dev [n][n], upper triangle P(i.j), diagonal P(i unpaired), lower triangle 0.
-// Workspace (4 S x S + LS x RS adjoint tables, 34 diagonals of I / G) is allocated for the call and freed before it returns.
+// Workspace (3 S x S + LS x RS adjoint tables, 34 diagonals of I / G / H / H1 / H2) is allocated for the call and freed before it returns.
 int cdz_launch_outside(cdz_tables* t, double* bpp_dev, cudaStream_t st) {
   const cdz_tt* tt = t->tt;
   const size_t n = tt->n, S = tt->S, LS = tt->LS, RS = tt->RS, MS = tt->MS;
   const size_t nSS = S * S, nAB = LS * RS, nAX = (n + 1) * MS, nR = (size_t)ORING * n * 16 * MS * MS;
   const size_t nH = (size_t)ORING * n * MS * MS;
-  const size_t total = 3 * nSS + nAB + nAX + 2 * nR + nH;
+  const size_t total = 3 * nSS + nAB + nAX + 2 * nR + 9 * nH;
   double* ws = nullptr;
   if (cudaMalloc(&ws, total * sizeof(double)) != cudaSuccess) {
     cudaGetLastError();
@@ -401,6 +454,8 @@ int cdz_launch_outside(cdz_tables* t, double* bpp_dev, cudaStream_t st) {
   A.IB = p; p += nR;
   A.G = p; p += nR;
   A.H = p; p += nH;
+  A.H1 = p; p += 4 * nH;
+  A.H2 = p; p += 4 * nH;
   cudaError_t e = cudaMemsetAsync(ws, 0, total * sizeof(double), st);
   if (e == cudaSuccess) e = cudaMemsetAsync(bpp_dev, 0, n * n * sizeof(double), st);
   if (e == cudaSuccess) {

@@ -74,9 +74,9 @@ def test_bpp_generic_operators_bond_dimension_8(B, O):
     np.testing.assert_allclose(tg.marginals().cpu().numpy(), bo, atol=BPP_ATOL, rtol=0)
 
 
-@pytest.mark.parametrize("cfg,L,J", [(1, 20, 40000), (5, 150, 4000)])
+@pytest.mark.parametrize("cfg,L,J", [(1, 20, 40000), (5, 150, 4000), (2, 300, 2000)])
 def test_bpp_sum_rules_and_sample_frequencies(B, cfg, L, J):
-    """Whole config 1 (60 nt) and config 5 item 0 (450 nt, codon-pair TT): 0 <= P <= 1, rows + unpaired = 1 by construction, every
+    """Whole config 1 (60 nt), config 5 item 0 (450 nt) and config 2 (900 nt, both codon-pair TT): 0 <= P <= 1, rows + unpaired = 1 by construction, every
     P(i.j) within 6 sigma of its frequency among J exact samples, and the expected number of pairs matches the sample mean."""
     m = I.nn_model()
     d = I.design(cfg, 0, L)
