@@ -5,7 +5,7 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = [os.path.join(HERE, f) for f in ("cdz_oracle.c", "cdz_oracle_outside.c")]
+SRC = [os.path.join(HERE, "cdz_oracle.c")]
 OUT = os.path.join(HERE, "libcdz_oracle.so")
 
 

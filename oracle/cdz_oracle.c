@@ -59,8 +59,10 @@ static int distinct_bases(const int* cod, int deg, int pos, int* out) {
   return k;
 }
 
-int orc_tt_build(const char* aa, int L, int kind, const double* codon_logw, const double* pair_logw,
-                 orc_tt** out) {
+/* cw_stride = 0: one codon table [64] for all residues; 64: one table per residue, codon_logw[L][64] (PAPER.md line 157:
+ * the soft constraint penalises codon c "at amino acid position i") */
+static int tt_build_impl(const char* aa, int L, int kind, const double* codon_logw, int cw_stride, const double* pair_logw,
+                         orc_tt** out) {
   if (L <= 0 || !aa || !out) return -1;
   int n = 3 * L;
   orc_tt* tt = (orc_tt*)calloc(1, sizeof(orc_tt));
@@ -87,7 +89,7 @@ int orc_tt_build(const char* aa, int L, int kind, const double* codon_logw, cons
       tt->start[3 * k + 1] = nops;
       for (int t = 0; t < deg; ++t) {
         int b0 = cod[t] >> 4, b1 = (cod[t] >> 2) & 3, b2 = cod[t] & 3;
-        double x = codon_logw ? exp(codon_logw[cod[t]]) : 1.0; /* line 157 */
+        double x = codon_logw ? exp(codon_logw[(size_t)k * cw_stride + cod[t]]) : 1.0; /* line 157 */
         tt->ops[nops++] = (orc_op){rank_in(fb, nf, b0), b1, rank_in(tb, nt, b2), x};
       }
       tt->start[3 * k + 2] = nops;
@@ -106,7 +108,7 @@ int orc_tt_build(const char* aa, int L, int kind, const double* codon_logw, cons
         }
       tt->start[3 * k + 1] = nops;
       for (int c = 0; c < deg; ++c) {
-        double x = codon_logw ? exp(codon_logw[cod[c]]) : 1.0;
+        double x = codon_logw ? exp(codon_logw[(size_t)k * cw_stride + cod[c]]) : 1.0;
         tt->ops[nops++] = (orc_op){c, (cod[c] >> 2) & 3, c, x};
       }
       tt->start[3 * k + 2] = nops;
@@ -119,6 +121,13 @@ int orc_tt_build(const char* aa, int L, int kind, const double* codon_logw, cons
   tt->sigma[n] = (kind == 0) ? 1 : pdeg;
   *out = tt;
   return 0;
+}
+
+int orc_tt_build(const char* aa, int L, int kind, const double* codon_logw, const double* pair_logw, orc_tt** out) {
+  return tt_build_impl(aa, L, kind, codon_logw, 0, pair_logw, out);
+}
+int orc_tt_build_pos(const char* aa, int L, int kind, const double* codon_logw_pos, const double* pair_logw, orc_tt** out) {
+  return tt_build_impl(aa, L, kind, codon_logw_pos, 64, pair_logw, out);
 }
 
 int orc_tt_from_ops(int n, const int* counts, const orc_op* ops, orc_tt** out) {

@@ -48,6 +48,9 @@ typedef struct orc_tables orc_tables;
  * pair_logw[64*64] or NULL (log-weight w means factor e^{+w}). */
 int  orc_tt_build(const char* aa, int L, int kind, const double* codon_logw,
                   const double* pair_logw, orc_tt** out);
+/* same with one codon table per residue, codon_logw_pos[L][64] (line 157: penalty on codon c "at amino acid position i") */
+int  orc_tt_build_pos(const char* aa, int L, int kind, const double* codon_logw_pos,
+                      const double* pair_logw, orc_tt** out);
 int  orc_tt_from_ops(int n, const int* counts, const orc_op* ops, orc_tt** out);
 void orc_tt_free(orc_tt* tt);
 int  orc_tt_n(const orc_tt* tt);
@@ -84,8 +87,7 @@ int orc_sample(const orc_tables* t, int J, uint64_t seed, uint8_t* seq /*[J][n]*
 double orc_uniform(uint64_t seed, uint64_t sample, uint64_t kind, uint64_t i, uint64_t j);
 
 /* ---- marginals, eqs 2.5-2.7 / 4.1-4.3, by their definitions as constrained sums: one inside pass per pair / nucleotide / codon
- *      (O(n^2) passes: small designs only).  Pinned by the brute-force marginals.  No CUDA counterpart exists yet (DESIGN.md
- *      section 9): parity unpinned for marginals. ---- */
+ *      (O(n^2) passes: small designs only).  Pinned by the brute-force marginals (tests/test_oracle_pins.py). ---- */
 int orc_marginals(orc_tables* t, double* bpp /*[n*n]*/, double* base /*[n*4]*/, double* codon /*[L*64]*/);
 
 #ifdef __cplusplus

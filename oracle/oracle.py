@@ -45,6 +45,7 @@ def lib():
         L = C.CDLL(path)
         vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
         L.orc_tt_build.argtypes = [C.c_char_p, C.c_int, C.c_int, dp, dp, C.POINTER(vp)]
+        L.orc_tt_build_pos.argtypes = [C.c_char_p, C.c_int, C.c_int, dp, dp, C.POINTER(vp)]
         L.orc_tt_from_ops.argtypes = [C.c_int, ip, C.POINTER(OrcOp), C.POINTER(vp)]
         L.orc_tt_free.argtypes = [vp]
         L.orc_tt_n.argtypes = [vp]
@@ -103,7 +104,11 @@ class TT:
         h = C.c_void_p()
         cw = np.ascontiguousarray(codon_logw, dtype=np.float64) if codon_logw is not None else None
         pw = np.ascontiguousarray(pair_logw, dtype=np.float64).reshape(-1) if pair_logw is not None else None
-        rc = lib().orc_tt_build(aa.encode(), len(aa), kind, _dp(cw), _dp(pw), C.byref(h))
+        if cw is not None and cw.ndim == 2:
+            assert cw.shape == (len(aa), 64)
+            rc = lib().orc_tt_build_pos(aa.encode(), len(aa), kind, _dp(cw.reshape(-1)), _dp(pw), C.byref(h))
+        else:
+            rc = lib().orc_tt_build(aa.encode(), len(aa), kind, _dp(cw), _dp(pw), C.byref(h))
         if rc != 0:
             raise ValueError(f"orc_tt_build failed rc={rc}")
         return cls(h)

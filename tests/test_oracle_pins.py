@@ -405,3 +405,51 @@ def test_marginals_sum_rules_24nt():
             for b in range(4):
                 sel = np.array([((c >> (2 * (2 - pos))) & 3) == b for c in range(64)])
                 assert abs(codon[k][sel].sum() - base[3 * k + pos, b]) < 1e-12
+
+
+# ---------------------------------------------------------------- decision uniforms, per-position codon weights
+def test_uniform_hash_known_answers():
+    """orc_uniform (SURVEY App. C "decision uniforms") against things other than itself: (a) its first round with seed 0 and
+    v = 0 is SplitMix64's first output for seed 0, the published test vector 0xE220A8397B1DCDAF; (b) every round is one
+    SplitMix64 step from state h + G*v, so the whole hash is a chain of `inputs.SplitMix64` (the generator that
+    test_generator_check_values pins to the values SURVEY App. C prints)."""
+    g = I.SplitMix64(0)
+    assert g.next() == 0xE220A8397B1DCDAF and g.next() == 0x6E789E6AA1B965F4
+
+    def chain(seed, vals):
+        h = seed
+        for v in vals:
+            h = I.SplitMix64((h + I.GOLDEN * v) & I.MASK64).next()
+        return (h >> 11) * 2.0 ** -53
+
+    for seed, vals in ((0, (0, 0, 0, 0)), (1007, (0, 2, 5, 17)), (5007, (255, 8, 449, 0)), (2 ** 63 + 11, (3, 6, 14999, 1))):
+        u = O.uniform(seed, *vals)
+        assert 0.0 <= u < 1.0 and u == chain(seed, vals)
+    # four rounds from seed 0 with v = 0: 0xE220A8397B1DCDAF -> ... -> 0x2130748aaac80268 (computed with Python integers)
+    assert O.uniform(0, 0, 0, 0, 0) == (0x2130748aaac80268 >> 11) * 2.0 ** -53
+
+
+def test_per_position_codon_weights():
+    """orc_tt_build_pos (penalty on codon c 'at amino acid position i'): a per-residue table that repeats one
+    row equals the shared table; adding delta to every codon of ONE residue shifts log Z by exactly delta (every sequence uses
+    exactly one codon there); the weight sum equals direct enumeration."""
+    m = I.tm1_model()
+    aa = "RSLGS"
+    cw = I.tm1_codon_logw()
+    for kind, pw in ((0, None), (1, I.tm1_pair_logw())):
+        base = O.inside(m, O.TT.build(aa, kind, cw, pw)).logZ
+        tiled = np.tile(cw, (len(aa), 1))
+        assert abs(O.inside(m, O.TT.build(aa, kind, tiled, pw)).logZ - base) < 1e-13
+        shifted = tiled.copy()
+        shifted[4] += 0.37  # the second S only
+        assert abs(O.inside(m, O.TT.build(aa, kind, shifted, pw)).logZ - base - 0.37) < 1e-12
+    # distinct rows: sum_phi W(phi) by direct enumeration over codon choices
+    import itertools
+
+    code = "KNKNTTTTRSRSIIMIQHQHPPPPRRRRLLLLEDEDAAAAGGGGVVVV*Y*YSSSS*CWCLFLF"
+    rng = np.random.default_rng(7)
+    cwp = rng.normal(0, 0.5, (4, 64))
+    cods = [[c for c in range(64) if code[c] == a] for a in "RSLG"]
+    tot = sum(math.exp(sum(cwp[k, c] for k, c in enumerate(ch))) for ch in itertools.product(*cods))
+    assert abs(O.TT.build("RSLG", 0, cwp).logsum() - math.log(tot)) < 1e-12
+    assert abs(O.TT.build("RSLG", 1, cwp).logsum() - math.log(tot)) < 1e-12
