@@ -88,11 +88,6 @@ typedef struct {
 const char* cdz_last_error(void);
 int cdz_version(void);
 
-/* Register-resident issue-rate microbenchmark on device 0 (blocking): kind 0 = fp64 FMA, 1 = fp64 mma.sync m8n8k4,
- * 2 = fp32 FMA; TFLOP/s (best of 3 after one warm-up).  Denominators of the fp64 / fp32 rooflines, which
- * MEASURED_PEAKS.json does not hold. */
-int cdz_measure_peak(int kind, double* tflops_out);
-
 /* ---- model ---------------------------------------------------------------- */
 int cdz_model_create(const cdz_nn_params* params, cdz_model** out);
 void cdz_model_destroy(cdz_model* m);
@@ -105,6 +100,9 @@ void cdz_model_destroy(cdz_model* m);
  * pair_logw : [64*64] row = 5' codon (or NULL; CODON_PAIR only): factor on the 5'-base operator (line 163).
  * Open chain: Sigma_0 = 1, the last bond is summed out. */
 int cdz_tt_build(const char* aa, int L, int kind, const double* codon_logw, const double* pair_logw, cdz_tt** out);
+/* Same with one codon table per residue, codon_logw_pos[L][64]: the paper's soft constraint penalises codon c "at amino acid
+ * position i" (line 157); row k applies to residue k only.  NULL = no codon weights. */
+int cdz_tt_build_pos(const char* aa, int L, int kind, const double* codon_logw_pos, const double* pair_logw, cdz_tt** out);
 /* Generic operator lists (lines 545-557, noncoding bases line 573). counts[n], ops[sum counts]. Bond dims <= 8. */
 int cdz_tt_from_operators(int n, const int32_t* counts, const cdz_op* ops, cdz_tt** out);
 void cdz_tt_destroy(cdz_tt* tt);

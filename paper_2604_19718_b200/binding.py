@@ -18,11 +18,11 @@ TT_SINGLE_CODON, TT_CODON_PAIR = 0, 1
 FP64, FP32_SCALED = 0, 1
 
 EXPORTS = [
-    "cdz_last_error", "cdz_version", "cdz_model_create", "cdz_model_destroy", "cdz_tt_build",
+    "cdz_last_error", "cdz_version", "cdz_model_create", "cdz_model_destroy", "cdz_tt_build", "cdz_tt_build_pos",
     "cdz_tt_from_operators", "cdz_tt_destroy", "cdz_tt_length", "cdz_tt_describe", "cdz_workspace_bytes",
     "cdz_inside", "cdz_inside_batch", "cdz_inside_rerun", "cdz_inside_rerun_batch", "cdz_tables_logz",
     "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample",
-    "cdz_marginals", "cdz_run_host", "cdz_set_profiling", "cdz_profile", "cdz_measure_peak",
+    "cdz_marginals", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
 ]
 
 
@@ -73,6 +73,7 @@ def lib():
     L.cdz_model_destroy.argtypes = [vp]
     L.cdz_model_destroy.restype = None
     L.cdz_tt_build.argtypes = [C.c_char_p, C.c_int, C.c_int, dp, dp, C.POINTER(vp)]
+    L.cdz_tt_build_pos.argtypes = [C.c_char_p, C.c_int, C.c_int, dp, dp, C.POINTER(vp)]
     L.cdz_tt_from_operators.argtypes = [C.c_int, C.POINTER(C.c_int32), C.POINTER(Op), C.POINTER(vp)]
     L.cdz_tt_destroy.argtypes = [vp]
     L.cdz_tt_destroy.restype = None
@@ -88,7 +89,6 @@ def lib():
     L.cdz_tables_info.argtypes = [vp, C.POINTER(Info)]
     L.cdz_tables_destroy.argtypes = [vp]
     L.cdz_tables_destroy.restype = None
-    L.cdz_measure_peak.argtypes = [C.c_int, dp]
     L.cdz_set_profiling.argtypes = [vp, C.c_int]
     L.cdz_profile.argtypes = [vp, dp, C.POINTER(C.c_int64)]
     L.cdz_tables_cell.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
@@ -116,13 +116,6 @@ def _stream_ptr(stream):
 
         return C.c_void_p(torch.cuda.current_stream().cuda_stream)
     return C.c_void_p(getattr(stream, "cuda_stream", stream))
-
-
-def measure_peak(kind: int) -> float:
-    """cdz_measure_peak: 0 fp64 FMA, 1 fp64 mma.sync, 2 fp32 FMA (TFLOP/s)."""
-    v = C.c_double()
-    _check(lib().cdz_measure_peak(kind, C.byref(v)))
-    return v.value
 
 
 class Model:
@@ -156,10 +149,16 @@ class TensorTrain:
 
     @classmethod
     def build(cls, aa: str, kind: int, codon_logw=None, pair_logw=None):
+        """codon_logw: [64] (cdz_tt_build) or [L][64] per residue (cdz_tt_build_pos)."""
         cw = np.ascontiguousarray(codon_logw, dtype=np.float64) if codon_logw is not None else None
         pw = np.ascontiguousarray(pair_logw, dtype=np.float64).reshape(-1) if pair_logw is not None else None
         h = C.c_void_p()
-        _check(lib().cdz_tt_build(aa.encode(), len(aa), kind, _dp(cw), _dp(pw), C.byref(h)))
+        if cw is not None and cw.ndim == 2:
+            if cw.shape != (len(aa), 64):
+                raise ValueError("per-position codon weights must have shape [L][64]")
+            _check(lib().cdz_tt_build_pos(aa.encode(), len(aa), kind, _dp(cw.reshape(-1)), _dp(pw), C.byref(h)))
+        else:
+            _check(lib().cdz_tt_build(aa.encode(), len(aa), kind, _dp(cw), _dp(pw), C.byref(h)))
         return cls(h)
 
     @classmethod

@@ -1,34 +1,62 @@
-"""Build libcdz.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a."""
+"""Build libcdz.so (the C-ABI CUDA library) and libcdz_peak.so (bench-only peak microbenchmarks) in-tree with nvcc for sm_100a."""
 from __future__ import annotations
 
 import os
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 OUT = os.path.join(HERE, "libcdz.so")
-SOURCES = ["cdz_host.cu", "cdz_inside.cu", "cdz_cell.cu", "cdz_outside.cu", "cdz_sample.cu", "cdz_peak.cu"]
+OUT_PEAK = os.path.join(HERE, "libcdz_peak.so")
+SOURCES = ["cdz_host.cu", "cdz_inside.cu", "cdz_cell.cu", "cdz_gemm.cu", "cdz_outside.cu", "cdz_usage.cu", "cdz_sample.cu",
+           "cdz_eval.cu"]
+PEAK_SOURCES = ["cdz_peak.cu"]  # not part of the product ABI: register-resident issue-rate loops for bench.py's roofline
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "--expt-relaxed-constexpr", "--extended-lambda",
+    "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "--extended-lambda",
 ]
 
 
-def _deps():
-    d = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".h", ".cuh"))]
+def _headers():
+    d = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))]
     d.append(os.path.join(HERE, "..", "include", "cdz.h"))
     return d
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    srcs = [os.path.join(CSRC, s) for s in SOURCES if os.path.exists(os.path.join(CSRC, s))]
-    if not force and os.path.exists(OUT) and all(os.path.getmtime(OUT) >= os.path.getmtime(d) for d in _deps()):
-        return OUT
+def _compile(src: str, extra, verbose: bool) -> str:
+    obj = os.path.join(OBJ, os.path.basename(src) + ".o")
+    deps = [src] + _headers()
+    if os.path.exists(obj) and all(os.path.getmtime(obj) >= os.path.getmtime(d) for d in deps):
+        return obj
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    extra = os.environ.get("CDZ_NVCC_EXTRA", "").split()  # development only (e.g. -DCDZ_PHASE_TIMING)
-    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", OUT] + srcs + ["-lcudart"]
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
     subprocess.run(cmd, check=True)
-    return OUT
+    return obj
+
+
+def _link(out: str, sources, force: bool, verbose: bool) -> str:
+    srcs = [os.path.join(CSRC, s) for s in sources if os.path.exists(os.path.join(CSRC, s))]
+    extra = os.environ.get("CDZ_NVCC_EXTRA", "").split()  # development only (e.g. -DCDZ_PHASE_TIMING)
+    os.makedirs(OBJ, exist_ok=True)
+    if force or extra:
+        for s in srcs:
+            o = os.path.join(OBJ, os.path.basename(s) + ".o")
+            if os.path.exists(o):
+                os.remove(o)
+    with ThreadPoolExecutor(max_workers=min(8, len(srcs))) as ex:
+        objs = list(ex.map(lambda s: _compile(s, extra, verbose), srcs))
+    if not force and os.path.exists(out) and all(os.path.getmtime(out) >= os.path.getmtime(o) for o in objs):
+        return out
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    subprocess.run([nvcc, "-shared", "-o", out] + objs + ["-lcudart"], check=True)
+    return out
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    _link(OUT_PEAK, PEAK_SOURCES, force, verbose)
+    return _link(OUT, SOURCES, force, verbose)
 
 
 if __name__ == "__main__":

@@ -177,14 +177,15 @@ int finalize_tt(cdz_tt* tt) {
 }
 }  // namespace
 
-extern "C" int cdz_tt_build(const char* aa, int L, int kind, const double* codon_logw, const double* pair_logw,
-                            cdz_tt** out) {
+// cw_stride = 0: one table codon_logw[64] for every residue; 64: per-position tables codon_logw[L][64]
+static int tt_build(const char* aa, int L, int kind, const double* codon_logw, int cw_stride, const double* pair_logw,
+                    cdz_tt** out) {
   if (!aa || L <= 0 || !out || (kind != CDZ_TT_SINGLE_CODON && kind != CDZ_TT_CODON_PAIR)) {
     cdz_set_error("cdz_tt_build: bad argument");
     return CDZ_EINVAL;
   }
   if (codon_logw)
-    for (int c = 0; c < 64; ++c)
+    for (size_t c = 0; c < (cw_stride ? (size_t)L * 64 : (size_t)64); ++c)
       if (!std::isfinite(codon_logw[c])) { cdz_set_error("cdz_tt_build: non-finite codon weight"); return CDZ_EINVAL; }
   if (pair_logw)
     for (int c = 0; c < 4096; ++c)
@@ -204,7 +205,7 @@ extern "C" int cdz_tt_build(const char* aa, int L, int kind, const double* codon
       return CDZ_EINVAL;
     }
     const int deg = (int)cod.size();
-    auto cw = [&](int c) { return codon_logw ? exp(codon_logw[c]) : 1.0; };
+    auto cw = [&](int c) { return codon_logw ? exp(codon_logw[(size_t)k * cw_stride + c]) : 1.0; };
     if (kind == CDZ_TT_SINGLE_CODON) {
       // bonds carry the first base (after 3k) and the third base (after 3k+1), compacted (eq 3.4)
       std::vector<int> firsts, thirds;
@@ -216,7 +217,7 @@ extern "C" int cdz_tt_build(const char* aa, int L, int kind, const double* codon
       tt->opstart[3 * k] = (int)tt->ops.size();
       for (auto& kv : rf) tt->ops.push_back(cdz_op{0, kv.first, kv.second, 1.0});
       tt->opstart[3 * k + 1] = (int)tt->ops.size();
-      for (int c : cod) tt->ops.push_back(cdz_op{rf[c >> 4], (c >> 2) & 3, rt[c & 3], cw(c)});
+      for (int c : cod) { tt->ops.push_back(cdz_op{rf[c >> 4], (c >> 2) & 3, rt[c & 3], cw(c)}); tt->mid_codon.push_back(c); }
       tt->opstart[3 * k + 2] = (int)tt->ops.size();
       for (auto& kv : rt) tt->ops.push_back(cdz_op{kv.second, kv.first, 0, 1.0});
     } else {
@@ -232,7 +233,7 @@ extern "C" int cdz_tt_build(const char* aa, int L, int kind, const double* codon
           tt->ops.push_back(cdz_op{a, cod[c] >> 4, c, x});
         }
       tt->opstart[3 * k + 1] = (int)tt->ops.size();
-      for (int c = 0; c < deg; ++c) tt->ops.push_back(cdz_op{c, (cod[c] >> 2) & 3, c, cw(cod[c])});
+      for (int c = 0; c < deg; ++c) { tt->ops.push_back(cdz_op{c, (cod[c] >> 2) & 3, c, cw(cod[c])}); tt->mid_codon.push_back(cod[c]); }
       tt->opstart[3 * k + 2] = (int)tt->ops.size();
       for (int c = 0; c < deg; ++c) tt->ops.push_back(cdz_op{c, cod[c] & 3, c, 1.0});
       prev = cod;
@@ -244,6 +245,15 @@ extern "C" int cdz_tt_build(const char* aa, int L, int kind, const double* codon
   if (rc != CDZ_OK) { delete tt; return rc; }
   *out = tt;
   return CDZ_OK;
+}
+
+extern "C" int cdz_tt_build(const char* aa, int L, int kind, const double* codon_logw, const double* pair_logw,
+                            cdz_tt** out) {
+  return tt_build(aa, L, kind, codon_logw, 0, pair_logw, out);
+}
+extern "C" int cdz_tt_build_pos(const char* aa, int L, int kind, const double* codon_logw_pos, const double* pair_logw,
+                                cdz_tt** out) {
+  return tt_build(aa, L, kind, codon_logw_pos, 64, pair_logw, out);
 }
 
 extern "C" int cdz_tt_from_operators(int n, const int32_t* counts, const cdz_op* ops, cdz_tt** out) {
@@ -315,6 +325,7 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   t.NB = tt->NB;
   Ctx* dc = k.take<Ctx>(1);
   if (d_ctx) *d_ctx = dc;
+  x.batch = k.take<Ctx>(CDZ_MAX_BATCH);  // device copy of the handles of a batched launch (used on the first handle of the batch)
   t.sig = k.take<int>(n + 1);
   t.off = k.take<int>(n + 2);
   t.opstart = k.take<int>(n + 1);
@@ -344,8 +355,9 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   b.ER = k.take<int>(RS);
   b.R = k.take<double>(S);
   {
+    // worst case over every batch size the design may be launched in: cdz_nsplit(.., D, B) <= min(CDZ_MAX_SPLIT, D - 1)
     size_t tiles = 1;
-    for (int D = 2; D < tt->NB; ++D) tiles = std::max(tiles, (size_t)(tt->NB - D) * cdz_nsplit(tt->NB, D, 1));
+    for (int D = 2; D < tt->NB; ++D) tiles = std::max(tiles, (size_t)(tt->NB - D) * (size_t)std::min(CDZ_MAX_SPLIT, D - 1));
     b.GP = k.take<double>(tiles * CDZ_TB * CDZ_TB);
   }
   b.ctrl = k.take<int>(64);
@@ -677,10 +689,18 @@ extern "C" int cdz_tables_logqext(cdz_tables* t, int j, int c, double* out) {
   return CDZ_OK;
 }
 
+// Work on `st` that reads the tables must run after the inside pass, which may have been launched on another stream.
+int cdz_wait_pass(cdz_tables* t, cudaStream_t st) {
+  if (st != t->stream) CDZ_CUDA(cudaStreamWaitEvent(st, t->ev1, 0));
+  return CDZ_OK;
+}
+
 extern "C" int cdz_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* pair_dev, void* stream) {
   if (!t || J < 0 || !seq_dev || !pair_dev) { cdz_set_error("cdz_sample: bad argument"); return CDZ_EINVAL; }
   if (!t->done) { cdz_set_error("cdz_sample before cdz_inside"); return CDZ_ESTATE; }
   if (J == 0) return CDZ_OK;
+  const int rc = cdz_wait_pass(t, (cudaStream_t)stream);
+  if (rc != CDZ_OK) return rc;
   return cdz_launch_sample(t, J, seed, seq_dev, pair_dev, (cudaStream_t)stream);
 }
 

@@ -124,7 +124,10 @@ __global__ void __launch_bounds__(1024) plan_kernel(const Ctx* ctxs, int D) {
   const DevTT& t = cx.tt;
   const DevTab& b = cx.tab;
   const int n = t.n, NB = t.NB, nw = NB - D;
-  if (nw <= 0) return;
+  if (nw <= 0) {  // a shorter design of a heterogeneous batch that has already finished: nothing to rescale
+    if (threadIdx.x == 0) b.ctrl[3] = 0;
+    return;
+  }
   const size_t S = (size_t)t.S;
   if (threadIdx.x == 0) s_maxe = 0;
   __syncthreads();
@@ -375,6 +378,13 @@ __global__ void zero_kernel(const Ctx* ctxs) {
 }  // namespace
 
 int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
+  if (B > CDZ_MAX_BATCH) {  // independent designs: chunks of CDZ_MAX_BATCH, one launch sequence each
+    for (int b0 = 0; b0 < B; b0 += CDZ_MAX_BATCH) {
+      const int rc = cdz_launch_inside(ts + b0, std::min(CDZ_MAX_BATCH, B - b0), st);
+      if (rc != CDZ_OK) return rc;
+    }
+    return CDZ_OK;
+  }
   int NBmax = 1, Smax = 0, nrmax = 0;
   for (int b = 0; b < B; ++b) {
     const cdz_tt* tt = ts[b]->tt;
@@ -383,14 +393,13 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
     nrmax = std::max(nrmax, std::max(tt->S, std::max(tt->LS, tt->RS)));
   }
   const Ctx* d_ctxs = ts[0]->d_ctx;
-  Ctx* tmp = nullptr;
   if (B > 1) {
+    // the handle array of the batch lives in the first handle's workspace: no allocation, no synchronisation (the copy from
+    // pageable host memory is staged before cudaMemcpyAsync returns)
     std::vector<Ctx> h(B);
     for (int b = 0; b < B; ++b) h[b] = ts[b]->h;
-    CDZ_CUDA(cudaMallocAsync((void**)&tmp, sizeof(Ctx) * B, st));
-    CDZ_CUDA(cudaMemcpyAsync(tmp, h.data(), sizeof(Ctx) * B, cudaMemcpyHostToDevice, st));
-    CDZ_CUDA(cudaStreamSynchronize(st));
-    d_ctxs = tmp;
+    CDZ_CUDA(cudaMemcpyAsync(ts[0]->h.batch, h.data(), sizeof(Ctx) * B, cudaMemcpyHostToDevice, st));
+    d_ctxs = ts[0]->h.batch;
   }
   cdz_cell_cfg ccfg;
   {
@@ -442,7 +451,7 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
     ext_kernel<<<dim3(gx, B), 256, 0, st>>>(d_ctxs, K);
   }
   mark(7, 0);  // closing event
+  T0->nev_inside = T0->ev_class.size();
   CDZ_CUDA(cudaGetLastError());
-  if (tmp) CDZ_CUDA(cudaFreeAsync(tmp, st));
   return CDZ_OK;
 }

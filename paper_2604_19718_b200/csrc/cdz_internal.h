@@ -13,6 +13,7 @@
 #define CDZ_TB 64          // bond-space tile: every position block holds at most CDZ_TB bonds, padded to exactly CDZ_TB
 #define CDZ_NCLASS 8       // kernel classes of cdz_profile: 0 gemm, 1 block, 2 rescale, 3 exterior, 4 init, 5 sample
 #define CDZ_MAX_SPLIT 16   // split-K limit of the split-point GEMM
+#define CDZ_MAX_BATCH 256  // designs advanced together by one launch sequence (larger batches run in chunks)
 
 // ---- Boltzmann factors of the loop model (constant memory image) -------------------------------
 struct CModel {
@@ -39,6 +40,7 @@ struct cdz_tt {
   std::vector<int> sigma;    // [n+1]
   std::vector<int> opstart;  // [n+1]
   std::vector<cdz_op> ops;
+  std::vector<int> mid_codon;  // codon index of every middle-base operator, residue by residue in list order (cdz_tt_build only)
   // derived
   int S = 0, LS = 0, RS = 0, MS = 1, maxL = 1, maxR = 1, maxOps = 1;
   std::vector<int> off;                   // [n+2] padded bond offsets: block b owns [b*CDZ_TB, (b+1)*CDZ_TB)
@@ -110,6 +112,7 @@ struct Ctx {
   DevTT tt;
   DevTab tab;
   const CModel* cm;  // Boltzmann tables (device copy inside the workspace)
+  Ctx* batch;        // [CDZ_MAX_BATCH] scratch for the handle array of a batched launch
 };
 
 struct cdz_tables {
@@ -127,6 +130,7 @@ struct cdz_tables {
   bool profile = false;
   std::vector<cudaEvent_t> evs;
   std::vector<int> ev_class;
+  size_t nev_inside = 0;  // events recorded by the last inside pass (later calls append after them, never beyond one call's worth)
   long launches[CDZ_NCLASS] = {0, 0, 0, 0, 0, 0, 0, 0};
   double inside_ms = 0;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;

@@ -1,9 +1,10 @@
-// cdz_peak.cu -- register-resident fp64 / fp32 issue-rate microbenchmarks.
+// cdz_peak.cu -- register-resident fp64 / fp32 issue-rate microbenchmarks (libcdz_peak.so: used by bench.py only, NOT part of the
+// product ABI of include/cdz.h).
 // MEASURED_PEAKS.json holds HBM and bf16 numbers only; the roofline of the fp64 split-point contraction needs the
 // fp64 vector (DFMA) and tensor (mma.sync m8n8k4 f64, "DMMA") peaks of the same GPU under the same clocks.
-#include <algorithm>
+#include <cuda_runtime.h>
 
-#include "cdz_internal.h"
+#include <algorithm>
 
 namespace {
 __global__ void __launch_bounds__(512) peak_dfma(double* out, int iters) {
@@ -53,13 +54,16 @@ __global__ void __launch_bounds__(512) peak_ffma(float* out, int iters) {
 }
 }  // namespace
 
-extern "C" int cdz_measure_peak(int kind, double* tflops_out) {
-  if (!tflops_out || kind < 0 || kind > 2) { cdz_set_error("cdz_measure_peak: bad argument"); return CDZ_EINVAL; }
+// kind 0 = fp64 FMA, 1 = fp64 mma.sync m8n8k4, 2 = fp32 FMA; TFLOP/s on the current device (best of 3 after one warm-up).
+// Returns 0 on success, -1 on a bad argument, -3 on a CUDA error.
+extern "C" int cdz_peak_measure(int kind, double* tflops_out) {
+  if (!tflops_out || kind < 0 || kind > 2) return -1;
   cudaDeviceProp prop;
-  CDZ_CUDA(cudaGetDeviceProperties(&prop, 0));
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return -3;
   const int threads = 512, blocks = prop.multiProcessorCount * 4, iters = 20000;
   double* out = nullptr;
-  CDZ_CUDA(cudaMalloc((void**)&out, sizeof(double) * threads * blocks));
+  if (cudaMalloc((void**)&out, sizeof(double) * threads * blocks) != cudaSuccess) return -3;
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0);
   cudaEventCreate(&e1);
@@ -80,7 +84,7 @@ extern "C" int cdz_measure_peak(int kind, double* tflops_out) {
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   cudaFree(out);
-  CDZ_CUDA(cudaGetLastError());
+  if (cudaGetLastError() != cudaSuccess) return -3;
   *tflops_out = best;
-  return CDZ_OK;
+  return 0;
 }

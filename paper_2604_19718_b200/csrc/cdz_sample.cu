@@ -578,6 +578,7 @@ int cdz_launch_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int
   CDZ_CUDA(cudaMallocAsync((void**)&stacks, sizeof(Item) * (size_t)cap * J, st));
   const int wpb = 4;
   t->launches[5] = 1;
+  if (t->ev_class.size() > t->nev_inside) t->ev_class.resize(t->nev_inside);  // one traceback's events after the pass's, not a growing list
   auto mark = [&](int cls) {
     if (!t->profile) return;
     const size_t k = t->ev_class.size();
