@@ -98,6 +98,33 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+_peak_lib = None
+
+
+def peak_lib():
+    """libcdz_peak.so: register-resident issue-rate loops and latency probes (bench only, not part of the product ABI)."""
+    global _peak_lib
+    if _peak_lib is None:
+        import ctypes as C
+
+        _peak_lib = C.CDLL(os.path.join(ROOT, "paper_2604_19718_b200", "libcdz_peak.so"))
+        _peak_lib.cdz_peak_measure.argtypes = [C.c_int, C.POINTER(C.c_double)]
+        _peak_lib.cdz_peak_launch_us.argtypes = [C.c_int, C.POINTER(C.c_double)]
+        _peak_lib.cdz_peak_barrier_us.argtypes = [C.c_int, C.POINTER(C.c_double)]
+    return _peak_lib
+
+
+def measure_peak(kind: int) -> float:
+    """0 fp64 FMA, 1 fp64 mma.sync m8n8k4, 2 fp32 FMA (TFLOP/s)."""
+    import ctypes as C
+
+    v = C.c_double()
+    rc = peak_lib().cdz_peak_measure(kind, C.byref(v))
+    if rc != 0:
+        raise RuntimeError(f"cdz_peak_measure rc={rc}")
+    return v.value
+
+
 def reduce_max(value: float, device="cpu") -> float:
     """Max over ranks of a per-rank time (the only collective besides the barrier: replicas share no data)."""
     import torch
@@ -248,10 +275,10 @@ def run_cdz(args):
     marg = None
     if args.marginals and rank == 0:
         tab.rerun(stream)
-        bpp = tab.marginals(stream)  # warm-up (allocates / frees its own workspace)
+        bpp, base_m, codon_m = tab.marginals(stream)  # warm-up
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        bpp = tab.marginals(stream)
+        bpp, base_m, codon_m = tab.marginals(stream)
         torch.cuda.synchronize()
         marg_ms = 1e3 * (time.perf_counter() - t0)
         up = torch.triu(bpp, 1)
@@ -272,8 +299,8 @@ def run_cdz(args):
             peaks = json.load(f)
     except OSError:
         pass
-    dmma = B.measure_peak(1)
-    dfma = B.measure_peak(0)
+    dmma = measure_peak(1)
+    dfma = measure_peak(0)
     bf16 = peaks.get("bf16_tflops")
     sbar_n = info["sigma_bar"] / n
     loop_mac = nloop * 2.0 * sbar_n ** 3

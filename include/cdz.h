@@ -150,13 +150,23 @@ int cdz_tables_logqext(cdz_tables* t, int j, int c, double* out_host);
 int cdz_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* pair_dev, void* stream);
 
 /* ---- marginals (device) ---------------------------------------------------- */
-/* Outside (adjoint) pass over the tables of a finished inside pass (eq 2.5 line 85, eq 4.1; DESIGN.md
- * section 9).  bpp_dev: device, [n][n] doubles, caller-owned, fully overwritten: upper triangle P(i.j), diagonal
- * P(i unpaired), lower triangle 0.  May be NULL (no work).  The adjoint workspace is allocated and freed inside the call
- * (CDZ_ENOMEM if it does not fit); the call synchronises `stream` before it returns.
- * base_dev [n][4] (eq 2.6) and codon_dev [L][64] (eq 2.7) are NOT BUILT YET: they must be NULL, otherwise the call returns
- * CDZ_ESTATE and writes nothing.  CDZ_ESTATE also before cdz_inside. */
-int cdz_marginals(cdz_tables* t, double* bpp_dev, double* base_dev, double* codon_dev, void* stream);
+/* Outside (adjoint) pass over the tables of a finished inside pass: the paper's ComputeReverse (Alg S4.3) as the
+ * reverse-mode adjoint of the recursion.  Asynchronous on `stream` (it waits for the inside pass by an event
+ * if that ran on another stream); outputs are valid after the stream has been synchronised.  Every output may be NULL:
+ *   bpp_dev   [n][n] doubles, fully overwritten: upper triangle P(i.j) (eq 2.5 line 85, eq 4.1), diagonal P(i unpaired)
+ *             (computed from the unpaired operator usages, NOT as 1 - row sum), lower triangle 0;
+ *   base_dev  [n][4]  P(phi_m = b), eq 2.6 line 90 / eq 4.2;
+ *   codon_dev [L][64] p_k(c), c = 16 b0 + 4 b1 + b2, eq 2.7 line 96 / eq 4.3; exactly 0 on codons that do not encode
+ *             residue k.  Needs a tensor train from cdz_tt_build / cdz_tt_build_pos (CDZ_EINVAL for generic operator lists).
+ * workspace_dev: device buffer of >= cdz_marginals_workspace_bytes bytes, caller-owned, or NULL (the library then takes and
+ * returns the memory with the stream-ordered allocator; CDZ_ENOMEM if it does not fit).  No host synchronisation either way.
+ * CDZ_ESTATE before cdz_inside. */
+int cdz_marginals_workspace_bytes(const cdz_tables* t, size_t* bytes);
+int cdz_marginals(cdz_tables* t, void* workspace_dev, size_t workspace_bytes, double* bpp_dev, double* base_dev,
+                  double* codon_dev, void* stream);
+/* Synchronises the stream of the last cdz_marginals call and reports its device-side checks: CDZ_EOVERFLOW when an operator
+ * usage left [0,1] or the usages at some position do not sum to 1 within 1e-6 (non-finite values included), else CDZ_OK. */
+int cdz_marginals_status(cdz_tables* t);
 
 /* ---- convenience: host buffers end to end (used for the e2e timing) -------- */
 /* Builds nothing: runs cdz_inside_rerun, samples J states and copies them to host buffers. */

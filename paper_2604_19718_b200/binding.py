@@ -22,7 +22,7 @@ EXPORTS = [
     "cdz_tt_from_operators", "cdz_tt_destroy", "cdz_tt_length", "cdz_tt_describe", "cdz_workspace_bytes",
     "cdz_inside", "cdz_inside_batch", "cdz_inside_rerun", "cdz_inside_rerun_batch", "cdz_tables_logz",
     "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample",
-    "cdz_marginals", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
+    "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
 ]
 
 
@@ -94,7 +94,9 @@ def lib():
     L.cdz_tables_cell.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
     L.cdz_tables_logqext.argtypes = [vp, C.c_int, C.c_int, dp]
     L.cdz_sample.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, vp]
-    L.cdz_marginals.argtypes = [vp, vp, vp, vp, vp]
+    L.cdz_marginals.argtypes = [vp, vp, C.c_size_t, vp, vp, vp, vp]
+    L.cdz_marginals_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
+    L.cdz_marginals_status.argtypes = [vp]
     L.cdz_run_host.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, dp, vp]
     _lib = L
     return L
@@ -241,15 +243,26 @@ class Tables:
                                 _stream_ptr(stream)))
         return seq, pair
 
-    def marginals(self, stream=None):
-        """cdz_marginals: base-pair probabilities [n][n] (upper triangle P(i.j), diagonal P(i unpaired)) by the outside pass.
-        Base and codon marginals are not built yet (the C call rejects non-NULL buffers for them)."""
+    def marginals(self, stream=None, bpp=True, base=True, codon=True, own_workspace=True):
+        """cdz_marginals: (bpp [n][n], base [n][4], codon [L][64]) as CUDA tensors (None where not requested), by the outside pass.
+        The workspace is a torch tensor unless own_workspace=False (then the library uses the stream-ordered allocator).
+        cdz_marginals_status is called before returning (it synchronises the stream)."""
         import torch
 
         n = self.n
-        bpp = torch.zeros((n, n), dtype=torch.float64, device="cuda")
-        _check(lib().cdz_marginals(self.h, C.c_void_p(bpp.data_ptr()), None, None, _stream_ptr(stream)))
-        return bpp
+        o_bpp = torch.empty((n, n), dtype=torch.float64, device="cuda") if bpp else None
+        o_base = torch.empty((n, 4), dtype=torch.float64, device="cuda") if base else None
+        o_codon = torch.empty((n // 3, 64), dtype=torch.float64, device="cuda") if codon else None
+        ws, nb = None, 0
+        if own_workspace:
+            b = C.c_size_t()
+            _check(lib().cdz_marginals_workspace_bytes(self.h, C.byref(b)))
+            nb = b.value
+            ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+        ptr = lambda x: C.c_void_p(x.data_ptr()) if x is not None else None  # noqa: E731
+        _check(lib().cdz_marginals(self.h, ptr(ws), nb, ptr(o_bpp), ptr(o_base), ptr(o_codon), _stream_ptr(stream)))
+        _check(lib().cdz_marginals_status(self.h))
+        return o_bpp, o_base, o_codon
 
     def run_host(self, J: int, seed: int, seq_host=None, pair_host=None, stream=None) -> float:
         """cdz_run_host: host buffers in / out (pinned torch tensors or numpy arrays), returns log Z."""

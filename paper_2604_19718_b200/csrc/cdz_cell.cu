@@ -124,7 +124,7 @@ template <int MA, int W>
 __device__ __forceinline__ void x_cell(int lane, double* xs, int Mst, int Sa, int Sa3, int Sc, bool hasold, bool closed, int mh1,
                                        int maxint, int i, int j, const double* Tb, int MS, const double* gi, const double* em,
                                        size_t S, const PosMeta* colm, int cbase, const double* win, double hpw,
-                                       const double* emh, double* xe_out, int Mxe) {
+                                       const double* emh, double* xe_out, int Mxe, double* xe_glob) {
   const int u = 4 + lane;
   const bool live = lane < XU;
   const int cp = j + 3 - u;
@@ -203,7 +203,11 @@ __device__ __forceinline__ void x_cell(int lane, double* xs, int Mst, int Sa, in
     v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
     if ((lane & 1) == 0) {
       const int e = lane >> 1, a = e / W, w = e % W;
-      if (a < Sa && w < ncw) xe_out[a * Mxe + cc + w] = v[0] + (closed ? hpw * emh[(size_t)a * S + cc + w] : 0.0);
+      if (a < Sa && w < ncw) {
+        const double xv = v[0] + (closed ? hpw * emh[(size_t)a * S + cc + w] : 0.0);
+        xe_out[a * Mxe + cc + w] = xv;
+        xe_glob[(size_t)a * S + cc + w] = xv;  // same index as emh: row (i+2, a), column (j-1, c)
+      }
     }
     __syncwarp();
   }
@@ -398,14 +402,15 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           const double* gi = b.GI + (size_t)rowm[kp2].off * S;
           const double* em = b.EMT + (size_t)mq.off * S;
           const double* emh = b.EM + (size_t)rowm[kp2].off * S + mq.off;
+          double* xeg = b.XE + (size_t)rowm[kp2].off * S + mq.off;
           double* xe = scr_of(scrb, dm, i - clo).XE;
           const double hpw = closed ? t.wh[d - 1] : 0.0;
           if (M <= 4)
             x_cell<4, 4>(lane, xs, M, rowm[kp2].sig, rowm[kp2 + 1].sig, mq.sig, d - 1 >= 4, closed, mh1, maxint, i, j, Tb, MS, gi, em, S,
-                         colm.p, cbase, cm.win, hpw, emh, xe, M);
+                         colm.p, cbase, cm.win, hpw, emh, xe, M, xeg);
           else
             x_cell<8, 2>(lane, xs, M, rowm[kp2].sig, rowm[kp2 + 1].sig, mq.sig, d - 1 >= 4, closed, mh1, maxint, i, j, Tb, MS, gi, em, S,
-                         colm.p, cbase, cm.win, hpw, emh, xe, M);
+                         colm.p, cbase, cm.win, hpw, emh, xe, M, xeg);
         }
       }
       // ---- cooperative row items: GL consecutive lanes share one row object (a bond row or a left state of one cell), split

@@ -8,6 +8,7 @@
 #include <new>
 
 #include "cdz_internal.h"
+#include "cdz_outside.h"
 
 static thread_local std::string g_err;
 void cdz_set_error(const std::string& s) { g_err = s; }
@@ -331,6 +332,7 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   t.opstart = k.take<int>(n + 1);
   t.op_a = k.take<uint8_t>(nops); t.op_b = k.take<uint8_t>(nops); t.op_c = k.take<uint8_t>(nops);
   t.op_l = k.take<uint8_t>(nops); t.op_r = k.take<uint8_t>(nops);
+  t.op_codon = k.take<int8_t>(nops);
   t.op_x = k.take<double>(nops);
   t.op_x0 = k.take<double>(nops);
   t.blk_start = k.take<int>(tt->NB + 1);
@@ -376,6 +378,7 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
   b.EM = k.take<double>(S * S);
   b.EMT = k.take<double>(S * S);
   b.QBST = k.take<double>(S * S);
+  b.XE = k.take<double>(S * S);
   b.XS = k.take<double>(n * 27 * MS * MS);
   x.cm = k.take<CModel>(1);
   return (k.used + 255) & ~size_t(255);
@@ -401,6 +404,12 @@ static int upload(cdz_tables* T) {
   std::vector<uint8_t> oa, ob, oc;
   std::vector<double> ox;
   for (const cdz_op& o : tt->ops) { oa.push_back(o.a); ob.push_back(o.b); oc.push_back(o.c); ox.push_back(o.x); }
+  std::vector<int8_t> ocod(tt->ops.size(), -1);
+  if (tt->kind >= 0 && !tt->mid_codon.empty()) {
+    size_t k = 0;
+    for (int r = 0; 3 * r + 1 < n; ++r)
+      for (int z = tt->opstart[3 * r + 1]; z < tt->opstart[3 * r + 2]; ++z) ocod[z] = (int8_t)tt->mid_codon[k++];
+  }
   // padding bond indices map to the first position of the next block (their table entries are zero)
   std::vector<int> bondpos(tt->S + 1, n), lspos(tt->LS), rspos(tt->RS);
   for (int kb = 0; kb < tt->S; ++kb) bondpos[kb] = std::min(n, tt->blk_start[kb / CDZ_TB + 1]);
@@ -431,6 +440,7 @@ static int upload(cdz_tables* T) {
   CDZ_CUDA(up(t.op_c, oc.data(), oc.size()));
   CDZ_CUDA(up(t.op_l, tt->op_l.data(), oa.size()));
   CDZ_CUDA(up(t.op_r, tt->op_r.data(), oa.size()));
+  CDZ_CUDA(up(t.op_codon, ocod.data(), ocod.size()));
   CDZ_CUDA(up(t.op_x, ox.data(), sizeof(double) * ox.size()));
   CDZ_CUDA(up(t.op_x0, ox.data(), sizeof(double) * ox.size()));
   CDZ_CUDA(up(t.blk_start, tt->blk_start.data(), sizeof(int) * (tt->NB + 1)));
@@ -704,15 +714,54 @@ extern "C" int cdz_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev,
   return cdz_launch_sample(t, J, seed, seq_dev, pair_dev, (cudaStream_t)stream);
 }
 
-extern "C" int cdz_marginals(cdz_tables* t, double* bpp_dev, double* base_dev, double* codon_dev, void* stream) {
+extern "C" int cdz_marginals_workspace_bytes(const cdz_tables* t, size_t* bytes) {
+  if (!t || !bytes) { cdz_set_error("cdz_marginals_workspace_bytes: null argument"); return CDZ_EINVAL; }
+  *bytes = cdz_outside_carve(t->tt, nullptr, nullptr);
+  return CDZ_OK;
+}
+
+extern "C" int cdz_marginals(cdz_tables* t, void* workspace_dev, size_t workspace_bytes, double* bpp_dev, double* base_dev,
+                             double* codon_dev, void* stream) {
   if (!t) { cdz_set_error("cdz_marginals: null handle"); return CDZ_EINVAL; }
   if (!t->done) { cdz_set_error("cdz_marginals before cdz_inside"); return CDZ_ESTATE; }
-  if (base_dev || codon_dev) {
-    cdz_set_error("cdz_marginals: base / codon marginals are not implemented yet (pass NULL); base-pair probabilities are");
-    return CDZ_ESTATE;
+  if (!bpp_dev && !base_dev && !codon_dev) return CDZ_OK;
+  if (codon_dev && (t->tt->kind < 0 || t->tt->mid_codon.empty())) {
+    cdz_set_error("cdz_marginals: codon marginals need a tensor train made by cdz_tt_build (generic operator lists carry no codon labels)");
+    return CDZ_EINVAL;
   }
-  if (!bpp_dev) return CDZ_OK;
-  return cdz_launch_outside(t, bpp_dev, (cudaStream_t)stream);
+  if (t->tt->maxOps > 256) { cdz_set_error("cdz_marginals: more than 256 operators at one position"); return CDZ_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc = cdz_wait_pass(t, st);
+  if (rc != CDZ_OK) return rc;
+  const size_t need = cdz_outside_carve(t->tt, nullptr, nullptr);
+  void* ws = workspace_dev;
+  if (ws) {
+    if (workspace_bytes < need) { cdz_set_error("cdz_marginals: workspace too small (cdz_marginals_workspace_bytes)"); return CDZ_ENOMEM; }
+  } else if (cudaMallocAsync(&ws, need, st) != cudaSuccess) {  // stream-ordered: no synchronisation
+    cudaGetLastError();
+    cdz_set_error("cdz_marginals: out of device memory for the adjoint tables");
+    return CDZ_ENOMEM;
+  }
+  Adj A;
+  cdz_outside_carve(t->tt, ws, &A);
+  A.status = t->h.tab.ctrl + 8;  // lives in the tables' own workspace: readable after a library-owned workspace has been freed
+  CDZ_CUDA(cudaMemsetAsync(A.status, 0, sizeof(int), st));
+  rc = cdz_launch_outside(t, A, need, bpp_dev, base_dev, codon_dev, st);
+  if (!workspace_dev) cudaFreeAsync(ws, st);
+  t->marg_stream = st;
+  return rc;
+}
+
+extern "C" int cdz_marginals_status(cdz_tables* t) {
+  if (!t) { cdz_set_error("cdz_marginals_status: null handle"); return CDZ_EINVAL; }
+  int flag = 0;
+  CDZ_CUDA(cudaMemcpyAsync(&flag, t->h.tab.ctrl + 8, sizeof(int), cudaMemcpyDeviceToHost, t->marg_stream));
+  CDZ_CUDA(cudaStreamSynchronize(t->marg_stream));
+  if (flag != 0) {
+    cdz_set_error("cdz_marginals: an operator usage left [0,1] or the usages of a position do not sum to 1 (dynamic range exceeded)");
+    return CDZ_EOVERFLOW;
+  }
+  return CDZ_OK;
 }
 
 extern "C" int cdz_run_host(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_host, int32_t* pair_host,

@@ -210,6 +210,7 @@ __global__ void __launch_bounds__(256) rescale_kernel(const Ctx* ctxs, int which
     case 9: tab = b.EM; break;
     case 10: tab = b.EMT; lower = 1; break;
     case 11: tab = b.QBST; lower = 1; break;
+    case 13: tab = b.XE; break;
     default: tab = b.QM1T; lower = 1; break;
   }
   const int nrows = rowsp == 1 ? t.LS : rowsp == 2 ? t.RS : t.S;
@@ -436,10 +437,10 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
     cdz_launch_cells(d_ctxs, B, nblk, D, nsplit, &ccfg, st);
     if (D == next_event && D + 1 < NBmax) {
       next_event *= 2;
-      mark(2, 15);
+      mark(2, 16);
       plan_kernel<<<B, 1024, NBmax * sizeof(double), st>>>(d_ctxs, D);
       const int gx = std::min(nrmax, 148 * 8);
-      for (int which = 0; which <= 12; ++which) rescale_kernel<<<dim3(gx, B), 256, 0, st>>>(d_ctxs, which, D);
+      for (int which = 0; which <= 13; ++which) rescale_kernel<<<dim3(gx, B), 256, 0, st>>>(d_ctxs, which, D);
       rescale_xs_kernel<<<dim3(std::min(nmax, 148 * 8), B), 256, 0, st>>>(d_ctxs, D);
     }
   }

@@ -64,6 +64,7 @@ struct DevTT {
   const int* off;      // [n+2]
   const int* opstart;  // [n+1]
   const uint8_t *op_a, *op_b, *op_c, *op_l, *op_r;
+  const int8_t* op_codon;  // codon index (16 b0 + 4 b1 + b2) of a middle-base operator of a cdz_tt_build train, -1 otherwise
   double* op_x;        // scaled operator weights
   const int* loff;     // [n+1]
   const int* roff;     // [n+1]
@@ -94,6 +95,8 @@ struct DevTabT {
   T *EM;    // S x S   : E(i,j) = Tbar_i..Tbar_j; the diagonal holds E(i,i-1) = identity
   T *EMT;   // S x S   : EM transposed (row (j+1,c), column (i,a))
   T *QBST;  // S x S   : QBS transposed
+  T *XE;    // S x S   : XE(i,j) = sum_u w_In(u) X_u(i,j) + w_H(d-1) E(i+2,j-2), row (i+2, a2), column (j-1, c2): the loop body between the two
+            //           closing-mismatch positions of cell (i,j) (read by the outside pass for the operator usages)
   T *XS;    // [n][27][MS*MS] : interior-loop bodies X_u(i0,j), u = 4..30, of the top row of the last block of every column j
   T *Qext;  // [n+1][MS]
   T *GP;    // split-point GEMM partial sums: [block row I][split][CDZ_TB*CDZ_TB]
@@ -120,6 +123,7 @@ struct cdz_tables {
   const cdz_tt* tt = nullptr;
   int precision = CDZ_FP64;
   cudaStream_t stream = nullptr;
+  cudaStream_t marg_stream = nullptr;  // stream of the last cdz_marginals call
   void* base = nullptr;  // device allocation (owned if owns_base)
   bool owns_base = false;
   size_t bytes = 0;
@@ -158,7 +162,7 @@ struct cdz_cell_cfg { int M, ML, MR, nps, maxpos, span, C; size_t smem; };
 int cdz_cell_config(cdz_tables* const* ts, int B, cdz_cell_cfg* cfg);
 void cdz_launch_cells(const Ctx* d_ctxs, int B, int nblk, int D, int nsplit, const cdz_cell_cfg* cfg, cudaStream_t st);
 int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st);
-int cdz_launch_outside(cdz_tables* t, double* bpp_dev, cudaStream_t st);
+int cdz_wait_pass(cdz_tables* t, cudaStream_t st);
 int cdz_launch_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* pair_dev, cudaStream_t st);
 
 #define CDZ_CUDA(call)                                                                       \

@@ -1,147 +1,224 @@
-// cdz_outside.cu -- outside (adjoint) pass over the stored inside tables: base-pair probabilities (sm_100a).
+// cdz_outside.cu -- outside (adjoint) pass over the stored inside tables (sm_100a): base-pair probabilities (eq 2.5 line 85,
+// eq 4.1) and the operator usages  u_z = x_z dlogZ/dx_z  from which the base marginals (eq 2.6 line 90, eq 4.2) and the
+// codon marginals (eq 2.7 line 96, eq 4.3) follow (the paper's ComputeReverse, Alg S4.3, re-expressed
+// as the reverse-mode adjoint of the recursion of DESIGN.md section 3).
 //
-//   P(i.j) = sum_{a,x,y,c} Qb(i,j)[a,x,y,c] * dZ/dQb(i,j)[a,x,y,c] / Z            (eq 2.5 line 85; eq 4.1;
-//                                                                                 SURVEY 8a-9 "outside / adjoint pass")
-// The adjoint tables are gathered diagonal by diagonal, d = n-1 .. 0, from the cells that use cell (i,j) in the plain
-// recursion of DESIGN.md section 3:
-//   Qext-bar(k)   = Tbar_k Qext-bar(k+1) + sum_{j>=k} Qbs(k,j) Qext-bar(j+1),    Qext-bar(n) = 1/Z
-//   Qm-bar(i,j)   = sum_{j'>j} M2-bar(i,j') Qm1(j+1,j')^T
-//   M2-bar(i,j)   = Qm-bar(i,j) + w_a w_c sum_{x,y} I(i-1,j+1)[x,y]
-//   Qml-bar(i,j)  = Qm-bar(i,j) + w_b Tbar_{i-1}^T Qml-bar(i-1,j)
-//   Qm1-bar(i,j)  = Qml-bar(i,j) + w_b Qm1-bar(i,j+1) Tbar_{j+1}^T + sum_{i'<i} Qm(i',i-1)^T M2-bar(i',j)
-//   Qbs-bar(i,j)  = w_c Qm1-bar(i,j) + Qext(i-1)^T Qext-bar(j+1)
-//   Qb-bar(k,l)   = Qbs-bar(k,l) + sum over the closing pairs (i,j) = (k-1-l1, l+1+l2), l1+l2 <= 30, of the stack / bulge / interior
-//                   term of Qb(i,j) differentiated with respect to Qb(k,l)
-//   I(i,j)[x,y;a',c'] = sum_{a,c} T_i[a,x,a'] T_j[c',y,c] Qb-bar(i,j)[a,x,y,c]   (adjoint of `inner`),
-//   G(i,j)[a',u,v,c'] = sum_{x,y} I(i,j)[x,y;a',c'] e^{-beta tmm[p(x,y)][u][v]}  (closing mismatch applied once per cell).
-// All tables are the scaled ones the inside pass leaves behind: scaling every core by a power of two is a change of the
-// operator weights under which the recursion is unchanged, and the probabilities are ratios.
-// This version is a plain gather (one CTA per cell, one launch per diagonal, no tensor cores); the interior-loop term goes through
-// per-closing-pair tables H / H1 / H2 (loop-side operators pre-contracted with G), so the inner cell only sums bond-indexed products.
-#include "cdz_internal.h"
+// All adjoints are derivatives of log Z with respect to the STORED (scaled) table entries; a power-of-two scale per position is a change of
+// operator weights under which the recursion is unchanged, so every probability  entry x adjoint  is scale-free.
+//
+// Diagonals d = n-1 .. 0, one launch each, one CTA per cell (i, j = i+d).  Per cell, in this order:
+//   1  bond-level adjoints (the two split-point gathers are dot products of contiguous table rows: QM1 / QMT are plain transposes made
+//      at the start of the call, AM2T is written beside AM2):
+//        Qm-bar(i,j)  = sum_{j'>j} M2-bar(i,j') Qm1(j+1,j')^T            M2-bar = Qm-bar + w_a w_c sum_{x,y} I(i-1,j+1)[x,y]
+//        Qml-bar      = Qm-bar + w_b Tbar_{i-1}^T Qml-bar(i-1,j)
+//        Qm1-bar      = Qml-bar + w_b Qm1-bar(i,j+1) Tbar_{j+1}^T + sum_{i'<i} Qm(i',i-1)^T M2-bar(i',j)
+//        Qbs-bar      = w_c Qm1-bar + Qext(i-1)^T Qext-bar(j+1)
+//   2  Qb-bar(i,j) = Qbs-bar + stack / bulge terms pulled from the I tables of the <= 61 closing pairs (ring of 36 diagonals)
+//                  + the interior-loop terms, which closing cells PUSHED earlier into this cell's ring slot as adjoints of its dressed
+//                    extensions DD / D1 / D2T / GI;   P(i.j) = sum Qb (.) Qb-bar;   usages of the inner-mismatch operators at i-1, j+1
+//   3  I = adjoint of `inner`, G = I with the closing mismatch applied, H / H1 / H2 = G with the loop-side operators contracted
+//      (= adjoints of the loop bodies XE, Z1, Z2 of the inside pass)
+//   4  as closing pair: adjoint row / column recursions of the interior-loop bodies X_u (27 small products per cell instead of 378),
+//      pushes into the ring slots of the inner cells and into the stretch adjoints E-bar (hairpin interiors: table AET; loop sides:
+//      per-role accumulators AES), and -- with `inner`, Y, Z1, Z2, Bl, Br, SB recomputed from the stored tables exactly as the inside
+//      pass does -- the usages of the operators at i, j (pair ends), i+1, j-1 (closing mismatch, size-1 bulges).
+// Every accumulator has a single writer per launch (role-separated), every sum a fixed order: results are bit-reproducible.
+// cdz_usage.cu finishes: E-bar chain, multiloop / exterior unpaired usages, base / codon marginals, unpaired probabilities.
+#include "cdz_outside.h"
 
 namespace {
 
-constexpr int OT = 256;    // threads per CTA
-constexpr int OPV = 1024;   // doubles of the per-operator scratch of the interior-loop term
-constexpr int OZC = OPV / CDZ_MAX_BOND;  // operators per pass
-constexpr int ORING = 34;  // diagonals of I / G / H / H1 / H2 kept: a closing pair lies at most 32 diagonals above its inner pair
+constexpr int OT = 256;  // threads per CTA
+constexpr int NW = OT / 32;
 
-struct Adj {
-  double *AB, *AM2, *AML, *AM1, *AX, *IB, *G, *H, *H1, *H2;
-};
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
 
-// Qext-bar, sequential over bond positions k = n .. 0 (one CTA)
-__global__ void __launch_bounds__(OT) oext_kernel(const Ctx* ctx, Adj A) {
+// dot product of two contiguous row segments [k0,k1), lanes stride the range (coalesced), fixed order
+__device__ __forceinline__ double warp_dot(const double* __restrict__ x, const double* __restrict__ y, int k0, int k1, int lane) {
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  int k = k0 + lane;
+  for (; k + 96 < k1; k += 128) {
+    a0 += x[k] * y[k];
+    a1 += x[k + 32] * y[k + 32];
+    a2 += x[k + 64] * y[k + 64];
+    a3 += x[k + 96] * y[k + 96];
+  }
+  for (; k < k1; k += 32) a0 += x[k] * y[k];
+  return warp_sum((a0 + a1) + (a2 + a3));
+}
+
+// Qext-bar, sequential over bond positions k = n .. 0 (one CTA):  AX(k) = Tbar_k AX(k+1) + sum_{j>=k} Qbs(k,j) AX(j+1), AX(n) = 1/Z
+__global__ void __launch_bounds__(1024) oext_kernel(const Ctx* ctx, Adj A) {
   const DevTT& t = ctx->tt;
   const DevTab& b = ctx->tab;
   const int n = t.n, S = t.S, MS = t.MS;
-  __shared__ double part[OT];
+  __shared__ double part[32][CDZ_MAX_BOND];
   __shared__ double zinv;
-  if (threadIdx.x == 0) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
+  if (tid == 0) {
     double Z = 0.0;
     for (int c = 0; c < t.sig[n]; ++c) Z += b.Qext[t.off[n] + c];
     zinv = 1.0 / Z;
   }
   __syncthreads();
-  if (threadIdx.x < MS) A.AX[(size_t)n * MS + threadIdx.x] = threadIdx.x < t.sig[n] ? zinv : 0.0;
+  // AXB: Qext-bar laid out over the bond index space (AXB[off[k]+s]) so that the gather is a dot product with a row of QBS
+  for (int k = tid; k < S; k += blockDim.x) A.AXB[k] = 0.0;
   __syncthreads();
-  const int grp = threadIdx.x / CDZ_MAX_BOND, s = threadIdx.x % CDZ_MAX_BOND, ngrp = OT / CDZ_MAX_BOND;
+  if (tid < t.sig[n]) { A.AX[(size_t)n * MS + tid] = zinv; A.AXB[t.off[n] + tid] = zinv; }
+  __syncthreads();
+  const int send = t.off[n] + t.sig[n];
   for (int k = n - 1; k >= 0; --k) {
-    double acc = 0.0;
-    if (s < t.sig[k]) {
-      for (int j = k + grp; j < n; j += ngrp) {
-        const double* q = b.QBS + (size_t)(t.off[k] + s) * S + t.off[j + 1];
-        const double* ax = A.AX + (size_t)(j + 1) * MS;
-        for (int c = 0; c < t.sig[j + 1]; ++c) acc += q[c] * ax[c];
-      }
+    const int Sk = t.sig[k], ok = t.off[k], k0 = t.off[k + 1];
+    // every warp takes a slice of the bond range [off[k+1], send) for all s < Sk
+    const int len = send - k0, per = (len + nwarp - 1) / nwarp;
+    const int w0 = k0 + warp * per, w1 = min(send, w0 + per);
+    for (int s = 0; s < Sk; ++s) {
+      const double* q = b.QBS + (size_t)(ok + s) * S;
+      double acc = 0.0;
+      for (int kb = w0 + lane; kb < w1; kb += 32) acc += q[kb] * A.AXB[kb];
+      acc = warp_sum(acc);
+      if (lane == 0) part[warp][s] = acc;
     }
-    part[threadIdx.x] = acc;
     __syncthreads();
-    if (threadIdx.x < MS) {
+    if (tid < Sk) {
       double v = 0.0;
-      if (threadIdx.x < t.sig[k]) {
-        for (int g = 0; g < ngrp; ++g) v += part[g * CDZ_MAX_BOND + threadIdx.x];
-        for (int c = 0; c < t.sig[k + 1]; ++c)
-          v += t.Tbar[((size_t)k * MS + threadIdx.x) * MS + c] * A.AX[(size_t)(k + 1) * MS + c];
-      }
-      A.AX[(size_t)k * MS + threadIdx.x] = v;
+      for (int w = 0; w < nwarp; ++w) v += part[w][tid];
+      for (int c = 0; c < t.sig[k + 1]; ++c) v += t.Tbar[((size_t)k * MS + tid) * MS + c] * A.AX[(size_t)(k + 1) * MS + c];
+      A.AX[(size_t)k * MS + tid] = v;
+      A.AXB[ok + tid] = v;
     }
     __syncthreads();
+  }
+}
+
+// plain copies with the other orientation, upper block triangle only: QM1[(j+1,s)][(j'+1,c)] from QM1T, QMT[(k,s)][(i,a)] from QM
+__global__ void __launch_bounds__(256) transpose_kernel(const double* __restrict__ src, double* __restrict__ dst, int S, int src_lower) {
+  __shared__ double tile[CDZ_TB][CDZ_TB + 1];
+  const int bi = blockIdx.y, bj = blockIdx.x;  // source tile (bi, bj)
+  if (src_lower ? (bj > bi) : (bj < bi)) return;
+  for (int e = threadIdx.x; e < CDZ_TB * CDZ_TB; e += blockDim.x) {
+    const int r = e / CDZ_TB, c = e % CDZ_TB;
+    tile[r][c] = src[(size_t)(bi * CDZ_TB + r) * S + bj * CDZ_TB + c];
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < CDZ_TB * CDZ_TB; e += blockDim.x) {
+    const int r = e / CDZ_TB, c = e % CDZ_TB;
+    dst[(size_t)(bj * CDZ_TB + r) * S + bi * CDZ_TB + c] = tile[c][r];
   }
 }
 
 struct OV {
   const DevTT& t;
   const DevTab& b;
-  __device__ double E(int p, int q, int a, int c) const {
+  __device__ __forceinline__ double E(int p, int q, int a, int c) const {
     if (q < p) return a == c ? 1.0 : 0.0;
     return b.EM[(size_t)(t.off[p] + a) * t.S + t.off[q + 1] + c];
   }
 };
 
-// deterministic block sum: every thread holds the partial of entry e = tid % nent, group tid / nent; returns the total to tid < nent
+// shared-memory plan of ocell_kernel (doubles); identical on host and device
+struct OPlan {
+  int am, aml, abs_, ab, qb, ibs, go, h, h1, h2, ibsum, sbb, xe, bl, br, z1, z2, sb, y, inn, ddb, tl, tr, part, total;
+};
+__host__ __device__ inline OPlan oplan(int MS, int ML, int MR, int nps) {
+  OPlan p;
+  const int MS2 = MS * MS;
+  int o = 0;
+  auto take = [&](int k) { int r = o; o += (k + 1) & ~1; return r; };
+  p.am = take(MS2); p.aml = take(MS2); p.abs_ = take(MS2);
+  p.ab = take(ML * MR); p.qb = take(ML * MR);
+  p.ibs = take(nps * MS2); p.go = take(16 * MS2);
+  p.h = take(MS2); p.h1 = take(4 * MS2); p.h2 = take(4 * MS2);
+  p.ibsum = take(MS2); p.sbb = take(nps * MS2);
+  p.xe = take(MS2); p.bl = take(MS2); p.br = take(MS2);
+  p.z1 = take(ML * MS); p.z2 = take(MS * MR);
+  p.sb = take(nps * MS2); p.y = take(ML * MR); p.inn = take(nps * MS2);
+  p.ddb = take(ML * MR);
+  p.tl = take(3 * ML * MS); p.tr = take(3 * MS * MR);
+  p.part = take(OT);
+  p.total = o;
+  return p;
+}
+
+// deterministic block sum of per-thread partials laid out as [group][entry]: entry e = tid % nent, group tid / nent
 __device__ __forceinline__ double group_total(double* part, double v, int nent) {
   __syncthreads();
   part[threadIdx.x] = v;
   __syncthreads();
   double s = 0.0;
   if ((int)threadIdx.x < nent)
-    for (int g = 0; g * nent + (int)threadIdx.x < OT; ++g)
-      if (g < OT / nent) s += part[g * nent + threadIdx.x];
+    for (int g = 0; g < OT / nent; ++g) s += part[g * nent + threadIdx.x];
   return s;
 }
 
-// one diagonal d of the outside pass: CTA = cell (i, j = i + d)
-__global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d, double* __restrict__ bpp) {
+__global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d, int want_usage, double* __restrict__ bpp) {
+  extern __shared__ double osm[];
   const DevTT& t = ctx->tt;
   const DevTab& b = ctx->tab;
   const CModel& m = *ctx->cm;
   const OV V{t, b};
-  const int n = t.n, S = t.S, RS = t.RS, MS = t.MS, MS2 = MS * MS, tid = threadIdx.x;
-  const int i = blockIdx.x, j = i + d;
+  const int n = t.n, MS = t.MS, MS2 = MS * MS, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const size_t S = (size_t)t.S, RS = (size_t)t.RS;
+  const int ML = A.ML, MR = A.MR, nps = m.nps;
+  const OPlan pl = oplan(MS, ML, MR, nps);
+  double *am = osm + pl.am, *aml = osm + pl.aml, *abs_ = osm + pl.abs_, *ab = osm + pl.ab, *qbv = osm + pl.qb, *ibs = osm + pl.ibs,
+         *go = osm + pl.go, *h = osm + pl.h, *h1 = osm + pl.h1, *h2 = osm + pl.h2, *ibsum = osm + pl.ibsum, *sbb = osm + pl.sbb,
+         *xe = osm + pl.xe, *bl = osm + pl.bl, *br = osm + pl.br, *z1 = osm + pl.z1, *z2 = osm + pl.z2, *sb = osm + pl.sb,
+         *y = osm + pl.y, *inn = osm + pl.inn, *ddb = osm + pl.ddb, *part = osm + pl.part;
+  double* TLm = osm + pl.tl;            // T_{i-1}[lst][c]   (ML x MS)
+  double* TLi = TLm + ML * MS;          // T_i
+  double* TLp = TLi + ML * MS;          // T_{i+1}
+  double* TRq = osm + pl.tr;            // T_{j-1}[a][r]     (MS x MR)
+  double* TRj = TRq + MS * MR;          // T_j
+  double* TRn = TRj + MS * MR;          // T_{j+1}
+
+  const int i = blockIdx.x, j = i + d, p = i + 1, q = j - 1;
   const int Si = t.sig[i], Sj1 = t.sig[j + 1], offi = t.off[i], offj1 = t.off[j + 1];
   const int nent = Si * Sj1;
-  __shared__ double part[OT];
-  __shared__ double am[64], aml[64], abs_[64], ab[256], ibs[16 * 64];
-  __shared__ uint8_t lp1[128], lp2[128];
-  __shared__ double pv[OPV], pvg[64];
-  __shared__ int nlp;
-  if (tid == 0) {
-    int c = 0;
-    for (int l1 = 0; l1 <= m.max_interior; ++l1)
-      for (int l2 = 0; l1 + l2 <= m.max_interior; ++l2)
-        if (l1 == 0 || l2 == 0) { lp1[c] = (uint8_t)l1; lp2[c] = (uint8_t)l2; ++c; }  // stack + bulges; interior loops below
-    nlp = c;
-  }
-  const int ngrp = OT / nent, e = tid % nent, grp = tid / nent;
-  const bool act = grp < ngrp;
-  const int ea = e / Sj1, ec = e % Sj1;
-  // ---- Qm-bar(i,j)[a,s] = sum_{j'>j} sum_c M2-bar(i,j')[a,c] Qm1(j+1,j')[s,c]
-  {
-    double acc = 0.0;
-    if (act)
-      for (int jp = j + 1 + grp; jp < n; jp += ngrp) {
-        const int o = t.off[jp + 1];
-        const double* x = A.AM2 + (size_t)(offi + ea) * S + o;
-        const double* q = b.QM1T + (size_t)o * S + offj1 + ec;
-        for (int c = 0; c < t.sig[jp + 1]; ++c) acc += x[c] * q[(size_t)c * S];
+  const int mh1 = m.min_hairpin + 1, MI = m.max_interior;
+  const bool closed = d >= mh1;
+  const int nL = t.loff[i + 1] - t.loff[i], nR = t.roff[j + 1] - t.roff[j], npair = nL * nR;
+  const int Li0 = t.loff[i], Rj0 = t.roff[j];
+  const int send = t.off[n] + t.sig[n];
+
+  // ---- dense cores of the six positions around the cell ------------------------------------------------------------------------------
+  for (int k = tid; k < 3 * ML * MS + 3 * MS * MR; k += OT) (k < 3 * ML * MS ? TLm[k] : TRq[k - 3 * ML * MS]) = 0.0;
+  __syncthreads();
+  if (tid < 6) {
+    const int pos = tid < 3 ? i - 1 + tid : j - 1 + (tid - 3);
+    if (pos >= 0 && pos < n) {
+      for (int z = t.opstart[pos]; z < t.opstart[pos + 1]; ++z) {
+        if (tid < 3) TLm[tid * ML * MS + t.op_l[z] * MS + t.op_c[z]] += t.op_x[z];
+        else TRq[(tid - 3) * MS * MR + t.op_a[z] * MR + t.op_r[z]] += t.op_x[z];
       }
-    const double v = group_total(part, acc, nent);
-    if (tid < nent) am[tid] = v;
+    }
+  }
+  // ---- 1: bond-level adjoints ------------------------------------------------------------------------------------------------------------
+  // Qm-bar(i,j)[a,s] = sum_{kb >= off[j+2]} AM2[(i,a)][kb] QM1[(j+1,s)][kb]
+  for (int e = warp; e < nent; e += NW) {
+    const int ea = e / Sj1, ec = e % Sj1;
+    double v = 0.0;
+    if (j + 1 <= n - 1) v = warp_dot(A.AM2 + (size_t)(offi + ea) * S, A.QM1 + (size_t)(offj1 + ec) * S, t.off[j + 2], send, lane);
+    if (lane == 0) am[e] = v;
   }
   __syncthreads();
   if (tid < nent) {
-    // ---- M2-bar = Qm-bar + w_a w_c sum_{x,y} I(i-1,j+1)[x,y]
+    const int ea = tid / Sj1, ec = tid % Sj1;
+    // M2-bar = Qm-bar + w_a w_c sum_{x,y} I(i-1,j+1)[x,y]
     double v = am[tid];
     if (i >= 1 && j + 1 <= n - 1) {
       const double* ib = A.IB + ((size_t)((d + 2) % ORING) * n + (i - 1)) * 16 * MS2 + ea * MS + ec;
       double s = 0.0;
-      for (int sl = 0; sl < m.nps; ++sl) s += ib[sl * MS2];
+      for (int sl = 0; sl < nps; ++sl) s += ib[sl * MS2];
       v += m.wac * s;
     }
     A.AM2[(size_t)(offi + ea) * S + offj1 + ec] = v;
-    // ---- Qml-bar = Qm-bar + w_b Tbar_{i-1}^T Qml-bar(i-1,j)
+    A.AM2T[(size_t)(offj1 + ec) * S + offi + ea] = v;
+    // Qml-bar = Qm-bar + w_b Tbar_{i-1}^T Qml-bar(i-1,j)
     double w = am[tid];
     if (i >= 1) {
       double s = 0.0;
@@ -152,187 +229,94 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     aml[tid] = w;
     A.AML[(size_t)(offi + ea) * S + offj1 + ec] = w;
   }
-  // ---- Qm1-bar = Qml-bar + w_b Qm1-bar(i,j+1) Tbar_{j+1}^T + sum_{i'<i} Qm(i',i-1)^T M2-bar(i',j)
-  {
-    double acc = 0.0;
-    if (act)
-      for (int ip = grp; ip < i; ip += ngrp) {
-        const int o = t.off[ip];
-        for (int a2 = 0; a2 < t.sig[ip]; ++a2)
-          acc += b.QM[(size_t)(o + a2) * S + offi + ea] * A.AM2[(size_t)(o + a2) * S + offj1 + ec];
-      }
-    const double v = group_total(part, acc, nent);
-    if (tid < nent) {
-      double w = aml[tid] + v;
-      if (j + 1 <= n - 1) {
-        double s = 0.0;
-        for (int c2 = 0; c2 < t.sig[j + 2]; ++c2)
-          s += A.AM1[(size_t)(offi + ea) * S + t.off[j + 2] + c2] * t.Tbar[((size_t)(j + 1) * MS + ec) * MS + c2];
-        w += m.wb * s;
-      }
-      A.AM1[(size_t)(offi + ea) * S + offj1 + ec] = w;
-      // ---- Qbs-bar = w_c Qm1-bar + Qext(i-1)^T Qext-bar(j+1)
-      abs_[tid] = m.wc * w + b.Qext[offi + ea] * A.AX[(size_t)(j + 1) * MS + ec];
-    }
+  // Qm1-bar = Qml-bar + w_b Qm1-bar(i,j+1) Tbar_{j+1}^T + sum_{rb < off[i]} QMT[(i,a)][rb] AM2T[(j+1,c)][rb]
+  for (int e = warp; e < nent; e += NW) {
+    const int ea = e / Sj1, ec = e % Sj1;
+    const double v = warp_dot(A.QMT + (size_t)(offi + ea) * S, A.AM2T + (size_t)(offj1 + ec) * S, 0, offi, lane);
+    if (lane == 0) abs_[e] = v;
   }
   __syncthreads();
-  // ---- Qb-bar(k,l), (k,l) = this cell; closing pairs (i0,j0) = (k-1-l1, l+1+l2)
-  const int k = i, l = j;
-  const int nL = t.loff[k + 1] - t.loff[k], nR = t.roff[l + 1] - t.roff[l], npair = nL * nR;
-  const bool closable = d >= m.min_hairpin + 1;
-  // ---- interior loops l1, l2 >= 1 of the closing pairs (i0,j0) = (k-1-l1, l+1+l2).  With z2 at k-1 and z1' at l+1 the operators next to
-  //      the inner pair,   Qb-bar(k,l)[s,x',y',t] += sum_{z2: c = s} sum_{z1': a = t} e^{-beta tmm[p(y',x')][b(z1')][b(z2)]} x_z2 x_z1' * in(z2,z1'),
-  //      in = win[2] G(k-2,l+2)[a(z2),b(z2),b(z1'),c(z1')]  (1 x 1)  +  pv1[z2,c(z1')]  (l1 = 1)  +  pv2[z1',a(z2)]  (l2 = 1)  +  pvg[a(z2),c(z1')]
-  //      where the loop-side operators of the closing pair were pre-contracted with G by the closing cell (H, H1, H2 below) and the
-  //      unpaired stretches are E products.  Every sum runs in a fixed order: deterministic.
-  double accI = 0.0;
-  if (closable && k >= 2 && l + 2 <= n - 1) {
-    const int e2 = tid % npair;
-    const int ll = e2 / nR, rr = e2 % nR;
-    const int s = t.ls_a[t.loff[k] + ll], xp = t.ls_x[t.loff[k] + ll];
-    const int yp = t.rs_y[t.roff[l] + rr], tt_ = t.rs_c[t.roff[l] + rr];
-    const bool mine = tid < npair && m.pslot[xp * 4 + yp] >= 0;
-    const int Pin_il = m.ptype[yp * 4 + xp];
-    const int z2b = t.opstart[k - 1], z1pb = t.opstart[l + 1], nz1p = t.opstart[l + 2] - z1pb;
-    const int MI = m.max_interior;
-    // l1, l2 >= 2: both side stretches are E products, so the term depends on (z2, z1') only through the bonds a(z2), c(z1'):
-    //   pvg[a2,c1'] = sum_{l1,l2>=2} win[l1+l2] sum_{c1,a2'} E(i0+2,k-2)[c1,a2] H(i0,j0)[c1,a2'] E(l+2,j0-2)[c1',a2']
-    const int Sk1 = t.sig[k - 1], Sl2 = t.sig[l + 2], nentg = Sk1 * Sl2;
-    {
-      const int eg = tid % nentg, gg = tid / nentg, ngg = OT / nentg;
-      const int a2 = eg / Sl2, c1p = eg % Sl2;
-      double acc = 0.0;
-      if (gg < ngg)
-        for (int l1 = 2 + gg; l1 <= MI - 2; l1 += ngg) {
-          const int i0 = k - 1 - l1;
-          if (i0 < 0) break;
-          const int S1 = t.sig[i0 + 2];
-          for (int l2 = 2; l1 + l2 <= MI; ++l2) {
-            const int j0 = l + 1 + l2;
-            if (j0 > n - 1) break;
-            const int S2 = t.sig[j0 - 1];
-            const double* H = A.H + ((size_t)((j0 - i0) % ORING) * n + i0) * MS2;
-            double in = 0.0;
-            for (int c1 = 0; c1 < S1; ++c1) {
-              const double wl = V.E(i0 + 2, k - 2, c1, a2);
-              if (wl == 0.0) continue;
-              double r = 0.0;
-              for (int a2p = 0; a2p < S2; ++a2p) r += H[c1 * MS + a2p] * V.E(l + 2, j0 - 2, c1p, a2p);
-              in += wl * r;
-            }
-            acc += m.win[l1 + l2] * in;
-          }
-        }
-      const double tot = group_total(part, acc, nentg);
-      if (tid < nentg) pvg[tid] = tot;
+  if (tid < nent) {
+    const int ea = tid / Sj1, ec = tid % Sj1;
+    double w = aml[tid] + abs_[tid];
+    if (j + 1 <= n - 1) {
+      double s = 0.0;
+      for (int c2 = 0; c2 < t.sig[j + 2]; ++c2)
+        s += A.AM1T[(size_t)(t.off[j + 2] + c2) * S + offi + ea] * t.Tbar[((size_t)(j + 1) * MS + ec) * MS + c2];
+      w += m.wb * s;
     }
-    __syncthreads();  // pvg
-    // 1 x 1 loops (closing pair (k-2, l+2): G directly) and the generic part
-    const int nz2 = t.opstart[k] - z2b;
-    if (mine) {
-      const double* G11 = A.G + ((size_t)(((l + 2) - (k - 2)) % ORING) * n + (k - 2)) * 16 * MS2;
-      for (int z2 = z2b; z2 < z2b + nz2; ++z2) {
-        if (t.op_c[z2] != s) continue;
-        for (int z1p = z1pb; z1p < z1pb + nz1p; ++z1p) {
-          if (t.op_a[z1p] != tt_) continue;
-          accI += m.wtm[Pin_il][t.op_b[z1p]][t.op_b[z2]] * t.op_x[z2] * t.op_x[z1p] *
-                  (pvg[t.op_a[z2] * Sl2 + t.op_c[z1p]] +
-                   m.win[2] * G11[(t.op_b[z2] * 4 + t.op_b[z1p]) * MS2 + t.op_a[z2] * MS + t.op_c[z1p]]);
-        }
-      }
+    A.AM1T[(size_t)(offj1 + ec) * S + offi + ea] = w;
+    // Qbs-bar = w_c Qm1-bar + Qext(i-1)^T Qext-bar(j+1)
+    abs_[tid] = m.wc * w + b.Qext[offi + ea] * A.AX[(size_t)(j + 1) * MS + ec];
+  }
+  __syncthreads();
+  if (!closed) {
+    // cells below the minimum hairpin span: nothing pairs; the interior-body adjoint chains still pass through (d >= 4 only matters
+    // when min_hairpin + 1 > 4)
+    if (d >= 4) {
+      double* xa = A.XA + ((size_t)(d & 1) * n + i) * XU * MS2;
+      double* xb = A.XB + ((size_t)(d & 1) * n + i) * XU * MS2;
+      for (int e = tid; e < XU * MS2; e += OT) { xa[e] = 0.0; xb[e] = 0.0; }
     }
-    // l1 = 1, l2 >= 2: z1 = z2 carries both left mismatches; the right side is an E product ->
-    //   pv[z2,c1'] = sum_{l2} win[1+l2] sum_{a2'} E(l+2,j0-2)[c1',a2'] H1(k-2,j0)[a(z2),b(z2),a2']
-    for (int zb = 0; zb < nz2; zb += OZC) {
-      const int zc = min(OZC, nz2 - zb);
-      for (int e = tid; e < zc * Sl2; e += OT) {
-        const int z2 = z2b + zb + e / Sl2, c1p = e % Sl2, i0 = k - 2;
-        double v = 0.0;
-        for (int l2 = 2; l2 <= MI - 1; ++l2) {
-          const int j0 = l + 1 + l2;
-          if (j0 > n - 1) break;
-          const double* H1 = A.H1 + ((size_t)((j0 - i0) % ORING) * n + i0) * 4 * MS2 + (t.op_b[z2] * MS + t.op_a[z2]) * MS;
-          const int S2 = t.sig[j0 - 1];
-          double r = 0.0;
-          for (int a2p = 0; a2p < S2; ++a2p) r += V.E(l + 2, j0 - 2, c1p, a2p) * H1[a2p];
-          v += m.win[1 + l2] * r;
-        }
-        pv[e] = v;
-      }
-      __syncthreads();
-      if (mine)
-        for (int z2 = z2b + zb; z2 < z2b + zb + zc; ++z2) {
-          if (t.op_c[z2] != s) continue;
-          for (int z1p = z1pb; z1p < z1pb + nz1p; ++z1p) {
-            if (t.op_a[z1p] != tt_) continue;
-            accI += m.wtm[Pin_il][t.op_b[z1p]][t.op_b[z2]] * t.op_x[z2] * t.op_x[z1p] * pv[(z2 - z2b - zb) * Sl2 + t.op_c[z1p]];
-          }
-        }
-      __syncthreads();
-    }
-    // l2 = 1, l1 >= 2: z2' = z1' carries both right mismatches ->
-    //   pv[z1',a2] = sum_{l1} win[l1+1] sum_{c1} E(i0+2,k-2)[c1,a2] H2(i0,l+2)[c1,b(z1'),c(z1')]
-    for (int zb = 0; zb < nz1p; zb += OZC) {
-      const int zc = min(OZC, nz1p - zb);
-      for (int e = tid; e < zc * Sk1; e += OT) {
-        const int z1p = z1pb + zb + e / Sk1, a2 = e % Sk1, j0 = l + 2;
-        double v = 0.0;
-        for (int l1 = 2; l1 <= MI - 1; ++l1) {
-          const int i0 = k - 1 - l1;
-          if (i0 < 0) break;
-          const double* H2 = A.H2 + ((size_t)((j0 - i0) % ORING) * n + i0) * 4 * MS2 + (t.op_b[z1p] * MS) * MS + t.op_c[z1p];
-          const int S1 = t.sig[i0 + 2];
-          double r = 0.0;
-          for (int c1 = 0; c1 < S1; ++c1) r += V.E(i0 + 2, k - 2, c1, a2) * H2[c1 * MS];
-          v += m.win[l1 + 1] * r;
-        }
-        pv[e] = v;
-      }
-      __syncthreads();
-      if (mine)
-        for (int z1p = z1pb + zb; z1p < z1pb + zb + zc; ++z1p) {
-          if (t.op_a[z1p] != tt_) continue;
-          for (int z2 = z2b; z2 < z2b + nz2; ++z2) {
-            if (t.op_c[z2] != s) continue;
-            accI += m.wtm[Pin_il][t.op_b[z1p]][t.op_b[z2]] * t.op_x[z2] * t.op_x[z1p] * pv[(z1p - z1pb - zb) * Sk1 + t.op_a[z2]];
-          }
-        }
-      __syncthreads();
+    // the I slot of this diagonal is read by the M2-bar of cell (i+1, j-1): it must not keep the values of diagonal d + ORING
+    double* ibz = A.IB + ((size_t)(d % ORING) * n + i) * 16 * MS2;
+    for (int e = tid; e < 16 * MS2; e += OT) ibz[e] = 0.0;
+    return;
+  }
+
+  // ---- 2: Qb-bar(i,j) -------------------------------------------------------------------------------------------------------------------------
+  // the ring slot of this cell holds what closing cells pushed: adjoints of DD / GI / D1 / D2T stored at (i-1, j+1)
+  const bool dressed = MI >= 2 && i >= 1 && j <= n - 2;
+  const int nLm = dressed ? t.loff[i] - t.loff[i - 1] : 0, nRn = dressed ? t.roff[j + 2] - t.roff[j + 1] : 0;
+  const int RDS = ML * MR + MS2 + ML * MS + MR * MS;
+  double* rd = A.RD + ((size_t)(d % ORING) * n + i) * RDS;
+  if (dressed) {
+    const double *add = rd, *agi = rd + ML * MR, *ad1 = agi + MS2, *ad2 = ad1 + ML * MS;
+    for (int e = tid; e < nLm * nRn; e += OT) {
+      const int lst = e / nRn, rr = e % nRn;
+      const int a = t.ls_a[t.loff[i - 1] + lst], c = t.rs_c[t.roff[j + 1] + rr];
+      ddb[lst * MR + rr] = add[lst * MR + rr] + agi[a * MS + c] + ad1[lst * MS + c] + ad2[rr * MS + a];
     }
   }
+  for (int e = tid; e < npair; e += OT) qbv[e] = b.QB[(size_t)(Li0 + e / nR) * RS + Rj0 + e % nR];
+  __syncthreads();
+  if (dressed)
+    for (int e = tid; e < RDS; e += OT) rd[e] = 0.0;  // consumed: the slot is clean for diagonal d - ORING
   {
+    // stack / bulge terms: pulled from the I tables of the closing pairs (i0,j0) = (i-1-l1, j+1+l2), l1 = 0 or l2 = 0
     const int ng2 = OT / npair, e2 = tid % npair, g2 = tid / npair;
     const int ll = e2 / nR, rr = e2 % nR;
-    const int s = t.ls_a[t.loff[k] + ll], xp = t.ls_x[t.loff[k] + ll];
-    const int yp = t.rs_y[t.roff[l] + rr], tt_ = t.rs_c[t.roff[l] + rr];
+    const int s = t.ls_a[Li0 + ll], xp = t.ls_x[Li0 + ll];
+    const int yp = t.rs_y[Rj0 + rr], tt_ = t.rs_c[Rj0 + rr];
     const bool pairable = m.pslot[xp * 4 + yp] >= 0;
     double acc = 0.0;
-    if (g2 < ng2 && closable && pairable) {
+    if (g2 < ng2 && pairable) {
       const int Pin_st = m.ptype[xp * 4 + yp];  // inner pair as (phi_k, phi_l): stacks and size-1 bulges
-      for (int q = g2; q < nlp; q += ng2) {
-        const int l1 = lp1[q], l2 = lp2[q];
-        const int i0 = k - 1 - l1, j0 = l + 1 + l2;
+      const int nlp = 2 * MI + 1;
+      for (int qq = g2; qq < nlp; qq += ng2) {
+        const int l1 = qq <= MI ? qq : 0, l2 = qq <= MI ? 0 : qq - MI;
+        const int i0 = i - 1 - l1, j0 = j + 1 + l2;
         if (i0 < 0 || j0 > n - 1) continue;
         const int dd = j0 - i0;
         const int Sa = t.sig[i0 + 1], Sc = t.sig[j0];
         const double* ib = A.IB + ((size_t)(dd % ORING) * n + i0) * 16 * MS2;
         if (l1 == 0 && l2 == 0) {
-          for (int sl = 0; sl < m.nps; ++sl)
+          for (int sl = 0; sl < nps; ++sl)
             acc += m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][Pin_st] * ib[sl * MS2 + s * MS + tt_];
         } else if (l2 == 0) {
-          // left bulge: sum_{a'} E(i0+1,k-1)[a',s] I[x,y;a',t]
-          for (int sl = 0; sl < m.nps; ++sl) {
+          // left bulge: sum_{a'} E(i0+1,i-1)[a',s] I[x,y;a',t]
+          for (int sl = 0; sl < nps; ++sl) {
             const double w = m.wbu[l1] * (l1 == 1 ? m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][Pin_st] : 1.0);
             double v = 0.0;
-            for (int a = 0; a < Sa; ++a) v += V.E(i0 + 1, k - 1, a, s) * ib[sl * MS2 + a * MS + tt_];
+            for (int a = 0; a < Sa; ++a) v += V.E(i0 + 1, i - 1, a, s) * ib[sl * MS2 + a * MS + tt_];
             acc += w * v;
           }
-        } else if (l1 == 0) {
-          // right bulge: sum_{c'} I[x,y;s,c'] E(l+1,j0-1)[t,c']
-          for (int sl = 0; sl < m.nps; ++sl) {
+        } else {
+          // right bulge: sum_{c'} I[x,y;s,c'] E(j+1,j0-1)[t,c']
+          for (int sl = 0; sl < nps; ++sl) {
             const double w = m.wbu[l2] * (l2 == 1 ? m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][Pin_st] : 1.0);
             double v = 0.0;
-            for (int c = 0; c < Sc; ++c) v += ib[sl * MS2 + s * MS + c] * V.E(l + 1, j0 - 1, tt_, c);
+            for (int c = 0; c < Sc; ++c) v += ib[sl * MS2 + s * MS + c] * V.E(j + 1, j0 - 1, tt_, c);
             acc += w * v;
           }
         }
@@ -341,134 +325,546 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     const double v = group_total(part, acc, npair);
     if (tid < npair) {
       double w = 0.0;
-      if (closable && pairable) w = v + accI + abs_[s * Sj1 + tt_];
+      if (pairable) {
+        w = v + abs_[s * Sj1 + tt_];
+        if (dressed) {
+          // interior loops: Qb(i,j) enters through its dressed extension DD(i-1,j+1)[lst][rr] = sum T_{i-1}[lst][s] T_{j+1}[t][rr]
+          // e^{-beta tmm[p(y',x')][y(rr)][x(lst)]} Qb[(s,x')][(y',t)]
+          const int Pil = m.ptype[yp * 4 + xp];
+          double u = 0.0;
+          for (int lst = 0; lst < nLm; ++lst) {
+            const double tl = TLm[lst * MS + s];
+            if (tl == 0.0) continue;
+            const int up = t.ls_x[t.loff[i - 1] + lst];
+            double r2 = 0.0;
+            for (int r = 0; r < nRn; ++r)
+              r2 += TRn[tt_ * MR + r] * m.wtm[Pil][t.rs_y[t.roff[j + 1] + r]][up] * ddb[lst * MR + r];
+            u += tl * r2;
+          }
+          w += u;
+        }
+      }
       ab[tid] = w;
-      A.AB[(size_t)(t.loff[k] + ll) * RS + t.roff[l] + rr] = w;
-      part[tid] = w * b.QB[(size_t)(t.loff[k] + ll) * RS + t.roff[l] + rr];
+      A.AB[(size_t)(Li0 + ll) * RS + Rj0 + rr] = w;
+      part[tid] = w * qbv[tid];
     }
     __syncthreads();
-    if (tid == 0) {
-      double p = 0.0;
-      for (int q = 0; q < npair; ++q) p += part[q];
-      if (d > 0) bpp[(size_t)i * n + j] = p;
+    if (tid == 0 && bpp && d > 0) {
+      double pr = 0.0;
+      for (int e = 0; e < npair; ++e) pr += part[e];
+      bpp[(size_t)i * n + j] = pr;
+    }
+    __syncthreads();
+  }
+  // usages of the inner-mismatch operators z2 at i-1 (role IL) and z1' at j+1 (role IR)
+  if (want_usage && dressed) {
+    const int z2b = t.opstart[i - 1], nz2 = t.opstart[i] - z2b, z1b = t.opstart[j + 1], nz1 = t.opstart[j + 2] - z1b;
+    for (int e = tid; e < nz2 + nz1; e += OT) {
+      double u = 0.0;
+      if (e < nz2) {
+        const int z = z2b + e, lst = t.op_l[z], s = t.op_c[z], up = t.op_b[z];
+        for (int ll = 0; ll < nL; ++ll) {
+          if (t.ls_a[Li0 + ll] != s) continue;
+          const int xp = t.ls_x[Li0 + ll];
+          for (int rr = 0; rr < nR; ++rr) {
+            const int yp = t.rs_y[Rj0 + rr], tt_ = t.rs_c[Rj0 + rr];
+            if (m.pslot[xp * 4 + yp] < 0) continue;
+            const int Pil = m.ptype[yp * 4 + xp];
+            double r2 = 0.0;
+            for (int r = 0; r < nRn; ++r)
+              r2 += TRn[tt_ * MR + r] * m.wtm[Pil][t.rs_y[t.roff[j + 1] + r]][up] * ddb[lst * MR + r];
+            u += r2 * qbv[ll * nR + rr];
+          }
+        }
+        A.U[(size_t)ROLE_IL * A.nops + z] += t.op_x[z] * u;
+      } else {
+        const int z = z1b + (e - nz2), r = t.op_r[z], tt_ = t.op_a[z], vp = t.op_b[z];
+        for (int rr = 0; rr < nR; ++rr) {
+          if (t.rs_c[Rj0 + rr] != tt_) continue;
+          const int yp = t.rs_y[Rj0 + rr];
+          for (int ll = 0; ll < nL; ++ll) {
+            const int xp = t.ls_x[Li0 + ll], s = t.ls_a[Li0 + ll];
+            if (m.pslot[xp * 4 + yp] < 0) continue;
+            const int Pil = m.ptype[yp * 4 + xp];
+            double r2 = 0.0;
+            for (int lst = 0; lst < nLm; ++lst)
+              r2 += TLm[lst * MS + s] * m.wtm[Pil][vp][t.ls_x[t.loff[i - 1] + lst]] * ddb[lst * MR + r];
+            u += r2 * qbv[ll * nR + rr];
+          }
+        }
+        A.U[(size_t)ROLE_IR * A.nops + z] += t.op_x[z] * u;
+      }
     }
   }
-  __syncthreads();
-  // ---- I(i,j)[slot][a'][c'] and G(i,j)[u,v][a'][c'] for the inner cells of this pair
-  const int Sa = t.sig[i + 1], Sc = t.sig[j];
+
+  // ---- 3: I(i,j)[slot][a'][c'], G[u,v][a'][c'], H, H1, H2 ----------------------------------------------------------------------------------
+  const int Sa = t.sig[p], Sc = t.sig[j];  // a' in Sigma_{i+1}, c' in Sigma_j
   double* ibo = A.IB + ((size_t)(d % ORING) * n + i) * 16 * MS2;
-  double* go = A.G + ((size_t)(d % ORING) * n + i) * 16 * MS2;
-  for (int q = tid; q < 16 * MS2; q += OT) {
-    const int sl = q / MS2, ap = (q % MS2) / MS, cp = q % MS;
+  for (int e = tid; e < 16 * MS2; e += OT) {
+    const int sl = e / MS2, ap = (e % MS2) / MS, cp = e % MS;
     double v = 0.0;
-    if (sl < m.nps && ap < Sa && cp < Sc && closable && d >= 1) {
-      const int x = m.slot_x[sl], y = m.slot_y[sl];
+    if (sl < nps && ap < Sa && cp < Sc) {
+      const int x = m.slot_x[sl], yy = m.slot_y[sl];
       for (int z = t.opstart[i]; z < t.opstart[i + 1]; ++z) {
         if (t.op_b[z] != x || t.op_c[z] != ap) continue;
         for (int zz = t.opstart[j]; zz < t.opstart[j + 1]; ++zz) {
-          if (t.op_b[zz] != y || t.op_a[zz] != cp) continue;
+          if (t.op_b[zz] != yy || t.op_a[zz] != cp) continue;
           v += t.op_x[z] * t.op_x[zz] * ab[t.op_l[z] * nR + t.op_r[zz]];
         }
       }
     }
-    ibs[q] = v;
-    ibo[q] = v;
+    if (sl < nps) ibs[e] = v;
+    ibo[e] = v;
   }
   __syncthreads();
-  for (int q = tid; q < 16 * MS2; q += OT) {
-    const int uv = q / MS2, r = q % MS2;
+  for (int e = tid; e < 16 * MS2; e += OT) {
+    const int uv = e / MS2, r = e % MS2;
     double v = 0.0;
-    for (int sl = 0; sl < m.nps; ++sl)
-      v += ibs[sl * MS2 + r] * m.wtm[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][uv >> 2][uv & 3];
-    go[q] = v;
+    for (int sl = 0; sl < nps; ++sl) v += ibs[sl * MS2 + r] * m.wtm[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][uv >> 2][uv & 3];
+    go[e] = v;
   }
-  // ---- H(i,j)[c1,a2'] = sum_{z1 at i+1: c = c1} sum_{z2' at j-1: a = a2'} x_z1 x_z2' G(i,j)[a(z1),b(z1),b(z2'),c(z2')]
-  //      (both loop-side operators of an interior loop with l1, l2 >= 2 closed by this pair)
-  __syncthreads();
-  double* ho = A.H + ((size_t)(d % ORING) * n + i) * MS2;
-  for (int q = tid; q < MS2; q += OT) {
-    const int c1 = q / MS, a2p = q % MS;
+  for (int e = tid; e < MS2; e += OT) {
     double v = 0.0;
-    if (closable && j - 1 > i + 1)
-      for (int z1 = t.opstart[i + 1]; z1 < t.opstart[i + 2]; ++z1) {
+    for (int sl = 0; sl < nps; ++sl) v += ibs[sl * MS2 + e];
+    ibsum[e] = v;  // adjoint of Bl / Br / the multiloop closure: they enter `inner` of every pairable slot
+  }
+  for (int e = tid; e < nps * MS2; e += OT) {
+    // adjoint of SB[a'][slot'][c'] (stored [slot'][a'][c']):  sum_slot wst[P][P'] I[slot]
+    const int sl2 = e / MS2, r = e % MS2;
+    const int P2 = m.ptype[m.slot_x[sl2] * 4 + m.slot_y[sl2]];
+    double v = 0.0;
+    for (int sl = 0; sl < nps; ++sl) v += m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][P2] * ibs[sl * MS2 + r];
+    sbb[e] = v;
+  }
+  __syncthreads();
+  const bool has_loop = q > p;  // positions i+1 and j-1 are distinct unpaired positions (always true for min_hairpin >= 3)
+  // H[c1][a2'] = sum_{z1 at p: c = c1} sum_{z2' at q: a = a2'} x x' G[b(z1),b(z2')][a(z1)][c(z2')]     (adjoint of XE)
+  for (int e = tid; e < MS2; e += OT) {
+    const int c1 = e / MS, a2p = e % MS;
+    double v = 0.0;
+    if (has_loop)
+      for (int z1 = t.opstart[p]; z1 < t.opstart[p + 1]; ++z1) {
         if (t.op_c[z1] != c1) continue;
         const double* Gz = go + (t.op_b[z1] * 4) * MS2 + t.op_a[z1] * MS;
-        for (int z2p = t.opstart[j - 1]; z2p < t.opstart[j]; ++z2p)
+        for (int z2p = t.opstart[q]; z2p < t.opstart[q + 1]; ++z2p)
           if (t.op_a[z2p] == a2p) v += t.op_x[z1] * t.op_x[z2p] * Gz[t.op_b[z2p] * MS2 + t.op_c[z2p]];
       }
-    ho[q] = v;
+    h[e] = v;
   }
-  // ---- H1(i,j)[u,a,a2'] = sum_{z2' at j-1: a = a2'} x_z2' G[a,u,b(z2'),c(z2')]   (l1 = 1: the operator at i+1 stays open)
-  //      H2(i,j)[v,c1,c'] = sum_{z1 at i+1: c = c1} x_z1 G[a(z1),b(z1),v,c']       (l2 = 1: the operator at j-1 stays open)
-  double* h1o = A.H1 + ((size_t)(d % ORING) * n + i) * 4 * MS2;
-  double* h2o = A.H2 + ((size_t)(d % ORING) * n + i) * 4 * MS2;
-  for (int q = tid; q < 8 * MS2; q += OT) {
-    const int which = q / (4 * MS2), r = q % (4 * MS2);
+  // H1[u][a][a2'] = sum_{z2' at q: a = a2'} x' G[u,b(z2')][a][c(z2')]   (adjoint of Z1);  H2[v][c1][c'] = sum_{z1 at p: c = c1} x G[b(z1),v][a(z1)][c']
+  for (int e = tid; e < 8 * MS2; e += OT) {
+    const int which = e / (4 * MS2), r = e % (4 * MS2);
     const int uv = r / MS2, x1 = (r % MS2) / MS, x2 = r % MS;
     double v = 0.0;
-    if (closable && j - 1 > i + 1) {
-      if (which == 0) {  // u = uv, a = x1, a2' = x2
-        for (int z2p = t.opstart[j - 1]; z2p < t.opstart[j]; ++z2p)
+    if (has_loop) {
+      if (which == 0) {
+        for (int z2p = t.opstart[q]; z2p < t.opstart[q + 1]; ++z2p)
           if (t.op_a[z2p] == x2) v += t.op_x[z2p] * go[(uv * 4 + t.op_b[z2p]) * MS2 + x1 * MS + t.op_c[z2p]];
-      } else {  // v = uv, c1 = x1, c' = x2
-        for (int z1 = t.opstart[i + 1]; z1 < t.opstart[i + 2]; ++z1)
+      } else {
+        for (int z1 = t.opstart[p]; z1 < t.opstart[p + 1]; ++z1)
           if (t.op_c[z1] == x1) v += t.op_x[z1] * go[(t.op_b[z1] * 4 + uv) * MS2 + t.op_a[z1] * MS + x2];
       }
     }
-    (which == 0 ? h1o : h2o)[r] = v;
+    (which == 0 ? h1 : h2)[r] = v;
   }
-}
+  __syncthreads();
 
-__global__ void unpaired_kernel(int n, double* __restrict__ bpp) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  double s = 0.0;
-  for (int j = i + 1; j < n; ++j) s += bpp[(size_t)i * n + j];
-  for (int j = 0; j < i; ++j) s += bpp[(size_t)j * n + i];
-  bpp[(size_t)i * n + i] = 1.0 - s;
+  // ---- 4: this cell as closing pair ---------------------------------------------------------------------------------------------------------
+  const int Sp1 = t.sig[p + 1], Sq = t.sig[q];  // bonds after i+1 / before j-1: XE, H are Sp1 x Sq
+  const int nLp = t.loff[p + 1] - t.loff[p], nRq = t.roff[q + 1] - t.roff[q];
+  const int Lp0 = t.loff[p], Rq0 = t.roff[q];
+  // 4a hairpin interior E(p+1,q-1): its adjoint is w_H(d-1) H (single writer: plain store into the transposed table)
+  {
+    const double wh = t.wh[d - 1];
+    for (int e = tid; e < Sp1 * Sq; e += OT) {
+      const int cz = e / Sq, aw = e % Sq;
+      A.AET[(size_t)(t.off[q] + aw) * S + t.off[p + 1] + cz] = wh * h[cz * MS + aw];
+    }
+  }
+  // 4b adjoint row / column recursions of the interior-loop bodies (u = 4..30):
+  //      XA_u(i,j) = w_In(u) H + Tbar_{i+1}^T XA_{u+1}(i-1,j)          XB_u(i,j) = w_In(u) H + XB_{u+1}(i,j+1) Tbar_{j-1}^T
+  double* xa = A.XA + ((size_t)(d & 1) * n + i) * XU * MS2;
+  double* xb = A.XB + ((size_t)(d & 1) * n + i) * XU * MS2;
+  {
+    const double* xa1 = i >= 1 ? A.XA + ((size_t)((d + 1) & 1) * n + (i - 1)) * XU * MS2 : nullptr;
+    const double* xb1 = j + 1 <= n - 1 ? A.XB + ((size_t)((d + 1) & 1) * n + i) * XU * MS2 : nullptr;
+    for (int e = tid; e < XU * MS2; e += OT) {
+      const int u4 = e / MS2, cz = (e % MS2) / MS, aw = e % MS, u = u4 + 4;
+      double va = 0.0, vb = 0.0;
+      if (cz < Sp1 && aw < Sq) {
+        const double w = u <= MI ? m.win[u] * h[cz * MS + aw] : 0.0;
+        va = vb = w;
+        if (u4 + 1 < XU) {
+          if (xa1) {
+            const double* src = xa1 + (u4 + 1) * MS2 + aw;
+            for (int a = 0; a < t.sig[p]; ++a) va += t.Tbar[((size_t)p * MS + a) * MS + cz] * src[a * MS];
+          }
+          if (xb1) {
+            const double* src = xb1 + (u4 + 1) * MS2 + cz * MS;
+            for (int c = 0; c < t.sig[j]; ++c) vb += src[c] * t.Tbar[((size_t)q * MS + aw) * MS + c];
+          }
+        }
+      }
+      xa[e] = va;
+      xb[e] = vb;
+    }
+  }
+  __syncthreads();
+  // 4c pushes of the generic interior loops (l1, l2 >= 2).  All terms of X_u(i,j) have the inner span d-2-u.
+  if (MI >= 4) {
+    // row recursion, new term GI(i+3, l) E(l+2,j-2), l = j+1-u:  adjoint of GI into the ring slot of cell (i+3,l); E-bar of the right stretch
+    for (int e = tid; e < XU * MS2; e += OT) {
+      const int u4 = e / MS2, x1 = (e % MS2) / MS, x2 = e % MS, u = u4 + 4;
+      if (d - 2 - u < mh1) continue;
+      const int l = j + 1 - u, k = i + 3;  // inner pair (k,l): l1 = 2, l2 = u-2
+      const int Sk1 = Sp1 /* Sigma_{k-1} = Sigma_{i+2} */, Sl2 = t.sig[l + 2];
+      const double* xau = xa + u4 * MS2;
+      // AGI(k,l)[s2 = x1][t2 = x2] += sum_aw XA_u[s2][aw] E(l+2,j-2)[t2][aw]
+      if (x1 < Sk1 && x2 < Sl2) {
+        double v = 0.0;
+        for (int aw = 0; aw < Sq; ++aw) v += xau[x1 * MS + aw] * V.E(l + 2, j - 2, x2, aw);
+        double* rdk = A.RD + ((size_t)((l - k) % ORING) * n + k) * RDS + ML * MR;
+        rdk[x1 * MS + x2] += v;
+      }
+      // E-bar(l+2, j-2)[t2 = x1][aw = x2] += sum_s2 GI(k,l)[s2][t2] XA_u[s2][aw]       (length u-4 >= 1)
+      if (want_usage && u > 4 && x1 < Sl2 && x2 < Sq) {
+        const double* gi = b.GI + (size_t)t.off[k - 1] * S + t.off[l + 2] + x1;
+        double v = 0.0;
+        for (int s2 = 0; s2 < Sk1; ++s2) v += gi[(size_t)s2 * S] * xau[s2 * MS + x2];
+        A.AES[(((size_t)AES_XR * n + (l + 2)) * SLEN + (u - 4)) * MS2 + x1 * MS + x2] += v;
+      }
+    }
+    // column recursion, new term E(i+2,k-2) GI(k, j-3), k = i+u-1:  E-bar of the left stretch (length u-4 >= 1)
+    if (want_usage)
+      for (int e = tid; e < XU * MS2; e += OT) {
+        const int u4 = e / MS2, cz = (e % MS2) / MS, s2 = e % MS, u = u4 + 4;
+        if (u == 4 || d - 2 - u < mh1) continue;
+        const int k = i + u - 1, l = j - 3;
+        if (cz >= Sp1 || s2 >= t.sig[k - 1]) continue;
+        const double* gi = b.GI + (size_t)(t.off[k - 1] + s2) * S + t.off[l + 2];  // columns: bonds of position l+2 = j-1
+        const double* xbu = xb + u4 * MS2 + cz * MS;
+        double v = 0.0;
+        for (int aw = 0; aw < Sq; ++aw) v += xbu[aw] * gi[aw];
+        A.AES[(((size_t)AES_XL * n + (i + 2)) * SLEN + (u - 4)) * MS2 + cz * MS + s2] += v;
+      }
+  }
+  // 4d pushes of the l1 = 1 / l2 = 1 / 1x1 interior loops
+  if (MI >= 2) {
+    // 1 x 1: inner pair (i+2, j-2), DD(p,q) enters Y with w_In(2)
+    if (d - 4 >= mh1) {
+      double* rdk = A.RD + ((size_t)((d - 4) % ORING) * n + (i + 2)) * RDS;
+      for (int e = tid; e < nLp * nRq; e += OT) {
+        const int lst = e / nRq, r = e % nRq;
+        rdk[lst * MR + r] += m.win[2] * go[(t.ls_x[Lp0 + lst] * 4 + t.rs_y[Rq0 + r]) * MS2 + t.ls_a[Lp0 + lst] * MS + t.rs_c[Rq0 + r]];
+      }
+    }
+    // l1 = 1, l2 = 2..: Z1[lst][c2] = sum_l2 w_In(1+l2) sum_u D1(p; l+2)[lst][u] E(l+2,q-1)[u][c2],  l = q - l2; inner pair (i+2, l)
+    {
+      const int lmax = min(MI - 1, q - mh1 - (p + 1));
+      for (int l2 = 2; l2 <= lmax; ++l2) {
+        const int l = q - l2, Su = t.sig[l + 2];
+        double* rdk = A.RD + ((size_t)((l - (i + 2)) % ORING) * n + (i + 2)) * RDS + ML * MR + MS2;  // AD1[lst][u]
+        const double w = m.win[1 + l2];
+        for (int e = tid; e < nLp * Su; e += OT) {
+          const int lst = e / Su, u = e % Su;
+          const double* hz = h1 + (t.ls_x[Lp0 + lst] * MS + t.ls_a[Lp0 + lst]) * MS;  // Z1-bar[lst][c2] = H1[x(lst)][a(lst)][c2]
+          double v = 0.0;
+          for (int c2 = 0; c2 < Sq; ++c2) v += hz[c2] * V.E(l + 2, q - 1, u, c2);
+          rdk[lst * MS + u] += w * v;
+        }
+        if (want_usage && l2 > 2)
+          for (int e = tid; e < Su * Sq; e += OT) {
+            const int u = e / Sq, c2 = e % Sq;
+            double v = 0.0;
+            for (int lst = 0; lst < nLp; ++lst)
+              v += b.D1[(size_t)(Lp0 + lst) * S + t.off[l + 2] + u] * h1[(t.ls_x[Lp0 + lst] * MS + t.ls_a[Lp0 + lst]) * MS + c2];
+            A.AES[(((size_t)AES_Z1R * n + (l + 2)) * SLEN + (l2 - 2)) * MS2 + u * MS + c2] += w * v;
+          }
+      }
+    }
+    // l2 = 1, l1 = 2..: Z2[a2][r] = sum_l1 w_In(l1+1) sum_s E(p+1,k-2)[a2][s] D2(k-1; q)[s][r],  k = p + l1; inner pair (k, j-2)
+    {
+      const int lmax = min(MI - 1, (q - 1) - mh1 - p);
+      for (int l1 = 2; l1 <= lmax; ++l1) {
+        const int k = p + l1, Ss = t.sig[k - 1];
+        double* rdk = A.RD + ((size_t)(((j - 2) - k) % ORING) * n + k) * RDS + ML * MR + MS2 + ML * MS;  // AD2[r][s]
+        const double w = m.win[l1 + 1];
+        for (int e = tid; e < nRq * Ss; e += OT) {
+          const int r = e / Ss, s = e % Ss;
+          const double* hz = h2 + (t.rs_y[Rq0 + r] * MS) * MS + t.rs_c[Rq0 + r];  // Z2-bar[a2][r] = H2[y(r)][a2][c(r)]
+          double v = 0.0;
+          for (int a2 = 0; a2 < Sp1; ++a2) v += V.E(p + 1, k - 2, a2, s) * hz[a2 * MS];
+          rdk[r * MS + s] += w * v;
+        }
+        if (want_usage && l1 > 2)
+          for (int e = tid; e < Sp1 * Ss; e += OT) {
+            const int a2 = e / Ss, s = e % Ss;
+            double v = 0.0;
+            for (int r = 0; r < nRq; ++r)
+              v += h2[(t.rs_y[Rq0 + r] * MS + a2) * MS + t.rs_c[Rq0 + r]] * b.D2T[(size_t)(Rq0 + r) * S + t.off[k - 1] + s];
+            A.AES[(((size_t)AES_Z2L * n + (p + 1)) * SLEN + (l1 - 2)) * MS2 + a2 * MS + s] += w * v;
+          }
+      }
+    }
+  }
+  if (!want_usage) return;
+  // 4e stretch adjoints of the bulges of size >= 2:  Bl = .. + sum_l1 w_Bu(l1) E(p,k-1) Qbs(k,q),  Br = sum_l2 w_Bu(l2) Qbs(p,l) E(l+1,q)
+  {
+    const int lmax = min(MI, q - mh1 - p);
+    for (int e = tid; e < (lmax >= 2 ? (lmax - 1) * 2 * MS2 : 0); e += OT) {
+      const int side = e / ((lmax - 1) * MS2), r = e % ((lmax - 1) * MS2);
+      const int len = 2 + r / MS2, x1 = (r % MS2) / MS, x2 = r % MS;
+      if (side == 0) {
+        const int k = p + len;  // E(p,k-1)[a1 = x1][s = x2]
+        if (x1 >= Sa || x2 >= t.sig[k]) continue;
+        const double* qs = b.QBS + (size_t)(t.off[k] + x2) * S + t.off[j];
+        double v = 0.0;
+        for (int c1 = 0; c1 < Sc; ++c1) v += ibsum[x1 * MS + c1] * qs[c1];
+        A.AES[(((size_t)AES_BL * n + p) * SLEN + len) * MS2 + x1 * MS + x2] += m.wbu[len] * v;
+      } else {
+        const int l = q - len;  // E(l+1,q)[u = x1][c1 = x2]
+        if (x1 >= t.sig[l + 1] || x2 >= Sc) continue;
+        double v = 0.0;
+        for (int a1 = 0; a1 < Sa; ++a1) v += b.QBS[(size_t)(t.off[p] + a1) * S + t.off[l + 1] + x1] * ibsum[a1 * MS + x2];
+        A.AES[(((size_t)AES_BR * n + (l + 1)) * SLEN + len) * MS2 + x1 * MS + x2] += m.wbu[len] * v;
+      }
+    }
+  }
+  // 4f forward quantities of this cell, recomputed from the stored tables exactly as the inside pass builds them
+  {
+    const int lmaxB = min(MI, q - mh1 - p);
+    const int lmaxZ1 = min(MI - 1, q - mh1 - (p + 1)), lmaxZ2 = min(MI - 1, (q - 1) - mh1 - p);
+    for (int e = tid; e < Sp1 * Sq; e += OT) xe[(e / Sq) * MS + e % Sq] = b.XE[(size_t)(t.off[p + 1] + e / Sq) * S + t.off[q] + e % Sq];
+    // Bl, Br  [a1 < Sa][c1 < Sc]
+    for (int e = tid; e < 2 * Sa * Sc; e += OT) {
+      const int side = e / (Sa * Sc), a1 = (e % (Sa * Sc)) / Sc, c1 = e % Sc;
+      double v = 0.0;
+      if (side == 0) {
+        v = m.wac * b.M2[(size_t)(t.off[p] + a1) * S + t.off[j] + c1];
+        const double* A_ = b.EM + (size_t)(t.off[p] + a1) * S;
+        const double* B_ = b.QBST + (size_t)(t.off[j] + c1) * S;
+        for (int l1 = 2; l1 <= lmaxB; ++l1) {
+          const int k = p + l1;
+          double s = 0.0;
+          for (int kb = t.off[k]; kb < t.off[k] + t.sig[k]; ++kb) s += A_[kb] * B_[kb];
+          v += m.wbu[l1] * s;
+        }
+        bl[a1 * MS + c1] = v;
+      } else {
+        const double* A_ = b.QBS + (size_t)(t.off[p] + a1) * S;
+        const double* B_ = b.EMT + (size_t)(t.off[j] + c1) * S;
+        for (int l2 = 2; l2 <= lmaxB; ++l2) {
+          const int l = q - l2;
+          double s = 0.0;
+          for (int kb = t.off[l + 1]; kb < t.off[l + 1] + t.sig[l + 1]; ++kb) s += A_[kb] * B_[kb];
+          v += m.wbu[l2] * s;
+        }
+        br[a1 * MS + c1] = v;
+      }
+    }
+    // Z1[lst][c2 < Sq], Z2[a2 < Sp1][r]
+    for (int e = tid; e < nLp * Sq + Sp1 * nRq; e += OT) {
+      double v = 0.0;
+      if (e < nLp * Sq) {
+        const int lst = e / Sq, c2 = e % Sq;
+        const double* A_ = b.D1 + (size_t)(Lp0 + lst) * S;
+        const double* B_ = b.EMT + (size_t)(t.off[q] + c2) * S;
+        for (int l2 = 2; l2 <= lmaxZ1; ++l2) {
+          const int l = q - l2;
+          double s = 0.0;
+          for (int kb = t.off[l + 2]; kb < t.off[l + 2] + t.sig[l + 2]; ++kb) s += A_[kb] * B_[kb];
+          v += m.win[1 + l2] * s;
+        }
+        z1[lst * MS + c2] = v;
+      } else {
+        const int a2 = (e - nLp * Sq) / nRq, r = (e - nLp * Sq) % nRq;
+        const double* A_ = b.EM + (size_t)(t.off[p + 1] + a2) * S;
+        const double* B_ = b.D2T + (size_t)(Rq0 + r) * S;
+        for (int l1 = 2; l1 <= lmaxZ2; ++l1) {
+          const int k = p + l1;
+          double s = 0.0;
+          for (int kb = t.off[k - 1]; kb < t.off[k - 1] + t.sig[k - 1]; ++kb) s += A_[kb] * B_[kb];
+          v += m.win[l1 + 1] * s;
+        }
+        z2[a2 * MR + r] = v;
+      }
+    }
+    // SB[slot'][a1][c1]: stack + size-1 bulges (the inner pair keeps its identity)
+    for (int e = tid; e < nps * Sa * Sc; e += OT) {
+      const int sl = e / (Sa * Sc), a1 = (e % (Sa * Sc)) / Sc, c1 = e % Sc;
+      const int xp = m.slot_x[sl], yp = m.slot_y[sl];
+      const int lst = t.lsidx[((size_t)p * MS + a1) * 4 + xp], r = t.rsidx[((size_t)q * 4 + yp) * MS + c1];
+      double v = 0.0;
+      if (q - p >= mh1 && lst >= 0 && r >= 0) v = b.QB[(size_t)(Lp0 + lst) * RS + Rq0 + r];
+      if (MI >= 1 && q - (p + 1) >= mh1) {
+        double s1 = 0.0, s2 = 0.0;
+        if (r >= 0)
+          for (int l2 = t.loff[p + 1]; l2 < t.loff[p + 2]; ++l2)
+            if (t.ls_x[l2] == xp) s1 += t.Tbar[((size_t)p * MS + a1) * MS + t.ls_a[l2]] * b.QB[(size_t)l2 * RS + Rq0 + r];
+        if (lst >= 0)
+          for (int r2 = t.roff[q - 1]; r2 < t.roff[q]; ++r2)
+            if (t.rs_y[r2] == yp) s2 += b.QB[(size_t)(Lp0 + lst) * RS + r2] * t.Tbar[((size_t)q * MS + t.rs_c[r2]) * MS + c1];
+        v += m.wbu[1] * (s1 + s2);
+      }
+      sb[sl * MS2 + a1 * MS + c1] = v;
+    }
+  }
+  __syncthreads();
+  {
+    // Y[lst][r] = w_In(2) DD(p,q) + sum_cz T_p[lst][cz] (Z2[cz][r] + sum_aw XE[cz][aw] T_q[aw][r]) + sum_aw Z1[lst][aw] T_q[aw][r]
+    const bool v11 = MI >= 2 && d - 4 >= mh1;
+    for (int e = tid; e < nLp * nRq; e += OT) {
+      const int lst = e / nRq, r = e % nRq;
+      double v = v11 ? m.win[2] * b.DD[(size_t)(Lp0 + lst) * RS + Rq0 + r] : 0.0;
+      for (int cz = 0; cz < Sp1; ++cz) {
+        const double tl = TLp[lst * MS + cz];
+        if (tl == 0.0) continue;
+        double s = z2[cz * MR + r];
+        for (int aw = 0; aw < Sq; ++aw) s += xe[cz * MS + aw] * TRq[aw * MR + r];
+        v += tl * s;
+      }
+      for (int aw = 0; aw < Sq; ++aw) v += z1[lst * MS + aw] * TRq[aw * MR + r];
+      y[lst * MR + r] = v;
+    }
+  }
+  __syncthreads();
+  // inner[slot][a1][c1] = Bl + Br + sum_slot' wst[P][P'] SB[slot'] + sum_{(a1,u),(v,c1)} wtm[P][u][v] Y
+  for (int e = tid; e < nps * Sa * Sc; e += OT) {
+    const int sl = e / (Sa * Sc), a1 = (e % (Sa * Sc)) / Sc, c1 = e % Sc;
+    const int P = m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]];
+    double v = bl[a1 * MS + c1] + br[a1 * MS + c1];
+    for (int s2 = 0; s2 < nps; ++s2) v += m.wst[P][m.ptype[m.slot_x[s2] * 4 + m.slot_y[s2]]] * sb[s2 * MS2 + a1 * MS + c1];
+    for (int lst = 0; lst < nLp; ++lst) {
+      if (t.ls_a[Lp0 + lst] != a1) continue;
+      const int u = t.ls_x[Lp0 + lst];
+      for (int r = 0; r < nRq; ++r)
+        if (t.rs_c[Rq0 + r] == c1) v += m.wtm[P][u][t.rs_y[Rq0 + r]] * y[lst * MR + r];
+    }
+    inn[sl * MS2 + a1 * MS + c1] = v;
+  }
+  __syncthreads();
+  // ---- usages ----------------------------------------------------------------------------------------------------------------------------------
+  {
+    const int zi0 = t.opstart[i], ni = t.opstart[i + 1] - zi0, zj0 = t.opstart[j], nj = t.opstart[j + 1] - zj0;
+    const int zp0 = t.opstart[p], np_ = t.opstart[p + 1] - zp0, zq0 = t.opstart[q], nq = t.opstart[q + 1] - zq0;
+    const size_t no = A.nops;
+    for (int e = tid; e < ni + nj + 2 * np_ + 2 * nq; e += OT) {
+      if (e < ni) {
+        // pair end i:  x_z sum_{z' at j} x_z' Qb-bar[l(z)][r(z')] inner[slot(x,y)][c(z)][a(z')]
+        const int z = zi0 + e, x = t.op_b[z];
+        double u = 0.0;
+        for (int zz = zj0; zz < zj0 + nj; ++zz) {
+          const int sl = m.pslot[x * 4 + t.op_b[zz]];
+          if (sl >= 0) u += t.op_x[zz] * ab[t.op_l[z] * nR + t.op_r[zz]] * inn[sl * MS2 + t.op_c[z] * MS + t.op_a[zz]];
+        }
+        A.U[(size_t)ROLE_PL * no + z] += t.op_x[z] * u;
+      } else if (e < ni + nj) {
+        const int zz = zj0 + (e - ni), yy = t.op_b[zz];
+        double u = 0.0;
+        for (int z = zi0; z < zi0 + ni; ++z) {
+          const int sl = m.pslot[t.op_b[z] * 4 + yy];
+          if (sl >= 0) u += t.op_x[z] * ab[t.op_l[z] * nR + t.op_r[zz]] * inn[sl * MS2 + t.op_c[z] * MS + t.op_a[zz]];
+        }
+        A.U[(size_t)ROLE_PR * no + zz] += t.op_x[zz] * u;
+      } else if (e < ni + nj + np_) {
+        // closing mismatch at p = i+1 (hairpins and interior loops with l1 >= 2):
+        //   x_z1 ( sum_r G[u, y(r)][a1][c(r)] Z2[cz][r] + sum_aw XE[cz][aw] H1[u][a1][aw] )
+        const int z1_ = zp0 + (e - ni - nj), a1 = t.op_a[z1_], u_ = t.op_b[z1_], cz = t.op_c[z1_];
+        double u = 0.0;
+        if (has_loop) {
+          for (int r = 0; r < nRq; ++r)
+            u += go[(u_ * 4 + t.rs_y[Rq0 + r]) * MS2 + a1 * MS + t.rs_c[Rq0 + r]] * z2[cz * MR + r];
+          for (int aw = 0; aw < Sq; ++aw) u += xe[cz * MS + aw] * h1[(u_ * MS + a1) * MS + aw];
+        }
+        A.U[(size_t)ROLE_CL * no + z1_] += t.op_x[z1_] * u;
+      } else if (e < ni + nj + np_ + nq) {
+        // closing mismatch at q = j-1:  x_z2' ( sum_cz XE[cz][aw] H2[v][cz][c1] + sum_lst G[x(lst), v][a(lst)][c1] Z1[lst][aw] )
+        const int z2_ = zq0 + (e - ni - nj - np_), aw = t.op_a[z2_], v_ = t.op_b[z2_], c1 = t.op_c[z2_];
+        double u = 0.0;
+        if (has_loop) {
+          for (int cz = 0; cz < Sp1; ++cz) u += xe[cz * MS + aw] * h2[(v_ * MS + cz) * MS + c1];
+          for (int lst = 0; lst < nLp; ++lst)
+            u += go[(t.ls_x[Lp0 + lst] * 4 + v_) * MS2 + t.ls_a[Lp0 + lst] * MS + c1] * z1[lst * MS + aw];
+        }
+        A.U[(size_t)ROLE_CR * no + z2_] += t.op_x[z2_] * u;
+      } else if (e < ni + nj + 2 * np_ + nq) {
+        // size-1 left bulge at p (unpaired, no mismatch): x_z w_Bu(1) sum_{slot',c1} SB-bar[slot'][a1][c1] Qb(p+1,q)[(s,x')][(y',c1)]
+        const int z = zp0 + (e - ni - nj - np_ - nq), a1 = t.op_a[z], s = t.op_c[z];
+        double u = 0.0;
+        if (MI >= 1 && q - (p + 1) >= mh1)
+          for (int sl = 0; sl < nps; ++sl) {
+            const int lst = t.lsidx[((size_t)(p + 1) * MS + s) * 4 + m.slot_x[sl]];
+            if (lst < 0) continue;
+            for (int c1 = 0; c1 < Sc; ++c1) {
+              const int r = t.rsidx[((size_t)q * 4 + m.slot_y[sl]) * MS + c1];
+              if (r >= 0) u += sbb[sl * MS2 + a1 * MS + c1] * b.QB[(size_t)(t.loff[p + 1] + lst) * RS + Rq0 + r];
+            }
+          }
+        A.U[(size_t)ROLE_B1L * no + z] += t.op_x[z] * m.wbu[1] * u;
+      } else {
+        // size-1 right bulge at q: x_z w_Bu(1) sum_{slot',a1} SB-bar[slot'][a1][c1] Qb(p,q-1)[(a1,x')][(y',t)]
+        const int z = zq0 + (e - ni - nj - 2 * np_ - nq), tt_ = t.op_a[z], c1 = t.op_c[z];
+        double u = 0.0;
+        if (MI >= 1 && q - (p + 1) >= mh1)
+          for (int sl = 0; sl < nps; ++sl) {
+            const int r = t.rsidx[((size_t)(q - 1) * 4 + m.slot_y[sl]) * MS + tt_];
+            if (r < 0) continue;
+            for (int a1 = 0; a1 < Sa; ++a1) {
+              const int lst = t.lsidx[((size_t)p * MS + a1) * 4 + m.slot_x[sl]];
+              if (lst >= 0) u += sbb[sl * MS2 + a1 * MS + c1] * b.QB[(size_t)(Lp0 + lst) * RS + t.roff[q - 1] + r];
+            }
+          }
+        A.U[(size_t)ROLE_B1R * no + z] += t.op_x[z] * m.wbu[1] * u;
+      }
+    }
+  }
 }
 
 }  // namespace
 
-// Base-pair probabilities of a finished inside pass: bpp_dev [n][n], upper triangle P(i.j), diagonal P(i unpaired), lower triangle 0.
-// Workspace (3 S x S + LS x RS adjoint tables, 34 diagonals of I / G / H / H1 / H2) is allocated for the call and freed before it returns.
-int cdz_launch_outside(cdz_tables* t, double* bpp_dev, cudaStream_t st) {
-  const cdz_tt* tt = t->tt;
-  const size_t n = tt->n, S = tt->S, LS = tt->LS, RS = tt->RS, MS = tt->MS;
-  const size_t nSS = S * S, nAB = LS * RS, nAX = (n + 1) * MS, nR = (size_t)ORING * n * 16 * MS * MS;
-  const size_t nH = (size_t)ORING * n * MS * MS;
-  const size_t total = 3 * nSS + nAB + nAX + 2 * nR + 9 * nH;
-  double* ws = nullptr;
-  if (cudaMalloc(&ws, total * sizeof(double)) != cudaSuccess) {
-    cudaGetLastError();
-    cdz_set_error("cdz_marginals: out of device memory for the adjoint tables");
-    return CDZ_ENOMEM;
-  }
+// ------------------------------------------------------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------------------------------------------------------
+size_t cdz_outside_carve(const cdz_tt* tt, void* base, Adj* out) {
+  const size_t n = tt->n, S = tt->S, LS = tt->LS, RS = tt->RS, MS = tt->MS, MS2 = MS * MS, nops = tt->ops.size();
+  const size_t ML = tt->maxL, MR = tt->maxR;
   Adj A;
-  double* p = ws;
-  A.AM2 = p; p += nSS;
-  A.AML = p; p += nSS;
-  A.AM1 = p; p += nSS;
-  A.AB = p; p += nAB;
-  A.AX = p; p += nAX;
-  A.IB = p; p += nR;
-  A.G = p; p += nR;
-  A.H = p; p += nH;
-  A.H1 = p; p += 4 * nH;
-  A.H2 = p; p += 4 * nH;
-  cudaError_t e = cudaMemsetAsync(ws, 0, total * sizeof(double), st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(bpp_dev, 0, n * n * sizeof(double), st);
-  if (e == cudaSuccess) {
-    oext_kernel<<<1, OT, 0, st>>>(t->d_ctx, A);
-    for (int d = (int)n - 1; d >= 0; --d) ocell_kernel<<<(unsigned)(n - d), OT, 0, st>>>(t->d_ctx, A, d, bpp_dev);
-    unpaired_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>((int)n, bpp_dev);
-    e = cudaGetLastError();
-  }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  cudaFree(ws);
-  if (e != cudaSuccess) {
-    cdz_set_error(std::string("cdz_marginals (outside pass): ") + cudaGetErrorString(e));
-    return CDZ_ECUDA;
-  }
-  return CDZ_OK;
+  memset(&A, 0, sizeof(A));
+  size_t used = 0;
+  auto take = [&](size_t count) {
+    used = (used + 255) & ~size_t(255);
+    double* p = base ? (double*)((char*)base + used) : nullptr;
+    used += count * sizeof(double);
+    return p;
+  };
+  A.ML = (int)ML; A.MR = (int)MR; A.nops = nops;
+  A.AM2 = take(S * S); A.AM2T = take(S * S); A.AML = take(S * S); A.AM1T = take(S * S); A.AET = take(S * S);
+  A.QM1 = take(S * S); A.QMT = take(S * S);
+  A.AB = take(LS * RS);
+  A.AX = take((n + 1) * MS); A.AXB = take(S);
+  A.IB = take((size_t)ORING * n * 16 * MS2);
+  A.RD = take((size_t)ORING * n * (ML * MR + MS2 + ML * MS + MR * MS));
+  A.XA = take(2 * n * XU * MS2); A.XB = take(2 * n * XU * MS2);
+  A.AES = take((size_t)AES_NROLE * n * SLEN * MS2);
+  A.U = take((size_t)NROLE * nops);
+  A.status = (int*)take(8);
+  if (out) *out = A;
+  return (used + 255) & ~size_t(255);
+}
+
+int cdz_launch_outside(cdz_tables* t, const Adj& A, size_t ws_bytes, double* bpp_dev, double* base_dev, double* codon_dev, cudaStream_t st) {
+  const cdz_tt* tt = t->tt;
+  const int n = tt->n, NB = tt->NB;
+  const int want_usage = 1;  // the unpaired diagonal of bpp also comes from the usages (independent of the pair sums)
+  CDZ_CUDA(cudaMemsetAsync(A.AM2, 0, ws_bytes, st));  // AM2 is the first array of the workspace
+  if (bpp_dev) CDZ_CUDA(cudaMemsetAsync(bpp_dev, 0, (size_t)n * n * sizeof(double), st));
+  transpose_kernel<<<dim3(NB, NB), 256, 0, st>>>(t->h.tab.QM1T, A.QM1, tt->S, 1);
+  transpose_kernel<<<dim3(NB, NB), 256, 0, st>>>(t->h.tab.QM, A.QMT, tt->S, 0);
+  oext_kernel<<<1, 1024, 0, st>>>(t->d_ctx, A);
+  const OPlan pl = oplan(tt->MS, tt->maxL, tt->maxR, t->model->c.nps);
+  const size_t smem = sizeof(double) * pl.total;
+  CDZ_CUDA(cudaFuncSetAttribute(ocell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  for (int d = n - 1; d >= 0; --d) ocell_kernel<<<(unsigned)(n - d), OT, smem, st>>>(t->d_ctx, A, d, want_usage, bpp_dev);
+  CDZ_CUDA(cudaGetLastError());
+  return cdz_launch_usage(t, A, bpp_dev, base_dev, codon_dev, st);
 }

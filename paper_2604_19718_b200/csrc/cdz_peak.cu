@@ -88,3 +88,61 @@ extern "C" int cdz_peak_measure(int kind, double* tflops_out) {
   *tflops_out = best;
   return 0;
 }
+
+// ---- dependency-latency floor of the blocked wavefront (SURVEY.md 8d "the third number") -----------------------------------
+namespace {
+__global__ void empty_kernel() {}
+__global__ void __launch_bounds__(512) barrier_rounds(int rounds, int* sink) {
+  __shared__ int s;
+  if (threadIdx.x == 0) s = 0;
+  for (int r = 0; r < rounds; ++r) {
+    __syncthreads();
+    if ((int)threadIdx.x == (r & 511)) s += r;  // a dependent shared-memory update per round, as the phases of the cell kernel have
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) sink[blockIdx.x] = s;
+}
+}  // namespace
+
+// Average microseconds per launch of `count` dependent empty kernels on one stream (launch + completion chain).
+extern "C" int cdz_peak_launch_us(int count, double* us_out) {
+  if (!us_out || count <= 0) return -1;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  for (int k = 0; k < 64; ++k) empty_kernel<<<1, 32>>>();
+  cudaEventRecord(e0);
+  for (int k = 0; k < count; ++k) empty_kernel<<<148, 128>>>();
+  cudaEventRecord(e1);
+  cudaEventSynchronize(e1);
+  float ms = 0;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (cudaGetLastError() != cudaSuccess) return -3;
+  *us_out = 1e3 * ms / count;
+  return 0;
+}
+
+// Microseconds per __syncthreads round of a 512-thread CTA (one CTA per SM, `rounds` dependent rounds).
+extern "C" int cdz_peak_barrier_us(int rounds, double* us_out) {
+  if (!us_out || rounds <= 0) return -1;
+  int* sink = nullptr;
+  if (cudaMalloc((void**)&sink, sizeof(int) * 148) != cudaSuccess) return -3;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  barrier_rounds<<<148, 512>>>(rounds, sink);
+  cudaEventRecord(e0);
+  barrier_rounds<<<148, 512>>>(rounds, sink);
+  cudaEventRecord(e1);
+  cudaEventSynchronize(e1);
+  float ms = 0;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  if (cudaGetLastError() != cudaSuccess) return -3;
+  *us_out = 1e3 * ms / rounds;
+  return 0;
+}

@@ -196,6 +196,44 @@ def test_batch_equals_single_and_oracle(B, O):
         assert (s1 == s2).all() and (p1 == p2).all()
 
 
+def test_batch_many_blocks_split_k_scratch(B):
+    """with B > 1 the wave-aware split-K choice can pick more splits than a single-design launch; the partial-tile
+    scratch GP must hold them.  NB >= 48 blocks, B = 12: batched == single, bit for bit."""
+    m = I.nn_model()
+    mg = B.Model(m)
+    ds = [I.design(2, item, 350) for item in range(12)]  # codon-pair TT, ~50 blocks
+    tts = [B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw) for d in ds]
+    tabs, lzs = B.inside_batch(mg, tts)
+    assert tabs[0].info()["n"] == 1050
+    for item in (0, 5, 11):
+        t1, lz1 = B.inside(mg, tts[item])
+        assert lzs[item] == lz1
+        n = ds[item].n
+        for (i, j) in ((0, n - 1), (10, n - 20), (n // 3, 2 * n // 3), (400, 900)):
+            for which in (0, 4, 5):
+                g, sh = tabs[item].cell(which, i, j)
+                g1, sh1 = t1.cell(which, i, j)
+                assert sh == sh1 and (g == g1).all()
+
+
+def test_batch_mixed_lengths(B, O):
+    """designs of different length in one batch; a shorter design that has finished must not be rescaled again
+    at the later events of the longer ones.  Lengths chosen so that powers of two fall between the block counts."""
+    m = I.nn_model()
+    mg = B.Model(m)
+    ds = [I.design(5, 0, 24), I.design(5, 1, 100), I.design(2, 0, 300), I.design(5, 2, 60)]
+    tts = [B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw) for d in ds]
+    tabs, lzs = B.inside_batch(mg, tts)
+    for d, tt, tab, lz in zip(ds, tts, tabs, lzs):
+        t1, lz1 = B.inside(mg, tt)
+        assert lz == lz1, (d.name, lz, lz1)
+        s1, p1 = t1.sample(16, d.sample_seed)
+        s2, p2 = tab.sample(16, d.sample_seed)
+        assert (s1 == s2).all() and (p1 == p2).all()
+    lo = O.inside(m, O.TT.build(ds[0].aa, ds[0].kind, ds[0].codon_logw, ds[0].pair_logw)).logZ
+    assert abs(lzs[0] - lo) <= LOGZ_RTOL * abs(lo)
+
+
 def test_config5_full_batch(B, O):
     """64 x 150 aa in one batched pass: equal to the designs run one at a time; item 0's prefix checked against the oracle."""
     m = I.nn_model()
