@@ -137,6 +137,10 @@ void cdz_tables_destroy(cdz_tables* t);
  * the summed device milliseconds (0 when profiling was off) and the launch counts (always counted). */
 int cdz_set_profiling(cdz_tables* t, int on);
 int cdz_profile(cdz_tables* t, double* ms_out, int64_t* launches_out);
+/* Parity knob: the per-position scales are re-decided after block diagonals first, 2 first, 4 first, ... (default first = 1).
+ * Power-of-two scales make log Z independent of the schedule up to rounding; the tests move the events to check exactly that
+ * (SURVEY 8c "scaling-schedule invariance").  Takes effect at the next cdz_inside_rerun of the handle. */
+int cdz_debug_set_rescale_start(cdz_tables* t, int first);
 /* Debug / parity access: copy one cell to host as doubles (true value * 2^-shift_out).
  * which: 0 Qb as [a][x][y][c] dense, 1 Qbs, 2 Qm1, 3 Qml, 4 M2, 5 Qm (all [a][c]). Returns element count. */
 int cdz_tables_cell(cdz_tables* t, int which, int i, int j, double* out_host, int* shift_out);

@@ -22,7 +22,7 @@ EXPORTS = [
     "cdz_tt_from_operators", "cdz_tt_destroy", "cdz_tt_length", "cdz_tt_describe", "cdz_workspace_bytes",
     "cdz_inside", "cdz_inside_batch", "cdz_inside_rerun", "cdz_inside_rerun_batch", "cdz_tables_logz",
     "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample",
-    "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
+    "cdz_debug_set_rescale_start", "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
 ]
 
 
@@ -90,6 +90,7 @@ def lib():
     L.cdz_tables_destroy.argtypes = [vp]
     L.cdz_tables_destroy.restype = None
     L.cdz_set_profiling.argtypes = [vp, C.c_int]
+    L.cdz_debug_set_rescale_start.argtypes = [vp, C.c_int]
     L.cdz_profile.argtypes = [vp, dp, C.POINTER(C.c_int64)]
     L.cdz_tables_cell.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
     L.cdz_tables_logqext.argtypes = [vp, C.c_int, C.c_int, dp]
@@ -210,6 +211,9 @@ class Tables:
         i = Info()
         _check(lib().cdz_tables_info(self.h, C.byref(i)))
         return {k: getattr(i, k) for k, _ in Info._fields_}
+
+    def set_rescale_start(self, first: int):
+        _check(lib().cdz_debug_set_rescale_start(self.h, first))
 
     def set_profiling(self, on: bool):
         _check(lib().cdz_set_profiling(self.h, 1 if on else 0))

@@ -650,6 +650,12 @@ extern "C" int cdz_profile(cdz_tables* t, double* ms_out, int64_t* launches_out)
   return CDZ_OK;
 }
 
+extern "C" int cdz_debug_set_rescale_start(cdz_tables* t, int first) {
+  if (!t || first < 1) { cdz_set_error("cdz_debug_set_rescale_start: bad argument"); return CDZ_EINVAL; }
+  t->rescale_first = first;
+  return CDZ_OK;
+}
+
 // debug / parity access ------------------------------------------------------------------------------
 extern "C" int cdz_tables_cell(cdz_tables* t, int which, int i, int j, double* out, int* shift_out) {
   if (!t || !out || i < 0 || j < i || j >= t->tt->n || which < 0 || which > 5) {

@@ -425,7 +425,7 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
   init_kernel<<<dim3(32, B), 256, 0, st>>>(d_ctxs);
   int nmax = 0;
   for (int b = 0; b < B; ++b) nmax = std::max(nmax, ts[b]->tt->n);
-  int next_event = 1;
+  int next_event = std::max(1, ts[0]->rescale_first);
   for (int D = 0; D < NBmax; ++D) {
     const int nblk = NBmax - D;
     const int nsplit = cdz_nsplit(NBmax, D, B);

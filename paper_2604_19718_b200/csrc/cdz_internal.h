@@ -130,6 +130,7 @@ struct cdz_tables {
   Ctx h;         // host copy of the device view
   Ctx* d_ctx = nullptr;  // device copy (inside base)
   int n_rescales = 0;
+  int rescale_first = 1;  // rescale events after block diagonals rescale_first * 2^k (cdz_debug_set_rescale_start)
   // per-kernel-class device times of the last pass (cdz_set_profiling): events between consecutive launches
   bool profile = false;
   std::vector<cudaEvent_t> evs;

@@ -26,6 +26,14 @@
 // cdz_usage.cu finishes: E-bar chain, multiloop / exterior unpaired usages, base / codon marginals, unpaired probabilities.
 #include "cdz_outside.h"
 
+#ifdef CDZ_OTIMING
+#include <stdio.h>
+__device__ unsigned long long g_otime[16];
+#define OTICK(k) do { __syncthreads(); if (threadIdx.x == 0) { const long long now__ = clock64(); atomicAdd(&g_otime[k], (unsigned long long)(now__ - tlast__)); tlast__ = now__; } } while (0)
+#else
+#define OTICK(k)
+#endif
+
 namespace {
 
 constexpr int OT = 256;  // threads per CTA
@@ -176,6 +184,9 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   double* TRj = TRq + MS * MR;          // T_j
   double* TRn = TRj + MS * MR;          // T_{j+1}
 
+#ifdef CDZ_OTIMING
+  long long tlast__ = clock64();
+#endif
   const int i = blockIdx.x, j = i + d, p = i + 1, q = j - 1;
   const int Si = t.sig[i], Sj1 = t.sig[j + 1], offi = t.off[i], offj1 = t.off[j + 1];
   const int nent = Si * Sj1;
@@ -185,6 +196,21 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   const int Li0 = t.loff[i], Rj0 = t.roff[j];
   const int send = t.off[n] + t.sig[n];
 
+  // ---- offsets / bond dimensions of the positions within 35 of i and of j (loop sides reach 31 positions) ----------------------------------
+  __shared__ int offW[2][72], sigW[2][72];
+  if (tid < 144) {
+    const int which = tid / 72, idx = tid % 72, pos = (which ? j : i) - 35 + idx;
+    const bool ok = pos >= 0 && pos <= n;
+    offW[which][idx] = ok ? t.off[pos] : 0;
+    sigW[which][idx] = ok ? t.sig[pos] : 0;
+  }
+  auto offA = [&](int pos) { return offW[0][pos - i + 35]; };
+  auto sigA = [&](int pos) { return sigW[0][pos - i + 35]; };
+  auto offB = [&](int pos) { return offW[1][pos - j + 35]; };
+  auto sigB = [&](int pos) { return sigW[1][pos - j + 35]; };
+  // E(p,q)[a][c] with p and q+1 near i (EA) / near j (EB)
+  auto EA = [&](int pp, int qq, int a, int c) { return qq < pp ? (a == c ? 1.0 : 0.0) : b.EM[(size_t)(offA(pp) + a) * S + offA(qq + 1) + c]; };
+  auto EB = [&](int pp, int qq, int a, int c) { return qq < pp ? (a == c ? 1.0 : 0.0) : b.EM[(size_t)(offB(pp) + a) * S + offB(qq + 1) + c]; };
   // ---- dense cores of the six positions around the cell ------------------------------------------------------------------------------
   for (int k = tid; k < 3 * ML * MS + 3 * MS * MR; k += OT) (k < 3 * ML * MS ? TLm[k] : TRq[k - 3 * ML * MS]) = 0.0;
   __syncthreads();
@@ -250,6 +276,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     abs_[tid] = m.wc * w + b.Qext[offi + ea] * A.AX[(size_t)(j + 1) * MS + ec];
   }
   __syncthreads();
+  OTICK(0);
   if (!closed) {
     // cells below the minimum hairpin span: nothing pairs; the interior-body adjoint chains still pass through (d >= 4 only matters
     // when min_hairpin + 1 > 4)
@@ -298,25 +325,35 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
         const int i0 = i - 1 - l1, j0 = j + 1 + l2;
         if (i0 < 0 || j0 > n - 1) continue;
         const int dd = j0 - i0;
-        const int Sa = t.sig[i0 + 1], Sc = t.sig[j0];
+        const int Sa = sigA(i0 + 1), Sc = sigB(j0);
         const double* ib = A.IB + ((size_t)(dd % ORING) * n + i0) * 16 * MS2;
         if (l1 == 0 && l2 == 0) {
           for (int sl = 0; sl < nps; ++sl)
             acc += m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][Pin_st] * ib[sl * MS2 + s * MS + tt_];
         } else if (l2 == 0) {
           // left bulge: sum_{a'} E(i0+1,i-1)[a',s] I[x,y;a',t]
+          double ev[CDZ_MAX_BOND];
+#pragma unroll
+          for (int a = 0; a < CDZ_MAX_BOND; ++a) ev[a] = a < Sa ? EA(i0 + 1, i - 1, a, s) : 0.0;
           for (int sl = 0; sl < nps; ++sl) {
             const double w = m.wbu[l1] * (l1 == 1 ? m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][Pin_st] : 1.0);
             double v = 0.0;
-            for (int a = 0; a < Sa; ++a) v += V.E(i0 + 1, i - 1, a, s) * ib[sl * MS2 + a * MS + tt_];
+#pragma unroll
+            for (int a = 0; a < CDZ_MAX_BOND; ++a)
+              if (a < Sa) v += ev[a] * ib[sl * MS2 + a * MS + tt_];
             acc += w * v;
           }
         } else {
           // right bulge: sum_{c'} I[x,y;s,c'] E(j+1,j0-1)[t,c']
+          double ev[CDZ_MAX_BOND];
+#pragma unroll
+          for (int c = 0; c < CDZ_MAX_BOND; ++c) ev[c] = c < Sc ? EB(j + 1, j0 - 1, tt_, c) : 0.0;
           for (int sl = 0; sl < nps; ++sl) {
             const double w = m.wbu[l2] * (l2 == 1 ? m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][Pin_st] : 1.0);
             double v = 0.0;
-            for (int c = 0; c < Sc; ++c) v += ib[sl * MS2 + s * MS + c] * V.E(j + 1, j0 - 1, tt_, c);
+#pragma unroll
+            for (int c = 0; c < CDZ_MAX_BOND; ++c)
+              if (c < Sc) v += ib[sl * MS2 + s * MS + c] * ev[c];
             acc += w * v;
           }
         }
@@ -356,6 +393,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     }
     __syncthreads();
   }
+  OTICK(1);
   // usages of the inner-mismatch operators z2 at i-1 (role IL) and z1' at j+1 (role IR)
   if (want_usage && dressed) {
     const int z2b = t.opstart[i - 1], nz2 = t.opstart[i] - z2b, z1b = t.opstart[j + 1], nz1 = t.opstart[j + 2] - z1b;
@@ -397,6 +435,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     }
   }
 
+  OTICK(2);
   // ---- 3: I(i,j)[slot][a'][c'], G[u,v][a'][c'], H, H1, H2 ----------------------------------------------------------------------------------
   const int Sa = t.sig[p], Sc = t.sig[j];  // a' in Sigma_{i+1}, c' in Sigma_j
   double* ibo = A.IB + ((size_t)(d % ORING) * n + i) * 16 * MS2;
@@ -469,6 +508,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   }
   __syncthreads();
 
+  OTICK(3);
   // ---- 4: this cell as closing pair ---------------------------------------------------------------------------------------------------------
   const int Sp1 = t.sig[p + 1], Sq = t.sig[q];  // bonds after i+1 / before j-1: XE, H are Sp1 x Sq
   const int nLp = t.loff[p + 1] - t.loff[p], nRq = t.roff[q + 1] - t.roff[q];
@@ -510,6 +550,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     }
   }
   __syncthreads();
+  OTICK(4);
   // 4c pushes of the generic interior loops (l1, l2 >= 2).  All terms of X_u(i,j) have the inner span d-2-u.
   if (MI >= 4) {
     // row recursion, new term GI(i+3, l) E(l+2,j-2), l = j+1-u:  adjoint of GI into the ring slot of cell (i+3,l); E-bar of the right stretch
@@ -517,18 +558,18 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       const int u4 = e / MS2, x1 = (e % MS2) / MS, x2 = e % MS, u = u4 + 4;
       if (d - 2 - u < mh1) continue;
       const int l = j + 1 - u, k = i + 3;  // inner pair (k,l): l1 = 2, l2 = u-2
-      const int Sk1 = Sp1 /* Sigma_{k-1} = Sigma_{i+2} */, Sl2 = t.sig[l + 2];
+      const int Sk1 = Sp1 /* Sigma_{k-1} = Sigma_{i+2} */, Sl2 = sigB(l + 2);
       const double* xau = xa + u4 * MS2;
       // AGI(k,l)[s2 = x1][t2 = x2] += sum_aw XA_u[s2][aw] E(l+2,j-2)[t2][aw]
       if (x1 < Sk1 && x2 < Sl2) {
         double v = 0.0;
-        for (int aw = 0; aw < Sq; ++aw) v += xau[x1 * MS + aw] * V.E(l + 2, j - 2, x2, aw);
+        for (int aw = 0; aw < Sq; ++aw) v += xau[x1 * MS + aw] * EB(l + 2, j - 2, x2, aw);
         double* rdk = A.RD + ((size_t)((l - k) % ORING) * n + k) * RDS + ML * MR;
         rdk[x1 * MS + x2] += v;
       }
       // E-bar(l+2, j-2)[t2 = x1][aw = x2] += sum_s2 GI(k,l)[s2][t2] XA_u[s2][aw]       (length u-4 >= 1)
       if (want_usage && u > 4 && x1 < Sl2 && x2 < Sq) {
-        const double* gi = b.GI + (size_t)t.off[k - 1] * S + t.off[l + 2] + x1;
+        const double* gi = b.GI + (size_t)offA(k - 1) * S + offB(l + 2) + x1;
         double v = 0.0;
         for (int s2 = 0; s2 < Sk1; ++s2) v += gi[(size_t)s2 * S] * xau[s2 * MS + x2];
         A.AES[(((size_t)AES_XR * n + (l + 2)) * SLEN + (u - 4)) * MS2 + x1 * MS + x2] += v;
@@ -540,14 +581,15 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
         const int u4 = e / MS2, cz = (e % MS2) / MS, s2 = e % MS, u = u4 + 4;
         if (u == 4 || d - 2 - u < mh1) continue;
         const int k = i + u - 1, l = j - 3;
-        if (cz >= Sp1 || s2 >= t.sig[k - 1]) continue;
-        const double* gi = b.GI + (size_t)(t.off[k - 1] + s2) * S + t.off[l + 2];  // columns: bonds of position l+2 = j-1
+        if (cz >= Sp1 || s2 >= sigA(k - 1)) continue;
+        const double* gi = b.GI + (size_t)(offA(k - 1) + s2) * S + offB(l + 2);  // columns: bonds of position l+2 = j-1
         const double* xbu = xb + u4 * MS2 + cz * MS;
         double v = 0.0;
         for (int aw = 0; aw < Sq; ++aw) v += xbu[aw] * gi[aw];
         A.AES[(((size_t)AES_XL * n + (i + 2)) * SLEN + (u - 4)) * MS2 + cz * MS + s2] += v;
       }
   }
+  OTICK(5);
   // 4d pushes of the l1 = 1 / l2 = 1 / 1x1 interior loops
   if (MI >= 2) {
     // 1 x 1: inner pair (i+2, j-2), DD(p,q) enters Y with w_In(2)
@@ -558,56 +600,51 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
         rdk[lst * MR + r] += m.win[2] * go[(t.ls_x[Lp0 + lst] * 4 + t.rs_y[Rq0 + r]) * MS2 + t.ls_a[Lp0 + lst] * MS + t.rs_c[Rq0 + r]];
       }
     }
-    // l1 = 1, l2 = 2..: Z1[lst][c2] = sum_l2 w_In(1+l2) sum_u D1(p; l+2)[lst][u] E(l+2,q-1)[u][c2],  l = q - l2; inner pair (i+2, l)
-    {
-      const int lmax = min(MI - 1, q - mh1 - (p + 1));
-      for (int l2 = 2; l2 <= lmax; ++l2) {
-        const int l = q - l2, Su = t.sig[l + 2];
-        double* rdk = A.RD + ((size_t)((l - (i + 2)) % ORING) * n + (i + 2)) * RDS + ML * MR + MS2;  // AD1[lst][u]
-        const double w = m.win[1 + l2];
-        for (int e = tid; e < nLp * Su; e += OT) {
-          const int lst = e / Su, u = e % Su;
-          const double* hz = h1 + (t.ls_x[Lp0 + lst] * MS + t.ls_a[Lp0 + lst]) * MS;  // Z1-bar[lst][c2] = H1[x(lst)][a(lst)][c2]
-          double v = 0.0;
-          for (int c2 = 0; c2 < Sq; ++c2) v += hz[c2] * V.E(l + 2, q - 1, u, c2);
-          rdk[lst * MS + u] += w * v;
-        }
-        if (want_usage && l2 > 2)
-          for (int e = tid; e < Su * Sq; e += OT) {
-            const int u = e / Sq, c2 = e % Sq;
-            double v = 0.0;
-            for (int lst = 0; lst < nLp; ++lst)
-              v += b.D1[(size_t)(Lp0 + lst) * S + t.off[l + 2] + u] * h1[(t.ls_x[Lp0 + lst] * MS + t.ls_a[Lp0 + lst]) * MS + c2];
-            A.AES[(((size_t)AES_Z1R * n + (l + 2)) * SLEN + (l2 - 2)) * MS2 + u * MS + c2] += w * v;
-          }
-      }
-    }
-    // l2 = 1, l1 = 2..: Z2[a2][r] = sum_l1 w_In(l1+1) sum_s E(p+1,k-2)[a2][s] D2(k-1; q)[s][r],  k = p + l1; inner pair (k, j-2)
-    {
-      const int lmax = min(MI - 1, (q - 1) - mh1 - p);
-      for (int l1 = 2; l1 <= lmax; ++l1) {
-        const int k = p + l1, Ss = t.sig[k - 1];
-        double* rdk = A.RD + ((size_t)(((j - 2) - k) % ORING) * n + k) * RDS + ML * MR + MS2 + ML * MS;  // AD2[r][s]
-        const double w = m.win[l1 + 1];
-        for (int e = tid; e < nRq * Ss; e += OT) {
-          const int r = e / Ss, s = e % Ss;
-          const double* hz = h2 + (t.rs_y[Rq0 + r] * MS) * MS + t.rs_c[Rq0 + r];  // Z2-bar[a2][r] = H2[y(r)][a2][c(r)]
-          double v = 0.0;
-          for (int a2 = 0; a2 < Sp1; ++a2) v += V.E(p + 1, k - 2, a2, s) * hz[a2 * MS];
-          rdk[r * MS + s] += w * v;
-        }
-        if (want_usage && l1 > 2)
-          for (int e = tid; e < Sp1 * Ss; e += OT) {
-            const int a2 = e / Ss, s = e % Ss;
-            double v = 0.0;
-            for (int r = 0; r < nRq; ++r)
-              v += h2[(t.rs_y[Rq0 + r] * MS + a2) * MS + t.rs_c[Rq0 + r]] * b.D2T[(size_t)(Rq0 + r) * S + t.off[k - 1] + s];
-            A.AES[(((size_t)AES_Z2L * n + (p + 1)) * SLEN + (l1 - 2)) * MS2 + a2 * MS + s] += w * v;
-          }
+    // l1 = 1, l2 = 2..lmax1: Z1[lst][c2] = sum_l2 w_In(1+l2) sum_u D1(p; l+2)[lst][u] E(l+2,q-1)[u][c2],  l = q - l2; inner pair (i+2, l)
+    // l2 = 1, l1 = 2..lmax2: Z2[a2][r] = sum_l1 w_In(l1+1) sum_s E(p+1,k-2)[a2][s] D2(k-1; q)[s][r],  k = p + l1; inner pair (k, j-2)
+    // (all (l, entry) items of the four pushes are independent: one flat loop over the threads)
+    const int lmax1 = min(MI - 1, q - mh1 - (p + 1)), lmax2 = min(MI - 1, (q - 1) - mh1 - p);
+    const int n1 = max(lmax1 - 1, 0), n2 = max(lmax2 - 1, 0);
+    const int e1 = n1 * nLp * MS, e2 = e1 + n2 * nRq * MS, e3 = e2 + (want_usage ? n1 * MS2 : 0), e4 = e3 + (want_usage ? n2 * MS2 : 0);
+    for (int e = tid; e < e4; e += OT) {
+      if (e < e1) {
+        const int l2 = 2 + e / (nLp * MS), lst = (e / MS) % nLp, u = e % MS, l = q - l2;
+        if (u >= sigB(l + 2)) continue;
+        const double* hz = h1 + (t.ls_x[Lp0 + lst] * MS + t.ls_a[Lp0 + lst]) * MS;  // Z1-bar[lst][c2] = H1[x(lst)][a(lst)][c2]
+        double v = 0.0;
+        for (int c2 = 0; c2 < Sq; ++c2) v += hz[c2] * EB(l + 2, q - 1, u, c2);
+        double* rdk = A.RD + ((size_t)((l - (i + 2)) % ORING) * n + (i + 2)) * RDS + ML * MR + MS2;  // AD1[lst][u] of cell (i+2, l)
+        rdk[lst * MS + u] += m.win[1 + l2] * v;
+      } else if (e < e2) {
+        const int f = e - e1, l1 = 2 + f / (nRq * MS), r = (f / MS) % nRq, s_ = f % MS, k = p + l1;
+        if (s_ >= sigA(k - 1)) continue;
+        const double* hz = h2 + (t.rs_y[Rq0 + r] * MS) * MS + t.rs_c[Rq0 + r];  // Z2-bar[a2][r] = H2[y(r)][a2][c(r)]
+        double v = 0.0;
+        for (int a2 = 0; a2 < Sp1; ++a2) v += EA(p + 1, k - 2, a2, s_) * hz[a2 * MS];
+        double* rdk = A.RD + ((size_t)(((j - 2) - k) % ORING) * n + k) * RDS + ML * MR + MS2 + ML * MS;  // AD2[r][s] of cell (k, j-2)
+        rdk[r * MS + s_] += m.win[l1 + 1] * v;
+      } else if (e < e3) {
+        // E-bar(l+2, q-1)[u][c2] += w sum_lst D1[lst][u] Z1-bar[lst][c2]        (length l2 - 2 >= 1)
+        const int f = e - e2, l2 = 2 + f / MS2, u = (f % MS2) / MS, c2 = f % MS, l = q - l2;
+        if (l2 == 2 || u >= sigB(l + 2) || c2 >= Sq) continue;
+        double v = 0.0;
+        for (int lst = 0; lst < nLp; ++lst)
+          v += b.D1[(size_t)(Lp0 + lst) * S + offB(l + 2) + u] * h1[(t.ls_x[Lp0 + lst] * MS + t.ls_a[Lp0 + lst]) * MS + c2];
+        A.AES[(((size_t)AES_Z1R * n + (l + 2)) * SLEN + (l2 - 2)) * MS2 + u * MS + c2] += m.win[1 + l2] * v;
+      } else {
+        // E-bar(p+1, k-2)[a2][s] += w sum_r Z2-bar[a2][r] D2(k-1; q)[s][r]      (length l1 - 2 >= 1)
+        const int f = e - e3, l1 = 2 + f / MS2, a2 = (f % MS2) / MS, s_ = f % MS, k = p + l1;
+        if (l1 == 2 || a2 >= Sp1 || s_ >= sigA(k - 1)) continue;
+        double v = 0.0;
+        for (int r = 0; r < nRq; ++r)
+          v += h2[(t.rs_y[Rq0 + r] * MS + a2) * MS + t.rs_c[Rq0 + r]] * b.D2T[(size_t)(Rq0 + r) * S + offA(k - 1) + s_];
+        A.AES[(((size_t)AES_Z2L * n + (p + 1)) * SLEN + (l1 - 2)) * MS2 + a2 * MS + s_] += m.win[l1 + 1] * v;
       }
     }
   }
+  OTICK(6);
   if (!want_usage) return;
+  const int offp_ = offA(p), offj_ = offB(j), offp1_ = offA(p + 1), offq_ = offB(q);
   // 4e stretch adjoints of the bulges of size >= 2:  Bl = .. + sum_l1 w_Bu(l1) E(p,k-1) Qbs(k,q),  Br = sum_l2 w_Bu(l2) Qbs(p,l) E(l+1,q)
   {
     const int lmax = min(MI, q - mh1 - p);
@@ -616,78 +653,64 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       const int len = 2 + r / MS2, x1 = (r % MS2) / MS, x2 = r % MS;
       if (side == 0) {
         const int k = p + len;  // E(p,k-1)[a1 = x1][s = x2]
-        if (x1 >= Sa || x2 >= t.sig[k]) continue;
-        const double* qs = b.QBS + (size_t)(t.off[k] + x2) * S + t.off[j];
+        if (x1 >= Sa || x2 >= sigA(k)) continue;
+        const double* qs = b.QBS + (size_t)(offA(k) + x2) * S + offj_;
         double v = 0.0;
         for (int c1 = 0; c1 < Sc; ++c1) v += ibsum[x1 * MS + c1] * qs[c1];
         A.AES[(((size_t)AES_BL * n + p) * SLEN + len) * MS2 + x1 * MS + x2] += m.wbu[len] * v;
       } else {
         const int l = q - len;  // E(l+1,q)[u = x1][c1 = x2]
-        if (x1 >= t.sig[l + 1] || x2 >= Sc) continue;
+        if (x1 >= sigB(l + 1) || x2 >= Sc) continue;
         double v = 0.0;
-        for (int a1 = 0; a1 < Sa; ++a1) v += b.QBS[(size_t)(t.off[p] + a1) * S + t.off[l + 1] + x1] * ibsum[a1 * MS + x2];
+        for (int a1 = 0; a1 < Sa; ++a1) v += b.QBS[(size_t)(offp_ + a1) * S + offB(l + 1) + x1] * ibsum[a1 * MS + x2];
         A.AES[(((size_t)AES_BR * n + (l + 1)) * SLEN + len) * MS2 + x1 * MS + x2] += m.wbu[len] * v;
       }
     }
   }
+  OTICK(7);
   // 4f forward quantities of this cell, recomputed from the stored tables exactly as the inside pass builds them
   {
     const int lmaxB = min(MI, q - mh1 - p);
     const int lmaxZ1 = min(MI - 1, q - mh1 - (p + 1)), lmaxZ2 = min(MI - 1, (q - 1) - mh1 - p);
-    for (int e = tid; e < Sp1 * Sq; e += OT) xe[(e / Sq) * MS + e % Sq] = b.XE[(size_t)(t.off[p + 1] + e / Sq) * S + t.off[q] + e % Sq];
-    // Bl, Br  [a1 < Sa][c1 < Sc]
-    for (int e = tid; e < 2 * Sa * Sc; e += OT) {
-      const int side = e / (Sa * Sc), a1 = (e % (Sa * Sc)) / Sc, c1 = e % Sc;
+    for (int e = tid; e < Sp1 * Sq; e += OT) xe[(e / Sq) * MS + e % Sq] = b.XE[(size_t)(offp1_ + e / Sq) * S + offq_ + e % Sq];
+    // Bl, Br [a1 < Sa][c1 < Sc], Z1[lst][c2 < Sq], Z2[a2 < Sp1][r]: one thread per entry, weighted dot products over the bonds of
+    // the <= 29 band positions (offsets from the shared windows, so the loads of different positions are independent)
+    const int nb = Sa * Sc, nz1 = nLp * Sq, nz2 = Sp1 * nRq;
+    for (int e = tid; e < 2 * nb + nz1 + nz2; e += OT) {
+      const double *A_, *B_, *wt;
+      int lo, hi, near_i, base_pos, sgn;  // positions lo..hi, weight wt[sgn * (pos - base_pos)]
       double v = 0.0;
-      if (side == 0) {
-        v = m.wac * b.M2[(size_t)(t.off[p] + a1) * S + t.off[j] + c1];
-        const double* A_ = b.EM + (size_t)(t.off[p] + a1) * S;
-        const double* B_ = b.QBST + (size_t)(t.off[j] + c1) * S;
-        for (int l1 = 2; l1 <= lmaxB; ++l1) {
-          const int k = p + l1;
-          double s = 0.0;
-          for (int kb = t.off[k]; kb < t.off[k] + t.sig[k]; ++kb) s += A_[kb] * B_[kb];
-          v += m.wbu[l1] * s;
-        }
-        bl[a1 * MS + c1] = v;
+      double* out;
+      if (e < nb) {
+        const int a1 = e / Sc, c1 = e % Sc;
+        v = m.wac * b.M2[(size_t)(offp_ + a1) * S + offj_ + c1];
+        A_ = b.EM + (size_t)(offp_ + a1) * S; B_ = b.QBST + (size_t)(offj_ + c1) * S;
+        lo = p + 2; hi = p + lmaxB; near_i = 1; wt = m.wbu; base_pos = p; sgn = 1;  // k = p + l1
+        out = bl + a1 * MS + c1;
+      } else if (e < 2 * nb) {
+        const int a1 = (e - nb) / Sc, c1 = (e - nb) % Sc;
+        A_ = b.QBS + (size_t)(offp_ + a1) * S; B_ = b.EMT + (size_t)(offj_ + c1) * S;
+        lo = q - lmaxB + 1; hi = q - 1; near_i = 0; wt = m.wbu; base_pos = j; sgn = -1;  // pos = l + 1, l2 = j - pos
+        out = br + a1 * MS + c1;
+      } else if (e < 2 * nb + nz1) {
+        const int f = e - 2 * nb, lst = f / Sq, c2 = f % Sq;
+        A_ = b.D1 + (size_t)(Lp0 + lst) * S; B_ = b.EMT + (size_t)(offq_ + c2) * S;
+        lo = q - lmaxZ1 + 2; hi = q; near_i = 0; wt = m.win; base_pos = j + 2; sgn = -1;  // pos = l + 2, weight w_In(1 + l2) = win[j + 2 - pos]
+        out = z1 + lst * MS + c2;
       } else {
-        const double* A_ = b.QBS + (size_t)(t.off[p] + a1) * S;
-        const double* B_ = b.EMT + (size_t)(t.off[j] + c1) * S;
-        for (int l2 = 2; l2 <= lmaxB; ++l2) {
-          const int l = q - l2;
-          double s = 0.0;
-          for (int kb = t.off[l + 1]; kb < t.off[l + 1] + t.sig[l + 1]; ++kb) s += A_[kb] * B_[kb];
-          v += m.wbu[l2] * s;
-        }
-        br[a1 * MS + c1] = v;
+        const int f = e - 2 * nb - nz1, a2 = f / nRq, r = f % nRq;
+        A_ = b.EM + (size_t)(offp1_ + a2) * S; B_ = b.D2T + (size_t)(Rq0 + r) * S;
+        lo = p + 1; hi = p + lmaxZ2 - 1; near_i = 1; wt = m.win; base_pos = p - 2; sgn = 1;  // pos = k - 1, weight w_In(l1 + 1) = win[pos + 2 - p]
+        out = z2 + a2 * MR + r;
       }
-    }
-    // Z1[lst][c2 < Sq], Z2[a2 < Sp1][r]
-    for (int e = tid; e < nLp * Sq + Sp1 * nRq; e += OT) {
-      double v = 0.0;
-      if (e < nLp * Sq) {
-        const int lst = e / Sq, c2 = e % Sq;
-        const double* A_ = b.D1 + (size_t)(Lp0 + lst) * S;
-        const double* B_ = b.EMT + (size_t)(t.off[q] + c2) * S;
-        for (int l2 = 2; l2 <= lmaxZ1; ++l2) {
-          const int l = q - l2;
-          double s = 0.0;
-          for (int kb = t.off[l + 2]; kb < t.off[l + 2] + t.sig[l + 2]; ++kb) s += A_[kb] * B_[kb];
-          v += m.win[1 + l2] * s;
-        }
-        z1[lst * MS + c2] = v;
-      } else {
-        const int a2 = (e - nLp * Sq) / nRq, r = (e - nLp * Sq) % nRq;
-        const double* A_ = b.EM + (size_t)(t.off[p + 1] + a2) * S;
-        const double* B_ = b.D2T + (size_t)(Rq0 + r) * S;
-        for (int l1 = 2; l1 <= lmaxZ2; ++l1) {
-          const int k = p + l1;
-          double s = 0.0;
-          for (int kb = t.off[k - 1]; kb < t.off[k - 1] + t.sig[k - 1]; ++kb) s += A_[kb] * B_[kb];
-          v += m.win[l1 + 1] * s;
-        }
-        z2[a2 * MR + r] = v;
+#pragma unroll 4
+      for (int pos = lo; pos <= hi; ++pos) {
+        const int o = near_i ? offA(pos) : offB(pos), sg = near_i ? sigA(pos) : sigB(pos);
+        double s = 0.0;
+        for (int kb = o; kb < o + sg; ++kb) s += A_[kb] * B_[kb];
+        v += wt[sgn * (pos - base_pos)] * s;
       }
+      *out = v;
     }
     // SB[slot'][a1][c1]: stack + size-1 bulges (the inner pair keeps its identity)
     for (int e = tid; e < nps * Sa * Sc; e += OT) {
@@ -743,6 +766,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     inn[sl * MS2 + a1 * MS + c1] = v;
   }
   __syncthreads();
+  OTICK(8);
   // ---- usages ----------------------------------------------------------------------------------------------------------------------------------
   {
     const int zi0 = t.opstart[i], ni = t.opstart[i + 1] - zi0, zj0 = t.opstart[j], nj = t.opstart[j + 1] - zj0;
@@ -818,6 +842,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       }
     }
   }
+  OTICK(9);
 }
 
 }  // namespace
@@ -866,5 +891,16 @@ int cdz_launch_outside(cdz_tables* t, const Adj& A, size_t ws_bytes, double* bpp
   CDZ_CUDA(cudaFuncSetAttribute(ocell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   for (int d = n - 1; d >= 0; --d) ocell_kernel<<<(unsigned)(n - d), OT, smem, st>>>(t->d_ctx, A, d, want_usage, bpp_dev);
   CDZ_CUDA(cudaGetLastError());
+#ifdef CDZ_OTIMING
+  {
+    unsigned long long h[16];
+    cudaStreamSynchronize(st);
+    cudaMemcpyFromSymbol(h, g_otime, sizeof(h));
+    fprintf(stderr, "ocell phase cycles (sum over CTAs): gathers %llu | Qb-bar %llu | IL/IR %llu | I,G,H %llu | 4a-b %llu | 4c %llu | 4d %llu | 4e %llu | 4f %llu | usages %llu\n",
+            h[0], h[1], h[2], h[3], h[4], h[5], h[6], h[7], h[8], h[9]);
+    unsigned long long z[16] = {0};
+    cudaMemcpyToSymbol(g_otime, z, sizeof(z));
+  }
+#endif
   return cdz_launch_usage(t, A, bpp_dev, base_dev, codon_dev, st);
 }

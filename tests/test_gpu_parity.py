@@ -161,7 +161,7 @@ def test_config4_full_size_prefix_and_samples(B, O):
     seq, pair = seq.cpu().numpy(), pair.cpu().numpy()
     tto = O.TT.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
     m = I.nn_model()
-    for k in range(0, 100, 10):
+    for k in range(100):  # every sample: a coding sequence of the protein with a valid structure of finite weight
         assert (seq[k] < 4).all()
         assert np.isfinite(O.logweight(m, tto, seq[k], pair[k]))
     tfull.rerun()
@@ -207,13 +207,14 @@ def test_batch_many_blocks_split_k_scratch(B):
     assert tabs[0].info()["n"] == 1050
     for item in (0, 5, 11):
         t1, lz1 = B.inside(mg, tts[item])
-        assert lzs[item] == lz1
+        assert abs(lzs[item] - lz1) <= 1e-12 * abs(lz1)
         n = ds[item].n
         for (i, j) in ((0, n - 1), (10, n - 20), (n // 3, 2 * n // 3), (400, 900)):
             for which in (0, 4, 5):
                 g, sh = tabs[item].cell(which, i, j)
                 g1, sh1 = t1.cell(which, i, j)
-                assert sh == sh1 and (g == g1).all()
+                # (the number of K-splits differs between the two launches, so the sums associate differently: last bits may differ)
+                assert sh == sh1 and np.abs(g - g1).max() <= 1e-12 * max(np.abs(g1).max(), 1e-300)
 
 
 def test_batch_mixed_lengths(B, O):
@@ -262,3 +263,77 @@ def test_full_size_logz_vs_stored_oracle(B, row):
     assert d.n == int(row[3])
     tg, lz = B.inside(B.Model(I.nn_model()), B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw))
     assert abs(lz - want) <= LOGZ_RTOL * abs(want), (lz, want)
+
+
+def _stored_sample_rows():
+    path = os.path.join(GOLD, "oracle_samples.txt")
+    return rows("oracle_samples.txt") if os.path.exists(path) else []
+
+
+@pytest.mark.parametrize("row", _stored_sample_rows(), ids=lambda r: f"config{r[0]}-J{r[3]}")
+def test_full_size_samples_vs_stored_oracle(B, row):
+    """Bit-exact samples at the BASELINE sizes the oracle can reach (config 1: 1000 x 60 nt; config 5 item 0: 256 x 450 nt, 15 blocks,
+    multiloop-segment skip and 32-wide prefix sums exercised): SHA-256 of the raw arrays orc_sample produced for the same seed
+    (tests/golden/oracle_samples.txt, written by tests/golden/make_golden.py samples; oracle only), plus sample 0 as text."""
+    import hashlib
+
+    cfg, item, L, J, seed = (int(v) for v in row[:5])
+    d = I.design(cfg, item, L)
+    assert d.sample_seed == seed and d.n_samples == J
+    tg, lz = B.inside(B.Model(I.nn_model()), B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw))
+    seq, pair = tg.sample(J, seed)
+    seq, pair = seq.cpu().numpy(), pair.cpu().numpy()
+    assert "".join("ACGU"[b] for b in seq[0]) == row[7]
+    assert "".join("." if q < 0 else ("(" if q > k else ")") for k, q in enumerate(pair[0])) == row[8]
+    assert hashlib.sha256(seq.astype("uint8").tobytes()).hexdigest() == row[5]
+    assert hashlib.sha256(pair.astype("<i4").tobytes()).hexdigest() == row[6]
+
+
+# ---- large pins that do not go through the tensor recursion of the oracle (VERDICT r1 item 2) ---------------------------------------
+def _closed_rows():
+    path = os.path.join(GOLD, "oracle_closed_forms.txt")
+    return rows("oracle_closed_forms.txt") if os.path.exists(path) else []
+
+
+@pytest.mark.parametrize("row", _closed_rows(), ids=lambda r: f"{r[0]}-{r[1]}")
+def test_closed_form_large(B, row):
+    """zero8: zero-energy, all-pairs model on a generic bond-dimension-8 operator list (16 boundary states per position): every
+    sequence has the same number of structures, so  log Z = log sum_phi W(phi) + log S_30(n)  (orc_tt_logsum, eq 3.2, + the scalar
+    orc_mccaskill count).  At n = 3000 this is 375 blocks: every block diagonal, 16-way split-K and the rescale events up to D = 256
+    of the headline run, against a closed form.   mettrp: Met/Trp-only protein (one codon each) under the NN model: the design space
+    is one sequence, log Z = scalar McCaskill + codon log-weights (north_star).  Expected values: tests/golden/oracle_closed_forms.txt
+    (make_golden.py closed; oracle only)."""
+    import importlib.util
+
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(GOLD, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)  # input recipe only (the golden writer itself calls nothing but oracle/)
+    closed_form_inputs = mg.closed_form_inputs
+
+    kind, n, want = row[0], int(row[1]), float(row[2])
+    if kind == "zero8":
+        m = I.zero_energy_model()
+        tt = B.TensorTrain.from_operators(closed_form_inputs("zero8", n))
+    else:
+        m = I.nn_model()
+        aa, cw = closed_form_inputs("mettrp", n)
+        tt = B.TensorTrain.build(aa, B.TT_SINGLE_CODON, cw)
+    tg, lz = B.inside(B.Model(m), tt)
+    assert abs(lz - want) <= LOGZ_RTOL * abs(want), (lz, want)
+    tg.destroy()
+
+
+@pytest.mark.parametrize("cfg", [2, 4])
+def test_rescale_schedule_invariance(B, cfg):
+    """The per-position scales are exact powers of two, so moving the rescale events (after block diagonals 1,2,4,.. -> 3,6,12,.. ->
+    5,10,20,..) must leave log Z unchanged to rounding: 1e-12 relative at config 2 (900 nt) and at the headline config 4 (15000 nt)."""
+    d = I.design(cfg, 0)
+    tg, lz = B.inside(B.Model(I.nn_model()), B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw))
+    n0 = tg.info()["n_rescales"]
+    for first in (3, 5):
+        tg.set_rescale_start(first)
+        tg.rerun()
+        lz2 = tg.logz()
+        assert abs(lz2 - lz) <= 1e-12 * abs(lz), (first, lz, lz2)
+        assert tg.info()["n_rescales"] != n0 or cfg == 2
+    tg.destroy()
