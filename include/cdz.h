@@ -38,7 +38,12 @@ typedef enum {
 } cdz_status;
 
 enum { CDZ_TT_SINGLE_CODON = 0, CDZ_TT_CODON_PAIR = 1 };
-enum { CDZ_FP64 = 0, CDZ_FP32_SCALED = 1 };  /* CDZ_FP32_SCALED is declared but not built: CDZ_EINVAL */
+/* CDZ_FP64: everything in fp64 (tolerance 1e-9 relative in log Z).
+ * CDZ_FP32_SCALED (BASELINE.json configs[2], "single precision", line 622 row renormalisation): the split-point
+ * contraction -- the O(n^3) part -- runs in single precision on the tensor cores (3 x TF32 split operands, fp32 accumulation) with
+ * an exact power-of-two scale per operand row, re-decided every block diagonal; tables, loop terms, scale bookkeeping and the
+ * exterior sum stay fp64.  Tolerance 1e-4 relative in log Z.  All designs of a batch share one precision. */
+enum { CDZ_FP64 = 0, CDZ_FP32_SCALED = 1 };
 
 /* Nearest-neighbour loop model (BASELINE.json configs[0]); energies in kcal/mol.
  *   hairpin(l)  = hairpin_a + hairpin_b * kT * ln(l / hairpin_l0) + tmm[p(i,j)][phi_{i+1}][phi_{j-1}],  l >= min_hairpin

@@ -362,6 +362,8 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
     for (int D = 2; D < tt->NB; ++D) tiles = std::max(tiles, (size_t)(tt->NB - D) * (size_t)std::min(CDZ_MAX_SPLIT, D - 1));
     b.GP = k.take<double>(tiles * CDZ_TB * CDZ_TB);
   }
+  b.eA = k.take<int>(S);
+  b.eB = k.take<int>(S);
   b.ctrl = k.take<int>(64);
   b.result = k.take<double>(16);
   b.Qext = k.take<double>(S);
@@ -387,7 +389,7 @@ size_t carve(const cdz_tt* tt, void* base, Ctx* c, Ctx** d_ctx) {
 
 extern "C" int cdz_workspace_bytes(const cdz_tt* tt, int precision, size_t* bytes) {
   if (!tt || !bytes) { cdz_set_error("cdz_workspace_bytes: null argument"); return CDZ_EINVAL; }
-  if (precision != CDZ_FP64) { cdz_set_error("only CDZ_FP64 is implemented"); return CDZ_EINVAL; }
+  if (precision != CDZ_FP64 && precision != CDZ_FP32_SCALED) { cdz_set_error("unknown precision"); return CDZ_EINVAL; }
   *bytes = carve(tt, nullptr, nullptr, nullptr);
   return CDZ_OK;
 }
@@ -468,7 +470,7 @@ static int upload(cdz_tables* T) {
 static int make_tables(const cdz_model* m, const cdz_tt* tt, int precision, void* ws, size_t ws_bytes,
                        cudaStream_t st, cdz_tables** out) {
   if (!m || !tt || !out) { cdz_set_error("cdz_inside: null argument"); return CDZ_EINVAL; }
-  if (precision != CDZ_FP64) { cdz_set_error("only CDZ_FP64 is implemented"); return CDZ_EINVAL; }
+  if (precision != CDZ_FP64 && precision != CDZ_FP32_SCALED) { cdz_set_error("unknown precision"); return CDZ_EINVAL; }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
     cdz_set_error("no CUDA device: this library has no CPU fallback");

@@ -112,6 +112,160 @@ __global__ void __launch_bounds__(GEMM_THREADS) gemm_kernel(const Ctx* ctxs, int
 }
 
 // ------------------------------------------------------------------------------------------------
+// CDZ_FP32_SCALED: the same contraction in single precision on the tensor cores.  Every operand row is divided by an exact power of two
+// (the binary exponent of its largest finished entry, eA / eB, kept up to date by rowmax_kernel), converted to fp32 and split into two
+// TF32 numbers hi + lo; a.b ~ hi.hi + hi.lo + lo.hi on mma.sync.m16n8k8.tf32 with fp32 accumulators (the dropped lo.lo term is 2^-22
+// relative); the epilogue multiplies the partial tile back by 2^(eA[row] + eB[col]) in fp64 (single precision;
+// line 622: rows renormalised so that the products stay in range).
+// ------------------------------------------------------------------------------------------------
+constexpr int CDZ_NO_EXP = -(1 << 20);
+__device__ __forceinline__ unsigned f2tf32(float x) {
+  unsigned r;
+  asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ void mma_tf32(float (&c)[4], const unsigned (&a)[4], const unsigned (&b)[2]) {
+  asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+               : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+}
+__device__ __forceinline__ void split_tf32(double v, double scale, unsigned& hi, unsigned& lo) {
+  const float x = (float)(v * scale);
+  hi = f2tf32(x);
+  lo = f2tf32(x - __uint_as_float(hi));
+}
+
+__global__ void __launch_bounds__(GEMM_THREADS) gemm32_kernel(const Ctx* ctxs, int D, int nsplit) {
+  extern __shared__ double gsm[];
+  const Ctx& cx = ctxs[blockIdx.y];
+  const int I = blockIdx.x / nsplit, sp = blockIdx.x % nsplit, J = I + D;
+  if (J >= cx.tt.NB) return;
+  const size_t S = (size_t)cx.tt.S;
+  const int nk = D - 1;
+  const int kbeg = (I + 1 + (int)((long long)sp * nk / nsplit)) * CDZ_TB;
+  const int kend = (I + 1 + (int)((long long)(sp + 1) * nk / nsplit)) * CDZ_TB;
+  const double* A = cx.tab.QM + (size_t)I * CDZ_TB * S;
+  const double* Bm = cx.tab.QM1T + (size_t)J * CDZ_TB * S;
+  double* As = gsm;
+  double* Bs = gsm + GEMM_STAGES * CDZ_TB * GEMM_LD;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = (warp >> 1) * 32, wn = (warp & 1) * 32;
+  const int g = lane >> 2, tq = lane & 3;
+  // exact power-of-two row scales of the fragments this thread touches
+  double sa[4], sb[4];
+  int ea[4], eb[4];
+#pragma unroll
+  for (int r = 0; r < 4; ++r) {
+    ea[r] = max(cx.tab.eA[I * CDZ_TB + wm + r * 8 + g], -1000);  // (CDZ_NO_EXP: an all-zero row; any finite scale will do)
+    eb[r] = max(cx.tab.eB[J * CDZ_TB + wn + r * 8 + g], -1000);
+    sa[r] = scalbn(1.0, -ea[r]);
+    sb[r] = scalbn(1.0, -eb[r]);
+  }
+  auto load_stage = [&](int st, int kk) {
+    double* as = As + st * CDZ_TB * GEMM_LD;
+    double* bs = Bs + st * CDZ_TB * GEMM_LD;
+#pragma unroll
+    for (int r = 0; r < (CDZ_TB * GEMM_BK / 2) / GEMM_THREADS; ++r) {
+      const int c = tid + r * GEMM_THREADS, row = c >> 3, ch = (c & 7) * 2;
+      cp_async16(as + row * GEMM_LD + ch, A + (size_t)row * S + kk + ch);
+      cp_async16(bs + row * GEMM_LD + ch, Bm + (size_t)row * S + kk + ch);
+    }
+  };
+  float acc[2][4][4];
+#pragma unroll
+  for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni)
+#pragma unroll
+      for (int k = 0; k < 4; ++k) acc[mi][ni][k] = 0.0f;
+  const int nkt = (kend - kbeg) / GEMM_BK;
+#pragma unroll
+  for (int st = 0; st < GEMM_STAGES - 1; ++st) {
+    if (st < nkt) load_stage(st, kbeg + st * GEMM_BK);
+    asm volatile("cp.async.commit_group;\n" ::);
+  }
+  for (int kt = 0; kt < nkt; ++kt) {
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(GEMM_STAGES - 2));
+    __syncthreads();
+    const int nxt = kt + GEMM_STAGES - 1;
+    if (nxt < nkt) load_stage(nxt % GEMM_STAGES, kbeg + nxt * GEMM_BK);
+    asm volatile("cp.async.commit_group;\n" ::);
+    const double* as = As + (kt % GEMM_STAGES) * CDZ_TB * GEMM_LD;
+    const double* bs = Bs + (kt % GEMM_STAGES) * CDZ_TB * GEMM_LD;
+#pragma unroll
+    for (int k8 = 0; k8 < GEMM_BK / 8; ++k8) {
+      unsigned ah[2][4], al[2][4], bh[4][2], bl[4][2];
+#pragma unroll
+      for (int mi = 0; mi < 2; ++mi) {
+        // a0 = (row g, k tq), a1 = (row g+8, k tq), a2 = (row g, k tq+4), a3 = (row g+8, k tq+4)
+        const double* ap = as + (wm + mi * 16 + g) * GEMM_LD + k8 * 8 + tq;
+        split_tf32(ap[0], sa[mi * 2], ah[mi][0], al[mi][0]);
+        split_tf32(ap[8 * GEMM_LD], sa[mi * 2 + 1], ah[mi][1], al[mi][1]);
+        split_tf32(ap[4], sa[mi * 2], ah[mi][2], al[mi][2]);
+        split_tf32(ap[8 * GEMM_LD + 4], sa[mi * 2 + 1], ah[mi][3], al[mi][3]);
+      }
+#pragma unroll
+      for (int ni = 0; ni < 4; ++ni) {
+        // b0 = (k tq, n g), b1 = (k tq+4, n g)
+        const double* bp = bs + (wn + ni * 8 + g) * GEMM_LD + k8 * 8 + tq;
+        split_tf32(bp[0], sb[ni], bh[ni][0], bl[ni][0]);
+        split_tf32(bp[4], sb[ni], bh[ni][1], bl[ni][1]);
+      }
+#pragma unroll
+      for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+        for (int ni = 0; ni < 4; ++ni) {
+          mma_tf32(acc[mi][ni], al[mi], bh[ni]);
+          mma_tf32(acc[mi][ni], ah[mi], bl[ni]);
+          mma_tf32(acc[mi][ni], ah[mi], bh[ni]);
+        }
+    }
+  }
+  asm volatile("cp.async.wait_group 0;\n" ::);
+  double* C = cx.tab.GP + ((size_t)I * nsplit + sp) * (CDZ_TB * CDZ_TB);
+#pragma unroll
+  for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni) {
+      // c0 = (row g, col 2 tq), c1 = (g, 2 tq + 1), c2 = (g+8, 2 tq), c3 = (g+8, 2 tq + 1)
+      const int r0 = wm + mi * 16 + g, c0 = wn + ni * 8 + 2 * tq;
+      const int ec0 = max(cx.tab.eB[J * CDZ_TB + c0], -1000), ec1 = max(cx.tab.eB[J * CDZ_TB + c0 + 1], -1000);
+      *reinterpret_cast<double2*>(C + r0 * CDZ_TB + c0) =
+          make_double2(scalbn((double)acc[mi][ni][0], ea[mi * 2] + ec0), scalbn((double)acc[mi][ni][1], ea[mi * 2] + ec1));
+      *reinterpret_cast<double2*>(C + (r0 + 8) * CDZ_TB + c0) =
+          make_double2(scalbn((double)acc[mi][ni][2], ea[mi * 2 + 1] + ec0), scalbn((double)acc[mi][ni][3], ea[mi * 2 + 1] + ec1));
+    }
+}
+
+// Row scales of the fp32 contraction: eA[row] / eB[row] = binary exponent of the largest entry of the QM / QM1T row over the finished
+// blocks (0 for an all-zero row).  full = 0: fold in the block finished on diagonal D; full = 1 (after a rescale event, which shifts
+// the entries of a row by column-dependent powers of two): recompute over all finished blocks.
+__global__ void __launch_bounds__(256) rowmax_kernel(const Ctx* ctxs, int D, int full) {
+  const Ctx& cx = ctxs[blockIdx.y];
+  const DevTT& t = cx.tt;
+  const DevTab& b = cx.tab;
+  const int NB = t.NB, lane = threadIdx.x & 31;
+  const size_t S = (size_t)t.S;
+  for (int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); w < 2 * t.S; w += gridDim.x * (blockDim.x >> 5)) {
+    const int which = w >= t.S, row = which ? w - t.S : w, rb = row / CDZ_TB;
+    // QM row of block-row I: finished column blocks I .. I+D;  QM1T row of block J: finished column blocks J-D .. J
+    int c0, c1;
+    if (!which) { c0 = (full ? rb : rb + D) * CDZ_TB; c1 = min(NB, rb + D + 1) * CDZ_TB; }
+    else { c0 = max(0, rb - D) * CDZ_TB; c1 = (full ? rb + 1 : max(0, rb - D) + 1) * CDZ_TB; if (!full && rb - D < 0) c1 = c0; }
+    const double* p = (which ? b.QM1T : b.QM) + (size_t)row * S;
+    double mx = 0.0;
+    for (int c = c0 + lane; c < c1; c += 32) mx = fmax(mx, fabs(p[c]));
+    for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if (lane == 0) {
+      int* e = which ? b.eB : b.eA;
+      const int ex = (mx > 0.0 && mx < 1.0e308) ? ilogb(mx) : CDZ_NO_EXP;  // CDZ_NO_EXP: no non-zero entry yet
+      e[row] = (full || D == 0) ? ex : max(e[row], ex);
+      if (!(mx < 1.0e308)) b.ctrl[1] = 1;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // per-position power-of-two scaling (replaces the random-vector Renormalize of PAPER.md line 622)
 // ------------------------------------------------------------------------------------------------
 // One CTA per design.  After block diagonal D: the longest cell of every block (I, I+D) gives a local growth
@@ -408,6 +562,10 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
     if (rc != CDZ_OK) return rc;
   }
   CDZ_CUDA(cudaFuncSetAttribute(gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
+  CDZ_CUDA(cudaFuncSetAttribute(gemm32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
+  const bool fp32 = ts[0]->precision == CDZ_FP32_SCALED;
+  for (int b = 1; b < B; ++b)
+    if (ts[b]->precision != ts[0]->precision) { cdz_set_error("all designs of a batch must share one precision"); return CDZ_EINVAL; }
   // accounting: launch counts always; with profiling on, one event before every launch group (class of the group
   // that follows) so that consecutive event pairs give per-class device time on this stream
   cdz_tables* T0 = ts[0];
@@ -431,10 +589,15 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
     const int nsplit = cdz_nsplit(NBmax, D, B);
     if (nsplit > 0) {
       mark(0, 1);
-      gemm_kernel<<<dim3(nblk * nsplit, B), GEMM_THREADS, GEMM_SMEM, st>>>(d_ctxs, D, nsplit);
+      if (fp32) gemm32_kernel<<<dim3(nblk * nsplit, B), GEMM_THREADS, GEMM_SMEM, st>>>(d_ctxs, D, nsplit);
+      else gemm_kernel<<<dim3(nblk * nsplit, B), GEMM_THREADS, GEMM_SMEM, st>>>(d_ctxs, D, nsplit);
     }
     mark(1, 1);
     cdz_launch_cells(d_ctxs, B, nblk, D, nsplit, &ccfg, st);
+    if (fp32 && D + 2 < NBmax) {  // (the last contraction is on diagonal NB-1 and reads the blocks finished up to NB-2)
+      mark(2, 1);
+      rowmax_kernel<<<dim3(148, B), 256, 0, st>>>(d_ctxs, D, 0);
+    }
     if (D == next_event && D + 1 < NBmax) {
       next_event *= 2;
       mark(2, 16);
@@ -442,6 +605,7 @@ int cdz_launch_inside(cdz_tables* const* ts, int B, cudaStream_t st) {
       const int gx = std::min(nrmax, 148 * 8);
       for (int which = 0; which <= 13; ++which) rescale_kernel<<<dim3(gx, B), 256, 0, st>>>(d_ctxs, which, D);
       rescale_xs_kernel<<<dim3(std::min(nmax, 148 * 8), B), 256, 0, st>>>(d_ctxs, D);
+      if (fp32) rowmax_kernel<<<dim3(148, B), 256, 0, st>>>(d_ctxs, D, 1);
     }
   }
   mark(3, 1 + NBmax);

@@ -106,6 +106,8 @@ struct DevTabT {
   int* EB;       // [S]  dP at the position of every bond index
   int* EL;       // [LS] dP at the position of every left state
   int* ER;       // [RS] dP at (position + 1) of every right state
+  int* eA;       // [S] CDZ_FP32_SCALED: binary exponent of the largest finished entry of every QM row (row scale of the fp32 contraction)
+  int* eB;       // [S] the same for the rows of QM1T
   int* ctrl;     // control block: [0]=n_rescales [1]=overflow flag [2]=max |exponent| seen at an event
   double* result; // [0]=logZ [1]=Z mantissa [2]=log scale
 };

@@ -337,3 +337,50 @@ def test_rescale_schedule_invariance(B, cfg):
         assert abs(lz2 - lz) <= 1e-12 * abs(lz), (first, lz, lz2)
         assert tg.info()["n_rescales"] != n0 or cfg == 2
     tg.destroy()
+
+
+# ---- CDZ_FP32_SCALED: single-precision split-point contraction (BASELINE.json configs[2], tolerance 1e-4 relative in log Z) ---------
+FP32_RTOL = 1e-4
+
+
+@pytest.mark.parametrize("cfg,L", [(1, 20), (5, 40), (2, 100), (1, 200), (5, 150), (2, 300)])
+def test_fp32_scaled_vs_oracle_and_fp64(B, O, cfg, L):
+    """The fp32-scaled path against the oracle where it finishes in seconds (or is stored) and against the fp64 GPU path."""
+    m = I.nn_model()
+    d = I.design(cfg, 0, L)
+    tt = B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
+    t32, lz32 = B.inside(B.Model(m), tt, precision=B.FP32_SCALED)
+    t64, lz64 = B.inside(B.Model(m), tt)
+    assert abs(lz32 - lz64) <= FP32_RTOL * abs(lz64)
+    assert t32.info()["precision"] == B.FP32_SCALED
+    if d.n <= 300:
+        lo = O.inside(m, O.TT.build(d.aa, d.kind, d.codon_logw, d.pair_logw)).logZ
+        assert abs(lz32 - lo) <= FP32_RTOL * abs(lo)
+    stored = {(int(r[0]), int(r[2])): float(r[4]) for r in _stored_oracle_rows()}
+    if (cfg, L) in stored:
+        assert abs(lz32 - stored[(cfg, L)]) <= FP32_RTOL * abs(stored[(cfg, L)])
+    # samples drawn from the fp32-contracted tables are valid states
+    if d.n <= 450:
+        seq, pair = t32.sample(8, d.sample_seed)
+        tto = O.TT.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
+        for k in range(8):
+            assert np.isfinite(O.logweight(m, tto, seq[k].cpu().numpy(), pair[k].cpu().numpy()))
+
+
+def test_fp32_scaled_config3_and_config4(B):
+    """configs[2] (1000 aa, codon-pair TT, 3000 nt) through the fp32-scaled path: against the fp64 GPU path and, when the hours-long
+    oracle run has been stored (tests/golden/oracle_logz.txt), against the oracle; the same at the headline size."""
+    stored = {(int(r[0]), int(r[2])): float(r[4]) for r in _stored_oracle_rows()}
+    for cfg in (3, 4):
+        d = I.design(cfg, 0)
+        tt = B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
+        t32, lz32 = B.inside(B.Model(I.nn_model()), tt, precision=B.FP32_SCALED)
+        t32.destroy()
+        t64, lz64 = B.inside(B.Model(I.nn_model()), tt)
+        t64.destroy()
+        assert abs(lz32 - lz64) <= FP32_RTOL * abs(lz64), (cfg, lz32, lz64)
+        if (cfg, len(d.aa)) in stored:
+            want = stored[(cfg, len(d.aa))]
+            assert abs(lz32 - want) <= FP32_RTOL * abs(want)
+            assert abs(lz64 - want) <= LOGZ_RTOL * abs(want)
+        print(f"config {cfg}: fp32-scaled {lz32:.9f} fp64 {lz64:.9f} rel diff {abs(lz32 - lz64) / abs(lz64):.2e}")
