@@ -33,6 +33,7 @@ SAMPLES = {1: 1000, 2: 0, 3: 0, 4: 100, 5: 256}
 WORKLOADS = {
     1: "configs[0]: 20-aa protein, single-codon TT, fp64, 1000 samples",
     2: "configs[1]: 300-aa protein, codon-pair TT, fp64",
+    3: "configs[2]: 1000-aa protein (3000 nt), codon-pair TT, fp32-scaled split-point contraction (3xTF32, fp64 tables)",
     4: "configs[3]: 5000-aa protein (15000 nt), single-codon TT, codon weights, fp64 inside pass + 100 samples",
     5: "configs[4]: 150-aa protein, codon-pair TT, fp64, 256 samples (one item of the batch)",
 }
@@ -158,12 +159,41 @@ def oracle_sample(cfg: int, L_sample: int):
                        f"({d.n} nt) of the workload's design: {ncc + nloop:.3e} cell-contractions in {dt:.1f} s")
 
 
+ORACLE_L = {1: 20, 2: 60, 3: 60, 4: 100, 5: 60}  # residues of the bounded oracle sample (config 1: the whole design)
+
+
+def oracle_full_size(cfg: int, sample: dict):
+    """The oracle on the WHOLE workload: the stored run of tests/golden/oracle_logz.txt where one exists (measured once on the
+    8-core build box by tests/golden/make_golden.py, oracle only), otherwise an extrapolation from the live sample, labelled."""
+    path = os.path.join(ROOT, "tests", "golden", "oracle_logz.txt")
+    full_L = {1: 20, 2: 300, 3: 1000, 4: 5000, 5: 150}[cfg]
+    try:
+        for ln in open(path):
+            f = ln.split()
+            if f and f[0] == str(cfg) and int(f[2]) == full_L:
+                n = int(f[3])
+                ncc, nloop = counts(n)
+                sec = max(float(f[5]), 0.5)
+                return {"kind": "stored", "seconds": sec, "cores": 8, "value": (ncc + nloop) / sec, "unit": UNIT,
+                        "note": "whole design, plain long-double recursion, measured on the 8-core build box (tests/golden/oracle_logz.txt)"}
+    except OSError:
+        pass
+    n_full = 3 * full_L
+    ncc, nloop = counts(n_full)
+    ncs, nls = counts(sample["n"])
+    # loop terms scale with their count; the split-point sum with N_cc (the sample's cost is dominated by the loop terms)
+    sec = sample["seconds"] * ((nloop + ncc) / max(nls + ncs, 1.0))
+    return {"kind": "EXTRAPOLATED", "seconds": sec, "cores": sample["cores"], "value": (ncc + nloop) / sec, "unit": UNIT,
+            "note": "EXTRAPOLATED from the live sample by the ratio of cell-contraction counts (the plain oracle cannot hold a "
+                    f"{n_full}-nt design: long-double range and hours of CPU time); not a measurement"}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     cfg = args.config
-    L_sample = args.oracle_L or {1: 20, 2: 60, 4: 100, 5: 60}[cfg]
+    L_sample = args.oracle_L or ORACLE_L[cfg]
     vals = []
     for _ in range(args.warmup):
         pass  # the oracle has no warm state; warm-up steps are no-ops
@@ -209,7 +239,8 @@ def run_cdz(args):
     J = SAMPLES[cfg] if args.samples is None else args.samples
     model = B.Model(I.nn_model())
     tt = B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
-    tab, logz0 = B.inside(model, tt)  # allocation + first pass (untimed)
+    fp32 = (args.precision == "fp32") if args.precision else (cfg == 3)
+    tab, logz0 = B.inside(model, tt, precision=B.FP32_SCALED if fp32 else B.FP64)  # allocation + first pass (untimed)
     n = d.n
     ncc, nloop = counts(n)
     units = ncc + nloop
@@ -232,7 +263,6 @@ def run_cdz(args):
     # ---- device-timed region -------------------------------------------------------------------------------------
     for _ in range(max(args.warmup, 3)):
         step()
-    tab.set_profiling(True)
     barrier()
     clocks = ClockSampler(local)
     if rank == 0:
@@ -246,12 +276,17 @@ def run_cdz(args):
     ev1.record(stream)
     barrier()
     ms_total = ev0.elapsed_time(ev1)
-    prof = tab.profile()  # events of the last timed step
+    clk = clocks.stop() if rank == 0 else None
+    # per-kernel-class device times: ONE extra, untimed step with an event between consecutive launches (the timed steps above run
+    # with profiling off, so no event records sit inside the timed region)
+    tab.set_profiling(True)
+    step()
+    torch.cuda.synchronize()
+    prof = tab.profile()
     prof_ms, prof_launches = prof["ms"], prof["launches"]
+    tab.set_profiling(False)
     logz = tab.logz()
     info = tab.info()
-    clk = clocks.stop() if rank == 0 else None
-    tab.set_profiling(False)
     ms_step = reduce_max(ms_total, "cuda") / args.steps
     value = whole_job_value(units, world, ms_step)
 
@@ -266,7 +301,11 @@ def run_cdz(args):
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
+        # the user's call sequence: build the tensor train from the protein and the weights (host, O(n)), then one host-buffer call
+        # (operator lists and cores host -> device, inside pass, traceback, samples device -> host, log Z)
+        tt_step = B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
         lz_e2e = tab.run_host(J, d.sample_seed, seq_h if J else None, pair_h if J else None, stream)
+        del tt_step
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
     e2e_value = whole_job_value(units, world, 1e3 * reduce_max(e2e_s, "cuda"))
@@ -277,15 +316,23 @@ def run_cdz(args):
         tab.rerun(stream)
         bpp, base_m, codon_m = tab.marginals(stream)  # warm-up
         torch.cuda.synchronize()
-        t0 = time.perf_counter()
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        m0.record(stream)
         bpp, base_m, codon_m = tab.marginals(stream)
+        m1.record(stream)
         torch.cuda.synchronize()
-        marg_ms = 1e3 * (time.perf_counter() - t0)
         up = torch.triu(bpp, 1)
-        marg = {"what": "base-pair probabilities P(i.j), eq 2.5 (cdz_marginals: outside / adjoint pass, DESIGN.md section 9)",
-                "ms": marg_ms, "gpu_launches": n + 2, "expected_pairs": float(up.sum()),
+        marg = {"what": "cdz_marginals: outside / adjoint pass -> base-pair probabilities (eq 2.5), base (eq 2.6) and codon (eq 2.7) "
+                        "marginals, DESIGN.md section 9",
+                "ms": m0.elapsed_time(m1), "ratio_to_inside": m0.elapsed_time(m1) / info["inside_ms"], "gpu_launches": n + 7,
+                "expected_pairs": float(up.sum()),
                 "max_row_sum_error": float(((up + up.T).sum(1) + torch.diagonal(bpp) - 1.0).abs().max()),
-                "timing": "host clock around the call (it synchronises the stream before returning), workspace allocation included"}
+                "max_base_sum_error": float((base_m.sum(1) - 1.0).abs().max()),
+                "max_codon_sum_error": float((codon_m.sum(1) - 1.0).abs().max()),
+                "note": "the unpaired diagonal and the base / codon marginals come from the operator usages, so none of the three sum "
+                        "rules holds by construction; device time by CUDA events, workspace allocated by the caller beforehand "
+                        "(allocation of the torch tensor inside the timed call)"}
+        del bpp, base_m, codon_m, up
 
     if rank != 0:
         if world > 1:
@@ -301,6 +348,7 @@ def run_cdz(args):
         pass
     dmma = measure_peak(1)
     dfma = measure_peak(0)
+    ffma = measure_peak(2)
     bf16 = peaks.get("bf16_tflops")
     sbar_n = info["sigma_bar"] / n
     loop_mac = nloop * 2.0 * sbar_n ** 3
@@ -308,7 +356,16 @@ def run_cdz(args):
     dominant = max(cls, key=cls.get) if cls else "gemm"
     gemm_ms, gemm_l = prof_ms.get("gemm", 0.0), prof_launches.get("gemm", 0)
     roof_gemm = None
-    if gemm_ms > 0:
+    if gemm_ms > 0 and fp32:
+        ach = 2.0 * info["split_mac"] / (gemm_ms * 1e-3) / 1e12
+        roof_gemm = {"kernel": "gemm32_kernel (split-point contraction, 3xTF32 on mma.sync m16n8k8, fp32 accumulate, fp64 operands in HBM)",
+                     "bound": "tensor", "achieved": ach, "peak": ffma, "unit": "TFLOP/s", "frac": ach / ffma, "traffic": None,
+                     "launches": gemm_l, "avg_launch_ms": gemm_ms / max(gemm_l, 1),
+                     "algorithmic_flop_per_step": 2.0 * info["split_mac"],
+                     "peak_source": "in-run register-resident fp32 FMA loop (libcdz_peak.so): the vector fp32 rate is the bar an "
+                                    "exact-to-fp32 contraction has to beat; the 3xTF32 split issues 3 MMAs per product",
+                     "share_of_step": gemm_ms / ms_step}
+    elif gemm_ms > 0:
         ach = 2.0 * info["split_mac"] / (gemm_ms * 1e-3) / 1e12
         roof_gemm = {"kernel": "gemm_kernel (split-point contraction, fp64 mma.sync m8n8k4)", "bound": "tensor",
                      "achieved": ach, "peak": dmma, "unit": "TFLOP/s", "frac": ach / dmma, "traffic": None,
@@ -318,12 +375,11 @@ def run_cdz(args):
                                     "MEASURED_PEAKS.json has no fp64 entry; rule-derived alternative = bf16_tflops x "
                                     "45/2250 = %s" % (None if bf16 is None else round(bf16 * 45.0 / 2250.0, 2)),
                      "share_of_step": gemm_ms / ms_step}
-    # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch near block diagonal D = 100 of this workload, from the
-    # single-pass ncu capture summarised in profiles/r1h_launches.md (only meaningful for config 4 at full length)
-    ncu_traffic = {"gemm": 1908146432 + 0, "block": 376736768 + 0} if (cfg == 4 and not args.L) else {}
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed ncu summary of THIS source state only: the file
+    # records a hash of the kernel sources; if the sources have changed since the capture the traffic is reported as null
+    ncu_traffic = committed_traffic(cfg if not args.L else None)
     if roof_gemm:
         roof_gemm["traffic"] = ncu_traffic.get("gemm")
-        roof_gemm["traffic_note"] = "one launch at D~100: no operand reuse across a block diagonal"
     block_ms, block_l = prof_ms.get("block", 0.0), prof_launches.get("block", 0)
     roof_block = None
     if block_ms > 0:
@@ -332,19 +388,40 @@ def run_cdz(args):
                       "bound": "alu", "achieved": ach, "peak": dfma, "unit": "TFLOP/s", "frac": ach / dfma,
                       "traffic": ncu_traffic.get("block"), "launches": block_l, "avg_launch_ms": block_ms / max(block_l, 1),
                       "algorithmic_flop_per_step": 2.0 * loop_mac,
-                      "note": "latency-bound, not ALU-bound: ~35 us per in-block anti-diagonal x 2n-step chain (DESIGN.md 8.1)",
+                      "note": "latency-bound, not ALU-bound: see latency_floor (DESIGN.md 8.1)",
                       "peak_source": "in-run register-resident fp64 FMA loop (cdz_measure_peak)",
                       "share_of_step": block_ms / ms_step}
     roofline = roof_block if dominant == "block" and roof_block else (roof_gemm or roof_block)
 
+    # the third number: dependency-latency floor of the blocked wavefront = launches x (empty dependent launch) +
+    # in-block anti-diagonal steps x barrier rounds per step x (one __syncthreads round of a 512-thread CTA), both measured here
+    import ctypes as C
+
+    t_launch, t_bar = C.c_double(), C.c_double()
+    peak_lib().cdz_peak_launch_us(2000, C.byref(t_launch))
+    peak_lib().cdz_peak_barrier_us(20000, C.byref(t_bar))
+    sigma, _, _ = tt.describe()
+    nb_blocks = int(prof_launches.get("block", 0))
+    pos_per_block = (n + 1) / max(nb_blocks, 1)
+    inblock_steps = nb_blocks * (2.0 * pos_per_block - 1.0)
+    barriers_per_step = 6
+    n_launch = sum(int(v) for k, v in prof_launches.items() if k != "sample")
+    latency_floor = {"launches": n_launch, "t_launch_us": t_launch.value, "in_block_steps": inblock_steps,
+                     "barrier_rounds_per_step": barriers_per_step, "t_barrier_round_us": t_bar.value,
+                     "floor_ms": 1e-3 * (n_launch * t_launch.value + inblock_steps * barriers_per_step * t_bar.value),
+                     "note": "lower bound from empty dependent launches and empty barrier rounds only; the measured step also waits "
+                             "on dependent global / shared memory loads inside every round"}
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        o = oracle_sample(cfg, args.oracle_L or {1: 20, 2: 60, 4: 100, 5: 60}[cfg])
-        cpu = {"value": o["value"], "unit": UNIT, "cores": o["cores"], "kind": "oracle", "sample": o["sample"]}
+        o = oracle_sample(cfg, args.oracle_L or ORACLE_L[cfg])
+        cpu = {"value": o["value"], "unit": UNIT, "cores": o["cores"], "kind": "oracle", "sample": o["sample"],
+               "full_size": oracle_full_size(cfg, o)}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32 contraction (3xTF32) + f64 tables" if fp32 else "f64",
         "data": "synthetic",
         "config": {"workload": WORKLOADS.get(cfg, f"config {cfg}") + (f" [L overridden to {args.L}]" if args.L else ""),
                    "n_nt": n, "sigma_bar": info["sigma_bar"], "samples_per_step": J, "parallelism": "replicas only",
@@ -357,11 +434,14 @@ def run_cdz(args):
         "kernel_ms": prof_ms, "kernel_launches": prof_launches,
         "gpu_launches": int(sum(prof_launches.values())) * args.steps,
         "roofline": roofline, "roofline_gemm": roof_gemm, "roofline_block": roof_block,
-        "peaks": {"fp64_fma_tflops": dfma, "fp64_mma_tflops": dmma, "hbm_gbs": peaks.get("hbm_gbs"),
+        "peaks": {"fp64_fma_tflops": dfma, "fp64_mma_tflops": dmma, "fp32_fma_tflops": ffma, "hbm_gbs": peaks.get("hbm_gbs"),
                   "bf16_tflops": bf16},
+        "latency_floor": latency_floor,
         "cpu_baseline": cpu,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                "ms_per_step": 1e3 * e2e_s, "logZ": lz_e2e},
+                "ms_per_step": 1e3 * e2e_s, "logZ": lz_e2e,
+                "timed_region": "cdz_tt_build (host) + cdz_run_host: h2d of operator lists / cores, inside pass, traceback, d2h of "
+                                "samples and log Z; the device workspace and the model handle are created once before it"},
         "clocks": clk,
     }
     if marg is not None:
@@ -443,6 +523,30 @@ def run_batch(args):
     print(json.dumps(out), flush=True)
 
 
+def kernel_source_hash() -> str:
+    import hashlib
+
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2604_19718_b200", "csrc")
+    for name in sorted(os.listdir(csrc)):
+        if name.endswith((".cu", ".h")):
+            h.update(open(os.path.join(csrc, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def committed_traffic(cfg):
+    """profiles/traffic.json: {"source_hash": "...", "config": 4, "gemm": bytes per launch, "block": bytes per launch, "from": "..."}.
+    Only used when it was captured from exactly these kernel sources and this config; otherwise {} (traffic: null)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            rec = json.load(f)
+    except (OSError, ValueError):
+        return {}
+    if rec.get("source_hash") != kernel_source_hash() or rec.get("config") != cfg:
+        return {}
+    return rec
+
+
 def info_ms2(sigma) -> int:
     ms = max(sigma)
     return ms * ms
@@ -454,7 +558,8 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cdz", choices=["cdz", "reference"])
-    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 4, 5])
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--precision", default=None, choices=["fp64", "fp32"], help="default: fp32 for config 3, fp64 otherwise")
     ap.add_argument("--L", type=int, default=None, help="override the protein length (development only)")
     ap.add_argument("--samples", type=int, default=None)
     ap.add_argument("--oracle-L", type=int, default=None, dest="oracle_L")

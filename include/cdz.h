@@ -177,6 +177,18 @@ int cdz_marginals(cdz_tables* t, void* workspace_dev, size_t workspace_bytes, do
  * usage left [0,1] or the usages at some position do not sum to 1 within 1e-6 (non-finite values included), else CDZ_OK. */
 int cdz_marginals_status(cdz_tables* t);
 
+/* ---- fixed-sequence evaluation of sampled sequences (PAPER.md S4f line 779) ---- */
+/* For J sequences seq_host[J][n] (nucleotides 0..3, host) -- typically the output of cdz_sample -- computes with the same kernels
+ *   logZ_host[J]      log Z(phi) of the fixed sequence under the loop model (= -q(phi); ordinary McCaskill), required;
+ *   logW_host[J]      log W(phi), the sequence's weight in the design's tensor train (-inf if phi is outside the design space);
+ *                     NULL or needs `design`;
+ *   unpaired_host[J][n]  P(i unpaired | phi) from the outside pass; NULL to skip.
+ * Each sequence is the tensor train with one operator (0, phi_i, 0, 1) per position (lines 545-557); the sequences are advanced
+ * together in chunks by cdz_inside_batch (chunk size from the free device memory, at most max_batch if max_batch > 0).
+ * Blocking: returns after the results are in the host buffers.  Tables are created and released inside the call. */
+int cdz_eval_sequences(const cdz_model* m, const cdz_tt* design, int n, int J, const uint8_t* seq_host, int max_batch,
+                       double* logZ_host, double* logW_host, double* unpaired_host, void* stream);
+
 /* ---- convenience: host buffers end to end (used for the e2e timing) -------- */
 /* Builds nothing: runs cdz_inside_rerun, samples J states and copies them to host buffers. */
 int cdz_run_host(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_host, int32_t* pair_host, double* logZ_host,

@@ -22,7 +22,7 @@ EXPORTS = [
     "cdz_tt_from_operators", "cdz_tt_destroy", "cdz_tt_length", "cdz_tt_describe", "cdz_workspace_bytes",
     "cdz_inside", "cdz_inside_batch", "cdz_inside_rerun", "cdz_inside_rerun_batch", "cdz_tables_logz",
     "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample",
-    "cdz_debug_set_rescale_start", "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
+    "cdz_debug_set_rescale_start", "cdz_eval_sequences", "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
 ]
 
 
@@ -98,6 +98,7 @@ def lib():
     L.cdz_marginals.argtypes = [vp, vp, C.c_size_t, vp, vp, vp, vp]
     L.cdz_marginals_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
     L.cdz_marginals_status.argtypes = [vp]
+    L.cdz_eval_sequences.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, dp, dp, dp, vp]
     L.cdz_run_host.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, dp, vp]
     _lib = L
     return L
@@ -321,3 +322,15 @@ def inside_rerun_batch(tables, stream=None):
     B = len(tables)
     arr = (C.c_void_p * B)(*[t.h.value for t in tables])
     _check(lib().cdz_inside_rerun_batch(arr, B, _stream_ptr(stream)))
+
+
+def eval_sequences(model: Model, design: TensorTrain | None, seqs, want_unpaired=False, max_batch=0, stream=None):
+    """cdz_eval_sequences: seqs [J][n] uint8 (numpy or CPU tensor).  Returns (logZ [J], logW [J] or None, unpaired [J][n] or None)."""
+    seqs = np.ascontiguousarray(np.asarray(seqs), dtype=np.uint8)
+    J, n = seqs.shape
+    lz = np.zeros(J)
+    lw = np.zeros(J) if design is not None else None
+    un = np.zeros((J, n)) if want_unpaired else None
+    _check(lib().cdz_eval_sequences(model.h, design.h if design is not None else None, n, J,
+                                    seqs.ctypes.data_as(C.c_void_p), max_batch, _dp(lz), _dp(lw), _dp(un), _stream_ptr(stream)))
+    return lz, lw, un

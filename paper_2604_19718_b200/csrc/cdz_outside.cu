@@ -36,7 +36,7 @@ __device__ unsigned long long g_otime[16];
 
 namespace {
 
-constexpr int OT = 256;  // threads per CTA
+constexpr int OT = 512;  // threads per CTA
 constexpr int NW = OT / 32;
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -144,7 +144,7 @@ __host__ __device__ inline OPlan oplan(int MS, int ML, int MR, int nps) {
   p.ibsum = take(MS2); p.sbb = take(nps * MS2);
   p.xe = take(MS2); p.bl = take(MS2); p.br = take(MS2);
   p.z1 = take(ML * MS); p.z2 = take(MS * MR);
-  p.sb = take(nps * MS2); p.y = take(ML * MR); p.inn = take(nps * MS2);
+  p.sb = take(nps * MS2); p.y = take(ML * MR > 4 * MS * MR ? ML * MR : 4 * MS * MR); p.inn = take(nps * MS2);
   p.ddb = take(ML * MR);
   p.tl = take(3 * ML * MS); p.tr = take(3 * MS * MR);
   p.part = take(OT);
@@ -439,18 +439,26 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   // ---- 3: I(i,j)[slot][a'][c'], G[u,v][a'][c'], H, H1, H2 ----------------------------------------------------------------------------------
   const int Sa = t.sig[p], Sc = t.sig[j];  // a' in Sigma_{i+1}, c' in Sigma_j
   double* ibo = A.IB + ((size_t)(d % ORING) * n + i) * 16 * MS2;
+  // I[slot][a'][c'] = sum_{z at i: b = x, c = a'} sum_{z' at j: b = y, a = c'} x_z x_z' Qb-bar[l(z)][r(z')], in two steps through the dense
+  // cores: T1[x][a'][r] = sum_{l: x(l) = x} T_i[l][a'] Qb-bar[l][r], then I = sum_{r: y(r) = y} T_j[c'][r] T1[x][a'][r]
+  double* t1 = y;  // (Y and Z1 are not in use yet; T1 needs 4 MS MR <= ML MR + ML MS doubles, see oplan)
+  for (int e = tid; e < 4 * MS * nR; e += OT) {
+    const int x = e / (MS * nR), ap = (e / nR) % MS, r = e % nR;
+    double v = 0.0;
+    if (ap < Sa)
+      for (int l = 0; l < nL; ++l)
+        if (t.ls_x[Li0 + l] == x) v += TLi[l * MS + ap] * ab[l * nR + r];
+    t1[e] = v;
+  }
+  __syncthreads();
   for (int e = tid; e < 16 * MS2; e += OT) {
     const int sl = e / MS2, ap = (e % MS2) / MS, cp = e % MS;
     double v = 0.0;
     if (sl < nps && ap < Sa && cp < Sc) {
       const int x = m.slot_x[sl], yy = m.slot_y[sl];
-      for (int z = t.opstart[i]; z < t.opstart[i + 1]; ++z) {
-        if (t.op_b[z] != x || t.op_c[z] != ap) continue;
-        for (int zz = t.opstart[j]; zz < t.opstart[j + 1]; ++zz) {
-          if (t.op_b[zz] != yy || t.op_a[zz] != cp) continue;
-          v += t.op_x[z] * t.op_x[zz] * ab[t.op_l[z] * nR + t.op_r[zz]];
-        }
-      }
+      const double* tp = t1 + (x * MS + ap) * nR;
+      for (int r = 0; r < nR; ++r)
+        if (t.rs_y[Rj0 + r] == yy) v += TRj[cp * MR + r] * tp[r];
     }
     if (sl < nps) ibs[e] = v;
     ibo[e] = v;
