@@ -24,19 +24,21 @@
 //      pass does -- the usages of the operators at i, j (pair ends), i+1, j-1 (closing mismatch, size-1 bulges).
 // Every accumulator has a single writer per launch (role-separated), every sum a fixed order: results are bit-reproducible.
 // cdz_usage.cu finishes: E-bar chain, multiloop / exterior unpaired usages, base / codon marginals, unpaired probabilities.
+#include <vector>
+
 #include "cdz_outside.h"
 
 #ifdef CDZ_OTIMING
 #include <stdio.h>
-__device__ unsigned long long g_otime[16];
-#define OTICK(k) do { __syncthreads(); if (threadIdx.x == 0) { const long long now__ = clock64(); atomicAdd(&g_otime[k], (unsigned long long)(now__ - tlast__)); tlast__ = now__; } } while (0)
+__device__ unsigned long long g_otime[16], g_omax[16];
+#define OTICK(k) do { __syncthreads(); if (threadIdx.x == 0) { const long long now__ = clock64(); atomicAdd(&g_otime[k], (unsigned long long)(now__ - tlast__)); atomicMax(&g_omax[k], (unsigned long long)(now__ - tlast__)); tlast__ = now__; } } while (0)
 #else
 #define OTICK(k)
 #endif
 
 namespace {
 
-constexpr int OT = 512;  // threads per CTA
+constexpr int OT = 256;  // threads per CTA (512 measured slower: 0.33 vs 0.30 s at config 2)
 constexpr int NW = OT / 32;
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -57,6 +59,51 @@ __device__ __forceinline__ double warp_dot(const double* __restrict__ x, const d
   }
   for (; k < k1; k += 32) a0 += x[k] * y[k];
   return warp_sum((a0 + a1) + (a2 + a3));
+}
+
+// All nx x ny dot products  out[a * ny + c] = sum_{kb in [k0,k1)} X[a * S + kb] Y[c * S + kb]  of two small groups of table rows at once: every
+// thread strides the bond range (coalesced), loads the nx + ny values of its column once and keeps the nx x ny accumulators; warp shuffle
+// trees, then a fixed-order sum over the warps.  MSX = compile-time bound of nx, ny (4 or 8).
+template <int MSX, int NT_>
+__device__ __forceinline__ void gather_all(const double* __restrict__ X, int nx, const double* __restrict__ Y, int ny, size_t S, int k0,
+                                           int k1, double* out, double* red) {
+  constexpr int RC = MSX == 4 ? 4 : 2;  // rows per pass: 16 accumulators per thread (register budget of 4 CTAs per SM)
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int a0 = 0; a0 < nx; a0 += RC) {
+    double acc[RC][MSX];
+#pragma unroll
+    for (int a = 0; a < RC; ++a)
+#pragma unroll
+      for (int c = 0; c < MSX; ++c) acc[a][c] = 0.0;
+    for (int kb = k0 + (int)threadIdx.x; kb < k1; kb += NT_) {
+      double x[RC], y[MSX];
+#pragma unroll
+      for (int a = 0; a < RC; ++a) x[a] = a0 + a < nx ? X[(size_t)(a0 + a) * S + kb] : 0.0;
+#pragma unroll
+      for (int c = 0; c < MSX; ++c) y[c] = c < ny ? Y[(size_t)c * S + kb] : 0.0;
+#pragma unroll
+      for (int a = 0; a < RC; ++a)
+#pragma unroll
+        for (int c = 0; c < MSX; ++c) acc[a][c] += x[a] * y[c];
+    }
+#pragma unroll
+    for (int a = 0; a < RC; ++a)
+#pragma unroll
+      for (int c = 0; c < MSX; ++c) {
+        if (a0 + a < nx && c < ny) {  // (uniform across the CTA)
+          const double v = warp_sum(acc[a][c]);
+          if (lane == 0) red[warp * (MSX * MSX) + (a0 + a) * MSX + c] = v;
+        }
+      }
+  }
+  __syncthreads();
+  if ((int)threadIdx.x < nx * ny) {
+    const int a = threadIdx.x / ny, c = threadIdx.x % ny;
+    double v = 0.0;
+    for (int w = 0; w < NT_ / 32; ++w) v += red[w * (MSX * MSX) + a * MSX + c];
+    out[a * ny + c] = v;
+  }
+  __syncthreads();
 }
 
 // Qext-bar, sequential over bond positions k = n .. 0 (one CTA):  AX(k) = Tbar_k AX(k+1) + sum_{j>=k} Qbs(k,j) AX(j+1), AX(n) = 1/Z
@@ -119,18 +166,9 @@ __global__ void __launch_bounds__(256) transpose_kernel(const double* __restrict
   }
 }
 
-struct OV {
-  const DevTT& t;
-  const DevTab& b;
-  __device__ __forceinline__ double E(int p, int q, int a, int c) const {
-    if (q < p) return a == c ? 1.0 : 0.0;
-    return b.EM[(size_t)(t.off[p] + a) * t.S + t.off[q + 1] + c];
-  }
-};
-
 // shared-memory plan of ocell_kernel (doubles); identical on host and device
 struct OPlan {
-  int am, aml, abs_, ab, qb, ibs, go, h, h1, h2, ibsum, sbb, xe, bl, br, z1, z2, sb, y, inn, ddb, tl, tr, part, total;
+  int am, aml, abs_, ab, qb, ibs, go, h, h1, h2, ibsum, sbb, xe, bl, br, z1, z2, sb, y, inn, ddb, tl, tr, part, red, total;
 };
 __host__ __device__ inline OPlan oplan(int MS, int ML, int MR, int nps) {
   OPlan p;
@@ -148,6 +186,7 @@ __host__ __device__ inline OPlan oplan(int MS, int ML, int MR, int nps) {
   p.ddb = take(ML * MR);
   p.tl = take(3 * ML * MS); p.tr = take(3 * MS * MR);
   p.part = take(OT);
+  p.red = take((OT / 32) * 64);
   p.total = o;
   return p;
 }
@@ -163,12 +202,15 @@ __device__ __forceinline__ double group_total(double* part, double v, int nent) 
   return s;
 }
 
-__global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d, int want_usage, double* __restrict__ bpp) {
+// PART 0: phases 1-3 and 4a-4b, the chain every later diagonal waits for; leaves Qb-bar, the pushed adjoints it consumed, G, H1, H2, sum I
+// and SB-bar of the cell in a scratch record.  PART 1: everything that only later consumers need (the pushes into the inner cells at least
+// four diagonals below, the stretch adjoints, the usages), run on a second stream so that it overlaps the chain of the next diagonals.
+template <int PART, int MSX>
+__global__ void __launch_bounds__(OT, 4) ocell_kernel(const Ctx* ctx, Adj A, int d, int want_usage, double* __restrict__ bpp) {
   extern __shared__ double osm[];
   const DevTT& t = ctx->tt;
   const DevTab& b = ctx->tab;
   const CModel& m = *ctx->cm;
-  const OV V{t, b};
   const int n = t.n, MS = t.MS, MS2 = MS * MS, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const size_t S = (size_t)t.S, RS = (size_t)t.RS;
   const int ML = A.ML, MR = A.MR, nps = m.nps;
@@ -176,7 +218,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   double *am = osm + pl.am, *aml = osm + pl.aml, *abs_ = osm + pl.abs_, *ab = osm + pl.ab, *qbv = osm + pl.qb, *ibs = osm + pl.ibs,
          *go = osm + pl.go, *h = osm + pl.h, *h1 = osm + pl.h1, *h2 = osm + pl.h2, *ibsum = osm + pl.ibsum, *sbb = osm + pl.sbb,
          *xe = osm + pl.xe, *bl = osm + pl.bl, *br = osm + pl.br, *z1 = osm + pl.z1, *z2 = osm + pl.z2, *sb = osm + pl.sb,
-         *y = osm + pl.y, *inn = osm + pl.inn, *ddb = osm + pl.ddb, *part = osm + pl.part;
+         *y = osm + pl.y, *inn = osm + pl.inn, *ddb = osm + pl.ddb, *part = osm + pl.part, *red = osm + pl.red;
   double* TLm = osm + pl.tl;            // T_{i-1}[lst][c]   (ML x MS)
   double* TLi = TLm + ML * MS;          // T_i
   double* TLp = TLi + ML * MS;          // T_{i+1}
@@ -204,6 +246,21 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     offW[which][idx] = ok ? t.off[pos] : 0;
     sigW[which][idx] = ok ? t.sig[pos] : 0;
   }
+  // boundary states of positions i-1, i, i+1 (left states) and j-1, j, j+1 (right states)
+  __shared__ uint8_t sLa[3][CDZ_MAX_STATES], sLx[3][CDZ_MAX_STATES], sRy[3][CDZ_MAX_STATES], sRc[3][CDZ_MAX_STATES];
+  if (tid >= 160 && tid < 160 + 6 * CDZ_MAX_STATES) {
+    const int w6 = (tid - 160) / CDZ_MAX_STATES, k = (tid - 160) % CDZ_MAX_STATES;
+    const int pos = w6 < 3 ? i - 1 + w6 : j - 1 + (w6 - 3);
+    if (pos >= 0 && pos < n) {
+      if (w6 < 3) {
+        const int l0 = t.loff[pos], nl = t.loff[pos + 1] - l0;
+        if (k < nl) { sLa[w6][k] = t.ls_a[l0 + k]; sLx[w6][k] = t.ls_x[l0 + k]; }
+      } else {
+        const int r0 = t.roff[pos], nr = t.roff[pos + 1] - r0;
+        if (k < nr) { sRy[w6 - 3][k] = t.rs_y[r0 + k]; sRc[w6 - 3][k] = t.rs_c[r0 + k]; }
+      }
+    }
+  }
   auto offA = [&](int pos) { return offW[0][pos - i + 35]; };
   auto sigA = [&](int pos) { return sigW[0][pos - i + 35]; };
   auto offB = [&](int pos) { return offW[1][pos - j + 35]; };
@@ -214,24 +271,30 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   // ---- dense cores of the six positions around the cell ------------------------------------------------------------------------------
   for (int k = tid; k < 3 * ML * MS + 3 * MS * MR; k += OT) (k < 3 * ML * MS ? TLm[k] : TRq[k - 3 * ML * MS]) = 0.0;
   __syncthreads();
-  if (tid < 6) {
-    const int pos = tid < 3 ? i - 1 + tid : j - 1 + (tid - 3);
-    if (pos >= 0 && pos < n) {
-      for (int z = t.opstart[pos]; z < t.opstart[pos + 1]; ++z) {
-        if (tid < 3) TLm[tid * ML * MS + t.op_l[z] * MS + t.op_c[z]] += t.op_x[z];
-        else TRq[(tid - 3) * MS * MR + t.op_a[z] * MR + t.op_r[z]] += t.op_x[z];
+  {
+    // one thread per operator of the six positions (<= 36 each); distinct operators hit distinct core entries, duplicates of a generic
+    // operator list add up (shared-memory atomics)
+    for (int e = tid; e < 6 * 64; e += OT) {
+      const int w6 = e / 64, k = e % 64;
+      const int pos = w6 < 3 ? i - 1 + w6 : j - 1 + (w6 - 3);
+      if (pos < 0 || pos >= n) continue;
+      const int z0 = t.opstart[pos], nz = t.opstart[pos + 1] - z0;
+      for (int zz = k; zz < nz; zz += 64) {
+        const int z = z0 + zz;
+        if (w6 < 3) atomicAdd(&TLm[w6 * ML * MS + t.op_l[z] * MS + t.op_c[z]], t.op_x[z]);
+        else atomicAdd(&TRq[(w6 - 3) * MS * MR + t.op_a[z] * MR + t.op_r[z]], t.op_x[z]);
       }
     }
   }
+  if constexpr (PART == 0) {
   // ---- 1: bond-level adjoints ------------------------------------------------------------------------------------------------------------
   // Qm-bar(i,j)[a,s] = sum_{kb >= off[j+2]} AM2[(i,a)][kb] QM1[(j+1,s)][kb]
-  for (int e = warp; e < nent; e += NW) {
-    const int ea = e / Sj1, ec = e % Sj1;
-    double v = 0.0;
-    if (j + 1 <= n - 1) v = warp_dot(A.AM2 + (size_t)(offi + ea) * S, A.QM1 + (size_t)(offj1 + ec) * S, t.off[j + 2], send, lane);
-    if (lane == 0) am[e] = v;
+  if (j + 1 <= n - 1) {
+    gather_all<MSX, OT>(A.AM2 + (size_t)offi * S, Si, A.QM1 + (size_t)offj1 * S, Sj1, S, t.off[j + 2], send, am, red);
+  } else {
+    if (tid < nent) am[tid] = 0.0;
+    __syncthreads();
   }
-  __syncthreads();
   if (tid < nent) {
     const int ea = tid / Sj1, ec = tid % Sj1;
     // M2-bar = Qm-bar + w_a w_c sum_{x,y} I(i-1,j+1)[x,y]
@@ -256,12 +319,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     A.AML[(size_t)(offi + ea) * S + offj1 + ec] = w;
   }
   // Qm1-bar = Qml-bar + w_b Qm1-bar(i,j+1) Tbar_{j+1}^T + sum_{rb < off[i]} QMT[(i,a)][rb] AM2T[(j+1,c)][rb]
-  for (int e = warp; e < nent; e += NW) {
-    const int ea = e / Sj1, ec = e % Sj1;
-    const double v = warp_dot(A.QMT + (size_t)(offi + ea) * S, A.AM2T + (size_t)(offj1 + ec) * S, 0, offi, lane);
-    if (lane == 0) abs_[e] = v;
-  }
-  __syncthreads();
+  gather_all<MSX, OT>(A.QMT + (size_t)offi * S, Si, A.AM2T + (size_t)offj1 * S, Sj1, S, 0, offi, abs_, red);
   if (tid < nent) {
     const int ea = tid / Sj1, ec = tid % Sj1;
     double w = aml[tid] + abs_[tid];
@@ -276,18 +334,20 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     abs_[tid] = m.wc * w + b.Qext[offi + ea] * A.AX[(size_t)(j + 1) * MS + ec];
   }
   __syncthreads();
+  }
   OTICK(0);
   if (!closed) {
-    // cells below the minimum hairpin span: nothing pairs; the interior-body adjoint chains still pass through (d >= 4 only matters
-    // when min_hairpin + 1 > 4)
+    if constexpr (PART == 1) return;
+    // cells below the minimum hairpin span: nothing pairs and none of their loop bodies exists
     if (d >= 4) {
-      double* xa = A.XA + ((size_t)(d & 1) * n + i) * XU * MS2;
-      double* xb = A.XB + ((size_t)(d & 1) * n + i) * XU * MS2;
+      double* xa = A.XA + ((size_t)(d % XRING) * n + i) * XU * MS2;
+      double* xb = A.XB + ((size_t)(d % XRING) * n + i) * XU * MS2;
       for (int e = tid; e < XU * MS2; e += OT) { xa[e] = 0.0; xb[e] = 0.0; }
     }
     // the I slot of this diagonal is read by the M2-bar of cell (i+1, j-1): it must not keep the values of diagonal d + ORING
     double* ibz = A.IB + ((size_t)(d % ORING) * n + i) * 16 * MS2;
     for (int e = tid; e < 16 * MS2; e += OT) ibz[e] = 0.0;
+    for (int e = tid; e < MS2; e += OT) A.IBS[((size_t)(d % ORING) * n + i) * MS2 + e] = 0.0;
     return;
   }
 
@@ -296,70 +356,95 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   const bool dressed = MI >= 2 && i >= 1 && j <= n - 2;
   const int nLm = dressed ? t.loff[i] - t.loff[i - 1] : 0, nRn = dressed ? t.roff[j + 2] - t.roff[j + 1] : 0;
   const int RDS = ML * MR + MS2 + ML * MS + MR * MS;
+  // scratch record of the cell (PART 0 -> PART 1): Qb-bar | DD-bar | G | H1 | H2 | sum I | SB-bar | flag
+  const int SCRS = scr_size(MS, ML, MR, nps);
+  double* scr = A.SC + ((size_t)(d % SRING) * n + i) * SCRS;
+  double *scr_ab = scr, *scr_ddb = scr_ab + ML * MR, *scr_go = scr_ddb + ML * MR, *scr_h1 = scr_go + 16 * MS2, *scr_h2 = scr_h1 + 4 * MS2,
+         *scr_ibsum = scr_h2 + 4 * MS2, *scr_sbb = scr_ibsum + MS2, *scr_flag = scr_sbb + nps * MS2;
+  if constexpr (PART == 1) {
+    for (int e = tid; e < ML * MR; e += OT) { ab[e] = scr_ab[e]; ddb[e] = scr_ddb[e]; }
+    for (int e = tid; e < 16 * MS2; e += OT) go[e] = scr_go[e];
+    for (int e = tid; e < 4 * MS2; e += OT) { h1[e] = scr_h1[e]; h2[e] = scr_h2[e]; }
+    for (int e = tid; e < MS2; e += OT) ibsum[e] = scr_ibsum[e];
+    for (int e = tid; e < nps * MS2; e += OT) sbb[e] = scr_sbb[e];
+  }
   double* rd = A.RD + ((size_t)(d % ORING) * n + i) * RDS;
-  if (dressed) {
+  if (PART == 0 && dressed) {
     const double *add = rd, *agi = rd + ML * MR, *ad1 = agi + MS2, *ad2 = ad1 + ML * MS;
     for (int e = tid; e < nLm * nRn; e += OT) {
       const int lst = e / nRn, rr = e % nRn;
-      const int a = t.ls_a[t.loff[i - 1] + lst], c = t.rs_c[t.roff[j + 1] + rr];
+      const int a = sLa[0][lst], c = sRc[2][rr];
       ddb[lst * MR + rr] = add[lst * MR + rr] + agi[a * MS + c] + ad1[lst * MS + c] + ad2[rr * MS + a];
     }
   }
   for (int e = tid; e < npair; e += OT) qbv[e] = b.QB[(size_t)(Li0 + e / nR) * RS + Rj0 + e % nR];
   __syncthreads();
+  bool anyp = true;
+  if constexpr (PART == 0) {
   if (dressed)
     for (int e = tid; e < RDS; e += OT) rd[e] = 0.0;  // consumed: the slot is clean for diagonal d - ORING
   {
-    // stack / bulge terms: pulled from the I tables of the closing pairs (i0,j0) = (i-1-l1, j+1+l2), l1 = 0 or l2 = 0
-    const int ng2 = OT / npair, e2 = tid % npair, g2 = tid / npair;
+    // stack / bulge terms: pulled from the I tables of the closing pairs (i0,j0) = (i-1-l1, j+1+l2), l1 = 0 or l2 = 0.
+    // Bulges of size >= 2 do not see the inner nucleotides: one sum per BOND pair (s,t) over the slot-summed tables IBS,
+    //   bb[s][t] = sum_l1 w_Bu(l1) sum_a' E(i0+1,i-1)[a',s] IBS(i0,j+1)[a',t] + sum_l2 w_Bu(l2) sum_c' IBS(i-1,j0)[s,c'] E(j+1,j0-1)[t,c']
+    {
+      const int eb = tid % nent, gb = tid / nent, ngb = OT / nent;
+      const int s_ = eb / Sj1, t_ = eb % Sj1;
+      double accb = 0.0;
+      if (gb < ngb)
+        for (int qq = gb; qq < 2 * (MI - 1); qq += ngb) {
+          const int left = qq < MI - 1, len = 2 + (left ? qq : qq - (MI - 1));
+          const int i0 = left ? i - 1 - len : i - 1, j0 = left ? j + 1 : j + 1 + len;
+          if (i0 < 0 || j0 > n - 1) continue;
+          const double* ibsr = A.IBS + ((size_t)((j0 - i0) % ORING) * n + i0) * MS2;
+          double v = 0.0;
+          if (left) {
+            const int Sa_ = sigA(i0 + 1);
+            for (int a = 0; a < Sa_; ++a) v += EA(i0 + 1, i - 1, a, s_) * ibsr[a * MS + t_];
+          } else {
+            const int Sc_ = sigB(j0);
+            for (int c = 0; c < Sc_; ++c) v += ibsr[s_ * MS + c] * EB(j + 1, j0 - 1, t_, c);
+          }
+          accb += m.wbu[len] * v;
+        }
+      const double tot = group_total(part, accb, nent);
+      if (tid < nent) am[tid] = tot;  // (Qm-bar is no longer needed)
+      __syncthreads();
+    }
+    // stacks and size-1 bulges keep the identity of the inner pair (weights by slot): one thread per state pair
+    const int e2 = tid % npair;
     const int ll = e2 / nR, rr = e2 % nR;
-    const int s = t.ls_a[Li0 + ll], xp = t.ls_x[Li0 + ll];
-    const int yp = t.rs_y[Rj0 + rr], tt_ = t.rs_c[Rj0 + rr];
+    const int s = sLa[1][ll], xp = sLx[1][ll];
+    const int yp = sRy[1][rr], tt_ = sRc[1][rr];
     const bool pairable = m.pslot[xp * 4 + yp] >= 0;
     double acc = 0.0;
-    if (g2 < ng2 && pairable) {
-      const int Pin_st = m.ptype[xp * 4 + yp];  // inner pair as (phi_k, phi_l): stacks and size-1 bulges
-      const int nlp = 2 * MI + 1;
-      for (int qq = g2; qq < nlp; qq += ng2) {
-        const int l1 = qq <= MI ? qq : 0, l2 = qq <= MI ? 0 : qq - MI;
+    if (tid < npair && pairable) {
+      const int Pin_st = m.ptype[xp * 4 + yp];  // inner pair as (phi_k, phi_l)
+      for (int qq = 0; qq < 3; ++qq) {
+        const int l1 = qq == 1, l2 = qq == 2;
+        if (l1 + l2 > MI) continue;
         const int i0 = i - 1 - l1, j0 = j + 1 + l2;
         if (i0 < 0 || j0 > n - 1) continue;
-        const int dd = j0 - i0;
-        const int Sa = sigA(i0 + 1), Sc = sigB(j0);
-        const double* ib = A.IB + ((size_t)(dd % ORING) * n + i0) * 16 * MS2;
-        if (l1 == 0 && l2 == 0) {
-          for (int sl = 0; sl < nps; ++sl)
-            acc += m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][Pin_st] * ib[sl * MS2 + s * MS + tt_];
-        } else if (l2 == 0) {
-          // left bulge: sum_{a'} E(i0+1,i-1)[a',s] I[x,y;a',t]
-          double ev[CDZ_MAX_BOND];
-#pragma unroll
-          for (int a = 0; a < CDZ_MAX_BOND; ++a) ev[a] = a < Sa ? EA(i0 + 1, i - 1, a, s) : 0.0;
-          for (int sl = 0; sl < nps; ++sl) {
-            const double w = m.wbu[l1] * (l1 == 1 ? m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][Pin_st] : 1.0);
-            double v = 0.0;
-#pragma unroll
-            for (int a = 0; a < CDZ_MAX_BOND; ++a)
-              if (a < Sa) v += ev[a] * ib[sl * MS2 + a * MS + tt_];
-            acc += w * v;
+        const double* ib = A.IB + ((size_t)((j0 - i0) % ORING) * n + i0) * 16 * MS2;
+        const int Sa_ = sigA(i0 + 1), Sc_ = sigB(j0);
+        for (int sl = 0; sl < nps; ++sl) {
+          const double w = m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][Pin_st];
+          double v = 0.0;
+          if (qq == 0) v = ib[sl * MS2 + s * MS + tt_];
+          else if (qq == 1) {  // left bulge of size 1: sum_a' Tbar_{i-1}[a',s] I[x,y;a',t]
+            for (int a = 0; a < Sa_; ++a) v += EA(i0 + 1, i - 1, a, s) * ib[sl * MS2 + a * MS + tt_];
+            v *= m.wbu[1];
+          } else {  // right bulge of size 1
+            for (int c = 0; c < Sc_; ++c) v += ib[sl * MS2 + s * MS + c] * EB(j + 1, j0 - 1, tt_, c);
+            v *= m.wbu[1];
           }
-        } else {
-          // right bulge: sum_{c'} I[x,y;s,c'] E(j+1,j0-1)[t,c']
-          double ev[CDZ_MAX_BOND];
-#pragma unroll
-          for (int c = 0; c < CDZ_MAX_BOND; ++c) ev[c] = c < Sc ? EB(j + 1, j0 - 1, tt_, c) : 0.0;
-          for (int sl = 0; sl < nps; ++sl) {
-            const double w = m.wbu[l2] * (l2 == 1 ? m.wst[m.ptype[m.slot_x[sl] * 4 + m.slot_y[sl]]][Pin_st] : 1.0);
-            double v = 0.0;
-#pragma unroll
-            for (int c = 0; c < CDZ_MAX_BOND; ++c)
-              if (c < Sc) v += ib[sl * MS2 + s * MS + c] * ev[c];
-            acc += w * v;
-          }
+          acc += w * v;
         }
       }
+      acc += am[s * Sj1 + tt_];
     }
-    const double v = group_total(part, acc, npair);
+    const double v = acc;
+    anyp = __syncthreads_or(tid < npair && pairable) != 0;  // can any nucleotide of i pair with any of j?
     if (tid < npair) {
       double w = 0.0;
       if (pairable) {
@@ -372,10 +457,10 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
           for (int lst = 0; lst < nLm; ++lst) {
             const double tl = TLm[lst * MS + s];
             if (tl == 0.0) continue;
-            const int up = t.ls_x[t.loff[i - 1] + lst];
+            const int up = sLx[0][lst];
             double r2 = 0.0;
             for (int r = 0; r < nRn; ++r)
-              r2 += TRn[tt_ * MR + r] * m.wtm[Pil][t.rs_y[t.roff[j + 1] + r]][up] * ddb[lst * MR + r];
+              r2 += TRn[tt_ * MR + r] * m.wtm[Pil][sRy[2][r]][up] * ddb[lst * MR + r];
             u += tl * r2;
           }
           w += u;
@@ -393,24 +478,29 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     }
     __syncthreads();
   }
+  }
   OTICK(1);
+  if constexpr (PART == 1) {
+    anyp = scr_flag[0] != 0.0;
+    __syncthreads();  // the scratch record is in shared memory
+  }
   // usages of the inner-mismatch operators z2 at i-1 (role IL) and z1' at j+1 (role IR)
-  if (want_usage && dressed) {
+  if (PART == 1 && want_usage && dressed && anyp) {
     const int z2b = t.opstart[i - 1], nz2 = t.opstart[i] - z2b, z1b = t.opstart[j + 1], nz1 = t.opstart[j + 2] - z1b;
     for (int e = tid; e < nz2 + nz1; e += OT) {
       double u = 0.0;
       if (e < nz2) {
         const int z = z2b + e, lst = t.op_l[z], s = t.op_c[z], up = t.op_b[z];
         for (int ll = 0; ll < nL; ++ll) {
-          if (t.ls_a[Li0 + ll] != s) continue;
-          const int xp = t.ls_x[Li0 + ll];
+          if (sLa[1][ll] != s) continue;
+          const int xp = sLx[1][ll];
           for (int rr = 0; rr < nR; ++rr) {
-            const int yp = t.rs_y[Rj0 + rr], tt_ = t.rs_c[Rj0 + rr];
+            const int yp = sRy[1][rr], tt_ = sRc[1][rr];
             if (m.pslot[xp * 4 + yp] < 0) continue;
             const int Pil = m.ptype[yp * 4 + xp];
             double r2 = 0.0;
             for (int r = 0; r < nRn; ++r)
-              r2 += TRn[tt_ * MR + r] * m.wtm[Pil][t.rs_y[t.roff[j + 1] + r]][up] * ddb[lst * MR + r];
+              r2 += TRn[tt_ * MR + r] * m.wtm[Pil][sRy[2][r]][up] * ddb[lst * MR + r];
             u += r2 * qbv[ll * nR + rr];
           }
         }
@@ -418,15 +508,15 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       } else {
         const int z = z1b + (e - nz2), r = t.op_r[z], tt_ = t.op_a[z], vp = t.op_b[z];
         for (int rr = 0; rr < nR; ++rr) {
-          if (t.rs_c[Rj0 + rr] != tt_) continue;
-          const int yp = t.rs_y[Rj0 + rr];
+          if (sRc[1][rr] != tt_) continue;
+          const int yp = sRy[1][rr];
           for (int ll = 0; ll < nL; ++ll) {
-            const int xp = t.ls_x[Li0 + ll], s = t.ls_a[Li0 + ll];
+            const int xp = sLx[1][ll], s = sLa[1][ll];
             if (m.pslot[xp * 4 + yp] < 0) continue;
             const int Pil = m.ptype[yp * 4 + xp];
             double r2 = 0.0;
             for (int lst = 0; lst < nLm; ++lst)
-              r2 += TLm[lst * MS + s] * m.wtm[Pil][vp][t.ls_x[t.loff[i - 1] + lst]] * ddb[lst * MR + r];
+              r2 += TLm[lst * MS + s] * m.wtm[Pil][vp][sLx[0][lst]] * ddb[lst * MR + r];
             u += r2 * qbv[ll * nR + rr];
           }
         }
@@ -435,9 +525,11 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     }
   }
 
+  const int Sa = t.sig[p], Sc = t.sig[j];  // a' in Sigma_{i+1}, c' in Sigma_j
+  const bool has_loop = q > p;            // positions i+1 and j-1 are distinct unpaired positions (always true for min_hairpin >= 3)
+  if constexpr (PART == 0) {
   OTICK(2);
   // ---- 3: I(i,j)[slot][a'][c'], G[u,v][a'][c'], H, H1, H2 ----------------------------------------------------------------------------------
-  const int Sa = t.sig[p], Sc = t.sig[j];  // a' in Sigma_{i+1}, c' in Sigma_j
   double* ibo = A.IB + ((size_t)(d % ORING) * n + i) * 16 * MS2;
   // I[slot][a'][c'] = sum_{z at i: b = x, c = a'} sum_{z' at j: b = y, a = c'} x_z x_z' Qb-bar[l(z)][r(z')], in two steps through the dense
   // cores: T1[x][a'][r] = sum_{l: x(l) = x} T_i[l][a'] Qb-bar[l][r], then I = sum_{r: y(r) = y} T_j[c'][r] T1[x][a'][r]
@@ -447,7 +539,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     double v = 0.0;
     if (ap < Sa)
       for (int l = 0; l < nL; ++l)
-        if (t.ls_x[Li0 + l] == x) v += TLi[l * MS + ap] * ab[l * nR + r];
+        if (sLx[1][l] == x) v += TLi[l * MS + ap] * ab[l * nR + r];
     t1[e] = v;
   }
   __syncthreads();
@@ -458,7 +550,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       const int x = m.slot_x[sl], yy = m.slot_y[sl];
       const double* tp = t1 + (x * MS + ap) * nR;
       for (int r = 0; r < nR; ++r)
-        if (t.rs_y[Rj0 + r] == yy) v += TRj[cp * MR + r] * tp[r];
+        if (sRy[1][r] == yy) v += TRj[cp * MR + r] * tp[r];
     }
     if (sl < nps) ibs[e] = v;
     ibo[e] = v;
@@ -474,6 +566,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     double v = 0.0;
     for (int sl = 0; sl < nps; ++sl) v += ibs[sl * MS2 + e];
     ibsum[e] = v;  // adjoint of Bl / Br / the multiloop closure: they enter `inner` of every pairable slot
+    A.IBS[((size_t)(d % ORING) * n + i) * MS2 + e] = v;
   }
   for (int e = tid; e < nps * MS2; e += OT) {
     // adjoint of SB[a'][slot'][c'] (stored [slot'][a'][c']):  sum_slot wst[P][P'] I[slot]
@@ -484,43 +577,52 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     sbb[e] = v;
   }
   __syncthreads();
-  const bool has_loop = q > p;  // positions i+1 and j-1 are distinct unpaired positions (always true for min_hairpin >= 3)
-  // H[c1][a2'] = sum_{z1 at p: c = c1} sum_{z2' at q: a = a2'} x x' G[b(z1),b(z2')][a(z1)][c(z2')]     (adjoint of XE)
-  for (int e = tid; e < MS2; e += OT) {
-    const int c1 = e / MS, a2p = e % MS;
-    double v = 0.0;
-    if (has_loop)
-      for (int z1 = t.opstart[p]; z1 < t.opstart[p + 1]; ++z1) {
-        if (t.op_c[z1] != c1) continue;
-        const double* Gz = go + (t.op_b[z1] * 4) * MS2 + t.op_a[z1] * MS;
-        for (int z2p = t.opstart[q]; z2p < t.opstart[q + 1]; ++z2p)
-          if (t.op_a[z2p] == a2p) v += t.op_x[z1] * t.op_x[z2p] * Gz[t.op_b[z2p] * MS2 + t.op_c[z2p]];
+  // Loop-side operators contracted with G through the dense cores T_p[lst][c], T_q[a][r] (shared memory only):
+  //   H1[u][a][a2'] = sum_{z2' at q: a = a2'} x' G[u,b(z2')][a][c(z2')] = sum_r T_q[a2'][r] G[u,y(r)][a][c(r)]        (adjoint of Z1)
+  //   H2[v][c1][c'] = sum_{z1 at p: c = c1} x G[b(z1),v][a(z1)][c']     = sum_lst T_p[lst][c1] G[x(lst),v][a(lst)][c']  (adjoint of Z2)
+  //   H[c1][a2']    = sum_lst T_p[lst][c1] H1[x(lst)][a(lst)][a2']                                                    (adjoint of XE)
+  {
+    const int nLp_ = t.loff[p + 1] - t.loff[p], nRq_ = t.roff[q + 1] - t.roff[q], Lp0_ = t.loff[p], Rq0_ = t.roff[q];
+    for (int e = tid; e < 8 * MS2; e += OT) {
+      const int which = e / (4 * MS2), r = e % (4 * MS2);
+      const int uv = r / MS2, x1 = (r % MS2) / MS, x2 = r % MS;
+      double v = 0.0;
+      if (has_loop) {
+        if (which == 0) {
+          for (int rr = 0; rr < nRq_; ++rr) v += TRq[x2 * MR + rr] * go[(uv * 4 + sRy[0][rr]) * MS2 + x1 * MS + sRc[0][rr]];
+        } else {
+          for (int lst = 0; lst < nLp_; ++lst) v += TLp[lst * MS + x1] * go[(sLx[2][lst] * 4 + uv) * MS2 + sLa[2][lst] * MS + x2];
+        }
       }
-    h[e] = v;
-  }
-  // H1[u][a][a2'] = sum_{z2' at q: a = a2'} x' G[u,b(z2')][a][c(z2')]   (adjoint of Z1);  H2[v][c1][c'] = sum_{z1 at p: c = c1} x G[b(z1),v][a(z1)][c']
-  for (int e = tid; e < 8 * MS2; e += OT) {
-    const int which = e / (4 * MS2), r = e % (4 * MS2);
-    const int uv = r / MS2, x1 = (r % MS2) / MS, x2 = r % MS;
-    double v = 0.0;
-    if (has_loop) {
-      if (which == 0) {
-        for (int z2p = t.opstart[q]; z2p < t.opstart[q + 1]; ++z2p)
-          if (t.op_a[z2p] == x2) v += t.op_x[z2p] * go[(uv * 4 + t.op_b[z2p]) * MS2 + x1 * MS + t.op_c[z2p]];
-      } else {
-        for (int z1 = t.opstart[p]; z1 < t.opstart[p + 1]; ++z1)
-          if (t.op_c[z1] == x1) v += t.op_x[z1] * go[(t.op_b[z1] * 4 + uv) * MS2 + t.op_a[z1] * MS + x2];
-      }
+      (which == 0 ? h1 : h2)[r] = v;
     }
-    (which == 0 ? h1 : h2)[r] = v;
+    __syncthreads();
+    for (int e = tid; e < MS2; e += OT) {
+      const int c1 = e / MS, a2p = e % MS;
+      double v = 0.0;
+      if (has_loop)
+        for (int lst = 0; lst < nLp_; ++lst) v += TLp[lst * MS + c1] * h1[(sLx[2][lst] * MS + sLa[2][lst]) * MS + a2p];
+      h[e] = v;
+    }
   }
   __syncthreads();
 
+    // hand the cell over to PART 1
+    for (int e = tid; e < ML * MR; e += OT) { scr_ab[e] = e < npair ? ab[(e / nR) * nR + e % nR] : 0.0; scr_ddb[e] = ddb[e]; }
+    for (int e = tid; e < 16 * MS2; e += OT) scr_go[e] = go[e];
+    for (int e = tid; e < 4 * MS2; e += OT) { scr_h1[e] = h1[e]; scr_h2[e] = h2[e]; }
+    for (int e = tid; e < MS2; e += OT) scr_ibsum[e] = ibsum[e];
+    for (int e = tid; e < nps * MS2; e += OT) scr_sbb[e] = sbb[e];
+    if (tid == 0) scr_flag[0] = anyp ? 1.0 : 0.0;
+  }
   OTICK(3);
   // ---- 4: this cell as closing pair ---------------------------------------------------------------------------------------------------------
   const int Sp1 = t.sig[p + 1], Sq = t.sig[q];  // bonds after i+1 / before j-1: XE, H are Sp1 x Sq
   const int nLp = t.loff[p + 1] - t.loff[p], nRq = t.roff[q + 1] - t.roff[q];
   const int Lp0 = t.loff[p], Rq0 = t.roff[q];
+  double* xa = A.XA + ((size_t)(d % XRING) * n + i) * XU * MS2;
+  double* xb = A.XB + ((size_t)(d % XRING) * n + i) * XU * MS2;
+  if constexpr (PART == 0) {
   // 4a hairpin interior E(p+1,q-1): its adjoint is w_H(d-1) H (single writer: plain store into the transposed table)
   {
     const double wh = t.wh[d - 1];
@@ -531,11 +633,9 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
   }
   // 4b adjoint row / column recursions of the interior-loop bodies (u = 4..30):
   //      XA_u(i,j) = w_In(u) H + Tbar_{i+1}^T XA_{u+1}(i-1,j)          XB_u(i,j) = w_In(u) H + XB_{u+1}(i,j+1) Tbar_{j-1}^T
-  double* xa = A.XA + ((size_t)(d & 1) * n + i) * XU * MS2;
-  double* xb = A.XB + ((size_t)(d & 1) * n + i) * XU * MS2;
   {
-    const double* xa1 = i >= 1 ? A.XA + ((size_t)((d + 1) & 1) * n + (i - 1)) * XU * MS2 : nullptr;
-    const double* xb1 = j + 1 <= n - 1 ? A.XB + ((size_t)((d + 1) & 1) * n + i) * XU * MS2 : nullptr;
+    const double* xa1 = i >= 1 ? A.XA + ((size_t)((d + 1) % XRING) * n + (i - 1)) * XU * MS2 : nullptr;
+    const double* xb1 = j + 1 <= n - 1 ? A.XB + ((size_t)((d + 1) % XRING) * n + i) * XU * MS2 : nullptr;
     for (int e = tid; e < XU * MS2; e += OT) {
       const int u4 = e / MS2, cz = (e % MS2) / MS, aw = e % MS, u = u4 + 4;
       double va = 0.0, vb = 0.0;
@@ -558,6 +658,9 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     }
   }
   __syncthreads();
+    OTICK(4);
+    return;
+  }
   OTICK(4);
   // 4c pushes of the generic interior loops (l1, l2 >= 2).  All terms of X_u(i,j) have the inner span d-2-u.
   if (MI >= 4) {
@@ -598,6 +701,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       }
   }
   OTICK(5);
+  if (!anyp) return;  // no nucleotide of i pairs with one of j: G = H = 0, only the chains above pass through this cell
   // 4d pushes of the l1 = 1 / l2 = 1 / 1x1 interior loops
   if (MI >= 2) {
     // 1 x 1: inner pair (i+2, j-2), DD(p,q) enters Y with w_In(2)
@@ -605,7 +709,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       double* rdk = A.RD + ((size_t)((d - 4) % ORING) * n + (i + 2)) * RDS;
       for (int e = tid; e < nLp * nRq; e += OT) {
         const int lst = e / nRq, r = e % nRq;
-        rdk[lst * MR + r] += m.win[2] * go[(t.ls_x[Lp0 + lst] * 4 + t.rs_y[Rq0 + r]) * MS2 + t.ls_a[Lp0 + lst] * MS + t.rs_c[Rq0 + r]];
+        rdk[lst * MR + r] += m.win[2] * go[(sLx[2][lst] * 4 + sRy[0][r]) * MS2 + sLa[2][lst] * MS + sRc[0][r]];
       }
     }
     // l1 = 1, l2 = 2..lmax1: Z1[lst][c2] = sum_l2 w_In(1+l2) sum_u D1(p; l+2)[lst][u] E(l+2,q-1)[u][c2],  l = q - l2; inner pair (i+2, l)
@@ -618,7 +722,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       if (e < e1) {
         const int l2 = 2 + e / (nLp * MS), lst = (e / MS) % nLp, u = e % MS, l = q - l2;
         if (u >= sigB(l + 2)) continue;
-        const double* hz = h1 + (t.ls_x[Lp0 + lst] * MS + t.ls_a[Lp0 + lst]) * MS;  // Z1-bar[lst][c2] = H1[x(lst)][a(lst)][c2]
+        const double* hz = h1 + (sLx[2][lst] * MS + sLa[2][lst]) * MS;  // Z1-bar[lst][c2] = H1[x(lst)][a(lst)][c2]
         double v = 0.0;
         for (int c2 = 0; c2 < Sq; ++c2) v += hz[c2] * EB(l + 2, q - 1, u, c2);
         double* rdk = A.RD + ((size_t)((l - (i + 2)) % ORING) * n + (i + 2)) * RDS + ML * MR + MS2;  // AD1[lst][u] of cell (i+2, l)
@@ -626,7 +730,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
       } else if (e < e2) {
         const int f = e - e1, l1 = 2 + f / (nRq * MS), r = (f / MS) % nRq, s_ = f % MS, k = p + l1;
         if (s_ >= sigA(k - 1)) continue;
-        const double* hz = h2 + (t.rs_y[Rq0 + r] * MS) * MS + t.rs_c[Rq0 + r];  // Z2-bar[a2][r] = H2[y(r)][a2][c(r)]
+        const double* hz = h2 + (sRy[0][r] * MS) * MS + sRc[0][r];  // Z2-bar[a2][r] = H2[y(r)][a2][c(r)]
         double v = 0.0;
         for (int a2 = 0; a2 < Sp1; ++a2) v += EA(p + 1, k - 2, a2, s_) * hz[a2 * MS];
         double* rdk = A.RD + ((size_t)(((j - 2) - k) % ORING) * n + k) * RDS + ML * MR + MS2 + ML * MS;  // AD2[r][s] of cell (k, j-2)
@@ -637,7 +741,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
         if (l2 == 2 || u >= sigB(l + 2) || c2 >= Sq) continue;
         double v = 0.0;
         for (int lst = 0; lst < nLp; ++lst)
-          v += b.D1[(size_t)(Lp0 + lst) * S + offB(l + 2) + u] * h1[(t.ls_x[Lp0 + lst] * MS + t.ls_a[Lp0 + lst]) * MS + c2];
+          v += b.D1[(size_t)(Lp0 + lst) * S + offB(l + 2) + u] * h1[(sLx[2][lst] * MS + sLa[2][lst]) * MS + c2];
         A.AES[(((size_t)AES_Z1R * n + (l + 2)) * SLEN + (l2 - 2)) * MS2 + u * MS + c2] += m.win[1 + l2] * v;
       } else {
         // E-bar(p+1, k-2)[a2][s] += w sum_r Z2-bar[a2][r] D2(k-1; q)[s][r]      (length l1 - 2 >= 1)
@@ -645,7 +749,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
         if (l1 == 2 || a2 >= Sp1 || s_ >= sigA(k - 1)) continue;
         double v = 0.0;
         for (int r = 0; r < nRq; ++r)
-          v += h2[(t.rs_y[Rq0 + r] * MS + a2) * MS + t.rs_c[Rq0 + r]] * b.D2T[(size_t)(Rq0 + r) * S + offA(k - 1) + s_];
+          v += h2[(sRy[0][r] * MS + a2) * MS + sRc[0][r]] * b.D2T[(size_t)(Rq0 + r) * S + offA(k - 1) + s_];
         A.AES[(((size_t)AES_Z2L * n + (p + 1)) * SLEN + (l1 - 2)) * MS2 + a2 * MS + s_] += m.win[l1 + 1] * v;
       }
     }
@@ -766,10 +870,10 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
     double v = bl[a1 * MS + c1] + br[a1 * MS + c1];
     for (int s2 = 0; s2 < nps; ++s2) v += m.wst[P][m.ptype[m.slot_x[s2] * 4 + m.slot_y[s2]]] * sb[s2 * MS2 + a1 * MS + c1];
     for (int lst = 0; lst < nLp; ++lst) {
-      if (t.ls_a[Lp0 + lst] != a1) continue;
-      const int u = t.ls_x[Lp0 + lst];
+      if (sLa[2][lst] != a1) continue;
+      const int u = sLx[2][lst];
       for (int r = 0; r < nRq; ++r)
-        if (t.rs_c[Rq0 + r] == c1) v += m.wtm[P][u][t.rs_y[Rq0 + r]] * y[lst * MR + r];
+        if (sRc[0][r] == c1) v += m.wtm[P][u][sRy[0][r]] * y[lst * MR + r];
     }
     inn[sl * MS2 + a1 * MS + c1] = v;
   }
@@ -805,7 +909,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
         double u = 0.0;
         if (has_loop) {
           for (int r = 0; r < nRq; ++r)
-            u += go[(u_ * 4 + t.rs_y[Rq0 + r]) * MS2 + a1 * MS + t.rs_c[Rq0 + r]] * z2[cz * MR + r];
+            u += go[(u_ * 4 + sRy[0][r]) * MS2 + a1 * MS + sRc[0][r]] * z2[cz * MR + r];
           for (int aw = 0; aw < Sq; ++aw) u += xe[cz * MS + aw] * h1[(u_ * MS + a1) * MS + aw];
         }
         A.U[(size_t)ROLE_CL * no + z1_] += t.op_x[z1_] * u;
@@ -816,7 +920,7 @@ __global__ void __launch_bounds__(OT) ocell_kernel(const Ctx* ctx, Adj A, int d,
         if (has_loop) {
           for (int cz = 0; cz < Sp1; ++cz) u += xe[cz * MS + aw] * h2[(v_ * MS + cz) * MS + c1];
           for (int lst = 0; lst < nLp; ++lst)
-            u += go[(t.ls_x[Lp0 + lst] * 4 + v_) * MS2 + t.ls_a[Lp0 + lst] * MS + c1] * z1[lst * MS + aw];
+            u += go[(sLx[2][lst] * 4 + v_) * MS2 + sLa[2][lst] * MS + c1] * z1[lst * MS + aw];
         }
         A.U[(size_t)ROLE_CR * no + z2_] += t.op_x[z2_] * u;
       } else if (e < ni + nj + 2 * np_ + nq) {
@@ -876,8 +980,10 @@ size_t cdz_outside_carve(const cdz_tt* tt, void* base, Adj* out) {
   A.AB = take(LS * RS);
   A.AX = take((n + 1) * MS); A.AXB = take(S);
   A.IB = take((size_t)ORING * n * 16 * MS2);
+  A.IBS = take((size_t)ORING * n * MS2);
   A.RD = take((size_t)ORING * n * (ML * MR + MS2 + ML * MS + MR * MS));
-  A.XA = take(2 * n * XU * MS2); A.XB = take(2 * n * XU * MS2);
+  A.XA = take((size_t)XRING * n * XU * MS2); A.XB = take((size_t)XRING * n * XU * MS2);
+  A.SC = take((size_t)SRING * n * scr_size((int)MS, (int)ML, (int)MR, 16));
   A.AES = take((size_t)AES_NROLE * n * SLEN * MS2);
   A.U = take((size_t)NROLE * nops);
   A.status = (int*)take(8);
@@ -896,8 +1002,72 @@ int cdz_launch_outside(cdz_tables* t, const Adj& A, size_t ws_bytes, double* bpp
   oext_kernel<<<1, 1024, 0, st>>>(t->d_ctx, A);
   const OPlan pl = oplan(tt->MS, tt->maxL, tt->maxR, t->model->c.nps);
   const size_t smem = sizeof(double) * pl.total;
-  CDZ_CUDA(cudaFuncSetAttribute(ocell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  for (int d = n - 1; d >= 0; --d) ocell_kernel<<<(unsigned)(n - d), OT, smem, st>>>(t->d_ctx, A, d, want_usage, bpp_dev);
+  const bool small = tt->MS <= 4;  // compile-time bound of the bond dimension in the gathers: 4 (single-codon trains) or 8
+  auto k0 = small ? ocell_kernel<0, 4> : ocell_kernel<0, 8>;
+  auto k1 = small ? ocell_kernel<1, 4> : ocell_kernel<1, 8>;
+  CDZ_CUDA(cudaFuncSetAttribute(k0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  CDZ_CUDA(cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  // Two internal streams forked from the caller's: sA runs the chain (PART 0 of diagonal d needs PART 0 of d+1), sB the consumers
+  // (PART 1 of d needs PART 0 of d).  PART 0 of d waits for PART 1 of d+4: the pushes into the cells of diagonal d come from closing
+  // cells at least four diagonals above, and the scratch / X rings are reused with that period.
+  cudaStream_t sA = nullptr, sB = nullptr;
+  // the chain gets the higher priority: when PART 0 of diagonal d-1 and PART 1 of diagonal d become runnable together, the CTAs of the
+  // chain are placed first and the consumers fill the remaining slots
+  int prio_lo = 0, prio_hi = 0;
+  CDZ_CUDA(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+  CDZ_CUDA(cudaStreamCreateWithPriority(&sA, cudaStreamNonBlocking, prio_hi));
+  CDZ_CUDA(cudaStreamCreateWithPriority(&sB, cudaStreamNonBlocking, prio_lo));
+  const int mh1 = t->model->p.min_hairpin + 1;
+  {
+    cudaEvent_t fork;
+    CDZ_CUDA(cudaEventCreateWithFlags(&fork, cudaEventDisableTiming));
+    CDZ_CUDA(cudaEventRecord(fork, st));
+    CDZ_CUDA(cudaStreamWaitEvent(sA, fork, 0));
+    CDZ_CUDA(cudaStreamWaitEvent(sB, fork, 0));
+    cudaEventDestroy(fork);
+  }
+  std::vector<cudaEvent_t> evB(n, nullptr);
+  for (int d = n - 1; d >= 0; --d) {
+    if (d + 4 <= n - 1 && evB[d + 4]) {
+      CDZ_CUDA(cudaStreamWaitEvent(sA, evB[d + 4], 0));
+      cudaEventDestroy(evB[d + 4]);  // (released when it has completed)
+      evB[d + 4] = nullptr;
+    }
+    k0<<<(unsigned)(n - d), OT, smem, sA>>>(t->d_ctx, A, d, want_usage, bpp_dev);
+#ifdef CDZ_EXP_NO_PART1
+    if (false) {
+#else
+    if (d >= mh1) {
+#endif
+      cudaEvent_t evA;
+      CDZ_CUDA(cudaEventCreateWithFlags(&evA, cudaEventDisableTiming));
+      CDZ_CUDA(cudaEventRecord(evA, sA));
+      CDZ_CUDA(cudaStreamWaitEvent(sB, evA, 0));
+      cudaEventDestroy(evA);
+#ifdef CDZ_EXP_ONE_STREAM
+      k1<<<(unsigned)(n - d), OT, smem, sA>>>(t->d_ctx, A, d, want_usage, bpp_dev);
+#else
+      k1<<<(unsigned)(n - d), OT, smem, sB>>>(t->d_ctx, A, d, want_usage, bpp_dev);
+#endif
+      CDZ_CUDA(cudaEventCreateWithFlags(&evB[d], cudaEventDisableTiming));
+      CDZ_CUDA(cudaEventRecord(evB[d], sB));
+    }
+  }
+  for (cudaEvent_t e : evB)
+    if (e) cudaEventDestroy(e);
+  {
+    cudaEvent_t ja, jb;
+    CDZ_CUDA(cudaEventCreateWithFlags(&ja, cudaEventDisableTiming));
+    CDZ_CUDA(cudaEventCreateWithFlags(&jb, cudaEventDisableTiming));
+    CDZ_CUDA(cudaEventRecord(ja, sA));
+    CDZ_CUDA(cudaEventRecord(jb, sB));
+    CDZ_CUDA(cudaStreamWaitEvent(st, ja, 0));
+    CDZ_CUDA(cudaStreamWaitEvent(st, jb, 0));
+    cudaEventDestroy(ja);
+    cudaEventDestroy(jb);
+  }
+  cudaStreamDestroy(sA);  // (streams with pending work are released when it has drained)
+  cudaStreamDestroy(sB);
   CDZ_CUDA(cudaGetLastError());
 #ifdef CDZ_OTIMING
   {
@@ -906,8 +1076,13 @@ int cdz_launch_outside(cdz_tables* t, const Adj& A, size_t ws_bytes, double* bpp
     cudaMemcpyFromSymbol(h, g_otime, sizeof(h));
     fprintf(stderr, "ocell phase cycles (sum over CTAs): gathers %llu | Qb-bar %llu | IL/IR %llu | I,G,H %llu | 4a-b %llu | 4c %llu | 4d %llu | 4e %llu | 4f %llu | usages %llu\n",
             h[0], h[1], h[2], h[3], h[4], h[5], h[6], h[7], h[8], h[9]);
+    unsigned long long mx[16];
+    cudaMemcpyFromSymbol(mx, g_omax, sizeof(mx));
+    fprintf(stderr, "ocell phase cycles (max over CTAs):  gathers %llu | Qb-bar %llu | IL/IR %llu | I,G,H %llu | 4a-b %llu | 4c %llu | 4d %llu | 4e %llu | 4f %llu | usages %llu\n",
+            mx[0], mx[1], mx[2], mx[3], mx[4], mx[5], mx[6], mx[7], mx[8], mx[9]);
     unsigned long long z[16] = {0};
     cudaMemcpyToSymbol(g_otime, z, sizeof(z));
+    cudaMemcpyToSymbol(g_omax, z, sizeof(z));
   }
 #endif
   return cdz_launch_usage(t, A, bpp_dev, base_dev, codon_dev, st);
