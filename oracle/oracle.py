@@ -244,3 +244,49 @@ def seq_str(seq) -> str:
 
 def dot_bracket(pair) -> str:
     return "".join("." if p < 0 else ("(" if p > k else ")") for k, p in enumerate(pair))
+
+
+# ---- frequency matching, PAPER.md S4e (lines 751-771), Alg S4.6 "Naive iterative algorithm for frequency matching" -------------------
+GENETIC_CODE = ("KNKNTTTTRSRSIIMI" "QHQHPPPPRRRRLLLL" "EDEDAAAAGGGGVVVV" "*Y*YSSSS*CWCLFLF")  # codon index 16 b0 + 4 b1 + b2, A,C,G,U = 0..3
+
+
+def codon_marginals(tab: Tables) -> np.ndarray:
+    """p_k(c) of eq 2.7 / 4.3 only (orc_marginals with the pair and base outputs switched off)."""
+    codon = np.zeros((tab.n // 3, 64))
+    rc = lib().orc_marginals(tab.h, None, None, _dp(codon))
+    if rc != 0:
+        raise RuntimeError(f"orc_marginals rc={rc}")
+    return codon
+
+
+def target_frequencies(aa: str, logf_star) -> np.ndarray:
+    """b_* of Alg S4.6: "computed frequencies from U(psi) with applied multiplicative bonuses f_*" -- every residue picks a codon
+    with probability proportional to its bonus, accumulated over the residues."""
+    fs = np.exp(np.asarray(logf_star, dtype=np.float64))
+    b = np.zeros(64)
+    for a in aa:
+        cod = [c for c in range(64) if GENETIC_CODE[c] == a]
+        tot = sum(fs[c] for c in cod)
+        for c in cod:
+            b[c] += fs[c] / tot
+    return b
+
+
+def match_frequencies(model, aa: str, kind: int, logf_star, pair_logw=None, rtol: float = 2e-3, max_iter: int = 50, nthreads: int = 1):
+    """Alg S4.6 line by line (naive iteration, no acceleration).  The update follows the prose of S4e step 2 ("multiply the current
+    soft constraint bonus values by the ratio of desired frequencies divided by the achieved frequencies"): f <- f b_*/b; the update
+    line of the printed pseudo-code has the ratio the other way round.  Requested frequencies equal to zero
+    are left out (line 769).  Returns (log f, errors of the evaluated iterates)."""
+    bstar = target_frequencies(aa, logf_star)
+    act = bstar > 0
+    logf = np.array(logf_star, dtype=np.float64)
+    errs = []
+    for _ in range(max_iter):
+        tab = inside(model, TT.build(aa, kind, logf, pair_logw), nthreads)  # "Compute Q and free energy q_psi using bonuses f"
+        b = codon_marginals(tab).sum(0)                               # "accumulated codon ... frequencies from these marginal probabilities"
+        err = float(np.abs(np.log(b[act] / bstar[act])).max())        # "|| log(b / b_*) ||_inf"
+        errs.append(err)
+        if err < rtol:
+            break
+        logf[act] += np.log(bstar[act] / b[act])
+    return logf, np.array(errs)

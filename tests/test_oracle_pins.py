@@ -453,3 +453,22 @@ def test_per_position_codon_weights():
     tot = sum(math.exp(sum(cwp[k, c] for k, c in enumerate(ch))) for ch in itertools.product(*cods))
     assert abs(O.TT.build("RSLG", 0, cwp).logsum() - math.log(tot)) < 1e-12
     assert abs(O.TT.build("RSLG", 1, cwp).logsum() - math.log(tot)) < 1e-12
+
+
+# ---------------------------------------------------------------- frequency matching (Alg S4.6)
+def test_frequency_matching_fixed_point_vs_brute_force():
+    """O.match_frequencies (PAPER.md Alg S4.6) against what the algorithm is for: with the returned bonuses the accumulated codon
+    frequencies -- computed by explicit enumeration of every (sequence, structure), not by the routine's own marginals -- equal the
+    targets; the first iterate is off by far more than the tolerance (the pairing model does bias codon usage), and the error
+    of the naive iteration decreases."""
+    m = I.tm1_model()
+    rng = np.random.default_rng(3)
+    logf_star = rng.normal(0.0, 0.7, 64)
+    for aa, kind in (("RSLG", 0), ("LSR", 1)):
+        pw = I.tm1_pair_logw() if kind else None
+        logf, errs = O.match_frequencies(m, aa, kind, logf_star, pw, rtol=1e-8, max_iter=200)
+        assert errs[0] > 1e-3 and errs[-1] < 1e-8 and (np.diff(errs[3:]) < 0).all()  # (the first steps may overshoot)
+        bstar = O.target_frequencies(aa, logf_star)
+        bf = O.brute_force(m, O.TT.build(aa, kind, logf, pw), marginals=True)
+        np.testing.assert_allclose(bf["codon"].sum(0), bstar, atol=1e-7)
+        assert abs(bstar.sum() - len(aa)) < 1e-12
