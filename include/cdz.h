@@ -189,6 +189,18 @@ int cdz_marginals_status(cdz_tables* t);
 int cdz_eval_sequences(const cdz_model* m, const cdz_tt* design, int n, int J, const uint8_t* seq_host, int max_batch,
                        double* logZ_host, double* logW_host, double* unpaired_host, void* stream);
 
+/* ---- frequency matching (PAPER.md S4e lines 751-771, Alg S4.6) ---- */
+/* Finds per-codon bonuses f (log f = a codon_logw table for cdz_tt_build) such that the accumulated exact codon marginals of the design
+ * distribution, b[c] = sum_k p_k(c), match the target frequencies bstar[c] = sum_{k: c codes aa_k} fstar_c / sum_{c' codes aa_k} fstar_c'
+ * (the frequencies of the structure-free uniform distribution with bonuses fstar = exp(logf_star), as in Alg S4.6).  Fixed-point iteration
+ * f <- f bstar / b from f = fstar, stopped when || log(b / bstar) ||_inf < rtol (the paper uses 0.002) or after max_iter iterations; anderson != 0
+ * applies Anderson acceleration over the whole history (line 771).  Every iteration is cdz_tt_build + cdz_inside + cdz_marginals on
+ * the device.  logf_out[64]: final log-bonuses; err_history[max_iter] (may be NULL): the error of every evaluated iterate;
+ * n_iter_out: number of evaluated iterates.  pair_logw as in cdz_tt_build.  Blocking.  Not converged is not an error: check err_history. */
+int cdz_match_frequencies(const cdz_model* m, const char* aa, int L, int kind, const double* logf_star, const double* pair_logw,
+                          double rtol, int max_iter, int anderson, double* logf_out, double* err_history, int* n_iter_out,
+                          void* stream);
+
 /* ---- convenience: host buffers end to end (used for the e2e timing) -------- */
 /* Builds nothing: runs cdz_inside_rerun, samples J states and copies them to host buffers. */
 int cdz_run_host(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_host, int32_t* pair_host, double* logZ_host,

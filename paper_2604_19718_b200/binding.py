@@ -22,7 +22,7 @@ EXPORTS = [
     "cdz_tt_from_operators", "cdz_tt_destroy", "cdz_tt_length", "cdz_tt_describe", "cdz_workspace_bytes",
     "cdz_inside", "cdz_inside_batch", "cdz_inside_rerun", "cdz_inside_rerun_batch", "cdz_tables_logz",
     "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample",
-    "cdz_debug_set_rescale_start", "cdz_eval_sequences", "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
+    "cdz_debug_set_rescale_start", "cdz_eval_sequences", "cdz_match_frequencies", "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
 ]
 
 
@@ -99,6 +99,8 @@ def lib():
     L.cdz_marginals_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
     L.cdz_marginals_status.argtypes = [vp]
     L.cdz_eval_sequences.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, dp, dp, dp, vp]
+    L.cdz_match_frequencies.argtypes = [vp, C.c_char_p, C.c_int, C.c_int, dp, dp, C.c_double, C.c_int, C.c_int, dp, dp,
+                                        C.POINTER(C.c_int), vp]
     L.cdz_run_host.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, dp, vp]
     _lib = L
     return L
@@ -334,3 +336,15 @@ def eval_sequences(model: Model, design: TensorTrain | None, seqs, want_unpaired
     _check(lib().cdz_eval_sequences(model.h, design.h if design is not None else None, n, J,
                                     seqs.ctypes.data_as(C.c_void_p), max_batch, _dp(lz), _dp(lw), _dp(un), _stream_ptr(stream)))
     return lz, lw, un
+
+
+def match_frequencies(model: Model, aa: str, kind: int, logf_star, pair_logw=None, rtol=2e-3, max_iter=50, anderson=True, stream=None):
+    """cdz_match_frequencies (Alg S4.6): returns (logf [64], errors of the evaluated iterates)."""
+    fs = np.ascontiguousarray(logf_star, dtype=np.float64)
+    pw = np.ascontiguousarray(pair_logw, dtype=np.float64).reshape(-1) if pair_logw is not None else None
+    out = np.zeros(64)
+    errs = np.zeros(max_iter)
+    nit = C.c_int()
+    _check(lib().cdz_match_frequencies(model.h, aa.encode(), len(aa), kind, _dp(fs), _dp(pw), rtol, max_iter, 1 if anderson else 0,
+                                       _dp(out), _dp(errs), C.byref(nit), _stream_ptr(stream)))
+    return out, errs[:nit.value].copy()

@@ -248,6 +248,12 @@ static int tt_build(const char* aa, int L, int kind, const double* codon_logw, i
   return CDZ_OK;
 }
 
+int cdz_codons_of(char aa, int* out) {
+  const std::vector<int> v = codon_set(aa);
+  for (size_t k = 0; k < v.size(); ++k) out[k] = v[k];
+  return (int)v.size();
+}
+
 extern "C" int cdz_tt_build(const char* aa, int L, int kind, const double* codon_logw, const double* pair_logw,
                             cdz_tt** out) {
   return tt_build(aa, L, kind, codon_logw, 0, pair_logw, out);

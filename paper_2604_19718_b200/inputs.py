@@ -204,3 +204,25 @@ def design(config: int, item: int = 0, L: int | None = None) -> Design:
         seed=seed,
         n_samples=samples[config],
     )
+
+
+def closed_form_inputs(kind: str, n: int):
+    """Seeded inputs of the two large closed-form pins (tests/golden/make_golden.py closed, tests/test_gpu_parity.py):
+    'zero8'  : generic operator list of bond dimension 8 (16 boundary states per position), n nucleotides; with the zero-energy,
+               all-pairs model  Z = (sum_phi W(phi)) x S_30(n)  (BASELINE.json north_star "zero-energy closed forms");
+    'mettrp' : protein of n/3 residues drawn from {M, W} (one codon each: a fixed sequence), codon weights of seed 424242; with the NN
+               model  log Z = log Z_McCaskill(sequence) + sum of the codon log-weights (north_star "Met/Trp only")."""
+    if kind == "zero8":
+        ops = []
+        for i in range(n):
+            sa = 1 if i == 0 else 8
+            sc = 1 if i == n - 1 else 8
+            pos = []
+            for a in range(sa):
+                for b in (i % 4, (i + 1) % 4):
+                    pos.append((a, b, (a + 3 * b + i) % sc, 0.5 + 0.03 * ((3 * a + 5 * b + i) % 11)))
+            ops.append(pos)
+        return ops
+    g = SplitMix64(424242, TAG_PROTEIN)
+    aa = "".join("MW"[g.next() & 1] for _ in range(n // 3))
+    return aa, codon_logw(424242)

@@ -109,30 +109,6 @@ def do_marginals(cfgs):
         print("marginals", cfg, f"{time.time() - t0:.0f} s", flush=True)
 
 
-def closed_form_inputs(kind: str, n: int):
-    """Seeded inputs of the two large closed-form pins (shared with tests/test_gpu_parity.py, which imports this function):
-    'zero8'  : generic operator list of bond dimension 8 (16 boundary states per position), n nucleotides; with the zero-energy,
-               all-pairs model  Z = (sum_phi W(phi)) x S_30(n)  (BASELINE.json north_star "zero-energy closed forms");
-    'mettrp' : protein of n/3 residues drawn from {M, W} (one codon each: a fixed sequence), codon weights of seed 424242; with the NN
-               model  log Z = log Z_McCaskill(sequence) + sum of the codon log-weights (north_star "Met/Trp only")."""
-    from paper_2604_19718_b200 import inputs as I
-
-    if kind == "zero8":
-        ops = []
-        for i in range(n):
-            sa = 1 if i == 0 else 8
-            sc = 1 if i == n - 1 else 8
-            pos = []
-            for a in range(sa):
-                for b in (i % 4, (i + 1) % 4):
-                    pos.append((a, b, (a + 3 * b + i) % sc, 0.5 + 0.03 * ((3 * a + 5 * b + i) % 11)))
-            ops.append(pos)
-        return ops
-    g = I.SplitMix64(424242, I.TAG_PROTEIN)
-    aa = "".join("MW"[g.next() & 1] for _ in range(n // 3))
-    return aa, I.codon_logw(424242)
-
-
 def do_closed(sizes):
     """Expected log Z of the closed-form pins from oracle pieces that share nothing with the tensor recursion: orc_tt_logsum (eq 3.2)
     and the scalar fixed-sequence orc_mccaskill.  -> oracle_closed_forms.txt"""
@@ -150,12 +126,12 @@ def do_closed(sizes):
                 have[(f[0], int(f[1]))] = f[2:]
     for n in sizes:
         t0 = time.time()
-        ops = closed_form_inputs("zero8", n)
+        ops = I.closed_form_inputs("zero8", n)
         logw = O.TT.from_ops(ops).logsum()
         logs = O.mccaskill(I.zero_energy_model(), np.zeros(n, dtype=np.uint8))  # log S_30(n): any fixed sequence, all pairs allowed
         have[("zero8", n)] = [f"{logw + logs:.12f}", f"{logw:.12f}", f"{logs:.12f}", f"{time.time() - t0:.0f}"]
         t0 = time.time()
-        aa, cw = closed_form_inputs("mettrp", n)
+        aa, cw = I.closed_form_inputs("mettrp", n)
         cod = {"M": (0, 3, 2), "W": (3, 2, 2)}  # AUG, UGG
         seq = np.array([b for a in aa for b in cod[a]], dtype=np.uint8)
         logw = float(sum(cw[16 * cod[a][0] + 4 * cod[a][1] + cod[a][2]] for a in aa))

@@ -303,12 +303,7 @@ def test_closed_form_large(B, row):
     of the headline run, against a closed form.   mettrp: Met/Trp-only protein (one codon each) under the NN model: the design space
     is one sequence, log Z = scalar McCaskill + codon log-weights (north_star).  Expected values: tests/golden/oracle_closed_forms.txt
     (make_golden.py closed; oracle only)."""
-    import importlib.util
-
-    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(GOLD, "make_golden.py"))
-    mg = importlib.util.module_from_spec(spec)
-    spec.loader.exec_module(mg)  # input recipe only (the golden writer itself calls nothing but oracle/)
-    closed_form_inputs = mg.closed_form_inputs
+    closed_form_inputs = I.closed_form_inputs
 
     kind, n, want = row[0], int(row[1]), float(row[2])
     if kind == "zero8":
