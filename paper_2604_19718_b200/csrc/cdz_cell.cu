@@ -221,6 +221,9 @@ struct KArgs {
   Dims dm;
 };
 
+// FIX = 1: the dimensions of the single-codon tensor train of cdz_tt_build (bond dimension 4, 4 left / 6 right boundary states, 6 pair slots) as
+// compile-time constants, so that the small loops unroll and the item decoding folds; FIX = 0: run-time dimensions.
+template <int FIX>
 __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, KArgs ka) {
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ CModel cm;
@@ -231,7 +234,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   const DevTab& b = cx.tab;
   const int I = blockIdx.x, J = I + ka.D;
   if (J >= t.NB) return;
-  const Dims dm = ka.dm;
+  Dims dm = ka.dm;
+  if (FIX) { dm.M = 4; dm.ML = 4; dm.MR = 6; dm.nps = 6; dm.lgM = 2; dm.lgR = 3; dm.lgP = 3; dm.pc = dm.percell(); }
   const Plan pl = make_plan(ka.maxpos, ka.span, dm, ka.C);
   MetaWin rowm{(PosMeta*)(smraw + pl.o_rowm), 0, 0};
   MetaWin colm{(PosMeta*)(smraw + pl.o_colm), 0, 1};
@@ -928,7 +932,8 @@ int cdz_cell_config(cdz_tables* const* ts, int B, cdz_cell_cfg* cfg) {
   if (pl.total > budget) { cdz_set_error("cell kernel: shared-memory need exceeds 200 KB"); return CDZ_ENOMEM; }
   cfg->M = dm.M; cfg->ML = dm.ML; cfg->MR = dm.MR; cfg->nps = dm.nps;
   cfg->maxpos = maxpos; cfg->span = span; cfg->C = C; cfg->smem = pl.total;
-  CDZ_CUDA(cudaFuncSetAttribute(cell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.total));
+  CDZ_CUDA(cudaFuncSetAttribute(cell_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.total));
+  CDZ_CUDA(cudaFuncSetAttribute(cell_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.total));
   return CDZ_OK;
 }
 
@@ -938,5 +943,6 @@ void cdz_launch_cells(const Ctx* d_ctxs, int B, int nblk, int D, int nsplit, con
   ka.dm.M = cfg->M; ka.dm.ML = cfg->ML; ka.dm.MR = cfg->MR; ka.dm.nps = cfg->nps;
   ka.dm.lgM = clog2(cfg->M); ka.dm.lgR = clog2(cfg->MR); ka.dm.lgP = clog2(cfg->nps);
   ka.dm.pc = ka.dm.percell();
-  cell_kernel<<<dim3(nblk, B), CELL_THREADS, cfg->smem, st>>>(d_ctxs, ka);
+  if (cfg->M == 4 && cfg->ML == 4 && cfg->MR == 6 && cfg->nps == 6) cell_kernel<1><<<dim3(nblk, B), CELL_THREADS, cfg->smem, st>>>(d_ctxs, ka);
+  else cell_kernel<0><<<dim3(nblk, B), CELL_THREADS, cfg->smem, st>>>(d_ctxs, ka);
 }
