@@ -1351,3 +1351,647 @@ int orc_marginals(orc_tables* t, double* bpp, double* base, double* codon) {
       }
   return 0;
 }
+
+/* ------------------------------------------------------------------------- */
+/* Minimisation, eq 2.8 (line 102), S4d (lines 245-260), Alg S4.5     */
+/* (lines 706-749): the same recursion with every (+, x) of the SumProduct     */
+/* semiring replaced by (min, +) of the tropical semiring.                     */
+/*   f(z, s) = E(phi(z), s)/kT + sum_i -log x(z_i)    over operator paths z    */
+/*   (one operator per position, bonds matching) and structures s;             */
+/*   f_min = min f,  one minimiser returned.                                   */
+/* "The soft constraint bonus is returned as a free energy ... by taking the   */
+/* negative logarithm" (line 749).  Values in units of kT: f_min >= -log Z.    */
+/* ------------------------------------------------------------------------- */
+#define FINF (1.0e300L)
+typedef struct {
+  int n;
+  const orc_tt* tt;
+  const orc_model* m;
+  int* sig;
+  double beta;
+  real** Tc;  /* Tc[i][(a*4+x)*sig[i+1]+c] = min over operators (a,x,c) of -log x   */
+  real** Tm;  /* Tm[i][a*sig[i+1]+c]       = min over x                              */
+  real** E;   /* min-plus stretch products, index i*(n+1)+(j+1)                      */
+  real **fb, **fbs, **fm1, **fml, **fm2, **fm, **fext;
+} mfe_tab;
+
+static real rmin(real a, real b) { return a < b ? a : b; }
+static real* inf_alloc(size_t k) {
+  real* p = (real*)malloc(sizeof(real) * (k ? k : 1));
+  for (size_t q = 0; q < (k ? k : 1); ++q) p[q] = FINF;
+  return p;
+}
+static const real* mfeE(const mfe_tab* t, int i, int j) { return t->E[(size_t)i * (t->n + 1) + (j + 1)]; }
+
+/* Up(p,q)[a,u,v,c] = min T_p[a,u,.] + E(p+1,q-1) + T_q[.,v,c]  (p<q);  Up(p,p)[a,u,u,c] = T_p[a,u,c] */
+static void mfe_Up(const mfe_tab* t, int p, int q, real* out) {
+  int Sa = t->sig[p], Sc = t->sig[q + 1];
+  for (int k = 0; k < Sa * 16 * Sc; ++k) out[k] = FINF;
+  const orc_tt* tt = t->tt;
+  if (p == q) {
+    for (int z = tt->start[p]; z < tt->start[p + 1]; ++z) {
+      const orc_op* o = &tt->ops[z];
+      real* e = &out[((o->a * 4 + o->b) * 4 + o->b) * Sc + o->c];
+      *e = rmin(*e, -logl((real)o->x));
+    }
+    return;
+  }
+  const real* Em = mfeE(t, p + 1, q - 1);
+  int Sm = t->sig[q];
+  for (int z = tt->start[p]; z < tt->start[p + 1]; ++z)
+    for (int y = tt->start[q]; y < tt->start[q + 1]; ++y) {
+      const orc_op *o = &tt->ops[z], *r = &tt->ops[y];
+      real* e = &out[((o->a * 4 + o->b) * 4 + r->b) * Sc + r->c];
+      *e = rmin(*e, -logl((real)o->x) + Em[o->c * Sm + r->a] - logl((real)r->x));
+    }
+}
+
+/* one closed cell in the tropical semiring: SURVEY App. A.2 term by term, (+, x) -> (min, +) */
+static void mfe_fb(mfe_tab* t, int i, int j) {
+  const orc_model* m = t->m;
+  int n = t->n, d = j - i;
+  int Si = t->sig[i], Sj1 = t->sig[j + 1];
+  real* fb = t->fb[(size_t)i * n + j];
+  if (d < m->min_hairpin + 1) return;
+  real B = (real)t->beta;
+  int Sa = t->sig[i + 1], Sc = t->sig[j];
+  real* inner = inf_alloc((size_t)16 * Sa * Sc);
+#define INNER(x, y, a, c) inner[(((x) * 4 + (y)) * Sa + (a)) * Sc + (c)]
+  int maxS = 1;
+  for (int p = i; p <= j + 1; ++p) if (t->sig[p] > maxS) maxS = t->sig[p];
+  real* UpL = inf_alloc((size_t)maxS * 16 * maxS);
+  real* UpR = inf_alloc((size_t)maxS * 16 * maxS);
+  real* A1 = inf_alloc((size_t)maxS * 16 * 16 * maxS);
+  real* A2 = inf_alloc((size_t)maxS * 16 * maxS);
+  real* A3 = inf_alloc((size_t)maxS * 16 * maxS);
+  /* hairpin */
+  {
+    mfe_Up(t, i + 1, j - 1, UpL);
+    real gh = B * (real)hairpin_init(m, d - 1);
+    for (int x = 0; x < 4; ++x)
+      for (int y = 0; y < 4; ++y) {
+        if (!can_pair(m, x, y)) continue;
+        int P = ptype(x, y);
+        for (int a = 0; a < Sa; ++a)
+          for (int u = 0; u < 4; ++u)
+            for (int v = 0; v < 4; ++v)
+              for (int c = 0; c < Sc; ++c)
+                INNER(x, y, a, c) = rmin(INNER(x, y, a, c), gh + B * (real)m->tmm[P][u][v] + UpL[((a * 4 + u) * 4 + v) * Sc + c]);
+      }
+  }
+  for (int k = i + 1; k < j; ++k)
+    for (int l = j - 1; l > k; --l) {
+      int l1 = k - i - 1, l2 = j - l - 1;
+      if (l1 + l2 > m->max_interior) break;
+      if (l - k < m->min_hairpin + 1) continue;
+      const real* qin = t->fb[(size_t)k * n + l];
+      int Ss = t->sig[k], St = t->sig[l + 1];
+      if (l1 == 0 || l2 == 0) {
+        /* stack / bulges: weight by size (+ stack term for sizes 0 and 1), side stretch = min-plus E */
+        const real* El = l1 > 0 ? mfeE(t, i + 1, k - 1) : NULL;
+        const real* Er = l2 > 0 ? mfeE(t, l + 1, j - 1) : NULL;
+        for (int x = 0; x < 4; ++x)
+          for (int y = 0; y < 4; ++y) {
+            if (!can_pair(m, x, y)) continue;
+            for (int xp = 0; xp < 4; ++xp)
+              for (int yp = 0; yp < 4; ++yp) {
+                if (!can_pair(m, xp, yp)) continue;
+                real w = (l1 + l2 == 0) ? B * (real)m->stack[ptype(x, y)][ptype(xp, yp)]
+                                        : B * (real)(m->bulge_init[l1 + l2] + (l1 + l2 == 1 ? m->stack[ptype(x, y)][ptype(xp, yp)] : 0.0));
+                for (int a = 0; a < Sa; ++a)
+                  for (int c = 0; c < Sc; ++c) {
+                    real best = FINF;
+                    if (l1 == 0 && l2 == 0) best = qin[((a * 4 + xp) * 4 + yp) * St + c];
+                    else if (l2 == 0) { for (int s = 0; s < Ss; ++s) best = rmin(best, El[a * Ss + s] + qin[((s * 4 + xp) * 4 + yp) * St + c]); }
+                    else { for (int tt_ = 0; tt_ < St; ++tt_) best = rmin(best, qin[((a * 4 + xp) * 4 + yp) * St + tt_] + Er[tt_ * Sc + c]); }
+                    INNER(x, y, a, c) = rmin(INNER(x, y, a, c), w + best);
+                  }
+              }
+          }
+      } else {
+        /* generic interior loop, the four stages of compute_qb in (min, +) */
+        mfe_Up(t, i + 1, k - 1, UpL);
+        mfe_Up(t, l + 1, j - 1, UpR);
+        for (int q = 0; q < Sa * 16 * 16 * St; ++q) A1[q] = FINF;
+        for (int a = 0; a < Sa; ++a)
+          for (int u = 0; u < 4; ++u)
+            for (int up = 0; up < 4; ++up)
+              for (int s = 0; s < Ss; ++s) {
+                real w = UpL[((a * 4 + u) * 4 + up) * Ss + s];
+                if (w >= FINF) continue;
+                for (int xy = 0; xy < 16; ++xy)
+                  for (int tt_ = 0; tt_ < St; ++tt_) {
+                    real* e = &A1[((((a * 4 + u) * 4 + up) * 16) + xy) * St + tt_];
+                    *e = rmin(*e, w + qin[(s * 16 + xy) * St + tt_]);
+                  }
+              }
+        for (int q = 0; q < Sa * 16 * St; ++q) A2[q] = FINF;
+        for (int a = 0; a < Sa; ++a)
+          for (int u = 0; u < 4; ++u)
+            for (int up = 0; up < 4; ++up)
+              for (int xp = 0; xp < 4; ++xp)
+                for (int yp = 0; yp < 4; ++yp) {
+                  if (!can_pair(m, xp, yp)) continue;
+                  int Pin = ptype(yp, xp);
+                  for (int vp = 0; vp < 4; ++vp)
+                    for (int tt_ = 0; tt_ < St; ++tt_) {
+                      real* e = &A2[((a * 4 + u) * 4 + vp) * St + tt_];
+                      *e = rmin(*e, B * (real)m->tmm[Pin][vp][up] + A1[((((a * 4 + u) * 4 + up) * 16) + xp * 4 + yp) * St + tt_]);
+                    }
+                }
+        for (int q = 0; q < Sa * 16 * Sc; ++q) A3[q] = FINF;
+        for (int a = 0; a < Sa; ++a)
+          for (int u = 0; u < 4; ++u)
+            for (int vp = 0; vp < 4; ++vp)
+              for (int tt_ = 0; tt_ < St; ++tt_) {
+                real w = A2[((a * 4 + u) * 4 + vp) * St + tt_];
+                if (w >= FINF) continue;
+                for (int v = 0; v < 4; ++v)
+                  for (int c = 0; c < Sc; ++c) {
+                    real* e = &A3[((a * 4 + u) * 4 + v) * Sc + c];
+                    *e = rmin(*e, w + UpR[((tt_ * 4 + vp) * 4 + v) * Sc + c]);
+                  }
+              }
+        real gi = B * (real)m->interior_init[l1 + l2];
+        for (int x = 0; x < 4; ++x)
+          for (int y = 0; y < 4; ++y) {
+            if (!can_pair(m, x, y)) continue;
+            int P = ptype(x, y);
+            for (int a = 0; a < Sa; ++a)
+              for (int u = 0; u < 4; ++u)
+                for (int v = 0; v < 4; ++v)
+                  for (int c = 0; c < Sc; ++c)
+                    INNER(x, y, a, c) = rmin(INNER(x, y, a, c), gi + B * (real)m->tmm[P][u][v] + A3[((a * 4 + u) * 4 + v) * Sc + c]);
+          }
+      }
+    }
+  /* multiloop closure */
+  if (j - 1 >= i + 1) {
+    const real* m2 = t->fm2[(size_t)(i + 1) * n + (j - 1)];
+    real gac = B * (real)(m->ml_a + m->ml_c);
+    for (int x = 0; x < 4; ++x)
+      for (int y = 0; y < 4; ++y) {
+        if (!can_pair(m, x, y)) continue;
+        for (int a = 0; a < Sa; ++a)
+          for (int c = 0; c < Sc; ++c) INNER(x, y, a, c) = rmin(INNER(x, y, a, c), gac + m2[a * Sc + c]);
+      }
+  }
+  const real *Ti = t->Tc[i], *Tj = t->Tc[j];
+  for (int a = 0; a < Si; ++a)
+    for (int x = 0; x < 4; ++x)
+      for (int y = 0; y < 4; ++y) {
+        if (!can_pair(m, x, y)) continue;
+        for (int c = 0; c < Sj1; ++c) {
+          real s = FINF;
+          for (int ap = 0; ap < Sa; ++ap)
+            for (int cp = 0; cp < Sc; ++cp) s = rmin(s, Ti[(a * 4 + x) * Sa + ap] + Tj[(cp * 4 + y) * Sj1 + c] + INNER(x, y, ap, cp));
+          fb[((a * 4 + x) * 4 + y) * Sj1 + c] = s;
+        }
+      }
+#undef INNER
+  free(inner); free(UpL); free(UpR); free(A1); free(A2); free(A3);
+}
+
+static void mfe_cell(mfe_tab* t, int i, int j) {
+  const orc_model* m = t->m;
+  int n = t->n, Si = t->sig[i], Sj1 = t->sig[j + 1];
+  size_t ci = (size_t)i * n + j;
+  real B = (real)t->beta, gb = B * (real)m->ml_b, gc = B * (real)m->ml_c;
+  mfe_fb(t, i, j);
+  real *fb = t->fb[ci], *fbs = t->fbs[ci], *fm1 = t->fm1[ci], *fml = t->fml[ci], *fm2 = t->fm2[ci], *fm = t->fm[ci];
+  for (int a = 0; a < Si; ++a)
+    for (int xy = 0; xy < 16; ++xy)
+      for (int c = 0; c < Sj1; ++c) fbs[a * Sj1 + c] = rmin(fbs[a * Sj1 + c], fb[(a * 16 + xy) * Sj1 + c]);
+  for (int k = 0; k < Si * Sj1; ++k) fm1[k] = gc + fbs[k];
+  if (j - 1 >= i) {
+    const real* p = t->fm1[(size_t)i * n + (j - 1)];
+    int Sj = t->sig[j];
+    for (int a = 0; a < Si; ++a)
+      for (int s = 0; s < Sj; ++s)
+        for (int c = 0; c < Sj1; ++c) fm1[a * Sj1 + c] = rmin(fm1[a * Sj1 + c], gb + p[a * Sj + s] + t->Tm[j][s * Sj1 + c]);
+  }
+  for (int k = 0; k < Si * Sj1; ++k) fml[k] = fm1[k];
+  if (i + 1 <= j) {
+    const real* p = t->fml[(size_t)(i + 1) * n + j];
+    int Si1 = t->sig[i + 1];
+    for (int a = 0; a < Si; ++a)
+      for (int s = 0; s < Si1; ++s)
+        for (int c = 0; c < Sj1; ++c) fml[a * Sj1 + c] = rmin(fml[a * Sj1 + c], gb + t->Tm[i][a * Si1 + s] + p[s * Sj1 + c]);
+  }
+  for (int k = i + 1; k <= j; ++k) {
+    const real* A = t->fm[(size_t)i * n + (k - 1)];
+    const real* Bq = t->fm1[(size_t)k * n + j];
+    int Sk = t->sig[k];
+    for (int a = 0; a < Si; ++a)
+      for (int s = 0; s < Sk; ++s)
+        for (int c = 0; c < Sj1; ++c) fm2[a * Sj1 + c] = rmin(fm2[a * Sj1 + c], A[a * Sk + s] + Bq[s * Sj1 + c]);
+  }
+  for (int k = 0; k < Si * Sj1; ++k) fm[k] = rmin(fml[k], fm2[k]);
+}
+
+static mfe_tab* mfe_build(const orc_model* m, const orc_tt* tt) {
+  int n = tt->n;
+  mfe_tab* t = (mfe_tab*)calloc(1, sizeof(mfe_tab));
+  t->n = n; t->tt = tt; t->m = m; t->sig = tt->sigma;
+  t->beta = 1.0 / model_kT(m);
+  t->Tc = (real**)calloc(n, sizeof(real*));
+  t->Tm = (real**)calloc(n, sizeof(real*));
+  for (int i = 0; i < n; ++i) {
+    int Sa = t->sig[i], Sc = t->sig[i + 1];
+    t->Tc[i] = inf_alloc((size_t)Sa * 4 * Sc);
+    t->Tm[i] = inf_alloc((size_t)Sa * Sc);
+    for (int z = tt->start[i]; z < tt->start[i + 1]; ++z) {
+      const orc_op* o = &tt->ops[z];
+      real c = -logl((real)o->x);
+      real* e = &t->Tc[i][(o->a * 4 + o->b) * Sc + o->c];
+      *e = rmin(*e, c);
+      e = &t->Tm[i][o->a * Sc + o->c];
+      *e = rmin(*e, c);
+    }
+  }
+  t->E = (real**)calloc((size_t)(n + 1) * (n + 1), sizeof(real*));
+  for (int i = 0; i <= n; ++i) {
+    int Sa = t->sig[i];
+    real* id = inf_alloc((size_t)Sa * Sa);
+    for (int a = 0; a < Sa; ++a) id[a * Sa + a] = 0;
+    t->E[(size_t)i * (n + 1) + i] = id;
+    for (int j = i; j < n; ++j) {
+      int Sj = t->sig[j], Sj1 = t->sig[j + 1];
+      const real* prev = t->E[(size_t)i * (n + 1) + j];
+      real* e = inf_alloc((size_t)Sa * Sj1);
+      for (int a = 0; a < Sa; ++a)
+        for (int s = 0; s < Sj; ++s)
+          for (int c = 0; c < Sj1; ++c) e[a * Sj1 + c] = rmin(e[a * Sj1 + c], prev[a * Sj + s] + t->Tm[j][s * Sj1 + c]);
+      t->E[(size_t)i * (n + 1) + (j + 1)] = e;
+    }
+  }
+  size_t nn = (size_t)n * n;
+  real*** tabs[6] = {&t->fb, &t->fbs, &t->fm1, &t->fml, &t->fm2, &t->fm};
+  for (int w = 0; w < 6; ++w) *tabs[w] = (real**)calloc(nn, sizeof(real*));
+  for (int i = 0; i < n; ++i)
+    for (int j = i; j < n; ++j) {
+      size_t ci = (size_t)i * n + j, s2 = (size_t)t->sig[i] * t->sig[j + 1];
+      t->fb[ci] = inf_alloc(s2 * 16);
+      for (int w = 1; w < 6; ++w) (*tabs[w])[ci] = inf_alloc(s2);
+    }
+  for (int d = 0; d < n; ++d) {
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int i = 0; i < n - d; ++i) mfe_cell(t, i, i + d);
+  }
+  t->fext = (real**)calloc(n + 1, sizeof(real*));
+  t->fext[0] = inf_alloc(t->sig[0]);
+  t->fext[0][0] = 0;
+  for (int j = 0; j < n; ++j) {
+    int Sj = t->sig[j], Sj1 = t->sig[j + 1];
+    real* q = inf_alloc(Sj1);
+    for (int s = 0; s < Sj; ++s)
+      for (int c = 0; c < Sj1; ++c) q[c] = rmin(q[c], t->fext[j][s] + t->Tm[j][s * Sj1 + c]);
+    for (int k = 0; k <= j; ++k) {
+      const real* fbs = t->fbs[(size_t)k * n + j];
+      int Sk = t->sig[k];
+      for (int s = 0; s < Sk; ++s)
+        for (int c = 0; c < Sj1; ++c) q[c] = rmin(q[c], t->fext[k][s] + fbs[s * Sj1 + c]);
+    }
+    t->fext[j + 1] = q;
+  }
+  return t;
+}
+
+static void mfe_free(mfe_tab* t) {
+  int n = t->n;
+  for (int i = 0; i < n; ++i) { free(t->Tc[i]); free(t->Tm[i]); }
+  free(t->Tc); free(t->Tm);
+  for (size_t k = 0; k < (size_t)(n + 1) * (n + 1); ++k) free(t->E[k]);
+  free(t->E);
+  for (size_t k = 0; k < (size_t)n * n; ++k) { free(t->fb[k]); free(t->fbs[k]); free(t->fm1[k]); free(t->fml[k]); free(t->fm2[k]); free(t->fm[k]); }
+  free(t->fb); free(t->fbs); free(t->fm1); free(t->fml); free(t->fm2); free(t->fm);
+  for (int j = 0; j <= n; ++j) free(t->fext[j]);
+  free(t->fext);
+  free(t);
+}
+
+/* ---- argmin traceback: every decision recomputes its alternatives in the plain form and follows the smallest ------------------ */
+typedef struct { const mfe_tab* t; uint8_t* seq; int32_t* pair; } mfe_tb;
+static real opcost(const orc_op* o) { return -logl((real)o->x); }
+
+/* unpaired stretch p..q with end bonds (s, tend): operator by operator, smallest remaining cost */
+static void mfe_chain(mfe_tb* c, int p, int q, int s, int tend) {
+  const mfe_tab* t = c->t;
+  int cur = s;
+  for (int mp = p; mp <= q; ++mp) {
+    const real* Er = mfeE(t, mp + 1, q);
+    int Sq1 = t->sig[q + 1], best = -1;
+    real bv = FINF;
+    for (int z = t->tt->start[mp]; z < t->tt->start[mp + 1]; ++z) {
+      const orc_op* o = &t->tt->ops[z];
+      if (o->a != cur) continue;
+      real v = opcost(o) + Er[o->c * Sq1 + tend];
+      if (v < bv) { bv = v; best = z; }
+    }
+    c->seq[mp] = (uint8_t)t->tt->ops[best].b;
+    cur = t->tt->ops[best].c;
+  }
+}
+
+static void mfe_tb_fm(mfe_tb* c, int i, int j, int a, int cc);
+static void mfe_tb_fm1(mfe_tb* c, int i, int j, int a, int cc);
+
+static void mfe_tb_fb(mfe_tb* c, int i, int j, int a, int x, int y, int cc) {
+  const mfe_tab* t = c->t;
+  const orc_model* m = t->m;
+  const orc_tt* tt = t->tt;
+  int n = t->n, d = j - i, P = ptype(x, y);
+  real B = (real)t->beta;
+  c->seq[i] = (uint8_t)x; c->seq[j] = (uint8_t)y;
+  c->pair[i] = j; c->pair[j] = i;
+  /* best alternative: kind 0 hairpin (zp,zq) | 1 inner pair (k,l) with side operators | 2 multiloop (k,s) */
+  real bv = FINF;
+  int bk = -1, bzi = -1, bzj = -1, b1 = -1, b2 = -1, b3 = -1, b4 = -1, bkk = 0, bll = 0, bxp = 0, byp = 0, bs = 0, bt = 0;
+  for (int zi = tt->start[i]; zi < tt->start[i + 1]; ++zi)
+    for (int zj = tt->start[j]; zj < tt->start[j + 1]; ++zj) {
+      const orc_op *oi = &tt->ops[zi], *oj = &tt->ops[zj];
+      if (oi->a != a || oi->b != x || oj->b != y || oj->c != cc) continue;
+      real w0 = opcost(oi) + opcost(oj);
+      int ap = oi->c, cp = oj->a, p = i + 1, q = j - 1;
+      /* hairpin */
+      {
+        const real* Em = mfeE(t, p + 1, q - 1);
+        int Sm = t->sig[q];
+        real gh = B * (real)hairpin_init(m, d - 1);
+        for (int zp = tt->start[p]; zp < tt->start[p + 1]; ++zp)
+          for (int zq = tt->start[q]; zq < tt->start[q + 1]; ++zq) {
+            const orc_op *o = &tt->ops[zp], *r = &tt->ops[zq];
+            if (o->a != ap || r->c != cp) continue;
+            real v = w0 + gh + B * (real)m->tmm[P][o->b][r->b] + opcost(o) + Em[o->c * Sm + r->a] + opcost(r);
+            if (v < bv) { bv = v; bk = 0; bzi = zi; bzj = zj; b1 = zp; b2 = zq; }
+          }
+      }
+      /* one inner pair */
+      for (int k = i + 1; k < j; ++k)
+        for (int l = j - 1; l > k; --l) {
+          int l1 = k - i - 1, l2 = j - l - 1;
+          if (l1 + l2 > m->max_interior) break;
+          if (l - k < m->min_hairpin + 1) continue;
+          const real* qin = t->fb[(size_t)k * n + l];
+          int St = t->sig[l + 1];
+          /* left side: (z1 at i+1, z2 at k-1) -> (u, u', s, cost); right side: (z1' at l+1, z2' at j-1) -> (v', v, t, cost) */
+          int nl = l1 == 0 ? 1 : (l1 == 1 ? tt->start[i + 2] - tt->start[i + 1] : (tt->start[i + 2] - tt->start[i + 1]) * (tt->start[k] - tt->start[k - 1]));
+          int nr = l2 == 0 ? 1 : (l2 == 1 ? tt->start[j] - tt->start[j - 1] : (tt->start[l + 2] - tt->start[l + 1]) * (tt->start[j] - tt->start[j - 1]));
+          for (int la = 0; la < nl; ++la) {
+            int z1 = -1, z2 = -1, u = 0, up = 0, s = ap;
+            real wl = 0;
+            if (l1 == 1) {
+              z1 = tt->start[i + 1] + la;
+              const orc_op* o = &tt->ops[z1];
+              if (o->a != ap) continue;
+              u = up = o->b; s = o->c; wl = opcost(o);
+            } else if (l1 >= 2) {
+              int n2 = tt->start[k] - tt->start[k - 1];
+              z1 = tt->start[i + 1] + la / n2; z2 = tt->start[k - 1] + la % n2;
+              const orc_op *o = &tt->ops[z1], *r = &tt->ops[z2];
+              if (o->a != ap) continue;
+              u = o->b; up = r->b; s = r->c;
+              wl = opcost(o) + mfeE(t, i + 2, k - 2)[o->c * t->sig[k - 1] + r->a] + opcost(r);
+            }
+            if (wl >= FINF) continue;
+            for (int ra = 0; ra < nr; ++ra) {
+              int z3 = -1, z4 = -1, v = 0, vp = 0, tb = cp;
+              real wr = 0;
+              if (l2 == 1) {
+                z4 = tt->start[j - 1] + ra;
+                const orc_op* o = &tt->ops[z4];
+                if (o->c != cp) continue;
+                v = vp = o->b; tb = o->a; wr = opcost(o);
+              } else if (l2 >= 2) {
+                int n2 = tt->start[j] - tt->start[j - 1];
+                z3 = tt->start[l + 1] + ra / n2; z4 = tt->start[j - 1] + ra % n2;
+                const orc_op *o = &tt->ops[z3], *r = &tt->ops[z4];
+                if (r->c != cp) continue;
+                vp = o->b; v = r->b; tb = o->a;
+                wr = opcost(o) + mfeE(t, l + 2, j - 2)[o->c * t->sig[j - 1] + r->a] + opcost(r);
+              }
+              if (wr >= FINF) continue;
+              for (int xp = 0; xp < 4; ++xp)
+                for (int yp = 0; yp < 4; ++yp) {
+                  if (!can_pair(m, xp, yp)) continue;
+                  real e;
+                  if (l1 == 0 && l2 == 0) e = B * (real)m->stack[P][ptype(xp, yp)];
+                  else if (l1 == 0 || l2 == 0) e = B * (real)(m->bulge_init[l1 + l2] + (l1 + l2 == 1 ? m->stack[P][ptype(xp, yp)] : 0.0));
+                  else e = B * (real)(m->interior_init[l1 + l2] + m->tmm[P][u][v] + m->tmm[ptype(yp, xp)][vp][up]);
+                  real val = w0 + e + wl + wr + qin[((s * 4 + xp) * 4 + yp) * St + tb];
+                  if (val < bv) { bv = val; bk = 1; bzi = zi; bzj = zj; b1 = z1; b2 = z2; b3 = z3; b4 = z4; bkk = k; bll = l; bxp = xp; byp = yp; bs = s; bt = tb; }
+                }
+            }
+          }
+        }
+      /* multiloop */
+      for (int k = i + 2; k <= j - 1; ++k) {
+        const real* A = t->fm[(size_t)(i + 1) * n + (k - 1)];
+        const real* Bq = t->fm1[(size_t)k * n + (j - 1)];
+        int Sk = t->sig[k], Scq = t->sig[j];
+        for (int s = 0; s < Sk; ++s) {
+          real val = w0 + B * (real)(m->ml_a + m->ml_c) + A[ap * Sk + s] + Bq[s * Scq + cp];
+          if (val < bv) { bv = val; bk = 2; bzi = zi; bzj = zj; bkk = k; bs = s; }
+        }
+      }
+    }
+  const orc_op *oi = &tt->ops[bzi], *oj = &tt->ops[bzj];
+  int ap = oi->c, cp = oj->a;
+  if (bk == 0) {
+    const orc_op *o = &tt->ops[b1], *r = &tt->ops[b2];
+    c->seq[i + 1] = (uint8_t)o->b; c->seq[j - 1] = (uint8_t)r->b;
+    mfe_chain(c, i + 2, j - 2, o->c, r->a);
+  } else if (bk == 1) {
+    int k = bkk, l = bll, l1 = k - i - 1, l2 = j - l - 1;
+    if (l1 == 1) c->seq[i + 1] = (uint8_t)tt->ops[b1].b;
+    else if (l1 >= 2) {
+      c->seq[i + 1] = (uint8_t)tt->ops[b1].b; c->seq[k - 1] = (uint8_t)tt->ops[b2].b;
+      mfe_chain(c, i + 2, k - 2, tt->ops[b1].c, tt->ops[b2].a);
+    }
+    if (l2 == 1) c->seq[j - 1] = (uint8_t)tt->ops[b4].b;
+    else if (l2 >= 2) {
+      c->seq[l + 1] = (uint8_t)tt->ops[b3].b; c->seq[j - 1] = (uint8_t)tt->ops[b4].b;
+      mfe_chain(c, l + 2, j - 2, tt->ops[b3].c, tt->ops[b4].a);
+    }
+    mfe_tb_fb(c, k, l, bs, bxp, byp, bt);
+  } else {
+    mfe_tb_fm(c, i + 1, bkk - 1, ap, bs);
+    mfe_tb_fm1(c, bkk, j - 1, bs, cp);
+  }
+}
+
+static void mfe_tb_fml(mfe_tb* c, int i, int j, int a, int cc) {
+  const mfe_tab* t = c->t;
+  int n = t->n;
+  real gb = (real)t->beta * (real)t->m->ml_b;
+  for (;;) {  /* peel leading unpaired positions until the branch starts */
+    int Sj1 = t->sig[j + 1], best = -1;
+    real bv = t->fm1[(size_t)i * n + j][a * Sj1 + cc];
+    if (i + 1 <= j)
+      for (int z = t->tt->start[i]; z < t->tt->start[i + 1]; ++z) {
+        const orc_op* o = &t->tt->ops[z];
+        if (o->a != a) continue;
+        real v = gb + opcost(o) + t->fml[(size_t)(i + 1) * n + j][o->c * Sj1 + cc];
+        if (v < bv) { bv = v; best = z; }
+      }
+    if (best < 0) { mfe_tb_fm1(c, i, j, a, cc); return; }
+    c->seq[i] = (uint8_t)t->tt->ops[best].b;
+    a = t->tt->ops[best].c;
+    ++i;
+  }
+}
+
+static void mfe_tb_fm1(mfe_tb* c, int i, int j, int a, int cc) {
+  const mfe_tab* t = c->t;
+  int n = t->n;
+  real B = (real)t->beta, gb = B * (real)t->m->ml_b, gc = B * (real)t->m->ml_c;
+  for (;;) {  /* peel trailing unpaired positions until the closing pair of the branch */
+    int Sj1 = t->sig[j + 1], best = -1, bxy = -1;
+    real bv = FINF;
+    const real* fb = t->fb[(size_t)i * n + j];
+    for (int xy = 0; xy < 16; ++xy) {
+      real v = gc + fb[(a * 16 + xy) * Sj1 + cc];
+      if (v < bv) { bv = v; bxy = xy; }
+    }
+    if (j - 1 >= i)
+      for (int z = t->tt->start[j]; z < t->tt->start[j + 1]; ++z) {
+        const orc_op* o = &t->tt->ops[z];
+        if (o->c != cc) continue;
+        real v = gb + t->fm1[(size_t)i * n + (j - 1)][a * t->sig[j] + o->a] + opcost(o);
+        if (v < bv) { bv = v; best = z; }
+      }
+    if (best < 0) { mfe_tb_fb(c, i, j, a, bxy / 4, bxy % 4, cc); return; }
+    c->seq[j] = (uint8_t)t->tt->ops[best].b;
+    cc = t->tt->ops[best].a;
+    --j;
+  }
+}
+
+static void mfe_tb_fm(mfe_tb* c, int i, int j, int a, int cc) {
+  const mfe_tab* t = c->t;
+  int n = t->n, Sj1 = t->sig[j + 1], bk = -1, bs = 0;
+  real bv = t->fml[(size_t)i * n + j][a * Sj1 + cc];
+  for (int k = i + 1; k <= j; ++k) {
+    const real* A = t->fm[(size_t)i * n + (k - 1)];
+    const real* Bq = t->fm1[(size_t)k * n + j];
+    int Sk = t->sig[k];
+    for (int s = 0; s < Sk; ++s) {
+      real v = A[a * Sk + s] + Bq[s * Sj1 + cc];
+      if (v < bv) { bv = v; bk = k; bs = s; }
+    }
+  }
+  if (bk < 0) { mfe_tb_fml(c, i, j, a, cc); return; }
+  mfe_tb_fm(c, i, bk - 1, a, bs);
+  mfe_tb_fm1(c, bk, j, bs, cc);
+}
+
+/* f_min = min over operator paths and structures of E/kT - sum log x (eq 2.8), and one minimiser (seq, pair; either may be NULL) */
+int orc_mfe(const orc_model* m, const orc_tt* tt, int nthreads, double* fmin, uint8_t* seq, int32_t* pair) {
+#ifdef _OPENMP
+  if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+  (void)nthreads;
+#endif
+  mfe_tab* t = mfe_build(m, tt);
+  int n = t->n, cb = 0;
+  real best = FINF;
+  for (int c = 0; c < t->sig[n]; ++c)
+    if (t->fext[n][c] < best) { best = t->fext[n][c]; cb = c; }
+  if (fmin) *fmin = (double)best;
+  if (seq && pair) {
+    mfe_tb tb = {t, seq, pair};
+    for (int p = 0; p < n; ++p) { seq[p] = 255; pair[p] = -1; }
+    int j = n - 1;
+    while (j >= 0) {
+      int Sj1 = t->sig[j + 1], bz = -1, bk = -1, bs = 0, bxy = 0;
+      real bv = FINF;
+      for (int z = tt->start[j]; z < tt->start[j + 1]; ++z) {
+        const orc_op* o = &tt->ops[z];
+        if (o->c != cb) continue;
+        real v = t->fext[j][o->a] + opcost(o);
+        if (v < bv) { bv = v; bz = z; }
+      }
+      for (int k = 0; k <= j - (m->min_hairpin + 1); ++k) {
+        const real* fb = t->fb[(size_t)k * n + j];
+        for (int s = 0; s < t->sig[k]; ++s)
+          for (int xy = 0; xy < 16; ++xy) {
+            real v = t->fext[k][s] + fb[(s * 16 + xy) * Sj1 + cb];
+            if (v < bv) { bv = v; bz = -1; bk = k; bs = s; bxy = xy; }
+          }
+      }
+      if (bz >= 0) {
+        seq[j] = (uint8_t)tt->ops[bz].b;
+        cb = tt->ops[bz].a;
+        --j;
+      } else {
+        mfe_tb_fb(&tb, bk, j, bs, bxy / 4, bxy % 4, cb);
+        cb = bs;
+        j = bk - 1;
+      }
+    }
+  }
+  mfe_free(t);
+  return 0;
+}
+
+/* the definition: enumerate every operator path and every structure, keep the smallest f (tiny designs only) */
+typedef struct { const orc_model* m; const orc_tt* tt; int n; uint8_t* seq; int32_t* pair; int* stack; int sp; real cost; real best; double beta;
+                 uint8_t* bseq; int32_t* bpair; } bfm_ctx;
+static void bfm_structures(bfm_ctx* c, int i) {
+  int n = c->n;
+  if (i == n) {
+    int valid;
+    double E = orc_energy(c->m, n, c->seq, c->pair, &valid);
+    if (!valid) return;
+    real f = c->cost + (real)E * (real)c->beta;
+    if (f < c->best) {
+      c->best = f;
+      if (c->bseq) memcpy(c->bseq, c->seq, n);
+      if (c->bpair) memcpy(c->bpair, c->pair, sizeof(int32_t) * n);
+    }
+    return;
+  }
+  if (c->sp > 0 && c->stack[c->sp - 1] == i) { --c->sp; bfm_structures(c, i + 1); c->stack[c->sp++] = i; return; }
+  c->pair[i] = -1;
+  bfm_structures(c, i + 1);
+  int lim = c->sp > 0 ? c->stack[c->sp - 1] : n;
+  for (int j = i + c->m->min_hairpin + 1; j < lim; ++j) {
+    if (!can_pair(c->m, c->seq[i], c->seq[j])) continue;
+    c->pair[i] = j; c->pair[j] = i;
+    c->stack[c->sp++] = j;
+    bfm_structures(c, i + 1);
+    --c->sp;
+    c->pair[i] = -1; c->pair[j] = -1;
+  }
+}
+static void bfm_paths(bfm_ctx* c, int i, int bond, real cost) {
+  if (i == c->n) {
+    c->cost = cost;
+    for (int p = 0; p < c->n; ++p) c->pair[p] = -1;
+    c->sp = 0;
+    bfm_structures(c, 0);
+    return;
+  }
+  for (int z = c->tt->start[i]; z < c->tt->start[i + 1]; ++z) {
+    const orc_op* o = &c->tt->ops[z];
+    if (o->a != bond) continue;
+    c->seq[i] = (uint8_t)o->b;
+    bfm_paths(c, i + 1, o->c, cost - logl((real)o->x));
+  }
+}
+int orc_brute_force_min(const orc_model* m, const orc_tt* tt, double* fmin, uint8_t* seq, int32_t* pair) {
+  int n = tt->n;
+  bfm_ctx c;
+  memset(&c, 0, sizeof(c));
+  c.m = m; c.tt = tt; c.n = n;
+  c.seq = (uint8_t*)calloc(n, 1);
+  c.pair = (int32_t*)calloc(n, sizeof(int32_t));
+  c.stack = (int*)calloc(n + 1, sizeof(int));
+  c.beta = 1.0 / model_kT(m);
+  c.best = FINF;
+  c.bseq = seq; c.bpair = pair;
+  bfm_paths(&c, 0, 0, 0.0L);
+  if (fmin) *fmin = (double)c.best;
+  free(c.seq); free(c.pair); free(c.stack);
+  return 0;
+}

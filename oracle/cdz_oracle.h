@@ -90,6 +90,12 @@ double orc_uniform(uint64_t seed, uint64_t sample, uint64_t kind, uint64_t i, ui
  *      (O(n^2) passes: small designs only).  Pinned by the brute-force marginals (tests/test_oracle_pins.py). ---- */
 int orc_marginals(orc_tables* t, double* bpp /*[n*n]*/, double* base /*[n*4]*/, double* codon /*[L*64]*/);
 
+/* ---- minimisation, eq 2.8 (line 102), S4d (lines 245-260), Alg S4.5 (lines 706-749): the recursion in the tropical (min, +)
+ *      semiring.  f(z, s) = E(phi(z), s)/kT - sum_i log x(z_i) over operator paths z and structures s (units of kT, so
+ *      f_min >= -log Z); one minimiser is returned (seq / pair may be NULL).  orc_brute_force_min is the definition by enumeration. */
+int orc_mfe(const orc_model* m, const orc_tt* tt, int nthreads, double* fmin, uint8_t* seq /*[n]*/, int32_t* pair /*[n]*/);
+int orc_brute_force_min(const orc_model* m, const orc_tt* tt, double* fmin, uint8_t* seq, int32_t* pair);
+
 #ifdef __cplusplus
 }
 #endif

@@ -72,6 +72,8 @@ def lib():
         L.orc_uniform.argtypes = [C.c_uint64] * 5
         L.orc_uniform.restype = C.c_double
         L.orc_marginals.argtypes = [vp, dp, dp, dp]
+        L.orc_mfe.argtypes = [C.POINTER(OrcModel), vp, C.c_int, dp, u8p, i32p]
+        L.orc_brute_force_min.argtypes = [C.POINTER(OrcModel), vp, dp, u8p, i32p]
         _lib = L
     return _lib
 
@@ -290,3 +292,17 @@ def match_frequencies(model, aa: str, kind: int, logf_star, pair_logw=None, rtol
             break
         logf[act] += np.log(bstar[act] / b[act])
     return logf, np.array(errs)
+
+
+def mfe(model, tt: TT, nthreads: int = 0, brute: bool = False):
+    """orc_mfe / orc_brute_force_min: (f_min in units of kT, seq uint8 [n], pair int32 [n]) -- PAPER.md eq 2.8."""
+    m = make_model(model)
+    f = C.c_double()
+    seq = np.zeros(tt.n, dtype=np.uint8)
+    pair = np.zeros(tt.n, dtype=np.int32)
+    sp, pp = seq.ctypes.data_as(C.POINTER(C.c_uint8)), pair.ctypes.data_as(C.POINTER(C.c_int32))
+    if brute:
+        lib().orc_brute_force_min(C.byref(m), tt.h, C.byref(f), sp, pp)
+    else:
+        lib().orc_mfe(C.byref(m), tt.h, nthreads, C.byref(f), sp, pp)
+    return f.value, seq, pair

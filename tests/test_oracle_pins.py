@@ -472,3 +472,37 @@ def test_frequency_matching_fixed_point_vs_brute_force():
         bf = O.brute_force(m, O.TT.build(aa, kind, logf, pw), marginals=True)
         np.testing.assert_allclose(bf["codon"].sum(0), bstar, atol=1e-7)
         assert abs(bstar.sum() - len(aa)) < 1e-12
+
+
+# ---------------------------------------------------------------- minimisation (tropical semiring, eq 2.8)
+@pytest.mark.parametrize("aa,kind,cw,pw", [("MW", 0, 0, 0), ("LSR", 0, 1, 0), ("LSR", 1, 1, 1), ("RSLG", 0, 1, 0), ("GRL", 1, 1, 1),
+                                            ("MWFMWM", 0, 1, 0)])
+def test_mfe_equals_enumeration(aa, kind, cw, pw):
+    """orc_mfe (the recursion with (+, x) -> (min, +), PAPER.md S4d) against the definition: the smallest
+    f = E/kT - log W over every (operator path, structure) by explicit enumeration; the returned state attains it
+    (its own log-weight, evaluated by orc_logweight, equals -f_min); f_min >= -log Z."""
+    m = I.tm1_model()
+    m.ml_a = 0.4  # make multiloops competitive on these tiny designs
+    tt = build(aa, kind, cw, pw)
+    fb, sb, pb = O.mfe(m, tt, brute=True)
+    fd, sd, pd = O.mfe(m, tt)
+    assert abs(fd - fb) < 1e-12 * max(1.0, abs(fb))
+    assert abs(-O.logweight(m, tt, sd, pd) - fd) < 1e-12 * max(1.0, abs(fd))
+    assert abs(-O.logweight(m, tt, sb, pb) - fb) < 1e-12 * max(1.0, abs(fb))
+    assert fd >= -O.inside(m, tt).logZ - 1e-12
+
+
+def test_mfe_fixed_sequence_and_larger():
+    """Beyond enumeration: for a Met/Trp protein (one sequence) the minimiser's energy is that sequence's structure MFE and no
+    sampled structure of the same sequence lies below it; for a 13-aa design no sampled state lies below f_min."""
+    m = I.nn_model()
+    for aa, kind in (("MWMWMWMMWWMW", 0), (I.protein(1000, 13), 0), (I.protein(5000, 9), 1)):
+        d = I.design(1 if kind == 0 else 5, 0, len(aa))
+        tt = O.TT.build(aa, kind, d.codon_logw, d.pair_logw)
+        f, s, p = O.mfe(m, tt)
+        assert abs(-O.logweight(m, tt, s, p) - f) < 1e-11 * max(1.0, abs(f))
+        tab = O.inside(m, tt)
+        assert f >= -tab.logZ
+        seqs, pairs = tab.sample(200, 77)
+        lw = np.array([O.logweight(m, tt, seqs[k], pairs[k]) for k in range(200)])
+        assert (-lw >= f - 1e-10).all()
