@@ -189,6 +189,15 @@ int cdz_marginals_status(cdz_tables* t);
 int cdz_eval_sequences(const cdz_model* m, const cdz_tt* design, int n, int J, const uint8_t* seq_host, int max_batch,
                        double* logZ_host, double* logW_host, double* unpaired_host, void* stream);
 
+/* ---- minimisation (eq 2.8, S4d lines 245-260, Alg S4.5) ---- */
+/* The recursion in the tropical (min, +) semiring: fmin_host = min over operator paths z (one operator per position, bonds matching)
+ * and structures s of  f(z, s) = E(phi(z), s)/kT - sum_i log x(z_i)  (units of kT; fmin >= -log Z), and one minimiser:
+ * seq_dev [n] uint8 (0..3), pair_dev [n] int32 (partner or -1); both NULL to skip the traceback.  workspace_dev: a device buffer of
+ * >= cdz_workspace_bytes(tt, CDZ_FP64) bytes or NULL (library allocation); the tropical tables live in it during the call only.
+ * Blocking: returns after fmin_host has been written.  Ties between minimisers are broken by the enumeration order. */
+int cdz_mfe(const cdz_model* m, const cdz_tt* tt, void* workspace_dev, size_t workspace_bytes, void* stream, double* fmin_host,
+            uint8_t* seq_dev, int32_t* pair_dev);
+
 /* ---- frequency matching (PAPER.md S4e lines 751-771, Alg S4.6) ---- */
 /* Finds per-codon bonuses f (log f = a codon_logw table for cdz_tt_build) such that the accumulated exact codon marginals of the design
  * distribution, b[c] = sum_k p_k(c), match the target frequencies bstar[c] = sum_{k: c codes aa_k} fstar_c / sum_{c' codes aa_k} fstar_c'

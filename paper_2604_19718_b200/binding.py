@@ -22,7 +22,7 @@ EXPORTS = [
     "cdz_tt_from_operators", "cdz_tt_destroy", "cdz_tt_length", "cdz_tt_describe", "cdz_workspace_bytes",
     "cdz_inside", "cdz_inside_batch", "cdz_inside_rerun", "cdz_inside_rerun_batch", "cdz_tables_logz",
     "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample",
-    "cdz_debug_set_rescale_start", "cdz_eval_sequences", "cdz_match_frequencies", "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
+    "cdz_debug_set_rescale_start", "cdz_eval_sequences", "cdz_match_frequencies", "cdz_mfe", "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
 ]
 
 
@@ -101,6 +101,7 @@ def lib():
     L.cdz_eval_sequences.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, dp, dp, dp, vp]
     L.cdz_match_frequencies.argtypes = [vp, C.c_char_p, C.c_int, C.c_int, dp, dp, C.c_double, C.c_int, C.c_int, dp, dp,
                                         C.POINTER(C.c_int), vp]
+    L.cdz_mfe.argtypes = [vp, vp, vp, C.c_size_t, vp, dp, vp, vp]
     L.cdz_run_host.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, dp, vp]
     _lib = L
     return L
@@ -348,3 +349,16 @@ def match_frequencies(model: Model, aa: str, kind: int, logf_star, pair_logw=Non
     _check(lib().cdz_match_frequencies(model.h, aa.encode(), len(aa), kind, _dp(fs), _dp(pw), rtol, max_iter, 1 if anderson else 0,
                                        _dp(out), _dp(errs), C.byref(nit), _stream_ptr(stream)))
     return out, errs[:nit.value].copy()
+
+
+def mfe(model: Model, tt: TensorTrain, traceback=True, stream=None):
+    """cdz_mfe: (f_min in units of kT, seq uint8 [n] CUDA tensor or None, pair int32 [n] CUDA tensor or None) -- PAPER.md eq 2.8."""
+    import torch
+
+    ws = _alloc_workspace(tt, FP64)
+    f = C.c_double()
+    seq = torch.empty(tt.n, dtype=torch.uint8, device="cuda") if traceback else None
+    pair = torch.empty(tt.n, dtype=torch.int32, device="cuda") if traceback else None
+    _check(lib().cdz_mfe(model.h, tt.h, C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(stream), C.byref(f),
+                         C.c_void_p(seq.data_ptr()) if traceback else None, C.c_void_p(pair.data_ptr()) if traceback else None))
+    return f.value, seq, pair

@@ -513,6 +513,10 @@ static int make_tables(const cdz_model* m, const cdz_tt* tt, int precision, void
   return CDZ_OK;
 }
 
+int cdz_make_tables(const cdz_model* m, const cdz_tt* tt, int precision, void* ws, size_t ws_bytes, cudaStream_t st, cdz_tables** out) {
+  return make_tables(m, tt, precision, ws, ws_bytes, st, out);
+}
+
 extern "C" void cdz_tables_destroy(cdz_tables* t) {
   if (!t) return;
   if (t->owns_base && t->base) cudaFree(t->base);

@@ -39,26 +39,11 @@ __device__ unsigned long long g_otime[16], g_omax[16];
 namespace {
 
 constexpr int OT = 256;  // threads per CTA (512 measured slower: 0.33 vs 0.30 s at config 2)
-constexpr int NW = OT / 32;
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
-}
-
-// dot product of two contiguous row segments [k0,k1), lanes stride the range (coalesced), fixed order
-__device__ __forceinline__ double warp_dot(const double* __restrict__ x, const double* __restrict__ y, int k0, int k1, int lane) {
-  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-  int k = k0 + lane;
-  for (; k + 96 < k1; k += 128) {
-    a0 += x[k] * y[k];
-    a1 += x[k + 32] * y[k + 32];
-    a2 += x[k + 64] * y[k + 64];
-    a3 += x[k + 96] * y[k + 96];
-  }
-  for (; k < k1; k += 32) a0 += x[k] * y[k];
-  return warp_sum((a0 + a1) + (a2 + a3));
 }
 
 // All nx x ny dot products  out[a * ny + c] = sum_{kb in [k0,k1)} X[a * S + kb] Y[c * S + kb]  of two small groups of table rows at once: every
@@ -211,7 +196,7 @@ __global__ void __launch_bounds__(OT, 4) ocell_kernel(const Ctx* ctx, Adj A, int
   const DevTT& t = ctx->tt;
   const DevTab& b = ctx->tab;
   const CModel& m = *ctx->cm;
-  const int n = t.n, MS = t.MS, MS2 = MS * MS, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int n = t.n, MS = t.MS, MS2 = MS * MS, tid = threadIdx.x;
   const size_t S = (size_t)t.S, RS = (size_t)t.RS;
   const int ML = A.ML, MR = A.MR, nps = m.nps;
   const OPlan pl = oplan(MS, ML, MR, nps);
@@ -582,7 +567,7 @@ __global__ void __launch_bounds__(OT, 4) ocell_kernel(const Ctx* ctx, Adj A, int
   //   H2[v][c1][c'] = sum_{z1 at p: c = c1} x G[b(z1),v][a(z1)][c']     = sum_lst T_p[lst][c1] G[x(lst),v][a(lst)][c']  (adjoint of Z2)
   //   H[c1][a2']    = sum_lst T_p[lst][c1] H1[x(lst)][a(lst)][a2']                                                    (adjoint of XE)
   {
-    const int nLp_ = t.loff[p + 1] - t.loff[p], nRq_ = t.roff[q + 1] - t.roff[q], Lp0_ = t.loff[p], Rq0_ = t.roff[q];
+    const int nLp_ = t.loff[p + 1] - t.loff[p], nRq_ = t.roff[q + 1] - t.roff[q];
     for (int e = tid; e < 8 * MS2; e += OT) {
       const int which = e / (4 * MS2), r = e % (4 * MS2);
       const int uv = r / MS2, x1 = (r % MS2) / MS, x2 = r % MS;
