@@ -109,7 +109,7 @@ def test_invalid_inputs_are_rejected(B):
         B.Model(bad)
     tt = B.TensorTrain.build("MW", 0)
     with pytest.raises(B.CdzError):
-        B.inside(B.Model(I.nn_model()), tt, precision=B.FP32_SCALED)  # declared, not built
+        B.inside(B.Model(I.nn_model()), tt, precision=7)  # unknown precision code
 
 
 @pytest.mark.parametrize("aa,kind", [("RSLG", 0), ("LSR", 1)])
