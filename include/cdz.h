@@ -158,6 +158,18 @@ int cdz_tables_logqext(cdz_tables* t, int j, int c, double* out_host);
  * pair_dev [J][n] int32 partner or -1.  Uniforms are U(seed, sample, kind, i, j). */
 int cdz_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* pair_dev, void* stream);
 
+/* cdz_sample for callers that must not allocate device memory (CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): same arguments, same kernel, bit-identical samples for the same (tables, J, seed).  The traceback stacks, the
+ * only scratch of the sampler (n/4 + 16 items of 20 bytes per sample), live in a static device array of
+ * CDZ_NOALLOC_STACK_ITEMS items (8.0 MB) that every GPU loading the library holds until the process exits, instead of a
+ * stream-ordered allocation.  The call makes no cudaMalloc / cudaFree / cudaMallocAsync and creates no events.
+ * Limit: J * (n/4 + 16) <= CDZ_NOALLOC_STACK_ITEMS (J <= 106 at n = 15000, J <= 3125 at n = 450); CDZ_EINVAL with a message
+ * beyond it (use cdz_sample).  All calls on one GPU share the array: calls that overlap on the GPU (two streams, two host
+ * threads) race; serialise them.  The array keeps the previous call's contents and needs no clearing (every item is written
+ * before it is read).  Asynchronous on `stream`; seq_dev / pair_dev are caller-owned as in cdz_sample. */
+#define CDZ_NOALLOC_STACK_ITEMS 400000
+int cdz_sample_noalloc(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* pair_dev, void* stream);
+
 /* ---- marginals (device) ---------------------------------------------------- */
 /* Outside (adjoint) pass over the tables of a finished inside pass: the paper's ComputeReverse (Alg S4.3) as the
  * reverse-mode adjoint of the recursion.  Asynchronous on `stream` (it waits for the inside pass by an event

@@ -16,12 +16,13 @@ LIB_PATH = os.path.join(_HERE, "libcdz.so")
 
 TT_SINGLE_CODON, TT_CODON_PAIR = 0, 1
 FP64, FP32_SCALED = 0, 1
+NOALLOC_STACK_ITEMS = 400000  # CDZ_NOALLOC_STACK_ITEMS of include/cdz.h (limit of cdz_sample_noalloc)
 
 EXPORTS = [
     "cdz_last_error", "cdz_version", "cdz_model_create", "cdz_model_destroy", "cdz_tt_build", "cdz_tt_build_pos",
     "cdz_tt_from_operators", "cdz_tt_destroy", "cdz_tt_length", "cdz_tt_describe", "cdz_workspace_bytes",
     "cdz_inside", "cdz_inside_batch", "cdz_inside_rerun", "cdz_inside_rerun_batch", "cdz_tables_logz",
-    "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample",
+    "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample", "cdz_sample_noalloc",
     "cdz_debug_set_rescale_start", "cdz_eval_sequences", "cdz_match_frequencies", "cdz_mfe", "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
 ]
 
@@ -95,6 +96,7 @@ def lib():
     L.cdz_tables_cell.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
     L.cdz_tables_logqext.argtypes = [vp, C.c_int, C.c_int, dp]
     L.cdz_sample.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, vp]
+    L.cdz_sample_noalloc.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, vp]
     L.cdz_marginals.argtypes = [vp, vp, C.c_size_t, vp, vp, vp, vp]
     L.cdz_marginals_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
     L.cdz_marginals_status.argtypes = [vp]
@@ -250,6 +252,11 @@ class Tables:
         _check(lib().cdz_sample(self.h, J, seed, C.c_void_p(seq.data_ptr()), C.c_void_p(pair.data_ptr()),
                                 _stream_ptr(stream)))
         return seq, pair
+
+    def sample_noalloc(self, J: int, seed: int, seq, pair, stream=None):
+        """cdz_sample_noalloc: writes into the caller's CUDA tensors seq uint8 [J,n] and pair int32 [J,n]; allocates nothing."""
+        _check(lib().cdz_sample_noalloc(self.h, J, seed, C.c_void_p(seq.data_ptr()), C.c_void_p(pair.data_ptr()),
+                                        _stream_ptr(stream)))
 
     def marginals(self, stream=None, bpp=True, base=True, codon=True, own_workspace=True):
         """cdz_marginals: (bpp [n][n], base [n][4], codon [L][64]) as CUDA tensors (None where not requested), by the outside pass.

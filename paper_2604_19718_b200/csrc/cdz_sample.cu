@@ -6,6 +6,9 @@
 // uniform.  Lanes evaluate 32 alternatives at a time (shuffle prefix scan), cheapest / likeliest segments first,
 // and stop at the first hit, so the expensive interior-loop alternatives are only evaluated when needed.
 #include <math.h>
+#include <stdio.h>
+
+#include <mutex>
 
 #include "cdz_internal.h"
 
@@ -591,5 +594,59 @@ int cdz_launch_sample(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int
   mark(7);
   CDZ_CUDA(cudaGetLastError());
   CDZ_CUDA(cudaFreeAsync(stacks, st));
+  return CDZ_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// cdz_sample_noalloc: the same traceback for callers that cannot allocate device memory (CUDA graph capture, serving loops,
+// harnesses that forbid cudaMalloc).  The per-sample decision stacks -- the only scratch sample_kernel needs -- live in a
+// file-scope device array instead of a stream-ordered allocation.  Every GPU that loads the library holds the array
+// (CDZ_NOALLOC_STACK_ITEMS x 20 bytes = 8.0 MB) until the process exits; every call on a device shares it, so calls that overlap
+// on one GPU race.  Nothing in it has to start at zero: a warp pushes an item before it pops it.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) Item g_noalloc_stacks[CDZ_NOALLOC_STACK_ITEMS];
+
+namespace {
+constexpr int NOALLOC_MAX_DEV = 64;
+Item* g_noalloc_ptr[NOALLOC_MAX_DEV];  // device address of g_noalloc_stacks, per device (the symbol itself is only a host-side stand-in)
+std::mutex g_noalloc_mu;
+}  // namespace
+
+extern "C" int cdz_sample_noalloc(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_dev, int32_t* pair_dev, void* stream) {
+  static_assert(sizeof(Item) == 20, "cdz.h documents 20 bytes per stack item");
+  if (!t || J < 0 || !seq_dev || !pair_dev) { cdz_set_error("cdz_sample_noalloc: bad argument"); return CDZ_EINVAL; }
+  if (!t->done) { cdz_set_error("cdz_sample_noalloc before cdz_inside"); return CDZ_ESTATE; }
+  if (J == 0) return CDZ_OK;
+  const int cap = t->tt->n / 4 + 16;  // stack depth per sample, as in cdz_sample
+  if ((long long)cap * J > (long long)CDZ_NOALLOC_STACK_ITEMS) {
+    char msg[256];
+    snprintf(msg, sizeof(msg), "cdz_sample_noalloc: J x (n/4 + 16) = %d x %d stack items exceed the static scratch of %d items (J <= %d at n = %d); "
+             "use cdz_sample", J, cap, CDZ_NOALLOC_STACK_ITEMS, CDZ_NOALLOC_STACK_ITEMS / cap, t->tt->n);
+    cdz_set_error(msg);
+    return CDZ_EINVAL;
+  }
+  int dev = -1;
+  CDZ_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEV) { cdz_set_error("cdz_sample_noalloc: device ordinal beyond 63"); return CDZ_EINVAL; }
+  Item* stacks = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {  // once per device, with that device current
+      void* p = nullptr;
+      if (cudaGetSymbolAddress(&p, g_noalloc_stacks) != cudaSuccess || !p) {
+        cudaGetLastError();
+        cdz_set_error("cdz_sample_noalloc: cudaGetSymbolAddress of the static scratch failed");
+        return CDZ_ECUDA;
+      }
+      g_noalloc_ptr[dev] = (Item*)p;
+    }
+    stacks = g_noalloc_ptr[dev];
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  const int rc = cdz_wait_pass(t, st);
+  if (rc != CDZ_OK) return rc;
+  const int wpb = 4;
+  sample_kernel<<<(J + wpb - 1) / wpb, wpb * 32, 0, st>>>(t->d_ctx, J, seed, seq_dev, pair_dev, stacks, cap);
+  CDZ_CUDA(cudaGetLastError());
   return CDZ_OK;
 }
