@@ -33,6 +33,28 @@ def O():
     return oracle
 
 
+_ORACLE_TABLES = {}
+
+
+def oracle_design(O, cfg, L):
+    """Oracle inside pass of a BASELINE design prefix under the NN model; computed once per process for the sizes several tests share
+    (the long-double recursion dominates the run time of this file)."""
+    key = (cfg, L)
+    if key in _ORACLE_TABLES:
+        return _ORACLE_TABLES[key]
+    d = I.design(cfg, 0, L)
+    to = O.inside(I.nn_model(), O.TT.build(d.aa, d.kind, d.codon_logw, d.pair_logw))
+    if d.n <= 300:
+        _ORACLE_TABLES[key] = to
+    return to
+
+
+def both_design(B, O, cfg, L):
+    d = I.design(cfg, 0, L)
+    tg, lz = B.inside(B.Model(I.nn_model()), B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw))
+    return oracle_design(O, cfg, L), tg, lz
+
+
 def both(B, O, model, aa, kind, cw, pw):
     tto = O.TT.build(aa, kind, cw, pw)
     ttg = B.TensorTrain.build(aa, kind, cw, pw)
@@ -54,9 +76,8 @@ def test_logz_appendix_b(B, O, row):
 @pytest.mark.parametrize("cfg,L", [(1, 20), (2, 20), (5, 10), (5, 40), (2, 45), (1, 67), (1, 200), (2, 100)])
 def test_logz_and_tables_vs_oracle(B, O, cfg, L):
     """Every stored cell (Qb, Qbs, Qm1, Qml, M2, Qm) of every (i,j) agrees with the oracle."""
-    m = I.nn_model()
     d = I.design(cfg, 0, L)
-    to, tg, lz = both(B, O, m, d.aa, d.kind, d.codon_logw, d.pair_logw)
+    to, tg, lz = both_design(B, O, cfg, L)
     assert abs(lz - to.logZ) <= LOGZ_RTOL * abs(to.logZ)
     n = d.n
     rng = np.random.default_rng(0)
@@ -107,7 +128,7 @@ def test_samples_bit_exact(B, O, cfg, L, J):
     """Same seed, same decision uniforms -> identical (sequence, structure) as the oracle traceback."""
     m = I.nn_model()
     d = I.design(cfg, 0, L)
-    to, tg, lz = both(B, O, m, d.aa, d.kind, d.codon_logw, d.pair_logw)
+    to, tg, lz = both_design(B, O, cfg, L)
     so, po = to.sample(J, d.sample_seed)
     sg, pg = tg.sample(J, d.sample_seed)
     sg, pg = sg.cpu().numpy(), pg.cpu().numpy()
@@ -349,7 +370,7 @@ def test_fp32_scaled_vs_oracle_and_fp64(B, O, cfg, L):
     assert abs(lz32 - lz64) <= FP32_RTOL * abs(lz64)
     assert t32.info()["precision"] == B.FP32_SCALED
     if d.n <= 300:
-        lo = O.inside(m, O.TT.build(d.aa, d.kind, d.codon_logw, d.pair_logw)).logZ
+        lo = oracle_design(O, cfg, L).logZ
         assert abs(lz32 - lo) <= FP32_RTOL * abs(lo)
     stored = {(int(r[0]), int(r[2])): float(r[4]) for r in _stored_oracle_rows()}
     if (cfg, L) in stored:
