@@ -226,3 +226,54 @@ def closed_form_inputs(kind: str, n: int):
     g = SplitMix64(424242, TAG_PROTEIN)
     aa = "".join("MW"[g.next() & 1] for _ in range(n // 3))
     return aa, codon_logw(424242)
+
+
+TAG_TENSOR_MODEL = 5
+
+
+@dataclass
+class TensorModel:
+    """Parameters of the paper's tensor-based free-energy model (PAPER.md S2b lines 430-437; chi of eq 3.6): V[x] for an
+    unpaired base x, B[x][y][rho] for the 5' side of a pair with 5' base x and 3' base y (B[y][x][rho] is its 3' side), S of the
+    weighted trace Tr_S[X] = Tr[S X], gamma = model dimension, xi = number of pair conformations."""
+
+    gamma: int
+    xi: int
+    V: np.ndarray          # [4][gamma][gamma]
+    B: np.ndarray          # [4][4][xi][gamma][gamma], zero where x.y cannot pair
+    S: np.ndarray          # [gamma][gamma]
+    min_hairpin: int = 3   # PAPER.md line 483: B_{i,j} = 0 for |j - i| < 4
+
+
+def tensor_model(gamma: int, xi: int, seed: int = 19718, unit: bool = False) -> TensorModel:
+    """Synthetic non-negative parameters (the fitted parameters of ref [15] are not in the container): entries ~ U(0,1) scaled so
+    that an unpaired step has row sums near 1 (the renormalisation of S3a, line 499, in spirit) and a canonical pair carries a
+    weight of order e^{1..2}; ``unit`` = all-ones model of dimension 1 in which every two bases may pair (Z = number of sequences x number of structures)."""
+    can = {(0, 3), (3, 0), (1, 2), (2, 1), (2, 3), (3, 2)}  # AU UA CG GC GU UG
+    V = np.zeros((4, gamma, gamma))
+    B = np.zeros((4, 4, xi, gamma, gamma))
+    S = np.zeros((gamma, gamma))
+    if unit:
+        assert gamma == 1 and xi == 1
+        V[:] = 1.0
+        S[:] = 1.0
+        B[:] = 1.0  # every two bases may pair: the structure counts S(n) of tests/golden/structure_counts.txt apply
+        return TensorModel(gamma, xi, V, B, S)
+    g = SplitMix64(seed, TAG_TENSOR_MODEL)
+    for x in range(4):
+        for a in range(gamma):
+            for b in range(gamma):
+                V[x, a, b] = (0.2 + g.uniform()) / (0.7 * gamma)
+    strength = {(1, 2): 2.2, (2, 1): 2.2, (0, 3): 1.5, (3, 0): 1.5, (2, 3): 1.0, (3, 2): 1.0}
+    for x in range(4):
+        for y in range(4):
+            for r in range(xi):
+                for a in range(gamma):
+                    for b in range(gamma):
+                        u = g.uniform()
+                        if (x, y) in can:
+                            B[x, y, r, a, b] = strength[(x, y)] * (0.2 + u) / gamma
+    for a in range(gamma):
+        for b in range(gamma):
+            S[a, b] = (1.0 if a == b else 0.0) + 0.15 * g.uniform()
+    return TensorModel(gamma, xi, V, B, S)
