@@ -222,6 +222,45 @@ int cdz_match_frequencies(const cdz_model* m, const char* aa, int L, int kind, c
                           double rtol, int max_iter, int anderson, double* logf_out, double* err_history, int* n_iter_out,
                           void* stream);
 
+/* ---- the paper's tensor-based free-energy model (PAPER.md S2b lines 430-437; eqs 3.5-3.8; Alg S4.1 / S4.2 lines 586-622) ---- */
+/* Parameters (host pointers, read during the call only): gamma = model dimension (<= 8), xi = number of pair conformations (<= 4),
+ *   V [4][gamma][gamma]           matrix of an unpaired base x (eq 3.6, second case),
+ *   B [4][4][xi][gamma][gamma]    B[x][y][rho] = tensor of the 5' side of a pair with 5' base x and 3' base y ("B_{i,j}^rho"); B[y][x][rho] is the
+ *                                 tensor of its 3' side ("B_{j,i}^rho"); all-zero B[x][y] = x.y cannot pair,
+ *   S [gamma][gamma]              weighted trace Tr_S[X] = Tr[S X] (line 178),
+ * min_hairpin: a pair k.l needs l - k - 1 >= min_hairpin (line 483: 3).  All entries finite and >= 0.  Limits of this version:
+ * gamma x (largest bond dimension of tt) <= 32 and (number of pairable (x,y)) x xi x bond^2 <= 512; CDZ_EINVAL beyond. */
+typedef struct {
+  int32_t gamma, xi, min_hairpin;
+  const double* V;
+  const double* B;
+  const double* S;
+} cdz_tm_params;
+typedef struct {
+  double device_ms;        /* device time of the full-size pass (CUDA events on `stream`: table clear, all block diagonals, final trace) */
+  double gemm_flop;        /* FLOP of the tensor-core tiles: 2 x 64^3 x (number of K blocks), padding included */
+  double table_bytes;      /* the two S x S tables */
+  int64_t launches;
+  int32_t S, NB;           /* flattened (block-padded) dimension sum_i gamma Sigma_i and its number of 64-blocks */
+  int32_t scale_exponent;  /* e: every operator weight was multiplied by 2^-e; log Z = log Z_stored + e n ln 2 */
+} cdz_tm_info;
+/* log Z = -q_psi (eq 2.4 line 72) of the design distribution under the tensor model: the sum over every operator path (coding sequence,
+ * weights included) of `tt` and every unpseudoknotted structure of the state's tensor diagram (eq S2.1), by the recursion
+ *   Q_{i,j} = sum_{k in [i:j)} Q_{i,k} Q_{j,k}^T (i < j),  Q_{j,k} = chi-hat_{k,j}(Q_{k+1,j-1}) (j > k),  Z = sum_{sigma_n} Tr_S[Q_{0,n}]
+ * run as a block wavefront with fp64 tensor-core tiles (csrc/cdz_tm.cu).  Open chain as in cdz_tt_build.  workspace_dev: a device
+ * buffer of >= cdz_tm_workspace_bytes bytes (it then holds the tables after the call: cdz_tm_block) or NULL (allocated and freed
+ * inside).  Blocking: returns after logZ_host has been written.  info may be NULL.  CDZ_EOVERFLOW if Z leaves the fp64 range in the
+ * stored scale (one uniform power-of-two scale per position, measured by a pilot pass over the first 60 positions). */
+int cdz_tm_workspace_bytes(const cdz_tm_params* p, const cdz_tt* tt, size_t* bytes);
+int cdz_tm_inside(const cdz_tm_params* p, const cdz_tt* tt, void* workspace_dev, size_t workspace_bytes, void* stream, double* logZ_host,
+                  cdz_tm_info* info);
+/* Debug / parity access to the tables a cdz_tm_inside call left in a caller workspace (same p, tt; scale_exponent from its info):
+ * which = 0: the upper block Q_{i,j}, 0 <= i <= j <= n, as [gamma Sigma_i][gamma Sigma_j]; which = 1: the lower block Q_{j,i}, i < j, as
+ * [gamma Sigma_j][gamma Sigma_i] (index (sigma, zeta) -> sigma gamma + zeta, line 211).  true value = out x 2^shift_out.  Returns the
+ * element count. */
+int cdz_tm_block(const cdz_tm_params* p, const cdz_tt* tt, const void* workspace_dev, int scale_exponent, int which, int i, int j,
+                 double* out_host, int* shift_out);
+
 /* ---- convenience: host buffers end to end (used for the e2e timing) -------- */
 /* Builds nothing: runs cdz_inside_rerun, samples J states and copies them to host buffers. */
 int cdz_run_host(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_host, int32_t* pair_host, double* logZ_host,

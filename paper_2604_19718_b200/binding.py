@@ -24,6 +24,7 @@ EXPORTS = [
     "cdz_inside", "cdz_inside_batch", "cdz_inside_rerun", "cdz_inside_rerun_batch", "cdz_tables_logz",
     "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample", "cdz_sample_noalloc",
     "cdz_debug_set_rescale_start", "cdz_eval_sequences", "cdz_match_frequencies", "cdz_mfe", "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
+    "cdz_tm_workspace_bytes", "cdz_tm_inside", "cdz_tm_block",
 ]
 
 
@@ -54,6 +55,16 @@ class Info(C.Structure):
         ("split_mac", C.c_double), ("table_bytes", C.c_double), ("bytes_per_cell", C.c_double),
         ("log_scale", C.c_double), ("inside_ms", C.c_double),
     ]
+
+
+class TMParams(C.Structure):
+    _fields_ = [("gamma", C.c_int32), ("xi", C.c_int32), ("min_hairpin", C.c_int32),
+                ("V", C.POINTER(C.c_double)), ("B", C.POINTER(C.c_double)), ("S", C.POINTER(C.c_double))]
+
+
+class TMInfo(C.Structure):
+    _fields_ = [("device_ms", C.c_double), ("gemm_flop", C.c_double), ("table_bytes", C.c_double), ("launches", C.c_int64),
+                ("S", C.c_int32), ("NB", C.c_int32), ("scale_exponent", C.c_int32)]
 
 
 _lib = None
@@ -105,6 +116,9 @@ def lib():
                                         C.POINTER(C.c_int), vp]
     L.cdz_mfe.argtypes = [vp, vp, vp, C.c_size_t, vp, dp, vp, vp]
     L.cdz_run_host.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, dp, vp]
+    L.cdz_tm_workspace_bytes.argtypes = [C.POINTER(TMParams), vp, C.POINTER(C.c_size_t)]
+    L.cdz_tm_inside.argtypes = [C.POINTER(TMParams), vp, vp, C.c_size_t, vp, dp, C.POINTER(TMInfo)]
+    L.cdz_tm_block.argtypes = [C.POINTER(TMParams), vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
     _lib = L
     return L
 
@@ -369,3 +383,39 @@ def mfe(model: Model, tt: TensorTrain, traceback=True, stream=None):
     _check(lib().cdz_mfe(model.h, tt.h, C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(stream), C.byref(f),
                          C.c_void_p(seq.data_ptr()) if traceback else None, C.c_void_p(pair.data_ptr()) if traceback else None))
     return f.value, seq, pair
+
+
+class TensorModelPass:
+    """cdz_tm_inside: the paper's tensor-model recursion (eqs 3.5-3.8) over a tensor train; keeps the workspace so that blocks can be read back."""
+
+    def __init__(self, tm, tt: TensorTrain, stream=None):
+        import torch
+
+        self._V = np.ascontiguousarray(tm.V, dtype=np.float64)
+        self._B = np.ascontiguousarray(tm.B, dtype=np.float64)
+        self._S = np.ascontiguousarray(tm.S, dtype=np.float64)
+        self.p = TMParams(int(tm.gamma), int(tm.xi), int(tm.min_hairpin), _dp(self._V), _dp(self._B), _dp(self._S))
+        self.tt = tt
+        nb = C.c_size_t()
+        _check(lib().cdz_tm_workspace_bytes(C.byref(self.p), tt.h, C.byref(nb)))
+        self.ws = torch.empty(nb.value, dtype=torch.uint8, device="cuda")
+        self.info = TMInfo()
+        lz = C.c_double()
+        _check(lib().cdz_tm_inside(C.byref(self.p), tt.h, C.c_void_p(self.ws.data_ptr()), nb.value, _stream_ptr(stream), C.byref(lz),
+                                   C.byref(self.info)))
+        self.logZ = lz.value
+
+    def rerun(self, stream=None):
+        lz = C.c_double()
+        _check(lib().cdz_tm_inside(C.byref(self.p), self.tt.h, C.c_void_p(self.ws.data_ptr()), self.ws.numel(), _stream_ptr(stream),
+                                   C.byref(lz), C.byref(self.info)))
+        self.logZ = lz.value
+        return lz.value
+
+    def block(self, which: int, i: int, j: int):
+        """(values as stored, shift): true block = values * 2**shift.  which 0: Q_{i,j} upper, 1: Q_{j,i} lower."""
+        out = np.zeros(32 * 32)
+        sh = C.c_int()
+        cnt = _check(lib().cdz_tm_block(C.byref(self.p), self.tt.h, C.c_void_p(self.ws.data_ptr()), self.info.scale_exponent, which, i, j,
+                                        _dp(out), C.byref(sh)))
+        return out[:cnt].copy(), sh.value

@@ -10,8 +10,8 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 OUT = os.path.join(HERE, "libcdz.so")
 OUT_PEAK = os.path.join(HERE, "libcdz_peak.so")
-SOURCES = ["cdz_host.cu", "cdz_inside.cu", "cdz_cell.cu", "cdz_gemm.cu", "cdz_outside.cu", "cdz_usage.cu", "cdz_sample.cu",
-           "cdz_eval.cu", "cdz_freq.cu", "cdz_mfe.cu"]
+SOURCES = ["cdz_host.cu", "cdz_inside.cu", "cdz_cell.cu", "cdz_outside.cu", "cdz_usage.cu", "cdz_sample.cu",
+           "cdz_eval.cu", "cdz_freq.cu", "cdz_mfe.cu", "cdz_tm.cu"]
 PEAK_SOURCES = ["cdz_peak.cu"]  # not part of the product ABI: register-resident issue-rate loops for bench.py's roofline
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -1,0 +1,420 @@
+// cdz_tm.cu -- the paper's OWN recursion on the CUDA path: partition function of the tensor-based free-energy model with a
+// codon tensor train, summed over every coding sequence and every unpseudoknotted structure (eqs 3.5-3.8,
+// Alg S4.1 / S4.2 lines 586-622).
+//
+//   Q_{i,j} = sum_{k in [i:j)} Q_{i,k} Q_{j,k}^T   (i < j; eq 3.5),      Q_{j,k} = chi-hat_{k,j}(Q_{k+1,j-1})   (j > k; eqs 3.6 / 3.8)
+//
+// over boundary points 0..n; a block Q_{i,j} is a (gamma Sigma_i) x (gamma Sigma_j) matrix, index (sigma, zeta) -> sigma * gamma + zeta
+// (line 211).  The paper evaluates the first line as one TRMM per row on the GPU (eq S4.1) and chi-hat on CPU cores (line 282);
+// a row-wise TRMM re-reads the whole triangle for every row (HBM-bound).  Here both lines run on the GPU as a BLOCK WAVEFRONT: the boundary
+// points are grouped into blocks of <= 64 flattened indices, block diagonals D = J - I are swept in order, and on each one
+//   tm_gemm_kernel   U[I,J] partial = sum_{I<K<J} U[I,K] CT[J,K]^T over the finished blocks: fp64 DMMA tiles (cdz_gemm.cuh), split-K;
+//   tm_block_kernel  one CTA per block walks the in-block anti-diagonals: (A) the closed elements chi-hat of the step's cells, one warp per
+//                    cell, contracted through the dense tensor-train cores in three small stages; (B) U(i,j) = GEMM partial + the two
+//                    in-block edge ranges of the k-sum as dot products of contiguous rows.
+// Tables: U[(i,a)][(j,b)] = Q_{i,j} (upper, identity on the diagonal blocks) and CT[(j,d)][(k,a)] = Q_{j,k} (the lower blocks as printed),
+// both S x S row-major over the block-padded flattened index space, so the k-sum of a cell is a dot product of two contiguous rows.
+// Scaling: every term of every Q_{i,j} contains exactly one operator of each position i..j-1, so all operator weights are multiplied by
+// 2^-e (exact) and log Z = log Z_stored + e n ln 2; e is the growth rate measured by a pilot pass over the first <= 60 positions.
+// Readings: DESIGN.md section 17 (the same as oracle/tensor_model.py states in its header; the two share no code).
+#include <math.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "cdz_gemm.cuh"
+#include "cdz_internal.h"
+
+namespace {
+
+constexpr int TM_MAXG = 8;        // gamma
+constexpr int TM_MAXXI = 4;       // xi
+constexpr int TM_MAXM = 32;       // gamma * Sigma: dimension of one boundary point
+constexpr int TM_THREADS = 256;
+constexpr int TM_WARPS = TM_THREADS / 32;
+constexpr int TM_WSCR = 512;      // doubles of each of the two per-warp scratch arrays: npair * xi * Sigma^2 must fit
+constexpr int TM_MAXCELL = 64;    // cells of one in-block anti-diagonal (a block holds <= 64 boundary points)
+constexpr int TM_BLOCK_SMEM = TM_WARPS * 2 * TM_WSCR * (int)sizeof(double);
+
+struct TmDev {
+  int n, gamma, xi, mh, MS, NB, S, npair;
+  int px[16], py[16];  // the nucleotide pairs with a non-zero B
+  const int* sig;      // [n+1]  Sigma of every boundary point
+  const int* off;      // [n+2]  padded offset of every boundary point in the flattened index space
+  const int* blk;      // [NB+1] first boundary point of every block; blk[NB] = n+1
+  const double* T;     // [n][4][MS][MS] dense tensor-train cores (operator weights summed, scaled by 2^-e)
+  const double* V;     // [4][g][g]
+  const double* B;     // [4][4][xi][g][g]
+  const double* SB;    // [4][4][xi][g][g]   SB[y][x][rho][d][c] = sum_e S[d][e] B[y][x][rho][e][c]   (Tr_S[B X] = sum_{c,d} SB[d][c] X[c][d])
+  const double* Sm;    // [g][g]
+  double* U;           // S x S
+  double* CT;          // S x S
+  double* GP;          // split-K partial tiles [block row][split][64 x 64]
+  double* result;      // [0] = Z in the stored scale
+};
+
+__global__ void tm_init_kernel(TmDev t) {
+  for (int p = blockIdx.x * blockDim.x + threadIdx.x; p <= t.n; p += gridDim.x * blockDim.x)
+    for (int a = 0; a < t.gamma * t.sig[p]; ++a) t.U[(size_t)(t.off[p] + a) * t.S + t.off[p] + a] = 1.0;  // Q_{i,i} = I (eq 3.6, first case)
+}
+
+__global__ void __launch_bounds__(GEMM_THREADS) tm_gemm_kernel(TmDev t, int D, int nsplit) {
+  extern __shared__ double gsm[];
+  const int I = blockIdx.x / nsplit, sp = blockIdx.x % nsplit, J = I + D;
+  const int nk = D - 1;  // K blocks I+1 .. J-1
+  const int kbeg = (I + 1 + (int)((long long)sp * nk / nsplit)) * CDZ_TB;
+  const int kend = (I + 1 + (int)((long long)(sp + 1) * nk / nsplit)) * CDZ_TB;
+  cdz_gemm_tile(t.U + (size_t)I * CDZ_TB * t.S, t.CT + (size_t)J * CDZ_TB * t.S, (size_t)t.S, kbeg, kend,
+                t.GP + ((size_t)I * nsplit + sp) * (CDZ_TB * CDZ_TB), gsm);
+}
+
+__global__ void __launch_bounds__(TM_THREADS) tm_block_kernel(TmDev t, int D, int nsplit) {
+  __shared__ int pre[TM_MAXCELL + 1];
+  extern __shared__ double wscr[];  // [TM_WARPS][2][TM_WSCR]
+  const int I = blockIdx.x, J = I + D;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int g = t.gamma, g2 = g * g, xi = t.xi, MS = t.MS, MS2 = MS * MS;
+  const size_t S = (size_t)t.S;
+  const int i0 = t.blk[I], i1 = t.blk[I + 1], j0 = t.blk[J], j1 = t.blk[J + 1];
+  const int dmin = max(1, j0 - (i1 - 1)), dmax = (j1 - 1) - i0;
+  double* tW = wscr + (size_t)warp * 2 * TM_WSCR;
+  double* mW = tW + TM_WSCR;
+  for (int d = dmin; d <= dmax; ++d) {
+    const int ilo = max(i0, j0 - d), ihi = min(i1 - 1, j1 - 1 - d);
+    const int ncell = ihi - ilo + 1;
+    if (ncell <= 0) continue;
+    if (tid == 0) {
+      int acc = 0;
+      for (int c = 0; c < ncell; ++c) { pre[c] = acc; acc += g2 * t.sig[ilo + c] * t.sig[ilo + c + d]; }
+      pre[ncell] = acc;
+    }
+    // ---- (A) closed elements Q_{j,i} = chi-hat_{i,j}(Q_{i+1,j-1}) of the step's cells (eq 3.8), one warp per cell ------------------------
+    for (int c = warp; c < ncell; c += TM_WARPS) {
+      const int i = ilo + c, j = i + d;
+      const int si = t.sig[i], sj = t.sig[j], mi = g * si, mj = g * sj;
+      double* ct = t.CT + (size_t)t.off[j] * S + t.off[i];
+      if (d == 1) {
+        // unpaired base i:  sum_x T_i[x] (x) V[x]
+        const double* Ti = t.T + (size_t)i * 4 * MS2;
+        for (int e = lane; e < mi * mj; e += 32) {
+          const int al = e / mj, de = e - al * mj, sa = al / g, za = al - sa * g, sd = de / g, zd = de - sd * g;
+          double v = 0.0;
+#pragma unroll
+          for (int x = 0; x < 4; ++x) v += Ti[x * MS2 + sa * MS + sd] * t.V[x * g2 + za * g + zd];
+          ct[(size_t)de * S + al] = v;
+        }
+      } else if (d - 2 >= t.mh) {
+        // base pair i.(j-1) around the block X = Q_{i+1,j-1}
+        const int l = j - 1, s1 = t.sig[i + 1], s2 = t.sig[l];
+        const double* X = t.U + (size_t)t.off[i + 1] * S + t.off[l];
+        const double* Ti = t.T + (size_t)i * 4 * MS2;
+        const double* Tl = t.T + (size_t)l * 4 * MS2;
+        // 1: t[pr][rho][a'][c'] = Tr_S[ B_{j,i}^rho X^{a',c'} ] = sum_{c,d} SB[y][x][rho][d][c] X[(a',c)][(c',d)]
+        for (int e = lane; e < t.npair * xi * s1 * s2; e += 32) {
+          const int c1 = e % s2, a1 = (e / s2) % s1, rho = (e / (s1 * s2)) % xi, pr = e / (s1 * s2 * xi);
+          const double* sb = t.SB + (size_t)((t.py[pr] * 4 + t.px[pr]) * xi + rho) * g2;
+          const double* xb = X + (size_t)(a1 * g) * S + c1 * g;
+          double v = 0.0;
+          for (int cc = 0; cc < g; ++cc)
+            for (int dd = 0; dd < g; ++dd) v += sb[dd * g + cc] * xb[(size_t)cc * S + dd];
+          tW[e] = v;
+        }
+        __syncwarp();
+        // 2: m[pr][rho][sa][sd] = sum_{a',c'} T_i[x][sa][a'] t[pr][rho][a'][c'] T_l[y][c'][sd]
+        for (int e = lane; e < t.npair * xi * si * sj; e += 32) {
+          const int sd = e % sj, sa = (e / sj) % si, rho = (e / (si * sj)) % xi, pr = e / (si * sj * xi);
+          const double* ti = Ti + t.px[pr] * MS2 + sa * MS;
+          const double* tl = Tl + t.py[pr] * MS2 + sd;
+          const double* tw = tW + (size_t)(pr * xi + rho) * s1 * s2;
+          double v = 0.0;
+          for (int a1 = 0; a1 < s1; ++a1) {
+            const double ta = ti[a1];
+            if (ta == 0.0) continue;
+            double s = 0.0;
+            for (int c1 = 0; c1 < s2; ++c1) s += tw[a1 * s2 + c1] * tl[c1 * MS];
+            v += ta * s;
+          }
+          mW[e] = v;
+        }
+        __syncwarp();
+        // 3: C[(sa,za)][(sd,zd)] = sum_{pr,rho} B[x][y][rho][za][zd] m[pr][rho][sa][sd]
+        for (int e = lane; e < mi * mj; e += 32) {
+          const int al = e / mj, de = e - al * mj, sa = al / g, za = al - sa * g, sd = de / g, zd = de - sd * g;
+          double v = 0.0;
+          for (int pr = 0; pr < t.npair; ++pr)
+            for (int rho = 0; rho < xi; ++rho)
+              v += t.B[(size_t)((t.px[pr] * 4 + t.py[pr]) * xi + rho) * g2 + za * g + zd] * mW[((pr * xi + rho) * si + sa) * sj + sd];
+          ct[(size_t)de * S + al] = v;
+        }
+        __syncwarp();
+      }
+      // spans 2 .. min_hairpin + 1 close nothing: the zero-initialised table entry stands (line 483)
+    }
+    __syncthreads();
+    // ---- (B) Q_{i,j} = sum_{k in [i:j)} Q_{i,k} Q_{j,k}^T: the partial tiles of the GEMM + the bonds of block I from i on + those of block J before j ----
+    const int total = pre[ncell];
+    for (int it = tid; it < total; it += TM_THREADS) {
+      int c = 0;
+      while (pre[c + 1] <= it) ++c;
+      const int i = ilo + c, j = i + d, mj = g * t.sig[j];
+      const int e = it - pre[c], al = e / mj, de = e - al * mj;
+      const int ri = t.off[i] + al, rj = t.off[j] + de;
+      const double* ru = t.U + (size_t)ri * S;
+      const double* rc = t.CT + (size_t)rj * S;
+      double v = 0.0;
+      for (int sp = 0; sp < nsplit; ++sp)
+        v += t.GP[((size_t)I * nsplit + sp) * (CDZ_TB * CDZ_TB) + (size_t)(ri - I * CDZ_TB) * CDZ_TB + (rj - J * CDZ_TB)];
+      if (I == J) {
+        for (int kb = t.off[i]; kb < t.off[j]; ++kb) v += ru[kb] * rc[kb];
+      } else {
+        for (int kb = t.off[i]; kb < (I + 1) * CDZ_TB; ++kb) v += ru[kb] * rc[kb];
+        for (int kb = J * CDZ_TB; kb < t.off[j]; ++kb) v += ru[kb] * rc[kb];
+      }
+      t.U[(size_t)ri * S + rj] = v;
+    }
+    __syncthreads();
+  }
+}
+
+// Z = sum_{sigma_n} Tr_S[ Q_{0,n}^{(0, sigma_n)} ]  (eq 3.7 with the open chain of lines 561-567)
+__global__ void tm_final_kernel(TmDev t) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  const int g = t.gamma;
+  double z = 0.0;
+  for (int s = 0; s < t.sig[t.n]; ++s)
+    for (int d = 0; d < g; ++d)
+      for (int e = 0; e < g; ++e) z += t.Sm[d * g + e] * t.U[(size_t)(t.off[0] + e) * t.S + t.off[t.n] + s * g + d];
+  t.result[0] = z;
+}
+
+// ---- host side ---------------------------------------------------------------------------------------------------------------------------
+struct TmLayout {
+  int n = 0, NB = 0, S = 0, MS = 1, maxsplit_tiles = 0;
+  std::vector<int> sig, off, blk;
+  size_t o_U = 0, o_CT = 0, o_GP = 0, o_T = 0, o_V = 0, o_B = 0, o_SB = 0, o_S = 0, o_sig = 0, o_off = 0, o_blk = 0, o_res = 0, total = 0;
+};
+
+int tm_check(const cdz_tm_params* p, const cdz_tt* tt) {
+  if (!p || !tt || !p->V || !p->B || !p->S) { cdz_set_error("cdz_tm: null argument"); return CDZ_EINVAL; }
+  if (p->gamma < 1 || p->gamma > TM_MAXG || p->xi < 1 || p->xi > TM_MAXXI || p->min_hairpin < 0) {
+    cdz_set_error("cdz_tm: need 1 <= gamma <= 8, 1 <= xi <= 4, min_hairpin >= 0");
+    return CDZ_EINVAL;
+  }
+  if (p->gamma * tt->MS > TM_MAXM) { cdz_set_error("cdz_tm: gamma x bond dimension exceeds 32"); return CDZ_EINVAL; }
+  int npair = 0;
+  const int g2 = p->gamma * p->gamma;
+  for (int xy = 0; xy < 16; ++xy) {
+    bool nz = false;
+    for (int k = 0; k < p->xi * g2; ++k) {
+      const double b = p->B[(size_t)xy * p->xi * g2 + k];
+      if (!std::isfinite(b) || b < 0) { cdz_set_error("cdz_tm: B must be finite and non-negative"); return CDZ_EINVAL; }
+      nz = nz || b != 0.0;
+    }
+    npair += nz;
+  }
+  for (int k = 0; k < 4 * g2; ++k)
+    if (!std::isfinite(p->V[k]) || p->V[k] < 0) { cdz_set_error("cdz_tm: V must be finite and non-negative"); return CDZ_EINVAL; }
+  for (int k = 0; k < g2; ++k)
+    if (!std::isfinite(p->S[k]) || p->S[k] < 0) { cdz_set_error("cdz_tm: S must be finite and non-negative"); return CDZ_EINVAL; }
+  if (npair * p->xi * tt->MS * tt->MS > TM_WSCR) { cdz_set_error("cdz_tm: pairs x xi x bond^2 exceeds the per-warp scratch (512)"); return CDZ_EINVAL; }
+  return CDZ_OK;
+}
+
+// boundary points 0..n of the first n positions of tt, grouped greedily into blocks of <= 64 flattened indices
+TmLayout tm_layout(const cdz_tm_params* p, const cdz_tt* tt, int n) {
+  TmLayout L;
+  L.n = n;
+  L.MS = tt->MS;
+  L.sig.assign(tt->sigma.begin(), tt->sigma.begin() + n + 1);
+  L.off.assign(n + 2, 0);
+  int b = 0, used = 0;
+  L.blk.push_back(0);
+  for (int q = 0; q <= n; ++q) {
+    const int m = p->gamma * L.sig[q];
+    if (used + m > CDZ_TB) { ++b; used = 0; L.blk.push_back(q); }
+    L.off[q] = b * CDZ_TB + used;
+    used += m;
+  }
+  L.NB = b + 1;
+  L.blk.push_back(n + 1);
+  L.S = L.NB * CDZ_TB;
+  L.off[n + 1] = L.S;
+  for (int D = 2; D < L.NB; ++D) L.maxsplit_tiles = std::max(L.maxsplit_tiles, (L.NB - D) * cdz_nsplit(L.NB, D, 1));
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 255) & ~size_t(255); return r; };
+  const size_t g2 = (size_t)p->gamma * p->gamma;
+  L.o_res = take(64);
+  L.o_U = take(sizeof(double) * (size_t)L.S * L.S);
+  L.o_CT = take(sizeof(double) * (size_t)L.S * L.S);
+  L.o_GP = take(sizeof(double) * (size_t)std::max(1, L.maxsplit_tiles) * CDZ_TB * CDZ_TB);
+  L.o_T = take(sizeof(double) * (size_t)std::max(1, n) * 4 * L.MS * L.MS);
+  L.o_V = take(sizeof(double) * 4 * g2);
+  L.o_B = take(sizeof(double) * 16 * p->xi * g2);
+  L.o_SB = take(sizeof(double) * 16 * p->xi * g2);
+  L.o_S = take(sizeof(double) * g2);
+  L.o_sig = take(sizeof(int) * (n + 1));
+  L.o_off = take(sizeof(int) * (n + 2));
+  L.o_blk = take(sizeof(int) * (L.NB + 1));
+  L.total = o;
+  return L;
+}
+
+// one pass over the first n positions with all operator weights times 2^-e; Z_stored to *z_out (host), device time to *ms (may be NULL)
+int tm_pass(const cdz_tm_params* p, const cdz_tt* tt, int n, int e, char* base, cudaStream_t st, double* z_out, cdz_tm_info* info) {
+  const TmLayout L = tm_layout(p, tt, n);
+  const int g = p->gamma, g2 = g * g, xi = p->xi, MS = L.MS, MS2 = MS * MS;
+  std::vector<double> T((size_t)std::max(1, n) * 4 * MS2, 0.0), SB((size_t)16 * xi * g2, 0.0);
+  const double sc = ldexp(1.0, -e);
+  for (int q = 0; q < n; ++q)
+    for (int z = tt->opstart[q]; z < tt->opstart[q + 1]; ++z) {
+      const cdz_op& o = tt->ops[z];
+      T[((size_t)q * 4 + o.b) * MS2 + o.a * MS + o.c] += o.x * sc;
+    }
+  for (int xy = 0; xy < 16; ++xy)
+    for (int r = 0; r < xi; ++r)
+      for (int d = 0; d < g; ++d)
+        for (int c = 0; c < g; ++c) {
+          double v = 0.0;
+          for (int ee = 0; ee < g; ++ee) v += p->S[d * g + ee] * p->B[((size_t)xy * xi + r) * g2 + ee * g + c];
+          SB[((size_t)xy * xi + r) * g2 + d * g + c] = v;
+        }
+  TmDev t;
+  t.n = n; t.gamma = g; t.xi = xi; t.mh = p->min_hairpin; t.MS = MS; t.NB = L.NB; t.S = L.S; t.npair = 0;
+  for (int xy = 0; xy < 16; ++xy) {
+    bool nz = false;
+    for (int k = 0; k < xi * g2; ++k) nz = nz || p->B[(size_t)xy * xi * g2 + k] != 0.0;
+    if (nz) { t.px[t.npair] = xy / 4; t.py[t.npair] = xy % 4; ++t.npair; }
+  }
+  for (int k = t.npair; k < 16; ++k) t.px[k] = t.py[k] = 0;
+  t.result = (double*)(base + L.o_res);
+  t.U = (double*)(base + L.o_U);
+  t.CT = (double*)(base + L.o_CT);
+  t.GP = (double*)(base + L.o_GP);
+  t.T = (const double*)(base + L.o_T);
+  t.V = (const double*)(base + L.o_V);
+  t.B = (const double*)(base + L.o_B);
+  t.SB = (const double*)(base + L.o_SB);
+  t.Sm = (const double*)(base + L.o_S);
+  t.sig = (const int*)(base + L.o_sig);
+  t.off = (const int*)(base + L.o_off);
+  t.blk = (const int*)(base + L.o_blk);
+  CDZ_CUDA(cudaMemcpyAsync(base + L.o_T, T.data(), sizeof(double) * T.size(), cudaMemcpyHostToDevice, st));
+  CDZ_CUDA(cudaMemcpyAsync(base + L.o_V, p->V, sizeof(double) * 4 * g2, cudaMemcpyHostToDevice, st));
+  CDZ_CUDA(cudaMemcpyAsync(base + L.o_B, p->B, sizeof(double) * 16 * xi * g2, cudaMemcpyHostToDevice, st));
+  CDZ_CUDA(cudaMemcpyAsync(base + L.o_SB, SB.data(), sizeof(double) * SB.size(), cudaMemcpyHostToDevice, st));
+  CDZ_CUDA(cudaMemcpyAsync(base + L.o_S, p->S, sizeof(double) * g2, cudaMemcpyHostToDevice, st));
+  CDZ_CUDA(cudaMemcpyAsync(base + L.o_sig, L.sig.data(), sizeof(int) * (n + 1), cudaMemcpyHostToDevice, st));
+  CDZ_CUDA(cudaMemcpyAsync(base + L.o_off, L.off.data(), sizeof(int) * (n + 2), cudaMemcpyHostToDevice, st));
+  CDZ_CUDA(cudaMemcpyAsync(base + L.o_blk, L.blk.data(), sizeof(int) * (L.NB + 1), cudaMemcpyHostToDevice, st));
+  CDZ_CUDA(cudaStreamSynchronize(st));  // the staging vectors above are pageable host memory about to go out of scope
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (info) { CDZ_CUDA(cudaEventCreate(&e0)); CDZ_CUDA(cudaEventCreate(&e1)); CDZ_CUDA(cudaEventRecord(e0, st)); }
+  CDZ_CUDA(cudaMemsetAsync(t.U, 0, sizeof(double) * (size_t)L.S * L.S, st));
+  CDZ_CUDA(cudaMemsetAsync(t.CT, 0, sizeof(double) * (size_t)L.S * L.S, st));
+  CDZ_CUDA(cudaFuncSetAttribute(tm_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
+  CDZ_CUDA(cudaFuncSetAttribute(tm_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TM_BLOCK_SMEM));
+  tm_init_kernel<<<32, 256, 0, st>>>(t);
+  long launches = 3;
+  double flop = 0.0;
+  for (int D = 0; D < L.NB; ++D) {
+    const int nblk = L.NB - D, nsplit = cdz_nsplit(L.NB, D, 1);
+    if (nsplit > 0) {
+      tm_gemm_kernel<<<nblk * nsplit, GEMM_THREADS, GEMM_SMEM, st>>>(t, D, nsplit);
+      flop += 2.0 * nblk * (double)(D - 1) * CDZ_TB * CDZ_TB * CDZ_TB;
+      ++launches;
+    }
+    tm_block_kernel<<<nblk, TM_THREADS, TM_BLOCK_SMEM, st>>>(t, D, nsplit);
+    ++launches;
+  }
+  tm_final_kernel<<<1, 32, 0, st>>>(t);
+  ++launches;
+  if (info) CDZ_CUDA(cudaEventRecord(e1, st));
+  CDZ_CUDA(cudaMemcpyAsync(z_out, t.result, sizeof(double), cudaMemcpyDeviceToHost, st));
+  CDZ_CUDA(cudaStreamSynchronize(st));
+  CDZ_CUDA(cudaGetLastError());
+  if (info) {
+    float ms = 0.f;
+    CDZ_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    info->device_ms = ms;
+    info->gemm_flop = flop;
+    info->launches = launches;
+    info->S = L.S;
+    info->NB = L.NB;
+    info->scale_exponent = e;
+    info->table_bytes = (double)(2 * sizeof(double)) * L.S * L.S;
+  }
+  return CDZ_OK;
+}
+
+constexpr int TM_PILOT = 60;
+
+}  // namespace
+
+extern "C" int cdz_tm_workspace_bytes(const cdz_tm_params* p, const cdz_tt* tt, size_t* bytes) {
+  const int rc = tm_check(p, tt);
+  if (rc != CDZ_OK) return rc;
+  if (!bytes) { cdz_set_error("cdz_tm_workspace_bytes: null argument"); return CDZ_EINVAL; }
+  *bytes = tm_layout(p, tt, tt->n).total;
+  return CDZ_OK;
+}
+
+extern "C" int cdz_tm_inside(const cdz_tm_params* p, const cdz_tt* tt, void* workspace_dev, size_t workspace_bytes, void* stream,
+                             double* logZ_host, cdz_tm_info* info) {
+  int rc = tm_check(p, tt);
+  if (rc != CDZ_OK) return rc;
+  if (!logZ_host) { cdz_set_error("cdz_tm_inside: logZ_host is required"); return CDZ_EINVAL; }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cdz_set_error("cdz_tm_inside: no CUDA device (the library has no CPU path)"); return CDZ_ECUDA; }
+  cudaStream_t st = (cudaStream_t)stream;
+  const int n = tt->n;
+  const size_t need = tm_layout(p, tt, n).total;
+  char* base = (char*)workspace_dev;
+  bool own = false;
+  if (!base) {
+    if (cudaMalloc((void**)&base, need) != cudaSuccess) { cudaGetLastError(); cdz_set_error("cdz_tm_inside: device allocation failed"); return CDZ_ENOMEM; }
+    own = true;
+  } else if (workspace_bytes < need) {
+    cdz_set_error("cdz_tm_inside: workspace too small (cdz_tm_workspace_bytes)");
+    return CDZ_EINVAL;
+  }
+  // pilot pass over a prefix: the growth rate of the partition function per position, in bits
+  int e = 0;
+  double z = 0.0;
+  if (n > TM_PILOT) {
+    rc = tm_pass(p, tt, TM_PILOT, 0, base, st, &z, nullptr);
+    if (rc == CDZ_OK && (!(z > 0.0) || !std::isfinite(z))) { cdz_set_error("cdz_tm_inside: pilot pass left the fp64 range"); rc = CDZ_EOVERFLOW; }
+    if (rc == CDZ_OK) e = (int)lround(log2(z) / TM_PILOT);
+  }
+  if (rc == CDZ_OK) rc = tm_pass(p, tt, n, e, base, st, &z, info);
+  if (rc == CDZ_OK && (!(z > 0.0) || !std::isfinite(z))) { cdz_set_error("cdz_tm_inside: partition function left the fp64 range"); rc = CDZ_EOVERFLOW; }
+  if (rc == CDZ_OK) *logZ_host = log(z) + (double)e * n * M_LN2;
+  if (own) cudaFree(base);
+  return rc;
+}
+
+// parity access after cdz_tm_inside with a caller workspace: which = 0 the upper block Q_{i,j} (i <= j) as [gamma Sigma_i][gamma Sigma_j],
+// which = 1 the lower block Q_{j,i} (j > i) as [gamma Sigma_j][gamma Sigma_i]; true value = stored * 2^shift
+extern "C" int cdz_tm_block(const cdz_tm_params* p, const cdz_tt* tt, const void* workspace_dev, int scale_exponent, int which, int i,
+                            int j, double* out_host, int* shift_out) {
+  const int rc = tm_check(p, tt);
+  if (rc != CDZ_OK) return rc;
+  const int n = tt->n;
+  if (!workspace_dev || !out_host || i < 0 || j < i || j > n || (which != 0 && which != 1) || (which == 1 && i == j)) {
+    cdz_set_error("cdz_tm_block: bad argument");
+    return CDZ_EINVAL;
+  }
+  const TmLayout L = tm_layout(p, tt, n);
+  const char* base = (const char*)workspace_dev;
+  const int mi = p->gamma * L.sig[i], mj = p->gamma * L.sig[j];
+  if (which == 0) {
+    CDZ_CUDA(cudaMemcpy2D(out_host, sizeof(double) * mj, base + L.o_U + sizeof(double) * ((size_t)L.off[i] * L.S + L.off[j]),
+                          sizeof(double) * L.S, sizeof(double) * mj, mi, cudaMemcpyDeviceToHost));
+  } else {
+    CDZ_CUDA(cudaMemcpy2D(out_host, sizeof(double) * mi, base + L.o_CT + sizeof(double) * ((size_t)L.off[j] * L.S + L.off[i]),
+                          sizeof(double) * L.S, sizeof(double) * mi, mj, cudaMemcpyDeviceToHost));
+  }
+  if (shift_out) *shift_out = scale_exponent * (j - i);
+  return which == 0 ? mi * mj : mj * mi;
+}

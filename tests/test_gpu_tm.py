@@ -1,0 +1,168 @@
+"""GPU parity of the tensor-model recursion (cdz_tm_inside; eqs 3.5-3.8) against oracle/tensor_model.py, through the
+C ABI: every block of Q (upper Q_{i,j} and lower Q_{j,i}) element by element, log Z at 1e-9 relative (DESIGN.md c-13), the closed forms of
+the oracle's pins at sizes the oracle cannot reach, and the edge cases."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2604_19718_b200 import binding
+
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def I():
+    from paper_2604_19718_b200 import inputs
+
+    return inputs
+
+
+def _both(B, I, aa, kind, seed=5):
+    from oracle import oracle as O
+
+    cw, pw = I.codon_logw(seed), (I.pair_logw(seed) if kind == I.TT_CODON_PAIR else None)
+    return B.TensorTrain.build(aa, kind, cw, pw), O.TT.build(aa, kind, cw, pw).get()
+
+
+@pytest.mark.parametrize("cfg,L,gamma,xi,mh", [
+    (1, 4, 2, 2, 3), (1, 20, 2, 2, 3), (1, 20, 4, 2, 3), (5, 12, 2, 2, 3), (5, 12, 4, 1, 1), (1, 30, 3, 3, 0), (2, 25, 2, 2, 3),
+    (1, 40, 8, 1, 3),
+])
+def test_blocks_and_logz_vs_oracle(B, I, cfg, L, gamma, xi, mh):
+    """Every stored block against the plain Alg S4.1 of the oracle: several 64-blocks (GEMM tiles, split-K, in-block edges of both kinds),
+    both tensor trains, gamma 2..8, ragged last block."""
+    from oracle import tensor_model as TM
+
+    d = I.design(cfg, 0, L)
+    tm = I.tensor_model(gamma, xi, seed=100 + gamma)
+    tm.min_hairpin = mh
+    tg, (sigma, ops) = _both(B, I, d.aa, d.kind, d.seed)
+    lz_o, Q = TM.tm_inside(tm, sigma, ops, return_Q=True)
+    run = B.TensorModelPass(tm, tg)
+    assert abs(run.logZ - lz_o) <= 1e-9 * abs(lz_o), (run.logZ, lz_o)
+    n = len(ops)
+    worst = 0.0
+    for i in range(n + 1):
+        for j in range(i, n + 1):
+            v, sh = run.block(0, i, j)
+            ref = Q[i][j].reshape(-1)
+            got = v * 2.0 ** sh
+            worst = max(worst, float(np.max(np.abs(got - ref) / (np.abs(ref) + 1e-300 + 1e-13 * np.max(np.abs(ref))))))
+            if j > i:
+                v, sh = run.block(1, i, j)
+                ref = Q[j][i].reshape(-1)
+                got = v * 2.0 ** sh
+                worst = max(worst, float(np.max(np.abs(got - ref) / (np.abs(ref) + 1e-300 + 1e-13 * max(1e-300, np.max(np.abs(ref)))))))
+    assert worst <= 1e-10, worst
+
+
+def _counts():
+    tab = {}
+    for line in open(os.path.join(GOLD, "structure_counts.txt")):
+        if line.startswith("unlimited"):
+            _, n, v = line.split()
+            tab[int(n)] = int(v)
+    return tab
+
+
+@pytest.mark.parametrize("n", [5, 20, 37, 38])
+def test_unit_model_structure_counts(B, I, n):
+    """gamma = xi = 1, all ones, every two bases pair, one operator per position: Z = S(n) of eq S2.3 (tests/golden/structure_counts.txt)."""
+    tm = I.tensor_model(1, 1, unit=True)
+    tg = B.TensorTrain.from_operators([[(0, p % 4, 0, 1.0)] for p in range(n)])
+    run = B.TensorModelPass(tm, tg)
+    assert abs(run.logZ - math.log(_counts()[n])) <= 1e-12 * run.logZ
+
+
+def _log_structure_count(n, mh=3):
+    """log S(n) by the scalar recursion S(m) = S(m-1) + sum_k S(k) S(m-2-k), hairpins >= mh (eq S2.3), in exact integers."""
+    S = [1] * (n + 1)
+    for m in range(1, n + 1):
+        v = S[m - 1]
+        for k in range(0, m - 1):  # first base paired with k+1 ... enclosed k bases, rest m-2-k
+            if k >= mh:
+                v += S[k] * S[m - 2 - k]
+        S[m] = v
+    return math.log(S[n])
+
+
+def test_unit_model_large_closed_form(B, I):
+    """2400 nt with a weightless single-codon tensor train (60+ blocks, split-K, the pilot scale in use): log Z = sum log deg + log S(n),
+    S(n) in exact integer arithmetic -- nothing of the recursion under test is used on the right-hand side."""
+    tm = I.tensor_model(1, 1, unit=True)
+    aa = I.protein(777, 800)
+    deg = {"A": 4, "C": 2, "D": 2, "E": 2, "F": 2, "G": 4, "H": 2, "I": 3, "K": 2, "L": 6, "M": 1, "N": 2, "P": 4, "Q": 2, "R": 6, "S": 6,
+           "T": 4, "V": 4, "W": 1, "Y": 2}
+    tg = B.TensorTrain.build(aa, I.TT_SINGLE_CODON, None, None)
+    run = B.TensorModelPass(tm, tg)
+    ref = sum(math.log(deg[a]) for a in aa) + _log_structure_count(3 * len(aa))
+    assert run.info.NB >= 50 and run.info.scale_exponent != 0
+    assert abs(run.logZ - ref) <= 1e-9 * ref, (run.logZ, ref)
+
+
+def test_no_pairs_transfer_product_and_determinism(B, I):
+    """B = 0 at 900 nt: Z = sum_{sigma_n} Tr_S of the product of the dressed transfer matrices (line 448), accumulated here in log space."""
+    tm = I.tensor_model(3, 2, seed=11)
+    tm.B = np.zeros_like(tm.B)
+    d = I.design(2, 0, 300)
+    tg, (sigma, ops) = _both(B, I, d.aa, d.kind, d.seed)
+    M, logs = np.eye(3), 0.0
+    for p, lst in enumerate(ops):
+        Tp = np.zeros((3 * sigma[p], 3 * sigma[p + 1]))
+        for (a, b, c, x) in lst:
+            Tp[a * 3:(a + 1) * 3, c * 3:(c + 1) * 3] += x * tm.V[b]
+        M = M @ Tp
+        s = M.max()
+        M, logs = M / s, logs + math.log(s)
+    ref = math.log(sum(np.trace(tm.S @ M[:, s * 3:(s + 1) * 3]) for s in range(sigma[-1]))) + logs
+    run = B.TensorModelPass(tm, tg)
+    assert abs(run.logZ - ref) <= 1e-9 * abs(ref), (run.logZ, ref)
+    first = run.logZ
+    assert run.rerun() == first
+
+
+def test_prefix_chain_config2(B, I):
+    """Config-2 design (300 aa, codon-pair tensor train, gamma 4, xi 2) at full size: finite, deterministic, and the blocks of its first
+    36 nt equal the oracle's run on that prefix (Q_{i,j} depends on positions i..j-1 only), the uniform scale undone."""
+    from oracle import oracle as O
+    from oracle import tensor_model as TM
+
+    d = I.design(2, 0)
+    tm = I.tensor_model(4, 2)
+    tg = B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
+    run = B.TensorModelPass(tm, tg)
+    assert math.isfinite(run.logZ) and run.info.scale_exponent != 0
+    sigma, ops = O.TT.build(d.aa[:12], d.kind, d.codon_logw, d.pair_logw).get()
+    _, Q = TM.tm_inside(tm, sigma, ops, return_Q=True)
+    for (i, j) in ((0, 36), (0, 20), (7, 33), (3, 4), (12, 35)):
+        if j == 36:
+            continue  # the last bond of the prefix train is not the bond of the full train at that point
+        v, sh = run.block(0, i, j)
+        ref = Q[i][j].reshape(-1)
+        assert np.allclose(v * 2.0 ** sh, ref, rtol=1e-10, atol=0.0), (i, j)
+        v, sh = run.block(1, i, j)
+        assert np.allclose(v * 2.0 ** sh, Q[j][i].reshape(-1), rtol=1e-10, atol=1e-300), (i, j)
+
+
+def test_errors(B, I):
+    tm = I.tensor_model(2, 2)
+    tg = B.TensorTrain.build("MF", I.TT_SINGLE_CODON, None, None)
+    bad = I.tensor_model(2, 2)
+    bad.V = -bad.V
+    with pytest.raises(B.CdzError):
+        B.TensorModelPass(bad, tg)
+    big = I.tensor_model(2, 2)
+    big.gamma = 9
+    with pytest.raises(B.CdzError):
+        B.TensorModelPass(big, tg)
+    assert math.isfinite(B.TensorModelPass(tm, tg).logZ)
