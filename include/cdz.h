@@ -229,7 +229,7 @@ int cdz_match_frequencies(const cdz_model* m, const char* aa, int L, int kind, c
  *                                 tensor of its 3' side ("B_{j,i}^rho"); all-zero B[x][y] = x.y cannot pair,
  *   S [gamma][gamma]              weighted trace Tr_S[X] = Tr[S X] (line 178),
  * min_hairpin: a pair k.l needs l - k - 1 >= min_hairpin (line 483: 3).  All entries finite and >= 0.  Limits of this version:
- * gamma x (largest bond dimension of tt) <= 32 and (number of pairable (x,y)) x xi x bond^2 <= 512; CDZ_EINVAL beyond. */
+ * gamma x (largest bond dimension of tt) <= 32 and (number of pairable (x,y)) x xi x bond x (96 / gamma) <= 6144; CDZ_EINVAL beyond. */
 typedef struct {
   int32_t gamma, xi, min_hairpin;
   const double* V;
@@ -242,7 +242,7 @@ typedef struct {
   double table_bytes;      /* the two S x S tables */
   int64_t launches;
   int32_t S, NB;           /* flattened (block-padded) dimension sum_i gamma Sigma_i and its number of 64-blocks */
-  int32_t scale_exponent;  /* e: every operator weight was multiplied by 2^-e; log Z = log Z_stored + e n ln 2 */
+  double scale_rate;       /* r: the operator weights of position q were multiplied by 2^-(P[q+1] - P[q]), P[q] = floor(q r); log Z = log Z_stored + P[n] ln 2 */
 } cdz_tm_info;
 /* log Z = -q_psi (eq 2.4 line 72) of the design distribution under the tensor model: the sum over every operator path (coding sequence,
  * weights included) of `tt` and every unpseudoknotted structure of the state's tensor diagram (eq S2.1), by the recursion
@@ -250,15 +250,15 @@ typedef struct {
  * run as a block wavefront with fp64 tensor-core tiles (csrc/cdz_tm.cu).  Open chain as in cdz_tt_build.  workspace_dev: a device
  * buffer of >= cdz_tm_workspace_bytes bytes (it then holds the tables after the call: cdz_tm_block) or NULL (allocated and freed
  * inside).  Blocking: returns after logZ_host has been written.  info may be NULL.  CDZ_EOVERFLOW if Z leaves the fp64 range in the
- * stored scale (one uniform power-of-two scale per position, measured by a pilot pass over the first 60 positions). */
+ * stored scale (power-of-two scales per position at a uniform rate, measured by pilot passes over the first 60 and 600 positions). */
 int cdz_tm_workspace_bytes(const cdz_tm_params* p, const cdz_tt* tt, size_t* bytes);
 int cdz_tm_inside(const cdz_tm_params* p, const cdz_tt* tt, void* workspace_dev, size_t workspace_bytes, void* stream, double* logZ_host,
                   cdz_tm_info* info);
-/* Debug / parity access to the tables a cdz_tm_inside call left in a caller workspace (same p, tt; scale_exponent from its info):
+/* Debug / parity access to the tables a cdz_tm_inside call left in a caller workspace (same p, tt; scale_rate from its info):
  * which = 0: the upper block Q_{i,j}, 0 <= i <= j <= n, as [gamma Sigma_i][gamma Sigma_j]; which = 1: the lower block Q_{j,i}, i < j, as
  * [gamma Sigma_j][gamma Sigma_i] (index (sigma, zeta) -> sigma gamma + zeta, line 211).  true value = out x 2^shift_out.  Returns the
  * element count. */
-int cdz_tm_block(const cdz_tm_params* p, const cdz_tt* tt, const void* workspace_dev, int scale_exponent, int which, int i, int j,
+int cdz_tm_block(const cdz_tm_params* p, const cdz_tt* tt, const void* workspace_dev, double scale_rate, int which, int i, int j,
                  double* out_host, int* shift_out);
 
 /* ---- convenience: host buffers end to end (used for the e2e timing) -------- */

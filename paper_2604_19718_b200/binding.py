@@ -64,7 +64,7 @@ class TMParams(C.Structure):
 
 class TMInfo(C.Structure):
     _fields_ = [("device_ms", C.c_double), ("gemm_flop", C.c_double), ("table_bytes", C.c_double), ("launches", C.c_int64),
-                ("S", C.c_int32), ("NB", C.c_int32), ("scale_exponent", C.c_int32)]
+                ("S", C.c_int32), ("NB", C.c_int32), ("scale_rate", C.c_double)]
 
 
 _lib = None
@@ -118,7 +118,7 @@ def lib():
     L.cdz_run_host.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, dp, vp]
     L.cdz_tm_workspace_bytes.argtypes = [C.POINTER(TMParams), vp, C.POINTER(C.c_size_t)]
     L.cdz_tm_inside.argtypes = [C.POINTER(TMParams), vp, vp, C.c_size_t, vp, dp, C.POINTER(TMInfo)]
-    L.cdz_tm_block.argtypes = [C.POINTER(TMParams), vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
+    L.cdz_tm_block.argtypes = [C.POINTER(TMParams), vp, vp, C.c_double, C.c_int, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
     _lib = L
     return L
 
@@ -416,6 +416,6 @@ class TensorModelPass:
         """(values as stored, shift): true block = values * 2**shift.  which 0: Q_{i,j} upper, 1: Q_{j,i} lower."""
         out = np.zeros(32 * 32)
         sh = C.c_int()
-        cnt = _check(lib().cdz_tm_block(C.byref(self.p), self.tt.h, C.c_void_p(self.ws.data_ptr()), self.info.scale_exponent, which, i, j,
+        cnt = _check(lib().cdz_tm_block(C.byref(self.p), self.tt.h, C.c_void_p(self.ws.data_ptr()), self.info.scale_rate, which, i, j,
                                         _dp(out), C.byref(sh)))
         return out[:cnt].copy(), sh.value

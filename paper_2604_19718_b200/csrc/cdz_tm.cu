@@ -15,7 +15,9 @@
 // Tables: U[(i,a)][(j,b)] = Q_{i,j} (upper, identity on the diagonal blocks) and CT[(j,d)][(k,a)] = Q_{j,k} (the lower blocks as printed),
 // both S x S row-major over the block-padded flattened index space, so the k-sum of a cell is a dot product of two contiguous rows.
 // Scaling: every term of every Q_{i,j} contains exactly one operator of each position i..j-1, so all operator weights are multiplied by
-// 2^-e (exact) and log Z = log Z_stored + e n ln 2; e is the growth rate measured by a pilot pass over the first <= 60 positions.
+// an exact power of two: position q by 2^-(P[q+1] - P[q]), P[q] = floor(q r), so that a stored block is the true one times 2^-(P[j] - P[i])
+// (products of adjacent intervals telescope) and log Z = log Z_stored + P[n] ln 2; r = growth rate of log2 Z per position, measured by pilot
+// passes over the first 60 and 600 positions.
 // Readings: DESIGN.md section 17 (the same as oracle/tensor_model.py states in its header; the two share no code).
 #include <math.h>
 
@@ -31,10 +33,13 @@ constexpr int TM_MAXG = 8;        // gamma
 constexpr int TM_MAXXI = 4;       // xi
 constexpr int TM_MAXM = 32;       // gamma * Sigma: dimension of one boundary point
 constexpr int TM_THREADS = 256;
-constexpr int TM_WARPS = TM_THREADS / 32;
-constexpr int TM_WSCR = 512;      // doubles of each of the two per-warp scratch arrays: npair * xi * Sigma^2 must fit
 constexpr int TM_MAXCELL = 64;    // cells of one in-block anti-diagonal (a block holds <= 64 boundary points)
-constexpr int TM_BLOCK_SMEM = TM_WARPS * 2 * TM_WSCR * (int)sizeof(double);
+// shared pools of one in-block anti-diagonal.  Its cells (i, j) have i+1 in block I or the first point after it and j-1 in block J or the last
+// point before it, so sum m_{i+1} <= 96, sum m_{i+1}^2 <= 32 * 96 (likewise for j-1) and by Cauchy-Schwarz sum m_{i+1} m_{j-1} <= 3072 staged X
+// entries (+ <= 96 row pads); the two intermediates of chi-hat hold pairs x xi x Sigma x Sigma' entries per cell, in total
+// <= pairs x xi x MS x 96 / gamma, which tm_check bounds by TM_POOL.
+constexpr int TM_XPOOL = 3200, TM_POOL = 6144;
+constexpr int TM_BLOCK_SMEM = (TM_XPOOL + 2 * TM_POOL) * (int)sizeof(double);
 
 struct TmDev {
   int n, gamma, xi, mh, MS, NB, S, npair;
@@ -69,108 +74,178 @@ __global__ void __launch_bounds__(GEMM_THREADS) tm_gemm_kernel(TmDev t, int D, i
 }
 
 __global__ void __launch_bounds__(TM_THREADS) tm_block_kernel(TmDev t, int D, int nsplit) {
-  __shared__ int pre[TM_MAXCELL + 1];
-  extern __shared__ double wscr[];  // [TM_WARPS][2][TM_WSCR]
+  // prefix sums over the cells of one in-block anti-diagonal: outputs | staged X entries | t entries | m entries | 4 x 4 output tiles
+  __shared__ int pre[TM_MAXCELL + 1], prx[TM_MAXCELL + 1], prt[TM_MAXCELL + 1], prm[TM_MAXCELL + 1], prb[TM_MAXCELL + 1];
+  extern __shared__ double pool[];  // X pool [TM_XPOOL] | t pool [TM_POOL] | m pool [TM_POOL]
+  double* xP = pool;
+  double* tP = pool + TM_XPOOL;
+  double* mP = tP + TM_POOL;
   const int I = blockIdx.x, J = I + D;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int g = t.gamma, g2 = g * g, xi = t.xi, MS = t.MS, MS2 = MS * MS;
+  const int tid = threadIdx.x;
+  const int g = t.gamma, g2 = g * g, xi = t.xi, MS = t.MS, MS2 = MS * MS, npx = t.npair * xi;
   const size_t S = (size_t)t.S;
   const int i0 = t.blk[I], i1 = t.blk[I + 1], j0 = t.blk[J], j1 = t.blk[J + 1];
   const int dmin = max(1, j0 - (i1 - 1)), dmax = (j1 - 1) - i0;
-  double* tW = wscr + (size_t)warp * 2 * TM_WSCR;
-  double* mW = tW + TM_WSCR;
+  // item -> (cell, index inside the cell) through a prefix array
+  auto cell_of = [&](const int* pr, int it, int& c) { c = 0; while (pr[c + 1] <= it) ++c; return it - pr[c]; };
   for (int d = dmin; d <= dmax; ++d) {
     const int ilo = max(i0, j0 - d), ihi = min(i1 - 1, j1 - 1 - d);
     const int ncell = ihi - ilo + 1;
     if (ncell <= 0) continue;
+    const bool pairs = d >= 2 && d - 2 >= t.mh;
     if (tid == 0) {
-      int acc = 0;
-      for (int c = 0; c < ncell; ++c) { pre[c] = acc; acc += g2 * t.sig[ilo + c] * t.sig[ilo + c + d]; }
-      pre[ncell] = acc;
-    }
-    // ---- (A) closed elements Q_{j,i} = chi-hat_{i,j}(Q_{i+1,j-1}) of the step's cells (eq 3.8), one warp per cell ------------------------
-    for (int c = warp; c < ncell; c += TM_WARPS) {
-      const int i = ilo + c, j = i + d;
-      const int si = t.sig[i], sj = t.sig[j], mi = g * si, mj = g * sj;
-      double* ct = t.CT + (size_t)t.off[j] * S + t.off[i];
-      if (d == 1) {
-        // unpaired base i:  sum_x T_i[x] (x) V[x]
-        const double* Ti = t.T + (size_t)i * 4 * MS2;
-        for (int e = lane; e < mi * mj; e += 32) {
-          const int al = e / mj, de = e - al * mj, sa = al / g, za = al - sa * g, sd = de / g, zd = de - sd * g;
-          double v = 0.0;
-#pragma unroll
-          for (int x = 0; x < 4; ++x) v += Ti[x * MS2 + sa * MS + sd] * t.V[x * g2 + za * g + zd];
-          ct[(size_t)de * S + al] = v;
+      int ao = 0, ax = 0, at = 0, am = 0, ab = 0;
+      for (int c = 0; c < ncell; ++c) {
+        const int i = ilo + c, j = i + d;
+        pre[c] = ao; prx[c] = ax; prt[c] = at; prm[c] = am; prb[c] = ab;
+        ao += g2 * t.sig[i] * t.sig[j];
+        ab += ((g * t.sig[i] + 3) >> 2) * ((g * t.sig[j] + 3) >> 2);  // 4 x 4 output tiles of phase B
+        if (pairs) {
+          ax += g * t.sig[i + 1] * (g * t.sig[j - 1] + 1);  // rows padded by one
+          at += npx * t.sig[i + 1] * t.sig[j - 1];
+          am += npx * t.sig[i] * t.sig[j];
         }
-      } else if (d - 2 >= t.mh) {
-        // base pair i.(j-1) around the block X = Q_{i+1,j-1}
-        const int l = j - 1, s1 = t.sig[i + 1], s2 = t.sig[l];
-        const double* X = t.U + (size_t)t.off[i + 1] * S + t.off[l];
-        const double* Ti = t.T + (size_t)i * 4 * MS2;
-        const double* Tl = t.T + (size_t)l * 4 * MS2;
-        // 1: t[pr][rho][a'][c'] = Tr_S[ B_{j,i}^rho X^{a',c'} ] = sum_{c,d} SB[y][x][rho][d][c] X[(a',c)][(c',d)]
-        for (int e = lane; e < t.npair * xi * s1 * s2; e += 32) {
-          const int c1 = e % s2, a1 = (e / s2) % s1, rho = (e / (s1 * s2)) % xi, pr = e / (s1 * s2 * xi);
-          const double* sb = t.SB + (size_t)((t.py[pr] * 4 + t.px[pr]) * xi + rho) * g2;
-          const double* xb = X + (size_t)(a1 * g) * S + c1 * g;
-          double v = 0.0;
-          for (int cc = 0; cc < g; ++cc)
-            for (int dd = 0; dd < g; ++dd) v += sb[dd * g + cc] * xb[(size_t)cc * S + dd];
-          tW[e] = v;
-        }
-        __syncwarp();
-        // 2: m[pr][rho][sa][sd] = sum_{a',c'} T_i[x][sa][a'] t[pr][rho][a'][c'] T_l[y][c'][sd]
-        for (int e = lane; e < t.npair * xi * si * sj; e += 32) {
-          const int sd = e % sj, sa = (e / sj) % si, rho = (e / (si * sj)) % xi, pr = e / (si * sj * xi);
-          const double* ti = Ti + t.px[pr] * MS2 + sa * MS;
-          const double* tl = Tl + t.py[pr] * MS2 + sd;
-          const double* tw = tW + (size_t)(pr * xi + rho) * s1 * s2;
-          double v = 0.0;
-          for (int a1 = 0; a1 < s1; ++a1) {
-            const double ta = ti[a1];
-            if (ta == 0.0) continue;
-            double s = 0.0;
-            for (int c1 = 0; c1 < s2; ++c1) s += tw[a1 * s2 + c1] * tl[c1 * MS];
-            v += ta * s;
-          }
-          mW[e] = v;
-        }
-        __syncwarp();
-        // 3: C[(sa,za)][(sd,zd)] = sum_{pr,rho} B[x][y][rho][za][zd] m[pr][rho][sa][sd]
-        for (int e = lane; e < mi * mj; e += 32) {
-          const int al = e / mj, de = e - al * mj, sa = al / g, za = al - sa * g, sd = de / g, zd = de - sd * g;
-          double v = 0.0;
-          for (int pr = 0; pr < t.npair; ++pr)
-            for (int rho = 0; rho < xi; ++rho)
-              v += t.B[(size_t)((t.px[pr] * 4 + t.py[pr]) * xi + rho) * g2 + za * g + zd] * mW[((pr * xi + rho) * si + sa) * sj + sd];
-          ct[(size_t)de * S + al] = v;
-        }
-        __syncwarp();
       }
-      // spans 2 .. min_hairpin + 1 close nothing: the zero-initialised table entry stands (line 483)
+      pre[ncell] = ao; prx[ncell] = ax; prt[ncell] = at; prm[ncell] = am; prb[ncell] = ab;
     }
     __syncthreads();
-    // ---- (B) Q_{i,j} = sum_{k in [i:j)} Q_{i,k} Q_{j,k}^T: the partial tiles of the GEMM + the bonds of block I from i on + those of block J before j ----
-    const int total = pre[ncell];
-    for (int it = tid; it < total; it += TM_THREADS) {
-      int c = 0;
-      while (pre[c + 1] <= it) ++c;
-      const int i = ilo + c, j = i + d, mj = g * t.sig[j];
-      const int e = it - pre[c], al = e / mj, de = e - al * mj;
-      const int ri = t.off[i] + al, rj = t.off[j] + de;
-      const double* ru = t.U + (size_t)ri * S;
-      const double* rc = t.CT + (size_t)rj * S;
-      double v = 0.0;
-      for (int sp = 0; sp < nsplit; ++sp)
-        v += t.GP[((size_t)I * nsplit + sp) * (CDZ_TB * CDZ_TB) + (size_t)(ri - I * CDZ_TB) * CDZ_TB + (rj - J * CDZ_TB)];
-      if (I == J) {
-        for (int kb = t.off[i]; kb < t.off[j]; ++kb) v += ru[kb] * rc[kb];
-      } else {
-        for (int kb = t.off[i]; kb < (I + 1) * CDZ_TB; ++kb) v += ru[kb] * rc[kb];
-        for (int kb = J * CDZ_TB; kb < t.off[j]; ++kb) v += ru[kb] * rc[kb];
+    // ---- (A) closed elements Q_{j,i} = chi-hat_{i,j}(Q_{i+1,j-1}) of the step's cells (eq 3.8); every stage spread over the whole CTA ----
+    if (d == 1) {
+      // unpaired base i:  sum_x T_i[x] (x) V[x]
+      for (int it = tid; it < pre[ncell]; it += TM_THREADS) {
+        int c;
+        const int e = cell_of(pre, it, c), i = ilo + c, j = i + 1, mj = g * t.sig[j];
+        const int al = e / mj, de = e - al * mj, sa = al / g, za = al - sa * g, sd = de / g, zd = de - sd * g;
+        const double* Ti = t.T + (size_t)i * 4 * MS2;
+        double v = 0.0;
+#pragma unroll
+        for (int x = 0; x < 4; ++x) v += Ti[x * MS2 + sa * MS + sd] * t.V[x * g2 + za * g + zd];
+        t.CT[(size_t)(t.off[j] + de) * S + t.off[i] + al] = v;
       }
-      t.U[(size_t)ri * S + rj] = v;
+    } else if (pairs) {
+      // base pair i.(j-1) around the block X = Q_{i+1,j-1}
+      // 0: stage every X (coalesced rows) into shared memory
+      for (int it = tid; it < prx[ncell]; it += TM_THREADS) {
+        int c;
+        const int e = cell_of(prx, it, c), i = ilo + c, l = i + d - 1, ld = g * t.sig[l] + 1;
+        const int r = e / ld, cc = e - r * ld;
+        if (cc < ld - 1) xP[it] = t.U[(size_t)(t.off[i + 1] + r) * S + t.off[l] + cc];
+      }
+      __syncthreads();
+      // 1: t[pr][rho][a'][c'] = Tr_S[ B_{j,i}^rho X^{a',c'} ] = sum_{c,d} SB[y][x][rho][d][c] X[(a',c)][(c',d)]
+      for (int it = tid; it < prt[ncell]; it += TM_THREADS) {
+        int c;
+        const int e = cell_of(prt, it, c), i = ilo + c, l = i + d - 1, s1 = t.sig[i + 1], s2 = t.sig[l], ld = g * s2 + 1;
+        const int c1 = e % s2, a1 = (e / s2) % s1, rho = (e / (s1 * s2)) % xi, pr = e / (s1 * s2 * xi);
+        const double* sb = t.SB + (size_t)((t.py[pr] * 4 + t.px[pr]) * xi + rho) * g2;
+        const double* xb = xP + prx[c] + (a1 * g) * ld + c1 * g;
+        double v = 0.0;
+        for (int cc = 0; cc < g; ++cc)
+#pragma unroll 4
+          for (int dd = 0; dd < g; ++dd) v += sb[dd * g + cc] * xb[cc * ld + dd];
+        tP[it] = v;
+      }
+      __syncthreads();
+      // 2: m[pr][rho][sa][sd] = sum_{a',c'} T_i[x][sa][a'] t[pr][rho][a'][c'] T_l[y][c'][sd]
+      for (int it = tid; it < prm[ncell]; it += TM_THREADS) {
+        int c;
+        const int e = cell_of(prm, it, c), i = ilo + c, j = i + d, l = j - 1;
+        const int si = t.sig[i], sj = t.sig[j], s1 = t.sig[i + 1], s2 = t.sig[l];
+        const int sd = e % sj, sa = (e / sj) % si, rho = (e / (si * sj)) % xi, pr = e / (si * sj * xi);
+        const double* ti = t.T + (size_t)i * 4 * MS2 + t.px[pr] * MS2 + sa * MS;
+        const double* tl = t.T + (size_t)l * 4 * MS2 + t.py[pr] * MS2 + sd;
+        const double* tw = tP + prt[c] + (pr * xi + rho) * s1 * s2;
+        double v = 0.0;
+        for (int a1 = 0; a1 < s1; ++a1) {
+          const double ta = ti[a1];
+          double sm = 0.0;
+#pragma unroll 2
+          for (int c1 = 0; c1 < s2; ++c1) sm += tw[a1 * s2 + c1] * tl[c1 * MS];
+          v += ta * sm;
+        }
+        mP[it] = v;
+      }
+      __syncthreads();
+      // 3: C[(sa,za)][(sd,zd)] = sum_{pr,rho} B[x][y][rho][za][zd] m[pr][rho][sa][sd]
+      for (int it = tid; it < pre[ncell]; it += TM_THREADS) {
+        int c;
+        const int e = cell_of(pre, it, c), i = ilo + c, j = i + d, si = t.sig[i], sj = t.sig[j], mj = g * sj;
+        const int al = e / mj, de = e - al * mj, sa = al / g, za = al - sa * g, sd = de / g, zd = de - sd * g;
+        const double* mw = mP + prm[c] + sa * sj + sd;
+        double v = 0.0;
+        for (int pr = 0; pr < t.npair; ++pr)
+          for (int rho = 0; rho < xi; ++rho)
+            v += t.B[(size_t)((t.px[pr] * 4 + t.py[pr]) * xi + rho) * g2 + za * g + zd] * mw[(pr * xi + rho) * si * sj];
+        t.CT[(size_t)(t.off[j] + de) * S + t.off[i] + al] = v;
+      }
+    }
+    // spans 2 .. min_hairpin + 1 close nothing: the zero-initialised table entry stands (line 483)
+    __syncthreads();
+    // ---- (B) Q_{i,j} = sum_{k in [i:j)} Q_{i,k} Q_{j,k}^T: the partial tiles of the GEMM + the bonds of block I from i on + those of block J before j.
+    //      4 x 4 output tiles, 8 lanes per tile striding the contiguous bond range (coalesced 64-byte row segments), butterfly over the 8 lanes ----
+    {
+      const int sub = tid & 7;
+      const unsigned gmask = 0xFFu << (tid & 24);
+      for (int tile = tid >> 3; tile < prb[ncell]; tile += TM_THREADS / 8) {
+        int c;
+        const int e = cell_of(prb, tile, c), i = ilo + c, j = i + d, mi = g * t.sig[i], mj = g * t.sig[j];
+        const int tbn = (mj + 3) >> 2, al0 = (e / tbn) * 4, de0 = (e % tbn) * 4;
+        const double* ru = t.U + (size_t)(t.off[i] + al0) * S;
+        const double* rc = t.CT + (size_t)(t.off[j] + de0) * S;
+        const int nr = min(4, mi - al0), nc = min(4, mj - de0);
+        // rows beyond the cell (nr, nc < 4) are read from row 0 of the tile and discarded
+        const size_t o1 = nr > 1 ? S : 0, o2 = nr > 2 ? 2 * S : 0, o3 = nr > 3 ? 3 * S : 0;
+        const size_t p1 = nc > 1 ? S : 0, p2 = nc > 2 ? 2 * S : 0, p3 = nc > 3 ? 3 * S : 0;
+        double acc[4][4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+          for (int q = 0; q < 4; ++q) acc[r][q] = 0.0;
+        auto range = [&](int lo, int hi) {
+#pragma unroll 2
+          for (int kb = lo + sub; kb < hi; kb += 8) {
+            const double u0 = ru[kb], u1 = ru[o1 + kb], u2 = ru[o2 + kb], u3 = ru[o3 + kb];
+            const double c0 = rc[kb], c1 = rc[p1 + kb], c2 = rc[p2 + kb], c3 = rc[p3 + kb];
+            acc[0][0] += u0 * c0; acc[0][1] += u0 * c1; acc[0][2] += u0 * c2; acc[0][3] += u0 * c3;
+            acc[1][0] += u1 * c0; acc[1][1] += u1 * c1; acc[1][2] += u1 * c2; acc[1][3] += u1 * c3;
+            acc[2][0] += u2 * c0; acc[2][1] += u2 * c1; acc[2][2] += u2 * c2; acc[2][3] += u2 * c3;
+            acc[3][0] += u3 * c0; acc[3][1] += u3 * c1; acc[3][2] += u3 * c2; acc[3][3] += u3 * c3;
+          }
+        };
+        if (I == J) {
+          range(t.off[i], t.off[j]);
+        } else {
+          range(t.off[i], (I + 1) * CDZ_TB);
+          range(J * CDZ_TB, t.off[j]);
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            double v = acc[r][q];
+            v += __shfl_xor_sync(gmask, v, 1);
+            v += __shfl_xor_sync(gmask, v, 2);
+            v += __shfl_xor_sync(gmask, v, 4);
+            acc[r][q] = v;
+          }
+        // lane `sub` finishes the two entries (r, 2 (sub & 1)) and (r, 2 (sub & 1) + 1), r = sub >> 1
+        const int r = sub >> 1;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int q = 2 * (sub & 1) + h;
+          double v = 0.0;
+#pragma unroll
+          for (int rr = 0; rr < 4; ++rr)
+#pragma unroll
+            for (int qq = 0; qq < 4; ++qq) v = (rr == r && qq == q) ? acc[rr][qq] : v;
+          if (r < nr && q < nc) {
+            const int ri = t.off[i] + al0 + r, rj = t.off[j] + de0 + q;
+            for (int sp = 0; sp < nsplit; ++sp)
+              v += t.GP[((size_t)I * nsplit + sp) * (CDZ_TB * CDZ_TB) + (size_t)(ri - I * CDZ_TB) * CDZ_TB + (rj - J * CDZ_TB)];
+            t.U[(size_t)ri * S + rj] = v;
+          }
+        }
+      }
     }
     __syncthreads();
   }
@@ -216,7 +291,10 @@ int tm_check(const cdz_tm_params* p, const cdz_tt* tt) {
     if (!std::isfinite(p->V[k]) || p->V[k] < 0) { cdz_set_error("cdz_tm: V must be finite and non-negative"); return CDZ_EINVAL; }
   for (int k = 0; k < g2; ++k)
     if (!std::isfinite(p->S[k]) || p->S[k] < 0) { cdz_set_error("cdz_tm: S must be finite and non-negative"); return CDZ_EINVAL; }
-  if (npair * p->xi * tt->MS * tt->MS > TM_WSCR) { cdz_set_error("cdz_tm: pairs x xi x bond^2 exceeds the per-warp scratch (512)"); return CDZ_EINVAL; }
+  if ((long long)npair * p->xi * tt->MS * (96 / p->gamma) > TM_POOL) {
+    cdz_set_error("cdz_tm: pairs x xi x bond x (96 / gamma) exceeds the shared pool (6144)");
+    return CDZ_EINVAL;
+  }
   return CDZ_OK;
 }
 
@@ -259,17 +337,20 @@ TmLayout tm_layout(const cdz_tm_params* p, const cdz_tt* tt, int n) {
   return L;
 }
 
-// one pass over the first n positions with all operator weights times 2^-e; Z_stored to *z_out (host), device time to *ms (may be NULL)
-int tm_pass(const cdz_tm_params* p, const cdz_tt* tt, int n, int e, char* base, cudaStream_t st, double* z_out, cdz_tm_info* info) {
+inline long long tm_P(int q, double rate) { return (long long)floor((double)q * rate); }
+
+// one pass over the first n positions, the operator weights of position q times 2^-(P[q+1] - P[q]); Z_stored to *z_out (host)
+int tm_pass(const cdz_tm_params* p, const cdz_tt* tt, int n, double rate, char* base, cudaStream_t st, double* z_out, cdz_tm_info* info) {
   const TmLayout L = tm_layout(p, tt, n);
   const int g = p->gamma, g2 = g * g, xi = p->xi, MS = L.MS, MS2 = MS * MS;
   std::vector<double> T((size_t)std::max(1, n) * 4 * MS2, 0.0), SB((size_t)16 * xi * g2, 0.0);
-  const double sc = ldexp(1.0, -e);
-  for (int q = 0; q < n; ++q)
+  for (int q = 0; q < n; ++q) {
+    const double sc = ldexp(1.0, -(int)(tm_P(q + 1, rate) - tm_P(q, rate)));
     for (int z = tt->opstart[q]; z < tt->opstart[q + 1]; ++z) {
       const cdz_op& o = tt->ops[z];
       T[((size_t)q * 4 + o.b) * MS2 + o.a * MS + o.c] += o.x * sc;
     }
+  }
   for (int xy = 0; xy < 16; ++xy)
     for (int r = 0; r < xi; ++r)
       for (int d = 0; d < g; ++d)
@@ -342,7 +423,7 @@ int tm_pass(const cdz_tm_params* p, const cdz_tt* tt, int n, int e, char* base, 
     info->launches = launches;
     info->S = L.S;
     info->NB = L.NB;
-    info->scale_exponent = e;
+    info->scale_rate = rate;
     info->table_bytes = (double)(2 * sizeof(double)) * L.S * L.S;
   }
   return CDZ_OK;
@@ -379,24 +460,25 @@ extern "C" int cdz_tm_inside(const cdz_tm_params* p, const cdz_tt* tt, void* wor
     cdz_set_error("cdz_tm_inside: workspace too small (cdz_tm_workspace_bytes)");
     return CDZ_EINVAL;
   }
-  // pilot pass over a prefix: the growth rate of the partition function per position, in bits
-  int e = 0;
-  double z = 0.0;
-  if (n > TM_PILOT) {
-    rc = tm_pass(p, tt, TM_PILOT, 0, base, st, &z, nullptr);
+  // pilot passes over prefixes: the growth rate of log2 Z per position (the second pilot, run with the rate of the first, pins it to
+  // ~1e-2 bits per position, i.e. well inside the fp64 exponent range at 15000 nt)
+  double rate = 0.0, z = 0.0;
+  for (int np : {TM_PILOT, 10 * TM_PILOT}) {
+    if (rc != CDZ_OK || n <= np) break;
+    rc = tm_pass(p, tt, np, rate, base, st, &z, nullptr);
     if (rc == CDZ_OK && (!(z > 0.0) || !std::isfinite(z))) { cdz_set_error("cdz_tm_inside: pilot pass left the fp64 range"); rc = CDZ_EOVERFLOW; }
-    if (rc == CDZ_OK) e = (int)lround(log2(z) / TM_PILOT);
+    if (rc == CDZ_OK) rate = (log2(z) + (double)tm_P(np, rate)) / np;
   }
-  if (rc == CDZ_OK) rc = tm_pass(p, tt, n, e, base, st, &z, info);
+  if (rc == CDZ_OK) rc = tm_pass(p, tt, n, rate, base, st, &z, info);
   if (rc == CDZ_OK && (!(z > 0.0) || !std::isfinite(z))) { cdz_set_error("cdz_tm_inside: partition function left the fp64 range"); rc = CDZ_EOVERFLOW; }
-  if (rc == CDZ_OK) *logZ_host = log(z) + (double)e * n * M_LN2;
+  if (rc == CDZ_OK) *logZ_host = log(z) + (double)tm_P(n, rate) * M_LN2;
   if (own) cudaFree(base);
   return rc;
 }
 
 // parity access after cdz_tm_inside with a caller workspace: which = 0 the upper block Q_{i,j} (i <= j) as [gamma Sigma_i][gamma Sigma_j],
 // which = 1 the lower block Q_{j,i} (j > i) as [gamma Sigma_j][gamma Sigma_i]; true value = stored * 2^shift
-extern "C" int cdz_tm_block(const cdz_tm_params* p, const cdz_tt* tt, const void* workspace_dev, int scale_exponent, int which, int i,
+extern "C" int cdz_tm_block(const cdz_tm_params* p, const cdz_tt* tt, const void* workspace_dev, double scale_rate, int which, int i,
                             int j, double* out_host, int* shift_out) {
   const int rc = tm_check(p, tt);
   if (rc != CDZ_OK) return rc;
@@ -415,6 +497,6 @@ extern "C" int cdz_tm_block(const cdz_tm_params* p, const cdz_tt* tt, const void
     CDZ_CUDA(cudaMemcpy2D(out_host, sizeof(double) * mi, base + L.o_CT + sizeof(double) * ((size_t)L.off[j] * L.S + L.off[i]),
                           sizeof(double) * L.S, sizeof(double) * mi, mj, cudaMemcpyDeviceToHost));
   }
-  if (shift_out) *shift_out = scale_exponent * (j - i);
+  if (shift_out) *shift_out = (int)(tm_P(j, scale_rate) - tm_P(i, scale_rate));
   return which == 0 ? mi * mj : mj * mi;
 }

@@ -106,7 +106,7 @@ def test_unit_model_large_closed_form(B, I):
     tg = B.TensorTrain.build(aa, I.TT_SINGLE_CODON, None, None)
     run = B.TensorModelPass(tm, tg)
     ref = sum(math.log(deg[a]) for a in aa) + _log_structure_count(3 * len(aa))
-    assert run.info.NB >= 50 and run.info.scale_exponent != 0
+    assert run.info.NB >= 50 and run.info.scale_rate != 0.0
     assert abs(run.logZ - ref) <= 1e-9 * ref, (run.logZ, ref)
 
 
@@ -141,7 +141,7 @@ def test_prefix_chain_config2(B, I):
     tm = I.tensor_model(4, 2)
     tg = B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
     run = B.TensorModelPass(tm, tg)
-    assert math.isfinite(run.logZ) and run.info.scale_exponent != 0
+    assert math.isfinite(run.logZ) and run.info.scale_rate != 0.0
     sigma, ops = O.TT.build(d.aa[:12], d.kind, d.codon_logw, d.pair_logw).get()
     _, Q = TM.tm_inside(tm, sigma, ops, return_Q=True)
     for (i, j) in ((0, 36), (0, 20), (7, 33), (3, 4), (12, 35)):
