@@ -523,13 +523,84 @@ def run_batch(args):
     print(json.dumps(out), flush=True)
 
 
+def run_tensor_model(args):
+    """Secondary measurement: the paper's own recursion -- tensor-based model (gamma, xi synthetic) x codon tensor train of a
+    BASELINE design -- through cdz_tm_inside.  One step = one full call (pilot passes, table clear, all block diagonals, final trace)."""
+    import time
+
+    import torch
+
+    from paper_2604_19718_b200 import binding as B
+    from paper_2604_19718_b200 import build
+    from paper_2604_19718_b200 import inputs as I
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the library has no CPU fallback)")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    build.build()
+    cfg = args.config if args.config != 4 or args.L else 3  # default workload of this mode: configs[2], 1000 aa, codon-pair tensor train
+    d = I.design(cfg, 0, args.L)
+    tm = I.tensor_model(args.gamma, args.xi)
+    tt = B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
+    run = B.TensorModelPass(tm, tt)
+    for _ in range(max(args.warmup, 3) - 1):
+        run.rerun()
+    clocks = ClockSampler(0)
+    clocks.start()
+    dev, gemm, block, wall = [], [], [], []
+    for _ in range(args.steps):
+        t0 = time.perf_counter()
+        run.rerun()
+        wall.append((time.perf_counter() - t0) * 1e3)
+        dev.append(run.info.device_ms); gemm.append(run.info.gemm_ms); block.append(run.info.block_ms)
+    clk = clocks.stop()
+    ms, gms, bms, wms = (sum(v) / len(v) for v in (dev, gemm, block, wall))
+    peak = measure_peak(1)
+    i = run.info
+    sig = tt.describe()[0]
+    flat = args.gamma * sum(sig)
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import oracle as O
+        from oracle import tensor_model as TM
+
+        Ls = 16
+        so, oo = O.TT.build(d.aa[:Ls], d.kind, d.codon_logw, d.pair_logw).get()
+        t0 = time.perf_counter()
+        TM.tm_inside(tm, so, oo)
+        sec = time.perf_counter() - t0
+        cpu = {"value": sec * 1e3, "unit": "ms", "cores": 1, "kind": "oracle",
+               "sample": f"oracle/tensor_model.py tm_inside (plain numpy Alg S4.1) on the first {Ls} aa ({3 * Ls} nt) of the same design: {sec:.1f} s; "
+                         "cost grows as n^3, not comparable with the full-size GPU time"}
+    out = {
+        "metric": "tensor-model partition function (PAPER.md eqs 3.5-3.8), device time of one full pass", "value": ms, "unit": "ms",
+        "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"configs[{cfg - 1}] design ({len(d.aa)} aa, {d.n} nt, {'codon-pair' if d.kind else 'single-codon'} tensor train) under a "
+                               f"synthetic tensor model gamma={args.gamma} xi={args.xi}", "n_nt": d.n, "flattened_dim": flat, "padded_dim": i.S,
+                   "blocks": i.NB, "l2": f"tables ({i.table_bytes / 1e9:.1f} GB) larger than L2" if i.table_bytes > 126e6 else "tables fit L2"},
+        "logZ": run.logZ, "scale_rate_bits_per_nt": i.scale_rate, "gemm_ms": gms, "block_ms": bms, "gpu_launches": int(i.launches),
+        "roofline": {"kernel": "tm_gemm_kernel (k-sum over finished blocks, fp64 mma.sync m8n8k4 tiles shared with the inside pass)",
+                     "bound": "tensor", "achieved": i.gemm_flop / (gms * 1e-3) / 1e12 if gms > 0 else None, "peak": peak, "unit": "TFLOP/s",
+                     "frac": (i.gemm_flop / (gms * 1e-3) / 1e12 / peak) if gms > 0 else None, "traffic": None,
+                     "launches": int(i.gemm_launches), "flop_per_step": i.gemm_flop,
+                     "note": "FLOP of the 64-padded tiles; the unpadded flattened dimension is config.flattened_dim",
+                     "peak_source": "in-run register-resident mma.sync.m8n8k4.f64 loop (libcdz_peak.so)", "share_of_step": gms / ms},
+        "cpu_baseline": cpu,
+        "e2e": {"value": wms, "unit": "ms", "h2d_bytes_per_step": int(8 * 4 * d.n * max(sig) ** 2), "d2h_bytes_per_step": 8,
+                "timed_region": "host wall clock of cdz_tm_inside: dense cores built on the host and copied, two pilot passes, the full pass, log Z read back"},
+        "clocks": clk,
+    }
+    print(json.dumps(out), flush=True)
+
+
 def kernel_source_hash() -> str:
     import hashlib
 
     h = hashlib.sha256()
     csrc = os.path.join(ROOT, "paper_2604_19718_b200", "csrc")
     for name in sorted(os.listdir(csrc)):
-        if name.endswith((".cu", ".h")):
+        if name.endswith((".cu", ".h", ".cuh")):
             h.update(open(os.path.join(csrc, name), "rb").read())
     return h.hexdigest()[:16]
 
@@ -566,9 +637,14 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--marginals", action="store_true", help="also time cdz_marginals (base-pair probabilities) after the timed steps")
     ap.add_argument("--batch", type=int, default=0, help="configs[4]: number of independent 150-aa designs advanced together")
+    ap.add_argument("--tensor-model", action="store_true", dest="tensor_model", help="time cdz_tm_inside (the paper's tensor-model recursion, f-4)")
+    ap.add_argument("--gamma", type=int, default=4)
+    ap.add_argument("--xi", type=int, default=2)
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.tensor_model:
+        run_tensor_model(args)
     elif args.batch > 0:
         run_batch(args)
     else:

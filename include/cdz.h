@@ -238,9 +238,11 @@ typedef struct {
 } cdz_tm_params;
 typedef struct {
   double device_ms;        /* device time of the full-size pass (CUDA events on `stream`: table clear, all block diagonals, final trace) */
+  double gemm_ms;          /* of which: the tensor-core tile kernels (tm_gemm_kernel) */
+  double block_ms;         /* of which: the per-block kernels (chi-hat + in-block edges, tm_block_kernel) */
   double gemm_flop;        /* FLOP of the tensor-core tiles: 2 x 64^3 x (number of K blocks), padding included */
   double table_bytes;      /* the two S x S tables */
-  int64_t launches;
+  int64_t launches, gemm_launches;
   int32_t S, NB;           /* flattened (block-padded) dimension sum_i gamma Sigma_i and its number of 64-blocks */
   double scale_rate;       /* r: the operator weights of position q were multiplied by 2^-(P[q+1] - P[q]), P[q] = floor(q r); log Z = log Z_stored + P[n] ln 2 */
 } cdz_tm_info;

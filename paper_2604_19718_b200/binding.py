@@ -63,7 +63,8 @@ class TMParams(C.Structure):
 
 
 class TMInfo(C.Structure):
-    _fields_ = [("device_ms", C.c_double), ("gemm_flop", C.c_double), ("table_bytes", C.c_double), ("launches", C.c_int64),
+    _fields_ = [("device_ms", C.c_double), ("gemm_ms", C.c_double), ("block_ms", C.c_double), ("gemm_flop", C.c_double),
+                ("table_bytes", C.c_double), ("launches", C.c_int64), ("gemm_launches", C.c_int64),
                 ("S", C.c_int32), ("NB", C.c_int32), ("scale_rate", C.c_double)]
 
 

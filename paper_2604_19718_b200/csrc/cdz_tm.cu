@@ -388,37 +388,58 @@ int tm_pass(const cdz_tm_params* p, const cdz_tt* tt, int n, double rate, char* 
   CDZ_CUDA(cudaMemcpyAsync(base + L.o_off, L.off.data(), sizeof(int) * (n + 2), cudaMemcpyHostToDevice, st));
   CDZ_CUDA(cudaMemcpyAsync(base + L.o_blk, L.blk.data(), sizeof(int) * (L.NB + 1), cudaMemcpyHostToDevice, st));
   CDZ_CUDA(cudaStreamSynchronize(st));  // the staging vectors above are pageable host memory about to go out of scope
-  cudaEvent_t e0 = nullptr, e1 = nullptr;
-  if (info) { CDZ_CUDA(cudaEventCreate(&e0)); CDZ_CUDA(cudaEventCreate(&e1)); CDZ_CUDA(cudaEventRecord(e0, st)); }
+  // with info: one event before every launch group, so that consecutive pairs give the device time of the GEMMs and of the block kernels
+  std::vector<cudaEvent_t> evs;
+  std::vector<int> cls;  // 0 clear / init / final, 1 gemm, 2 block
+  auto mark = [&](int c) {
+    if (!info) return;
+    cudaEvent_t ev;
+    cudaEventCreate(&ev);
+    cudaEventRecord(ev, st);
+    evs.push_back(ev);
+    cls.push_back(c);
+  };
+  mark(0);
   CDZ_CUDA(cudaMemsetAsync(t.U, 0, sizeof(double) * (size_t)L.S * L.S, st));
   CDZ_CUDA(cudaMemsetAsync(t.CT, 0, sizeof(double) * (size_t)L.S * L.S, st));
   CDZ_CUDA(cudaFuncSetAttribute(tm_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
   CDZ_CUDA(cudaFuncSetAttribute(tm_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TM_BLOCK_SMEM));
   tm_init_kernel<<<32, 256, 0, st>>>(t);
-  long launches = 3;
+  long launches = 3, gemm_launches = 0;
   double flop = 0.0;
   for (int D = 0; D < L.NB; ++D) {
     const int nblk = L.NB - D, nsplit = cdz_nsplit(L.NB, D, 1);
     if (nsplit > 0) {
+      mark(1);
       tm_gemm_kernel<<<nblk * nsplit, GEMM_THREADS, GEMM_SMEM, st>>>(t, D, nsplit);
       flop += 2.0 * nblk * (double)(D - 1) * CDZ_TB * CDZ_TB * CDZ_TB;
       ++launches;
+      ++gemm_launches;
     }
+    mark(2);
     tm_block_kernel<<<nblk, TM_THREADS, TM_BLOCK_SMEM, st>>>(t, D, nsplit);
     ++launches;
   }
+  mark(0);
   tm_final_kernel<<<1, 32, 0, st>>>(t);
   ++launches;
-  if (info) CDZ_CUDA(cudaEventRecord(e1, st));
+  mark(0);
   CDZ_CUDA(cudaMemcpyAsync(z_out, t.result, sizeof(double), cudaMemcpyDeviceToHost, st));
   CDZ_CUDA(cudaStreamSynchronize(st));
   CDZ_CUDA(cudaGetLastError());
   if (info) {
-    float ms = 0.f;
-    CDZ_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    info->device_ms = ms;
+    double tot = 0.0, by[3] = {0.0, 0.0, 0.0};
+    for (size_t k = 0; k + 1 < evs.size(); ++k) {
+      float ms = 0.f;
+      CDZ_CUDA(cudaEventElapsedTime(&ms, evs[k], evs[k + 1]));
+      by[cls[k]] += ms;
+      tot += ms;
+    }
+    for (cudaEvent_t ev : evs) cudaEventDestroy(ev);
+    info->device_ms = tot;
+    info->gemm_ms = by[1];
+    info->block_ms = by[2];
+    info->gemm_launches = gemm_launches;
     info->gemm_flop = flop;
     info->launches = launches;
     info->S = L.S;
