@@ -29,6 +29,11 @@ namespace {
 
 struct PosMeta { int off, sig, loff, nL, roff, nR, ops, nuc; };  // 32 bytes per position of a window; nuc = bit mask of the nucleotides possible there
 
+// boundary states of one position packed 4 bits each (|L_i|, |R_j| <= 16; bonds < 8, nucleotides < 4): left states (a, x) in lsa / lsx, right states
+// (y, c) in rsy / rsc.  Entry k = (word >> 4 k) & 15: a register shift instead of a dependent global load in the serial loops of P1-P5.
+struct PosPk { unsigned long long lsa, lsx, rsy, rsc; };
+__device__ __forceinline__ int pk(unsigned long long w, int k) { return (int)(w >> (4 * k)) & 15; }
+
 // window of position records in shared memory; -DCDZ_CHECK (development) traps on an index outside the window
 struct MetaWin {
   PosMeta* p;
@@ -83,7 +88,7 @@ struct Plan {
   int nrow, ncol;        // window lengths (positions)
   int maxbond, maxls;    // compact row lists (bonds / left states of the row window)
   int ntl, ntr;          // positions with a dense TL / TR core
-  size_t o_rowm, o_colm, o_crow, o_rbpos, o_rlpos, o_rbp, o_cbp, o_tl, o_tr, o_xoff, o_xst, o_scr, total;
+  size_t o_rowm, o_colm, o_rowpk, o_colpk, o_crow, o_rbpos, o_rlpos, o_rbp, o_cbp, o_tl, o_tr, o_xoff, o_xst, o_scr, total;
 };
 // span: largest extent, in global (block-padded) bond indices, of a row / column window
 __host__ __device__ inline Plan make_plan(int maxpos, int span, const Dims& D, int C) {
@@ -98,6 +103,8 @@ __host__ __device__ inline Plan make_plan(int maxpos, int span, const Dims& D, i
   auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 15) & ~size_t(15); return r; };
   p.o_rowm = take(sizeof(PosMeta) * p.nrow);
   p.o_colm = take(sizeof(PosMeta) * p.ncol);
+  p.o_rowpk = take(sizeof(PosPk) * p.nrow);
+  p.o_colpk = take(sizeof(PosPk) * p.ncol);
   p.o_crow = take(sizeof(int) * (p.nrow + 1));
   p.o_rbpos = take(sizeof(short) * p.maxbond);
   p.o_rlpos = take(sizeof(short) * p.maxls);
@@ -229,6 +236,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   __shared__ CModel cm;
   __shared__ int pmx[16];  // nucleotide mask of position i -> mask of the nucleotides at j that can pair with one of them
   __shared__ int p1ctr[4];  // work counters of P1: warps take X cells / 32-slot chunks of the item loops as they become free
+  __shared__ double wsl[6][16];  // stack factor by (closing pair type, inner pair slot): wst[P][ptype(slot)]
   const Ctx& cx = ctxs[blockIdx.y];
   const DevTT& t = cx.tt;
   const DevTab& b = cx.tab;
@@ -239,6 +247,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   const Plan pl = make_plan(ka.maxpos, ka.span, dm, ka.C);
   MetaWin rowm{(PosMeta*)(smraw + pl.o_rowm), 0, 0};
   MetaWin colm{(PosMeta*)(smraw + pl.o_colm), 0, 1};
+  PosPk* rowpk = (PosPk*)(smraw + pl.o_rowpk);
+  PosPk* colpk = (PosPk*)(smraw + pl.o_colpk);
   int* crow = (int*)(smraw + pl.o_crow);
   short* rbpos = (short*)(smraw + pl.o_rbpos);
   short* rlpos = (short*)(smraw + pl.o_rlpos);
@@ -288,8 +298,26 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
     }
     return m;
   };
+  auto load_pk = [&](int p) {
+    PosPk w{0ull, 0ull, 0ull, 0ull};
+    if (p < n) {
+      const int l0 = t.loff[p], nl = t.loff[p + 1] - l0, r0 = t.roff[p], nr = t.roff[p + 1] - r0;
+      for (int l = 0; l < nl; ++l) {
+        w.lsa |= (unsigned long long)t.ls_a[l0 + l] << (4 * l);
+        w.lsx |= (unsigned long long)t.ls_x[l0 + l] << (4 * l);
+      }
+      for (int r = 0; r < nr; ++r) {
+        w.rsy |= (unsigned long long)t.rs_y[r0 + r] << (4 * r);
+        w.rsc |= (unsigned long long)t.rs_c[r0 + r] << (4 * r);
+      }
+    }
+    return w;
+  };
   for (int k = tid; k < nrp; k += NT) rowm[k] = load_meta(rbase + k);
   for (int k = tid; k < ncp; k += NT) colm[k] = load_meta(cbase + k);
+  // (the threads at the other end of the CTA take the packed descriptors, so that both run concurrently)
+  for (int k = NT - 1 - tid; k < nrp; k += NT) rowpk[k] = load_pk(rbase + k);
+  for (int k = NT - 1 - tid; k < ncp; k += NT) colpk[k] = load_pk(cbase + k);
   const int rkb0 = t.off[rbase], rkb1 = t.off[rend] + t.sig[rend];
   const int ckb0 = t.off[cbase], ckb1 = t.off[cend] + t.sig[cend];
   for (int k = tid; k < rkb1 - rkb0; k += NT) rbp[k] = (uint8_t)min(t.bondpos[rkb0 + k] - rbase, 255);
@@ -304,6 +332,10 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
         for (int y = 0; y < 4; ++y)
           if (cm.pslot[x * 4 + y] >= 0) pm |= 1 << y;
     pmx[tid] = pm;
+  }
+  if (tid >= 32 && tid < 32 + 96) {
+    const int P = (tid - 32) >> 4, s2 = (tid - 32) & 15;
+    wsl[P][s2] = s2 < cm.nps ? cm.wst[P][cm.ptype[cm.slot_x[s2] * 4 + cm.slot_y[s2]]] : 0.0;
   }
   if (tid == 0) {
     p1ctr[0] = p1ctr[1] = p1ctr[2] = 0;
@@ -350,10 +382,6 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
   __syncthreads();
 
   const int mh1 = cm.min_hairpin + 1, maxint = cm.max_interior;
-  const uint8_t* __restrict__ ls_a = t.ls_a;
-  const uint8_t* __restrict__ ls_x = t.ls_x;
-  const uint8_t* __restrict__ rs_y = t.rs_y;
-  const uint8_t* __restrict__ rs_c = t.rs_c;
   const double* __restrict__ Tbar = t.Tbar;
 
   // compact row ranges of the bond rows / left-state rows of positions [lo, hi] of the row window
@@ -377,7 +405,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
 #else
 #define CDZ_TICK(k)
 #endif
-  // dynamic distribution of the P1 work: lane 0 takes the next unit, the warp follows
+  // dynamic distribution of the P1 work: every warp starts with the unit of its own number (the counters start at the number of warps), then
+  // lane 0 takes the next unit and the warp follows
   auto grab = [&](int* c) {
     int w = 0;
     if ((tid & 31) == 0) w = atomicAdd(c, 1);
@@ -632,17 +661,19 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
               double s1 = 0.0, s2 = 0.0;
               if (r >= 0) {
                 const PosMeta mp1 = rowm[kp + 1];
+                const PosPk wp1 = rowpk[kp + 1];
                 for (int l2 = 0; l2 < mp1.nL; ++l2)
-                  if (ls_x[mp1.loff + l2] == xp)
-                    s1 += Tbar[(size_t)p * MS2 + a1 * MS + ls_a[mp1.loff + l2]] *
+                  if (pk(wp1.lsx, l2) == xp)
+                    s1 += Tbar[(size_t)p * MS2 + a1 * MS + pk(wp1.lsa, l2)] *
                           b.QB[(size_t)(mp1.loff + l2) * RS + mq.roff + r];
               }
               if (lst >= 0) {
                 const PosMeta mq1 = colm[q - 1 - cbase];
+                const PosPk wq1 = colpk[q - 1 - cbase];
                 for (int r2 = 0; r2 < mq1.nR; ++r2)
-                  if (rs_y[mq1.roff + r2] == yp)
+                  if (pk(wq1.rsy, r2) == yp)
                     s2 += b.QB[(size_t)(mp.loff + lst) * RS + mq1.roff + r2] *
-                          Tbar[(size_t)q * MS2 + rs_c[mq1.roff + r2] * MS + c1];
+                          Tbar[(size_t)q * MS2 + pk(wq1.rsc, r2) * MS + c1];
               }
               v += cm.wbu[1] * (s1 + s2);
             }
@@ -721,7 +752,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           const Scr sc = scr_of(scrb, dm, i - clo);
           double v = 0.0;
           if (closed) {
-            const int x = ls_x[rowm[kp].loff + lst], y = rs_y[mj.roff + r];
+            const int x = pk(rowpk[kp].lsx, lst), y = pk(colpk[j - cbase].rsy, r);
             if (cm.pslot[x * 4 + y] >= 0) {
               // Qb = sum_{a',c'} T_i[a,x,a'] T_j[c',y,c] inner[x,y;a',c'] with inner expanded in place (no per-slot table):
               //   inner = Bl + Br + sum_slots wst[P][P'] SB[a'][slot'][c']  +  sum_{(a',u),(v,c')} wtm[P][u][v] Y[(a',u)][(v,c')]
@@ -737,17 +768,17 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
                   const double tr = TRj[c1 * MR];
                   if (tr == 0.0) continue;
                   double s = sc.Bl[a1 * M + c1] + sc.Br[a1 * M + c1];
-                  for (int s2 = 0; s2 < nps; ++s2)
-                    s += cm.wst[P][cm.ptype[cm.slot_x[s2] * 4 + cm.slot_y[s2]]] * sc.SB[(a1 * nps + s2) * M + c1];
+                  for (int s2 = 0; s2 < nps; ++s2) s += wsl[P][s2] * sc.SB[(a1 * nps + s2) * M + c1];
                   v += tl * tr * s;
                 }
               }
+              const PosPk wp = rowpk[kp + 1], wq = colpk[j - 1 - cbase];
               for (int l = 0; l < mp.nL; ++l) {
-                const double tl = TLi[ls_a[mp.loff + l]];
+                const double tl = TLi[pk(wp.lsa, l)];
                 if (tl == 0.0) continue;
-                const int u = ls_x[mp.loff + l];
+                const int u = pk(wp.lsx, l);
                 double s = 0.0;
-                for (int k = 0; k < mq.nR; ++k) s += TRj[rs_c[mq.roff + k] * MR] * cm.wtm[P][u][rs_y[mq.roff + k]] * sc.Y[l * MR + k];
+                for (int k = 0; k < mq.nR; ++k) s += TRj[pk(wq.rsc, k) * MR] * cm.wtm[P][u][pk(wq.rsy, k)] * sc.Y[l * MR + k];
                 v += tl * s;
               }
             }
@@ -778,10 +809,11 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             const PosMeta mi = rowm[kp], mj = colm[j - cbase];
             const Scr sc = scr_of(scrb, dm, i - clo);
             double qbs = 0.0;
+            const unsigned long long wla = rowpk[kp].lsa, wrc = colpk[j - cbase].rsc;
             for (int l = 0; l < mi.nL; ++l)
-              if (ls_a[mi.loff + l] == a)
+              if (pk(wla, l) == a)
                 for (int k = 0; k < mj.nR; ++k)
-                  if (rs_c[mj.roff + k] == c) qbs += sc.QBc[l * MR + k];
+                  if (pk(wrc, k) == c) qbs += sc.QBc[l * MR + k];
             const double qm1 = cm.wc * qbs + sc.R1[a * M + c];
             const double qml = qm1 + sc.R2[a * M + c];
             const double m2 = sc.M2s[a * M + c];
@@ -800,19 +832,20 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             if (r >= mpj.nR) continue;
             const PosMeta mi = rowm[kp + 1], mj = colm[j - cbase];
             const Scr sc = scr_of(scrb, dm, i - clo);
-            const int up = ls_x[rowm[kp].loff + lst], vp = rs_y[mpj.roff + r];
+            const int up = pk(rowpk[kp].lsx, lst), vp = pk(colpk[pj - cbase].rsy, r);
+            const PosPk wi = rowpk[kp + 1], wj = colpk[j - cbase];
             const double* TLm = TLs + ((pi - tlbase) * ML + lst) * M;
             const double* TRp = TRs + (size_t)(pj - trbase) * M * MR + r;
             double v = 0.0;
             for (int l2 = 0; l2 < mi.nL; ++l2) {
-              const double tl = TLm[ls_a[mi.loff + l2]];
+              const double tl = TLm[pk(wi.lsa, l2)];
               if (tl == 0.0) continue;
-              const int x = ls_x[mi.loff + l2];
+              const int x = pk(wi.lsx, l2);
               double s = 0.0;
               for (int r2 = 0; r2 < mj.nR; ++r2) {
-                const int y = rs_y[mj.roff + r2];
+                const int y = pk(wj.rsy, r2);
                 if (cm.pslot[x * 4 + y] < 0) continue;
-                s += TRp[rs_c[mj.roff + r2] * MR] * cm.wtm[cm.ptype[y * 4 + x]][vp][up] * sc.QBc[l2 * MR + r2];
+                s += TRp[pk(wj.rsc, r2) * MR] * cm.wtm[cm.ptype[y * 4 + x]][vp][up] * sc.QBc[l2 * MR + r2];
               }
               v += tl * s;
             }
@@ -834,10 +867,11 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             const PosMeta mpj = colm[pj - cbase], mpj1 = colm[pj + 1 - cbase];
             const double* y = scr_of(scrb, dm, i - clo).Y + lst * MR;
             double* out = b.D1 + (size_t)(rowm[kp].loff + lst) * S + mpj1.off;
+            const unsigned long long wrc = colpk[pj - cbase].rsc;
             for (int c = 0; c < mpj1.sig; ++c) {
               double v = 0.0;
               for (int k = 0; k < mpj.nR; ++k)
-                if (rs_c[mpj.roff + k] == c) v += y[k];
+                if (pk(wrc, k) == c) v += y[k];
               out[c] = v;
             }
           } else {
@@ -847,8 +881,9 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             const double* y = scr_of(scrb, dm, i - clo).Y;
             // left states with bond a are contiguous in the (a, x)-sorted list
             int l0 = 0, l1 = 0;
+            const unsigned long long wla = rowpk[kp].lsa, wrc = colpk[pj - cbase].rsc;
             for (int l = 0; l < mpi.nL; ++l) {
-              const int la = ls_a[mpi.loff + l];
+              const int la = pk(wla, l);
               l0 += la < a;
               l1 += la <= a;
             }
@@ -859,7 +894,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
               double v = 0.0;
               for (int l = l0; l < l1; ++l) v += y[l * MR + k];
               b.D2T[(size_t)(mpj.roff + k) * S + mpi.off + a] = v;
-              const int c = rs_c[mpj.roff + k];
+              const int c = pk(wrc, k);
 #pragma unroll
               for (int cc = 0; cc < CDZ_MAX_BOND; ++cc) gi[cc] += cc == c ? v : 0.0;
             }
