@@ -960,7 +960,11 @@ int cdz_cell_config(cdz_tables* const* ts, int B, cdz_cell_cfg* cfg) {
       span = std::max(span, tt->off[cend] + tt->sigma[cend] - tt->off[cbase]);
     }
   }
-  const size_t budget = 225 * 1024;
+  // dynamic shared memory available to one CTA: the 227 KB opt-in limit minus the static shared memory of the kernel
+  cudaFuncAttributes fa0, fa1;
+  CDZ_CUDA(cudaFuncGetAttributes(&fa0, cell_kernel<0>));
+  CDZ_CUDA(cudaFuncGetAttributes(&fa1, cell_kernel<1>));
+  const size_t budget = 227 * 1024 - std::max(fa0.sharedSizeBytes, fa1.sharedSizeBytes) - 256;
   int C = maxpos;
   while (C > 1 && make_plan(maxpos, span, dm, C).total > budget) --C;
   const Plan pl = make_plan(maxpos, span, dm, C);
