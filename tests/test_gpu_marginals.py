@@ -76,10 +76,10 @@ def test_marginals_equal_oracle_tm1(B, O, aa, kind):
     _check_rules(aa, bg, sg, cg)
 
 
-@pytest.mark.parametrize("cfg,L", [(1, 8), (1, 13), (2, 9), (5, 8)])
+@pytest.mark.parametrize("cfg,L", [(1, 8), (1, 12), (2, 9), (5, 8)])
 def test_marginals_equal_oracle_baseline_prefixes(B, O, cfg, L):
-    """Prefixes of the BASELINE designs (NN model of configs[0]; single-codon and codon-pair TT): n = 24 .. 39 (the oracle takes O(n^2)
-    restricted inside passes: minutes at 39 nt)."""
+    """Prefixes of the BASELINE designs (NN model of configs[0]; single-codon and codon-pair TT): n = 24 .. 36 (the oracle takes O(n^2)
+    restricted inside passes: minutes at 36 nt)."""
     m = I.nn_model()
     d = I.design(cfg, 0, L)
     bo, so, co = O.inside(m, O.TT.build(d.aa, d.kind, d.codon_logw, d.pair_logw)).marginals()
