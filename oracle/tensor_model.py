@@ -167,3 +167,120 @@ def tm_brute_force(tm, sigma, ops):
             Z += w * state_weight(tm, seq, pt)
             ns += 1
     return math.log(Z), ns
+
+
+# decision kinds of the tensor-model traceback (distinct from the kinds 0..8 of the nearest-neighbour traceback)
+TMK_TOP, TMK_UPPER, TMK_UNPAIRED, TMK_PAIR = 16, 17, 18, 19
+
+
+def _pick(alts, total, u):
+    """First alternative whose running sum exceeds u * total; zero-weight alternatives are skipped; if rounding leaves the threshold above
+    the last running sum the last positive alternative is taken (the rule of DESIGN.md section 5)."""
+    thr, run, last = u * total, 0.0, None
+    for key, w in alts:
+        if not (w > 0.0):
+            continue
+        run += w
+        last = key
+        if run > thr:
+            return key
+    return last
+
+
+def tm_sample(tm, sigma, ops, Q, J, seed, uniform):
+    """J exact samples (sequence, structure) ~ W(phi) Z(phi, s) / Z by stochastic traceback of the block matrix Q (section 4a
+    lines 215-217; the alternatives are those of Alg S4.4, taken per sample -- the simultaneous bookkeeping of Alg S4.4 changes
+    the cost, not the distribution).  One uniform per decision, uniform(seed, sample, kind, i, j); `total` is the stored block entry being
+    decomposed.  Recursion elements and their alternatives, in this order:
+      TOP                    (s, d, e) ascending:  S[d][e] Q_{0,n}[(0,e)][(s,d)]                                -> UPPER(0, n, (0,e), (s,d))
+      UPPER(i,j,a,b), i < j  k in [i:j) ascending, c ascending:  Q_{i,k}[a][c] Q_{j,k}[b][c]                    -> UPPER(i,k,a,c) if k > i, LOWER(j,k,b,c)
+      LOWER(j,k,b,c), j = k+1   x ascending:  T_k[x][sigma(c)][sigma(b)] V[x][zeta(c)][zeta(b)]                  -> base k = x
+      LOWER(j,k,b,c), j > k+1   (x, y, s1, s2, rho, cc, dd) ascending, l = j-1:
+                             T_k[x][sigma(c)][s1] T_l[y][s2][sigma(b)] B[x][y][rho][zeta(c)][zeta(b)] (S B[y][x][rho])[dd][cc] Q_{k+1,l}[(s1,cc)][(s2,dd)]
+                                                                                                                -> pair k.l, UPPER(k+1, l, (s1,cc), (s2,dd))
+    Nucleotides are chosen through the dense cores (operators with the same (a, b, c) are one alternative).  Returns (seq [J][n] uint8,
+    pair [J][n] int32 with -1 = unpaired)."""
+    n, g = len(ops), tm.gamma
+    T = cores(sigma, ops)
+    SB = np.zeros_like(tm.B)
+    for y in range(4):
+        for x in range(4):
+            for rho in range(tm.xi):
+                SB[y][x][rho] = tm.S @ tm.B[y][x][rho]
+    seqs = np.full((J, n), 255, dtype=np.uint8)
+    pairs = np.full((J, n), -1, dtype=np.int32)
+    for smp in range(J):
+        alts = []
+        for s in range(sigma[n]):
+            for d in range(g):
+                for e in range(g):
+                    alts.append(((e, s * g + d), tm.S[d, e] * Q[0][n][e, s * g + d]))
+        a, b = _pick(alts, sum(w for _, w in alts if w > 0.0), uniform(seed, smp, TMK_TOP, 0, 0))
+        stack = [("U", 0, n, a, b)]
+        while stack:
+            kind, i, j, a, b = stack.pop()
+            if kind == "U":
+                if i == j:
+                    continue
+                alts = []
+                for k in range(i, j):
+                    for c in range(g * sigma[k]):
+                        alts.append(((k, c), Q[i][k][a, c] * Q[j][k][b, c]))
+                k, c = _pick(alts, Q[i][j][a, b], uniform(seed, smp, TMK_UPPER, i, j))
+                if k > i:
+                    stack.append(("U", i, k, a, c))
+                stack.append(("L", j, k, b, c))
+            else:
+                j, k, b, c = i, j, a, b  # the item is ("L", j, k, b, c)
+                if j == k + 1:
+                    alts = [(x, T[k][x][c // g, b // g] * tm.V[x][c % g, b % g]) for x in range(4)]
+                    x = _pick(alts, Q[j][k][b, c], uniform(seed, smp, TMK_UNPAIRED, k, j))
+                    seqs[smp, k] = x
+                else:
+                    l = j - 1
+                    alts = []
+                    for x in range(4):
+                        for y in range(4):
+                            for s1 in range(sigma[k + 1]):
+                                tk = T[k][x][c // g, s1]
+                                for s2 in range(sigma[l]):
+                                    tl = T[l][y][s2, b // g]
+                                    for rho in range(tm.xi):
+                                        bo = tm.B[x][y][rho][c % g, b % g]
+                                        for cc in range(g):
+                                            for dd in range(g):
+                                                alts.append(((x, y, s1, s2, cc, dd),
+                                                             tk * tl * bo * SB[y][x][rho][dd, cc] * Q[k + 1][l][s1 * g + cc, s2 * g + dd]))
+                    x, y, s1, s2, cc, dd = _pick(alts, Q[j][k][b, c], uniform(seed, smp, TMK_PAIR, k, j))
+                    seqs[smp, k], seqs[smp, l] = x, y
+                    pairs[smp, k], pairs[smp, l] = l, k
+                    stack.append(("U", k + 1, l, s1 * g + cc, s2 * g + dd))
+    return seqs, pairs
+
+
+def tm_state_distribution(tm, sigma, ops):
+    """Exact distribution over (sequence, structure) by enumeration: {(seq tuple, pair tuple): probability}."""
+    n = len(ops)
+    paths = []
+
+    def walk(p, bond, seq, w):
+        if p == n:
+            paths.append((tuple(seq), w))
+            return
+        for (a, b, c, x) in ops[p]:
+            if a == bond:
+                seq.append(b)
+                walk(p + 1, c, seq, w * x)
+                seq.pop()
+
+    walk(0, 0, [], 1.0)
+    dist, Z = {}, 0.0
+    for seq, w in paths:
+        def can_pair(k, l, seq=seq):
+            return bool(np.any(tm.B[seq[k]][seq[l]] != 0.0))
+        for pt in _structures(n, can_pair, tm.min_hairpin):
+            v = w * state_weight(tm, list(seq), pt)
+            key = (seq, tuple(pt))
+            dist[key] = dist.get(key, 0.0) + v
+            Z += v
+    return {k: v / Z for k, v in dist.items()}

@@ -95,3 +95,56 @@ def test_fixed_sequence_reduction():
     fixed = [[(0, b, 0, 1.0)] for b in seq]
     logw = cw[16 * 0 + 4 * 3 + 2] * aa.count("M") + cw[16 * 3 + 4 * 2 + 2] * aa.count("W")  # AUG, UGG
     assert abs(TM.tm_inside(tm, sigma, ops) - TM.tm_inside(tm, [1] * 19, fixed) - logw) <= 1e-12
+
+
+def _chi2_states(dist, seqs, pairs):
+    """Pearson statistic of sampled (sequence, structure) counts against the exact distribution, states with expected count < 5 pooled."""
+    import collections
+
+    J = len(seqs)
+    cnt = collections.Counter((tuple(int(v) for v in seqs[k]), tuple(int(v) for v in pairs[k])) for k in range(J))
+    assert all(k in dist for k in cnt), "a sampled state lies outside the support"
+    exp, obs, pe, po = [], [], 0.0, 0.0
+    for k, p in sorted(dist.items(), key=lambda kv: -kv[1]):
+        e, o = p * J, cnt.get(k, 0)
+        if e >= 5:
+            exp.append(e)
+            obs.append(o)
+        else:
+            pe += e
+            po += o
+    if pe > 0:
+        exp.append(pe)
+        obs.append(po)
+    chi = sum((o - e) ** 2 / e for o, e in zip(obs, exp))
+    return chi, len(exp) - 1
+
+
+@pytest.mark.parametrize("aa,kind,gamma,xi,mh,J,seed", [("LSR", 0, 2, 2, 1, 5000, 1), ("FLM", 1, 2, 1, 0, 4000, 2)])
+def test_traceback_samples_the_exact_joint_distribution(aa, kind, gamma, xi, mh, J, seed):
+    """tm_sample against the exact distribution over (sequence, structure) from explicit enumeration (thousands of states): every sampled
+    state lies in the support and the pooled chi-square stays within 4 standard deviations (a wrong alternative weight, order or child
+    element shifts whole families of states); every decision's alternatives sum to the stored block entry it decomposes (1e-12)."""
+    tm = I.tensor_model(gamma, xi, seed=79)
+    tm.min_hairpin = mh
+    sigma, ops = _tt(aa, kind)
+    _, Q = TM.tm_inside(tm, sigma, ops, return_Q=True)
+    worst = [0.0]
+    orig = TM._pick
+
+    def checked(alts, total, u):
+        worst[0] = max(worst[0], abs(sum(w for _, w in alts if w > 0.0) - total) / total)
+        return orig(alts, total, u)
+
+    TM._pick = checked
+    try:
+        seqs, pairs = TM.tm_sample(tm, sigma, ops, Q, J, seed, O.uniform)
+    finally:
+        TM._pick = orig
+    assert worst[0] <= 1e-12
+    chi, dof = _chi2_states(TM.tm_state_distribution(tm, sigma, ops), seqs, pairs)
+    assert abs(chi - dof) <= 4.0 * math.sqrt(2.0 * dof), (chi, dof)
+    # the sampled sequences code for the protein: every codon of the sample translates to its residue
+    code = "KNKNTTTTRSRSIIMIQHQHPPPPRRRRLLLLEDEDAAAAGGGGVVVV*Y*YSSSS*CWCLFLF"  # index 16 b0 + 4 b1 + b2, A C G U
+    for k in range(0, J, 97):
+        assert "".join(code[16 * seqs[k][3 * r] + 4 * seqs[k][3 * r + 1] + seqs[k][3 * r + 2]] for r in range(len(aa))) == aa
