@@ -263,6 +263,13 @@ int cdz_tm_inside(const cdz_tm_params* p, const cdz_tt* tt, void* workspace_dev,
 int cdz_tm_block(const cdz_tm_params* p, const cdz_tt* tt, const void* workspace_dev, double scale_rate, int which, int i, int j,
                  double* out_host, int* shift_out);
 
+/* J exact samples (sequence, structure) ~ W(phi) Z(phi, s) / Z under the tensor model (section 4a) by stochastic traceback of
+ * the tables a cdz_tm_inside call left in a caller workspace (same p, tt): one warp per sample, the alternatives of Alg S4.4 (lines 657-701)
+ * in the fixed order of DESIGN.md section 17, uniforms U(seed, sample, kind, i, j) with kinds 16-19.  seq_dev [J][n] uint8 (0..3),
+ * pair_dev [J][n] int32 partner or -1.  Asynchronous on `stream` (the stacks are a stream-ordered allocation). */
+int cdz_tm_sample(const cdz_tm_params* p, const cdz_tt* tt, void* workspace_dev, int J, uint64_t seed, uint8_t* seq_dev,
+                  int32_t* pair_dev, void* stream);
+
 /* ---- convenience: host buffers end to end (used for the e2e timing) -------- */
 /* Builds nothing: runs cdz_inside_rerun, samples J states and copies them to host buffers. */
 int cdz_run_host(cdz_tables* t, int J, uint64_t seed, uint8_t* seq_host, int32_t* pair_host, double* logZ_host,

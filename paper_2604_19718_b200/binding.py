@@ -24,7 +24,7 @@ EXPORTS = [
     "cdz_inside", "cdz_inside_batch", "cdz_inside_rerun", "cdz_inside_rerun_batch", "cdz_tables_logz",
     "cdz_tables_info", "cdz_tables_destroy", "cdz_tables_cell", "cdz_tables_logqext", "cdz_sample", "cdz_sample_noalloc",
     "cdz_debug_set_rescale_start", "cdz_eval_sequences", "cdz_match_frequencies", "cdz_mfe", "cdz_marginals", "cdz_marginals_workspace_bytes", "cdz_marginals_status", "cdz_run_host", "cdz_set_profiling", "cdz_profile",
-    "cdz_tm_workspace_bytes", "cdz_tm_inside", "cdz_tm_block",
+    "cdz_tm_workspace_bytes", "cdz_tm_inside", "cdz_tm_block", "cdz_tm_sample",
 ]
 
 
@@ -119,6 +119,7 @@ def lib():
     L.cdz_run_host.argtypes = [vp, C.c_int, C.c_uint64, vp, vp, dp, vp]
     L.cdz_tm_workspace_bytes.argtypes = [C.POINTER(TMParams), vp, C.POINTER(C.c_size_t)]
     L.cdz_tm_inside.argtypes = [C.POINTER(TMParams), vp, vp, C.c_size_t, vp, dp, C.POINTER(TMInfo)]
+    L.cdz_tm_sample.argtypes = [C.POINTER(TMParams), vp, vp, C.c_int, C.c_uint64, vp, vp, vp]
     L.cdz_tm_block.argtypes = [C.POINTER(TMParams), vp, vp, C.c_double, C.c_int, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
     _lib = L
     return L
@@ -420,3 +421,14 @@ class TensorModelPass:
         cnt = _check(lib().cdz_tm_block(C.byref(self.p), self.tt.h, C.c_void_p(self.ws.data_ptr()), self.info.scale_rate, which, i, j,
                                         _dp(out), C.byref(sh)))
         return out[:cnt].copy(), sh.value
+
+    def sample(self, J: int, seed: int, stream=None):
+        """cdz_tm_sample: (seq uint8 [J][n], pair int32 [J][n]) CUDA tensors."""
+        import torch
+
+        n = self.tt.n
+        seq = torch.empty((J, n), dtype=torch.uint8, device="cuda")
+        pair = torch.empty((J, n), dtype=torch.int32, device="cuda")
+        _check(lib().cdz_tm_sample(C.byref(self.p), self.tt.h, C.c_void_p(self.ws.data_ptr()), J, seed, C.c_void_p(seq.data_ptr()),
+                                   C.c_void_p(pair.data_ptr()), _stream_ptr(stream)))
+        return seq, pair

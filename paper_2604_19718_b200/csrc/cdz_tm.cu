@@ -47,6 +47,7 @@ struct TmDev {
   const int* sig;      // [n+1]  Sigma of every boundary point
   const int* off;      // [n+2]  padded offset of every boundary point in the flattened index space
   const int* blk;      // [NB+1] first boundary point of every block; blk[NB] = n+1
+  const int* pos;      // [S]    boundary point of every flattened index (padding: the point of the block's last entry)
   const double* T;     // [n][4][MS][MS] dense tensor-train cores (operator weights summed, scaled by 2^-e)
   const double* V;     // [4][g][g]
   const double* B;     // [4][4][xi][g][g]
@@ -262,11 +263,145 @@ __global__ void tm_final_kernel(TmDev t) {
   t.result[0] = z;
 }
 
+// ---- stochastic traceback of Q (section 4a; the alternatives of Alg S4.4, taken per sample) -------------------------
+// One warp per sample; a stack of recursion elements; every decision lists its alternatives in the fixed order of DESIGN.md section 17, the
+// lanes take 32 at a time with a shuffle prefix sum and stop at the first whose running sum exceeds u x (stored entry).  All weights of one
+// decision carry the same power-of-two scale as the entry they decompose, so the scales never enter.
+struct TmItem { int upper, i, j, a, b; };
+enum { TMK_TOP = 16, TMK_UPPER = 17, TMK_UNPAIRED = 18, TMK_PAIR = 19 };
+
+__device__ __forceinline__ uint64_t tm_mix64(uint64_t z) {
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+  return z ^ (z >> 31);
+}
+__device__ __forceinline__ double tm_uniform(uint64_t seed, uint64_t sample, uint64_t kind, uint64_t i, uint64_t j) {
+  uint64_t h = seed;
+  h = tm_mix64(h + 0x9E3779B97F4A7C15ULL * (sample + 1));
+  h = tm_mix64(h + 0x9E3779B97F4A7C15ULL * (kind + 1));
+  h = tm_mix64(h + 0x9E3779B97F4A7C15ULL * (i + 1));
+  h = tm_mix64(h + 0x9E3779B97F4A7C15ULL * (j + 1));
+  return (double)(h >> 11) * (1.0 / 9007199254740992.0);
+}
+// index of the first of `count` alternatives whose running sum exceeds thr; the last positive one if rounding leaves thr above all
+template <typename F>
+__device__ __forceinline__ int tm_pick(int lane, double thr, int count, F weight) {
+  double run = 0.0;
+  int last = -1;
+  for (int b0 = 0; b0 < count; b0 += 32) {
+    const int idx = b0 + lane;
+    double w = idx < count ? weight(idx) : 0.0;
+    if (!(w > 0.0)) w = 0.0;
+    double sm = w;
+    for (int o = 1; o < 32; o <<= 1) {
+      const double v = __shfl_up_sync(0xffffffffu, sm, o);
+      if (lane >= o) sm += v;
+    }
+    const unsigned posm = __ballot_sync(0xffffffffu, w > 0.0);
+    const unsigned hit = __ballot_sync(0xffffffffu, w > 0.0 && run + sm > thr);
+    if (hit) return b0 + __ffs(hit) - 1;
+    if (posm) last = b0 + 31 - __clz(posm);
+    run += __shfl_sync(0xffffffffu, sm, 31);
+  }
+  return last;
+}
+
+__global__ void __launch_bounds__(128) tm_sample_kernel(TmDev t, int J, uint64_t seed, uint8_t* seq_out, int32_t* pair_out, TmItem* stacks,
+                                                        int cap) {
+  const int lane = threadIdx.x & 31;
+  const int smp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (smp >= J) return;
+  const int n = t.n, g = t.gamma, g2 = g * g, xi = t.xi, MS = t.MS, MS2 = MS * MS;
+  const size_t S = (size_t)t.S;
+  uint8_t* seq = seq_out + (size_t)smp * n;
+  int32_t* pair = pair_out + (size_t)smp * n;
+  TmItem* stk = stacks + (size_t)smp * cap;
+  for (int k = lane; k < n; k += 32) { seq[k] = 255; pair[k] = -1; }
+  __syncwarp();
+  int sp = 0;
+  {
+    // TOP: (s, d, e) ascending: S[d][e] Q_{0,n}[(0,e)][(s,d)]
+    const int cnt = t.sig[n] * g2;
+    auto wf = [&](int idx) {
+      const int e = idx % g, d = (idx / g) % g, s = idx / g2;
+      return t.Sm[d * g + e] * t.U[(size_t)(t.off[0] + e) * S + t.off[n] + s * g + d];
+    };
+    double tot = 0.0;
+    for (int idx = lane; idx < cnt; idx += 32) { const double w = wf(idx); if (w > 0.0) tot += w; }
+    for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    const int pick = tm_pick(lane, tm_uniform(seed, smp, TMK_TOP, 0, 0) * tot, cnt, wf);
+    const int e = pick % g, d = (pick / g) % g, s = pick / g2;
+    if (lane == 0) stk[0] = TmItem{1, 0, n, e, s * g + d};
+    sp = 1;
+    __syncwarp();
+  }
+  while (sp > 0) {
+    --sp;
+    const TmItem it = stk[sp];
+    __syncwarp();
+    if (it.upper) {
+      const int i = it.i, j = it.j;
+      if (i == j) continue;
+      // UPPER(i,j,a,b): k in [i:j) ascending, c ascending = the flattened indices off[i] .. off[j]-1 (padding entries are zero and skipped)
+      const double* ru = t.U + (size_t)(t.off[i] + it.a) * S;
+      const double* rc = t.CT + (size_t)(t.off[j] + it.b) * S;
+      const int kb0 = t.off[i], cnt = t.off[j] - kb0;
+      const double thr = tm_uniform(seed, smp, TMK_UPPER, i, j) * ru[t.off[j] + it.b];
+      const int pick = tm_pick(lane, thr, cnt, [&](int idx) { return ru[kb0 + idx] * rc[kb0 + idx]; });
+      const int kb = kb0 + pick, k = t.pos[kb], c = kb - t.off[k];
+      if (lane == 0) {
+        if (k > i) stk[sp] = TmItem{1, i, k, it.a, c};
+        stk[sp + (k > i ? 1 : 0)] = TmItem{0, j, k, it.b, c};
+      }
+      sp += k > i ? 2 : 1;
+      __syncwarp();
+    } else {
+      const int j = it.i, k = it.j, b = it.a, c = it.b;  // LOWER(j,k,b,c): row b of point j, column c of point k
+      const int sc_ = c / g, zc = c - sc_ * g, sb_ = b / g, zb = b - sb_ * g;
+      const double total = t.CT[(size_t)(t.off[j] + b) * S + t.off[k] + c];
+      if (j == k + 1) {
+        // unpaired base k: x ascending: T_k[x][sigma(c)][sigma(b)] V[x][zeta(c)][zeta(b)]
+        const double* Tk = t.T + (size_t)k * 4 * MS2;
+        const int x = tm_pick(lane, tm_uniform(seed, smp, TMK_UNPAIRED, k, j) * total, 4,
+                              [&](int xx) { return Tk[xx * MS2 + sc_ * MS + sb_] * t.V[xx * g2 + zc * g + zb]; });
+        if (lane == 0) seq[k] = (uint8_t)x;
+      } else {
+        // pair k.l, l = j-1: (x, y, s1, s2, rho, cc, dd) ascending
+        const int l = j - 1, s1n = t.sig[k + 1], s2n = t.sig[l];
+        const double* Tk = t.T + (size_t)k * 4 * MS2;
+        const double* Tl = t.T + (size_t)l * 4 * MS2;
+        const double* X = t.U + (size_t)t.off[k + 1] * S + t.off[l];
+        const int per = s1n * s2n * xi * g2, cnt = t.npair * per;
+        auto wf = [&](int idx) {
+          const int dd = idx % g, cc = (idx / g) % g, rho = (idx / g2) % xi, s2 = (idx / (g2 * xi)) % s2n, s1 = (idx / (g2 * xi * s2n)) % s1n;
+          const int pr = idx / per, x = t.px[pr], y = t.py[pr];
+          const double tk = Tk[x * MS2 + sc_ * MS + s1];
+          if (tk == 0.0) return 0.0;
+          return tk * Tl[y * MS2 + s2 * MS + sb_] * t.B[(size_t)((x * 4 + y) * xi + rho) * g2 + zc * g + zb] *
+                 t.SB[(size_t)((y * 4 + x) * xi + rho) * g2 + dd * g + cc] * X[(size_t)(s1 * g + cc) * S + s2 * g + dd];
+        };
+        const int pick = tm_pick(lane, tm_uniform(seed, smp, TMK_PAIR, k, j) * total, cnt, wf);
+        const int dd = pick % g, cc = (pick / g) % g, s2 = (pick / (g2 * xi)) % s2n, s1 = (pick / (g2 * xi * s2n)) % s1n, pr = pick / per;
+        if (lane == 0) {
+          seq[k] = (uint8_t)t.px[pr];
+          seq[l] = (uint8_t)t.py[pr];
+          pair[k] = l;
+          pair[l] = k;
+          stk[sp] = TmItem{1, k + 1, l, s1 * g + cc, s2 * g + dd};
+        }
+        ++sp;
+        __syncwarp();
+      }
+    }
+  }
+}
+
 // ---- host side ---------------------------------------------------------------------------------------------------------------------------
 struct TmLayout {
   int n = 0, NB = 0, S = 0, MS = 1, maxsplit_tiles = 0;
   std::vector<int> sig, off, blk;
-  size_t o_U = 0, o_CT = 0, o_GP = 0, o_T = 0, o_V = 0, o_B = 0, o_SB = 0, o_S = 0, o_sig = 0, o_off = 0, o_blk = 0, o_res = 0, total = 0;
+  size_t o_U = 0, o_CT = 0, o_GP = 0, o_T = 0, o_V = 0, o_B = 0, o_SB = 0, o_S = 0, o_sig = 0, o_off = 0, o_blk = 0, o_pos = 0, o_res = 0, total = 0;
+  std::vector<int> pos;
 };
 
 int tm_check(const cdz_tm_params* p, const cdz_tt* tt) {
@@ -333,8 +468,39 @@ TmLayout tm_layout(const cdz_tm_params* p, const cdz_tt* tt, int n) {
   L.o_sig = take(sizeof(int) * (n + 1));
   L.o_off = take(sizeof(int) * (n + 2));
   L.o_blk = take(sizeof(int) * (L.NB + 1));
+  L.o_pos = take(sizeof(int) * (size_t)L.S);
+  L.pos.assign(L.S, 0);
+  for (int q = 0; q <= n; ++q)
+    for (int k = L.off[q]; k < L.off[q + 1]; ++k) L.pos[k] = q;
   L.total = o;
   return L;
+}
+
+// device view of a workspace laid out by tm_layout
+TmDev tm_view(const cdz_tm_params* p, const TmLayout& L, char* base) {
+  const int g = p->gamma, g2 = g * g, xi = p->xi;
+  TmDev t;
+  t.n = L.n; t.gamma = g; t.xi = xi; t.mh = p->min_hairpin; t.MS = L.MS; t.NB = L.NB; t.S = L.S; t.npair = 0;
+  for (int xy = 0; xy < 16; ++xy) {
+    bool nz = false;
+    for (int k = 0; k < xi * g2; ++k) nz = nz || p->B[(size_t)xy * xi * g2 + k] != 0.0;
+    if (nz) { t.px[t.npair] = xy / 4; t.py[t.npair] = xy % 4; ++t.npair; }
+  }
+  for (int k = t.npair; k < 16; ++k) t.px[k] = t.py[k] = 0;
+  t.result = (double*)(base + L.o_res);
+  t.U = (double*)(base + L.o_U);
+  t.CT = (double*)(base + L.o_CT);
+  t.GP = (double*)(base + L.o_GP);
+  t.T = (const double*)(base + L.o_T);
+  t.V = (const double*)(base + L.o_V);
+  t.B = (const double*)(base + L.o_B);
+  t.SB = (const double*)(base + L.o_SB);
+  t.Sm = (const double*)(base + L.o_S);
+  t.sig = (const int*)(base + L.o_sig);
+  t.off = (const int*)(base + L.o_off);
+  t.blk = (const int*)(base + L.o_blk);
+  t.pos = (const int*)(base + L.o_pos);
+  return t;
 }
 
 inline long long tm_P(int q, double rate) { return (long long)floor((double)q * rate); }
@@ -359,26 +525,7 @@ int tm_pass(const cdz_tm_params* p, const cdz_tt* tt, int n, double rate, char* 
           for (int ee = 0; ee < g; ++ee) v += p->S[d * g + ee] * p->B[((size_t)xy * xi + r) * g2 + ee * g + c];
           SB[((size_t)xy * xi + r) * g2 + d * g + c] = v;
         }
-  TmDev t;
-  t.n = n; t.gamma = g; t.xi = xi; t.mh = p->min_hairpin; t.MS = MS; t.NB = L.NB; t.S = L.S; t.npair = 0;
-  for (int xy = 0; xy < 16; ++xy) {
-    bool nz = false;
-    for (int k = 0; k < xi * g2; ++k) nz = nz || p->B[(size_t)xy * xi * g2 + k] != 0.0;
-    if (nz) { t.px[t.npair] = xy / 4; t.py[t.npair] = xy % 4; ++t.npair; }
-  }
-  for (int k = t.npair; k < 16; ++k) t.px[k] = t.py[k] = 0;
-  t.result = (double*)(base + L.o_res);
-  t.U = (double*)(base + L.o_U);
-  t.CT = (double*)(base + L.o_CT);
-  t.GP = (double*)(base + L.o_GP);
-  t.T = (const double*)(base + L.o_T);
-  t.V = (const double*)(base + L.o_V);
-  t.B = (const double*)(base + L.o_B);
-  t.SB = (const double*)(base + L.o_SB);
-  t.Sm = (const double*)(base + L.o_S);
-  t.sig = (const int*)(base + L.o_sig);
-  t.off = (const int*)(base + L.o_off);
-  t.blk = (const int*)(base + L.o_blk);
+  const TmDev t = tm_view(p, L, base);
   CDZ_CUDA(cudaMemcpyAsync(base + L.o_T, T.data(), sizeof(double) * T.size(), cudaMemcpyHostToDevice, st));
   CDZ_CUDA(cudaMemcpyAsync(base + L.o_V, p->V, sizeof(double) * 4 * g2, cudaMemcpyHostToDevice, st));
   CDZ_CUDA(cudaMemcpyAsync(base + L.o_B, p->B, sizeof(double) * 16 * xi * g2, cudaMemcpyHostToDevice, st));
@@ -387,6 +534,7 @@ int tm_pass(const cdz_tm_params* p, const cdz_tt* tt, int n, double rate, char* 
   CDZ_CUDA(cudaMemcpyAsync(base + L.o_sig, L.sig.data(), sizeof(int) * (n + 1), cudaMemcpyHostToDevice, st));
   CDZ_CUDA(cudaMemcpyAsync(base + L.o_off, L.off.data(), sizeof(int) * (n + 2), cudaMemcpyHostToDevice, st));
   CDZ_CUDA(cudaMemcpyAsync(base + L.o_blk, L.blk.data(), sizeof(int) * (L.NB + 1), cudaMemcpyHostToDevice, st));
+  CDZ_CUDA(cudaMemcpyAsync(base + L.o_pos, L.pos.data(), sizeof(int) * (size_t)L.S, cudaMemcpyHostToDevice, st));
   CDZ_CUDA(cudaStreamSynchronize(st));  // the staging vectors above are pageable host memory about to go out of scope
   // with info: one event before every launch group, so that consecutive pairs give the device time of the GEMMs and of the block kernels
   std::vector<cudaEvent_t> evs;
@@ -520,4 +668,27 @@ extern "C" int cdz_tm_block(const cdz_tm_params* p, const cdz_tt* tt, const void
   }
   if (shift_out) *shift_out = (int)(tm_P(j, scale_rate) - tm_P(i, scale_rate));
   return which == 0 ? mi * mj : mj * mi;
+}
+
+extern "C" int cdz_tm_sample(const cdz_tm_params* p, const cdz_tt* tt, void* workspace_dev, int J, uint64_t seed, uint8_t* seq_dev,
+                             int32_t* pair_dev, void* stream) {
+  const int rc = tm_check(p, tt);
+  if (rc != CDZ_OK) return rc;
+  if (!workspace_dev || J < 0 || !seq_dev || !pair_dev) { cdz_set_error("cdz_tm_sample: bad argument"); return CDZ_EINVAL; }
+  if (J == 0) return CDZ_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  const TmLayout L = tm_layout(p, tt, tt->n);
+  const TmDev t = tm_view(p, L, (char*)workspace_dev);
+  // every element on the stack covers an interval disjoint from the others: at most n + 2 items
+  const int cap = tt->n + 2;
+  TmItem* stacks = nullptr;
+  if (cudaMallocAsync((void**)&stacks, sizeof(TmItem) * (size_t)J * cap, st) != cudaSuccess) {
+    cudaGetLastError();
+    cdz_set_error("cdz_tm_sample: device allocation of the traceback stacks failed");
+    return CDZ_ENOMEM;
+  }
+  tm_sample_kernel<<<(J + 3) / 4, 128, 0, st>>>(t, J, seed, seq_dev, pair_dev, stacks, cap);
+  CDZ_CUDA(cudaGetLastError());
+  CDZ_CUDA(cudaFreeAsync(stacks, st));
+  return CDZ_OK;
 }

@@ -166,3 +166,95 @@ def test_errors(B, I):
     with pytest.raises(B.CdzError):
         B.TensorModelPass(big, tg)
     assert math.isfinite(B.TensorModelPass(tm, tg).logZ)
+
+
+CODE = "KNKNTTTTRSRSIIMIQHQHPPPPRRRRLLLLEDEDAAAAGGGGVVVV*Y*YSSSS*CWCLFLF"  # index 16 b0 + 4 b1 + b2 over A C G U
+
+
+def _valid_state(aa, seq, pair, mh):
+    n = len(seq)
+    assert "".join(CODE[16 * seq[3 * r] + 4 * seq[3 * r + 1] + seq[3 * r + 2]] for r in range(len(aa))) == aa
+    can = {(0, 3), (3, 0), (1, 2), (2, 1), (2, 3), (3, 2)}
+    stack = []
+    for i in range(n):
+        jn = int(pair[i])
+        if jn < 0:
+            continue
+        assert int(pair[jn]) == i
+        if jn > i:
+            assert jn - i - 1 >= mh and (int(seq[i]), int(seq[jn])) in can
+            stack.append(jn)
+        else:
+            assert stack and stack.pop() == i  # non-crossing
+
+
+@pytest.mark.parametrize("cfg,L,gamma,xi,mh,J", [(1, 20, 2, 2, 3, 100), (1, 12, 3, 1, 0, 100), (5, 6, 2, 2, 1, 40), (1, 30, 4, 2, 3, 40)])
+def test_tm_samples_bit_exact(B, I, cfg, L, gamma, xi, mh, J):
+    """cdz_tm_sample == the oracle's traceback for the same seed: every nucleotide and every partner of every sample."""
+    from oracle import oracle as O
+    from oracle import tensor_model as TM
+
+    d = I.design(cfg, 0, L)
+    tm = I.tensor_model(gamma, xi, seed=100 + gamma)
+    tm.min_hairpin = mh
+    tg, (sigma, ops) = _both(B, I, d.aa, d.kind, d.seed)
+    _, Q = TM.tm_inside(tm, sigma, ops, return_Q=True)
+    so, po = TM.tm_sample(tm, sigma, ops, Q, J, d.sample_seed, O.uniform)
+    run = B.TensorModelPass(tm, tg)
+    sg, pg = run.sample(J, d.sample_seed)
+    assert (sg.cpu().numpy() == so).all() and (pg.cpu().numpy() == po).all()
+    for k in range(0, J, 7):
+        _valid_state(d.aa, so[k], po[k], mh)
+
+
+def test_tm_samples_follow_the_exact_distribution(B, I):
+    """40000 GPU samples of a 9-nt design against the exact (sequence, structure) distribution from enumeration (oracle): support and
+    pooled chi-square within 4 standard deviations."""
+    import collections
+
+    from oracle import oracle as O
+    from oracle import tensor_model as TM
+
+    tm = I.tensor_model(2, 2, seed=79)
+    tm.min_hairpin = 1
+    cw = I.codon_logw(5)
+    tg = B.TensorTrain.build("LSR", I.TT_SINGLE_CODON, cw, None)
+    sigma, ops = O.TT.build("LSR", I.TT_SINGLE_CODON, cw, None).get()
+    dist = TM.tm_state_distribution(tm, sigma, ops)
+    J = 40000
+    run = B.TensorModelPass(tm, tg)
+    sg, pg = run.sample(J, 4242)
+    sg, pg = sg.cpu().numpy(), pg.cpu().numpy()
+    cnt = collections.Counter((tuple(int(v) for v in sg[k]), tuple(int(v) for v in pg[k])) for k in range(J))
+    assert all(k in dist for k in cnt)
+    exp, obs, pe, po = [], [], 0.0, 0.0
+    for k, p in sorted(dist.items(), key=lambda kv: -kv[1]):
+        e, o = p * J, cnt.get(k, 0)
+        if e >= 5:
+            exp.append(e)
+            obs.append(o)
+        else:
+            pe += e
+            po += o
+    if pe > 0:
+        exp.append(pe)
+        obs.append(po)
+    chi = sum((o - e) ** 2 / e for o, e in zip(obs, exp))
+    dof = len(exp) - 1
+    assert abs(chi - dof) <= 4.0 * math.sqrt(2.0 * dof), (chi, dof)
+
+
+def test_tm_samples_full_size_valid_and_deterministic(B, I):
+    """Config-2 design (900 nt, codon-pair train, gamma 4, xi 2): 64 samples are coding sequences of the protein with unpseudoknotted
+    structures of canonical pairs and hairpins >= 3; the same seed gives the same samples."""
+    d = I.design(2, 0)
+    tm = I.tensor_model(4, 2)
+    tg = B.TensorTrain.build(d.aa, d.kind, d.codon_logw, d.pair_logw)
+    run = B.TensorModelPass(tm, tg)
+    s1, p1 = run.sample(64, 99)
+    s2, p2 = run.sample(64, 99)
+    assert (s1 == s2).all() and (p1 == p2).all()
+    s1, p1 = s1.cpu().numpy(), p1.cpu().numpy()
+    for k in range(64):
+        _valid_state(d.aa, s1[k], p1[k], 3)
+    assert (p1 >= 0).sum() > 0
