@@ -17,8 +17,9 @@
 //   P5  GI, D1, D2T (DD summed over one or both nucleotides)
 // Every band sum is a dot product of two CONTIGUOUS row segments of row-major tables (transposed copies EMT, QBST,
 // D2T, QM1T exist for that purpose), so the loads of the lanes of a group are coalesced and independent.
-// Position metadata and the dense cores TL_i[(a,x)][c], TR_j[a][(y,c)] of the block's rows / columns live in
-// shared memory; the per-cell intermediates live in a shared-memory scratch slab.
+// Position metadata, the boundary states of every window position packed 4 bits each (PosPk: the serial loops of SB / Qb / P4 / P5 extract a
+// state's bond or nucleotide with a register shift instead of a dependent load) and the dense cores TL_i[(a,x)][c], TR_j[a][(y,c)] of the
+// block's rows / columns live in shared memory; the per-cell intermediates live in a shared-memory scratch slab.
 #include <math.h>
 
 #include <algorithm>
@@ -405,8 +406,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
 #else
 #define CDZ_TICK(k)
 #endif
-  // dynamic distribution of the P1 work: every warp starts with the unit of its own number (the counters start at the number of warps), then
-  // lane 0 takes the next unit and the warp follows
+  // dynamic distribution of the P1 work: lane 0 takes the next unit, the warp follows
   auto grab = [&](int* c) {
     int w = 0;
     if ((tid & 31) == 0) w = atomicAdd(c, 1);

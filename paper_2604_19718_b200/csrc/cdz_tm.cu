@@ -77,6 +77,7 @@ __global__ void __launch_bounds__(GEMM_THREADS) tm_gemm_kernel(TmDev t, int D, i
 __global__ void __launch_bounds__(TM_THREADS) tm_block_kernel(TmDev t, int D, int nsplit) {
   // prefix sums over the cells of one in-block anti-diagonal: outputs | staged X entries | t entries | m entries | 4 x 4 output tiles
   __shared__ int pre[TM_MAXCELL + 1], prx[TM_MAXCELL + 1], prt[TM_MAXCELL + 1], prm[TM_MAXCELL + 1], prb[TM_MAXCELL + 1];
+  __shared__ int overflow;
   extern __shared__ double pool[];  // X pool [TM_XPOOL] | t pool [TM_POOL] | m pool [TM_POOL]
   double* xP = pool;
   double* tP = pool + TM_XPOOL;
@@ -108,8 +109,12 @@ __global__ void __launch_bounds__(TM_THREADS) tm_block_kernel(TmDev t, int D, in
         }
       }
       pre[ncell] = ao; prx[ncell] = ax; prt[ncell] = at; prm[ncell] = am; prb[ncell] = ab;
+      // guard of the pool bounds derived above (never expected to fire): report instead of writing out of bounds
+      overflow = (ncell > TM_MAXCELL || ax > TM_XPOOL || at > TM_POOL || am > TM_POOL) ? 1 : 0;
+      if (overflow) t.result[1] = 1.0;
     }
     __syncthreads();
+    if (overflow) return;
     // ---- (A) closed elements Q_{j,i} = chi-hat_{i,j}(Q_{i+1,j-1}) of the step's cells (eq 3.8); every stage spread over the whole CTA ----
     if (d == 1) {
       // unpaired base i:  sum_x T_i[x] (x) V[x]
@@ -548,6 +553,7 @@ int tm_pass(const cdz_tm_params* p, const cdz_tt* tt, int n, double rate, char* 
     cls.push_back(c);
   };
   mark(0);
+  CDZ_CUDA(cudaMemsetAsync(t.result, 0, 2 * sizeof(double), st));
   CDZ_CUDA(cudaMemsetAsync(t.U, 0, sizeof(double) * (size_t)L.S * L.S, st));
   CDZ_CUDA(cudaMemsetAsync(t.CT, 0, sizeof(double) * (size_t)L.S * L.S, st));
   CDZ_CUDA(cudaFuncSetAttribute(tm_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
@@ -572,9 +578,12 @@ int tm_pass(const cdz_tm_params* p, const cdz_tt* tt, int n, double rate, char* 
   tm_final_kernel<<<1, 32, 0, st>>>(t);
   ++launches;
   mark(0);
-  CDZ_CUDA(cudaMemcpyAsync(z_out, t.result, sizeof(double), cudaMemcpyDeviceToHost, st));
+  double res[2] = {0.0, 0.0};
+  CDZ_CUDA(cudaMemcpyAsync(res, t.result, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
   CDZ_CUDA(cudaStreamSynchronize(st));
   CDZ_CUDA(cudaGetLastError());
+  *z_out = res[0];
+  if (res[1] != 0.0) { cdz_set_error("cdz_tm_inside: internal shared-pool bound exceeded"); return CDZ_ESTATE; }
   if (info) {
     double tot = 0.0, by[3] = {0.0, 0.0, 0.0};
     for (size_t k = 0; k + 1 < evs.size(); ++k) {
