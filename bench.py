@@ -553,6 +553,16 @@ def run_tensor_model(args):
         run.rerun()
         wall.append((time.perf_counter() - t0) * 1e3)
         dev.append(run.info.device_ms); gemm.append(run.info.gemm_ms); block.append(run.info.block_ms)
+    # 100 exact samples from the tables of the last pass (cdz_tm_sample), device time by CUDA events on the launching stream
+    nsmp = 100
+    run.sample(nsmp, 1)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    seq, pair = run.sample(nsmp, d.sample_seed)
+    ev1.record()
+    torch.cuda.synchronize()
+    sample_ms = ev0.elapsed_time(ev1)
+    paired = float((pair >= 0).float().mean().item())
     clk = clocks.stop()
     ms, gms, bms, wms = (sum(v) / len(v) for v in (dev, gemm, block, wall))
     peak = measure_peak(1)
@@ -580,6 +590,7 @@ def run_tensor_model(args):
                                f"synthetic tensor model gamma={args.gamma} xi={args.xi}", "n_nt": d.n, "flattened_dim": flat, "padded_dim": i.S,
                    "blocks": i.NB, "l2": f"tables ({i.table_bytes / 1e9:.1f} GB) larger than L2" if i.table_bytes > 126e6 else "tables fit L2"},
         "logZ": run.logZ, "scale_rate_bits_per_nt": i.scale_rate, "gemm_ms": gms, "block_ms": bms, "gpu_launches": int(i.launches),
+        "samples": {"n": nsmp, "ms": sample_ms, "paired_fraction": paired, "what": "cdz_tm_sample: exact (sequence, structure) samples by stochastic traceback of the tables of the pass"},
         "roofline": {"kernel": "tm_gemm_kernel (k-sum over finished blocks, fp64 mma.sync m8n8k4 tiles shared with the inside pass)",
                      "bound": "tensor", "achieved": i.gemm_flop / (gms * 1e-3) / 1e12 if gms > 0 else None, "peak": peak, "unit": "TFLOP/s",
                      "frac": (i.gemm_flop / (gms * 1e-3) / 1e12 / peak) if gms > 0 else None, "traffic": None,
