@@ -258,3 +258,46 @@ def test_tm_samples_full_size_valid_and_deterministic(B, I):
     for k in range(64):
         _valid_state(d.aa, s1[k], p1[k], 3)
     assert (p1 >= 0).sum() > 0
+
+
+def test_generic_operator_list_bond_dimension_8(B, I):
+    """Generic operator list of bond dimension 8 with gamma = 4: 32-dimensional boundary points (the kernel limit), two points per 64-block,
+    so nearly every k-sum crosses blocks; every block of Q and 8 samples against the oracle."""
+    from oracle import oracle as O
+    from oracle import tensor_model as TM
+
+    ops = I.closed_form_inputs("zero8", 30)
+    tm = I.tensor_model(4, 2, seed=17)
+    tg = B.TensorTrain.from_operators(ops)
+    sigma, oo = O.TT.from_ops(ops).get()
+    lz_o, Q = TM.tm_inside(tm, sigma, oo, return_Q=True)
+    run = B.TensorModelPass(tm, tg)
+    assert run.info.NB >= 12
+    assert abs(run.logZ - lz_o) <= 1e-9 * abs(lz_o)
+    n = len(ops)
+    for i in range(0, n + 1, 3):
+        for j in range(i, n + 1):
+            v, sh = run.block(0, i, j)
+            ref = Q[i][j].reshape(-1)
+            assert np.allclose(v * 2.0 ** sh, ref, rtol=1e-10, atol=1e-13 * max(1e-300, np.abs(ref).max())), (i, j)
+    so, po = TM.tm_sample(tm, sigma, oo, Q, 8, 5, O.uniform)
+    sg, pg = run.sample(8, 5)
+    assert (sg.cpu().numpy() == so).all() and (pg.cpu().numpy() == po).all()
+
+
+def test_tiny_and_limits(B, I):
+    """One residue (3 nt, no pair possible), xi = 4, gamma = 8 with a bond-4 train (32-dimensional points), and the rejected sizes."""
+    from oracle import oracle as O
+    from oracle import tensor_model as TM
+
+    for aa, gamma, xi in (("M", 2, 2), ("L", 3, 4), ("LSRW", 8, 1)):
+        tm = I.tensor_model(gamma, xi, seed=5)
+        tm.min_hairpin = 1
+        tg = B.TensorTrain.build(aa, I.TT_SINGLE_CODON, None, None)
+        sigma, ops = O.TT.build(aa, I.TT_SINGLE_CODON, None, None).get()
+        lz = TM.tm_inside(tm, sigma, ops)
+        assert abs(B.TensorModelPass(tm, tg).logZ - lz) <= 1e-9 * max(1.0, abs(lz))
+    # gamma x bond > 32 is rejected: gamma 8 with a codon-pair train (bond 6)
+    tg = B.TensorTrain.build("LSR", I.TT_CODON_PAIR, None, None)
+    with pytest.raises(B.CdzError):
+        B.TensorModelPass(I.tensor_model(8, 1), tg)
