@@ -617,10 +617,10 @@ def kernel_source_hash() -> str:
 
 
 def committed_traffic(cfg):
-    """profiles/traffic.json: {"source_hash": "...", "config": 4, "gemm": bytes per launch, "block": bytes per launch, "from": "..."}.
+    """profiles/traffic.json.txt: {"source_hash": "...", "config": 4, "gemm": bytes per launch, "block": bytes per launch, "from": "..."}.
     Only used when it was captured from exactly these kernel sources and this config; otherwise {} (traffic: null)."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+        with open(os.path.join(ROOT, "profiles", "traffic.json.txt")) as f:
             rec = json.load(f)
     except (OSError, ValueError):
         return {}
