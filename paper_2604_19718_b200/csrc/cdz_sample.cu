@@ -247,6 +247,10 @@ __device__ double iloop_total(const View& V, int i, int j, int k, int l, int P, 
 __global__ void __launch_bounds__(128) sample_kernel(const Ctx* ctxp, int J, uint64_t seed, uint8_t* seq_out,
                                                      int32_t* pair_out, Item* stacks, int stack_cap) {
   __shared__ CModel cm;
+  // per warp: the operators compatible with the boundary state of the element being decomposed (weights and inner bonds), see QB / ILOOP
+  constexpr int CCAP = 40;
+  __shared__ double s_cw[4][2][CCAP];
+  __shared__ short s_cb[4][2][CCAP], s_cz[4][2][CCAP];
   const Ctx& cx = *ctxp;
   {
     const int* src = (const int*)cx.cm;
@@ -413,8 +417,41 @@ __global__ void __launch_bounds__(128) sample_kernel(const Ctx* ctxp, int J, uin
       const int x = it.x, y = it.y, d = j - i, P = V.pt(x, y);
       if (lane == 0) { seq[i] = (uint8_t)x; seq[j] = (uint8_t)y; pair[i] = j; pair[j] = i; }
       const int zi0 = t.opstart[i], ni = t.opstart[i + 1] - zi0, zj0 = t.opstart[j], nj = t.opstart[j + 1] - zj0;
-      const int npair = ni * nj;  // rectangular (z_i, z_j) space; mismatching operators weigh 0
+      // The (z_i, z_j) alternatives with non-zero weight are the product of the operators at i with (a, b) = (it.a, x) and those at j with
+      // (b, c) = (y, it.c), in list order.  Zero-weight alternatives never decide a pick, so only that product is
+      // scanned: the two compatible lists are compacted once per decision (weight and inner bond of every entry) into shared memory.
+      const int wrp = threadIdx.x >> 5;
+      double* cwi = s_cw[wrp][0];
+      double* cwj = s_cw[wrp][1];
+      short* cai = s_cb[wrp][0];
+      short* ccj = s_cb[wrp][1];
+      int ci = 0, cj = 0;
+      __syncwarp();
+      for (int b0 = 0; b0 < ni; b0 += 32) {
+        const int z = zi0 + b0 + lane;
+        const bool ok = b0 + lane < ni && t.op_a[z] == it.a && t.op_b[z] == x;
+        const unsigned m = __ballot_sync(0xffffffffu, ok);
+        const int pos = ci + __popc(m & ((1u << lane) - 1u));
+        if (ok && pos < CCAP) { cwi[pos] = t.op_x[z]; cai[pos] = (short)t.op_c[z]; }
+        ci += __popc(m);
+      }
+      for (int b0 = 0; b0 < nj; b0 += 32) {
+        const int z = zj0 + b0 + lane;
+        const bool ok = b0 + lane < nj && t.op_b[z] == y && t.op_c[z] == it.c;
+        const unsigned m = __ballot_sync(0xffffffffu, ok);
+        const int pos = cj + __popc(m & ((1u << lane) - 1u));
+        if (ok && pos < CCAP) { cwj[pos] = t.op_x[z]; ccj[pos] = (short)t.op_a[z]; }
+        cj += __popc(m);
+      }
+      __syncwarp();
+      const bool compact = ci <= CCAP && cj <= CCAP;  // (otherwise the rectangular space below; mismatching operators weigh 0)
+      const int npair = compact ? ci * cj : ni * nj;
       auto zw = [&](int pz, int& ap, int& cp) {
+        if (compact) {
+          const int ki = pz / cj, kj = pz - ki * cj;
+          ap = cai[ki]; cp = ccj[kj];
+          return cwi[ki] * cwj[kj];
+        }
         const int zi = zi0 + pz / nj, zj = zj0 + pz % nj;
         ap = t.op_c[zi]; cp = t.op_a[zj];
         if (t.op_a[zi] != it.a || t.op_b[zi] != x || t.op_b[zj] != y || t.op_c[zj] != it.c) return 0.0;
@@ -537,9 +574,38 @@ __global__ void __launch_bounds__(128) sample_kernel(const Ctx* ctxp, int J, uin
         term_l1l2(term, l1, l2);
         const int k = p + l1, l = q - l2;
         // level B (K_ILOOP): left side x right side x (x',y'), rectangular order
-        const int nl = left_count(t, i, k), nr = right_count(t, j, l);
+        // The left side runs over (operator at i+1) x (operator at k-1), the right side over (operator at l+1) x (operator at j-1); only the
+        // operators at i+1 with a = ap and at j-1 with c = cp can weigh in, so those two lists are compacted (operator indices) and the
+        // alternatives are numbered over the compact products, in the same order.
+        short* lz = s_cz[wrp][0];
+        short* rz = s_cz[wrp][1];
+        const int zl0 = t.opstart[i + 1], nl1 = l1 >= 1 ? t.opstart[i + 2] - zl0 : 0, nl2 = l1 >= 2 ? t.opstart[k] - t.opstart[k - 1] : 1;
+        const int zr0 = t.opstart[j - 1], nr2 = l2 >= 1 ? t.opstart[j] - zr0 : 0, nr1 = l2 >= 2 ? t.opstart[l + 2] - t.opstart[l + 1] : 1;
+        int cl = 0, cr = 0;
+        __syncwarp();
+        for (int b0 = 0; b0 < nl1; b0 += 32) {
+          const bool ok = b0 + lane < nl1 && t.op_a[zl0 + b0 + lane] == ap;
+          const unsigned m = __ballot_sync(0xffffffffu, ok);
+          const int pos = cl + __popc(m & ((1u << lane) - 1u));
+          if (ok && pos < CCAP) lz[pos] = (short)(b0 + lane);
+          cl += __popc(m);
+        }
+        for (int b0 = 0; b0 < nr2; b0 += 32) {
+          const bool ok = b0 + lane < nr2 && t.op_c[zr0 + b0 + lane] == cp;
+          const unsigned m = __ballot_sync(0xffffffffu, ok);
+          const int pos = cr + __popc(m & ((1u << lane) - 1u));
+          if (ok && pos < CCAP) rz[pos] = (short)(b0 + lane);
+          cr += __popc(m);
+        }
+        __syncwarp();
+        const bool cside = cl <= CCAP && cr <= CCAP;
+        // compact side index -> index of the rectangular numbering of left_side / right_side
+        auto lmap = [&](int la) { return (!cside || l1 == 0) ? la : l1 == 1 ? (int)lz[la] : lz[la / nl2] * nl2 + la % nl2; };
+        auto rmap = [&](int ra) { return (!cside || l2 == 0) ? ra : l2 == 1 ? (int)rz[ra] : (ra / cr) * nr2 + rz[ra % cr]; };
+        const int nl = (!cside || l1 == 0) ? left_count(t, i, k) : cl * nl2;
+        const int nr = (!cside || l2 == 0) ? right_count(t, j, l) : nr1 * cr;
         auto wf = [&](int f) {
-          const int xy = f & 15, ra = (f >> 4) % nr, la = (f >> 4) / nr;
+          const int xy = f & 15, ra = rmap((f >> 4) % nr), la = lmap((f >> 4) / nr);
           const int xp = xy >> 2, yp = xy & 3;
           if (!V.can(xp, yp)) return 0.0;
           const SideL L = left_side(V, i, k, ap, la);
@@ -552,7 +618,7 @@ __global__ void __launch_bounds__(128) sample_kernel(const Ctx* ctxp, int J, uin
         p2.thr = uniform(seed, smp, K_ILOOP, i, j) * warp_total(lane, nl * nr * 16, wf);
         scan_segment(lane, p2, 0, nl * nr * 16, wf);
         const int f = p2.hit >= 0 ? p2.hit : p2.last;
-        const int xy = f & 15, ra = (f >> 4) % nr, la = (f >> 4) / nr;
+        const int xy = f & 15, ra = rmap((f >> 4) % nr), la = lmap((f >> 4) / nr);
         const SideL L = left_side(V, i, k, ap, la);
         const SideL R = right_side(V, j, l, cp, ra);
         if (l1 >= 1 && lane == 0) seq[i + 1] = (uint8_t)L.u;
