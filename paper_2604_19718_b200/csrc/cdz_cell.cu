@@ -147,6 +147,13 @@ __device__ __forceinline__ void x_cell(int lane, double* xs, int Mst, int Sa, in
     for (int a = 0; a < MA; ++a)
 #pragma unroll
       for (int w = 0; w < W; ++w) acc[a][w] = 0.0;
+    // the hairpin entry this lane adds at the end of the pass (even lanes own one entry each): with a single pass per cell (bond dimension
+    // <= 4) it is loaded now and used last; with several passes the early load costs more than it hides (measured)
+    double ehp = 0.0;
+    if (MA == 4 && (lane & 1) == 0) {
+      const int e = lane >> 1, a = e / W, w = e % W;
+      if (closed && a < Sa && w < ncw) ehp = emh[(size_t)a * S + cc + w];
+    }
     if (live && hasold && u > 4) {
       const double* xo = xs + (size_t)(u - 5) * Mst * Sc + cc;
 #pragma unroll
@@ -212,7 +219,7 @@ __device__ __forceinline__ void x_cell(int lane, double* xs, int Mst, int Sa, in
     if ((lane & 1) == 0) {
       const int e = lane >> 1, a = e / W, w = e % W;
       if (a < Sa && w < ncw) {
-        const double xv = v[0] + (closed ? hpw * emh[(size_t)a * S + cc + w] : 0.0);
+        const double xv = v[0] + (MA == 4 ? hpw * ehp : closed ? hpw * emh[(size_t)a * S + cc + w] : 0.0);
         xe_out[a * Mxe + cc + w] = xv;
         xe_glob[(size_t)a * S + cc + w] = xv;  // same index as emh: row (i+2, a), column (j-1, c)
       }
@@ -726,7 +733,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           const int Sp1 = rowm[kp + 1].sig, Sq = mq.sig;
           const double* TLp = TLs + ((p - tlbase) * ML + lst) * M;
           const double* TRq = TRs + (size_t)(q - trbase) * M * MR + r;
-          double y = v11 ? cm.win[2] * b.DD[(size_t)(rowm[kp].loff + lst) * RS + mq.roff + r] : 0.0;
+          const double dd11 = v11 ? b.DD[(size_t)(rowm[kp].loff + lst) * RS + mq.roff + r] : 0.0;  // (needed last: the load overlaps the loops)
+          double y = 0.0;
           for (int cz = 0; cz < Sp1; ++cz) {
             const double tl = TLp[cz];
             if (tl == 0.0) continue;
@@ -735,7 +743,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             y += tl * s;
           }
           for (int aw = 0; aw < Sq; ++aw) y += sc.Z1[lst * M + aw] * TRq[aw * MR];
-          sc.Y[lst * MR + r] = y;
+          sc.Y[lst * MR + r] = cm.win[2] * dd11 + y;
         }
         __syncthreads();
       }
