@@ -666,21 +666,40 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             if (q - p >= mh1 && lst >= 0 && r >= 0) v = b.QB[(size_t)(mp.loff + lst) * RS + mq.roff + r];
             if (maxint >= 1 && q - (p + 1) >= mh1) {
               double s1 = 0.0, s2 = 0.0;
-              if (r >= 0) {
-                const PosMeta mp1 = rowm[kp + 1];
-                const PosPk wp1 = rowpk[kp + 1];
-                for (int l2 = 0; l2 < mp1.nL; ++l2)
-                  if (pk(wp1.lsx, l2) == xp)
-                    s1 += Tbar[(size_t)p * MS2 + a1 * MS + pk(wp1.lsa, l2)] *
-                          b.QB[(size_t)(mp1.loff + l2) * RS + mq.roff + r];
-              }
-              if (lst >= 0) {
-                const PosMeta mq1 = colm[q - 1 - cbase];
-                const PosPk wq1 = colpk[q - 1 - cbase];
-                for (int r2 = 0; r2 < mq1.nR; ++r2)
-                  if (pk(wq1.rsy, r2) == yp)
-                    s2 += b.QB[(size_t)(mp.loff + lst) * RS + mq1.roff + r2] *
-                          Tbar[(size_t)q * MS2 + pk(wq1.rsc, r2) * MS + c1];
+              const PosMeta mp1 = rowm[kp + 1], mq1 = colm[q - 1 - cbase];
+              const PosPk wp1 = rowpk[kp + 1], wq1 = colpk[q - 1 - cbase];
+              if (FIX) {
+                // fixed trip counts + predicates: every global load of the item is in flight before the first product (a skipped term adds 0)
+                double tb[4], qa[4], qc[6], tc[6];
+#pragma unroll
+                for (int l2 = 0; l2 < 4; ++l2) {
+                  const bool on = r >= 0 && l2 < mp1.nL && pk(wp1.lsx, l2) == xp;
+                  tb[l2] = on ? Tbar[(size_t)p * MS2 + a1 * MS + pk(wp1.lsa, l2)] : 0.0;
+                  qa[l2] = on ? b.QB[(size_t)(mp1.loff + l2) * RS + mq.roff + r] : 0.0;
+                }
+#pragma unroll
+                for (int r2 = 0; r2 < 6; ++r2) {
+                  const bool on = lst >= 0 && r2 < mq1.nR && pk(wq1.rsy, r2) == yp;
+                  qc[r2] = on ? b.QB[(size_t)(mp.loff + lst) * RS + mq1.roff + r2] : 0.0;
+                  tc[r2] = on ? Tbar[(size_t)q * MS2 + pk(wq1.rsc, r2) * MS + c1] : 0.0;
+                }
+#pragma unroll
+                for (int l2 = 0; l2 < 4; ++l2) s1 += tb[l2] * qa[l2];
+#pragma unroll
+                for (int r2 = 0; r2 < 6; ++r2) s2 += qc[r2] * tc[r2];
+              } else {
+                if (r >= 0) {
+                  for (int l2 = 0; l2 < mp1.nL; ++l2)
+                    if (pk(wp1.lsx, l2) == xp)
+                      s1 += Tbar[(size_t)p * MS2 + a1 * MS + pk(wp1.lsa, l2)] *
+                            b.QB[(size_t)(mp1.loff + l2) * RS + mq.roff + r];
+                }
+                if (lst >= 0) {
+                  for (int r2 = 0; r2 < mq1.nR; ++r2)
+                    if (pk(wq1.rsy, r2) == yp)
+                      s2 += b.QB[(size_t)(mp.loff + lst) * RS + mq1.roff + r2] *
+                            Tbar[(size_t)q * MS2 + pk(wq1.rsc, r2) * MS + c1];
+                }
               }
               v += cm.wbu[1] * (s1 + s2);
             }
@@ -700,17 +719,41 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
             if (rec) {
               double r1 = 0.0, r2 = 0.0;
               if (d >= 1) {
-                for (int s = 0; s < mj.sig; ++s) r1 += b.QM1T[(size_t)(mj.off + s) * S + offi + a] * Tj[s * MS];
                 const PosMeta mi1 = rowm[kp + 1];
                 const double* Ti = Tbar + (size_t)i * MS2 + a * MS;
-                for (int s = 0; s < mi1.sig; ++s) r2 += Ti[s] * b.QML[(size_t)(mi1.off + s) * S + mj1.off + c];
+                if (FIX) {
+                  double q1[4], t1[4], t2[4], q2[4];
+#pragma unroll
+                  for (int s = 0; s < 4; ++s) {
+                    q1[s] = s < mj.sig ? b.QM1T[(size_t)(mj.off + s) * S + offi + a] : 0.0;
+                    t1[s] = s < mj.sig ? Tj[s * MS] : 0.0;
+                    t2[s] = s < mi1.sig ? Ti[s] : 0.0;
+                    q2[s] = s < mi1.sig ? b.QML[(size_t)(mi1.off + s) * S + mj1.off + c] : 0.0;
+                  }
+#pragma unroll
+                  for (int s = 0; s < 4; ++s) { r1 += q1[s] * t1[s]; r2 += t2[s] * q2[s]; }
+                } else {
+                  for (int s = 0; s < mj.sig; ++s) r1 += b.QM1T[(size_t)(mj.off + s) * S + offi + a] * Tj[s * MS];
+                  for (int s = 0; s < mi1.sig; ++s) r2 += Ti[s] * b.QML[(size_t)(mi1.off + s) * S + mj1.off + c];
+                }
               }
               Scr sc = scr_of(scrb, dm, i - clo);
               sc.R1[a * M + c] = cm.wb * r1;
               sc.R2[a * M + c] = cm.wb * r2;
             } else {
               double v = 0.0;
-              for (int s = 0; s < mj.sig; ++s) v += b.EM[(size_t)(offi + a) * S + mj.off + s] * Tj[s * MS];
+              if (FIX) {
+                double e1[4], t1[4];
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                  e1[s] = s < mj.sig ? b.EM[(size_t)(offi + a) * S + mj.off + s] : 0.0;
+                  t1[s] = s < mj.sig ? Tj[s * MS] : 0.0;
+                }
+#pragma unroll
+                for (int s = 0; s < 4; ++s) v += e1[s] * t1[s];
+              } else {
+                for (int s = 0; s < mj.sig; ++s) v += b.EM[(size_t)(offi + a) * S + mj.off + s] * Tj[s * MS];
+              }
               b.EM[(size_t)(offi + a) * S + mj1.off + c] = v;
               b.EMT[(size_t)(mj1.off + c) * S + offi + a] = v;
             }
