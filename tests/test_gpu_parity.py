@@ -339,6 +339,24 @@ def test_closed_form_large(B, row):
     tg.destroy()
 
 
+@pytest.mark.parametrize("row", _closed_rows(), ids=lambda r: f"{r[0]}-{r[1]}")
+def test_closed_form_large_fp32_scaled(B, row):
+    """The same closed forms through CDZ_FP32_SCALED (3xTF32 split-point contraction, BASELINE configs[2] tolerance 1e-4): at 3000 nt the
+    fp32 path is pinned to a value that owes nothing to the fp64 GPU path (the plain oracle cannot reach the 3000-nt codon-pair design)."""
+    kind, n, want = row[0], int(row[1]), float(row[2])
+    if kind == "zero8":
+        m = I.zero_energy_model()
+        tt = B.TensorTrain.from_operators(I.closed_form_inputs("zero8", n))
+    else:
+        m = I.nn_model()
+        aa, cw = I.closed_form_inputs("mettrp", n)
+        tt = B.TensorTrain.build(aa, B.TT_SINGLE_CODON, cw)
+    tg, lz = B.inside(B.Model(m), tt, precision=B.FP32_SCALED)
+    assert tg.info()["precision"] == B.FP32_SCALED
+    assert abs(lz - want) <= FP32_RTOL * abs(want), (lz, want)
+    tg.destroy()
+
+
 @pytest.mark.parametrize("cfg", [2, 4])
 def test_rescale_schedule_invariance(B, cfg):
     """The per-position scales are exact powers of two, so moving the rescale events (after block diagonals 1,2,4,.. -> 3,6,12,.. ->
