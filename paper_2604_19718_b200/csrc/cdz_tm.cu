@@ -246,8 +246,15 @@ __global__ void __launch_bounds__(TM_THREADS) tm_block_kernel(TmDev t, int D, in
             for (int qq = 0; qq < 4; ++qq) v = (rr == r && qq == q) ? acc[rr][qq] : v;
           if (r < nr && q < nc) {
             const int ri = t.off[i] + al0 + r, rj = t.off[j] + de0 + q;
-            for (int sp = 0; sp < nsplit; ++sp)
-              v += t.GP[((size_t)I * nsplit + sp) * (CDZ_TB * CDZ_TB) + (size_t)(ri - I * CDZ_TB) * CDZ_TB + (rj - J * CDZ_TB)];
+            // split-K partials: batches of 8 loads in flight before the first add (same order of the adds as a plain loop)
+            const double* gp = t.GP + (size_t)I * nsplit * (CDZ_TB * CDZ_TB) + (size_t)(ri - I * CDZ_TB) * CDZ_TB + (rj - J * CDZ_TB);
+            for (int s0 = 0; s0 < nsplit; s0 += 8) {
+              double gv[8];
+#pragma unroll
+              for (int u = 0; u < 8; ++u) gv[u] = s0 + u < nsplit ? gp[(size_t)(s0 + u) * (CDZ_TB * CDZ_TB)] : 0.0;
+#pragma unroll
+              for (int u = 0; u < 8; ++u) v += gv[u];
+            }
             t.U[(size_t)ri * S + rj] = v;
           }
         }
