@@ -161,13 +161,23 @@ __global__ void __launch_bounds__(TM_THREADS) tm_block_kernel(TmDev t, int D, in
         const double* ti = t.T + (size_t)i * 4 * MS2 + t.px[pr] * MS2 + sa * MS;
         const double* tl = t.T + (size_t)l * 4 * MS2 + t.py[pr] * MS2 + sd;
         const double* tw = tP + prt[c] + (pr * xi + rho) * s1 * s2;
+        // the two core rows are loaded once, all loads in flight together (bond dimension <= CDZ_MAX_BOND; a missing entry is 0)
+        double tav[CDZ_MAX_BOND], tlv[CDZ_MAX_BOND];
+#pragma unroll
+        for (int u = 0; u < CDZ_MAX_BOND; ++u) {
+          tav[u] = u < s1 ? ti[u] : 0.0;
+          tlv[u] = u < s2 ? tl[u * MS] : 0.0;
+        }
         double v = 0.0;
-        for (int a1 = 0; a1 < s1; ++a1) {
-          const double ta = ti[a1];
-          double sm = 0.0;
-#pragma unroll 2
-          for (int c1 = 0; c1 < s2; ++c1) sm += tw[a1 * s2 + c1] * tl[c1 * MS];
-          v += ta * sm;
+#pragma unroll
+        for (int a1 = 0; a1 < CDZ_MAX_BOND; ++a1) {
+          if (a1 < s1) {
+            double sm = 0.0;
+#pragma unroll
+            for (int c1 = 0; c1 < CDZ_MAX_BOND; ++c1)
+              if (c1 < s2) sm += tw[a1 * s2 + c1] * tlv[c1];
+            v += tav[a1] * sm;
+          }
         }
         mP[it] = v;
       }
