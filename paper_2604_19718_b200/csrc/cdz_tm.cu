@@ -78,6 +78,7 @@ __global__ void __launch_bounds__(TM_THREADS) tm_block_kernel(TmDev t, int D, in
   // prefix sums over the cells of one in-block anti-diagonal: outputs | staged X entries | t entries | m entries | 4 x 4 output tiles
   __shared__ int pre[TM_MAXCELL + 1], prx[TM_MAXCELL + 1], prt[TM_MAXCELL + 1], prm[TM_MAXCELL + 1], prb[TM_MAXCELL + 1];
   __shared__ int overflow;
+  __shared__ int boff[16 * TM_MAXXI];  // offset of B[x][y][rho] for every (pairable (x, y), rho), in the order of the intermediates
   extern __shared__ double pool[];  // X pool [TM_XPOOL] | t pool [TM_POOL] | m pool [TM_POOL]
   double* xP = pool;
   double* tP = pool + TM_XPOOL;
@@ -88,6 +89,11 @@ __global__ void __launch_bounds__(TM_THREADS) tm_block_kernel(TmDev t, int D, in
   const size_t S = (size_t)t.S;
   const int i0 = t.blk[I], i1 = t.blk[I + 1], j0 = t.blk[J], j1 = t.blk[J + 1];
   const int dmin = max(1, j0 - (i1 - 1)), dmax = (j1 - 1) - i0;
+  for (int k = threadIdx.x; k < t.npair * t.xi; k += TM_THREADS) {
+    const int pr = k / t.xi, rho = k - pr * t.xi;
+    boff[k] = ((t.px[pr] * 4 + t.py[pr]) * t.xi + rho) * t.gamma * t.gamma;
+  }
+  __syncthreads();
   // item -> (cell, index inside the cell) through a prefix array
   auto cell_of = [&](const int* pr, int it, int& c) { c = 0; while (pr[c + 1] <= it) ++c; return it - pr[c]; };
   for (int d = dmin; d <= dmax; ++d) {
@@ -188,10 +194,11 @@ __global__ void __launch_bounds__(TM_THREADS) tm_block_kernel(TmDev t, int D, in
         const int e = cell_of(pre, it, c), i = ilo + c, j = i + d, si = t.sig[i], sj = t.sig[j], mj = g * sj;
         const int al = e / mj, de = e - al * mj, sa = al / g, za = al - sa * g, sd = de / g, zd = de - sd * g;
         const double* mw = mP + prm[c] + sa * sj + sd;
+        const double* bz = t.B + za * g + zd;
+        const int sij = si * sj;
         double v = 0.0;
-        for (int pr = 0; pr < t.npair; ++pr)
-          for (int rho = 0; rho < xi; ++rho)
-            v += t.B[(size_t)((t.px[pr] * 4 + t.py[pr]) * xi + rho) * g2 + za * g + zd] * mw[(pr * xi + rho) * si * sj];
+#pragma unroll 4
+        for (int k = 0; k < npx; ++k) v += bz[boff[k]] * mw[k * sij];
         t.CT[(size_t)(t.off[j] + de) * S + t.off[i] + al] = v;
       }
     }
