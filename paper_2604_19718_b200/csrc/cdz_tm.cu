@@ -74,6 +74,17 @@ __global__ void __launch_bounds__(GEMM_THREADS) tm_gemm_kernel(TmDev t, int D, i
                 t.GP + ((size_t)I * nsplit + sp) * (CDZ_TB * CDZ_TB), gsm);
 }
 
+// sum_{c,d} SB[d][c] X[c][d] for one gamma x gamma sub-block (row stride ld): compile-time gamma for the common model dimensions
+template <int G>
+__device__ __forceinline__ double tm_trace(const double* __restrict__ sb, const double* __restrict__ xb, int ld) {
+  double v = 0.0;
+#pragma unroll
+  for (int cc = 0; cc < G; ++cc)
+#pragma unroll
+    for (int dd = 0; dd < G; ++dd) v += sb[dd * G + cc] * xb[cc * ld + dd];
+  return v;
+}
+
 __global__ void __launch_bounds__(TM_THREADS) tm_block_kernel(TmDev t, int D, int nsplit) {
   // prefix sums over the cells of one in-block anti-diagonal: outputs | staged X entries | t entries | m entries | 4 x 4 output tiles
   __shared__ int pre[TM_MAXCELL + 1], prx[TM_MAXCELL + 1], prt[TM_MAXCELL + 1], prm[TM_MAXCELL + 1], prb[TM_MAXCELL + 1];
@@ -152,9 +163,12 @@ __global__ void __launch_bounds__(TM_THREADS) tm_block_kernel(TmDev t, int D, in
         const double* sb = t.SB + (size_t)((t.py[pr] * 4 + t.px[pr]) * xi + rho) * g2;
         const double* xb = xP + prx[c] + (a1 * g) * ld + c1 * g;
         double v = 0.0;
-        for (int cc = 0; cc < g; ++cc)
-#pragma unroll 4
-          for (int dd = 0; dd < g; ++dd) v += sb[dd * g + cc] * xb[cc * ld + dd];
+        if (g == 4) v = tm_trace<4>(sb, xb, ld);
+        else if (g == 2) v = tm_trace<2>(sb, xb, ld);
+        else if (g == 8) v = tm_trace<8>(sb, xb, ld);
+        else
+          for (int cc = 0; cc < g; ++cc)
+            for (int dd = 0; dd < g; ++dd) v += sb[dd * g + cc] * xb[cc * ld + dd];
         tP[it] = v;
       }
       __syncthreads();
