@@ -778,14 +778,32 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) cell_kernel(const Ctx* ctxs, 
           const double* TRq = TRs + (size_t)(q - trbase) * M * MR + r;
           const double dd11 = v11 ? b.DD[(size_t)(rowm[kp].loff + lst) * RS + mq.roff + r] : 0.0;  // (needed last: the load overlaps the loops)
           double y = 0.0;
-          for (int cz = 0; cz < Sp1; ++cz) {
-            const double tl = TLp[cz];
-            if (tl == 0.0) continue;
-            double s = sc.Z2[cz * MR + r];
-            for (int aw = 0; aw < Sq; ++aw) s += sc.XE[cz * M + aw] * TRq[aw * MR];
-            y += tl * s;
+          if (FIX) {
+            // fixed trip counts + predicates (bond dimension <= 4): all shared-memory operands in flight together; a skipped term adds 0
+            double trq[4];
+#pragma unroll
+            for (int aw = 0; aw < 4; ++aw) trq[aw] = aw < Sq ? TRq[aw * MR] : 0.0;
+#pragma unroll
+            for (int cz = 0; cz < 4; ++cz) {
+              const bool oc = cz < Sp1;
+              const double tl = oc ? TLp[cz] : 0.0;
+              double s = oc ? sc.Z2[cz * MR + r] : 0.0;
+#pragma unroll
+              for (int aw = 0; aw < 4; ++aw) s += ((oc && aw < Sq) ? sc.XE[cz * M + aw] : 0.0) * trq[aw];
+              y += tl * s;
+            }
+#pragma unroll
+            for (int aw = 0; aw < 4; ++aw) y += (aw < Sq ? sc.Z1[lst * M + aw] : 0.0) * trq[aw];
+          } else {
+            for (int cz = 0; cz < Sp1; ++cz) {
+              const double tl = TLp[cz];
+              if (tl == 0.0) continue;
+              double s = sc.Z2[cz * MR + r];
+              for (int aw = 0; aw < Sq; ++aw) s += sc.XE[cz * M + aw] * TRq[aw * MR];
+              y += tl * s;
+            }
+            for (int aw = 0; aw < Sq; ++aw) y += sc.Z1[lst * M + aw] * TRq[aw * MR];
           }
-          for (int aw = 0; aw < Sq; ++aw) y += sc.Z1[lst * M + aw] * TRq[aw * MR];
           sc.Y[lst * MR + r] = cm.win[2] * dd11 + y;
         }
         __syncthreads();
